@@ -1,0 +1,25 @@
+"""CPU fp64 oracle for the PSE grand-mobility path of arxiv 1709.06946 (Fiore & Swan).
+
+TEST INFRASTRUCTURE ONLY.  Nothing under ``paper_1709_06946_b200/`` (the CUDA product path) imports,
+links or calls this package, and this package imports nothing from the product path.  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may use it.
+
+It is a plain, slow, obviously-correct statement of what the path computes:
+
+* ``functions``  – shape factors, Hasimoto splitting function, the seven real-space scalar functions
+                   (free-space closed form minus a Gaussian-damped 1-D wave integral; SURVEY.md §8(c) O2,
+                   replacing the garbled Appendix A of PAPER.md:589-744).
+* ``mobility``   – direct O(N^2) Ewald sums of Eqs. (21)-(27): dense 8N x 8N assembly,
+                   and row-sampled application for larger N.
+* ``brownian``   – Eq. (71)/(74)/(76) sample: principal square root of the dense
+                   real-space matrix plus the direct non-uniform sum of the wave-space factor over the
+                   grid's wave vectors; the mid-point step Eqs. (76)-(79).
+* ``neighbors``  – brute-force fp32 neighbour sets.
+
+Pins (tests/test_oracle_*.py, ``-m "not gpu"``): Hasimoto periodic self-mobility, xi-independence of
+M_r + M_w, symmetry and positive-definiteness of M, M_r, M_w, textbook RPY / RPY-overlap free-space
+limits, printed closed forms F1, F2 of Appendix A, exact covariance identity
+A_w A_w^T = M_w(grid modes), Schur-complement constraint solve.
+
+Parity unpinned (not in the paper): the Heyes-Melrose hard-sphere force (reading R12 in DESIGN.md).
+"""

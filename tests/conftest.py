@@ -1,0 +1,19 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line('markers', 'gpu: needs a CUDA device (run on the B200 box with -m gpu)')
+
+
+@pytest.fixture(scope='session')
+def unit_params():
+    """a = 1, eta = 1/(6 pi): single-sphere free mobility 1 (BASELINE.json configs)."""
+    import numpy as np
+    return dict(a=1.0, eta=1.0 / (6.0 * np.pi))

@@ -1,0 +1,178 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only, -m "not gpu").
+
+P1 Hasimoto self-mobility, P2 xi-independence, P3 symmetry + positive-definiteness, P4 limits/continuity of the
+scalar functions, P5 free-space forms against the Fourier-space definition, P6 printed closed forms of
+Appendix A, P7 single-sphere cubic symmetry, P8 worked example, P9 exact covariance identity, P12 Schur solve.
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.join(os.path.dirname(__file__), 'golden'))
+import paper_appendix_a as app  # noqa: E402
+from oracle import brownian as brn  # noqa: E402
+from oracle import functions as fn  # noqa: E402
+from oracle import mobility as mob  # noqa: E402
+
+A, ETA = 1.0, 1.0 / (6.0 * np.pi)
+X4 = np.array([[0.5, 0.6, 0.7], [2.9, 1.0, 0.9], [1.1, 4.0, 5.5], [2.0, 2.0, 2.3]])  # pair 0-3 overlaps (r = 1.942)
+
+
+def test_basis_orthonormal_and_roundtrip():
+    e = fn.basis()
+    assert np.allclose(np.einsum('pij,qij->pq', e, e), np.eye(5), atol=1e-15)
+    assert np.allclose(np.einsum('qii->q', e), 0) and np.allclose(e, e.transpose(0, 2, 1))
+    s = np.random.default_rng(0).standard_normal((7, 5))
+    assert np.allclose(fn.to_coords(fn.to_tensor(s)), s, atol=1e-14)
+
+
+def test_P1_hasimoto_single_sphere():
+    """6 pi eta a mu = 1 - 2.8372974795 a/L + (4 pi/3)(a/L)^3 for one sphere per cubic cell."""
+    for L, xi in [(7.0, 0.55), (7.0, 0.9), (11.0, 0.4)]:
+        M = mob.dense(np.array([[1.0, 2.0, 3.0]]), L, A, ETA, xi)
+        want = 1 - app.HASIMOTO_C * A / L + 4 * np.pi / 3 * (A / L)**3
+        assert np.allclose(np.diag(M)[:3], want, atol=5e-10), (L, xi, M[0, 0], want)
+        assert np.allclose(M[:3, :3], want * np.eye(3), atol=5e-10)
+
+
+def test_P7_single_sphere_cubic_symmetry():
+    """M_EF,self = 0; self M_ES is diagonal with one value for e1,e2 and one for e3..e5 (cubic anisotropy)."""
+    M = mob.dense(np.array([[0.3, 0.2, 0.1]]), 7.0, A, ETA, 0.6)
+    assert np.abs(M[:3, 3:]).max() < 1e-13 and np.abs(M[3:, :3]).max() < 1e-13
+    d = np.diag(M)[3:]
+    assert np.abs(M[3:, 3:] - np.diag(d)).max() < 1e-13
+    assert abs(d[0] - d[1]) < 1e-12 and abs(d[2] - d[3]) < 1e-12 and abs(d[3] - d[4]) < 1e-12
+    assert abs(d[0] - d[2]) > 1e-2     # anisotropic: 0.8604 vs 0.9081 at L = 7a
+    assert abs(d[0] - 0.860374496914) < 1e-9 and abs(d[2] - 0.908098677547) < 1e-9
+
+
+def test_P2_P3_xi_independence_symmetry_spd():
+    Ms = [mob.dense(X4, 7.0, A, ETA, xi) for xi in (0.45, 0.7, 1.0)]
+    assert np.abs(Ms[0] - Ms[1]).max() < 1e-12 and np.abs(Ms[0] - Ms[2]).max() < 1e-12
+    for xi in (0.45, 1.0):
+        Mr, Mw = mob.dense(X4, 7.0, A, ETA, xi, 'real'), mob.dense(X4, 7.0, A, ETA, xi, 'wave')
+        for M in (Mr, Mw, Mr + Mw):
+            assert np.abs(M - M.T).max() < 1e-13
+        np.linalg.cholesky(Mr)                                  # strictly PD
+        np.linalg.cholesky(Mr + Mw)
+        assert np.linalg.eigvalsh(Mw).min() > -1e-13            # PSD
+    w = np.linalg.eigvalsh(Ms[0])
+    assert abs(w[0] - 0.183962406486) < 1e-9 and abs(w[-1] - 1.331372501993) < 1e-9
+
+
+def test_P8_worked_example():
+    """Entries of M for the 4-sphere example, computed independently during the survey."""
+    M = mob.dense(X4, 7.0, A, ETA, 0.55)
+    gold = {(0, 0): 0.606884004986, (0, 8): 0.218163662585, (0, 24): 0.027175723339, (0, 26): 0.047217809432,
+            (1, 25): 0.016352878862, (0, 27): 0.005564508157, (3, 24): -0.005564508157, (2, 29): -0.046712907241,
+            (3, 27): 0.024490765888, (5, 29): -0.026755324780, (7, 25): 0.078638421506, (3, 11): -0.150187216517,
+            (4, 4): 0.860374496914, (5, 5): 0.908098677547}
+    for ij, v in gold.items():
+        assert abs(M[ij] - v) < 2e-11, (ij, M[ij], v)
+
+
+def test_dense_matches_apply():
+    """The P^H B P matrix form (Eqs. 39-41) and the direct sums (Eqs. 21-24) are two codes for one operator."""
+    rng = np.random.default_rng(1)
+    F, S = rng.standard_normal((4, 3)), rng.standard_normal((4, 5))
+    U, E = mob.mobility_apply(X4, 7.0, A, ETA, 0.6, F, S)
+    o = (mob.dense(X4, 7.0, A, ETA, 0.6) @ np.concatenate([F, S], 1).ravel()).reshape(4, 8)
+    assert np.abs(o[:, :3] - U).max() < 1e-13 and np.abs(o[:, 3:] - E).max() < 1e-13
+    U2, E2 = mob.mobility_apply(X4, 7.0, A, ETA, 0.6, F, S, rows=[1, 3])
+    assert np.allclose(U2, U[[1, 3]], atol=1e-14) and np.allclose(E2, E[[1, 3]], atol=1e-14)
+
+
+def test_P4_limits_and_continuity():
+    r = np.array([0.0, 0.6, 1.7, 1.999999, 2.000001, 2.6, 4.5])
+    fr = fn.free_space(r, A)
+    lo = fn.real_space_functions(r, 1e-3, A)       # xi -> 0: everything stays in real space
+    hi = fn.real_space_functions(r[1:], 12.0, A)   # xi -> inf: everything moves to wave space (r > 0)
+    for n in fn.NAMES:
+        assert np.abs(lo[n] - fr[n]).max() < 2e-3, n     # W_X = O(xi a) as xi -> 0 (3 xi a/sqrt(pi) for F1)
+        assert np.abs(hi[n][4:]).max() < 1e-9, n    # exponentially small for r > 2a
+        assert np.abs(hi[n][:4]).max() < 1e-3, n    # only O(xi^-4) inside the overlap region (kink of the RPY forms)
+        assert abs(fr[n][3] - fr[n][4]) < 1e-5, n   # continuous at r = 2a
+
+
+def test_P5_free_space_is_the_unsplit_fourier_integral():
+    """Free_X(r) = W_X(r; xi -> inf): the closed forms are the inverse transforms of Eqs. (15)-(18); the
+    quadrature (with H -> 1 on the resolved band) reproduces them independently of the algebra."""
+    r = np.array([0.6, 1.2, 1.9, 2.6, 3.3, 4.5, 6.0])   # (r - 2a) xi >= 7 for the r > 2a points
+    fr, wv, wv2 = fn.free_space(r, A), fn.wave_integrals(r, 12.0, A), fn.wave_integrals(r, 24.0, A)
+    for n in fn.NAMES:
+        assert np.abs(fr[n] - wv[n])[3:].max() < 1e-9, (n, fr[n] - wv[n])        # r > 2a: exact
+        d1, d2 = np.abs(fr[n] - wv[n])[:3], np.abs(fr[n] - wv2[n])[:3]
+        assert d1.max() < 1e-3 and np.all(d2 < d1 / 8), (n, d1, d2)              # r < 2a: O(xi^-4) approach
+
+
+def test_P5_rpy_textbook_values():
+    """Rotne-Prager-Yamakawa numbers everyone knows: touching spheres and complete overlap."""
+    fr = fn.free_space(np.array([2.0, 0.0, 4.0]), A)
+    assert abs(fr['F1'][0] - (3 / 8 + 1 / 16)) < 1e-15 and abs(fr['F2'][0] - (3 / 4 - 1 / 8)) < 1e-15
+    assert fr['F1'][1] == 1.0 and fr['F2'][1] == 1.0
+    assert abs(fr['F2'][2] - (3 / 8 - 1 / 64)) < 1e-15       # (3a/2r)(1 - 2a^2/3r^2) at r = 4a
+    assert abs(fr['Z0'][1] - 4.5) < 1e-15                    # 6 pi eta a / (20/3 pi eta a^3) * ... = 9/(2 a^2) -> E = S/(20/3 pi eta a^3)
+
+
+@pytest.mark.parametrize('xi', [0.3, 0.45, 0.8])
+def test_P6_printed_closed_forms(xi):
+    r = np.array([0.6, 1.7, 1.999, 2.001, 2.6, 4.5])
+    R = fn.real_space_functions(r, xi, A)
+    for i, ri in enumerate(r):
+        assert abs(R['F1'][i] - app.F1(ri, A, xi)) < 1e-10
+        assert abs(R['F2'][i] - app.F2(ri, A, xi)) < 1e-10
+        assert abs(2 * R['G2'][i] - app.G2(ri, A, xi)) < 1e-9
+    assert abs(fn.real_space_functions(np.array([0.0]), xi, A)['F1'][0] - app.self_UF(A, xi)) < 1e-12
+
+
+def test_P9_exact_covariance_identity():
+    """A_w A_w^T = M_w restricted to the grid's wave vectors, for unit-variance noise (Eq. 73)."""
+    x = np.array([[0.3, 0.4, 0.5], [2.2, 1.0, 0.9], [1.1, 3.0, 2.5]])
+    L, xi = 5.0, 0.7
+    for Mg in (6, 5):
+        Aw = brn.wave_sqrt_dense(x, L, A, ETA, xi, Mg)
+        k = brn.grid_modes(Mg, L)
+        k2 = np.einsum('ki,ki->k', k, k)
+        Mw = mob.dense_wave_modes(x, A, k, fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2))
+        assert np.abs(Aw @ Aw.T - Mw).max() < 1e-13
+        # conjugate partners and Nyquist / k = 0 entries carry no weight
+        used = (np.abs(Aw).sum(axis=0) > 0).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
+        idx, _ = brn.canonical_modes(Mg)
+        canon = np.zeros((Mg, Mg, Mg // 2 + 1), bool)
+        canon[idx[:, 0], idx[:, 1], idx[:, 2]] = True
+        assert not used[:, ~canon, :].any() and used[:, canon, :].mean() > 0.9
+
+
+def test_P10_statistical_covariance_small():
+    """<u u^T> -> (2kT/dt) M over many seeds (Eq. B4); M_r^{1/2} part exact by construction."""
+    x = X4[:2]
+    L, xi, Mg, kT, dt = 7.0, 0.6, 6, 1.3, 0.5
+    Mr = mob.dense_real(x, L, A, ETA, xi)
+    Sr = brn.sqrtm_psd(Mr)
+    assert np.abs(Sr @ Sr - Mr).max() < 1e-13
+    Aw = brn.wave_sqrt_dense(x, L, A, ETA, xi, Mg)
+    g = np.random.default_rng(5)
+    n = 20000
+    u = np.sqrt(2 * kT / dt) * (g.standard_normal((n, 16)) @ Sr.T + g.standard_normal((n, Aw.shape[1])) @ Aw.T)
+    C = u.T @ u / n
+    want = 2 * kT / dt * (Mr + Aw @ Aw.T)
+    assert np.abs(C - want).max() < 6 * np.abs(want).max() / np.sqrt(n)
+
+
+def test_P12_schur_complement_solve():
+    """Constraint solve gives E = 0 exactly and U = (M_UF - M_US M_ES^-1 M_EF) F (Eqs. 36-38)."""
+    N = 4
+    M = mob.dense(X4, 7.0, A, ETA, 0.6)
+    rng = np.random.default_rng(2)
+    FP = rng.standard_normal((N, 3))
+    U, S = brn.constrained_solve(M, N, np.zeros((N, 3)), np.zeros((N, 5)), FP)
+    out = (M @ np.concatenate([FP, S], 1).ravel()).reshape(N, 8)
+    assert np.abs(out[:, 3:]).max() < 1e-13 and np.abs(out[:, :3] - U).max() < 1e-13
+    # the constrained mobility is symmetric positive definite and smaller than M_UF (rigidity adds dissipation)
+    iu = (8 * np.arange(N)[:, None] + np.arange(3)).ravel()
+    ie = (8 * np.arange(N)[:, None] + 3 + np.arange(5)).ravel()
+    Mc = M[np.ix_(iu, iu)] - M[np.ix_(iu, ie)] @ np.linalg.solve(M[np.ix_(ie, ie)], M[np.ix_(ie, iu)])
+    assert np.abs(Mc - Mc.T).max() < 1e-13
+    assert np.linalg.eigvalsh(Mc).min() > 0 and np.linalg.eigvalsh(M[np.ix_(iu, iu)] - Mc).min() > -1e-13
