@@ -1,0 +1,112 @@
+/* pse.h — C ABI of libpse: positively-split Ewald (PSE) grand mobility with stresslets on one B200 (sm_100a).
+ *
+ * Method: Fiore & Swan, arXiv 1709.06946 ("PAPER.md").  Every call below cites the passage that defines it.
+ *
+ * Conventions
+ *   - Pointers prefixed d_ are DEVICE pointers owned by the caller (e.g. torch tensors); h_ are HOST pointers.
+ *     The library never frees or reallocates caller buffers.  All internal buffers belong to the context.
+ *   - All work is enqueued on the CUDA stream given at pse_create (NULL = legacy default stream).  Calls that
+ *     return iteration counts or need host-side convergence decisions synchronise that stream.
+ *   - fp32 on the device.  Per-particle vectors: positions [N][4] (x,y,z,unused); forces/velocities [N][3];
+ *     stresslets / rates of strain [N][5] as coordinates in the orthonormal basis of symmetric traceless tensors
+ *       e1=(xx-yy)/sqrt2, e2=(2zz-xx-yy)/sqrt6, e3=(xy+yx)/sqrt2, e4=(xz+zx)/sqrt2, e5=(yz+zy)/sqrt2
+ *     (the paper says only "5 for the stresslet"; reading R9).
+ *   - Errors are return codes; pse_last_error gives a message.  No exceptions cross this boundary, no exit().
+ *   - There is no CPU fallback: without a CUDA device every compute call returns PSE_ECUDA.
+ */
+#ifndef PSE_H
+#define PSE_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pse_ctx pse_ctx;
+
+typedef enum {
+    PSE_OK = 0, PSE_EINVAL = 1, PSE_ENOMEM = 2, PSE_ECUDA = 3, PSE_ECUFFT = 4, PSE_ENOTREADY = 5,
+    PSE_ENOCONV = 6, PSE_EOVERFLOW = 7
+} pse_status;
+
+/* which half of the Ewald sum pse_mobility_apply evaluates (Eq. 30) */
+enum { PSE_REAL = 1, PSE_WAVE = 2, PSE_BOTH = 3 };
+
+/* phases reported by pse_get_timings */
+enum { PSE_T_NEIGHBORS = 0, PSE_T_REAL = 1, PSE_T_SPREAD = 2, PSE_T_FFT_FWD = 3, PSE_T_SCALE = 4, PSE_T_FFT_INV = 5,
+       PSE_T_INTERP = 6, PSE_T_VECTOR = 7, PSE_T_PACK = 8, PSE_T_COUNT = 9 };
+
+/* Parameter derivation from a tolerance (reading R6; paper: eps_r ~ exp(-xi^2 rcut^2) PAPER.md:207,
+ * quadrature bound Eq. (55) with m = sqrt(pi P) PAPER.md:308, 334).  Host only, no GPU needed.
+ *   in : N, L, a, tol, xi
+ *   out: *grid (FFT points per dimension, 2^a 3^b 5^c 7^d), *P (Gaussian support, points per dimension),
+ *        *rcut (real-space cutoff).  Returns PSE_EINVAL if no valid choice exists (rcut > L/2). */
+pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, int *grid, int *P, double *rcut);
+
+/* Create a context for N equal spheres of radius a in a cubic periodic box of edge L, viscosity eta, thermal
+ * energy kT, splitting parameter xi (Eq. 28), FFT grid `grid`^3, Gaussian support P^3 grid points
+ * (PAPER.md:227), real-space cutoff rcut, Krylov tolerance tol.  Builds the
+ * real-space tables (Eqs. 25-27 PAPER.md:127-143 via DESIGN.md §3), cuFFT plans and workspaces.
+ * PSE_EINVAL: non-positive sizes, rcut > L/2, rcut < 2a, P > grid, P > 16, Gaussian parameter eta_g >= 1. */
+pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
+                      int grid, int P, double rcut, double tol, void *cuda_stream);
+pse_status pse_destroy(pse_ctx *ctx);
+
+/* Bin the particles (positions may be unwrapped; they are wrapped into [0,L)) into linked cells of edge >= rcut
+ * and build the full neighbour list {beta != alpha : |x_alpha - x_beta|_min-image^2 < rcut^2}, plus
+ * the FFT-grid tile bins used by spread/interpolate.  Must be re-called whenever positions change.
+ * d_pos: [N][4] float, device.  Asynchronous except for one size read-back. */
+pse_status pse_neighbors(pse_ctx *ctx, const float *d_pos);
+
+/* [U;E] = M [F;S]  (Eqs. 30-31): real-space pair sum over the neighbour list with tabulated
+ * functions (Eqs. 25-27) plus the spectral-Ewald wave-space sum sigma Q^T F^H P^H B P F Q (Eq. 42).
+ * d_F [N][3], d_S [N][5] in; d_U [N][3], d_E [N][5] out (overwritten).  which = PSE_REAL | PSE_WAVE | PSE_BOTH.
+ * PSE_ENOTREADY before pse_neighbors.  Asynchronous. */
+pse_status pse_mobility_apply(pse_ctx *ctx, const float *d_F, const float *d_S, float *d_U, float *d_E, int which);
+
+/* Brownian slip velocities [U^B;E^B] = sqrt(2 kT/dt) ( M_r^{1/2} w1 + M_w^{1/2} w2 )  (Eqs. 71, 75, 76, B4;
+ * PAPER.md:409, 449, 462, 759).  M_r^{1/2} w1 by Lanczos to relative change <= tol;
+ * M_w^{1/2} w2 = sigma^{1/2} Q^T F^H P^H B^{1/2} w2 with conjugate-symmetric complex noise.
+ * d_noise_real: [N][8] i.i.d. N(0,1), per particle (Ux,Uy,Uz,e1..e5).
+ * d_noise_wave: [3][grid][grid][grid/2+1][2] i.i.d. N(0,1); layout and conjugacy rule: DESIGN.md reading R8.
+ * lanczos_iters (host, may be NULL) receives the iteration count.  Synchronises the stream. */
+pse_status pse_brownian(pse_ctx *ctx, double dt, const float *d_noise_real, const float *d_noise_wave,
+                        float *d_UB, float *d_EB, int *lanczos_iters);
+
+/* Stresslet-constrained velocities at the current positions (Eqs. 36-38, 78):
+ * solve M_ES S = -(E^B + M_EF F) by GMRES (relative residual <= tol), U = U^B + M_UF F + M_US S.
+ * d_F [N][3] (may be NULL = 0), d_UB [N][3], d_EB [N][5] (may be NULL = 0) in; d_U [N][3], d_S [N][5] out.
+ * gmres_iters (host, may be NULL).  PSE_ENOCONV if not converged in 50 iterations (best iterate written). */
+pse_status pse_constrained_solve(pse_ctx *ctx, const float *d_F, const float *d_UB, const float *d_EB,
+                                 float *d_U, float *d_S, int *gmres_iters);
+
+/* Heyes-Melrose hard-sphere overlap force at the current positions (named by BASELINE.json, not the paper;
+ * DESIGN.md reading R12): F_i = sum_{j: r_ij<2a} 3 pi eta a (2a - r_ij)/dt rhat_ij.  d_F [N][3] out. */
+pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);
+
+/* One mid-point step of the constrained overdamped Langevin dynamics, Eqs. (76)-(79):
+ * neighbours(x_k); Brownian slip; x_{k+1/2} = x_k + dt/2 U^B; neighbours(x_{k+1/2}); hard-sphere forces;
+ * constrained solve; x_{k+1} = x_k + dt U_{k+1/2} (wrapped into [0,L)).  d_pos [N][4] in/out.
+ * On return the context's neighbour structures refer to x_{k+1/2}; call pse_neighbors before further products. */
+pse_status pse_step(pse_ctx *ctx, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave,
+                    int *gmres_iters, int *lanczos_iters);
+
+/* Introspection for the parity tests and the harness. */
+/* Neighbour list in ORIGINAL particle numbering: d_count [N]; d_index holds the lists of particle 0,1,...
+ * concatenated (offsets = exclusive scan of d_count); order within a list is unspecified.  *total (host) gets
+ * the number of entries; if cap < total only *total is written (PSE_EOVERFLOW).  d_index may be NULL. */
+pse_status pse_get_neighbors(pse_ctx *ctx, int *d_count, int *d_index, size_t cap, size_t *total);
+/* Switch per-phase CUDA-event timing on/off (adds event records, no synchronisation until read). */
+pse_status pse_set_profiling(pse_ctx *ctx, int on);
+/* Accumulated per-phase milliseconds and launch counts since the last call (synchronises); arrays of n entries. */
+pse_status pse_get_timings(pse_ctx *ctx, float *h_ms, int *h_launches, int n);
+/* Number of kernels (own + cuFFT calls) enqueued since pse_create. */
+long long pse_kernel_launches(const pse_ctx *ctx);
+/* Copy the fp32 real-space table to the host: n nodes x 8 (F1,F2,G1+G2,G1+4G2,A,B,D,0), node i at r = i*dr. */
+pse_status pse_get_table(pse_ctx *ctx, float *h_table, int cap_nodes, int *n_nodes, double *dr);
+const char *pse_last_error(const pse_ctx *ctx);
+const char *pse_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

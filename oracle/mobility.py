@@ -168,7 +168,7 @@ def dense_wave_modes(x, a, k, weight):
     N = x.shape[0]
     e = fn.basis()
     M = np.zeros((8 * N, 8 * N))
-    chunk = max(1, 2_000_000 // (24 * N))
+    chunk = max(1, 16_000_000 // (24 * N))
     for lo in range(0, k.shape[0], chunk):
         kk, wk = k[lo:lo + chunk], weight[lo:lo + chunk]
         kn = np.linalg.norm(kk, axis=1)
@@ -180,7 +180,8 @@ def dense_wave_modes(x, a, k, weight):
         shape[:, :, 3:] = -1j * c1[:, None, None] * np.einsum('qij,kj->kiq', e, kk)
         b = (ph[:, None, :, None] * shape[:, :, None, :]).reshape(kk.shape[0], 3, 8 * N)
         Pb = b - kh[:, :, None] * np.einsum('ki,kin->kn', kh, b)[:, None, :]
-        M += np.real(np.einsum('k,kin,kim->nm', wk, np.conj(b), Pb))
+        nk = kk.shape[0]
+        M += np.real((np.conj(b) * wk[:, None, None]).reshape(nk * 3, 8 * N).T @ Pb.reshape(nk * 3, 8 * N))
     return M
 
 

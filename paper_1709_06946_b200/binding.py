@@ -1,0 +1,171 @@
+"""ctypes binding of libpse.so — argument marshalling only; every step of the path runs in the CUDA library.
+
+Function names mirror include/pse.h.  Tensors are torch CUDA tensors (torch is used for device memory and
+streams only).  There is no CPU fallback: if libpse.so is missing or no CUDA device is present the calls raise.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, 'libpse.so')
+
+PSE_OK, PSE_EINVAL, PSE_ENOMEM, PSE_ECUDA, PSE_ECUFFT, PSE_ENOTREADY, PSE_ENOCONV, PSE_EOVERFLOW = range(8)
+PSE_REAL, PSE_WAVE, PSE_BOTH = 1, 2, 3
+PHASES = ('neighbors', 'real', 'spread', 'fft_fwd', 'scale', 'fft_inv', 'interp', 'vector', 'pack')
+_STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PSE_ECUFFT', 5: 'PSE_ENOTREADY',
+           6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
+
+EXPORTS = ('pse_suggest_params', 'pse_create', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
+           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_step', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
+
+
+class PSEError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f'{_STATUS.get(status, status)}: {msg}')
+        self.status = status
+
+
+def load_library():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f'{LIB_PATH} not found: build it with `python -m paper_1709_06946_b200.build` '
+                          '(there is no CPU fallback)')
+    lib = C.CDLL(LIB_PATH)
+    vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
+    lib.pse_suggest_params.argtypes = [i32, dbl, dbl, dbl, dbl, C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
+    lib.pse_create.argtypes = [C.POINTER(vp), i32, dbl, dbl, dbl, dbl, dbl, i32, i32, dbl, dbl, vp]
+    lib.pse_destroy.argtypes = [vp]
+    lib.pse_neighbors.argtypes = [vp, vp]
+    lib.pse_mobility_apply.argtypes = [vp, vp, vp, vp, vp, i32]
+    lib.pse_brownian.argtypes = [vp, dbl, vp, vp, vp, vp, C.POINTER(i32)]
+    lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
+    lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
+    lib.pse_step.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
+    lib.pse_get_neighbors.argtypes = [vp, vp, vp, C.c_size_t, C.POINTER(C.c_size_t)]
+    lib.pse_set_profiling.argtypes = [vp, i32]
+    lib.pse_get_timings.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32), i32]
+    lib.pse_kernel_launches.argtypes = [vp]
+    lib.pse_kernel_launches.restype = C.c_longlong
+    lib.pse_get_table.argtypes = [vp, vp, i32, C.POINTER(i32), C.POINTER(dbl)]
+    lib.pse_last_error.argtypes = [vp]
+    lib.pse_last_error.restype = C.c_char_p
+    lib.pse_version.restype = C.c_char_p
+    return lib
+
+
+_lib = load_library()
+
+
+def _ptr(t, shape=None):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError('expected a contiguous CUDA tensor')
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f'expected shape {tuple(shape)}, got {tuple(t.shape)}')
+    return C.c_void_p(t.data_ptr())
+
+
+def pse_version():
+    return _lib.pse_version().decode()
+
+
+def pse_suggest_params(N, L, a, tol, xi):
+    """-> (status, grid, P, rcut); see include/pse.h."""
+    g, p, rc = C.c_int(), C.c_int(), C.c_double()
+    st = _lib.pse_suggest_params(N, L, a, tol, xi, C.byref(g), C.byref(p), C.byref(rc))
+    return st, g.value, p.value, rc.value
+
+
+class Context:
+    """Owns a pse_ctx*.  Methods are one-to-one with the C calls of the same name."""
+
+    def __init__(self, N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None):
+        self.N, self.L, self.grid, self.P = int(N), float(L), int(grid), int(P)
+        self._h = C.c_void_p()
+        sp = C.c_void_p(stream.cuda_stream) if stream is not None else None
+        st = _lib.pse_create(C.byref(self._h), N, L, a, eta, kT, xi, grid, P, rcut, tol, sp)
+        if st != PSE_OK:
+            msg = _lib.pse_last_error(self._h).decode() if self._h else 'allocation failed'
+            if self._h:
+                _lib.pse_destroy(self._h)
+                self._h = C.c_void_p()
+            raise PSEError(st, msg)
+
+    def _check(self, st, allow=()):
+        if st != PSE_OK and st not in allow:
+            raise PSEError(st, _lib.pse_last_error(self._h).decode())
+        return st
+
+    def close(self):
+        if getattr(self, '_h', None):
+            _lib.pse_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def pse_neighbors(self, pos):
+        self._check(_lib.pse_neighbors(self._h, _ptr(pos, (self.N, 4))))
+
+    def pse_mobility_apply(self, F, S, U, E, which=PSE_BOTH):
+        N = self.N
+        self._check(_lib.pse_mobility_apply(self._h, _ptr(F, (N, 3)), _ptr(S, (N, 5)), _ptr(U, (N, 3)), _ptr(E, (N, 5)), which))
+
+    def pse_brownian(self, dt, noise_real, noise_wave, UB, EB, allow_noconv=False):
+        N, M = self.N, self.grid
+        it = C.c_int()
+        self._check(_lib.pse_brownian(self._h, dt, _ptr(noise_real, (N, 8)), _ptr(noise_wave, (3, M, M, M // 2 + 1, 2)),
+                                      _ptr(UB, (N, 3)), _ptr(EB, (N, 5)), C.byref(it)), (PSE_ENOCONV,) if allow_noconv else ())
+        return it.value
+
+    def pse_constrained_solve(self, F, UB, EB, U, S):
+        N = self.N
+        it = C.c_int()
+        self._check(_lib.pse_constrained_solve(self._h, _ptr(F, (N, 3)), _ptr(UB, (N, 3)), _ptr(EB, (N, 5)),
+                                               _ptr(U, (N, 3)), _ptr(S, (N, 5)), C.byref(it)))
+        return it.value
+
+    def pse_hard_sphere_forces(self, dt, F):
+        self._check(_lib.pse_hard_sphere_forces(self._h, dt, _ptr(F, (self.N, 3))))
+
+    def pse_step(self, pos, dt, noise_real, noise_wave):
+        N, M = self.N, self.grid
+        gi, li = C.c_int(), C.c_int()
+        self._check(_lib.pse_step(self._h, _ptr(pos, (N, 4)), dt, _ptr(noise_real, (N, 8)),
+                                  _ptr(noise_wave, (3, M, M, M // 2 + 1, 2)), C.byref(gi), C.byref(li)))
+        return gi.value, li.value
+
+    def pse_get_neighbors(self):
+        """-> (count [N] int32 tensor, index [total] int32 tensor) in original particle numbering."""
+        total = C.c_size_t()
+        count = torch.empty(self.N, dtype=torch.int32, device='cuda')
+        self._check(_lib.pse_get_neighbors(self._h, _ptr(count), None, 0, C.byref(total)))
+        index = torch.empty(max(total.value, 1), dtype=torch.int32, device='cuda')
+        self._check(_lib.pse_get_neighbors(self._h, _ptr(count), _ptr(index), index.numel(), C.byref(total)))
+        return count, index[:total.value]
+
+    def pse_set_profiling(self, on):
+        self._check(_lib.pse_set_profiling(self._h, int(bool(on))))
+
+    def pse_get_timings(self):
+        n = len(PHASES)
+        ms, cnt = (C.c_float * n)(), (C.c_int * n)()
+        self._check(_lib.pse_get_timings(self._h, ms, cnt, n))
+        return {PHASES[i]: (float(ms[i]), int(cnt[i])) for i in range(n)}
+
+    def pse_kernel_launches(self):
+        return int(_lib.pse_kernel_launches(self._h))
+
+    def pse_get_table(self):
+        import numpy as np
+        n, dr = C.c_int(), C.c_double()
+        self._check(_lib.pse_get_table(self._h, None, 0, C.byref(n), C.byref(dr)))
+        tab = np.empty((n.value, 8), dtype=np.float32)
+        self._check(_lib.pse_get_table(self._h, tab.ctypes.data_as(C.c_void_p), n.value, C.byref(n), C.byref(dr)))
+        return tab, dr.value
+
+
+def pse_create(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None):
+    return Context(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream)

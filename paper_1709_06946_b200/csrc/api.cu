@@ -1,0 +1,226 @@
+// C-ABI entry points of libpse (include/pse.h).
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include "pse_internal.h"
+
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which);
+
+namespace {
+
+__global__ void k_advance(const float4 *pos_in, const float *U, float dt, float L, float invL, int N, float4 *pos_out, int wrap) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float4 p = pos_in[i];
+    p.x += dt * U[3 * i]; p.y += dt * U[3 * i + 1]; p.z += dt * U[3 * i + 2];
+    if (wrap) {
+        p.x -= L * floorf(p.x * invL); p.y -= L * floorf(p.y * invL); p.z -= L * floorf(p.z * invL);
+        if (p.x >= L || p.x < 0.f) p.x = 0.f;
+        if (p.y >= L || p.y < 0.f) p.y = 0.f;
+        if (p.z >= L || p.z < 0.f) p.z = 0.f;
+    }
+    pos_out[i] = p;
+}
+
+bool smooth7(int n) { for (int p : {2, 3, 5, 7}) while (n % p == 0) n /= p; return n == 1; }
+
+}  // namespace
+
+extern "C" {
+
+const char *pse_version(void) { return "libpse 0.1 (sm_100a)"; }
+
+const char *pse_last_error(const pse_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+long long pse_kernel_launches(const pse_ctx *c) { return c ? c->launches : 0; }
+
+pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, int *grid, int *P, double *rcut) {
+    if (N <= 0 || !(L > 0) || !(a > 0) || !(tol > 0 && tol < 1) || !(xi > 0)) return PSE_EINVAL;
+    const double s = std::sqrt(-std::log(tol));
+    // C1: functions decay like exp(-xi^2 (r-2a)^2), so the paper's estimate r = s/xi
+    // is shifted by the sphere diameter.
+    double rc = s / xi + 2.0 * a;
+    // C2: wave cutoff k_cut = 2 xi s (H(k) ~ exp(-k^2/4 xi^2)); M >= k_cut L / pi, rounded up to a 2,3,5,7-smooth size
+    int M = std::max(8, (int)std::ceil(2.0 * xi * s * L / M_PI));
+    while (!smooth7(M)) ++M;
+    // C3: quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1)
+    int p = 2;
+    while (p < PSE_MAXP && std::exp(-M_PI * p / 2.0) + std::erfc(std::sqrt(M_PI * p / 2.0)) > tol) ++p;
+    if (grid) *grid = M;
+    if (P) *P = p;
+    if (rcut) *rcut = rc;
+    if (rc > 0.5 * L || p > M) return PSE_EINVAL;
+    return PSE_OK;
+}
+
+pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
+                      int grid, int P, double rcut, double tol, void *cuda_stream) {
+    if (!out) return PSE_EINVAL;
+    *out = nullptr;
+    pse_ctx *c = new (std::nothrow) pse_ctx;
+    if (!c) return PSE_ENOMEM;
+    *out = c;                                   // returned even on failure so pse_last_error works; caller destroys
+    c->stream = (cudaStream_t)cuda_stream;
+    if (N <= 0 || !(L > 0) || !(a > 0) || !(eta > 0) || !(kT >= 0) || !(xi > 0) || grid < 2 || P < 2 || !(rcut > 0) || !(tol > 0)) {
+        c->err = "pse_create: non-positive or missing parameter"; return PSE_EINVAL;
+    }
+    if (rcut > 0.5 * L) { c->err = "pse_create: rcut > L/2 (minimum-image real-space sum)"; return PSE_EINVAL; }
+    if (rcut < 2.0 * a) { c->err = "pse_create: rcut < 2a (overlap forces need contact pairs)"; return PSE_EINVAL; }
+    if (P > grid || P > PSE_MAXP) { c->err = "pse_create: P > grid or P > 16"; return PSE_EINVAL; }
+    c->N = N; c->L = L; c->a = a; c->eta = eta; c->kT = kT; c->xi = xi; c->M = grid; c->P = P; c->rcut = rcut; c->tol = tol;
+    c->h = L / grid;
+    c->eta_g = (c->h * P * xi) * (c->h * P * xi) / (M_PI * P);         // (h P xi/m)^2, m^2 = pi P
+    if (!(c->eta_g < 1.0)) { c->err = "pse_create: Gaussian shape parameter eta_g >= 1 (grid too coarse for this xi and P)"; return PSE_EINVAL; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { c->err = "no CUDA device (libpse has no CPU fallback)"; return PSE_ECUDA; }
+    // real-space table
+    std::vector<float> tab;
+    pse_build_table(a, eta, xi, rcut, PSE_NTAB, tab, &c->tab_dr);
+    CUDA_TRY(c, cudaMalloc(&c->d_table, tab.size() * sizeof(float)));
+    CUDA_TRY(c, cudaMemcpy(c->d_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    // cells: edge >= rcut with a relative margin far above fp32 rounding of the binning
+    c->nc = std::max(1, (int)std::floor(L / (rcut * 1.0001)));
+    c->ncell = c->nc * c->nc * c->nc;
+    const size_t n8 = (size_t)N * 8 * sizeof(float);
+    CUDA_TRY(c, cudaMalloc(&c->d_pos, (size_t)N * sizeof(float4)));
+    CUDA_TRY(c, cudaMalloc(&c->d_posw, (size_t)N * sizeof(float4)));
+    CUDA_TRY(c, cudaMalloc(&c->d_order, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_cell_of, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_cell_count, (size_t)(c->ncell + 1) * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_cell_start, (size_t)(c->ncell + 1) * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_cell_fill, (size_t)(c->ncell + 1) * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_nbr_count, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_nbr_off, (size_t)(N + 1) * sizeof(unsigned long long)));
+    for (float **p : {&c->d_in, &c->d_out, &c->d_tmp, &c->d_tmp2, &c->d_vecA, &c->d_vecB, &c->d_vecC, &c->d_vecD}) CUDA_TRY(c, cudaMalloc(p, n8));
+    c->krylov_cap = PSE_MAX_KRYLOV + 1;
+    CUDA_TRY(c, cudaMalloc(&c->d_krylov, (size_t)c->krylov_cap * n8));
+    CUDA_TRY(c, cudaMalloc(&c->d_zu, (size_t)PSE_MAX_KRYLOV * n8));
+    CUDA_TRY(c, cudaMalloc(&c->d_scal, 64 * sizeof(double)));
+    CUDA_TRY(c, cudaMallocHost(&c->h_scal, 256 * sizeof(double)));
+    CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
+    PSE_TRY(pse_wave_init(c));
+    return PSE_OK;
+}
+
+pse_status pse_destroy(pse_ctx *c) {
+    if (!c) return PSE_OK;
+    cudaStreamSynchronize(c->stream);
+    pse_wave_free(c);
+    for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
+    cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_cell_of);
+    cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_fill); cudaFree(c->d_nbr_count);
+    cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx);
+    for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
+    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    delete c;
+    return PSE_OK;
+}
+
+pse_status pse_neighbors(pse_ctx *c, const float *d_pos) {
+    if (!c || !d_pos) return PSE_EINVAL;
+    return pse_neighbors_impl(c, d_pos);
+}
+
+pse_status pse_get_neighbors(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total) {
+    if (!c) return PSE_EINVAL;
+    return pse_get_neighbors_impl(c, d_count, d_index, cap, total);
+}
+
+pse_status pse_mobility_apply(pse_ctx *c, const float *d_F, const float *d_S, float *d_U, float *d_E, int which) {
+    if (!c || !(which & PSE_BOTH) || (!d_F && !d_S)) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_mobility_apply before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(pse_pack(c, d_F, d_S, c->d_in));
+    PSE_TRY(pse_apply_packed(c, c->d_in, c->d_out, which));
+    return pse_unpack(c, c->d_out, 1.f, d_U, d_E);
+}
+
+pse_status pse_brownian(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters) {
+    if (!c || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_brownian before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(pse_pack8(c, d_noise_real, c->d_in));
+    pse_status st = pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters);
+    if (st != PSE_OK && st != PSE_ENOCONV) return st;
+    PSE_TRY(pse_wave_brownian(c, d_noise_wave, c->d_out, true));
+    PSE_TRY(pse_unpack(c, c->d_out, (float)std::sqrt(2.0 * c->kT / dt), d_UB, d_EB));
+    return st;
+}
+
+pse_status pse_hard_sphere_forces(pse_ctx *c, double dt, float *d_F) {
+    if (!c || !(dt > 0) || !d_F) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_hard_sphere_forces before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+    return pse_unpack(c, c->d_vecA, 1.f, d_F, nullptr);
+}
+
+pse_status pse_constrained_solve(pse_ctx *c, const float *d_F, const float *d_UB, const float *d_EB, float *d_U, float *d_S, int *gmres_iters) {
+    if (!c || !d_U || !d_S) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_constrained_solve before pse_neighbors"; return PSE_ENOTREADY; }
+    if (d_F) PSE_TRY(pse_pack(c, d_F, nullptr, c->d_vecA));
+    PSE_TRY(pse_pack(c, d_UB, d_EB, c->d_vecB));
+    pse_status st = pse_gmres_constraint(c, d_F ? c->d_vecA : nullptr, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
+    if (st != PSE_OK && st != PSE_ENOCONV) return st;
+    PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, d_U, d_S));
+    return st;
+}
+
+pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave, int *gmres_iters, int *lanczos_iters) {
+    if (!c || !d_pos || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
+    const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
+    const float L = (float)c->L, invL = 1.0f / L;
+    float *UB = c->d_vecD, *EB = c->d_vecD + (size_t)3 * N;           // original numbering: [N][3] then [N][5]
+    float4 *xh = reinterpret_cast<float4 *>(c->d_zu);                  // scratch for x_{k+1/2}; d_zu is rewritten by GMRES afterwards
+    pse_status soft = PSE_OK;
+    // (76) Brownian slip at x_k
+    PSE_TRY(pse_neighbors_impl(c, d_pos));
+    pse_status st = pse_brownian(c, dt, d_noise_real, d_noise_wave, UB, EB, lanczos_iters);
+    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
+    // (77) mid-point
+    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+    PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
+    // (78) constrained solve at the mid-point with hard-sphere forces (reading R12)
+    PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+    PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
+    st = pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
+    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
+    PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));     // U_{k+1/2}, original numbering [N][3]
+    // (79) full step from x_k
+    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
+                                        reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+    return soft;
+}
+
+pse_status pse_set_profiling(pse_ctx *c, int on) { if (!c) return PSE_EINVAL; c->profiling = on != 0; return PSE_OK; }
+
+pse_status pse_get_timings(pse_ctx *c, float *h_ms, int *h_launches, int n) {
+    if (!c) return PSE_EINVAL;
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (Timer &t : c->timers) {
+        float ms = 0; cudaEventElapsedTime(&ms, t.a, t.b);
+        c->acc_ms[t.phase] += ms; c->acc_n[t.phase]++;
+        cudaEventDestroy(t.a); cudaEventDestroy(t.b);
+    }
+    c->timers.clear();
+    for (int i = 0; i < n && i < PSE_T_COUNT; ++i) { if (h_ms) h_ms[i] = c->acc_ms[i]; if (h_launches) h_launches[i] = c->acc_n[i]; }
+    for (int i = 0; i < PSE_T_COUNT; ++i) { c->acc_ms[i] = 0; c->acc_n[i] = 0; }
+    return PSE_OK;
+}
+
+pse_status pse_get_table(pse_ctx *c, float *h_table, int cap_nodes, int *n_nodes, double *dr) {
+    if (!c) return PSE_EINVAL;
+    if (n_nodes) *n_nodes = PSE_NTAB;
+    if (dr) *dr = c->tab_dr;
+    if (h_table) {
+        if (cap_nodes < PSE_NTAB) return PSE_EOVERFLOW;
+        CUDA_TRY(c, cudaMemcpy(h_table, c->d_table, (size_t)PSE_NTAB * 8 * sizeof(float), cudaMemcpyDeviceToHost));
+    }
+    return PSE_OK;
+}
+
+}  // extern "C"
+
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which) {
+    if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out));
+    if (which & PSE_WAVE) PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0));
+    return PSE_OK;
+}

@@ -1,0 +1,340 @@
+// Device Krylov drivers (steps a8, a9): Lanczos for M_r^{1/2} w (Chow & Saad) and GMRES for the
+// stresslet constraint M_ES S = -(E^B + M_EF F) (Eqs. 36-38, 78; 8-10 iterations,
+// PAPER.md:561).  All vectors live on the device in the packed, cell-sorted layout [N][8] = (x,y,z,e1..e5); only
+// the few scalars per iteration (dots, norms) cross to the host, where the tiny tridiagonal / Hessenberg work is
+// done in fp64.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include "pse_internal.h"
+
+namespace {
+
+constexpr int VT = 256;
+inline int vgrid(size_t n4) { size_t b = (n4 + VT - 1) / VT; return (int)(b < 1184 ? (b ? b : 1) : 1184); }   // 8 x 148
+
+__device__ __forceinline__ double block_sum(double v) {
+    __shared__ double sh[VT / 32];
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double r = 0;
+    if (threadIdx.x < 32) {
+        r = threadIdx.x < VT / 32 ? sh[threadIdx.x] : 0.0;
+        for (int o = 16; o; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    }
+    __syncthreads();
+    return r;
+}
+
+__global__ void k_pack(const float *F, const float *S, const int *order, int N, float4 *packed) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    int o = order[s];
+    float f0 = 0, f1 = 0, f2 = 0, s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+    if (F) { f0 = F[3 * o]; f1 = F[3 * o + 1]; f2 = F[3 * o + 2]; }
+    if (S) { s0 = S[5 * o]; s1 = S[5 * o + 1]; s2 = S[5 * o + 2]; s3 = S[5 * o + 3]; s4 = S[5 * o + 4]; }
+    packed[2 * s] = make_float4(f0, f1, f2, s0); packed[2 * s + 1] = make_float4(s1, s2, s3, s4);
+}
+
+__global__ void k_pack8(const float4 *v8, const int *order, int N, float4 *packed) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    int o = order[s];
+    packed[2 * s] = v8[2 * o]; packed[2 * s + 1] = v8[2 * o + 1];
+}
+
+__global__ void k_unpack(const float4 *packed, const int *order, int N, float scale, float *U, float *E) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    int o = order[s];
+    float4 a = packed[2 * s], b = packed[2 * s + 1];
+    if (U) { U[3 * o] = scale * a.x; U[3 * o + 1] = scale * a.y; U[3 * o + 2] = scale * a.z; }
+    if (E) { E[5 * o] = scale * a.w; E[5 * o + 1] = scale * b.x; E[5 * o + 2] = scale * b.y; E[5 * o + 3] = scale * b.z; E[5 * o + 4] = scale * b.w; }
+}
+
+// out[j] += <V_j, w>, j < nvec  (V_j = base + j*stride)
+__global__ void __launch_bounds__(VT) k_multi_dot(const float4 *base, size_t stride4, int nvec, const float4 *w, size_t n4, double *out) {
+    for (int j = 0; j < nvec; ++j) {
+        const float4 *v = base + (size_t)j * stride4;
+        double acc = 0;
+        for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
+            float4 a = v[i], b = w[i];
+            acc += (double)(a.x * b.x + a.y * b.y) + (double)(a.z * b.z + a.w * b.w);
+        }
+        acc = block_sum(acc);
+        if (threadIdx.x == 0) atomicAdd(out + j, acc);
+    }
+}
+
+// u -= sum_j coef[j] V_j ;  *norm2 += |u|^2
+__global__ void __launch_bounds__(VT) k_sub_lincomb_norm(float4 *u, const float4 *base, size_t stride4, int nvec, const float *coef,
+                                                         size_t n4, double *norm2) {
+    double acc = 0;
+    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
+        float4 x = u[i];
+        for (int j = 0; j < nvec; ++j) {
+            float4 v = base[(size_t)j * stride4 + i]; float cj = coef[j];
+            x.x -= cj * v.x; x.y -= cj * v.y; x.z -= cj * v.z; x.w -= cj * v.w;
+        }
+        u[i] = x;
+        acc += (double)(x.x * x.x + x.y * x.y) + (double)(x.z * x.z + x.w * x.w);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) atomicAdd(norm2, acc);
+}
+
+// out = beta * init + sum_j coef[j] V_j   (init may be null)
+__global__ void __launch_bounds__(VT) k_lincomb(float4 *out, const float4 *init, float beta, const float4 *base, size_t stride4, int nvec,
+                                                const float *coef, size_t n4) {
+    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
+        float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (init) { x = init[i]; x.x *= beta; x.y *= beta; x.z *= beta; x.w *= beta; }
+        for (int j = 0; j < nvec; ++j) {
+            float4 v = base[(size_t)j * stride4 + i]; float cj = coef[j];
+            x.x += cj * v.x; x.y += cj * v.y; x.z += cj * v.z; x.w += cj * v.w;
+        }
+        out[i] = x;
+    }
+}
+
+// y = alpha x + beta y
+__global__ void __launch_bounds__(VT) k_axpby(size_t n, float alpha, const float *x, float beta, float *y) {
+    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n; i += (size_t)gridDim.x * VT)
+        y[i] = alpha * x[i] + (beta != 0.f ? beta * y[i] : 0.f);
+}
+
+// dst = scale * src with the velocity components (0..2 of every 8) zeroed: the E-part embedding used by GMRES
+__global__ void __launch_bounds__(VT) k_epart(float4 *dst, const float4 *src, float scale, int N) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    float4 a = src[2 * s], b = src[2 * s + 1];
+    dst[2 * s] = make_float4(0.f, 0.f, 0.f, scale * a.w);
+    dst[2 * s + 1] = make_float4(scale * b.x, scale * b.y, scale * b.z, scale * b.w);
+}
+
+// rhs = -(EB + E-part(z0)) embedded with zero velocity components (either input may be null)
+__global__ void __launch_bounds__(VT) k_rhs(float4 *dst, const float4 *EBp, const float4 *z0, int N) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    float4 a = make_float4(0, 0, 0, 0), b = a;
+    if (EBp) { a = EBp[2 * s]; b = EBp[2 * s + 1]; }
+    if (z0) { float4 c = z0[2 * s], d = z0[2 * s + 1]; a.w += c.w; b.x += d.x; b.y += d.y; b.z += d.z; b.w += d.w; }
+    dst[2 * s] = make_float4(0.f, 0.f, 0.f, -a.w);
+    dst[2 * s + 1] = make_float4(-b.x, -b.y, -b.z, -b.w);
+}
+
+// out = ( UB + U(z0) + sum_j y_j U(Z_j) ; sum_j y_j V_j )
+__global__ void __launch_bounds__(VT) k_constraint_result(float4 *out, const float4 *UBp, const float4 *z0, const float4 *Z, const float4 *V,
+                                                          size_t stride4, int nvec, const float *y, int N) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    float ux = 0, uy = 0, uz = 0;
+    float4 sa = make_float4(0, 0, 0, 0), sb = sa;
+    if (UBp) { float4 a = UBp[2 * s]; ux = a.x; uy = a.y; uz = a.z; }
+    if (z0) { float4 a = z0[2 * s]; ux += a.x; uy += a.y; uz += a.z; }
+    for (int j = 0; j < nvec; ++j) {
+        float yj = y[j];
+        float4 z = Z[(size_t)j * stride4 + 2 * s], va = V[(size_t)j * stride4 + 2 * s], vb = V[(size_t)j * stride4 + 2 * s + 1];
+        ux += yj * z.x; uy += yj * z.y; uz += yj * z.z;
+        sa.w += yj * va.w; sb.x += yj * vb.x; sb.y += yj * vb.y; sb.z += yj * vb.z; sb.w += yj * vb.w;
+    }
+    out[2 * s] = make_float4(ux, uy, uz, sa.w); out[2 * s + 1] = sb;
+}
+
+// cyclic Jacobi eigen-decomposition of a small symmetric matrix (n <= 51), fp64, host
+void jacobi_eigh(int n, std::vector<double> &A, std::vector<double> &Q) {
+    Q.assign((size_t)n * n, 0.0);
+    for (int i = 0; i < n; ++i) Q[(size_t)i * n + i] = 1.0;
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        double off = 0;
+        for (int p = 0; p < n; ++p) for (int q = p + 1; q < n; ++q) off += A[(size_t)p * n + q] * A[(size_t)p * n + q];
+        if (off < 1e-30) break;
+        for (int p = 0; p < n; ++p) for (int q = p + 1; q < n; ++q) {
+            double apq = A[(size_t)p * n + q];
+            if (std::fabs(apq) < 1e-300) continue;
+            double th = (A[(size_t)q * n + q] - A[(size_t)p * n + p]) / (2 * apq);
+            double t = (th >= 0 ? 1.0 : -1.0) / (std::fabs(th) + std::sqrt(th * th + 1)), cs = 1 / std::sqrt(t * t + 1), sn = t * cs;
+            for (int k = 0; k < n; ++k) {
+                double akp = A[(size_t)k * n + p], akq = A[(size_t)k * n + q];
+                A[(size_t)k * n + p] = cs * akp - sn * akq; A[(size_t)k * n + q] = sn * akp + cs * akq;
+            }
+            for (int k = 0; k < n; ++k) {
+                double apk = A[(size_t)p * n + k], aqk = A[(size_t)q * n + k];
+                A[(size_t)p * n + k] = cs * apk - sn * aqk; A[(size_t)q * n + k] = sn * apk + cs * aqk;
+            }
+            for (int k = 0; k < n; ++k) {
+                double qkp = Q[(size_t)k * n + p], qkq = Q[(size_t)k * n + q];
+                Q[(size_t)k * n + p] = cs * qkp - sn * qkq; Q[(size_t)k * n + q] = sn * qkp + cs * qkq;
+            }
+        }
+    }
+}
+
+pse_status read_scalars(pse_ctx *c, int n) {
+    CUDA_TRY(c, cudaMemcpyAsync(c->h_scal, c->d_scal, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PSE_OK;
+}
+pse_status zero_scalars(pse_ctx *c, int n) {
+    CUDA_TRY(c, cudaMemsetAsync(c->d_scal, 0, (size_t)n * sizeof(double), c->stream));
+    return PSE_OK;
+}
+pse_status upload_coefs(pse_ctx *c, const std::vector<float> &v) {
+    float *hp = reinterpret_cast<float *>(c->h_scal + 128);
+    std::memcpy(hp, v.data(), v.size() * sizeof(float));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_coef, hp, v.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    return PSE_OK;
+}
+
+}  // namespace
+
+pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed) {
+    ScopedPhase ph(c, PSE_T_PACK);
+    k_pack<<<(c->N + VT - 1) / VT, VT, 0, c->stream>>>(d_F, d_S, c->d_order, c->N, reinterpret_cast<float4 *>(d_packed)); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed) {
+    ScopedPhase ph(c, PSE_T_PACK);
+    k_pack8<<<(c->N + VT - 1) / VT, VT, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_v8), c->d_order, c->N, reinterpret_cast<float4 *>(d_packed)); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+pse_status pse_unpack(pse_ctx *c, const float *d_packed, float scale, float *d_U, float *d_E) {
+    ScopedPhase ph(c, PSE_T_PACK);
+    k_unpack<<<(c->N + VT - 1) / VT, VT, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_packed), c->d_order, c->N, scale, d_U, d_E); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+pse_status pse_axpby(pse_ctx *c, size_t n, float alpha, const float *x, float beta, float *y) {
+    ScopedPhase ph(c, PSE_T_VECTOR);
+    k_axpby<<<vgrid(n), VT, 0, c->stream>>>(n, alpha, x, beta, y); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
+// y = M_r^{1/2} w  by Lanczos:  v_1 = w/|w|,  T_m = V_m^T M_r V_m,  y_m = |w| V_m T_m^{1/2} e_1.
+// Stop when |y_m - y_{m-1}| <= tol |y_m|; with V orthonormal this is the change of the coefficient vector.
+pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters) {
+    const size_t n = (size_t)c->N * 8, n4 = n / 4;
+    float4 *V = reinterpret_cast<float4 *>(c->d_krylov);
+    float4 *u = reinterpret_cast<float4 *>(c->d_tmp);
+    const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap - 1);
+    PSE_TRY(zero_scalars(c, 1));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_w), 0, 1, reinterpret_cast<const float4 *>(d_w), n4, c->d_scal); KERNEL_CHECK(c); }
+    PSE_TRY(read_scalars(c, 1));
+    const double wn = std::sqrt(c->h_scal[0]);
+    if (iters) *iters = 0;
+    if (!(wn > 0)) { CUDA_TRY(c, cudaMemsetAsync(d_y, 0, n * sizeof(float), c->stream)); return PSE_OK; }
+    PSE_TRY(pse_axpby(c, n, (float)(1.0 / wn), d_w, 0.f, reinterpret_cast<float *>(V)));
+    std::vector<double> alpha, beta, cprev, ccur;
+    int m = 0;
+    bool converged = false;
+    for (int j = 0; j < maxit; ++j) {
+        PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(V + (size_t)j * n4), reinterpret_cast<float *>(u)));
+        PSE_TRY(zero_scalars(c, 2));
+        { ScopedPhase ph(c, PSE_T_VECTOR);
+          k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V + (size_t)j * n4, 0, 1, u, n4, c->d_scal); KERNEL_CHECK(c); }
+        PSE_TRY(read_scalars(c, 1));
+        alpha.push_back(c->h_scal[0]);
+        std::vector<float> cf;
+        int nv = 1; const float4 *base = V + (size_t)j * n4;
+        if (j > 0) { cf = {(float)beta[j - 1], (float)alpha[j]}; nv = 2; base = V + (size_t)(j - 1) * n4; } else cf = {(float)alpha[j]};
+        PSE_TRY(upload_coefs(c, cf));
+        { ScopedPhase ph(c, PSE_T_VECTOR);
+          k_sub_lincomb_norm<<<vgrid(n4), VT, 0, c->stream>>>(u, base, n4, nv, c->d_coef, n4, c->d_scal + 1); KERNEL_CHECK(c); }
+        PSE_TRY(read_scalars(c, 2));
+        beta.push_back(std::sqrt(c->h_scal[1]));
+        m = j + 1;
+        // coefficient vector  c = |w| T^{1/2} e_1  of the m x m tridiagonal
+        std::vector<double> Tm((size_t)m * m, 0.0), Q;
+        for (int i = 0; i < m; ++i) { Tm[(size_t)i * m + i] = alpha[i]; if (i + 1 < m) Tm[(size_t)i * m + i + 1] = Tm[(size_t)(i + 1) * m + i] = beta[i]; }
+        jacobi_eigh(m, Tm, Q);
+        ccur.assign(m, 0.0);
+        for (int e = 0; e < m; ++e) {
+            double lam = Tm[(size_t)e * m + e], sq = lam > 0 ? std::sqrt(lam) : 0.0, q0 = Q[e];       // Q[0][e]
+            for (int i = 0; i < m; ++i) ccur[i] += wn * Q[(size_t)i * m + e] * sq * q0;
+        }
+        double diff = 0, nrm = 0;
+        for (int i = 0; i < m; ++i) { double d = ccur[i] - (i < (int)cprev.size() ? cprev[i] : 0.0); diff += d * d; nrm += ccur[i] * ccur[i]; }
+        cprev = ccur;
+        if (j > 0 && std::sqrt(diff) <= c->tol * std::sqrt(nrm)) { converged = true; break; }
+        if (beta[j] <= 1e-7 * std::fabs(alpha[0])) { converged = true; break; }          // invariant subspace
+        if (j + 1 < maxit) PSE_TRY(pse_axpby(c, n, (float)(1.0 / beta[j]), reinterpret_cast<const float *>(u), 0.f, reinterpret_cast<float *>(V + (size_t)(j + 1) * n4)));
+    }
+    std::vector<float> cf(ccur.begin(), ccur.end());
+    PSE_TRY(upload_coefs(c, cf));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_lincomb<<<vgrid(n4), VT, 0, c->stream>>>(reinterpret_cast<float4 *>(d_y), nullptr, 0.f, V, n4, m, c->d_coef, n4); KERNEL_CHECK(c); }
+    if (iters) *iters = m;
+    if (!converged) { c->err = "Lanczos did not converge"; return PSE_ENOCONV; }
+    return PSE_OK;
+}
+
+// Forward declaration of the full product on packed vectors (api.cu)
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which);
+
+// GMRES on  M_ES S = -(E^B + M_EF F)  with S and E embedded in packed vectors whose velocity slots are zero.
+// Z_j = M [0; v_j] is kept whole: its E-part feeds Arnoldi, its U-part gives M_US S at the end without another
+// product.  out (packed) = (U, S) with U = U^B + M_UF F + M_US S.
+pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp, float *d_outp, int *iters) {
+    const int N = c->N;
+    const size_t n = (size_t)N * 8, n4 = n / 4;
+    float4 *V = reinterpret_cast<float4 *>(c->d_krylov), *Z = reinterpret_cast<float4 *>(c->d_zu);
+    float4 *w = reinterpret_cast<float4 *>(c->d_tmp), *z0 = reinterpret_cast<float4 *>(c->d_tmp2);
+    const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap - 1), nbN = (N + VT - 1) / VT;
+    if (iters) *iters = 0;
+    if (d_Fp) PSE_TRY(pse_apply_packed(c, d_Fp, reinterpret_cast<float *>(z0), PSE_BOTH));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_rhs<<<nbN, VT, 0, c->stream>>>(w, reinterpret_cast<const float4 *>(d_EBp), d_Fp ? z0 : nullptr, N); KERNEL_CHECK(c); }
+    PSE_TRY(zero_scalars(c, 1));
+    { ScopedPhase ph(c, PSE_T_VECTOR); k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(w, 0, 1, w, n4, c->d_scal); KERNEL_CHECK(c); }
+    PSE_TRY(read_scalars(c, 1));
+    const double bnorm = std::sqrt(c->h_scal[0]);
+    int m = 0;
+    std::vector<double> H((size_t)(maxit + 1) * maxit, 0.0), cs(maxit, 0.0), sn(maxit, 0.0), g(maxit + 1, 0.0), y;
+    bool converged = !(bnorm > 0);
+    if (!converged) {
+        g[0] = bnorm;
+        PSE_TRY(pse_axpby(c, n, (float)(1.0 / bnorm), reinterpret_cast<const float *>(w), 0.f, reinterpret_cast<float *>(V)));
+        for (int k = 0; k < maxit; ++k) {
+            PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Z + (size_t)k * n4), PSE_BOTH));
+            { ScopedPhase ph(c, PSE_T_VECTOR); k_epart<<<nbN, VT, 0, c->stream>>>(w, Z + (size_t)k * n4, 1.f, N); KERNEL_CHECK(c); }
+            PSE_TRY(zero_scalars(c, k + 2));
+            { ScopedPhase ph(c, PSE_T_VECTOR); k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, w, n4, c->d_scal); KERNEL_CHECK(c); }
+            PSE_TRY(read_scalars(c, k + 1));
+            std::vector<float> hf(k + 1);
+            for (int j = 0; j <= k; ++j) { H[(size_t)j * maxit + k] = c->h_scal[j]; hf[j] = (float)c->h_scal[j]; }
+            PSE_TRY(upload_coefs(c, hf));
+            { ScopedPhase ph(c, PSE_T_VECTOR);
+              k_sub_lincomb_norm<<<vgrid(n4), VT, 0, c->stream>>>(w, V, n4, k + 1, c->d_coef, n4, c->d_scal + k + 1); KERNEL_CHECK(c); }
+            PSE_TRY(read_scalars(c, k + 2));
+            const double hk1 = std::sqrt(c->h_scal[k + 1]);
+            H[(size_t)(k + 1) * maxit + k] = hk1;
+            for (int j = 0; j < k; ++j) {                        // apply previous Givens rotations to column k
+                double a = H[(size_t)j * maxit + k], b = H[(size_t)(j + 1) * maxit + k];
+                H[(size_t)j * maxit + k] = cs[j] * a + sn[j] * b; H[(size_t)(j + 1) * maxit + k] = -sn[j] * a + cs[j] * b;
+            }
+            double a = H[(size_t)k * maxit + k], b = H[(size_t)(k + 1) * maxit + k], r = std::hypot(a, b);
+            cs[k] = r > 0 ? a / r : 1.0; sn[k] = r > 0 ? b / r : 0.0;
+            H[(size_t)k * maxit + k] = r; H[(size_t)(k + 1) * maxit + k] = 0.0;
+            g[k + 1] = -sn[k] * g[k]; g[k] = cs[k] * g[k];
+            m = k + 1;
+            if (std::fabs(g[k + 1]) <= c->tol * bnorm) { converged = true; break; }
+            if (hk1 <= 1e-12 * bnorm) { converged = true; break; }
+            if (k + 1 < maxit) PSE_TRY(pse_axpby(c, n, (float)(1.0 / hk1), reinterpret_cast<const float *>(w), 0.f, reinterpret_cast<float *>(V + (size_t)(k + 1) * n4)));
+        }
+        y.assign(m, 0.0);
+        for (int i = m - 1; i >= 0; --i) {
+            double s = g[i];
+            for (int j = i + 1; j < m; ++j) s -= H[(size_t)i * maxit + j] * y[j];
+            y[i] = s / H[(size_t)i * maxit + i];
+        }
+    }
+    std::vector<float> yf(y.begin(), y.end());
+    if (m) PSE_TRY(upload_coefs(c, yf));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_constraint_result<<<nbN, VT, 0, c->stream>>>(reinterpret_cast<float4 *>(d_outp), reinterpret_cast<const float4 *>(d_UBp), d_Fp ? z0 : nullptr,
+                                                     Z, V, n4, m, c->d_coef, N); KERNEL_CHECK(c); }
+    if (iters) *iters = m;
+    if (!converged) { c->err = "GMRES did not converge"; return PSE_ENOCONV; }
+    return PSE_OK;
+}

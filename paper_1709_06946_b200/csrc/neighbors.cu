@@ -1,0 +1,278 @@
+// Cell list + full neighbour list (step a1; "linked-cell lists ... sub-cells of size r_cut").
+//
+// Design (sm_100a, not a translation of HOOMD's lists): counting sort of particles by cell (deterministic:
+// each cell's members are re-sorted by original index), positions gathered into cell order so that the pair
+// kernel's gathers hit 9 contiguous runs, then a warp-per-particle sweep of the 27-cell stencil with ballot
+// compaction, once to count and once to fill a CSR list.  The in/out decision is taken in fp32 with the exact
+// operation order of DESIGN.md reading R16 (no FMA contraction), so the sets are bit-identical to the oracle's.
+#include "pse_internal.h"
+
+namespace {
+
+constexpr int SCAN_ITEMS = 8, SCAN_THREADS = 256, SCAN_CHUNK = SCAN_ITEMS * SCAN_THREADS;
+
+__device__ __forceinline__ unsigned long long block_exclusive_scan(unsigned long long v, unsigned long long *total) {
+    __shared__ unsigned long long warp_sums[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    unsigned long long inc = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sums[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        unsigned long long s = (lane < (blockDim.x >> 5)) ? warp_sums[lane] : 0ull, si = s;
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long t = __shfl_up_sync(0xffffffffu, si, o);
+            if (lane >= o) si += t;
+        }
+        warp_sums[lane] = si - s;
+        if (lane == 31 && total) *total = si;
+    }
+    __syncthreads();
+    unsigned long long r = warp_sums[wid] + inc - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void scan_block_sums(const int *in, size_t n, unsigned long long *bsum) {
+    __shared__ unsigned long long tot;
+    size_t base = (size_t)blockIdx.x * SCAN_CHUNK + (size_t)threadIdx.x * SCAN_ITEMS;
+    unsigned long long s = 0;
+    for (int i = 0; i < SCAN_ITEMS; ++i) if (base + i < n) s += (unsigned long long)in[base + i];
+    block_exclusive_scan(s, &tot);
+    if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
+}
+
+__global__ void scan_of_sums(unsigned long long *bsum, size_t nb) {      // single block, in place, exclusive
+    __shared__ unsigned long long tot, carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (size_t lo = 0; lo < nb; lo += blockDim.x) {
+        size_t i = lo + threadIdx.x;
+        unsigned long long v = i < nb ? bsum[i] : 0ull;
+        unsigned long long e = block_exclusive_scan(v, &tot);
+        if (i < nb) bsum[i] = carry + e;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) bsum[nb] = carry;
+}
+
+template <typename OutT>
+__global__ void scan_apply(const int *in, size_t n, const unsigned long long *bsum, size_t nb, OutT *out) {
+    size_t base = (size_t)blockIdx.x * SCAN_CHUNK + (size_t)threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS]; unsigned long long s = 0;
+    for (int i = 0; i < SCAN_ITEMS; ++i) { v[i] = (base + i < n) ? in[base + i] : 0; s += (unsigned long long)v[i]; }
+    unsigned long long e = block_exclusive_scan(s, nullptr) + bsum[blockIdx.x];
+    for (int i = 0; i < SCAN_ITEMS; ++i) { if (base + i < n) out[base + i] = (OutT)e; e += (unsigned long long)v[i]; }
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = (OutT)bsum[nb];
+}
+
+template <typename OutT>
+pse_status scan_impl(pse_ctx *c, const int *d_in, OutT *d_out, size_t n) {
+    size_t nb = (n + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    if (nb == 0) nb = 1;
+    if (c->scan_tmp_n < nb + 1) {
+        if (c->d_scan_tmp) cudaFree(c->d_scan_tmp);
+        CUDA_TRY(c, cudaMalloc(&c->d_scan_tmp, (nb + 1) * sizeof(unsigned long long)));
+        c->scan_tmp_n = nb + 1;
+    }
+    scan_block_sums<<<(unsigned)nb, SCAN_THREADS, 0, c->stream>>>(d_in, n, c->d_scan_tmp); KERNEL_CHECK(c);
+    scan_of_sums<<<1, 1024, 0, c->stream>>>(c->d_scan_tmp, nb); KERNEL_CHECK(c);
+    scan_apply<OutT><<<(unsigned)nb, SCAN_THREADS, 0, c->stream>>>(d_in, n, c->d_scan_tmp, nb, d_out); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
+// ---- R16 arithmetic: every operation individually rounded, no contraction ----
+__device__ __forceinline__ float wrap_coord(float x, float L, float invL) {
+    float w = __fsub_rn(x, __fmul_rn(L, floorf(__fmul_rn(x, invL))));
+    return (w >= L || w < 0.f) ? 0.f : w;
+}
+__device__ __forceinline__ float min_image(float d, float L, float invL) {
+    return __fsub_rn(d, __fmul_rn(L, rintf(__fmul_rn(d, invL))));
+}
+__device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL) {
+    float dx = min_image(__fsub_rn(a.x, b.x), L, invL);
+    float dy = min_image(__fsub_rn(a.y, b.y), L, invL);
+    float dz = min_image(__fsub_rn(a.z, b.z), L, invL);
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
+__global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int nc, float cell_inv,
+                             float4 *posw, int *cell_of, int *cell_count) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float4 p = pos[i];
+    p.x = wrap_coord(p.x, L, invL); p.y = wrap_coord(p.y, L, invL); p.z = wrap_coord(p.z, L, invL); p.w = 0.f;
+    posw[i] = p;
+    int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
+    int cell = (cx * nc + cy) * nc + cz;
+    cell_of[i] = cell;
+    atomicAdd(&cell_count[cell], 1);
+}
+
+__global__ void scatter_to_cells(const int *cell_of, int N, const int *cell_start, int *cell_fill, int *order) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int cell = cell_of[i];
+    order[cell_start[cell] + atomicAdd(&cell_fill[cell], 1)] = i;
+}
+
+__global__ void sort_within_cells(const int *cell_start, int ncell, int *order) {   // deterministic order
+    int cell = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= ncell) return;
+    int lo = cell_start[cell], hi = cell_start[cell + 1];
+    for (int i = lo + 1; i < hi; ++i) {
+        int v = order[i], j = i - 1;
+        while (j >= lo && order[j] > v) { order[j + 1] = order[j]; --j; }
+        order[j + 1] = v;
+    }
+}
+
+__global__ void gather_positions(const float4 *posw, const int *order, int N, float4 *pos_sorted) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < N) pos_sorted[s] = posw[order[s]];
+}
+
+// One warp per (sorted) particle; FILL=false counts, FILL=true writes the list.
+template <bool FILL>
+__global__ void __launch_bounds__(256) neighbor_sweep(const float4 *__restrict__ pos, int N, const int *__restrict__ cell_start,
+                                                      int nc, float cell_inv, float L, float invL, float rc2,
+                                                      int *__restrict__ count, const unsigned long long *__restrict__ off,
+                                                      int *__restrict__ idx) {
+    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    float4 p = pos[s];
+    int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
+    int span = nc >= 3 ? 3 : nc;                   // fewer than 3 cells per side: visit each cell once
+    int found = 0;
+    unsigned long long base = FILL ? off[s] : 0ull;
+    for (int ix = 0; ix < span; ++ix) for (int iy = 0; iy < span; ++iy) {
+        int ccx = nc >= 3 ? (cx + ix - 1 + nc) % nc : ix, ccy = nc >= 3 ? (cy + iy - 1 + nc) % nc : iy;
+        for (int iz = 0; iz < span; ++iz) {
+            int ccz = nc >= 3 ? (cz + iz - 1 + nc) % nc : iz;
+            int cell = (ccx * nc + ccy) * nc + ccz;
+            int lo = cell_start[cell], hi = cell_start[cell + 1];
+            for (int j0 = lo; j0 < hi; j0 += 32) {
+                int j = j0 + lane;
+                bool in = false;
+                if (j < hi && j != s) in = dist2(p, pos[j], L, invL) < rc2;
+                unsigned m = __ballot_sync(0xffffffffu, in);
+                if (FILL && in) idx[base + found + __popc(m & ((1u << lane) - 1))] = j;
+                found += __popc(m);
+            }
+        }
+    }
+    if (!FILL && lane == 0) count[s] = found;
+}
+
+__global__ void counts_to_original(const int *count_sorted, const int *order, int N, int *count_orig) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < N) count_orig[order[s]] = count_sorted[s];
+}
+
+__global__ void lists_to_original(const int *idx, const unsigned long long *off_sorted, const int *order, int N,
+                                  const unsigned long long *off_orig, int *out) {
+    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    unsigned long long lo = off_sorted[s], n = off_sorted[s + 1] - lo, dst = off_orig[order[s]];
+    for (unsigned long long j = lane; j < n; j += 32) out[dst + j] = order[idx[lo + j]];
+}
+
+// Heyes-Melrose overlap force (reading R12), warp per particle over the neighbour list, packed output.
+__global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off,
+                          const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out) {
+    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    float4 p = pos[s];
+    float fx = 0, fy = 0, fz = 0;
+    for (unsigned long long j = off[s] + lane; j < off[s + 1]; j += 32) {
+        float4 q = pos[idx[j]];
+        float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
+        float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 < two_a * two_a && r2 > 0.f) {
+            float r = sqrtf(r2), g = coef * (two_a - r) / r;
+            fx += g * dx; fy += g * dy; fz += g * dz;
+        }
+    }
+    for (int o = 16; o; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (lane == 0) {
+        float4 *o4 = reinterpret_cast<float4 *>(out + (size_t)s * 8);
+        o4[0] = make_float4(fx, fy, fz, 0.f); o4[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+}  // namespace
+
+pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n) { return scan_impl(c, d_in, d_out, n); }
+pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n) { return scan_impl(c, d_in, d_out, n); }
+
+pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
+    ScopedPhase ph(c, PSE_T_NEIGHBORS);
+    const int N = c->N, T = 256, nb = (N + T - 1) / T, nbw = (int)(((size_t)N * 32 + T - 1) / T);
+    const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
+    const float rc = (float)c->rcut, rc2 = rc * rc;
+    c->have_nbrs = false;
+    CUDA_TRY(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
+    wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
+                                           c->d_posw, c->d_cell_of, c->d_cell_count); KERNEL_CHECK(c);
+    PSE_TRY(pse_scan_i32(c, c->d_cell_count, c->d_cell_start, (size_t)c->ncell));
+    scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order); KERNEL_CHECK(c);
+    sort_within_cells<<<(c->ncell + 127) / 128, 128, 0, c->stream>>>(c->d_cell_start, c->ncell, c->d_order); KERNEL_CHECK(c);
+    gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos); KERNEL_CHECK(c);
+    neighbor_sweep<false><<<nbw, T, 0, c->stream>>>(c->d_pos, N, c->d_cell_start, c->nc, cell_inv, L, invL, rc2,
+                                                    c->d_nbr_count, nullptr, nullptr); KERNEL_CHECK(c);
+    PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
+    unsigned long long total = 0;
+    CUDA_TRY(c, cudaMemcpyAsync(&total, c->d_nbr_off + N, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (total > 0x7fffffffull * 4ull) { c->err = "neighbour list too large"; return PSE_EOVERFLOW; }
+    if (total > c->nbr_cap) {
+        if (c->d_nbr_idx) cudaFree(c->d_nbr_idx);
+        c->d_nbr_idx = nullptr; c->nbr_cap = 0;
+        size_t cap = (size_t)(total * 1.25) + 1024;
+        if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
+        c->nbr_cap = cap;
+    }
+    c->nbr_total = (size_t)total;
+    neighbor_sweep<true><<<nbw, T, 0, c->stream>>>(c->d_pos, N, c->d_cell_start, c->nc, cell_inv, L, invL, rc2,
+                                                   nullptr, c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
+    PSE_TRY(pse_tile_bins(c));
+    c->have_nbrs = true;
+    return PSE_OK;
+}
+
+pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total) {
+    if (!c->have_nbrs) { c->err = "pse_get_neighbors before pse_neighbors"; return PSE_ENOTREADY; }
+    const int N = c->N, T = 256;
+    if (total) *total = c->nbr_total;
+    if (d_count) { counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, d_count); KERNEL_CHECK(c); }
+    if (!d_index) return PSE_OK;
+    if (cap < c->nbr_total) { c->err = "pse_get_neighbors: index buffer too small"; return PSE_EOVERFLOW; }
+    int *cnt = nullptr; unsigned long long *off = nullptr;
+    CUDA_TRY(c, cudaMalloc(&cnt, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&off, (size_t)(N + 1) * sizeof(unsigned long long)));
+    counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, cnt); KERNEL_CHECK(c);
+    PSE_TRY(pse_scan_u64(c, cnt, off, (size_t)N));
+    lists_to_original<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_nbr_idx, c->d_nbr_off, c->d_order, N, off, d_index);
+    KERNEL_CHECK(c);
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(cnt); cudaFree(off);
+    return PSE_OK;
+}
+
+pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {
+    ScopedPhase ph(c, PSE_T_REAL);
+    const int N = c->N, T = 256;
+    float coef = (float)(3.0 * M_PI * c->eta * c->a / dt);
+    hs_forces<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_idx, (float)c->L,
+                                                                            1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed);
+    KERNEL_CHECK(c);
+    return PSE_OK;
+}

@@ -1,0 +1,107 @@
+// Internal declarations of libpse (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+#include "pse.h"
+
+#define PSE_NTAB 2048          // nodes of the real-space table (8 floats each -> 64 KB, staged in shared memory)
+#define PSE_TILE 8             // spread / interpolate tile edge in grid points
+#define PSE_MAXP 16
+#define PSE_MAX_KRYLOV 50
+
+struct Timer { cudaEvent_t a, b; int phase; };
+
+struct pse_ctx {
+    // ---- parameters (pse_create) ----
+    int N = 0, M = 0, P = 0;
+    double L = 0, a = 0, eta = 0, kT = 0, xi = 0, rcut = 0, tol = 0;
+    double h = 0, eta_g = 0;                 // grid spacing, Gaussian shape parameter
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long launches = 0;
+    // ---- real-space table ----
+    float *d_table = nullptr;                // [PSE_NTAB][8]
+    double tab_dr = 0;
+    // ---- cell list / neighbour list (all in cell-sorted numbering unless noted) ----
+    int nc = 0, ncell = 0;                   // cells per dimension, total
+    bool have_nbrs = false;
+    float4 *d_pos = nullptr;                 // [N] wrapped positions, sorted
+    int *d_order = nullptr;                  // [N] sorted -> original
+    int *d_cell_of = nullptr;                // [N] cell of original particle
+    int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]
+    int *d_nbr_count = nullptr;              // [N]
+    unsigned long long *d_nbr_off = nullptr; // [N+1]
+    int *d_nbr_idx = nullptr; size_t nbr_cap = 0, nbr_total = 0;
+    // ---- FFT-grid tile bins ----
+    int nt = 0, ntile = 0, Mh = 0;           // tiles per dimension, total, M/2+1
+    int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]
+    int *d_tile_of = nullptr;                // [N] tile of (sorted) particle's support base
+    int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
+    // ---- grids ----
+    float *d_grid = nullptr;                 // [8][M][M][M]
+    cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
+    cufftHandle plan_r2c = 0, plan_c2r = 0; void *d_fft_work = nullptr; bool have_plans = false;
+    // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
+    float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
+    float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]
+    float *d_zu = nullptr;                               // [PSE_MAX_KRYLOV][N][8] full outputs M[0;v_j] (GMRES)
+    double *d_scal = nullptr;                // device scalars (dots, norms)
+    double *h_scal = nullptr;                // pinned mirror
+    float *d_coef = nullptr;                 // small coefficient vector upload
+    unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
+    float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
+    float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
+    // ---- profiling ----
+    bool profiling = false;
+    std::vector<Timer> timers;
+    float acc_ms[PSE_T_COUNT] = {0};
+    int acc_n[PSE_T_COUNT] = {0};
+};
+
+#define CUDA_TRY(ctx, expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
+    (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_); return PSE_ECUDA; } } while (0)
+#define CUFFT_TRY(ctx, expr) do { cufftResult r_ = (expr); if (r_ != CUFFT_SUCCESS) { \
+    (ctx)->err = std::string(#expr) + ": cufft error " + std::to_string((int)r_); return PSE_ECUFFT; } } while (0)
+#define PSE_TRY(expr) do { pse_status s_ = (expr); if (s_ != PSE_OK) return s_; } while (0)
+#define KERNEL_CHECK(ctx) do { (ctx)->launches++; CUDA_TRY(ctx, cudaGetLastError()); } while (0)
+
+struct ScopedPhase {
+    pse_ctx *c; int idx = -1;
+    ScopedPhase(pse_ctx *ctx, int phase) : c(ctx) {
+        if (!c->profiling) return;
+        Timer t; t.phase = phase;
+        cudaEventCreate(&t.a); cudaEventCreate(&t.b);
+        cudaEventRecord(t.a, c->stream);
+        c->timers.push_back(t); idx = (int)c->timers.size() - 1;
+    }
+    ~ScopedPhase() { if (idx >= 0) cudaEventRecord(c->timers[idx].b, c->stream); }
+};
+
+// tables.cu
+void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr);
+// neighbors.cu
+pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);
+pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n);   // exclusive, n+1 outputs
+pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n);
+pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total);
+pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
+// realspace.cu
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out);             // out = M_r in
+// wavespace.cu
+pse_status pse_wave_init(pse_ctx *c);
+void pse_wave_free(pse_ctx *c);
+pse_status pse_tile_bins(pse_ctx *c);
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate);   // out (+)= M_w in
+pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
+// krylov.cu
+pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted
+pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed);
+pse_status pse_unpack(pse_ctx *c, const float *d_packed, float scale, float *d_U, float *d_E);
+pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters);          // y = M_r^{1/2} w
+pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp,
+                                float *d_outp, int *iters);
+pse_status pse_axpby(pse_ctx *c, size_t n, float alpha, const float *x, float beta, float *y);

@@ -1,0 +1,100 @@
+// Real-space pair kernel (step a2): [U;E]_alpha = sum_beta M^(r)(x_alpha - x_beta) [F;S]_beta + self term
+// (Eqs. 25-27; self terms Eqs. A4/A12), over the neighbour list.
+//
+// Design: persistent CTAs (grid = 2 x #SM), the 64 KB table of (F1,F2,Ga,Gb | A,B,D,-) staged once per CTA in
+// shared memory, one warp per particle, lanes stride the CSR neighbour list, float4 gathers of the neighbour's
+// position and its two float4 of packed input, linear interpolation of the table in r, warp-shuffle reduction
+// of the 8 outputs.  The paper kept its tables in texture memory on a K40; shared memory gives
+// conflict-tolerant 16-byte reads with no L1 pressure on the gathers.
+//
+// Tensor algebra per pair (rh = unit separation, f = rh.F, t = S rh, q = rh.t):
+//   U += F1 (F - rh f) + F2 rh f + Ga t - Gb rh q
+//   E += A S + sym(rh (x) w),  w = -Ga F + 2B t + (Gb f + D q) rh     (projected on e1..e5; trace terms drop out)
+#include "pse_internal.h"
+
+namespace {
+
+constexpr float RS2 = 0.70710678118654752f;   // 1/sqrt2
+constexpr float RS6 = 0.40824829046386302f;   // 1/sqrt6
+
+__global__ void __launch_bounds__(512, 2)
+real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
+                  const unsigned long long *__restrict__ off, const int *__restrict__ idx,
+                  const float4 *__restrict__ table, float inv_dr, float L, float invL) {
+    extern __shared__ float4 tab[];               // [PSE_NTAB][2]
+    for (int i = threadIdx.x; i < PSE_NTAB * 2; i += blockDim.x) tab[i] = table[i];
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    for (int s = blockIdx.x * wpb + (threadIdx.x >> 5); s < N; s += gridDim.x * wpb) {
+        const float4 p = pos[s];
+        float u0 = 0, u1 = 0, u2 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
+        const unsigned long long lo = off[s], hi = off[s + 1];
+        for (unsigned long long j = lo + lane; j < hi; j += 32) {
+            const int b = idx[j];
+            const float4 q4 = pos[b], a0 = in[2 * b], a1 = in[2 * b + 1];
+            float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
+            dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float rinv = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * rinv;
+            const float rx = dx * rinv, ry = dy * rinv, rz = dz * rinv;
+            float tt = r * inv_dr;
+            int it = min((int)tt, PSE_NTAB - 2);
+            const float w1 = tt - (float)it, w0 = 1.f - w1;
+            const float4 ta = tab[2 * it], tb = tab[2 * it + 1], tc = tab[2 * it + 2], td = tab[2 * it + 3];
+            const float F1 = w0 * ta.x + w1 * tc.x, F2 = w0 * ta.y + w1 * tc.y, Ga = w0 * ta.z + w1 * tc.z, Gb = w0 * ta.w + w1 * tc.w;
+            const float A = w0 * tb.x + w1 * td.x, B = w0 * tb.y + w1 * td.y, D = w0 * tb.z + w1 * td.z;
+            // S_beta from its 5 coordinates
+            const float sxx = a0.w * RS2 - a1.x * RS6, syy = -a0.w * RS2 - a1.x * RS6, szz = 2.f * a1.x * RS6;
+            const float sxy = a1.y * RS2, sxz = a1.z * RS2, syz = a1.w * RS2;
+            const float f = rx * a0.x + ry * a0.y + rz * a0.z;
+            const float tx = sxx * rx + sxy * ry + sxz * rz, ty = sxy * rx + syy * ry + syz * rz, tz = sxz * rx + syz * ry + szz * rz;
+            const float q = rx * tx + ry * ty + rz * tz;
+            const float cu = (F2 - F1) * f - Gb * q;
+            u0 += F1 * a0.x + cu * rx + Ga * tx;
+            u1 += F1 * a0.y + cu * ry + Ga * ty;
+            u2 += F1 * a0.z + cu * rz + Ga * tz;
+            const float cw = Gb * f + D * q, B2 = 2.f * B;
+            const float wx = -Ga * a0.x + B2 * tx + cw * rx, wy = -Ga * a0.y + B2 * ty + cw * ry, wz = -Ga * a0.z + B2 * tz + cw * rz;
+            const float pxx = rx * wx, pyy = ry * wy, pzz = rz * wz;
+            e0 += A * a0.w + (pxx - pyy) * RS2;
+            e1 += A * a1.x + (2.f * pzz - pxx - pyy) * RS6;
+            e2 += A * a1.y + (rx * wy + ry * wx) * RS2;
+            e3 += A * a1.z + (rx * wz + rz * wx) * RS2;
+            e4 += A * a1.w + (ry * wz + rz * wy) * RS2;
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            u0 += __shfl_xor_sync(0xffffffffu, u0, o); u1 += __shfl_xor_sync(0xffffffffu, u1, o);
+            u2 += __shfl_xor_sync(0xffffffffu, u2, o); e0 += __shfl_xor_sync(0xffffffffu, e0, o);
+            e1 += __shfl_xor_sync(0xffffffffu, e1, o); e2 += __shfl_xor_sync(0xffffffffu, e2, o);
+            e3 += __shfl_xor_sync(0xffffffffu, e3, o); e4 += __shfl_xor_sync(0xffffffffu, e4, o);
+        }
+        if (lane == 0) {                                             // self term: r -> 0 limit, F1(0) F and A(0) S
+            const float4 a0 = in[2 * s], a1 = in[2 * s + 1], t0 = tab[0], t1 = tab[1];
+            out[2 * s] = make_float4(u0 + t0.x * a0.x, u1 + t0.x * a0.y, u2 + t0.x * a0.z, e0 + t1.x * a0.w);
+            out[2 * s + 1] = make_float4(e1 + t1.x * a1.x, e2 + t1.x * a1.y, e3 + t1.x * a1.z, e4 + t1.x * a1.w);
+        }
+    }
+}
+
+}  // namespace
+
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out) {
+    ScopedPhase ph(c, PSE_T_REAL);
+    static int nsm = 0;
+    if (!nsm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
+    const size_t smem = (size_t)PSE_NTAB * 2 * sizeof(float4);
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    int grid = 2 * nsm, wpb = 512 / 32;
+    if ((long long)grid * wpb > c->N) grid = (c->N + wpb - 1) / wpb;
+    real_pairs_kernel<<<grid, 512, smem, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in),
+                                                      reinterpret_cast<float4 *>(d_out), c->N, c->d_nbr_off, c->d_nbr_idx,
+                                                      reinterpret_cast<const float4 *>(c->d_table), (float)(1.0 / c->tab_dr),
+                                                      (float)c->L, 1.0f / (float)c->L);
+    KERNEL_CHECK(c);
+    return PSE_OK;
+}

@@ -1,0 +1,225 @@
+"""GPU parity: libpse (through its C ABI / ctypes binding) against the CPU fp64 oracle on the same seeded inputs.
+
+Tolerance (BASELINE.json north_star): neighbour lists bit-exact as sets; fp32 product and Brownian sample within
+relative L2 error max(2*tol, 1e-5) of the fp64 oracle, tol = configured Ewald tolerance.
+"""
+import numpy as np
+import pytest
+
+import synth
+from oracle import brownian as brn
+from oracle import functions as fn
+from oracle import mobility as mob
+from oracle import neighbors as nbo
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip('torch')
+
+A, ETA, KT = 1.0, 1.0 / (6.0 * np.pi), 1.0
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / np.linalg.norm(np.asarray(b, float)))
+
+
+def bar(tol):
+    return max(2 * tol, 1e-5)
+
+
+def dev(x, dtype=torch.float32):
+    return torch.as_tensor(np.ascontiguousarray(x), dtype=dtype).cuda().contiguous()
+
+
+def pos4(x):
+    p = np.zeros((x.shape[0], 4), np.float32)
+    p[:, :3] = x
+    return p
+
+
+def make_ctx(N, L, xi, grid, P, rcut, tol):
+    import paper_1709_06946_b200 as pse
+    return pse.pse_create(N, L, A, ETA, KT, xi, grid, P, rcut, tol)
+
+
+@pytest.fixture(scope='module')
+def config1():
+    """BASELINE.json configs[0]: N=64, phi=0.10, tol=1e-3, grid 32^3, P=8, xi=0.6 (R7)."""
+    import paper_1709_06946_b200 as pse
+    x, L = synth.rsa(64, 0.10, seed=1)
+    x32 = x.astype(np.float32)
+    xi, grid, P, tol = 0.6, 32, 8, 1e-3
+    st, _, _, rcut = pse.pse_suggest_params(64, L, A, tol, xi)
+    assert st == 0 and rcut <= L / 2
+    ctx = make_ctx(64, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    F, S = synth.gaussian_inputs(64, 0)
+    return dict(ctx=ctx, x=x32.astype(np.float64), x32=x32, L=L, xi=xi, grid=grid, P=P, tol=tol, rcut=rcut, F=F, S=S)
+
+
+def gpu_apply(ctx, F, S, which):
+    N = F.shape[0]
+    U, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_mobility_apply(dev(F), dev(S), U, E, which)
+    torch.cuda.synchronize()
+    return U.cpu().numpy(), E.cpu().numpy()
+
+
+def nbr_sets_from_gpu(ctx):
+    count, index = ctx.pse_get_neighbors()
+    count, index = count.cpu().numpy(), index.cpu().numpy()
+    off = np.concatenate([[0], np.cumsum(count)])
+    return [np.sort(index[off[i]:off[i + 1]]) for i in range(len(count))]
+
+
+def test_neighbors_bit_exact_config1(config1):
+    got = nbr_sets_from_gpu(config1['ctx'])
+    want = nbo.neighbor_sets(config1['x32'], config1['L'], config1['rcut'])
+    for g, w in zip(got, want):
+        assert np.array_equal(g, w)
+
+
+@pytest.mark.parametrize('N,phi,xi,seed,shift', [(500, 0.30, 0.9, 3, False), (777, 0.05, 0.5, 4, True), (30, 0.02, 0.35, 5, True)])
+def test_neighbors_bit_exact_other(N, phi, xi, seed, shift):
+    """Ragged sizes, dense and dilute, unwrapped inputs, and a box with fewer than 3 cells per side."""
+    import paper_1709_06946_b200 as pse
+    x, L = synth.rsa(N, phi, seed=seed)
+    if shift:
+        x = x + L * np.random.default_rng(seed).integers(-2, 3, size=x.shape)
+    x32 = x.astype(np.float32)
+    rcut = min(pse.pse_suggest_params(N, L, A, 1e-3, xi)[3], 0.5 * L)
+    ctx = make_ctx(N, L, xi, 32, 6, rcut, 1e-3)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    got, want = nbr_sets_from_gpu(ctx), nbo.neighbor_sets(x32, L, rcut)
+    assert sum(len(w) for w in want) > 0
+    for g, w in zip(got, want):
+        assert np.array_equal(g, w)
+
+
+def test_table_matches_oracle_functions(config1):
+    tab, dr = config1['ctx'].pse_get_table()
+    r = np.arange(tab.shape[0]) * dr
+    R = fn.real_space_functions(r, config1['xi'], A)
+    Aa, B, C, D = fn.rank4_combinations(R)
+    want = np.stack([R['F1'], R['F2'], R['G1'] + R['G2'], R['G1'] + 4 * R['G2'], Aa, B, D], 1) / (6 * np.pi * ETA * A)
+    assert np.abs(tab[:, :7] - want).max() < 2e-6
+    assert abs(r[-2] - config1['rcut']) < 1e-9
+
+
+def test_real_space_product(config1):
+    c = config1
+    U, E = gpu_apply(c['ctx'], c['F'], c['S'], 1)
+    # same truncated sum in fp64: isolates kernel arithmetic + table interpolation
+    Ut, Et = mob.real_apply(c['x'], c['L'], A, ETA, c['xi'], c['F'], c['S'], rcut=c['rcut'])
+    assert rel(np.hstack([U, E]), np.hstack([Ut, Et])) < 2e-5
+    # converged real-space sum: adds the truncation error, must stay inside the Ewald tolerance
+    Uc, Ec = mob.real_apply(c['x'], c['L'], A, ETA, c['xi'], c['F'], c['S'], eps=1e-12)
+    assert rel(np.hstack([U, E]), np.hstack([Uc, Ec])) < c['tol']
+
+
+def test_wave_space_product(config1):
+    c = config1
+    U, E = gpu_apply(c['ctx'], c['F'], c['S'], 2)
+    # direct sum over exactly the grid's modes: isolates the NUFFT quadrature (P, Gaussian) + fp32 error
+    k = brn.grid_modes(c['grid'], c['L'])
+    k2 = np.einsum('ki,ki->k', k, k)
+    w = fn.hasimoto_H(np.sqrt(k2), c['xi']) / (ETA * c['L']**3 * k2)
+    Ug, Eg = mob.wave_apply_modes(c['x'], c['L'], A, ETA, k, w, c['F'], c['S'])
+    assert rel(np.hstack([U, E]), np.hstack([Ug, Eg])) < c['tol']
+    Uc, Ec = mob.wave_apply(c['x'], c['L'], A, ETA, c['xi'], c['F'], c['S'], eps=1e-12)
+    assert rel(np.hstack([U, E]), np.hstack([Uc, Ec])) < c['tol']
+
+
+def test_full_product_config1(config1):
+    c = config1
+    U, E = gpu_apply(c['ctx'], c['F'], c['S'], 3)
+    Uo, Eo = mob.mobility_apply(c['x'], c['L'], A, ETA, c['xi'], c['F'], c['S'], eps=1e-12)
+    assert rel(U, Uo) < bar(c['tol']) and rel(E, Eo) < bar(c['tol'])
+    assert rel(np.hstack([U, E]), np.hstack([Uo, Eo])) < bar(c['tol'])
+
+
+def test_product_is_linear_and_symmetric(config1):
+    """x.(M y) = y.(M x) within fp32 + tolerance; M(ax+by) = aMx + bMy."""
+    c = config1
+    F2, S2 = synth.gaussian_inputs(64, 11)
+    U1, E1 = gpu_apply(c['ctx'], c['F'], c['S'], 3)
+    U2, E2 = gpu_apply(c['ctx'], F2, S2, 3)
+    d12 = float((c['F'] * U2).sum() + (c['S'] * E2).sum())
+    d21 = float((F2 * U1).sum() + (S2 * E1).sum())
+    assert abs(d12 - d21) < 1e-3 * max(abs(d12), abs(d21), 1.0)
+    U3, E3 = gpu_apply(c['ctx'], 2 * c['F'] - 3 * F2, 2 * c['S'] - 3 * S2, 3)
+    assert rel(U3, 2 * U1 - 3 * U2) < 1e-5 and rel(E3, 2 * E1 - 3 * E2) < 1e-5
+    assert float((c['F'] * U1).sum() + (c['S'] * E1).sum()) > 0
+
+
+def test_brownian_sample_config1(config1):
+    c = config1
+    w1, w2 = synth.brownian_noise(64, c['grid'], 0)
+    dt = 1e-3
+    UB, EB = torch.empty(64, 3, device='cuda'), torch.empty(64, 5, device='cuda')
+    it = c['ctx'].pse_brownian(dt, dev(w1.reshape(64, 8)), dev(w2), UB, EB)
+    torch.cuda.synchronize()
+    Uo, Eo = brn.brownian(c['x'], c['L'], A, ETA, KT, c['xi'], dt, c['grid'], w1, w2, eps=1e-12)
+    assert 2 <= it <= 30
+    assert rel(np.hstack([UB.cpu().numpy(), EB.cpu().numpy()]), np.hstack([Uo, Eo])) < bar(c['tol'])
+
+
+def test_brownian_wave_part_alone(config1):
+    """Zero real-space noise: the sample is sqrt(2kT/dt) A_w w2 exactly as the oracle's direct sum over grid modes."""
+    c = config1
+    _, w2 = synth.brownian_noise(64, c['grid'], 3)
+    UB, EB = torch.empty(64, 3, device='cuda'), torch.empty(64, 5, device='cuda')
+    c['ctx'].pse_brownian(0.5, torch.zeros(64, 8, device='cuda'), dev(w2), UB, EB)
+    Uw, Ew = brn.wave_sqrt_apply(c['x'], c['L'], A, ETA, c['xi'], c['grid'], w2)
+    amp = np.sqrt(2 * KT / 0.5)
+    assert rel(np.hstack([UB.cpu().numpy(), EB.cpu().numpy()]), amp * np.hstack([Uw, Ew])) < c['tol']
+
+
+def test_constrained_solve_and_hard_sphere_forces(config1):
+    c = config1
+    ctx, N = c['ctx'], 64
+    # overlapping configuration: shrink the box coordinates so that some pairs overlap
+    M = mob.dense(c['x'], c['L'], A, ETA, c['xi'], eps=1e-10)
+    rng = np.random.default_rng(7)
+    FP = rng.standard_normal((N, 3)).astype(np.float32)
+    UBh = rng.standard_normal((N, 3)).astype(np.float32)
+    EBh = rng.standard_normal((N, 5)).astype(np.float32)
+    U, S = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    it = ctx.pse_constrained_solve(dev(FP), dev(UBh), dev(EBh), U, S)
+    Uo, So = brn.constrained_solve(M, N, UBh.astype(float), EBh.astype(float), FP.astype(float))
+    assert 2 <= it <= 25
+    assert rel(S.cpu().numpy(), So) < 5 * c['tol'] and rel(U.cpu().numpy(), Uo) < bar(c['tol'])
+
+
+def test_hard_sphere_forces_match_oracle():
+    x, L = synth.rsa(200, 0.25, seed=9)
+    x = x * 0.93                      # compress: creates overlaps
+    L2 = L * 0.93
+    x32 = x.astype(np.float32)
+    ctx = make_ctx(200, L2, 0.6, 32, 6, min(6.0, L2 / 2), 1e-3)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    F = torch.empty(200, 3, device='cuda')
+    ctx.pse_hard_sphere_forces(1e-3, F)
+    Fo = brn.heyes_melrose(x32.astype(np.float64), L2, A, ETA, 1e-3)
+    assert np.abs(Fo).max() > 0
+    assert rel(F.cpu().numpy(), Fo) < 1e-4
+
+
+def test_step_small_against_dense_oracle():
+    """One mid-point step (Eqs. 76-79) on N=48 at phi=0.2, fp32 GPU vs dense fp64 oracle."""
+    import paper_1709_06946_b200 as pse
+    N, tol, xi, grid, P, dt = 48, 1e-4, 1.1, 32, 9, 1e-3
+    x, L = synth.rsa(N, 0.20, seed=6)
+    x32 = x.astype(np.float32)
+    st, _, _, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    w1, w2 = synth.brownian_noise(N, grid, 2)
+    pos = dev(pos4(x32))
+    gi, li = ctx.pse_step(pos, dt, dev(w1.reshape(N, 8)), dev(w2))
+    xn, Uo, So = brn.step(x32.astype(np.float64), L, A, ETA, KT, xi, dt, grid, w1, w2, eps=1e-10)
+    got = pos.cpu().numpy()[:, :3].astype(np.float64)
+    d = got - xn
+    d -= L * np.round(d / L)
+    disp = xn - x32.astype(np.float64)
+    assert 2 <= gi <= 30 and 2 <= li <= 40
+    assert np.linalg.norm(d) / np.linalg.norm(disp) < 5 * tol
