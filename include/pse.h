@@ -90,6 +90,15 @@ pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);
 pse_status pse_step(pse_ctx *ctx, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave,
                     int *gmres_iters, int *lanczos_iters);
 
+/* End-to-end variants with HOST buffers (pinned or pageable): the library copies inputs host->device, runs the
+ * device call of the same name, copies the results device->host and synchronises.  These are what bench.py's
+ * "e2e" number times.  h_pos [N][4] (in/out for pse_step_host), h_F [N][3], h_S [N][5], h_U [N][3], h_E [N][5],
+ * h_noise_real [N][8], h_noise_wave [3][grid][grid][grid/2+1][2]. */
+pse_status pse_mobility_apply_host(pse_ctx *ctx, const float *h_pos, const float *h_F, const float *h_S,
+                                   float *h_U, float *h_E);
+pse_status pse_step_host(pse_ctx *ctx, float *h_pos, double dt, const float *h_noise_real, const float *h_noise_wave,
+                         int *gmres_iters, int *lanczos_iters);
+
 /* Introspection for the parity tests and the harness. */
 /* Neighbour list in ORIGINAL particle numbering: d_count [N]; d_index holds the lists of particle 0,1,...
  * concatenated (offsets = exclusive scan of d_count); order within a list is unspecified.  *total (host) gets

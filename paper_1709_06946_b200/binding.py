@@ -18,7 +18,7 @@ _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PS
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
 EXPORTS = ('pse_suggest_params', 'pse_create', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
-           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_step', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
 
@@ -43,6 +43,8 @@ def load_library():
     lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
     lib.pse_step.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
+    lib.pse_mobility_apply_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.pse_step_host.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pse_get_neighbors.argtypes = [vp, vp, vp, C.c_size_t, C.POINTER(C.c_size_t)]
     lib.pse_set_profiling.argtypes = [vp, i32]
     lib.pse_get_timings.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32), i32]
@@ -64,6 +66,14 @@ def _ptr(t, shape=None):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
         raise TypeError('expected a contiguous CUDA tensor')
     if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f'expected shape {tuple(shape)}, got {tuple(t.shape)}')
+    return C.c_void_p(t.data_ptr())
+
+
+def _hptr(t, shape):
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+        raise TypeError('expected a contiguous float32 CPU tensor')
+    if tuple(t.shape) != tuple(shape):
         raise ValueError(f'expected shape {tuple(shape)}, got {tuple(t.shape)}')
     return C.c_void_p(t.data_ptr())
 
@@ -135,6 +145,19 @@ class Context:
         gi, li = C.c_int(), C.c_int()
         self._check(_lib.pse_step(self._h, _ptr(pos, (N, 4)), dt, _ptr(noise_real, (N, 8)),
                                   _ptr(noise_wave, (3, M, M, M // 2 + 1, 2)), C.byref(gi), C.byref(li)))
+        return gi.value, li.value
+
+    def pse_mobility_apply_host(self, pos, F, S, U, E):
+        """Host (CPU, ideally pinned) float32 tensors; copies are inside the call."""
+        N = self.N
+        self._check(_lib.pse_mobility_apply_host(self._h, _hptr(pos, (N, 4)), _hptr(F, (N, 3)), _hptr(S, (N, 5)),
+                                                 _hptr(U, (N, 3)), _hptr(E, (N, 5))))
+
+    def pse_step_host(self, pos, dt, noise_real, noise_wave):
+        N, M = self.N, self.grid
+        gi, li = C.c_int(), C.c_int()
+        self._check(_lib.pse_step_host(self._h, _hptr(pos, (N, 4)), dt, _hptr(noise_real, (N, 8)),
+                                       _hptr(noise_wave, (3, M, M, M // 2 + 1, 2)), C.byref(gi), C.byref(li)))
         return gi.value, li.value
 
     def pse_get_neighbors(self):

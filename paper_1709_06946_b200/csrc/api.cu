@@ -112,6 +112,7 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
     cudaFree(c->d_scal); cudaFree(c->d_scan_tmp);
+    cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
     return PSE_OK;
@@ -188,6 +189,45 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
                                         reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
     return soft;
+}
+
+static pse_status ensure_stage(pse_ctx *c, bool noise) {
+    const size_t N = (size_t)c->N;
+    if (!c->d_stage_pos) CUDA_TRY(c, cudaMalloc(&c->d_stage_pos, N * 4 * sizeof(float)));
+    if (!c->d_stage_a) CUDA_TRY(c, cudaMalloc(&c->d_stage_a, N * 8 * sizeof(float)));
+    if (!c->d_stage_b) CUDA_TRY(c, cudaMalloc(&c->d_stage_b, N * 8 * sizeof(float)));
+    if (noise && !c->d_stage_noise) CUDA_TRY(c, cudaMalloc(&c->d_stage_noise, (size_t)6 * c->M * c->M * c->Mh * sizeof(float)));
+    return PSE_OK;
+}
+
+pse_status pse_mobility_apply_host(pse_ctx *c, const float *h_pos, const float *h_F, const float *h_S, float *h_U, float *h_E) {
+    if (!c || !h_pos || !h_F || !h_S || !h_U || !h_E) return PSE_EINVAL;
+    PSE_TRY(ensure_stage(c, false));
+    const size_t N = (size_t)c->N;
+    float *dF = c->d_stage_a, *dS = c->d_stage_a + 3 * N, *dU = c->d_stage_b, *dE = c->d_stage_b + 3 * N;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_pos, h_pos, N * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(dF, h_F, N * 3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(dS, h_S, N * 5 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    PSE_TRY(pse_neighbors_impl(c, c->d_stage_pos));
+    PSE_TRY(pse_mobility_apply(c, dF, dS, dU, dE, PSE_BOTH));
+    CUDA_TRY(c, cudaMemcpyAsync(h_U, dU, N * 3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(h_E, dE, N * 5 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PSE_OK;
+}
+
+pse_status pse_step_host(pse_ctx *c, float *h_pos, double dt, const float *h_noise_real, const float *h_noise_wave, int *gmres_iters, int *lanczos_iters) {
+    if (!c || !h_pos || !h_noise_real || !h_noise_wave) return PSE_EINVAL;
+    PSE_TRY(ensure_stage(c, true));
+    const size_t N = (size_t)c->N, nw = (size_t)6 * c->M * c->M * c->Mh;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_pos, h_pos, N * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_a, h_noise_real, N * 8 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_noise, h_noise_wave, nw * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    pse_status st = pse_step(c, c->d_stage_pos, dt, c->d_stage_a, c->d_stage_noise, gmres_iters, lanczos_iters);
+    if (st != PSE_OK && st != PSE_ENOCONV) return st;
+    CUDA_TRY(c, cudaMemcpyAsync(h_pos, c->d_stage_pos, N * 4 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return st;
 }
 
 pse_status pse_set_profiling(pse_ctx *c, int on) { if (!c) return PSE_EINVAL; c->profiling = on != 0; return PSE_OK; }

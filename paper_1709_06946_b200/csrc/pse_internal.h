@@ -55,6 +55,8 @@ struct pse_ctx {
     unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
     float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
     float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
+    // ---- staging for the host-buffer entry points ----
+    float *d_stage_pos = nullptr, *d_stage_a = nullptr, *d_stage_b = nullptr, *d_stage_noise = nullptr;
     // ---- profiling ----
     bool profiling = false;
     std::vector<Timer> timers;
