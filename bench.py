@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py — constrained Brownian-dynamics steps/s (and grand-mobility products/s) of libpse on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config3|config4|config2|tiny] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path: pse_step = neighbour build, Brownian sample
+(Lanczos + wave-space square root), mid-point move, neighbour build, hard-sphere forces, GMRES stresslet solve
+(~10 full products), final move.  Inputs are seeded synthetic hard-sphere suspensions (synth/, recipe in DESIGN.md).
+Prints ONE JSON line on rank 0.  Multi-GPU (torchrun): independent replicas, no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+A, ETA, KT = 1.0, 1.0 / (6.0 * np.pi), 1.0
+
+WORKLOADS = {
+    # name: N, phi, tol, xi, dt, relax sweeps          (BASELINE.json configs; xi is the free tuning knob)
+    'tiny': dict(N=4096, phi=0.20, tol=1e-3, xi=0.5, dt=1e-3, relax=0),
+    'config2': dict(N=4096, phi=0.20, tol=1e-4, xi=0.5, dt=1e-3, relax=0),
+    'config3': dict(N=65536, phi=0.30, tol=1e-3, xi=0.5, dt=1e-4, relax=2),
+    'config4': dict(N=1048576, phi=0.10, tol=1e-3, xi=0.5, dt=1e-4, relax=0),
+}
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, 'MEASURED_PEAKS.json')) as f:
+            return float(json.load(f)['hbm_gbs']), 'measured (MEASURED_PEAKS.json hbm_gbs)'
+    except Exception:
+        return 6650.0, 'fallback (B200_PROFILING.md)'
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ('clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,'
+         'clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap')
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(['nvidia-smi', f'--id={self.index}', f'--query-gpu={self.Q}', '--format=csv,noheader,nounits',
+                                          '-lms', '100'], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(',')])
+
+    def stop(self):
+        if not self.proc:
+            return {'sm_mhz': None, 'sm_max_mhz': None, 'reasons': ['nvidia-smi unavailable']}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace('.', '').isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace('.', '').isdigit()]
+        names = ['hw_slowdown', 'hw_thermal_slowdown', 'sw_thermal_slowdown', 'sw_power_cap']
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith('active') for r in self.rows)]
+        return {'sm_mhz': float(np.median(sm)) if sm else None, 'sm_max_mhz': max(mx) if mx else None, 'reasons': reasons,
+                'samples': len(sm)}
+
+
+def make_suspension(wl, seed):
+    import synth
+    x, L = synth.rsa(wl['N'], wl['phi'], seed=seed)
+    if wl['relax']:
+        x = synth.relax_overlaps(x, L, sweeps=wl['relax'], seed=seed)
+    return x, L
+
+
+def choose_params(wl, L):
+    import paper_1709_06946_b200 as pse
+    st, grid, P, rcut = pse.pse_suggest_params(wl['N'], L, A, wl['tol'], wl['xi'])
+    if st != 0:
+        raise RuntimeError(f'no valid PSE parameters for {wl}')
+    return grid, P, rcut
+
+
+def algorithmic_bytes(N, M, nb_mean):
+    """Per-launch algorithmic bytes of each phase: fp32, G = M^3 grid points."""
+    G, Gh = float(M) ** 3, float(M) * M * (M // 2 + 1)
+    return {
+        'neighbors': 16 * N + 8 * N + 2 * 4 * N * nb_mean,      # positions, sort keys/permutation, list written (count + fill pass reads excluded)
+        'real': 16 * N + 32 * N + 32 * N + 4 * N * nb_mean,     # compulsory DRAM: pos, in, out, neighbour indices
+        'spread': 48 * N + 32 * G,                              # particles read, 8 grids written once
+        'fft_fwd': 32 * G + 64 * Gh,                            # one-pass lower bound: 8 real grids in, 8 half spectra out
+        'scale': 2 * 64 * Gh,                                   # 8 complex in, 8 complex out per half-spectrum mode
+        'fft_inv': 64 * Gh + 32 * G,
+        'interp': 32 * G + 48 * N,                              # 8 grids read once, particles read/written
+    }
+
+
+def run_ours(args, wl, rank, world):
+    import torch
+    import paper_1709_06946_b200 as pse
+    dev = torch.device('cuda', int(os.environ.get('LOCAL_RANK', 0)))
+    torch.cuda.set_device(dev)
+    N, dt = wl['N'], wl['dt']
+    x, L = make_suspension(wl, seed=100 + rank)
+    grid, P, rcut = choose_params(wl, L)
+    ctx = pse.pse_create(N, L, A, ETA, KT, wl['xi'], grid, P, rcut, wl['tol'])
+    pos = torch.zeros(N, 4, device=dev)
+    pos[:, :3] = torch.from_numpy(x.astype(np.float32)).to(dev)
+    gen = torch.Generator(device=dev); gen.manual_seed(1234 + rank)
+    K, W = args.steps, args.warmup
+    nshape = (3, grid, grid, grid // 2 + 1, 2)
+
+    def noise():
+        return (torch.randn(N, 8, device=dev, generator=gen), torch.randn(nshape, device=dev, generator=gen))
+
+    flush = torch.empty(256 * 1024 * 1024 // 4, device=dev)
+    iters = []
+
+    def timed_steps(n, profiled=False):
+        """n steps, each bracketed by its own CUDA events on the library's stream, L2 flushed in between."""
+        total = 0.0
+        for _ in range(n):
+            nr, nw = noise()
+            flush.fill_(1.0)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            gi, li = ctx.pse_step(pos, dt, nr, nw)
+            e1.record()
+            torch.cuda.synchronize()
+            total += e0.elapsed_time(e1)
+            iters.append((gi, li))
+        return total
+
+    timed_steps(W)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    l0 = ctx.pse_kernel_launches()
+    iters.clear()
+    ms = timed_steps(K)
+    launches = ctx.pse_kernel_launches() - l0
+    clocks = sampler.stop()
+    torch.cuda.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    gm = float(np.mean([i[0] for i in iters])); lz = float(np.mean([i[1] for i in iters]))
+    out = dict(ms=ms, launches=launches, clocks=clocks, gmres=gm, lanczos=lz, grid=grid, P=P, rcut=rcut, L=L)
+    if rank != 0:
+        return out
+    # ---- per-phase times (profiled pass, same steps, CUDA events inside the library) ----
+    ctx.pse_set_profiling(True)
+    ctx.pse_get_timings()
+    kp = max(1, min(K, 5))
+    timed_steps(kp)
+    phases = ctx.pse_get_timings()
+    ctx.pse_set_profiling(False)
+    ctx.pse_neighbors(pos)
+    count, _ = ctx.pse_get_neighbors()
+    nb_mean = float(count.float().mean().item())
+    out.update(phases=phases, nb_mean=nb_mean, profiled_steps=kp)
+    # ---- product throughput (device resident) ----
+    F, S = torch.randn(N, 3, device=dev, generator=gen), torch.randn(N, 5, device=dev, generator=gen)
+    U, E = torch.empty(N, 3, device=dev), torch.empty(N, 5, device=dev)
+    for _ in range(3):
+        ctx.pse_mobility_apply(F, S, U, E)
+    mv = 0.0
+    nmv = 20
+    for _ in range(nmv):
+        flush.fill_(1.0)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); ctx.pse_mobility_apply(F, S, U, E); e1.record()
+        torch.cuda.synchronize()
+        mv += e0.elapsed_time(e1)
+    out['matvec_ms'] = mv / nmv
+    # ---- end to end through the C ABI with host buffers ----
+    hpos = pos.cpu().pin_memory()
+    hnr = torch.randn(N, 8).pin_memory(); hnw = torch.randn(nshape).pin_memory()
+    ke = max(1, min(K, 10))
+    for _ in range(2):
+        ctx.pse_step_host(hpos, dt, hnr, hnw)
+    e2e = 0.0
+    for _ in range(ke):
+        hnr.normal_(); hnw.normal_()
+        flush.fill_(1.0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.pse_step_host(hpos, dt, hnr, hnw)          # synchronises internally after the D2H copy
+        e2e += (time.perf_counter() - t0) * 1e3
+    out.update(e2e_ms=e2e / ke, h2d=int(hpos.numel() * 4 + hnr.numel() * 4 + hnw.numel() * 4), d2h=int(hpos.numel() * 4), e2e_steps=ke)
+    return out
+
+
+def oracle_sample(wl, nsteps):
+    """The CPU oracle, as it stands, on a bounded sample of the workload: one dense mid-point step (Eqs. 76-79) of
+    N_s spheres at the workload's volume fraction and tolerance.  Returns (seconds per oracle step, N_s, cores, text)."""
+    import synth
+    from oracle import brownian as brn
+    Ns = 96
+    x, L = synth.rsa(Ns, wl['phi'], seed=7)
+    s = np.sqrt(-np.log(wl['tol']))
+    xi = max(wl['xi'], 1.02 * s / (0.5 * L - 2 * A))                 # keep rcut = s/xi + 2a <= L/2 in the small box
+    Mg = 16
+    while Mg < 2 * xi * s * L / np.pi:
+        Mg += 2
+    eps = min(1e-10, wl['tol'] * 1e-4)
+    times = []
+    for k in range(nsteps):
+        w1, w2 = synth.brownian_noise(Ns, Mg, seed=k)
+        t0 = time.perf_counter()
+        xn, _, _ = brn.step(x, L, A, ETA, KT, xi, wl['dt'], Mg, w1, w2, eps=eps)
+        times.append(time.perf_counter() - t0)
+        x = xn % L
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get('num_threads', 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = 1
+    text = (f'oracle.brownian.step (dense fp64 direct Ewald, eps={eps:g}) on N_s={Ns} spheres at phi={wl["phi"]}, xi={xi:.3f}, '
+            f'{nsteps} step(s); steps/s scaled to the workload by N_s/N (linear, generous: the oracle is O(N^2) and worse)')
+    return float(np.mean(times)), Ns, cores, text
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument('--gpus', type=int, default=1)
+    ap.add_argument('--steps', type=int, default=20)
+    ap.add_argument('--warmup', type=int, default=3)
+    ap.add_argument('--workload', default='config3', choices=sorted(WORKLOADS))
+    ap.add_argument('--impl', default='ours', choices=['ours', 'reference'])
+    ap.add_argument('--no-cpu-baseline', action='store_true')
+    args = ap.parse_args()
+    wl = dict(WORKLOADS[args.workload])
+    rank, world = int(os.environ.get('RANK', 0)), int(os.environ.get('WORLD_SIZE', 1))
+    config = {'workload': f'{args.workload}: N={wl["N"]} hard spheres, phi={wl["phi"]}, Ewald tol={wl["tol"]}, xi={wl["xi"]}, '
+                          f'dt={wl["dt"]}, kT=1, RSA placement' + (f' + {wl["relax"]} relax sweeps' if wl['relax'] else ''),
+              'N': wl['N'], 'phi': wl['phi'], 'tol': wl['tol'], 'xi': wl['xi']}
+    base = {'metric': 'constrained_bd_steps_per_sec', 'unit': 'steps/s', 'n_gpus': args.gpus, 'steps': args.steps, 'warmup': args.warmup,
+            'higher_is_better': True, 'scaling': 'weak', 'vs_baseline': None, 'dtype': 'f32', 'data': 'synthetic'}
+
+    if args.impl == 'reference':
+        if rank != 0:
+            return
+        for _ in range(min(args.warmup, 1)):
+            oracle_sample(wl, 1)
+        sec, Ns, cores, text = oracle_sample(wl, max(1, min(args.steps, 3)))
+        val = (1.0 / sec) * Ns / wl['N']
+        line = dict(base, impl='reference', value=val, ms_per_step=1e3 / val, config=config,
+                    cpu_baseline={'value': val, 'unit': 'steps/s', 'cores': cores, 'kind': 'oracle', 'sample': text},
+                    e2e={'value': val, 'unit': 'steps/s', 'h2d_bytes_per_step': 0, 'd2h_bytes_per_step': 0})
+        line['dtype'] = 'f64'
+        print(json.dumps(line))
+        return
+
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(int(os.environ.get('LOCAL_RANK', 0)))
+        dist.init_process_group('nccl')
+    r = run_ours(args, wl, rank, world)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    K = args.steps
+    ms_step = r['ms'] / K
+    value = world * 1e3 / ms_step                                     # replicas: all ranks' steps / max-over-ranks time
+    peak, peak_src = peaks()
+    ab = algorithmic_bytes(wl['N'], r['grid'], r['nb_mean'])
+    phases = {}
+    for name, (ms, n) in r['phases'].items():
+        if n == 0:
+            continue
+        avg = ms / n
+        e = {'ms_per_step': ms / r['profiled_steps'], 'launches_per_step': n / r['profiled_steps'], 'avg_ms': avg}
+        if name in ab:
+            e['alg_GBps'] = ab[name] / (avg * 1e-3) / 1e9
+            e['frac_of_hbm_peak'] = e['alg_GBps'] / peak
+        phases[name] = e
+    dom = max((p for p in phases if p in ab), key=lambda p: phases[p]['ms_per_step'])
+    fft_share = (phases.get('fft_fwd', {}).get('ms_per_step', 0) + phases.get('fft_inv', {}).get('ms_per_step', 0)) / \
+        max(sum(p['ms_per_step'] for p in phases.values()), 1e-9)
+    line = dict(base, value=value, ms_per_step=ms_step, config=dict(
+        config, grid=r['grid'], P=r['P'], rcut=round(r['rcut'], 4), L=round(r['L'], 4), mean_neighbors=round(r['nb_mean'], 2),
+        gmres_iters=r['gmres'], lanczos_iters=r['lanczos'], parallelism=f'replicas x{world}' if world > 1 else 'single GPU',
+        l2='flushed (256 MiB write) between timed steps; each step bracketed by its own CUDA events'))
+    line['matvecs_per_sec'] = 1e3 / r['matvec_ms']
+    line['ptps'] = value * wl['N']
+    line['clocks'] = r['clocks']
+    line['gpu_launches'] = int(r['launches'])
+    line['e2e'] = {'value': 1e3 / r['e2e_ms'], 'unit': 'steps/s', 'h2d_bytes_per_step': r['h2d'], 'd2h_bytes_per_step': r['d2h'],
+                   'api': 'pse_step_host (pinned host buffers, copies inside the timed call)', 'steps': r['e2e_steps']}
+    line['roofline'] = {'bound': 'hbm', 'kernel': dom, 'achieved': phases[dom]['alg_GBps'], 'peak': peak, 'unit': 'GB/s',
+                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': None, 'peak_source': peak_src,
+                        'note': 'algorithmic bytes per launch / mean launch duration from CUDA events inside the library over '
+                                f'{r["profiled_steps"]} profiled steps; at this size the grids are L2-resident (see DESIGN.md §5)'}
+    line['phases'] = phases
+    line['cufft_share_of_step'] = fft_share
+    if not args.no_cpu_baseline:
+        sec, Ns, cores, text = oracle_sample(wl, 1)
+        line['cpu_baseline'] = {'value': (1.0 / sec) * Ns / wl['N'], 'unit': 'steps/s', 'cores': cores, 'kind': 'oracle', 'sample': text,
+                                'seconds_per_sample_step': sec}
+    print(json.dumps(line))
+
+
+if __name__ == '__main__':
+    main()
