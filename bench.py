@@ -75,6 +75,22 @@ class ClockSampler:
                 'samples': len(sm)}
 
 
+def max_over_ranks(ms, device=None):
+    """Replica aggregation: the job's time is the slowest rank's; no data-path collective."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device if device is not None else 'cpu')
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(steps, world, ms_max):
+    """Whole-job steps/s of `world` independent replicas that each ran `steps` steps in at most ms_max ms."""
+    return world * steps * 1e3 / ms_max
+
+
 def make_suspension(wl, seed):
     import synth
     x, L = synth.rsa(wl['N'], wl['phi'], seed=seed)
@@ -158,9 +174,7 @@ def run_ours(args, wl, rank, world):
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+        ms = max_over_ranks(ms, dev)
     gm = float(np.mean([i[0] for i in iters])); lz = float(np.mean([i[1] for i in iters]))
     out = dict(ms=ms, launches=launches, clocks=clocks, gmres=gm, lanczos=lz, grid=grid, P=P, rcut=rcut, L=L)
     if rank != 0:
@@ -284,7 +298,7 @@ def main():
         return
     K = args.steps
     ms_step = r['ms'] / K
-    value = world * 1e3 / ms_step                                     # replicas: all ranks' steps / max-over-ranks time
+    value = replica_throughput(K, world, r['ms'])                     # replicas: all ranks' steps / max-over-ranks time
     peak, peak_src = peaks()
     ab = algorithmic_bytes(wl['N'], r['grid'], r['nb_mean'])
     phases = {}

@@ -38,14 +38,19 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
     if (N <= 0 || !(L > 0) || !(a > 0) || !(tol > 0 && tol < 1) || !(xi > 0)) return PSE_EINVAL;
     const double s = std::sqrt(-std::log(tol));
     // C1: functions decay like exp(-xi^2 (r-2a)^2), so the paper's estimate r = s/xi
-    // is shifted by the sphere diameter.
-    double rc = s / xi + 2.0 * a;
-    // C2: wave cutoff k_cut = 2 xi s (H(k) ~ exp(-k^2/4 xi^2)); M >= k_cut L / pi, rounded up to a 2,3,5,7-smooth size
-    int M = std::max(8, (int)std::ceil(2.0 * xi * s * L / M_PI));
+    // is optimistic; the shift of one radius is calibrated against the oracle (R6: truncation error
+    // 0.4-0.7 tol for xi in [0.5,0.7], phi in [0.1,0.3], tol in [1e-2,1e-4]).
+    double rc = s / xi + 1.0 * a;
+    // C2: wave cutoff k_cut = 2 xi s (H(k) ~ exp(-k^2/4 xi^2)); M >= 1.07 k_cut L / pi (the strain-rate rows carry an
+    // extra factor k, so the bare estimate leaves their truncation error at ~tol), rounded up to a 2,3,5,7-smooth size
+    int M = std::max(8, (int)std::ceil(1.07 * 2.0 * xi * s * L / M_PI));
     while (!smooth7(M)) ++M;
-    // C3: quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1)
+    // C3: quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1) gives P = 5 at 1e-3 as in
+    // Table I; measured against the oracle that P leaves 2-3 tol in the relative L2 norm of [U;E], so
+    // one more point per dimension is taken (R6).
     int p = 2;
     while (p < PSE_MAXP && std::exp(-M_PI * p / 2.0) + std::erfc(std::sqrt(M_PI * p / 2.0)) > tol) ++p;
+    p = std::min(PSE_MAXP, p + 1);
     if (grid) *grid = M;
     if (P) *P = p;
     if (rcut) *rcut = rc;
@@ -85,6 +90,8 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaMalloc(&c->d_pos, (size_t)N * sizeof(float4)));
     CUDA_TRY(c, cudaMalloc(&c->d_posw, (size_t)N * sizeof(float4)));
     CUDA_TRY(c, cudaMalloc(&c->d_order, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_order_tmp, (size_t)N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_tile_tmp, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_cell_of, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_cell_count, (size_t)(c->ncell + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_cell_start, (size_t)(c->ncell + 1) * sizeof(int)));
@@ -107,7 +114,7 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaStreamSynchronize(c->stream);
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
-    cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_cell_of);
+    cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
     cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_fill); cudaFree(c->d_nbr_count);
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);

@@ -121,14 +121,18 @@ __global__ void scatter_to_cells(const int *cell_of, int N, const int *cell_star
     order[cell_start[cell] + atomicAdd(&cell_fill[cell], 1)] = i;
 }
 
-__global__ void sort_within_cells(const int *cell_start, int ncell, int *order) {   // deterministic order
-    int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= ncell) return;
-    int lo = cell_start[cell], hi = cell_start[cell + 1];
-    for (int i = lo + 1; i < hi; ++i) {
-        int v = order[i], j = i - 1;
-        while (j >= lo && order[j] > v) { order[j + 1] = order[j]; --j; }
-        order[j + 1] = v;
+// Deterministic order inside every segment (cell or tile): warp per segment, rank sort out of place.
+// rank_i = #{j : v_j < v_i} (values are distinct particle indices), n^2/32 comparisons per warp.
+__global__ void rank_sort_segments(const int *__restrict__ seg_start, int nseg, const int *__restrict__ in, int *__restrict__ out) {
+    int seg = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (seg >= nseg) return;
+    const int lo = seg_start[seg], n = seg_start[seg + 1] - lo;
+    for (int i0 = 0; i0 < n; i0 += 32) {
+        const int i = i0 + lane;
+        const int v = i < n ? in[lo + i] : 0x7fffffff;
+        int rank = 0;
+        for (int j = 0; j < n; ++j) rank += (in[lo + j] < v);
+        if (i < n) out[lo + rank] = v;
     }
 }
 
@@ -147,20 +151,26 @@ __global__ void __launch_bounds__(256) neighbor_sweep(const float4 *__restrict__
     if (s >= N) return;
     float4 p = pos[s];
     int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
-    int span = nc >= 3 ? 3 : nc;                   // fewer than 3 cells per side: visit each cell once
+    const int span = nc >= 3 ? 3 : nc;             // fewer than 3 cells per side: visit each cell once
     int found = 0;
-    unsigned long long base = FILL ? off[s] : 0ull;
+    const unsigned long long base = FILL ? off[s] : 0ull;
     for (int ix = 0; ix < span; ++ix) for (int iy = 0; iy < span; ++iy) {
-        int ccx = nc >= 3 ? (cx + ix - 1 + nc) % nc : ix, ccy = nc >= 3 ? (cy + iy - 1 + nc) % nc : iy;
-        for (int iz = 0; iz < span; ++iz) {
-            int ccz = nc >= 3 ? (cz + iz - 1 + nc) % nc : iz;
-            int cell = (ccx * nc + ccy) * nc + ccz;
-            int lo = cell_start[cell], hi = cell_start[cell + 1];
+        int ccx = ix, ccy = iy;
+        if (nc >= 3) { ccx = cx + ix - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + iy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
+        const int col = (ccx * nc + ccy) * nc;
+        // cells cz-1..cz+1 of one (x,y) column are contiguous in the sorted order: one run, or two when z wraps
+        int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
+        int seg_lo[2], seg_hi[2], nseg = 1;
+        if (z0 < 0) { seg_lo[0] = cell_start[col]; seg_hi[0] = cell_start[col + z1 + 1]; seg_lo[1] = cell_start[col + nc - 1]; seg_hi[1] = cell_start[col + nc]; nseg = 2; }
+        else if (z1 >= nc) { seg_lo[0] = cell_start[col]; seg_hi[0] = cell_start[col + 1]; seg_lo[1] = cell_start[col + z0]; seg_hi[1] = cell_start[col + nc]; nseg = 2; }
+        else { seg_lo[0] = cell_start[col + z0]; seg_hi[0] = cell_start[col + z1 + 1]; }
+        for (int sg = 0; sg < nseg; ++sg) {
+            const int lo = seg_lo[sg], hi = seg_hi[sg];
             for (int j0 = lo; j0 < hi; j0 += 32) {
-                int j = j0 + lane;
+                const int j = j0 + lane;
                 bool in = false;
                 if (j < hi && j != s) in = dist2(p, pos[j], L, invL) < rc2;
-                unsigned m = __ballot_sync(0xffffffffu, in);
+                const unsigned m = __ballot_sync(0xffffffffu, in);
                 if (FILL && in) idx[base + found + __popc(m & ((1u << lane) - 1))] = j;
                 found += __popc(m);
             }
@@ -209,6 +219,11 @@ __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned 
 
 }  // namespace
 
+pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *in, int *out) {
+    rank_sort_segments<<<(unsigned)(((size_t)nseg * 32 + 255) / 256), 256, 0, c->stream>>>(seg_start, nseg, in, out); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
 pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n) { return scan_impl(c, d_in, d_out, n); }
 pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n) { return scan_impl(c, d_in, d_out, n); }
 
@@ -223,8 +238,8 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
                                            c->d_posw, c->d_cell_of, c->d_cell_count); KERNEL_CHECK(c);
     PSE_TRY(pse_scan_i32(c, c->d_cell_count, c->d_cell_start, (size_t)c->ncell));
-    scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order); KERNEL_CHECK(c);
-    sort_within_cells<<<(c->ncell + 127) / 128, 128, 0, c->stream>>>(c->d_cell_start, c->ncell, c->d_order); KERNEL_CHECK(c);
+    scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order_tmp); KERNEL_CHECK(c);
+    pse_rank_sort(c, c->d_cell_start, c->ncell, c->d_order_tmp, c->d_order);
     gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos); KERNEL_CHECK(c);
     neighbor_sweep<false><<<nbw, T, 0, c->stream>>>(c->d_pos, N, c->d_cell_start, c->nc, cell_inv, L, invL, rc2,
                                                     c->d_nbr_count, nullptr, nullptr); KERNEL_CHECK(c);

@@ -31,6 +31,7 @@ struct pse_ctx {
     bool have_nbrs = false;
     float4 *d_pos = nullptr;                 // [N] wrapped positions, sorted
     int *d_order = nullptr;                  // [N] sorted -> original
+    int *d_order_tmp = nullptr, *d_tile_tmp = nullptr;   // [N] unsorted scatter targets
     int *d_cell_of = nullptr;                // [N] cell of original particle
     int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]
     int *d_nbr_count = nullptr;              // [N]
@@ -83,12 +84,32 @@ struct ScopedPhase {
     ~ScopedPhase() { if (idx >= 0) cudaEventRecord(c->timers[idx].b, c->stream); }
 };
 
+#ifdef __CUDACC__
+// Warp reduction of 8 per-lane partial sums with 9 shuffles instead of 40: each step halves the number of values a
+// lane carries.  On return the lanes with (lane & 3) == 0 hold the full sum of component
+// comp = 4*bit4(lane) + 2*bit3(lane) + bit2(lane).
+__device__ __forceinline__ float warp_reduce8(const float (&a)[8], int lane, int &comp) {
+    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+    float r4[4], r2[2];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) r4[c] = (h16 ? a[c + 4] : a[c]) + __shfl_xor_sync(0xffffffffu, h16 ? a[c] : a[c + 4], 16);
+#pragma unroll
+    for (int c = 0; c < 2; ++c) r2[c] = (h8 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h8 ? r4[c] : r4[c + 2], 8);
+    float r = (h4 ? r2[1] : r2[0]) + __shfl_xor_sync(0xffffffffu, h4 ? r2[0] : r2[1], 4);
+    r += __shfl_xor_sync(0xffffffffu, r, 2);
+    r += __shfl_xor_sync(0xffffffffu, r, 1);
+    comp = (h16 ? 4 : 0) + (h8 ? 2 : 0) + (h4 ? 1 : 0);
+    return r;
+}
+#endif
+
 // tables.cu
 void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr);
 // neighbors.cu
 pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);
 pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n);   // exclusive, n+1 outputs
 pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n);
+pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *in, int *out);
 pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total);
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
 // realspace.cu

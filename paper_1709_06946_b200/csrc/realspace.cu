@@ -62,18 +62,16 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             e3 += A * a1.z + (rx * wz + rz * wx) * RS2;
             e4 += A * a1.w + (ry * wz + rz * wy) * RS2;
         }
-#pragma unroll
-        for (int o = 16; o; o >>= 1) {
-            u0 += __shfl_xor_sync(0xffffffffu, u0, o); u1 += __shfl_xor_sync(0xffffffffu, u1, o);
-            u2 += __shfl_xor_sync(0xffffffffu, u2, o); e0 += __shfl_xor_sync(0xffffffffu, e0, o);
-            e1 += __shfl_xor_sync(0xffffffffu, e1, o); e2 += __shfl_xor_sync(0xffffffffu, e2, o);
-            e3 += __shfl_xor_sync(0xffffffffu, e3, o); e4 += __shfl_xor_sync(0xffffffffu, e4, o);
-        }
-        if (lane == 0) {                                             // self term: r -> 0 limit, F1(0) F and A(0) S
+        // self term (r -> 0 limit: F1(0) F and A(0) S) added by lane 0 before the reduction
+        if (lane == 0) {
             const float4 a0 = in[2 * s], a1 = in[2 * s + 1], t0 = tab[0], t1 = tab[1];
-            out[2 * s] = make_float4(u0 + t0.x * a0.x, u1 + t0.x * a0.y, u2 + t0.x * a0.z, e0 + t1.x * a0.w);
-            out[2 * s + 1] = make_float4(e1 + t1.x * a1.x, e2 + t1.x * a1.y, e3 + t1.x * a1.z, e4 + t1.x * a1.w);
+            u0 += t0.x * a0.x; u1 += t0.x * a0.y; u2 += t0.x * a0.z; e0 += t1.x * a0.w;
+            e1 += t1.x * a1.x; e2 += t1.x * a1.y; e3 += t1.x * a1.z; e4 += t1.x * a1.w;
         }
+        const float part[8] = {u0, u1, u2, e0, e1, e2, e3, e4};
+        int comp;
+        const float r = warp_reduce8(part, lane, comp);
+        if ((lane & 3) == 0) reinterpret_cast<float *>(out)[(size_t)s * 8 + comp] = r;
     }
 }
 

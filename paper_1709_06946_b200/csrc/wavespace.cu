@@ -44,17 +44,6 @@ __global__ void scatter_to_tiles(const int *tile_of, int N, const int *tile_star
     tile_list[tile_start[t] + atomicAdd(&tile_fill[t], 1)] = s;
 }
 
-__global__ void sort_within_tiles(const int *tile_start, int ntile, int *tile_list) {
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntile) return;
-    int lo = tile_start[t], hi = tile_start[t + 1];
-    for (int i = lo + 1; i < hi; ++i) {
-        int v = tile_list[i], j = i - 1;
-        while (j >= lo && tile_list[j] > v) { tile_list[j + 1] = tile_list[j]; --j; }
-        tile_list[j + 1] = v;
-    }
-}
-
 // Tiles (along one axis) whose particles' supports can reach tile t: bases in [t*T-(P-1), t*T+T-1] mod M.
 __device__ int reach_tiles(int t, int M, int P, int nt, int *list) {
     int n = 0;
@@ -68,18 +57,29 @@ __device__ int reach_tiles(int t, int M, int P, int nt, int *list) {
     return n;
 }
 
-constexpr int SPREAD_BATCH = 64;
+constexpr int SPREAD_BATCH = 256;
 
-__global__ void __launch_bounds__(512)
+// wrapped offset of grid point gp (0 <= gp < M) from an unwrapped support base (-P < base < M + P)
+__device__ __forceinline__ int wrap_offset(int gp, int base, int M) {
+    int o = gp - base;
+    o += o < 0 ? M : 0;
+    o -= o >= M ? M : 0;
+    return o;
+}
+
+// 256 threads = 8 warps; warp a owns x-plane a of the tile, lane (b2 = lane>>3, c = lane&7) owns the two points
+// (a, b2, c) and (a, b2+4, c) with 2 x 8 accumulators in registers.  Candidates are staged 256 at a time (one
+// thread each: particle data + the 3 x 8 separable weights), then compacted into one list PER PLANE holding only
+// the particles whose support covers that plane, in candidate order (fixed summation order, no atomics).
+__global__ void __launch_bounds__(256)
 spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, const int *__restrict__ tile_start,
               const int *__restrict__ tile_list, float *__restrict__ grid, int M, int P, int nt, float inv_h, float wexp) {
     __shared__ float4 q[SPREAD_BATCH][2];
     __shared__ float W[SPREAD_BATCH][3][T];
-    __shared__ float gco[SPREAD_BATCH][3];
-    __shared__ int gbase[SPREAD_BATCH][3];
-    __shared__ int active[SPREAD_BATCH];
+    __shared__ unsigned short lst[T][SPREAD_BATCH];
+    __shared__ int cnt[T][9];                       // [plane][warp] counts, then exclusive prefix; [plane][8] = total
     __shared__ int bin_lo[64], bin_cum[65], nbins_s;
-    const int tid = threadIdx.x, a = tid >> 6, b = (tid >> 3) & 7, cc = tid & 7;
+    const int tid = threadIdx.x, lane = tid & 31, a = tid >> 5, b = lane >> 3, cc = lane & 7;
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int g0[3] = {t0 * T, t1 * T, t2 * T};
     if (tid == 0) {
@@ -94,49 +94,78 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
     }
     __syncthreads();
     const int nbins = nbins_s, total = bin_cum[nbins];
-    float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    float acc0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, acc1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (int lo = 0; lo < total; lo += SPREAD_BATCH) {
         const int nb = min(SPREAD_BATCH, total - lo);
+        unsigned xmask = 0;
         if (tid < nb) {
             int ci = lo + tid, k = 0;
             while (bin_cum[k + 1] <= ci) ++k;
-            int s = tile_list[bin_lo[k] + ci - bin_cum[k]];
-            float4 p = pos[s];
+            const int s = tile_list[bin_lo[k] + ci - bin_cum[k]];
+            const float4 p = pos[s];
             q[tid][0] = in[2 * s]; q[tid][1] = in[2 * s + 1];
-            float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
-            for (int d = 0; d < 3; ++d) { gco[tid][d] = g[d]; gbase[tid][d] = support_base(g[d], P); }
+            const float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
+            unsigned msk[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const int base = support_base(g[d], P);
+                msk[d] = 0;
+#pragma unroll
+                for (int i = 0; i < T; ++i) {
+                    const int gp = g0[d] + i, o = wrap_offset(gp, base, M);
+                    const float tt = (float)(base + o) - g[d];
+                    const bool inside = (o < P && gp < M);
+                    W[tid][d][i] = inside ? __expf(-wexp * tt * tt) : 0.f;
+                    msk[d] |= inside ? (1u << i) : 0u;
+                }
+            }
+            xmask = (msk[1] && msk[2]) ? msk[0] : 0u;
+        }
+        unsigned bal[T];
+#pragma unroll
+        for (int pl = 0; pl < T; ++pl) bal[pl] = __ballot_sync(0xffffffffu, (xmask >> pl) & 1u);
+#pragma unroll
+        for (int pl = 0; pl < T; ++pl) if (lane == pl) cnt[pl][a] = __popc(bal[pl]);
+        __syncthreads();
+        if (tid < T) {                                            // exclusive prefix over the 8 warps, per plane
+            int run = 0;
+            for (int w = 0; w < 8; ++w) { const int v = cnt[tid][w]; cnt[tid][w] = run; run += v; }
+            cnt[tid][8] = run;
         }
         __syncthreads();
-        for (int e = tid; e < nb * 3 * T; e += blockDim.x) {
-            int p = e / (3 * T), d = (e / T) % 3, i = e % T;
-            int gp = g0[d] + i, base = gbase[p][d];
-            int o = pmod(gp - base, M);
-            float tt = (float)(base + o) - gco[p][d];
-            W[p][d][i] = (o < P && gp < M) ? __expf(-wexp * tt * tt) : 0.f;
+        if (xmask) {
+#pragma unroll
+            for (int pl = 0; pl < T; ++pl)
+                if ((xmask >> pl) & 1u) lst[pl][cnt[pl][a] + __popc(bal[pl] & ((1u << lane) - 1))] = (unsigned short)tid;
         }
         __syncthreads();
-        if (tid < nb) {
-            bool any[3] = {false, false, false};
-            for (int d = 0; d < 3; ++d) for (int i = 0; i < T; ++i) any[d] |= (W[tid][d][i] != 0.f);
-            active[tid] = any[0] && any[1] && any[2];
-        }
-        __syncthreads();
-        for (int p = 0; p < nb; ++p) {
-            if (!active[p]) continue;
-            const float wx = W[p][0][a];
-            if (wx == 0.f) continue;                                  // warp-uniform (a is fixed within a warp)
-            const float w = wx * W[p][1][b] * W[p][2][cc];
+        const int nact = cnt[a][8];
+        for (int i = 0; i < nact; ++i) {
+            const int p = lst[a][i];
+            const float wx = W[p][0][a], wz = wx * W[p][2][cc];
+            const float w0 = wz * W[p][1][b], w1 = wz * W[p][1][b + 4];
             const float4 q0 = q[p][0], q1 = q[p][1];
-            acc[0] += w * q0.x; acc[1] += w * q0.y; acc[2] += w * q0.z; acc[3] += w * q0.w;
-            acc[4] += w * q1.x; acc[5] += w * q1.y; acc[6] += w * q1.z; acc[7] += w * q1.w;
+            acc0[0] += w0 * q0.x; acc0[1] += w0 * q0.y; acc0[2] += w0 * q0.z; acc0[3] += w0 * q0.w;
+            acc0[4] += w0 * q1.x; acc0[5] += w0 * q1.y; acc0[6] += w0 * q1.z; acc0[7] += w0 * q1.w;
+            acc1[0] += w1 * q0.x; acc1[1] += w1 * q0.y; acc1[2] += w1 * q0.z; acc1[3] += w1 * q0.w;
+            acc1[4] += w1 * q1.x; acc1[5] += w1 * q1.y; acc1[6] += w1 * q1.z; acc1[7] += w1 * q1.w;
         }
         __syncthreads();
     }
-    const int gx = g0[0] + a, gy = g0[1] + b, gz = g0[2] + cc;
-    if (gx < M && gy < M && gz < M) {
-        const size_t M3 = (size_t)M * M * M, o = ((size_t)gx * M + gy) * M + gz;
+    const int gx = g0[0] + a, gz = g0[2] + cc;
+    const size_t M3 = (size_t)M * M * M;
+    if (gx < M && gz < M) {
+        const int gy0 = g0[1] + b, gy1 = gy0 + 4;
+        if (gy0 < M) {
+            const size_t o = ((size_t)gx * M + gy0) * M + gz;
 #pragma unroll
-        for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc[c];
+            for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc0[c];
+        }
+        if (gy1 < M) {
+            const size_t o = ((size_t)gx * M + gy1) * M + gz;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc1[c];
+        }
     }
 }
 
@@ -185,6 +214,68 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
             r0.x += o0.x; r0.y += o0.y; r0.z += o0.z; r0.w += o0.w; r1.x += o1.x; r1.y += o1.y; r1.z += o1.z; r1.w += o1.w;
         }
         out[2 * s] = r0; out[2 * s + 1] = r1;
+    }
+}
+
+// Interpolation, tile-staged (default path): one CTA per tile bin.  The (T+P-1)^3 block of all 8 grids that the
+// bin's particles can touch is staged once in shared memory with coalesced loads (periodic wrap resolved while
+// loading), then each warp takes particles of the bin, lanes over the P^3 support, reading only shared memory.
+// Every particle belongs to exactly one bin, so the output is written once, with no atomics.
+__global__ void __launch_bounds__(256)
+interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_start, const int *__restrict__ tile_list,
+                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int P, int nt, float inv_h, float wexp,
+                   int accumulate) {
+    extern __shared__ float4 sm[];
+    const int E = T + P - 1, E3 = E * E * E;
+    float4 *lo = sm, *hi = sm + E3;
+    const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
+    const int first = tile_start[t], np = tile_start[t + 1] - first;
+    if (np == 0) return;
+    const size_t M3 = (size_t)M * M * M;
+    for (int idx = threadIdx.x; idx < E3; idx += blockDim.x) {
+        const int iz = idx % E, iy = (idx / E) % E, ix = idx / (E * E);
+        const size_t o = ((size_t)((t0 * T + ix) % M) * M + (t1 * T + iy) % M) * M + (t2 * T + iz) % M;
+        lo[idx] = make_float4(__ldg(grid + o), __ldg(grid + M3 + o), __ldg(grid + 2 * M3 + o), __ldg(grid + 3 * M3 + o));
+        hi[idx] = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int P2 = P * P, EE = E * E;
+    float *outf = reinterpret_cast<float *>(out);
+    // lane <-> (j,k) column of the support; the loop over i walks x with a uniform weight, so the inner loop is
+    // two 16-byte shared loads and 8 FMAs, no index arithmetic and no shuffles except the broadcast of wx[i].
+    for (int pi = wid; pi < np; pi += nw) {
+        const int s = tile_list[first + pi];
+        const float4 p = pos[s];
+        const float gx = p.x * inv_h, gy = p.y * inv_h, gz = p.z * inv_h;
+        const int b0 = support_base(gx, P), b1 = support_base(gy, P), b2 = support_base(gz, P);
+        const int r0 = pmod(b0, M) - t0 * T, r1 = pmod(b1, M) - t1 * T, r2 = pmod(b2, M) - t2 * T;
+        const float tx = (float)(b0 + lane) - gx;
+        const float wxr = lane < P ? __expf(-wexp * tx * tx) : 0.f;
+        float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int jk0 = 0; jk0 < P2; jk0 += 32) {
+            const int jk = jk0 + lane;
+            const bool ok = jk < P2;
+            const int j = ok ? jk / P : 0, k = ok ? jk % P : 0;
+            const float ty = (float)(b1 + j) - gy, tz = (float)(b2 + k) - gz;
+            const float wyz = ok ? __expf(-wexp * (ty * ty + tz * tz)) : 0.f;
+            int sidx = (r0 * E + r1 + j) * E + r2 + k;
+            float tsum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int i = 0; i < P; ++i, sidx += EE) {
+                const float wx = __shfl_sync(0xffffffffu, wxr, i);
+                const float4 v0 = lo[sidx], v1 = hi[sidx];
+                tsum[0] += wx * v0.x; tsum[1] += wx * v0.y; tsum[2] += wx * v0.z; tsum[3] += wx * v0.w;
+                tsum[4] += wx * v1.x; tsum[5] += wx * v1.y; tsum[6] += wx * v1.z; tsum[7] += wx * v1.w;
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) acc[c] += wyz * tsum[c];
+        }
+        int comp;
+        float r = warp_reduce8(acc, lane, comp);
+        if ((lane & 3) == 0) {
+            if (accumulate) r += outf[(size_t)s * 8 + comp];
+            outf[(size_t)s * 8 + comp] = r;
+        }
     }
 }
 
@@ -347,8 +438,8 @@ pse_status pse_tile_bins(pse_ctx *c) {
     CUDA_TRY(c, cudaMemsetAsync(c->d_tile_fill, 0, (size_t)(c->ntile + 1) * sizeof(int), c->stream));
     tile_of_particles<<<nb, TB, 0, c->stream>>>(c->d_pos, N, (float)(1.0 / c->h), c->M, c->P, c->nt, c->d_tile_of, c->d_tile_count); KERNEL_CHECK(c);
     PSE_TRY(pse_scan_i32(c, c->d_tile_count, c->d_tile_start, (size_t)c->ntile));
-    scatter_to_tiles<<<nb, TB, 0, c->stream>>>(c->d_tile_of, N, c->d_tile_start, c->d_tile_fill, c->d_tile_list); KERNEL_CHECK(c);
-    sort_within_tiles<<<(c->ntile + 127) / 128, 128, 0, c->stream>>>(c->d_tile_start, c->ntile, c->d_tile_list); KERNEL_CHECK(c);
+    scatter_to_tiles<<<nb, TB, 0, c->stream>>>(c->d_tile_of, N, c->d_tile_start, c->d_tile_fill, c->d_tile_tmp); KERNEL_CHECK(c);
+    PSE_TRY(pse_rank_sort(c, c->d_tile_start, c->ntile, c->d_tile_tmp, c->d_tile_list));
     return PSE_OK;
 }
 
@@ -366,10 +457,18 @@ static ScaleParams make_scale_params(const pse_ctx *c) {
 static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate) {
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r, c->d_spec, c->d_grid)); c->launches++; }
     ScopedPhase ph(c, PSE_T_INTERP);
-    const int TB = 256;
-    interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
-        c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
-        (float)(2.0 * M_PI / c->P), accumulate ? 1 : 0);
+    const int TB = 256, E = T + c->P - 1;
+    const size_t smem = (size_t)2 * E * E * E * sizeof(float4);
+    if (smem <= 200 * 1024) {
+        static size_t smem_set = 0;
+        if (smem > smem_set) { CUDA_TRY(c, cudaFuncSetAttribute(interp_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_set = smem; }
+        interp_tile_kernel<<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out),
+                                                             c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P), accumulate ? 1 : 0);
+    } else {
+        interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
+            c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
+            (float)(2.0 * M_PI / c->P), accumulate ? 1 : 0);
+    }
     KERNEL_CHECK(c);
     return PSE_OK;
 }
@@ -378,7 +477,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     const size_t nmode = (size_t)c->M * c->M * c->Mh;
     {
         ScopedPhase ph(c, PSE_T_SPREAD);
-        spread_kernel<<<c->ntile, 512, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
+        spread_kernel<<<c->ntile, 256, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
                                                        c->d_grid, c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P));
         KERNEL_CHECK(c);
     }

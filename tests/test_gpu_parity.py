@@ -223,3 +223,41 @@ def test_step_small_against_dense_oracle():
     disp = xn - x32.astype(np.float64)
     assert 2 <= gi <= 30 and 2 <= li <= 40
     assert np.linalg.norm(d) / np.linalg.norm(disp) < 5 * tol
+
+
+@pytest.mark.parametrize('N,phi,tol,xi,seed', [(3000, 0.20, 1e-3, 0.5, 21), (2500, 0.30, 1e-4, 0.6, 22), (3500, 0.10, 1e-2, 0.45, 23)])
+def test_product_mid_size_sampled_rows(N, phi, tol, xi, seed):
+    """Several cells and tiles per side, grid size not a multiple of the tile edge (ragged tail), parameters from
+    pse_suggest_params; oracle on sampled output rows."""
+    import paper_1709_06946_b200 as pse
+    x, L = synth.rsa(N, phi, seed=seed)
+    x32 = x.astype(np.float32)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    F, S = synth.gaussian_inputs(N, seed)
+    U, E = gpu_apply(ctx, F, S, 3)
+    rows = np.sort(np.random.default_rng(seed).choice(N, 24, replace=False))
+    Uo, Eo = mob.mobility_apply(x32.astype(np.float64), L, A, ETA, xi, F, S, rows=rows, eps=min(1e-7, tol * 1e-3))
+    assert rel(U[rows], Uo) < bar(tol) and rel(E[rows], Eo) < bar(tol)
+
+
+def test_large_support_uses_global_interpolation_path():
+    """P = 14 exceeds the shared-memory staging budget of the tiled interpolation: fallback kernel, same result."""
+    x, L = synth.rsa(200, 0.10, seed=31)
+    x32 = x.astype(np.float32)
+    xi, grid, tol = 0.6, 36, 1e-3
+    rcut = np.sqrt(-np.log(tol)) / xi + 1.0
+    F, S = synth.gaussian_inputs(200, 5)
+    outs = []
+    for P in (8, 14):
+        ctx = make_ctx(200, L, xi, grid, P, rcut, tol)
+        ctx.pse_neighbors(dev(pos4(x32)))
+        outs.append(np.hstack(gpu_apply(ctx, F, S, 2)))
+    k = brn.grid_modes(grid, L)
+    k2 = np.einsum('ki,ki->k', k, k)
+    w = fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2)
+    Ug, Eg = mob.wave_apply_modes(x32.astype(np.float64), L, A, ETA, k, w, F, S)
+    assert rel(outs[0], np.hstack([Ug, Eg])) < 1e-3
+    assert rel(outs[1], np.hstack([Ug, Eg])) < 2e-5      # P = 14: quadrature error ~1e-9, what is left is fp32
