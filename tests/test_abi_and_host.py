@@ -33,14 +33,14 @@ def test_library_exports_every_declared_symbol(pse):
 
 def test_suggest_params_rules(pse):
     st, grid, P, rcut = pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.6)
-    assert st == 0 and P == 6                       # Table I gives 5 at 1e-3; +1 calibrated (R6)
+    assert st == 0 and P == 6                       # Table I gives 5 at 1e-3; bound tightened 10x (R6)
     assert abs(rcut - (np.sqrt(-np.log(1e-3)) / 0.6 + 1.0)) < 1e-12 and rcut <= 13.892 / 2
     n = grid
     for p in (2, 3, 5, 7):
         while n % p == 0:
             n //= p
     assert n == 1 and grid >= 1.07 * 2 * 0.6 * np.sqrt(-np.log(1e-3)) * 13.892 / np.pi
-    for tol, want in [(1e-2, 5), (1e-3, 6), (1e-4, 7)]:
+    for tol, want in [(1e-2, 5), (1e-3, 6), (1e-4, 8)]:
         assert pse.pse_suggest_params(4096, 44.1, 1.0, tol, 0.5)[2] == want
     assert pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.3)[0] == pse.PSE_EINVAL      # rcut > L/2
     assert pse.pse_suggest_params(0, 13.892, 1.0, 1e-3, 0.6)[0] == pse.PSE_EINVAL
