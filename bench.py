@@ -261,8 +261,11 @@ def main():
     ap.add_argument('--workload', default='config3', choices=sorted(WORKLOADS))
     ap.add_argument('--impl', default='ours', choices=['ours', 'reference'])
     ap.add_argument('--no-cpu-baseline', action='store_true')
+    ap.add_argument('--xi', type=float, default=None, help='override the splitting parameter (tuning knob, PAPER.md:154)')
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
+    if args.xi:
+        wl['xi'] = args.xi
     rank, world = int(os.environ.get('RANK', 0)), int(os.environ.get('WORLD_SIZE', 1))
     config = {'workload': f'{args.workload}: N={wl["N"]} hard spheres, phi={wl["phi"]}, Ewald tol={wl["tol"]}, xi={wl["xi"]}, '
                           f'dt={wl["dt"]}, kT=1, RSA placement' + (f' + {wl["relax"]} relax sweeps' if wl['relax'] else ''),

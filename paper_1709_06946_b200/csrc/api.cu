@@ -24,6 +24,24 @@ __global__ void k_advance(const float4 *pos_in, const float *U, float dt, float 
 
 bool smooth7(int n) { for (int p : {2, 3, 5, 7}) while (n % p == 0) n /= p; return n == 1; }
 
+// cuFFT 11.4 on B200, batch of 8 R2C 3-D transforms, microseconds (profiles/r1_cufft_sizes.md).  The time is far
+// from monotone in the size, so the grid chooser takes the cheapest measured size that is large enough.
+const struct { int m; float us; } kFftCost[] = {
+    {64, 27}, {72, 34}, {80, 41}, {84, 47}, {90, 53}, {96, 76}, {100, 55}, {108, 78}, {112, 101}, {120, 99}, {125, 115},
+    {128, 96}, {135, 244}, {144, 137}, {150, 250}, {160, 226}, {162, 424}, {168, 432}, {175, 405}, {180, 494}, {192, 354},
+    {200, 586}, {216, 527}, {224, 959}, {225, 812}, {240, 982}, {243, 712}, {250, 1213}, {256, 692}, {270, 1396},
+    {288, 1653}, {300, 2053}, {320, 2381}, {324, 2310}, {336, 3089}, {343, 2156}, {350, 3931}, {360, 3217}, {375, 4921},
+    {384, 3964}, {400, 6977}};
+
+int choose_grid(int mmin) {
+    int best = 0; float cost = 1e30f;
+    for (const auto &e : kFftCost) if (e.m >= mmin && e.us < cost) { best = e.m; cost = e.us; }
+    if (best) return best;
+    int M = mmin;
+    while (!smooth7(M)) ++M;
+    return M;
+}
+
 }  // namespace
 
 extern "C" {
@@ -42,9 +60,9 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
     // 0.4-0.7 tol for xi in [0.5,0.7], phi in [0.1,0.3], tol in [1e-2,1e-4]).
     double rc = s / xi + 1.0 * a;
     // C2: wave cutoff k_cut = 2 xi s (H(k) ~ exp(-k^2/4 xi^2)); M >= 1.07 k_cut L / pi (the strain-rate rows carry an
-    // extra factor k, so the bare estimate leaves their truncation error at ~tol), rounded up to a 2,3,5,7-smooth size
+    // extra factor k, so the bare estimate leaves their truncation error at ~tol), then the cheapest measured cuFFT size >= that (2,3,5,7-smooth below 64)
     int M = std::max(8, (int)std::ceil(1.07 * 2.0 * xi * s * L / M_PI));
-    while (!smooth7(M)) ++M;
+    if (M > 64) M = choose_grid(M); else while (!smooth7(M)) ++M;
     // C3: quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1): e^{-pi P/2} + erfc(sqrt(pi P/2))
     // gives P = 5 at 1e-3 as in Table I.  Measured against the oracle, the relative L2 error of the
     // strain-rate rows is ~10-20x that bound (deconvolution amplifies the high-k quadrature error), so the bound is

@@ -179,6 +179,84 @@ __global__ void __launch_bounds__(256) neighbor_sweep(const float4 *__restrict__
     if (!FILL && lane == 0) count[s] = found;
 }
 
+// Neighbour sweep, CTA per cell (default path).  The candidates of a cell are the same for all of its particles:
+// up to 18 contiguous runs of the cell-sorted order (9 (x,y) columns, z-1..z+1 contiguous, split where z wraps).
+// They are staged once in shared memory in chunks of NS_CHUNK; each warp then takes particles of the cell and tests
+// 32 staged candidates per iteration with full lanes.  FILL=false accumulates counts, FILL=true writes the CSR
+// list in candidate order (deterministic).  Running per-particle positions live in `cursor` (global, zeroed).
+constexpr int NS_CHUNK = 1024, NS_THREADS = 128;
+
+template <bool FILL>
+__global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start,
+                                                                   int nc, float L, float invL, float rc2, int *__restrict__ cursor,
+                                                                   const unsigned long long *__restrict__ off, int *__restrict__ idx) {
+    __shared__ float4 cpos[NS_CHUNK];
+    __shared__ int run_lo[18], run_cum[19];
+    const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int first = cell_start[cell], np = cell_start[cell + 1] - first;
+    if (np == 0) return;
+    const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
+    const int span = nc >= 3 ? 3 : nc;
+    if (tid < 32) {
+        // lane r < 2*span*span describes run r: column (r>>1), part (r&1)
+        int lo = 0, len = 0;
+        const int col_i = lane >> 1, part = lane & 1;
+        if (col_i < span * span) {
+            int ccx = col_i / span, ccy = col_i % span;
+            if (nc >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + ccy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
+            const int col = (ccx * nc + ccy) * nc;
+            const int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
+            int a0, a1, b0 = 0, b1 = 0;                    // run A = cells [a0,a1), run B = cells [b0,b1)
+            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc - 1; b1 = nc; }
+            else if (z1 >= nc) { a0 = 0; a1 = 1; b0 = z0; b1 = nc; }
+            else { a0 = z0; a1 = z1 + 1; }
+            const int c0 = part ? b0 : a0, c1 = part ? b1 : a1;
+            lo = cell_start[col + c0]; len = cell_start[col + c1] - lo;
+        }
+        int inc = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+        if (lane < 18) { run_lo[lane] = lo; run_cum[lane] = inc - len; }
+        if (lane == 17) run_cum[18] = inc;
+    }
+    __syncthreads();
+    const int total = run_cum[18];
+    for (int c0 = 0; c0 < total; c0 += NS_CHUNK) {
+        const int nchunk = min(NS_CHUNK, total - c0);
+        for (int c = tid; c < nchunk; c += NS_THREADS) {
+            const int g = c0 + c;
+            int r = 0;
+            while (run_cum[r + 1] <= g) ++r;
+            const int j = run_lo[r] + g - run_cum[r];
+            float4 q = pos[j];
+            q.w = __int_as_float(j);
+            cpos[c] = q;
+        }
+        __syncthreads();
+        for (int pi = wid; pi < np; pi += NS_THREADS / 32) {
+            const int s = first + pi;
+            const float4 p = pos[s];
+            int found = (c0 == 0) ? 0 : cursor[s];
+            const unsigned long long base = FILL ? off[s] : 0ull;
+            for (int c = lane; c < nchunk + lane; c += 32) {        // all lanes take the same number of trips
+                bool in = false;
+                int j = -1;
+                if (c < nchunk) {
+                    const float4 q = cpos[c];
+                    j = __float_as_int(q.w);
+                    in = (j != s) && dist2(p, q, L, invL) < rc2;
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, in);
+                if (FILL && in) idx[base + found + __popc(m & ((1u << lane) - 1))] = j;
+                found += __popc(m);
+                if (c - lane + 32 >= nchunk) break;
+            }
+            if (lane == 0) cursor[s] = found;
+        }
+        __syncthreads();
+    }
+}
+
 __global__ void counts_to_original(const int *count_sorted, const int *order, int N, int *count_orig) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s < N) count_orig[order[s]] = count_sorted[s];
@@ -229,7 +307,7 @@ pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n) { ret
 
 pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     ScopedPhase ph(c, PSE_T_NEIGHBORS);
-    const int N = c->N, T = 256, nb = (N + T - 1) / T, nbw = (int)(((size_t)N * 32 + T - 1) / T);
+    const int N = c->N, T = 256, nb = (N + T - 1) / T;
     const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
     const float rc = (float)c->rcut, rc2 = rc * rc;
     c->have_nbrs = false;
@@ -241,8 +319,8 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order_tmp); KERNEL_CHECK(c);
     pse_rank_sort(c, c->d_cell_start, c->ncell, c->d_order_tmp, c->d_order);
     gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos); KERNEL_CHECK(c);
-    neighbor_sweep<false><<<nbw, T, 0, c->stream>>>(c->d_pos, N, c->d_cell_start, c->nc, cell_inv, L, invL, rc2,
-                                                    c->d_nbr_count, nullptr, nullptr); KERNEL_CHECK(c);
+    neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
+                                                                        nullptr, nullptr); KERNEL_CHECK(c);
     PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
     unsigned long long total = 0;
     CUDA_TRY(c, cudaMemcpyAsync(&total, c->d_nbr_off + N, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
@@ -256,8 +334,8 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         c->nbr_cap = cap;
     }
     c->nbr_total = (size_t)total;
-    neighbor_sweep<true><<<nbw, T, 0, c->stream>>>(c->d_pos, N, c->d_cell_start, c->nc, cell_inv, L, invL, rc2,
-                                                   nullptr, c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
+    neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
+                                                                       c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
     PSE_TRY(pse_tile_bins(c));
     c->have_nbrs = true;
     return PSE_OK;

@@ -82,17 +82,39 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
     const int tid = threadIdx.x, lane = tid & 31, a = tid >> 5, b = lane >> 3, cc = lane & 7;
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int g0[3] = {t0 * T, t1 * T, t2 * T};
-    if (tid == 0) {
-        int lx[4], ly[4], lz[4];
-        int nx = reach_tiles(t0, M, P, nt, lx), ny = reach_tiles(t1, M, P, nt, ly), nz = reach_tiles(t2, M, P, nt, lz);
-        int n = 0, cum = 0;
-        for (int i = 0; i < nx; ++i) for (int j = 0; j < ny; ++j) for (int k = 0; k < nz; ++k) {
-            int tb = (lx[i] * nt + ly[j]) * nt + lz[k];
-            bin_lo[n] = tile_start[tb]; bin_cum[n] = cum; cum += tile_start[tb + 1] - tile_start[tb]; ++n;
-        }
-        bin_cum[n] = cum; nbins_s = n;
-    }
+    __shared__ int reach[3][4], nreach[3];
+    if (tid < 3) nreach[tid] = reach_tiles(tid == 0 ? t0 : (tid == 1 ? t1 : t2), M, P, nt, reach[tid]);
     __syncthreads();
+    {
+        const int nx = nreach[0], ny = nreach[1], nz = nreach[2], n = nx * ny * nz;
+        int cntb = 0;
+        if (tid < n) {                                    // one thread per candidate bin: a single global round trip
+            const int i = tid / (ny * nz), j = (tid / nz) % ny, k = tid % nz;
+            const int tb = (reach[0][i] * nt + reach[1][j]) * nt + reach[2][k];
+            const int lo = tile_start[tb];
+            cntb = tile_start[tb + 1] - lo;
+            bin_lo[tid] = lo;
+        }
+        if (tid < 64) {                                   // n <= 64: inclusive scan over two warps
+            int inc = cntb;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+            if (tid == 31) bin_cum[64] = inc;             // total of warp 0, parked in the last slot
+            __syncwarp();
+            if (tid < 32) bin_cum[tid] = inc - cntb;
+        }
+        __syncthreads();
+        if (tid >= 32 && tid < 64) {
+            int inc = cntb;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+            bin_cum[tid] = bin_cum[64] + inc - cntb;
+            if (tid == 63) nbins_s = bin_cum[64] + inc;   // grand total
+        }
+        __syncthreads();
+        if (tid == 0) { const int tot = nbins_s; bin_cum[n] = tot; nbins_s = n; }
+        __syncthreads();
+    }
     const int nbins = nbins_s, total = bin_cum[nbins];
     float acc0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, acc1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (int lo = 0; lo < total; lo += SPREAD_BATCH) {
@@ -232,11 +254,23 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     const int first = tile_start[t], np = tile_start[t + 1] - first;
     if (np == 0) return;
     const size_t M3 = (size_t)M * M * M;
-    for (int idx = threadIdx.x; idx < E3; idx += blockDim.x) {
-        const int iz = idx % E, iy = (idx / E) % E, ix = idx / (E * E);
-        const size_t o = ((size_t)((t0 * T + ix) % M) * M + (t1 * T + iy) % M) * M + (t2 * T + iz) % M;
-        lo[idx] = make_float4(__ldg(grid + o), __ldg(grid + M3 + o), __ldg(grid + 2 * M3 + o), __ldg(grid + 3 * M3 + o));
-        hi[idx] = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
+    {   // stage row by row: a half-warp (E <= 16) or a warp per (ix,iy) row, lanes along z; wrap by subtraction
+        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        const int rpi = E <= 16 ? 2 : 1, lz = E <= 16 ? (lane & 15) : lane, sub = E <= 16 ? (lane >> 4) : 0;
+        int gz = t2 * T + lz;
+        while (gz >= M) gz -= M;
+        for (int row = wid * rpi + sub; row < E * E; row += nw * rpi) {
+            const int ix = row / E, iy = row - ix * E;
+            int gx = t0 * T + ix, gy = t1 * T + iy;
+            while (gx >= M) gx -= M;
+            while (gy >= M) gy -= M;
+            if (lz < E) {
+                const size_t o = ((size_t)gx * M + gy) * M + gz;
+                const int idx = row * E + lz;
+                lo[idx] = make_float4(__ldg(grid + o), __ldg(grid + M3 + o), __ldg(grid + 2 * M3 + o), __ldg(grid + 3 * M3 + o));
+                hi[idx] = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
+            }
+        }
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;

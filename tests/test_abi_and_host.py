@@ -40,6 +40,9 @@ def test_suggest_params_rules(pse):
         while n % p == 0:
             n //= p
     assert n == 1 and grid >= 1.07 * 2 * 0.6 * np.sqrt(-np.log(1e-3)) * 13.892 / np.pi
+    # above 64 the cheapest measured cuFFT size is taken (profiles/r1_cufft_sizes.md): 90 -> 90, 320 -> 343, 97 -> 100
+    assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.5)[1] == 90
+    assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.55)[1] == 100
     for tol, want in [(1e-2, 5), (1e-3, 6), (1e-4, 8)]:
         assert pse.pse_suggest_params(4096, 44.1, 1.0, tol, 0.5)[2] == want
     assert pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.3)[0] == pse.PSE_EINVAL      # rcut > L/2
