@@ -57,7 +57,7 @@ __device__ int reach_tiles(int t, int M, int P, int nt, int *list) {
     return n;
 }
 
-constexpr int SPREAD_BATCH = 256;
+constexpr int SPREAD_BATCH = 128, SPREAD_THREADS = 128;
 
 // wrapped offset of grid point gp (0 <= gp < M) from an unwrapped support base (-P < base < M + P)
 __device__ __forceinline__ int wrap_offset(int gp, int base, int M) {
@@ -67,26 +67,29 @@ __device__ __forceinline__ int wrap_offset(int gp, int base, int M) {
     return o;
 }
 
-// 256 threads = 8 warps; warp a owns x-plane a of the tile, lane (b2 = lane>>3, c = lane&7) owns the two points
-// (a, b2, c) and (a, b2+4, c) with 2 x 8 accumulators in registers.  Candidates are staged 256 at a time (one
-// thread each: particle data + the 3 x 8 separable weights), then compacted into one list PER PLANE holding only
-// the particles whose support covers that plane, in candidate order (fixed summation order, no atomics).
-__global__ void __launch_bounds__(256)
+// 128 threads = 4 warps per 8^3 tile.  Warp w owns the x-planes 2w and 2w+1 (one per half-warp); inside a half-warp
+// lane (b2 = bit 3, c = bits 0..2) owns the four points y = b2, b2+2, b2+4, b2+6 at z = c: 4 x 8 accumulators in
+// registers, 32 FMAs per particle for ~18 other instructions.  Candidates are staged 128 at a time (one thread each:
+// particle data + the 3 x 8 separable weights, y-weights stored permuted so that a lane's four are one float4), then
+// compacted into one list per plane PAIR holding only the particles whose support covers it, in candidate order
+// (fixed summation order, no atomics).
+__global__ void __launch_bounds__(SPREAD_THREADS)
 spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, const int *__restrict__ tile_start,
               const int *__restrict__ tile_list, float *__restrict__ grid, int M, int P, int nt, float inv_h, float wexp) {
     __shared__ float4 q[SPREAD_BATCH][2];
-    __shared__ float W[SPREAD_BATCH][3][T];
-    __shared__ unsigned short lst[T][SPREAD_BATCH];
-    __shared__ int cnt[T][9];                       // [plane][warp] counts, then exclusive prefix; [plane][8] = total
+    __shared__ __align__(16) float W[SPREAD_BATCH][3][T];
+    __shared__ unsigned short lst[4][SPREAD_BATCH];
+    __shared__ int cnt[4][5];                       // [plane pair][warp] counts -> exclusive prefix; [pair][4] = total
     __shared__ int bin_lo[64], bin_cum[65], nbins_s;
-    const int tid = threadIdx.x, lane = tid & 31, a = tid >> 5, b = lane >> 3, cc = lane & 7;
+    __shared__ int reach[3][4], nreach[3];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int half = lane >> 4, b2 = (lane >> 3) & 1, cc = lane & 7, a = 2 * wid + half;
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int g0[3] = {t0 * T, t1 * T, t2 * T};
-    __shared__ int reach[3][4], nreach[3];
     if (tid < 3) nreach[tid] = reach_tiles(tid == 0 ? t0 : (tid == 1 ? t1 : t2), M, P, nt, reach[tid]);
     __syncthreads();
     {
-        const int nx = nreach[0], ny = nreach[1], nz = nreach[2], n = nx * ny * nz;
+        const int ny = nreach[1], nz = nreach[2], n = nreach[0] * ny * nz;
         int cntb = 0;
         if (tid < n) {                                    // one thread per candidate bin: a single global round trip
             const int i = tid / (ny * nz), j = (tid / nz) % ny, k = tid % nz;
@@ -95,28 +98,23 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
             cntb = tile_start[tb + 1] - lo;
             bin_lo[tid] = lo;
         }
-        if (tid < 64) {                                   // n <= 64: inclusive scan over two warps
-            int inc = cntb;
+        int inc = cntb;                                   // n <= 64: inclusive scans in warps 0 and 1
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-            if (tid == 31) bin_cum[64] = inc;             // total of warp 0, parked in the last slot
-            __syncwarp();
-            if (tid < 32) bin_cum[tid] = inc - cntb;
-        }
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+        if (tid == 31) bin_cum[64] = inc;                 // total of warp 0, parked in the last slot
+        if (tid < 32) bin_cum[tid] = inc - cntb;
         __syncthreads();
-        if (tid >= 32 && tid < 64) {
-            int inc = cntb;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-            bin_cum[tid] = bin_cum[64] + inc - cntb;
-            if (tid == 63) nbins_s = bin_cum[64] + inc;   // grand total
-        }
+        if (wid == 1) { bin_cum[tid] = bin_cum[64] + inc - cntb; if (lane == 31) nbins_s = bin_cum[64] + inc; }
         __syncthreads();
         if (tid == 0) { const int tot = nbins_s; bin_cum[n] = tot; nbins_s = n; }
         __syncthreads();
     }
     const int nbins = nbins_s, total = bin_cum[nbins];
-    float acc0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, acc1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    float acc[4][8];
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[m][c] = 0.f;
     for (int lo = 0; lo < total; lo += SPREAD_BATCH) {
         const int nb = min(SPREAD_BATCH, total - lo);
         unsigned xmask = 0;
@@ -137,56 +135,57 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
                     const int gp = g0[d] + i, o = wrap_offset(gp, base, M);
                     const float tt = (float)(base + o) - g[d];
                     const bool inside = (o < P && gp < M);
-                    W[tid][d][i] = inside ? __expf(-wexp * tt * tt) : 0.f;
+                    W[tid][d][d == 1 ? ((i & 1) * 4 + (i >> 1)) : i] = inside ? __expf(-wexp * tt * tt) : 0.f;
                     msk[d] |= inside ? (1u << i) : 0u;
                 }
             }
             xmask = (msk[1] && msk[2]) ? msk[0] : 0u;
         }
-        unsigned bal[T];
+        unsigned bal[4];
 #pragma unroll
-        for (int pl = 0; pl < T; ++pl) bal[pl] = __ballot_sync(0xffffffffu, (xmask >> pl) & 1u);
+        for (int pr = 0; pr < 4; ++pr) bal[pr] = __ballot_sync(0xffffffffu, (xmask >> (2 * pr)) & 3u);
 #pragma unroll
-        for (int pl = 0; pl < T; ++pl) if (lane == pl) cnt[pl][a] = __popc(bal[pl]);
+        for (int pr = 0; pr < 4; ++pr) if (lane == pr) cnt[pr][wid] = __popc(bal[pr]);
         __syncthreads();
-        if (tid < T) {                                            // exclusive prefix over the 8 warps, per plane
+        if (tid < 4) {                                            // exclusive prefix over the 4 warps, per plane pair
             int run = 0;
-            for (int w = 0; w < 8; ++w) { const int v = cnt[tid][w]; cnt[tid][w] = run; run += v; }
-            cnt[tid][8] = run;
+#pragma unroll
+            for (int w = 0; w < 4; ++w) { const int v = cnt[tid][w]; cnt[tid][w] = run; run += v; }
+            cnt[tid][4] = run;
         }
         __syncthreads();
         if (xmask) {
 #pragma unroll
-            for (int pl = 0; pl < T; ++pl)
-                if ((xmask >> pl) & 1u) lst[pl][cnt[pl][a] + __popc(bal[pl] & ((1u << lane) - 1))] = (unsigned short)tid;
+            for (int pr = 0; pr < 4; ++pr)
+                if ((xmask >> (2 * pr)) & 3u) lst[pr][cnt[pr][wid] + __popc(bal[pr] & ((1u << lane) - 1))] = (unsigned short)tid;
         }
         __syncthreads();
-        const int nact = cnt[a][8];
+        const int nact = cnt[wid][4];
         for (int i = 0; i < nact; ++i) {
-            const int p = lst[a][i];
-            const float wx = W[p][0][a], wz = wx * W[p][2][cc];
-            const float w0 = wz * W[p][1][b], w1 = wz * W[p][1][b + 4];
+            const int p = lst[wid][i];
+            const float wxz = W[p][0][a] * W[p][2][cc];
+            const float4 wy = *reinterpret_cast<const float4 *>(&W[p][1][4 * b2]);
             const float4 q0 = q[p][0], q1 = q[p][1];
-            acc0[0] += w0 * q0.x; acc0[1] += w0 * q0.y; acc0[2] += w0 * q0.z; acc0[3] += w0 * q0.w;
-            acc0[4] += w0 * q1.x; acc0[5] += w0 * q1.y; acc0[6] += w0 * q1.z; acc0[7] += w0 * q1.w;
-            acc1[0] += w1 * q0.x; acc1[1] += w1 * q0.y; acc1[2] += w1 * q0.z; acc1[3] += w1 * q0.w;
-            acc1[4] += w1 * q1.x; acc1[5] += w1 * q1.y; acc1[6] += w1 * q1.z; acc1[7] += w1 * q1.w;
+            const float w[4] = {wxz * wy.x, wxz * wy.y, wxz * wy.z, wxz * wy.w};
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                acc[m][0] += w[m] * q0.x; acc[m][1] += w[m] * q0.y; acc[m][2] += w[m] * q0.z; acc[m][3] += w[m] * q0.w;
+                acc[m][4] += w[m] * q1.x; acc[m][5] += w[m] * q1.y; acc[m][6] += w[m] * q1.z; acc[m][7] += w[m] * q1.w;
+            }
         }
         __syncthreads();
     }
     const int gx = g0[0] + a, gz = g0[2] + cc;
     const size_t M3 = (size_t)M * M * M;
     if (gx < M && gz < M) {
-        const int gy0 = g0[1] + b, gy1 = gy0 + 4;
-        if (gy0 < M) {
-            const size_t o = ((size_t)gx * M + gy0) * M + gz;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc0[c];
-        }
-        if (gy1 < M) {
-            const size_t o = ((size_t)gx * M + gy1) * M + gz;
+        for (int m = 0; m < 4; ++m) {
+            const int gy = g0[1] + b2 + 2 * m;
+            if (gy < M) {
+                const size_t o = ((size_t)gx * M + gy) * M + gz;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc1[c];
+                for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc[m][c];
+            }
         }
     }
 }
@@ -243,13 +242,15 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
 // bin's particles can touch is staged once in shared memory with coalesced loads (periodic wrap resolved while
 // loading), then each warp takes particles of the bin, lanes over the P^3 support, reading only shared memory.
 // Every particle belongs to exactly one bin, so the output is written once, with no atomics.
+template <int PT>                                  // PT > 0: support size known at compile time (no integer divisions)
 __global__ void __launch_bounds__(256)
 interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_start, const int *__restrict__ tile_list,
-                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int P, int nt, float inv_h, float wexp,
+                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int Prt, int nt, float inv_h, float wexp,
                    int accumulate) {
     extern __shared__ float4 sm[];
-    const int E = T + P - 1, E3 = E * E * E;
-    float4 *lo = sm, *hi = sm + E3;
+    const int P = PT ? PT : Prt;
+    const int E = T + P - 1, Ez = E + ((P - E) & 7), E3 = E * E * Ez;   // z-rows padded so that Ez = P (mod 8): the
+    float4 *lo = sm, *hi = sm + E3;                                      // 16-byte chunks of a (j,k) lane set never collide
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int first = tile_start[t], np = tile_start[t + 1] - first;
     if (np == 0) return;
@@ -266,7 +267,7 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
             while (gy >= M) gy -= M;
             if (lz < E) {
                 const size_t o = ((size_t)gx * M + gy) * M + gz;
-                const int idx = row * E + lz;
+                const int idx = row * Ez + lz;
                 lo[idx] = make_float4(__ldg(grid + o), __ldg(grid + M3 + o), __ldg(grid + 2 * M3 + o), __ldg(grid + 3 * M3 + o));
                 hi[idx] = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
             }
@@ -274,7 +275,7 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    const int P2 = P * P, EE = E * E;
+    const int P2 = P * P, EE = E * Ez;
     float *outf = reinterpret_cast<float *>(out);
     // lane <-> (j,k) column of the support; the loop over i walks x with a uniform weight, so the inner loop is
     // two 16-byte shared loads and 8 FMAs, no index arithmetic and no shuffles except the broadcast of wx[i].
@@ -293,9 +294,11 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
             const int j = ok ? jk / P : 0, k = ok ? jk % P : 0;
             const float ty = (float)(b1 + j) - gy, tz = (float)(b2 + k) - gz;
             const float wyz = ok ? __expf(-wexp * (ty * ty + tz * tz)) : 0.f;
-            int sidx = (r0 * E + r1 + j) * E + r2 + k;
+            int sidx = (r0 * E + r1 + j) * Ez + r2 + k;
             float tsum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-            for (int i = 0; i < P; ++i, sidx += EE) {
+#pragma unroll
+            for (int i = 0; i < (PT ? PT : PSE_MAXP); ++i, sidx += EE) {
+                if (!PT && i >= P) break;
                 const float wx = __shfl_sync(0xffffffffu, wxr, i);
                 const float4 v0 = lo[sidx], v1 = hi[sidx];
                 tsum[0] += wx * v0.x; tsum[1] += wx * v0.y; tsum[2] += wx * v0.z; tsum[3] += wx * v0.w;
@@ -492,12 +495,29 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r, c->d_spec, c->d_grid)); c->launches++; }
     ScopedPhase ph(c, PSE_T_INTERP);
     const int TB = 256, E = T + c->P - 1;
-    const size_t smem = (size_t)2 * E * E * E * sizeof(float4);
+    const int Ez = E + ((c->P - E) & 7);
+    const size_t smem = (size_t)2 * E * E * Ez * sizeof(float4);
     if (smem <= 200 * 1024) {
-        static size_t smem_set = 0;
-        if (smem > smem_set) { CUDA_TRY(c, cudaFuncSetAttribute(interp_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); smem_set = smem; }
-        interp_tile_kernel<<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out),
-                                                             c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P), accumulate ? 1 : 0);
+#define PSE_LAUNCH_INTERP(PT)                                                                                              \
+    do {                                                                                                                   \
+        static size_t smem_set = 0;                                                                                        \
+        if (smem > smem_set) {                                                                                             \
+            CUDA_TRY(c, cudaFuncSetAttribute(interp_tile_kernel<PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+            smem_set = smem;                                                                                               \
+        }                                                                                                                  \
+        interp_tile_kernel<PT><<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid,       \
+            reinterpret_cast<float4 *>(d_out), c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P),          \
+            accumulate ? 1 : 0);                                                                                           \
+    } while (0)
+        switch (c->P) {
+            case 4: PSE_LAUNCH_INTERP(4); break;
+            case 5: PSE_LAUNCH_INTERP(5); break;
+            case 6: PSE_LAUNCH_INTERP(6); break;
+            case 7: PSE_LAUNCH_INTERP(7); break;
+            case 8: PSE_LAUNCH_INTERP(8); break;
+            default: PSE_LAUNCH_INTERP(0); break;
+        }
+#undef PSE_LAUNCH_INTERP
     } else {
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
@@ -511,7 +531,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     const size_t nmode = (size_t)c->M * c->M * c->Mh;
     {
         ScopedPhase ph(c, PSE_T_SPREAD);
-        spread_kernel<<<c->ntile, 256, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
+        spread_kernel<<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
                                                        c->d_grid, c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P));
         KERNEL_CHECK(c);
     }
