@@ -75,6 +75,11 @@ class ClockSampler:
                 'samples': len(sm)}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+# (profiles/r1_traffic.json.md), workload config3 only; other workloads report null.
+NCU_TRAFFIC = {'config3': {'real': 33551616, 'spread': 4061440, 'interp': 26755584}}
+
+
 def max_over_ranks(ms, device=None):
     """Replica aggregation: the job's time is the slowest rank's; no data-path collective."""
     import torch
@@ -328,7 +333,7 @@ def main():
     line['e2e'] = {'value': 1e3 / r['e2e_ms'], 'unit': 'steps/s', 'h2d_bytes_per_step': r['h2d'], 'd2h_bytes_per_step': r['d2h'],
                    'api': 'pse_step_host (pinned host buffers, copies inside the timed call)', 'steps': r['e2e_steps']}
     line['roofline'] = {'bound': 'hbm', 'kernel': dom, 'achieved': phases[dom]['alg_GBps'], 'peak': peak, 'unit': 'GB/s',
-                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': None, 'peak_source': peak_src,
+                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not args.xi else None, 'peak_source': peak_src,
                         'note': 'algorithmic bytes per launch / mean launch duration from CUDA events inside the library over '
                                 f'{r["profiled_steps"]} profiled steps; at this size the grids are L2-resident (see DESIGN.md §5)'}
     line['phases'] = phases
