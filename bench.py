@@ -233,7 +233,7 @@ def oracle_sample(wl, nsteps):
     N_s spheres at the workload's volume fraction and tolerance.  Returns (seconds per oracle step, N_s, cores, text)."""
     import synth
     from oracle import brownian as brn
-    Ns = 96
+    Ns = 128
     x, L = synth.rsa(Ns, wl['phi'], seed=7)
     s = np.sqrt(-np.log(wl['tol']))
     xi = max(wl['xi'], 1.02 * s / (0.5 * L - 2 * A))                 # keep rcut = s/xi + 2a <= L/2 in the small box

@@ -1,6 +1,7 @@
 // C-ABI entry points of libpse (include/pse.h).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <new>
 #include "pse_internal.h"
 
@@ -120,16 +121,23 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     c->krylov_cap = PSE_MAX_KRYLOV + 1;
     CUDA_TRY(c, cudaMalloc(&c->d_krylov, (size_t)c->krylov_cap * n8));
     CUDA_TRY(c, cudaMalloc(&c->d_zu, (size_t)PSE_MAX_KRYLOV * n8));
-    CUDA_TRY(c, cudaMalloc(&c->d_scal, 64 * sizeof(double)));
-    CUDA_TRY(c, cudaMallocHost(&c->h_scal, 256 * sizeof(double)));
+    CUDA_TRY(c, cudaMalloc(&c->d_scal, 2048 * sizeof(double)));
+    CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_real, cudaEventDisableTiming));
+    if (const char *e = getenv("PSE_OVERLAP")) c->overlap = (e[0] != '0');
     return PSE_OK;
 }
 
 pse_status pse_destroy(pse_ctx *c) {
     if (!c) return PSE_OK;
     cudaStreamSynchronize(c->stream);
+    if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_real) cudaEventDestroy(c->ev_real);
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
@@ -285,6 +293,16 @@ pse_status pse_get_table(pse_ctx *c, float *h_table, int cap_nodes, int *n_nodes
 }  // extern "C"
 
 pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which) {
+    if (which == PSE_BOTH && c->overlap && !c->profiling && c->stream2) {
+        // the two halves of the Ewald sum are independent: the pair kernel (one CTA per SM, so that it leaves half of
+        // every SM's registers free) runs on a second stream while spread / FFT / scale / FFT run on the main one;
+        // the interpolation, which accumulates into the same output, waits for it.
+        CUDA_TRY(c, cudaEventRecord(c->ev_fork, c->stream));
+        CUDA_TRY(c, cudaStreamWaitEvent(c->stream2, c->ev_fork, 0));
+        PSE_TRY(pse_real_apply(c, d_in, d_out, c->stream2, 1));
+        CUDA_TRY(c, cudaEventRecord(c->ev_real, c->stream2));
+        return pse_wave_apply(c, d_in, d_out, true, c->ev_real);
+    }
     if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out));
     if (which & PSE_WAVE) PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0));
     return PSE_OK;

@@ -67,22 +67,6 @@ __global__ void __launch_bounds__(VT) k_multi_dot(const float4 *base, size_t str
     }
 }
 
-// u -= sum_j coef[j] V_j ;  *norm2 += |u|^2
-__global__ void __launch_bounds__(VT) k_sub_lincomb_norm(float4 *u, const float4 *base, size_t stride4, int nvec, const float *coef,
-                                                         size_t n4, double *norm2) {
-    double acc = 0;
-    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
-        float4 x = u[i];
-        for (int j = 0; j < nvec; ++j) {
-            float4 v = base[(size_t)j * stride4 + i]; float cj = coef[j];
-            x.x -= cj * v.x; x.y -= cj * v.y; x.z -= cj * v.z; x.w -= cj * v.w;
-        }
-        u[i] = x;
-        acc += (double)(x.x * x.x + x.y * x.y) + (double)(x.z * x.z + x.w * x.w);
-    }
-    acc = block_sum(acc);
-    if (threadIdx.x == 0) atomicAdd(norm2, acc);
-}
 
 // out = beta * init + sum_j coef[j] V_j   (init may be null)
 __global__ void __launch_bounds__(VT) k_lincomb(float4 *out, const float4 *init, float beta, const float4 *base, size_t stride4, int nvec,
@@ -104,14 +88,6 @@ __global__ void __launch_bounds__(VT) k_axpby(size_t n, float alpha, const float
         y[i] = alpha * x[i] + (beta != 0.f ? beta * y[i] : 0.f);
 }
 
-// dst = scale * src with the velocity components (0..2 of every 8) zeroed: the E-part embedding used by GMRES
-__global__ void __launch_bounds__(VT) k_epart(float4 *dst, const float4 *src, float scale, int N) {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    float4 a = src[2 * s], b = src[2 * s + 1];
-    dst[2 * s] = make_float4(0.f, 0.f, 0.f, scale * a.w);
-    dst[2 * s + 1] = make_float4(scale * b.x, scale * b.y, scale * b.z, scale * b.w);
-}
 
 // rhs = -(EB + E-part(z0)) embedded with zero velocity components (either input may be null)
 __global__ void __launch_bounds__(VT) k_rhs(float4 *dst, const float4 *EBp, const float4 *z0, int N) {
@@ -140,6 +116,57 @@ __global__ void __launch_bounds__(VT) k_constraint_result(float4 *out, const flo
         sa.w += yj * va.w; sb.x += yj * vb.x; sb.y += yj * vb.y; sb.z += yj * vb.z; sb.w += yj * vb.w;
     }
     out[2 * s] = make_float4(ux, uy, uz, sa.w); out[2 * s + 1] = sb;
+}
+
+// ---- device-resident scalars: the update kernels read alpha / beta / h straight from the slots the dot kernels
+// accumulated into, so an iteration needs one host read-back (for the tiny T / Hessenberg algebra and the stopping
+// test) instead of a read-back plus a coefficient upload per reduction. ----
+
+// Lanczos three-term update: u -= alpha v_j + beta_{j-1} v_{j-1};  *beta2_out += |u|^2
+__global__ void __launch_bounds__(VT) k_lanczos_update(float4 *u, const float4 *vj, const float4 *vjm1, const double *alpha,
+                                                       const double *beta2_prev, size_t n4, double *beta2_out) {
+    const float a = (float)*alpha, b = beta2_prev ? (float)sqrt(*beta2_prev) : 0.f;
+    double acc = 0;
+    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
+        float4 x = u[i];
+        const float4 v = vj[i];
+        x.x -= a * v.x; x.y -= a * v.y; x.z -= a * v.z; x.w -= a * v.w;
+        if (vjm1) { const float4 p = vjm1[i]; x.x -= b * p.x; x.y -= b * p.y; x.z -= b * p.z; x.w -= b * p.w; }
+        u[i] = x;
+        acc += (double)(x.x * x.x + x.y * x.y) + (double)(x.z * x.z + x.w * x.w);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) atomicAdd(beta2_out, acc);
+}
+
+// dst = src / sqrt(*norm2)   (dst = 0 if the norm vanishes)
+__global__ void __launch_bounds__(VT) k_scale_dev(float4 *dst, const float4 *src, const double *norm2, size_t n4) {
+    const double n2 = *norm2;
+    const float sc = n2 > 0 ? (float)(1.0 / sqrt(n2)) : 0.f;
+    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
+        float4 x = src[i];
+        x.x *= sc; x.y *= sc; x.z *= sc; x.w *= sc;
+        dst[i] = x;
+    }
+}
+
+// Gram-Schmidt step of GMRES fused with the E-part embedding: w = Epart(Z) - sum_j h[j] V_j;  *norm2 += |w|^2
+__global__ void __launch_bounds__(VT) k_gs_update(float4 *w, const float4 *Z, const float4 *V, size_t stride4, int nvec, const double *h,
+                                                  int N, double *norm2) {
+    double acc = 0;
+    for (int s = blockIdx.x * VT + threadIdx.x; s < N; s += gridDim.x * VT) {
+        float4 a = Z[2 * s], b = Z[2 * s + 1];
+        a.x = a.y = a.z = 0.f;
+        for (int j = 0; j < nvec; ++j) {
+            const float hj = (float)h[j];
+            const float4 va = V[(size_t)j * stride4 + 2 * s], vb = V[(size_t)j * stride4 + 2 * s + 1];
+            a.w -= hj * va.w; b.x -= hj * vb.x; b.y -= hj * vb.y; b.z -= hj * vb.z; b.w -= hj * vb.w;
+        }
+        w[2 * s] = a; w[2 * s + 1] = b;
+        acc += (double)(a.w * a.w + b.x * b.x) + (double)(b.y * b.y + b.z * b.z) + (double)(b.w * b.w);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) atomicAdd(norm2, acc);
 }
 
 // cyclic Jacobi eigen-decomposition of a small symmetric matrix (n <= 51), fp64, host
@@ -181,7 +208,7 @@ pse_status zero_scalars(pse_ctx *c, int n) {
     return PSE_OK;
 }
 pse_status upload_coefs(pse_ctx *c, const std::vector<float> &v) {
-    float *hp = reinterpret_cast<float *>(c->h_scal + 128);
+    float *hp = reinterpret_cast<float *>(c->h_scal + 2048);
     std::memcpy(hp, v.data(), v.size() * sizeof(float));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_coef, hp, v.size() * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     return PSE_OK;
@@ -217,32 +244,32 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     float4 *V = reinterpret_cast<float4 *>(c->d_krylov);
     float4 *u = reinterpret_cast<float4 *>(c->d_tmp);
     const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap - 1);
-    PSE_TRY(zero_scalars(c, 1));
+    // slots: [0] = |w|^2, [1+2j] = alpha_j, [2+2j] = beta_j^2
+    const int nslots = 1 + 2 * maxit;
+    PSE_TRY(zero_scalars(c, nslots));
     { ScopedPhase ph(c, PSE_T_VECTOR);
-      k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_w), 0, 1, reinterpret_cast<const float4 *>(d_w), n4, c->d_scal); KERNEL_CHECK(c); }
-    PSE_TRY(read_scalars(c, 1));
-    const double wn = std::sqrt(c->h_scal[0]);
+      k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_w), 0, 1, reinterpret_cast<const float4 *>(d_w), n4, c->d_scal); KERNEL_CHECK(c);
+      k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V, reinterpret_cast<const float4 *>(d_w), c->d_scal, n4); KERNEL_CHECK(c); }
     if (iters) *iters = 0;
-    if (!(wn > 0)) { CUDA_TRY(c, cudaMemsetAsync(d_y, 0, n * sizeof(float), c->stream)); return PSE_OK; }
-    PSE_TRY(pse_axpby(c, n, (float)(1.0 / wn), d_w, 0.f, reinterpret_cast<float *>(V)));
     std::vector<double> alpha, beta, cprev, ccur;
+    double wn = 0;
     int m = 0;
     bool converged = false;
     for (int j = 0; j < maxit; ++j) {
-        PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(V + (size_t)j * n4), reinterpret_cast<float *>(u)));
-        PSE_TRY(zero_scalars(c, 2));
+        float4 *vj = V + (size_t)j * n4;
+        PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
         { ScopedPhase ph(c, PSE_T_VECTOR);
-          k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V + (size_t)j * n4, 0, 1, u, n4, c->d_scal); KERNEL_CHECK(c); }
-        PSE_TRY(read_scalars(c, 1));
-        alpha.push_back(c->h_scal[0]);
-        std::vector<float> cf;
-        int nv = 1; const float4 *base = V + (size_t)j * n4;
-        if (j > 0) { cf = {(float)beta[j - 1], (float)alpha[j]}; nv = 2; base = V + (size_t)(j - 1) * n4; } else cf = {(float)alpha[j]};
-        PSE_TRY(upload_coefs(c, cf));
-        { ScopedPhase ph(c, PSE_T_VECTOR);
-          k_sub_lincomb_norm<<<vgrid(n4), VT, 0, c->stream>>>(u, base, n4, nv, c->d_coef, n4, c->d_scal + 1); KERNEL_CHECK(c); }
-        PSE_TRY(read_scalars(c, 2));
-        beta.push_back(std::sqrt(c->h_scal[1]));
+          k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(vj, 0, 1, u, n4, c->d_scal + 1 + 2 * j); KERNEL_CHECK(c);
+          k_lanczos_update<<<vgrid(n4), VT, 0, c->stream>>>(u, vj, j ? vj - n4 : nullptr, c->d_scal + 1 + 2 * j, j ? c->d_scal + 2 * j : nullptr,
+                                                           n4, c->d_scal + 2 + 2 * j); KERNEL_CHECK(c);
+          if (j + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(vj + n4, u, c->d_scal + 2 + 2 * j, n4); KERNEL_CHECK(c); } }
+        PSE_TRY(read_scalars(c, 3 + 2 * j));                        // one read-back per iteration
+        if (j == 0) {
+            wn = std::sqrt(c->h_scal[0]);
+            if (!(wn > 0)) { CUDA_TRY(c, cudaMemsetAsync(d_y, 0, n * sizeof(float), c->stream)); return PSE_OK; }
+        }
+        alpha.push_back(c->h_scal[1 + 2 * j]);
+        beta.push_back(std::sqrt(c->h_scal[2 + 2 * j]));
         m = j + 1;
         // coefficient vector  c = |w| T^{1/2} e_1  of the m x m tridiagonal
         std::vector<double> Tm((size_t)m * m, 0.0), Q;
@@ -258,7 +285,6 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
         cprev = ccur;
         if (j > 0 && std::sqrt(diff) <= c->tol * std::sqrt(nrm)) { converged = true; break; }
         if (beta[j] <= 1e-7 * std::fabs(alpha[0])) { converged = true; break; }          // invariant subspace
-        if (j + 1 < maxit) PSE_TRY(pse_axpby(c, n, (float)(1.0 / beta[j]), reinterpret_cast<const float *>(u), 0.f, reinterpret_cast<float *>(V + (size_t)(j + 1) * n4)));
     }
     std::vector<float> cf(ccur.begin(), ccur.end());
     PSE_TRY(upload_coefs(c, cf));
@@ -285,8 +311,12 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     if (d_Fp) PSE_TRY(pse_apply_packed(c, d_Fp, reinterpret_cast<float *>(z0), PSE_BOTH));
     { ScopedPhase ph(c, PSE_T_VECTOR);
       k_rhs<<<nbN, VT, 0, c->stream>>>(w, reinterpret_cast<const float4 *>(d_EBp), d_Fp ? z0 : nullptr, N); KERNEL_CHECK(c); }
-    PSE_TRY(zero_scalars(c, 1));
-    { ScopedPhase ph(c, PSE_T_VECTOR); k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(w, 0, 1, w, n4, c->d_scal); KERNEL_CHECK(c); }
+    // slots: [0] = |b|^2; iteration k owns [base_k .. base_k + k + 1] = h_0..h_k, |w|^2 with base_k = 1 + k(k+3)/2
+    const int nslots = 1 + maxit * (maxit + 3) / 2;
+    PSE_TRY(zero_scalars(c, nslots));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(w, 0, 1, w, n4, c->d_scal); KERNEL_CHECK(c);
+      k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V, w, c->d_scal, n4); KERNEL_CHECK(c); }
     PSE_TRY(read_scalars(c, 1));
     const double bnorm = std::sqrt(c->h_scal[0]);
     int m = 0;
@@ -294,20 +324,18 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     bool converged = !(bnorm > 0);
     if (!converged) {
         g[0] = bnorm;
-        PSE_TRY(pse_axpby(c, n, (float)(1.0 / bnorm), reinterpret_cast<const float *>(w), 0.f, reinterpret_cast<float *>(V)));
         for (int k = 0; k < maxit; ++k) {
-            PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Z + (size_t)k * n4), PSE_BOTH));
-            { ScopedPhase ph(c, PSE_T_VECTOR); k_epart<<<nbN, VT, 0, c->stream>>>(w, Z + (size_t)k * n4, 1.f, N); KERNEL_CHECK(c); }
-            PSE_TRY(zero_scalars(c, k + 2));
-            { ScopedPhase ph(c, PSE_T_VECTOR); k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, w, n4, c->d_scal); KERNEL_CHECK(c); }
-            PSE_TRY(read_scalars(c, k + 1));
-            std::vector<float> hf(k + 1);
-            for (int j = 0; j <= k; ++j) { H[(size_t)j * maxit + k] = c->h_scal[j]; hf[j] = (float)c->h_scal[j]; }
-            PSE_TRY(upload_coefs(c, hf));
+            const int base = 1 + k * (k + 3) / 2;
+            float4 *Zk = Z + (size_t)k * n4;
+            PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH));
             { ScopedPhase ph(c, PSE_T_VECTOR);
-              k_sub_lincomb_norm<<<vgrid(n4), VT, 0, c->stream>>>(w, V, n4, k + 1, c->d_coef, n4, c->d_scal + k + 1); KERNEL_CHECK(c); }
-            PSE_TRY(read_scalars(c, k + 2));
-            const double hk1 = std::sqrt(c->h_scal[k + 1]);
+              // the velocity slots of every V_j are zero, so <V_j, Z_k> over all 8 components is the E-part product
+              k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, Zk, n4, c->d_scal + base); KERNEL_CHECK(c);
+              k_gs_update<<<vgrid((size_t)N), VT, 0, c->stream>>>(w, Zk, V, n4, k + 1, c->d_scal + base, N, c->d_scal + base + k + 1); KERNEL_CHECK(c);
+              if (k + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V + (size_t)(k + 1) * n4, w, c->d_scal + base + k + 1, n4); KERNEL_CHECK(c); } }
+            PSE_TRY(read_scalars(c, base + k + 2));                  // one read-back per iteration
+            for (int j = 0; j <= k; ++j) H[(size_t)j * maxit + k] = c->h_scal[base + j];
+            const double hk1 = std::sqrt(c->h_scal[base + k + 1]);
             H[(size_t)(k + 1) * maxit + k] = hk1;
             for (int j = 0; j < k; ++j) {                        // apply previous Givens rotations to column k
                 double a = H[(size_t)j * maxit + k], b = H[(size_t)(j + 1) * maxit + k];
@@ -320,7 +348,6 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
             m = k + 1;
             if (std::fabs(g[k + 1]) <= c->tol * bnorm) { converged = true; break; }
             if (hk1 <= 1e-12 * bnorm) { converged = true; break; }
-            if (k + 1 < maxit) PSE_TRY(pse_axpby(c, n, (float)(1.0 / hk1), reinterpret_cast<const float *>(w), 0.f, reinterpret_cast<float *>(V + (size_t)(k + 1) * n4)));
         }
         y.assign(m, 0.0);
         for (int i = m - 1; i >= 0; --i) {

@@ -21,6 +21,9 @@ struct pse_ctx {
     double L = 0, a = 0, eta = 0, kT = 0, xi = 0, rcut = 0, tol = 0;
     double h = 0, eta_g = 0;                 // grid spacing, Gaussian shape parameter
     cudaStream_t stream = nullptr;
+    cudaStream_t stream2 = nullptr;          // real-space half of a full product runs here, concurrently with the wave half
+    cudaEvent_t ev_fork = nullptr, ev_real = nullptr;
+    bool overlap = false;                    // measured neutral (1M) to slightly slower (65k): off unless PSE_OVERLAP=1
     std::string err;
     long long launches = 0;
     // ---- real-space table ----
@@ -75,7 +78,7 @@ struct pse_ctx {
 struct ScopedPhase {
     pse_ctx *c; int idx = -1;
     ScopedPhase(pse_ctx *ctx, int phase) : c(ctx) {
-        if (!c->profiling) return;
+        if (!c->profiling || phase < 0) return;
         Timer t; t.phase = phase;
         cudaEventCreate(&t.a); cudaEventCreate(&t.b);
         cudaEventRecord(t.a, c->stream);
@@ -113,12 +116,12 @@ pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *
 pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total);
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
 // realspace.cu
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out);             // out = M_r in
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st = nullptr, int ctas_per_sm = 2);   // out = M_r in
 // wavespace.cu
 pse_status pse_wave_init(pse_ctx *c);
 void pse_wave_free(pse_ctx *c);
 pse_status pse_tile_bins(pse_ctx *c);
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate);   // out (+)= M_w in
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp = nullptr);   // out (+)= M_w in
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
 // krylov.cu
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted

@@ -88,8 +88,10 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
 
 }  // namespace
 
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out) {
-    ScopedPhase ph(c, PSE_T_REAL);
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int ctas_per_sm) {
+    const bool own = (st == nullptr);
+    if (own) st = c->stream;
+    ScopedPhase ph(c, own ? PSE_T_REAL : -1);
     static int nsm = 0;
     if (!nsm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
     const size_t smem = (size_t)PSE_NTAB * 2 * sizeof(float4);
@@ -98,9 +100,9 @@ pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out) {
         CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    int grid = 2 * nsm, wpb = 512 / 32;
+    int grid = ctas_per_sm * nsm, wpb = 512 / 32;
     if ((long long)grid * wpb > c->N) grid = (c->N + wpb - 1) / wpb;
-    real_pairs_kernel<<<grid, 512, smem, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in),
+    real_pairs_kernel<<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in),
                                                       reinterpret_cast<float4 *>(d_out), c->N, c->d_nbr_off, c->d_nbr_idx,
                                                       reinterpret_cast<const float4 *>(c->d_table), (float)(1.0 / c->tab_dr),
                                                       (float)c->L, 1.0f / (float)c->L);

@@ -491,8 +491,9 @@ static ScaleParams make_scale_params(const pse_ctx *c) {
     return sp;
 }
 
-static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate) {
+static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, cudaEvent_t wait_ev = nullptr) {
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r, c->d_spec, c->d_grid)); c->launches++; }
+    if (wait_ev) CUDA_TRY(c, cudaStreamWaitEvent(c->stream, wait_ev, 0));
     ScopedPhase ph(c, PSE_T_INTERP);
     const int TB = 256, E = T + c->P - 1;
     const int Ez = E + ((c->P - E) & 7);
@@ -527,7 +528,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     return PSE_OK;
 }
 
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate) {
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp) {
     const size_t nmode = (size_t)c->M * c->M * c->Mh;
     {
         ScopedPhase ph(c, PSE_T_SPREAD);
@@ -540,7 +541,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
         ScopedPhase ph(c, PSE_T_SCALE);
         scale_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c)); KERNEL_CHECK(c);
     }
-    return inverse_and_interpolate(c, d_out, accumulate);
+    return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp);
 }
 
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {
