@@ -261,3 +261,85 @@ def test_large_support_uses_global_interpolation_path():
     Ug, Eg = mob.wave_apply_modes(x32.astype(np.float64), L, A, ETA, k, w, F, S)
     assert rel(outs[0], np.hstack([Ug, Eg])) < 1e-3
     assert rel(outs[1], np.hstack([Ug, Eg])) < 2e-5      # P = 14: quadrature error ~1e-9, what is left is fp32
+
+
+def test_config2_constrained_step_pieces_at_full_size():
+    """BASELINE.json configs[1] (N=4096, phi=0.20, tol=1e-4): Brownian slip, hard-sphere forces and the GMRES
+    stresslet solve at full size; the oracle checks, on sampled rows, that the solution really satisfies
+    Eq. (78): E-rows of M [F;S] + E^B = 0 and U = U^B + U-rows of M [F;S]."""
+    import paper_1709_06946_b200 as pse
+    N, phi, tol, xi, dt = 4096, 0.20, 1e-4, 0.5, 1e-3
+    x, L = synth.rsa(N, phi, seed=2)
+    x32 = (x * 0.995).astype(np.float32)          # slight compression: a few overlapping pairs, so F^P != 0
+    L = L * 0.995
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    w1, w2 = synth.brownian_noise(N, grid, 2)
+    UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    li = ctx.pse_brownian(dt, dev(w1.reshape(N, 8)), dev(w2), UB, EB)
+    F = torch.empty(N, 3, device='cuda')
+    ctx.pse_hard_sphere_forces(dt, F)
+    U, S = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    gi = ctx.pse_constrained_solve(F, UB, EB, U, S)
+    assert 3 <= li <= 30 and 3 <= gi <= 20        # the paper reports 8-10 constraint iterations at 1e-3 (PAPER.md:561)
+    Fh, Sh, UBh, EBh, Uh = (t.cpu().numpy().astype(np.float64) for t in (F, S, UB, EB, U))
+    assert np.abs(Fh).max() > 0
+    rows = np.sort(np.random.default_rng(4).choice(N, 12, replace=False))
+    Uo, Eo = mob.mobility_apply(x32.astype(np.float64), L, A, ETA, xi, Fh, Sh, rows=rows, eps=1e-8)
+    # constraint residual relative to the driving term, and the velocity relation
+    assert np.linalg.norm(Eo + EBh[rows]) / np.linalg.norm(EBh[rows]) < 3 * bar(tol)     # GMRES tol + product tol
+    assert rel(Uh[rows] - UBh[rows], Uo) < 3 * bar(tol)
+
+
+def test_fractal_aggregates_neighbors_and_product():
+    """BASELINE.json configs[4] stand-in at reduced N: clustered particles (very uneven cell and tile occupancy)."""
+    import paper_1709_06946_b200 as pse
+    N, tol, xi = 2048, 1e-3, 0.4
+    x, L = synth.fractal_aggregates(N, 0.05, seed=3)
+    x32 = x.astype(np.float32)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    got, want = nbr_sets_from_gpu(ctx), nbo.neighbor_sets(x32, L, rcut)
+    for g, w in zip(got, want):
+        assert np.array_equal(g, w)
+    counts = np.array([len(w) for w in want])
+    uniform = 0.05 * rcut**3                       # phi r_cut^3 neighbours for a homogeneous suspension (PAPER.md:207)
+    assert counts.mean() > 1.15 * uniform          # aggregates: more neighbours than a uniform suspension at the same phi
+    F, S = synth.gaussian_inputs(N, 9)
+    U, E = gpu_apply(ctx, F, S, 3)
+    rows = np.sort(np.random.default_rng(9).choice(N, 24, replace=False))
+    Uo, Eo = mob.mobility_apply(x32.astype(np.float64), L, A, ETA, xi, F, S, rows=rows, eps=1e-7)
+    assert rel(U[rows], Uo) < bar(tol) and rel(E[rows], Eo) < bar(tol)
+
+
+def test_config3_full_size_properties_and_sampled_rows():
+    """bench.py's workload (N=65536, phi=0.30, tol=1e-3) in its launch configuration.  The O(N^2) oracle cannot
+    finish here, so: (i) the real-space product is checked exactly on sampled rows; (ii) the full product must not
+    depend on the splitting parameter (xi = 0.5 vs 0.6: different r_cut, grid, tables) and must be symmetric."""
+    import paper_1709_06946_b200 as pse
+    N, phi, tol = 65536, 0.30, 1e-3
+    x, L = synth.rsa(N, phi, seed=100)
+    x32 = x.astype(np.float32)
+    F, S = synth.gaussian_inputs(N, 1)
+    F2, S2 = synth.gaussian_inputs(N, 2)
+    res = {}
+    for xi in (0.5, 0.6):
+        st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+        assert st == 0
+        ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+        ctx.pse_neighbors(dev(pos4(x32)))
+        res[xi] = dict(full=np.hstack(gpu_apply(ctx, F, S, 3)), real=np.hstack(gpu_apply(ctx, F, S, 1)), rcut=rcut,
+                       full2=np.hstack(gpu_apply(ctx, F2, S2, 3)))
+        ctx.close()
+    assert rel(res[0.5]['full'], res[0.6]['full']) < bar(tol)
+    v1, v2 = np.hstack([F, S]).astype(np.float64), np.hstack([F2, S2]).astype(np.float64)
+    d12, d21 = float((v1 * res[0.5]['full2']).sum()), float((v2 * res[0.5]['full']).sum())
+    assert abs(d12 - d21) < bar(tol) * np.sqrt(float((v1 * res[0.5]['full']).sum()) * float((v2 * res[0.5]['full2']).sum()))
+    assert float((v1 * res[0.5]['full']).sum()) > 0
+    rows = np.sort(np.random.default_rng(5).choice(N, 8, replace=False))
+    Ur, Er = mob.real_apply(x32.astype(np.float64), L, A, ETA, 0.5, F, S, rows=rows, rcut=res[0.5]['rcut'])
+    assert rel(res[0.5]['real'][rows], np.hstack([Ur, Er])) < 2e-5
