@@ -30,7 +30,7 @@ class PSEError(RuntimeError):
 
 def load_library():
     if not os.path.exists(LIB_PATH):
-        raise ImportError(f'{LIB_PATH} not found: build it with `python -m paper_1709_06946_b200.build` '
+        raise ImportError(f'{LIB_PATH} not found: build it with `python paper_1709_06946_b200/build.py` '
                           '(there is no CPU fallback)')
     lib = C.CDLL(LIB_PATH)
     vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
