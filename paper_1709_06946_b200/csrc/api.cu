@@ -64,12 +64,18 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
     // extra factor k, so the bare estimate leaves their truncation error at ~tol), then the cheapest measured cuFFT size >= that (2,3,5,7-smooth below 64)
     int M = std::max(8, (int)std::ceil(1.07 * 2.0 * xi * s * L / M_PI));
     if (M > 64) M = choose_grid(M); else while (!smooth7(M)) ++M;
-    // C3: quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1): e^{-pi P/2} + erfc(sqrt(pi P/2))
-    // gives P = 5 at 1e-3 as in Table I.  Measured against the oracle, the relative L2 error of the
-    // strain-rate rows is ~10-20x that bound (deconvolution amplifies the high-k quadrature error), so the bound is
-    // required to be <= tol/10: P = 5, 6, 8 at tol = 1e-2, 1e-3, 1e-4 (R6).
+    // C3: support size.  Default window = exponential of semicircle with beta = 2.2 P: measured against
+    // the oracle it reaches the tolerance with P = 3, 4, 5 points at tol = 1e-2, 1e-3, 1e-4, i.e. P = ceil(-log10 tol) + 1.
+    // PSE_WINDOW=gauss selects the paper's Gaussian: its quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1,
+    // PAPER.md:308, 334), e^{-pi P/2} + erfc(sqrt(pi P/2)), gives P = 5 at 1e-3 as in Table I, but the
+    // measured relative L2 error of the strain-rate rows is 10-20x that bound, so it is required to be <= tol/10:
+    // P = 5, 6, 8 (R6).
     int p = 2;
-    while (p < PSE_MAXP && 10.0 * (std::exp(-M_PI * p / 2.0) + std::erfc(std::sqrt(M_PI * p / 2.0))) > tol) ++p;
+    if (pse_window_kind_from_env() == 0) {
+        while (p < PSE_MAXP && 10.0 * (std::exp(-M_PI * p / 2.0) + std::erfc(std::sqrt(M_PI * p / 2.0))) > tol) ++p;
+    } else {
+        p = std::min(PSE_MAXP, std::max(3, (int)std::ceil(-std::log10(tol) - 1e-9) + 1));
+    }
     if (grid) *grid = M;
     if (P) *P = p;
     if (rcut) *rcut = rc;
@@ -93,8 +99,14 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     if (P > grid || P > PSE_MAXP) { c->err = "pse_create: P > grid or P > 16"; return PSE_EINVAL; }
     c->N = N; c->L = L; c->a = a; c->eta = eta; c->kT = kT; c->xi = xi; c->M = grid; c->P = P; c->rcut = rcut; c->tol = tol;
     c->h = L / grid;
-    c->eta_g = (c->h * P * xi) * (c->h * P * xi) / (M_PI * P);         // (h P xi/m)^2, m^2 = pi P
-    if (!(c->eta_g < 1.0)) { c->err = "pse_create: Gaussian shape parameter eta_g >= 1 (grid too coarse for this xi and P)"; return PSE_EINVAL; }
+    c->win_kind = pse_window_kind_from_env();
+    if (c->win_kind == 0) {
+        c->eta_g = (c->h * P * xi) * (c->h * P * xi) / (M_PI * P);     // (h P xi/m)^2, m^2 = pi P
+        if (!(c->eta_g < 1.0)) { c->err = "pse_create: Gaussian shape parameter eta_g >= 1 (grid too coarse for this xi and P)"; return PSE_EINVAL; }
+        c->win_a = 2.0 * M_PI / P; c->win_b = 0.0;
+    } else {
+        c->win_a = 4.0 / ((double)P * P); c->win_b = pse_es_beta_from_env(P);
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { c->err = "no CUDA device (libpse has no CPU fallback)"; return PSE_ECUDA; }
     // real-space table
@@ -125,6 +137,12 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
+    {
+        std::vector<float> dec;
+        pse_window_table(c->win_kind, P, c->win_a, c->win_b, grid, dec);
+        CUDA_TRY(c, cudaMalloc(&c->d_dec, dec.size() * sizeof(float)));
+        CUDA_TRY(c, cudaMemcpy(c->d_dec, dec.data(), dec.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
     CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_real, cudaEventDisableTiming));
@@ -144,7 +162,7 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_fill); cudaFree(c->d_nbr_count);
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
-    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp);
+    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec);
     cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;

@@ -20,6 +20,9 @@ struct pse_ctx {
     int N = 0, M = 0, P = 0;
     double L = 0, a = 0, eta = 0, kT = 0, xi = 0, rcut = 0, tol = 0;
     double h = 0, eta_g = 0;                 // grid spacing, Gaussian shape parameter
+    int win_kind = 1;                        // 0 = Gaussian (paper), 1 = exponential-of-semicircle window
+    double win_a = 0, win_b = 0;             // window parameters handed to the kernels (see win_arg in wavespace.cu)
+    float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index
     cudaStream_t stream = nullptr;
     cudaStream_t stream2 = nullptr;          // real-space half of a full product runs here, concurrently with the wave half
     cudaEvent_t ev_fork = nullptr, ev_real = nullptr;
@@ -108,6 +111,9 @@ __device__ __forceinline__ float warp_reduce8(const float (&a)[8], int lane, int
 
 // tables.cu
 void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr);
+void pse_window_table(int kind, int P, double wa, double wb, int M, std::vector<float> &dec);
+int pse_window_kind_from_env();
+double pse_es_beta_from_env(int P);
 // neighbors.cu
 pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);
 pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n);   // exclusive, n+1 outputs

@@ -7,7 +7,9 @@
 // functions and done by panelled Gauss-Legendre quadrature (Appendix A of the paper is garbled in
 // the extraction and is not used).  The table stores the combinations the pair kernel needs, already multiplied
 // by 1/(6 pi eta a):  (F1, F2, G1+G2, G1+4G2, A, B, D, 0)  at r_i = i * dr, i = 0..ntab-1, dr = rcut/(ntab-2).
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <vector>
 #include "pse_internal.h"
 
@@ -107,4 +109,41 @@ void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std
         t[6] = (float)(unit * (-R[6]));              t[7] = 0.f;
     }
     *dr_out = dr;
+}
+
+// ---- spreading / interpolation window and its transform ----
+// kappa(k_n) = int_{-P/2}^{P/2} w(t) cos(2 pi n t / M) dt  (t in grid units) is the continuous transform of the 1-D
+// window that the P-point sums approximate; the scale kernel multiplies by 1/kappa per dimension, once for spreading
+// and once for interpolation (R4).  dec[i] = 1/kappa for FFT index i (signed wave number n = i or i - M).
+void pse_window_table(int kind, int P, double wa, double wb, int M, std::vector<float> &dec) {
+    std::vector<double> gx, gw;
+    gauss_legendre(32, gx, gw);
+    const int npanel = 4 * P;                              // panels of width 1/4 grid spacing, 32 nodes each
+    dec.assign(M, 0.f);
+    for (int i = 0; i < M; ++i) {
+        const int n = i < (M + 1) / 2 ? i : i - M;
+        const double kh = 2.0 * M_PI * n / M;
+        double kap = 0;
+        for (int p = 0; p < npanel; ++p) {
+            const double lo = -0.5 * P + (double)P * p / npanel, hi = -0.5 * P + (double)P * (p + 1) / npanel;
+            for (int q = 0; q < 32; ++q) {
+                const double t = 0.5 * (lo + hi) + 0.5 * (hi - lo) * gx[q];
+                const double arg = kind ? wb * (std::sqrt(std::max(1.0 - wa * t * t, 0.0)) - 1.0) : -wa * t * t;
+                kap += 0.5 * (hi - lo) * gw[q] * std::exp(arg) * std::cos(kh * t);
+            }
+        }
+        dec[i] = (float)(1.0 / kap);
+    }
+}
+
+int pse_window_kind_from_env() {
+    const char *e = getenv("PSE_WINDOW");
+    return (e && (e[0] == 'g' || e[0] == 'G')) ? 0 : 1;
+}
+
+// shape parameter of the exponential-of-semicircle window; PSE_ES_BETA (a multiple of P) overrides the default
+double pse_es_beta_from_env(int P) {
+    const char *e = getenv("PSE_ES_BETA");
+    const double per_point = e ? atof(e) : 2.2;
+    return per_point * P;
 }

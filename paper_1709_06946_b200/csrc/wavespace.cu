@@ -26,6 +26,14 @@ __device__ __forceinline__ int support_base(float g, int P) {
 }
 __device__ __forceinline__ int pmod(int i, int M) { int r = i % M; return r < 0 ? r + M : r; }
 
+// Exponent of the 1-D window at offset tt (grid units) from the particle.  wb == 0: the paper's Gaussian,
+// exp(-wa tt^2) with wa = 2 pi / P.  wb > 0: "exponential of semicircle" window
+// exp(wb (sqrt(1 - z^2) - 1)), z = 2 tt / P, wa = 4 / P^2 — same support, much faster decay in k, so a given
+// tolerance needs fewer points per dimension.  The branch is uniform across the grid.
+__device__ __forceinline__ float win_arg(float tt, float wa, float wb) {
+    return wb > 0.f ? wb * (sqrtf(fmaxf(1.f - wa * tt * tt, 0.f)) - 1.f) : -wa * tt * tt;
+}
+
 __global__ void tile_of_particles(const float4 *pos, int N, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
@@ -75,7 +83,7 @@ __device__ __forceinline__ int wrap_offset(int gp, int base, int M) {
 // (fixed summation order, no atomics).
 __global__ void __launch_bounds__(SPREAD_THREADS)
 spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, const int *__restrict__ tile_start,
-              const int *__restrict__ tile_list, float *__restrict__ grid, int M, int P, int nt, float inv_h, float wexp) {
+              const int *__restrict__ tile_list, float *__restrict__ grid, int M, int P, int nt, float inv_h, float wa, float wb) {
     __shared__ float4 q[SPREAD_BATCH][2];
     __shared__ __align__(16) float W[SPREAD_BATCH][3][T];
     __shared__ unsigned short lst[4][SPREAD_BATCH];
@@ -135,7 +143,7 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
                     const int gp = g0[d] + i, o = wrap_offset(gp, base, M);
                     const float tt = (float)(base + o) - g[d];
                     const bool inside = (o < P && gp < M);
-                    W[tid][d][d == 1 ? ((i & 1) * 4 + (i >> 1)) : i] = inside ? __expf(-wexp * tt * tt) : 0.f;
+                    W[tid][d][d == 1 ? ((i & 1) * 4 + (i >> 1)) : i] = inside ? __expf(win_arg(tt, wa, wb)) : 0.f;
                     msk[d] |= inside ? (1u << i) : 0u;
                 }
             }
@@ -193,7 +201,7 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
 // Interpolation (a7): warp per particle (visited in tile order for L1/L2 locality), lanes over the P^3 support.
 __global__ void __launch_bounds__(256)
 interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list, const float *__restrict__ grid,
-              float4 *__restrict__ out, int N, int M, int P, float inv_h, float wexp, int accumulate) {
+              float4 *__restrict__ out, int N, int M, int P, float inv_h, float wa, float wb, int accumulate) {
     const int wi = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (wi >= N) return;
     const int s = tile_list[wi];
@@ -205,7 +213,7 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
     for (int h = 0; h < 2; ++h) {                       // entry e = d*P + i, e < 3P <= 48
         int e = lane + 32 * h, d = e / P, i = e % P;
         float tt = (d < 3) ? (float)(base[d] + i) - g[d] : 0.f;
-        wr[h] = (d < 3) ? __expf(-wexp * tt * tt) : 0.f;
+        wr[h] = (d < 3) ? __expf(win_arg(tt, wa, wb)) : 0.f;
     }
     const size_t M3 = (size_t)M * M * M;
     float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -245,7 +253,7 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
 template <int PT>                                  // PT > 0: support size known at compile time (no integer divisions)
 __global__ void __launch_bounds__(256)
 interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_start, const int *__restrict__ tile_list,
-                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int Prt, int nt, float inv_h, float wexp,
+                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int Prt, int nt, float inv_h, float wa, float wb,
                    int accumulate) {
     extern __shared__ float4 sm[];
     const int P = PT ? PT : Prt;
@@ -286,23 +294,30 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
         const int b0 = support_base(gx, P), b1 = support_base(gy, P), b2 = support_base(gz, P);
         const int r0 = pmod(b0, M) - t0 * T, r1 = pmod(b1, M) - t1 * T, r2 = pmod(b2, M) - t2 * T;
         const float tx = (float)(b0 + lane) - gx;
-        const float wxr = lane < P ? __expf(-wexp * tx * tx) : 0.f;
+        const float wxr = lane < P ? __expf(win_arg(tx, wa, wb)) : 0.f;
         float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        // lanes <-> (g, j, k): when P^2 <= 16 the warp holds nI = 32 / P^2 copies of the (j,k) face and copy g walks
+        // x = g, g + nI, ...; otherwise one copy, and faces larger than 32 columns take several passes.
+        const int nI = P2 <= 16 ? 32 / P2 : 1;
         for (int jk0 = 0; jk0 < P2; jk0 += 32) {
-            const int jk = jk0 + lane;
-            const bool ok = jk < P2;
+            const int g = nI > 1 ? lane / P2 : 0, jk = nI > 1 ? lane - g * P2 : jk0 + lane;
+            const bool ok = jk < P2 && g < nI;
             const int j = ok ? jk / P : 0, k = ok ? jk % P : 0;
             const float ty = (float)(b1 + j) - gy, tz = (float)(b2 + k) - gz;
-            const float wyz = ok ? __expf(-wexp * (ty * ty + tz * tz)) : 0.f;
-            int sidx = (r0 * E + r1 + j) * Ez + r2 + k;
+            const float wyz = ok ? __expf(win_arg(ty, wa, wb) + win_arg(tz, wa, wb)) : 0.f;
+            int sidx = ((r0 + (ok ? g : 0)) * E + r1 + j) * Ez + r2 + k;
             float tsum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #pragma unroll
-            for (int i = 0; i < (PT ? PT : PSE_MAXP); ++i, sidx += EE) {
-                if (!PT && i >= P) break;
-                const float wx = __shfl_sync(0xffffffffu, wxr, i);
-                const float4 v0 = lo[sidx], v1 = hi[sidx];
-                tsum[0] += wx * v0.x; tsum[1] += wx * v0.y; tsum[2] += wx * v0.z; tsum[3] += wx * v0.w;
-                tsum[4] += wx * v1.x; tsum[5] += wx * v1.y; tsum[6] += wx * v1.z; tsum[7] += wx * v1.w;
+            for (int i0 = 0; i0 < (PT ? PT : PSE_MAXP); ++i0) {
+                const int i = i0 * nI + g;                          // uniform trip count: every lane runs ceil(P / nI) rounds
+                if (i0 * nI >= P) break;
+                const float wx = __shfl_sync(0xffffffffu, wxr, i < P ? i : 0);
+                if (i < P) {
+                    const float4 v0 = lo[sidx], v1 = hi[sidx];
+                    tsum[0] += wx * v0.x; tsum[1] += wx * v0.y; tsum[2] += wx * v0.z; tsum[3] += wx * v0.w;
+                    tsum[4] += wx * v1.x; tsum[5] += wx * v1.y; tsum[6] += wx * v1.z; tsum[7] += wx * v1.w;
+                }
+                sidx += nI * EE;
             }
 #pragma unroll
             for (int c = 0; c < 8; ++c) acc[c] += wyz * tsum[c];
@@ -318,7 +333,8 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
 
 struct ScaleParams {
     int M, Mh;
-    float two_pi_over_L, a, inv4xi2, one_minus_etag, c_mv, c_br, inv_eta;
+    float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
+    const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
 };
 
 __device__ __forceinline__ float shape_s1(float x) {     // 3 (sin x - x cos x)/x^3, series below 0.5 (cancellation)
@@ -373,7 +389,8 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
     const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
     const float q = k2 * sp.inv4xi2;
-    const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-sp.one_minus_etag * q) / k2;
+    const float dw = __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);            // one window undone for spreading,
+    const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-q) / k2 * dw * dw;          // one for interpolation
     float2 F[3], S[5];
 #pragma unroll
     for (int c = 0; c < 3; ++c) F[c] = spec[c * nmode + o];
@@ -427,7 +444,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
     const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
     const float q = k2 * sp.inv4xi2;
-    const float Bh = sp.c_br * sqrtf(sp.inv_eta * (1.f + q) / k2) * __expf(-0.5f * sp.one_minus_etag * q);
+    const float Bh = sp.c_br * sqrtf(sp.inv_eta * (1.f + q) / k2) * __expf(-0.5f * q) * __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);
     const float ik2 = 1.f / k2;
     const float2 kw = make_float2((kx * W[0].x + ky * W[1].x + kz * W[2].x) * ik2, (kx * W[0].y + ky * W[1].y + kz * W[2].y) * ik2);
     const float2 ux = make_float2(Bh * (W[0].x - kx * kw.x), Bh * (W[0].y - kx * kw.y));
@@ -484,9 +501,9 @@ static ScaleParams make_scale_params(const pse_ctx *c) {
     ScaleParams sp;
     sp.M = c->M; sp.Mh = c->Mh;
     sp.two_pi_over_L = (float)(2.0 * M_PI / c->L); sp.a = (float)c->a;
-    sp.inv4xi2 = (float)(1.0 / (4.0 * c->xi * c->xi)); sp.one_minus_etag = (float)(1.0 - c->eta_g);
-    const double V = c->L * c->L * c->L, tp = 2.0 / c->P;
-    sp.c_mv = (float)(tp * tp * tp / V); sp.c_br = (float)(std::sqrt(tp * tp * tp / V));
+    sp.inv4xi2 = (float)(1.0 / (4.0 * c->xi * c->xi)); sp.dec = c->d_dec;
+    const double V = c->L * c->L * c->L;
+    sp.c_mv = (float)(1.0 / V); sp.c_br = (float)(1.0 / std::sqrt(V));
     sp.inv_eta = (float)(1.0 / c->eta);
     return sp;
 }
@@ -507,10 +524,11 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
             smem_set = smem;                                                                                               \
         }                                                                                                                  \
         interp_tile_kernel<PT><<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid,       \
-            reinterpret_cast<float4 *>(d_out), c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P),          \
+            reinterpret_cast<float4 *>(d_out), c->M, c->P, c->nt, (float)(1.0 / c->h), (float)c->win_a, (float)c->win_b, \
             accumulate ? 1 : 0);                                                                                           \
     } while (0)
         switch (c->P) {
+            case 3: PSE_LAUNCH_INTERP(3); break;
             case 4: PSE_LAUNCH_INTERP(4); break;
             case 5: PSE_LAUNCH_INTERP(5); break;
             case 6: PSE_LAUNCH_INTERP(6); break;
@@ -522,7 +540,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     } else {
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
-            (float)(2.0 * M_PI / c->P), accumulate ? 1 : 0);
+            (float)c->win_a, (float)c->win_b, accumulate ? 1 : 0);
     }
     KERNEL_CHECK(c);
     return PSE_OK;
@@ -533,7 +551,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     {
         ScopedPhase ph(c, PSE_T_SPREAD);
         spread_kernel<<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
-                                                       c->d_grid, c->M, c->P, c->nt, (float)(1.0 / c->h), (float)(2.0 * M_PI / c->P));
+                                                       c->d_grid, c->M, c->P, c->nt, (float)(1.0 / c->h), (float)c->win_a, (float)c->win_b);
         KERNEL_CHECK(c);
     }
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c, c->d_grid, c->d_spec)); c->launches++; }

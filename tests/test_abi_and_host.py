@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol(pse):
 
 def test_suggest_params_rules(pse):
     st, grid, P, rcut = pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.6)
-    assert st == 0 and P == 6                       # Table I gives 5 at 1e-3; bound tightened 10x (R6)
+    assert st == 0 and P == 4                       # exponential-of-semicircle window: P = ceil(-log10 tol) + 1
     assert abs(rcut - (np.sqrt(-np.log(1e-3)) / 0.6 + 1.0)) < 1e-12 and rcut <= 13.892 / 2
     n = grid
     for p in (2, 3, 5, 7):
@@ -43,7 +43,7 @@ def test_suggest_params_rules(pse):
     # above 64 the cheapest measured cuFFT size is taken (profiles/r1_cufft_sizes.md): 90 -> 90, 320 -> 343, 97 -> 100
     assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.5)[1] == 90
     assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.55)[1] == 100
-    for tol, want in [(1e-2, 5), (1e-3, 6), (1e-4, 8)]:
+    for tol, want in [(1e-2, 3), (1e-3, 4), (1e-4, 5)]:
         assert pse.pse_suggest_params(4096, 44.1, 1.0, tol, 0.5)[2] == want
     assert pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.3)[0] == pse.PSE_EINVAL      # rcut > L/2
     assert pse.pse_suggest_params(0, 13.892, 1.0, 1e-3, 0.6)[0] == pse.PSE_EINVAL
@@ -52,7 +52,7 @@ def test_suggest_params_rules(pse):
 def test_create_validates_arguments_and_fails_loudly_without_gpu(pse):
     import torch
     eta = 1 / (6 * np.pi)
-    bad = [dict(rcut=8.0), dict(rcut=1.5), dict(P=40), dict(grid=4), dict(N=0), dict(xi=3.0, grid=8, P=8)]
+    bad = [dict(rcut=8.0), dict(rcut=1.5), dict(P=40), dict(grid=4), dict(N=0)]
     base = dict(N=64, L=13.892, a=1.0, eta=eta, kT=1.0, xi=0.6, grid=32, P=8, rcut=5.3, tol=1e-3)
     for b in bad:
         with pytest.raises(pse.PSEError) as e:
