@@ -112,17 +112,29 @@ def choose_params(wl, L):
     return grid, P, rcut
 
 
-def algorithmic_bytes(N, M, nb_mean):
-    """Per-launch algorithmic bytes of each phase: fp32, G = M^3 grid points."""
+def planes_per_launch(g):
+    """Mean number of grids (planes) each wave-space kernel touches per launch inside one pse_step with g GMRES
+    iterations (the products carry only the components they need): M_EF F (3 in, 5 out), g x M_ES v
+    (5 in, 5 out), the final [F;S] -> U product (8 in, 3 out) and the Brownian half pass (3 noise planes in, 8 out)."""
+    fwd = (3 + 5 * g + 8) / (g + 2)
+    inv = (5 + 5 * g + 3 + 8) / (g + 3)
+    scale = ((3 + 5) + 10 * g + (8 + 3) + (3 + 8)) / (g + 3)
+    return {'spread': fwd, 'fft_fwd': fwd, 'scale': scale, 'fft_inv': inv, 'interp': inv}
+
+
+def algorithmic_bytes(N, M, nb_mean, g=None):
+    """Per-launch algorithmic bytes of each phase: fp32, G = M^3 grid points.
+    g = None: a full product (8 grids in, 8 out); else the launch mix of a step with g GMRES iterations."""
     G, Gh = float(M) ** 3, float(M) * M * (M // 2 + 1)
+    pl = planes_per_launch(g) if g is not None else {'spread': 8, 'fft_fwd': 8, 'scale': 16, 'fft_inv': 8, 'interp': 8}
     return {
         'neighbors': 16 * N + 8 * N + 2 * 4 * N * nb_mean,      # positions, sort keys/permutation, list written (count + fill pass reads excluded)
         'real': 16 * N + 32 * N + 32 * N + 4 * N * nb_mean,     # compulsory DRAM: pos, in, out, neighbour indices
-        'spread': 48 * N + 32 * G,                              # particles read, 8 grids written once
-        'fft_fwd': 32 * G + 64 * Gh,                            # one-pass lower bound: 8 real grids in, 8 half spectra out
-        'scale': 2 * 64 * Gh,                                   # 8 complex in, 8 complex out per half-spectrum mode
-        'fft_inv': 64 * Gh + 32 * G,
-        'interp': 32 * G + 48 * N,                              # 8 grids read once, particles read/written
+        'spread': 16 * N + pl['spread'] * (4 * N + 4 * G),      # particles read, each grid written once
+        'fft_fwd': pl['fft_fwd'] * (4 * G + 8 * Gh),            # one-pass lower bound: real grid in, half spectrum out
+        'scale': pl['scale'] * 8 * Gh,                          # one complex per half-spectrum mode per plane read or written
+        'fft_inv': pl['fft_inv'] * (8 * Gh + 4 * G),
+        'interp': 16 * N + pl['interp'] * (4 * G + 4 * N),      # each grid read once, particles read/written
     }
 
 
@@ -308,7 +320,7 @@ def main():
     ms_step = r['ms'] / K
     value = replica_throughput(K, world, r['ms'])                     # replicas: all ranks' steps / max-over-ranks time
     peak, peak_src = peaks()
-    ab = algorithmic_bytes(wl['N'], r['grid'], r['nb_mean'])
+    ab = algorithmic_bytes(wl['N'], r['grid'], r['nb_mean'], r['gmres'])
     phases = {}
     for name, (ms, n) in r['phases'].items():
         if n == 0:

@@ -5,7 +5,7 @@
 #include <new>
 #include "pse_internal.h"
 
-pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which);
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode = PSE_MODE_ALL);
 
 namespace {
 
@@ -182,8 +182,10 @@ pse_status pse_get_neighbors(pse_ctx *c, int *d_count, int *d_index, size_t cap,
 pse_status pse_mobility_apply(pse_ctx *c, const float *d_F, const float *d_S, float *d_U, float *d_E, int which) {
     if (!c || !(which & PSE_BOTH) || (!d_F && !d_S)) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_mobility_apply before pse_neighbors"; return PSE_ENOTREADY; }
+    if (!d_U && !d_E) return PSE_EINVAL;
+    const int mode = (d_F ? PSE_IN_F : 0) | (d_S ? PSE_IN_S : 0) | (d_U ? PSE_OUT_U : 0) | (d_E ? PSE_OUT_E : 0);
     PSE_TRY(pse_pack(c, d_F, d_S, c->d_in));
-    PSE_TRY(pse_apply_packed(c, c->d_in, c->d_out, which));
+    PSE_TRY(pse_apply_packed(c, c->d_in, c->d_out, which, mode));
     return pse_unpack(c, c->d_out, 1.f, d_U, d_E);
 }
 
@@ -310,18 +312,22 @@ pse_status pse_get_table(pse_ctx *c, float *h_table, int cap_nodes, int *n_nodes
 
 }  // extern "C"
 
-pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which) {
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode) {
     if (which == PSE_BOTH && c->overlap && !c->profiling && c->stream2) {
         // the two halves of the Ewald sum are independent: the pair kernel (one CTA per SM, so that it leaves half of
         // every SM's registers free) runs on a second stream while spread / FFT / scale / FFT run on the main one;
         // the interpolation, which accumulates into the same output, waits for it.
         CUDA_TRY(c, cudaEventRecord(c->ev_fork, c->stream));
         CUDA_TRY(c, cudaStreamWaitEvent(c->stream2, c->ev_fork, 0));
-        PSE_TRY(pse_real_apply(c, d_in, d_out, c->stream2, 1));
+        PSE_TRY(pse_real_apply(c, d_in, d_out, c->stream2, 1, mode));
         CUDA_TRY(c, cudaEventRecord(c->ev_real, c->stream2));
-        return pse_wave_apply(c, d_in, d_out, true, c->ev_real);
+        return pse_wave_apply(c, d_in, d_out, true, c->ev_real, mode);
     }
-    if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out));
-    if (which & PSE_WAVE) PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0));
+    if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out, nullptr, 2, mode));
+    if (which & PSE_WAVE) {
+        // wave-only products start from zero: the interpolation of a masked product writes only the requested planes
+        if (!(which & PSE_REAL) && mode != PSE_MODE_ALL) CUDA_TRY(c, cudaMemsetAsync(d_out, 0, (size_t)c->N * 8 * sizeof(float), c->stream));
+        PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0, nullptr, mode));
+    }
     return PSE_OK;
 }

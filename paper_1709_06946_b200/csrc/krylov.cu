@@ -100,22 +100,15 @@ __global__ void __launch_bounds__(VT) k_rhs(float4 *dst, const float4 *EBp, cons
     dst[2 * s + 1] = make_float4(-b.x, -b.y, -b.z, -b.w);
 }
 
-// out = ( UB + U(z0) + sum_j y_j U(Z_j) ; sum_j y_j V_j )
-__global__ void __launch_bounds__(VT) k_constraint_result(float4 *out, const float4 *UBp, const float4 *z0, const float4 *Z, const float4 *V,
-                                                          size_t stride4, int nvec, const float *y, int N) {
+// out = ( U^B + U-rows of Zfin ; S-rows of fin )
+__global__ void __launch_bounds__(VT) k_constraint_result(float4 *out, const float4 *UBp, const float4 *Zfin, const float4 *fin, int N) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
     float ux = 0, uy = 0, uz = 0;
-    float4 sa = make_float4(0, 0, 0, 0), sb = sa;
-    if (UBp) { float4 a = UBp[2 * s]; ux = a.x; uy = a.y; uz = a.z; }
-    if (z0) { float4 a = z0[2 * s]; ux += a.x; uy += a.y; uz += a.z; }
-    for (int j = 0; j < nvec; ++j) {
-        float yj = y[j];
-        float4 z = Z[(size_t)j * stride4 + 2 * s], va = V[(size_t)j * stride4 + 2 * s], vb = V[(size_t)j * stride4 + 2 * s + 1];
-        ux += yj * z.x; uy += yj * z.y; uz += yj * z.z;
-        sa.w += yj * va.w; sb.x += yj * vb.x; sb.y += yj * vb.y; sb.z += yj * vb.z; sb.w += yj * vb.w;
-    }
-    out[2 * s] = make_float4(ux, uy, uz, sa.w); out[2 * s + 1] = sb;
+    if (UBp) { const float4 a = UBp[2 * s]; ux = a.x; uy = a.y; uz = a.z; }
+    if (Zfin) { const float4 a = Zfin[2 * s]; ux += a.x; uy += a.y; uz += a.z; }
+    const float4 fa = fin[2 * s], fb = fin[2 * s + 1];
+    out[2 * s] = make_float4(ux, uy, uz, fa.w); out[2 * s + 1] = fb;
 }
 
 // ---- device-resident scalars: the update kernels read alpha / beta / h straight from the slots the dot kernels
@@ -296,7 +289,7 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
 }
 
 // Forward declaration of the full product on packed vectors (api.cu)
-pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which);
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode = PSE_MODE_ALL);
 
 // GMRES on  M_ES S = -(E^B + M_EF F)  with S and E embedded in packed vectors whose velocity slots are zero.
 // Z_j = M [0; v_j] is kept whole: its E-part feeds Arnoldi, its U-part gives M_US S at the end without another
@@ -308,7 +301,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     float4 *w = reinterpret_cast<float4 *>(c->d_tmp), *z0 = reinterpret_cast<float4 *>(c->d_tmp2);
     const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap - 1), nbN = (N + VT - 1) / VT;
     if (iters) *iters = 0;
-    if (d_Fp) PSE_TRY(pse_apply_packed(c, d_Fp, reinterpret_cast<float *>(z0), PSE_BOTH));
+    if (d_Fp) PSE_TRY(pse_apply_packed(c, d_Fp, reinterpret_cast<float *>(z0), PSE_BOTH, PSE_IN_F | PSE_OUT_E));     // M_EF F
     { ScopedPhase ph(c, PSE_T_VECTOR);
       k_rhs<<<nbN, VT, 0, c->stream>>>(w, reinterpret_cast<const float4 *>(d_EBp), d_Fp ? z0 : nullptr, N); KERNEL_CHECK(c); }
     // slots: [0] = |b|^2; iteration k owns [base_k .. base_k + k + 1] = h_0..h_k, |w|^2 with base_k = 1 + k(k+3)/2
@@ -327,7 +320,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
         for (int k = 0; k < maxit; ++k) {
             const int base = 1 + k * (k + 3) / 2;
             float4 *Zk = Z + (size_t)k * n4;
-            PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH));
+            PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH, PSE_IN_S | PSE_OUT_E));   // M_ES v_k: 5 grids in, 5 out
             { ScopedPhase ph(c, PSE_T_VECTOR);
               // the velocity slots of every V_j are zero, so <V_j, Z_k> over all 8 components is the E-part product
               k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, Zk, n4, c->d_scal + base); KERNEL_CHECK(c);
@@ -356,11 +349,18 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
             y[i] = s / H[(size_t)i * maxit + i];
         }
     }
+    // S = sum_j y_j v_j;  U = U^B + U-rows of M [F; S]: one last product with 3 output grids (the Arnoldi products
+    // carried only the E rows)
     std::vector<float> yf(y.begin(), y.end());
     if (m) PSE_TRY(upload_coefs(c, yf));
+    float4 *fin = w;                                               // [F; S] packed, reuses the Arnoldi work vector
     { ScopedPhase ph(c, PSE_T_VECTOR);
-      k_constraint_result<<<nbN, VT, 0, c->stream>>>(reinterpret_cast<float4 *>(d_outp), reinterpret_cast<const float4 *>(d_UBp), d_Fp ? z0 : nullptr,
-                                                     Z, V, n4, m, c->d_coef, N); KERNEL_CHECK(c); }
+      k_lincomb<<<vgrid(n4), VT, 0, c->stream>>>(fin, reinterpret_cast<const float4 *>(d_Fp), 1.f, V, n4, m, c->d_coef, n4); KERNEL_CHECK(c); }
+    const int fmode = (d_Fp ? PSE_IN_F : 0) | (m ? PSE_IN_S : 0) | PSE_OUT_U;
+    if (fmode & (PSE_IN_F | PSE_IN_S)) PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(fin), reinterpret_cast<float *>(Z), PSE_BOTH, fmode));
+    { ScopedPhase ph(c, PSE_T_VECTOR);
+      k_constraint_result<<<nbN, VT, 0, c->stream>>>(reinterpret_cast<float4 *>(d_outp), reinterpret_cast<const float4 *>(d_UBp),
+                                                     (fmode & (PSE_IN_F | PSE_IN_S)) ? Z : nullptr, fin, N); KERNEL_CHECK(c); }
     if (iters) *iters = m;
     if (!converged) { c->err = "GMRES did not converge"; return PSE_ENOCONV; }
     return PSE_OK;

@@ -13,6 +13,10 @@
 #define PSE_MAXP 16
 #define PSE_MAX_KRYLOV 50
 
+// which components a product carries: inputs F (3) and/or S (5), outputs U (3) and/or E (5).  Inside GMRES the operator
+// is S -> E only, so 5 + 5 grids are spread / transformed / interpolated instead of 8 + 8.
+enum { PSE_IN_F = 1, PSE_IN_S = 2, PSE_OUT_U = 4, PSE_OUT_E = 8, PSE_MODE_ALL = 15 };
+
 struct Timer { cudaEvent_t a, b; int phase; };
 
 struct pse_ctx {
@@ -51,7 +55,8 @@ struct pse_ctx {
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]
     cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
-    cufftHandle plan_r2c = 0, plan_c2r = 0; void *d_fft_work = nullptr; bool have_plans = false;
+    cufftHandle plan_r2c[3] = {0, 0, 0}, plan_c2r[3] = {0, 0, 0};   // [0] all 8 grids, [1] planes 0-2 (F / U), [2] planes 3-7 (S / E)
+    void *d_fft_work = nullptr; int nplans = 0;
     // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
     float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
     float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]
@@ -122,12 +127,12 @@ pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *
 pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total);
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
 // realspace.cu
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st = nullptr, int ctas_per_sm = 2);   // out = M_r in
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st = nullptr, int ctas_per_sm = 2, int mode = PSE_MODE_ALL);   // out = M_r in
 // wavespace.cu
 pse_status pse_wave_init(pse_ctx *c);
 void pse_wave_free(pse_ctx *c);
 pse_status pse_tile_bins(pse_ctx *c);
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp = nullptr);   // out (+)= M_w in
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp = nullptr, int mode = PSE_MODE_ALL);   // out (+)= M_w in
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
 // krylov.cu
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted

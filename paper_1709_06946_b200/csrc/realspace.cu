@@ -17,6 +17,9 @@ namespace {
 constexpr float RS2 = 0.70710678118654752f;   // 1/sqrt2
 constexpr float RS6 = 0.40824829046386302f;   // 1/sqrt6
 
+// MODE = PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: terms of absent inputs / outputs are removed at compile time
+// (inside GMRES the operator is S -> E: no U accumulation, no F terms, and only the E-part table is read).
+template <int MODE>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
                   const unsigned long long *__restrict__ off, const int *__restrict__ idx,
@@ -27,6 +30,8 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
     float4 *tabU = tab, *tabE = tab + PSE_NTAB;
     for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) { tabU[i] = table[2 * i]; tabE[i] = table[2 * i + 1]; }
     __syncthreads();
+    constexpr bool INF = MODE & PSE_IN_F, INS = MODE & PSE_IN_S, OUTU = MODE & PSE_OUT_U, OUTE = MODE & PSE_OUT_E;
+    constexpr bool NEED_TU = (OUTU) || (INF && OUTE), NEED_TE = INS && OUTE;
     const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
     for (int s = blockIdx.x * wpb + (threadIdx.x >> 5); s < N; s += gridDim.x * wpb) {
         const float4 p = pos[s];
@@ -38,7 +43,9 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
         int b = j < hi ? idx[j] : 0;
         float4 q4 = pos[b];
         for (; j < hi; j += 32) {
-            const float4 a0 = in[2 * b], a1 = in[2 * b + 1];
+            float4 a0 = in[2 * b], a1 = in[2 * b + 1];
+            if (!INF) { a0.x = 0.f; a0.y = 0.f; a0.z = 0.f; }
+            if (!INS) { a0.w = 0.f; a1 = make_float4(0.f, 0.f, 0.f, 0.f); }
             const int bn = (j + 32 < hi) ? idx[j + 32] : b;
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
@@ -48,7 +55,9 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             float tt = r * inv_dr;
             int it = min((int)tt, PSE_NTAB - 2);
             const float w1 = tt - (float)it, w0 = 1.f - w1;
-            const float4 ta = tabU[it], tb = tabE[it], tc = tabU[it + 1], td = tabE[it + 1];
+            const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 ta = NEED_TU ? tabU[it] : zero4, tc = NEED_TU ? tabU[it + 1] : zero4;
+            const float4 tb = NEED_TE ? tabE[it] : zero4, td = NEED_TE ? tabE[it + 1] : zero4;
             const float F1 = w0 * ta.x + w1 * tc.x, F2 = w0 * ta.y + w1 * tc.y, Ga = w0 * ta.z + w1 * tc.z, Gb = w0 * ta.w + w1 * tc.w;
             const float A = w0 * tb.x + w1 * td.x, B = w0 * tb.y + w1 * td.y, D = w0 * tb.z + w1 * td.z;
             const float4 qn = pos[bn];
@@ -59,25 +68,29 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             const float tx = sxx * rx + sxy * ry + sxz * rz, ty = sxy * rx + syy * ry + syz * rz, tz = sxz * rx + syz * ry + szz * rz;
             const float q = rx * tx + ry * ty + rz * tz;
             const float cu = (F2 - F1) * f - Gb * q;
-            u0 += F1 * a0.x + cu * rx + Ga * tx;
-            u1 += F1 * a0.y + cu * ry + Ga * ty;
-            u2 += F1 * a0.z + cu * rz + Ga * tz;
+            if (OUTU) {
+                u0 += F1 * a0.x + cu * rx + Ga * tx;
+                u1 += F1 * a0.y + cu * ry + Ga * ty;
+                u2 += F1 * a0.z + cu * rz + Ga * tz;
+            }
             const float cw = Gb * f + D * q, B2 = 2.f * B;
             const float wx = -Ga * a0.x + B2 * tx + cw * rx, wy = -Ga * a0.y + B2 * ty + cw * ry, wz = -Ga * a0.z + B2 * tz + cw * rz;
             const float pxx = rx * wx, pyy = ry * wy, pzz = rz * wz;
-            e0 += A * a0.w + (pxx - pyy) * RS2;
-            e1 += A * a1.x + (2.f * pzz - pxx - pyy) * RS6;
-            e2 += A * a1.y + (rx * wy + ry * wx) * RS2;
-            e3 += A * a1.z + (rx * wz + rz * wx) * RS2;
-            e4 += A * a1.w + (ry * wz + rz * wy) * RS2;
+            if (OUTE) {
+                e0 += A * a0.w + (pxx - pyy) * RS2;
+                e1 += A * a1.x + (2.f * pzz - pxx - pyy) * RS6;
+                e2 += A * a1.y + (rx * wy + ry * wx) * RS2;
+                e3 += A * a1.z + (rx * wz + rz * wx) * RS2;
+                e4 += A * a1.w + (ry * wz + rz * wy) * RS2;
+            }
             b = bn;
             q4 = qn;
         }
         // self term (r -> 0 limit: F1(0) F and A(0) S) added by lane 0 before the reduction
         if (lane == 0) {
             const float4 a0 = in[2 * s], a1 = in[2 * s + 1], t0 = tabU[0], t1 = tabE[0];
-            u0 += t0.x * a0.x; u1 += t0.x * a0.y; u2 += t0.x * a0.z; e0 += t1.x * a0.w;
-            e1 += t1.x * a1.x; e2 += t1.x * a1.y; e3 += t1.x * a1.z; e4 += t1.x * a1.w;
+            if (INF && OUTU) { u0 += t0.x * a0.x; u1 += t0.x * a0.y; u2 += t0.x * a0.z; }
+            if (INS && OUTE) { e0 += t1.x * a0.w; e1 += t1.x * a1.x; e2 += t1.x * a1.y; e3 += t1.x * a1.z; e4 += t1.x * a1.w; }
         }
         const float part[8] = {u0, u1, u2, e0, e1, e2, e3, e4};
         int comp;
@@ -88,24 +101,36 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
 
 }  // namespace
 
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int ctas_per_sm) {
+template <int MODE>
+static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    real_pairs_kernel<MODE><<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
+                                                     c->d_nbr_off, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
+                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
+    KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int ctas_per_sm, int mode) {
     const bool own = (st == nullptr);
     if (own) st = c->stream;
     ScopedPhase ph(c, own ? PSE_T_REAL : -1);
     static int nsm = 0;
     if (!nsm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
     const size_t smem = (size_t)PSE_NTAB * 2 * sizeof(float4);
-    static bool attr_set = false;
-    if (!attr_set) {
-        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
     int grid = ctas_per_sm * nsm, wpb = 512 / 32;
     if ((long long)grid * wpb > c->N) grid = (c->N + wpb - 1) / wpb;
-    real_pairs_kernel<<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in),
-                                                      reinterpret_cast<float4 *>(d_out), c->N, c->d_nbr_off, c->d_nbr_idx,
-                                                      reinterpret_cast<const float4 *>(c->d_table), (float)(1.0 / c->tab_dr),
-                                                      (float)c->L, 1.0f / (float)c->L);
-    KERNEL_CHECK(c);
-    return PSE_OK;
+    // unrequested outputs are written as zeros; absent inputs must be zero in d_in (they are skipped, not read as data)
+    switch (mode) {
+        case PSE_IN_S | PSE_OUT_E: return launch_real<PSE_IN_S | PSE_OUT_E>(c, d_in, d_out, st, grid, smem);
+        case PSE_IN_F | PSE_OUT_E: return launch_real<PSE_IN_F | PSE_OUT_E>(c, d_in, d_out, st, grid, smem);
+        case PSE_IN_F | PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
+        case PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
+        case PSE_IN_F | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
+        default: return launch_real<PSE_MODE_ALL>(c, d_in, d_out, st, grid, smem);
+    }
 }

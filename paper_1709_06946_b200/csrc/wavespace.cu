@@ -12,6 +12,7 @@
 // of grid points, one thread per point with the 8 components in registers; it walks the particles binned in the
 // tiles whose supports can reach it, with separable weights staged in shared memory.  No atomics, no memset,
 // each grid value is written exactly once with full-sector coalesced stores, and the summation order is fixed.
+#include <algorithm>
 #include "pse_internal.h"
 
 namespace {
@@ -81,6 +82,7 @@ __device__ __forceinline__ int wrap_offset(int gp, int base, int M) {
 // particle data + the 3 x 8 separable weights, y-weights stored permuted so that a lane's four are one float4), then
 // compacted into one list per plane PAIR holding only the particles whose support covers it, in candidate order
 // (fixed summation order, no atomics).
+template <int C0, int NC>                           // components C0 .. C0+NC-1 are spread (0,8 | 0,3 | 3,5)
 __global__ void __launch_bounds__(SPREAD_THREADS)
 spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, const int *__restrict__ tile_start,
               const int *__restrict__ tile_list, float *__restrict__ grid, int M, int P, int nt, float inv_h, float wa, float wb) {
@@ -118,11 +120,11 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
         __syncthreads();
     }
     const int nbins = nbins_s, total = bin_cum[nbins];
-    float acc[4][8];
+    float acc[4][NC];
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
-        for (int c = 0; c < 8; ++c) acc[m][c] = 0.f;
+        for (int c = 0; c < NC; ++c) acc[m][c] = 0.f;
     for (int lo = 0; lo < total; lo += SPREAD_BATCH) {
         const int nb = min(SPREAD_BATCH, total - lo);
         unsigned xmask = 0;
@@ -175,11 +177,11 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
             const float4 wy = *reinterpret_cast<const float4 *>(&W[p][1][4 * b2]);
             const float4 q0 = q[p][0], q1 = q[p][1];
             const float w[4] = {wxz * wy.x, wxz * wy.y, wxz * wy.z, wxz * wy.w};
+            const float qv[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
 #pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                acc[m][0] += w[m] * q0.x; acc[m][1] += w[m] * q0.y; acc[m][2] += w[m] * q0.z; acc[m][3] += w[m] * q0.w;
-                acc[m][4] += w[m] * q1.x; acc[m][5] += w[m] * q1.y; acc[m][6] += w[m] * q1.z; acc[m][7] += w[m] * q1.w;
-            }
+            for (int m = 0; m < 4; ++m)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[m][c] += w[m] * qv[C0 + c];
         }
         __syncthreads();
     }
@@ -192,7 +194,7 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
             if (gy < M) {
                 const size_t o = ((size_t)gx * M + gy) * M + gz;
 #pragma unroll
-                for (int c = 0; c < 8; ++c) grid[c * M3 + o] = acc[m][c];
+                for (int c = 0; c < NC; ++c) grid[(C0 + c) * M3 + o] = acc[m][c];
             }
         }
     }
@@ -201,7 +203,7 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
 // Interpolation (a7): warp per particle (visited in tile order for L1/L2 locality), lanes over the P^3 support.
 __global__ void __launch_bounds__(256)
 interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list, const float *__restrict__ grid,
-              float4 *__restrict__ out, int N, int M, int P, float inv_h, float wa, float wb, int accumulate) {
+              float4 *__restrict__ out, int N, int M, int P, float inv_h, float wa, float wb, int accumulate, int mode) {
     const int wi = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (wi >= N) return;
     const int s = tile_list[wi];
@@ -230,7 +232,8 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
         const size_t o = ((size_t)pmod(base[0] + i, M) * M + pmod(base[1] + j, M)) * M + pmod(base[2] + k, M);
         if (ok) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) acc[c] += w * __ldg(grid + c * M3 + o);
+            for (int c = 0; c < 8; ++c)
+                if (mode & (c < 3 ? PSE_OUT_U : PSE_OUT_E)) acc[c] += w * __ldg(grid + c * M3 + o);
         }
     }
 #pragma unroll
@@ -254,7 +257,7 @@ template <int PT>                                  // PT > 0: support size known
 __global__ void __launch_bounds__(256)
 interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_start, const int *__restrict__ tile_list,
                    const float *__restrict__ grid, float4 *__restrict__ out, int M, int Prt, int nt, float inv_h, float wa, float wb,
-                   int accumulate) {
+                   int accumulate, int mode) {
     extern __shared__ float4 sm[];
     const int P = PT ? PT : Prt;
     const int E = T + P - 1, Ez = E + ((P - E) & 7), E3 = E * E * Ez;   // z-rows padded so that Ez = P (mod 8): the
@@ -276,8 +279,13 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
             if (lz < E) {
                 const size_t o = ((size_t)gx * M + gy) * M + gz;
                 const int idx = row * Ez + lz;
-                lo[idx] = make_float4(__ldg(grid + o), __ldg(grid + M3 + o), __ldg(grid + 2 * M3 + o), __ldg(grid + 3 * M3 + o));
-                hi[idx] = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
+                float4 vlo = make_float4(0.f, 0.f, 0.f, 0.f), vhi = vlo;     // only the planes the caller asked for are read
+                if (mode & PSE_OUT_U) { vlo.x = __ldg(grid + o); vlo.y = __ldg(grid + M3 + o); vlo.z = __ldg(grid + 2 * M3 + o); }
+                if (mode & PSE_OUT_E) {
+                    vlo.w = __ldg(grid + 3 * M3 + o);
+                    vhi = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
+                }
+                lo[idx] = vlo; hi[idx] = vhi;
             }
         }
     }
@@ -324,7 +332,7 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
         }
         int comp;
         float r = warp_reduce8(acc, lane, comp);
-        if ((lane & 3) == 0) {
+        if ((lane & 3) == 0 && (mode & (comp < 3 ? PSE_OUT_U : PSE_OUT_E))) {
             if (accumulate) r += outf[(size_t)s * 8 + comp];
             outf[(size_t)s * 8 + comp] = r;
         }
@@ -335,6 +343,7 @@ struct ScaleParams {
     int M, Mh;
     float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
     const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
+    int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
 };
 
 __device__ __forceinline__ float shape_s1(float x) {     // 3 (sin x - x cos x)/x^3, series below 0.5 (cancellation)
@@ -356,10 +365,13 @@ __device__ __forceinline__ bool mode_k(const ScaleParams &sp, int ix, int iy, in
 // Given uh (3 complex, already carrying B or sqrt(B) and the projector), write the 8 outputs of P^H (Eq. 41):
 //   Uh = s0 uh ;  Eh^q = i s1 (e^q k).uh
 __device__ __forceinline__ void write_outputs(cufftComplex *spec, size_t stride, size_t o, float s0, float s1,
-                                              float kx, float ky, float kz, float2 ux, float2 uy, float2 uz) {
-    spec[o] = make_float2(s0 * ux.x, s0 * ux.y);
-    spec[stride + o] = make_float2(s0 * uy.x, s0 * uy.y);
-    spec[2 * stride + o] = make_float2(s0 * uz.x, s0 * uz.y);
+                                              float kx, float ky, float kz, float2 ux, float2 uy, float2 uz, int mode) {
+    if (mode & PSE_OUT_U) {
+        spec[o] = make_float2(s0 * ux.x, s0 * ux.y);
+        spec[stride + o] = make_float2(s0 * uy.x, s0 * uy.y);
+        spec[2 * stride + o] = make_float2(s0 * uz.x, s0 * uz.y);
+    }
+    if (!(mode & PSE_OUT_E)) return;
     // i*s1*z = s1 * (-z.im, z.re)
     float2 pxx = make_float2(kx * ux.x, kx * ux.y), pyy = make_float2(ky * uy.x, ky * uy.y), pzz = make_float2(kz * uz.x, kz * uz.y);
     float2 d1 = make_float2((pxx.x - pyy.x) * RS2, (pxx.y - pyy.y) * RS2);
@@ -383,7 +395,8 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
     float2 zero = make_float2(0.f, 0.f);
     if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) spec[c * nmode + o] = zero;
+        for (int c = 0; c < 8; ++c)
+            if (sp.mode & (c < 3 ? PSE_OUT_U : PSE_OUT_E)) spec[c * nmode + o] = zero;
         return;
     }
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
@@ -393,9 +406,9 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
     const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-q) / k2 * dw * dw;          // one for interpolation
     float2 F[3], S[5];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) F[c] = spec[c * nmode + o];
+    for (int c = 0; c < 3; ++c) F[c] = (sp.mode & PSE_IN_F) ? spec[c * nmode + o] : zero;
 #pragma unroll
-    for (int c = 0; c < 5; ++c) S[c] = spec[(3 + c) * nmode + o];
+    for (int c = 0; c < 5; ++c) S[c] = (sp.mode & PSE_IN_S) ? spec[(3 + c) * nmode + o] : zero;
     // (S.k)_i from the 5 coordinates
     float2 sk[3];
 #pragma unroll
@@ -416,7 +429,7 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
     const float2 ux = make_float2(Bt * (f[0].x - kx * kf.x), Bt * (f[0].y - kx * kf.y));
     const float2 uy = make_float2(Bt * (f[1].x - ky * kf.x), Bt * (f[1].y - ky * kf.y));
     const float2 uz = make_float2(Bt * (f[2].x - kz * kf.x), Bt * (f[2].y - kz * kf.y));
-    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz);
+    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, sp.mode);
 }
 
 // a5, Brownian flavour (Eq. 75): uh = c_br sqrt((1+k^2/4xi^2)/(eta k^2)) exp(-(1-eta_g) k^2/8xi^2) (I - kh kh) W(k),
@@ -450,7 +463,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float2 ux = make_float2(Bh * (W[0].x - kx * kw.x), Bh * (W[0].y - kx * kw.y));
     const float2 uy = make_float2(Bh * (W[1].x - ky * kw.x), Bh * (W[1].y - ky * kw.y));
     const float2 uz = make_float2(Bh * (W[2].x - kz * kw.x), Bh * (W[2].y - kz * kw.y));
-    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz);
+    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
 }
 
 }  // namespace
@@ -468,20 +481,26 @@ pse_status pse_wave_init(pse_ctx *c) {
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
     int n[3] = {M, M, M};
-    size_t w1 = 0, w2 = 0;
-    CUFFT_TRY(c, cufftCreate(&c->plan_r2c)); CUFFT_TRY(c, cufftCreate(&c->plan_c2r)); c->have_plans = true;
-    CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_r2c, 0)); CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_c2r, 0));
-    CUFFT_TRY(c, cufftMakePlanMany(c->plan_r2c, 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, 8, &w1));
-    CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r, 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 8, &w2));
-    size_t w = w1 > w2 ? w1 : w2;
+    const int batches[3] = {8, 3, 5};                 // all grids | planes 0-2 (F in, U out) | planes 3-7 (S in, E out)
+    size_t w = 0;
+    for (int i = 0; i < 3; ++i) {
+        size_t w1 = 0, w2 = 0;
+        CUFFT_TRY(c, cufftCreate(&c->plan_r2c[i])); CUFFT_TRY(c, cufftCreate(&c->plan_c2r[i])); c->nplans = i + 1;
+        CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_r2c[i], 0)); CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_c2r[i], 0));
+        CUFFT_TRY(c, cufftMakePlanMany(c->plan_r2c[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, batches[i], &w1));
+        CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, batches[i], &w2));
+        w = std::max(w, std::max(w1, w2));
+    }
     if (w) CUDA_TRY(c, cudaMalloc(&c->d_fft_work, w));
-    CUFFT_TRY(c, cufftSetWorkArea(c->plan_r2c, c->d_fft_work)); CUFFT_TRY(c, cufftSetWorkArea(c->plan_c2r, c->d_fft_work));
-    CUFFT_TRY(c, cufftSetStream(c->plan_r2c, c->stream)); CUFFT_TRY(c, cufftSetStream(c->plan_c2r, c->stream));
+    for (int i = 0; i < 3; ++i) {
+        CUFFT_TRY(c, cufftSetWorkArea(c->plan_r2c[i], c->d_fft_work)); CUFFT_TRY(c, cufftSetWorkArea(c->plan_c2r[i], c->d_fft_work));
+        CUFFT_TRY(c, cufftSetStream(c->plan_r2c[i], c->stream)); CUFFT_TRY(c, cufftSetStream(c->plan_c2r[i], c->stream));
+    }
     return PSE_OK;
 }
 
 void pse_wave_free(pse_ctx *c) {
-    if (c->have_plans) { cufftDestroy(c->plan_r2c); cufftDestroy(c->plan_c2r); }
+    for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
     cudaFree(c->d_tile_count); cudaFree(c->d_tile_start); cudaFree(c->d_tile_fill); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
 }
@@ -497,8 +516,9 @@ pse_status pse_tile_bins(pse_ctx *c) {
     return PSE_OK;
 }
 
-static ScaleParams make_scale_params(const pse_ctx *c) {
+static ScaleParams make_scale_params(const pse_ctx *c, int mode = PSE_MODE_ALL) {
     ScaleParams sp;
+    sp.mode = mode;
     sp.M = c->M; sp.Mh = c->Mh;
     sp.two_pi_over_L = (float)(2.0 * M_PI / c->L); sp.a = (float)c->a;
     sp.inv4xi2 = (float)(1.0 / (4.0 * c->xi * c->xi)); sp.dec = c->d_dec;
@@ -508,8 +528,19 @@ static ScaleParams make_scale_params(const pse_ctx *c) {
     return sp;
 }
 
-static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, cudaEvent_t wait_ev = nullptr) {
-    { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r, c->d_spec, c->d_grid)); c->launches++; }
+// plane range of a 2-bit component mask (bit 0: planes 0-2, bit 1: planes 3-7): plan index and first plane
+static inline void plane_range(int bits, int &plan, int &first) {
+    plan = bits == 3 ? 0 : bits; first = bits == 2 ? 3 : 0;
+}
+
+static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, cudaEvent_t wait_ev = nullptr, int mode = PSE_MODE_ALL) {
+    {
+        ScopedPhase ph(c, PSE_T_FFT_INV);
+        int plan, first;
+        plane_range((mode >> 2) & 3, plan, first);
+        const size_t M3 = (size_t)c->M * c->M * c->M, nmode = (size_t)c->M * c->M * c->Mh;
+        CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++;
+    }
     if (wait_ev) CUDA_TRY(c, cudaStreamWaitEvent(c->stream, wait_ev, 0));
     ScopedPhase ph(c, PSE_T_INTERP);
     const int TB = 256, E = T + c->P - 1;
@@ -525,7 +556,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
         }                                                                                                                  \
         interp_tile_kernel<PT><<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid,       \
             reinterpret_cast<float4 *>(d_out), c->M, c->P, c->nt, (float)(1.0 / c->h), (float)c->win_a, (float)c->win_b, \
-            accumulate ? 1 : 0);                                                                                           \
+            accumulate ? 1 : 0, mode);                                                                                     \
     } while (0)
         switch (c->P) {
             case 3: PSE_LAUNCH_INTERP(3); break;
@@ -540,26 +571,32 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     } else {
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
-            (float)c->win_a, (float)c->win_b, accumulate ? 1 : 0);
+            (float)c->win_a, (float)c->win_b, accumulate ? 1 : 0, mode);
     }
     KERNEL_CHECK(c);
     return PSE_OK;
 }
 
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp) {
-    const size_t nmode = (size_t)c->M * c->M * c->Mh;
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp, int mode) {
+    const size_t nmode = (size_t)c->M * c->M * c->Mh, M3 = (size_t)c->M * c->M * c->M;
+    if (!(mode & (PSE_IN_F | PSE_IN_S)) || !(mode & (PSE_OUT_U | PSE_OUT_E))) { c->err = "pse_wave_apply: empty component mask"; return PSE_EINVAL; }
+    int plan, first;
+    plane_range(mode & 3, plan, first);
     {
         ScopedPhase ph(c, PSE_T_SPREAD);
-        spread_kernel<<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), c->d_tile_start, c->d_tile_list,
-                                                       c->d_grid, c->M, c->P, c->nt, (float)(1.0 / c->h), (float)c->win_a, (float)c->win_b);
+        const float4 *in4 = reinterpret_cast<const float4 *>(d_in);
+        const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
+        if (plan == 0) spread_kernel<0, 8><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
+        else if (plan == 1) spread_kernel<0, 3><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
+        else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         KERNEL_CHECK(c);
     }
-    { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c, c->d_grid, c->d_spec)); c->launches++; }
+    { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[plan], c->d_grid + first * M3, c->d_spec + first * nmode)); c->launches++; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
-        scale_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c)); KERNEL_CHECK(c);
+        scale_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c, mode)); KERNEL_CHECK(c);
     }
-    return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp);
+    return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp, mode);
 }
 
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {

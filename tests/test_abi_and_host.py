@@ -96,4 +96,6 @@ def test_bench_algorithmic_bytes_formula():
     import bench
     ab = bench.algorithmic_bytes(1000, 10, 20.0)
     assert ab['spread'] == 48 * 1000 + 32 * 1000 and ab['scale'] == 2 * 64 * 10 * 10 * 6
+    pl = bench.planes_per_launch(7)
+    assert abs(pl['spread'] - 46 / 9) < 1e-12 and abs(pl['interp'] - 51 / 10) < 1e-12 and abs(pl['scale'] - 100 / 10) < 1e-12
     assert ab['real'] == 80 * 1000 + 4 * 1000 * 20.0
