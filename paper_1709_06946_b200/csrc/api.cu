@@ -129,6 +129,8 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaMalloc(&c->d_cell_fill, (size_t)(c->ncell + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_count, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_off, (size_t)(N + 1) * sizeof(unsigned long long)));
+    CUDA_TRY(c, cudaMalloc(&c->d_nbr_ctl, 2 * sizeof(unsigned long long)));
+    CUDA_TRY(c, cudaMallocHost(&c->h_nbr_ctl, 2 * sizeof(unsigned long long)));
     for (float **p : {&c->d_in, &c->d_out, &c->d_tmp, &c->d_tmp2, &c->d_vecA, &c->d_vecB, &c->d_vecC, &c->d_vecD}) CUDA_TRY(c, cudaMalloc(p, n8));
     c->krylov_cap = PSE_MAX_KRYLOV + 1;
     CUDA_TRY(c, cudaMalloc(&c->d_krylov, (size_t)c->krylov_cap * n8));
@@ -160,7 +162,8 @@ pse_status pse_destroy(pse_ctx *c) {
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
     cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_fill); cudaFree(c->d_nbr_count);
-    cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx);
+    cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx); cudaFree(c->d_nbr_ctl);
+    if (c->h_nbr_ctl) cudaFreeHost(c->h_nbr_ctl);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
     cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec);
     cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);

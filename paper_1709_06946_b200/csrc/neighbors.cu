@@ -257,27 +257,130 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
     }
 }
 
+// Single-pass neighbour build, CTA per cell (default path).  Pass A tests every (particle, candidate) pair once and
+// keeps the 32-bit hit masks in shared memory; the cell's total is then reserved with ONE atomicAdd on a global
+// cursor, and pass B expands the masks into the reserved segment.  A particle's list is deterministic (candidate
+// order); only the placement of whole cells in the index array depends on scheduling, which no consumer sees
+// (they go through off[s], count[s]).  Cells too large for the mask store (> NB_MAXP particles or > NS_CHUNK
+// candidates) set *fallback and are handled by the two-pass kernels above.
+constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32;
+
+__global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
+                                                                   float L, float invL, float rc2, int *__restrict__ count,
+                                                                   unsigned long long *__restrict__ off, int *__restrict__ idx,
+                                                                   unsigned long long cap, unsigned long long *__restrict__ cursor,
+                                                                   int *__restrict__ fallback) {
+    __shared__ float4 cpos[NS_CHUNK];
+    __shared__ unsigned masks[NB_MAXP][NB_WORDS];
+    __shared__ int cnt[NB_MAXP], loc[NB_MAXP];
+    __shared__ int run_lo[18], run_cum[19];
+    __shared__ unsigned long long base_s;
+    const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int first = cell_start[cell], np = cell_start[cell + 1] - first;
+    if (np == 0) return;
+    const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
+    const int span = nc >= 3 ? 3 : nc;
+    if (tid < 32) {
+        int lo = 0, len = 0;
+        const int col_i = lane >> 1, part = lane & 1;
+        if (col_i < span * span) {
+            int ccx = col_i / span, ccy = col_i % span;
+            if (nc >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + ccy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
+            const int col = (ccx * nc + ccy) * nc;
+            const int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
+            int a0, a1, b0 = 0, b1 = 0;
+            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc - 1; b1 = nc; }
+            else if (z1 >= nc) { a0 = 0; a1 = 1; b0 = z0; b1 = nc; }
+            else { a0 = z0; a1 = z1 + 1; }
+            const int c0 = part ? b0 : a0, c1 = part ? b1 : a1;
+            lo = cell_start[col + c0]; len = cell_start[col + c1] - lo;
+        }
+        int inc = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+        if (lane < 18) { run_lo[lane] = lo; run_cum[lane] = inc - len; }
+        if (lane == 17) run_cum[18] = inc;
+    }
+    __syncthreads();
+    const int total = run_cum[18];
+    if (np > NB_MAXP || total > NS_CHUNK) {                 // uniform over the CTA
+        if (tid == 0) atomicExch(fallback, 1);
+        return;
+    }
+    for (int c = tid; c < total; c += NS_THREADS) {
+        int r = 0;
+        while (run_cum[r + 1] <= c) ++r;
+        const int j = run_lo[r] + c - run_cum[r];
+        float4 q = pos[j];
+        q.w = __int_as_float(j);
+        cpos[c] = q;
+    }
+    __syncthreads();
+    const int nwords = (total + 31) >> 5;
+    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass A: distance tests, masks, counts
+        const int s = first + pi;
+        const float4 p = pos[s];
+        int found = 0;
+        for (int w = 0; w < nwords; ++w) {
+            const int c = w * 32 + lane;
+            bool in = false;
+            if (c < total) { const float4 q = cpos[c]; in = (__float_as_int(q.w) != s) && dist2(p, q, L, invL) < rc2; }
+            const unsigned m = __ballot_sync(0xffffffffu, in);
+            if (lane == 0) masks[pi][w] = m;
+            found += __popc(m);
+        }
+        if (lane == 0) cnt[pi] = found;
+    }
+    __syncthreads();
+    if (tid < 32) {                                           // exclusive prefix of the <= 64 counts, one reservation
+        const int c0 = tid < np ? cnt[tid] : 0, c1 = tid + 32 < np ? cnt[tid + 32] : 0;
+        int i0 = c0, i1 = c1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v0 = __shfl_up_sync(0xffffffffu, i0, o), v1 = __shfl_up_sync(0xffffffffu, i1, o);
+            if (lane >= o) { i0 += v0; i1 += v1; }
+        }
+        const int tot0 = __shfl_sync(0xffffffffu, i0, 31), tot1 = __shfl_sync(0xffffffffu, i1, 31);
+        loc[tid] = i0 - c0; loc[tid + 32] = tot0 + i1 - c1;
+        if (tid == 0) base_s = atomicAdd(cursor, (unsigned long long)(tot0 + tot1));
+    }
+    __syncthreads();
+    const unsigned long long base = base_s;
+    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks
+        const int s = first + pi;
+        const unsigned long long o = base + (unsigned long long)loc[pi];
+        if (lane == 0) { off[s] = o; count[s] = cnt[pi]; }
+        if (o + (unsigned long long)cnt[pi] > cap) continue;  // overflow: the host re-runs with a larger index array
+        int found = 0;
+        for (int w = 0; w < nwords; ++w) {
+            const unsigned m = masks[pi][w];
+            if ((m >> lane) & 1u) idx[o + found + __popc(m & ((1u << lane) - 1))] = __float_as_int(cpos[w * 32 + lane].w);
+            found += __popc(m);
+        }
+    }
+}
+
 __global__ void counts_to_original(const int *count_sorted, const int *order, int N, int *count_orig) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s < N) count_orig[order[s]] = count_sorted[s];
 }
 
-__global__ void lists_to_original(const int *idx, const unsigned long long *off_sorted, const int *order, int N,
+__global__ void lists_to_original(const int *idx, const unsigned long long *off_sorted, const int *count_sorted, const int *order, int N,
                                   const unsigned long long *off_orig, int *out) {
     int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (s >= N) return;
-    unsigned long long lo = off_sorted[s], n = off_sorted[s + 1] - lo, dst = off_orig[order[s]];
+    unsigned long long lo = off_sorted[s], n = (unsigned long long)count_sorted[s], dst = off_orig[order[s]];
     for (unsigned long long j = lane; j < n; j += 32) out[dst + j] = order[idx[lo + j]];
 }
 
 // Heyes-Melrose overlap force (reading R12), warp per particle over the neighbour list, packed output.
-__global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off,
+__global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off, const int *__restrict__ count,
                           const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out) {
     int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (s >= N) return;
     float4 p = pos[s];
     float fx = 0, fy = 0, fz = 0;
-    for (unsigned long long j = off[s] + lane; j < off[s + 1]; j += 32) {
+    for (unsigned long long j = off[s] + lane, hi = off[s] + (unsigned long long)count[s]; j < hi; j += 32) {
         float4 q = pos[idx[j]];
         float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
         float r2 = dx * dx + dy * dy + dz * dz;
@@ -319,24 +422,47 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order_tmp); KERNEL_CHECK(c);
     pse_rank_sort(c, c->d_cell_start, c->ncell, c->d_order_tmp, c->d_order);
     gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos); KERNEL_CHECK(c);
-    neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
-                                                                        nullptr, nullptr); KERNEL_CHECK(c);
-    PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
-    unsigned long long total = 0;
-    CUDA_TRY(c, cudaMemcpyAsync(&total, c->d_nbr_off + N, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    if (total > 0x7fffffffull * 4ull) { c->err = "neighbour list too large"; return PSE_EOVERFLOW; }
-    if (total > c->nbr_cap) {
-        if (c->d_nbr_idx) cudaFree(c->d_nbr_idx);
-        c->d_nbr_idx = nullptr; c->nbr_cap = 0;
-        size_t cap = (size_t)(total * 1.25) + 1024;
+    PSE_TRY(pse_tile_bins(c));                       // independent of the list; enqueued first so it overlaps the read-back
+    // ---- single-pass build into a cursor-allocated index array; grows and repeats if the array was too small ----
+    if (!c->d_nbr_idx) {
+        const size_t cap = (size_t)N * 48 + 1024;
         if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
         c->nbr_cap = cap;
     }
-    c->nbr_total = (size_t)total;
-    neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
-                                                                       c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
-    PSE_TRY(pse_tile_bins(c));
+    bool done = false;
+    for (int attempt = 0; attempt < 3 && !done; ++attempt) {
+        CUDA_TRY(c, cudaMemsetAsync(c->d_nbr_ctl, 0, 2 * sizeof(unsigned long long), c->stream));
+        neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count, c->d_nbr_off,
+                                                                   c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
+                                                                   reinterpret_cast<int *>(c->d_nbr_ctl + 1)); KERNEL_CHECK(c);
+        CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->h_nbr_ctl[1] != 0) break;                            // a cell exceeds the mask store: two-pass path below
+        const unsigned long long total = c->h_nbr_ctl[0];
+        if (total <= c->nbr_cap) { c->nbr_total = (size_t)total; done = true; break; }
+        cudaFree(c->d_nbr_idx); c->d_nbr_idx = nullptr; c->nbr_cap = 0;
+        const size_t cap = (size_t)(total * 1.25) + 1024;
+        if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
+        c->nbr_cap = cap;
+    }
+    if (!done) {                                                     // general two-pass path (count, scan, fill)
+        neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
+                                                                            nullptr, nullptr); KERNEL_CHECK(c);
+        PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
+        unsigned long long total = 0;
+        CUDA_TRY(c, cudaMemcpyAsync(&total, c->d_nbr_off + N, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (total > c->nbr_cap) {
+            if (c->d_nbr_idx) cudaFree(c->d_nbr_idx);
+            c->d_nbr_idx = nullptr; c->nbr_cap = 0;
+            size_t cap = (size_t)(total * 1.25) + 1024;
+            if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
+            c->nbr_cap = cap;
+        }
+        c->nbr_total = (size_t)total;
+        neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
+                                                                           c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
+    }
     c->have_nbrs = true;
     return PSE_OK;
 }
@@ -353,7 +479,7 @@ pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t
     CUDA_TRY(c, cudaMalloc(&off, (size_t)(N + 1) * sizeof(unsigned long long)));
     counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, cnt); KERNEL_CHECK(c);
     PSE_TRY(pse_scan_u64(c, cnt, off, (size_t)N));
-    lists_to_original<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_nbr_idx, c->d_nbr_off, c->d_order, N, off, d_index);
+    lists_to_original<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_nbr_idx, c->d_nbr_off, c->d_nbr_count, c->d_order, N, off, d_index);
     KERNEL_CHECK(c);
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     cudaFree(cnt); cudaFree(off);
@@ -364,7 +490,7 @@ pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {
     ScopedPhase ph(c, PSE_T_REAL);
     const int N = c->N, T = 256;
     float coef = (float)(3.0 * M_PI * c->eta * c->a / dt);
-    hs_forces<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_idx, (float)c->L,
+    hs_forces<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, (float)c->L,
                                                                             1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed);
     KERNEL_CHECK(c);
     return PSE_OK;

@@ -47,6 +47,7 @@ struct pse_ctx {
     int *d_nbr_count = nullptr;              // [N]
     unsigned long long *d_nbr_off = nullptr; // [N+1]
     int *d_nbr_idx = nullptr; size_t nbr_cap = 0, nbr_total = 0;
+    unsigned long long *d_nbr_ctl = nullptr, *h_nbr_ctl = nullptr;   // {allocation cursor, fallback flag}; pinned mirror
     // ---- FFT-grid tile bins ----
     int nt = 0, ntile = 0, Mh = 0;           // tiles per dimension, total, M/2+1
     int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]

@@ -22,7 +22,7 @@ constexpr float RS6 = 0.40824829046386302f;   // 1/sqrt6
 template <int MODE>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
-                  const unsigned long long *__restrict__ off, const int *__restrict__ idx,
+                  const unsigned long long *__restrict__ off, const int *__restrict__ cnt, const int *__restrict__ idx,
                   const float4 *__restrict__ table, float inv_dr, float L, float invL) {
     // two planar float4 arrays (U-part functions, E-part functions): a 16-byte row stride spreads random rows over
     // all eight 16-byte bank groups; the interleaved 32-byte rows reached only four (ncu: 17 wavefronts per LDS.128)
@@ -36,7 +36,7 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
     for (int s = blockIdx.x * wpb + (threadIdx.x >> 5); s < N; s += gridDim.x * wpb) {
         const float4 p = pos[s];
         float u0 = 0, u1 = 0, u2 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
-        const unsigned long long lo = off[s], hi = off[s + 1];
+        const unsigned long long lo = off[s], hi = lo + (unsigned long long)cnt[s];
         // software pipeline of depth one on the dependent chain idx -> pos: the next neighbour's index and position
         // are requested while the current pair is evaluated (ncu: 42 % of the stall samples sat on these two waits)
         unsigned long long j = lo + lane;
@@ -109,7 +109,7 @@ static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, cudaS
         attr_set = true;
     }
     real_pairs_kernel<MODE><<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
-                                                     c->d_nbr_off, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
+                                                     c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
                                                      (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
     KERNEL_CHECK(c);
     return PSE_OK;

@@ -78,9 +78,11 @@ def test_neighbors_bit_exact_config1(config1):
         assert np.array_equal(g, w)
 
 
-@pytest.mark.parametrize('N,phi,xi,seed,shift', [(500, 0.30, 0.9, 3, False), (777, 0.05, 0.5, 4, True), (30, 0.02, 0.35, 5, True)])
+@pytest.mark.parametrize('N,phi,xi,seed,shift', [(500, 0.30, 0.9, 3, False), (777, 0.05, 0.5, 4, True), (30, 0.02, 0.35, 5, True),
+                                                 (1500, 0.30, 0.23, 6, False)])
 def test_neighbors_bit_exact_other(N, phi, xi, seed, shift):
-    """Ragged sizes, dense and dilute, unwrapped inputs, and a box with fewer than 3 cells per side."""
+    """Ragged sizes, dense and dilute, unwrapped inputs, a box with fewer than 3 cells per side, and (last case) cells
+    with more than 1024 candidates, which take the two-pass fallback of the neighbour build."""
     import paper_1709_06946_b200 as pse
     x, L = synth.rsa(N, phi, seed=seed)
     if shift:
