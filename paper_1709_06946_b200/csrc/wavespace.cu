@@ -125,21 +125,50 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
     for (int m = 0; m < 4; ++m)
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[m][c] = 0.f;
-    for (int lo = 0; lo < total; lo += SPREAD_BATCH) {
-        const int nb = min(SPREAD_BATCH, total - lo);
+    __shared__ int hs[2 * SPREAD_BATCH];            // particles whose support really reaches this tile, in candidate order
+    __shared__ int hcnt[4];
+    int nh = 0, cand = 0;                           // uniform over the CTA
+    while (cand < total || nh > 0) {
+        // phase 1: cheap geometric test on 128 candidates at a time (2 of 3 miss the tile), hits compacted into hs
+        while (cand < total && nh <= SPREAD_BATCH) {
+            const int ci = cand + tid;
+            bool hit = false;
+            int s = 0;
+            if (ci < total) {
+                int k = 0;
+                while (bin_cum[k + 1] <= ci) ++k;
+                s = tile_list[bin_lo[k] + ci - bin_cum[k]];
+                const float4 p = pos[s];
+                const float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
+                hit = true;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const int o0 = wrap_offset(g0[d], support_base(g[d], P), M);
+                    hit = hit && (o0 < P || o0 > M - T);
+                }
+            }
+            const unsigned hb = __ballot_sync(0xffffffffu, hit);
+            if (lane == 0) hcnt[wid] = __popc(hb);
+            __syncthreads();
+            int woff = 0, tot = 0;
+#pragma unroll
+            for (int w = 0; w < 4; ++w) { const int v = hcnt[w]; woff += w < wid ? v : 0; tot += v; }
+            if (hit) hs[nh + woff + __popc(hb & ((1u << lane) - 1))] = s;
+            __syncthreads();
+            nh += tot; cand += SPREAD_BATCH;
+        }
+        // phase 2: weights for up to 128 hits, one thread each (dense lanes)
+        const int nb = min(nh, SPREAD_BATCH);
         unsigned xmask = 0;
         if (tid < nb) {
-            int ci = lo + tid, k = 0;
-            while (bin_cum[k + 1] <= ci) ++k;
-            const int s = tile_list[bin_lo[k] + ci - bin_cum[k]];
+            const int s = hs[tid];
             const float4 p = pos[s];
             q[tid][0] = in[2 * s]; q[tid][1] = in[2 * s + 1];
             const float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
-            unsigned msk[3];
+            unsigned msk[3] = {0u, 0u, 0u};
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const int base = support_base(g[d], P);
-                msk[d] = 0;
 #pragma unroll
                 for (int i = 0; i < T; ++i) {
                     const int gp = g0[d] + i, o = wrap_offset(gp, base, M);
@@ -184,6 +213,12 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
                 for (int c = 0; c < NC; ++c) acc[m][c] += w[m] * qv[C0 + c];
         }
         __syncthreads();
+        const int left = nh - nb;                     // leftover hits (<= 128) move to the front of the buffer
+        const int mv = tid < left ? hs[nb + tid] : 0;
+        __syncthreads();
+        if (tid < left) hs[tid] = mv;
+        __syncthreads();
+        nh = left;
     }
     const int gx = g0[0] + a, gz = g0[2] + cc;
     const size_t M3 = (size_t)M * M * M;
