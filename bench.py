@@ -76,8 +76,8 @@ class ClockSampler:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r1_traffic.json.md), workload config3 only; other workloads report null.
-NCU_TRAFFIC = {'config3': {'real': 33551616, 'spread': 4061440, 'interp': 26755584}}
+# (profiles/r1_traffic.md), default workload only; other workloads report null.
+NCU_TRAFFIC = {'config3': {'real': 18945536, 'spread': 3477248, 'interp': 23430144, 'scale': 20025600, 'neighbors': 1085184}}
 
 
 def max_over_ranks(ms, device=None):
