@@ -13,6 +13,7 @@
 // tiles whose supports can reach it, with separable weights staged in shared memory.  No atomics, no memset,
 // each grid value is written exactly once with full-sector coalesced stores, and the summation order is fixed.
 #include <algorithm>
+#include <cuda_pipeline.h>
 #include "pse_internal.h"
 
 namespace {
@@ -314,15 +315,22 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
             if (lz < E) {
                 const size_t o = ((size_t)gx * M + gy) * M + gz;
                 const int idx = row * Ez + lz;
-                float4 vlo = make_float4(0.f, 0.f, 0.f, 0.f), vhi = vlo;     // only the planes the caller asked for are read
-                if (mode & PSE_OUT_U) { vlo.x = __ldg(grid + o); vlo.y = __ldg(grid + M3 + o); vlo.z = __ldg(grid + 2 * M3 + o); }
+                // asynchronous 4-byte copies global -> shared (cp.async, LDGSTS): all rows of the block are in flight
+                // at once instead of one L2 round trip per row; planes the caller did not ask for are zero-filled
+                float *dlo = reinterpret_cast<float *>(lo + idx), *dhi = reinterpret_cast<float *>(hi + idx);
+                if (mode & PSE_OUT_U) {
+                    __pipeline_memcpy_async(dlo, grid + o, 4); __pipeline_memcpy_async(dlo + 1, grid + M3 + o, 4);
+                    __pipeline_memcpy_async(dlo + 2, grid + 2 * M3 + o, 4);
+                } else { dlo[0] = 0.f; dlo[1] = 0.f; dlo[2] = 0.f; }
                 if (mode & PSE_OUT_E) {
-                    vlo.w = __ldg(grid + 3 * M3 + o);
-                    vhi = make_float4(__ldg(grid + 4 * M3 + o), __ldg(grid + 5 * M3 + o), __ldg(grid + 6 * M3 + o), __ldg(grid + 7 * M3 + o));
-                }
-                lo[idx] = vlo; hi[idx] = vhi;
+                    __pipeline_memcpy_async(dlo + 3, grid + 3 * M3 + o, 4);
+                    __pipeline_memcpy_async(dhi, grid + 4 * M3 + o, 4); __pipeline_memcpy_async(dhi + 1, grid + 5 * M3 + o, 4);
+                    __pipeline_memcpy_async(dhi + 2, grid + 6 * M3 + o, 4); __pipeline_memcpy_async(dhi + 3, grid + 7 * M3 + o, 4);
+                } else { dlo[3] = 0.f; hi[idx] = make_float4(0.f, 0.f, 0.f, 0.f); }
             }
         }
+        __pipeline_commit();
+        __pipeline_wait_prior(0);
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -330,9 +338,15 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     float *outf = reinterpret_cast<float *>(out);
     // lane <-> (j,k) column of the support; the loop over i walks x with a uniform weight, so the inner loop is
     // two 16-byte shared loads and 8 FMAs, no index arithmetic and no shuffles except the broadcast of wx[i].
+    const int mycomp = ((lane & 16) ? 4 : 0) + ((lane & 8) ? 2 : 0) + ((lane & 4) ? 1 : 0);   // component this lane ends up holding
+    const bool writer = (lane & 3) == 0 && (mode & (mycomp < 3 ? PSE_OUT_U : PSE_OUT_E));
+    int s_next = wid < np ? tile_list[first + wid] : 0;
+    float4 p_next = pos[s_next];
     for (int pi = wid; pi < np; pi += nw) {
-        const int s = tile_list[first + pi];
-        const float4 p = pos[s];
+        const int s = s_next;
+        const float4 p = p_next;
+        if (pi + nw < np) { s_next = tile_list[first + pi + nw]; p_next = pos[s_next]; }       // next particle in flight
+        const float prev = (writer && accumulate) ? outf[(size_t)s * 8 + mycomp] : 0.f;         // read-modify-write operand early
         const float gx = p.x * inv_h, gy = p.y * inv_h, gz = p.z * inv_h;
         const int b0 = support_base(gx, P), b1 = support_base(gy, P), b2 = support_base(gz, P);
         const int r0 = pmod(b0, M) - t0 * T, r1 = pmod(b1, M) - t1 * T, r2 = pmod(b2, M) - t2 * T;
@@ -366,11 +380,8 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
             for (int c = 0; c < 8; ++c) acc[c] += wyz * tsum[c];
         }
         int comp;
-        float r = warp_reduce8(acc, lane, comp);
-        if ((lane & 3) == 0 && (mode & (comp < 3 ? PSE_OUT_U : PSE_OUT_E))) {
-            if (accumulate) r += outf[(size_t)s * 8 + comp];
-            outf[(size_t)s * 8 + comp] = r;
-        }
+        const float r = warp_reduce8(acc, lane, comp);
+        if (writer) outf[(size_t)s * 8 + mycomp] = r + prev;
     }
 }
 
