@@ -248,7 +248,13 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     double wn = 0;
     int m = 0;
     bool converged = false;
-    for (int j = 0; j < maxit; ++j) {
+    // The host only decides when to stop, so it need not look at every iteration: the read-back (a stream
+    // synchronisation that idles the GPU) is skipped until one iteration before the count the previous call needed;
+    // the skipped iterations are then examined in order and the first converged one is taken — same result as
+    // checking every time.
+    const int first_check = std::max(0, c->last_lanczos_iters - 2);
+    int examined = 0;
+    for (int j = 0; j < maxit && !converged; ++j) {
         float4 *vj = V + (size_t)j * n4;
         PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
         { ScopedPhase ph(c, PSE_T_VECTOR);
@@ -256,29 +262,34 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
           k_lanczos_update<<<vgrid(n4), VT, 0, c->stream>>>(u, vj, j ? vj - n4 : nullptr, c->d_scal + 1 + 2 * j, j ? c->d_scal + 2 * j : nullptr,
                                                            n4, c->d_scal + 2 + 2 * j); KERNEL_CHECK(c);
           if (j + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(vj + n4, u, c->d_scal + 2 + 2 * j, n4); KERNEL_CHECK(c); } }
-        PSE_TRY(read_scalars(c, 3 + 2 * j));                        // one read-back per iteration
-        if (j == 0) {
-            wn = std::sqrt(c->h_scal[0]);
-            if (!(wn > 0)) { CUDA_TRY(c, cudaMemsetAsync(d_y, 0, n * sizeof(float), c->stream)); return PSE_OK; }
+        if (j < first_check && j + 1 < maxit) continue;
+        PSE_TRY(read_scalars(c, 3 + 2 * j));
+        for (; examined <= j && !converged; ++examined) {
+            const int e_j = examined;
+            if (e_j == 0) {
+                wn = std::sqrt(c->h_scal[0]);
+                if (!(wn > 0)) { CUDA_TRY(c, cudaMemsetAsync(d_y, 0, n * sizeof(float), c->stream)); return PSE_OK; }
+            }
+            alpha.push_back(c->h_scal[1 + 2 * e_j]);
+            beta.push_back(std::sqrt(c->h_scal[2 + 2 * e_j]));
+            m = e_j + 1;
+            // coefficient vector  c = |w| T^{1/2} e_1  of the m x m tridiagonal
+            std::vector<double> Tm((size_t)m * m, 0.0), Q;
+            for (int i = 0; i < m; ++i) { Tm[(size_t)i * m + i] = alpha[i]; if (i + 1 < m) Tm[(size_t)i * m + i + 1] = Tm[(size_t)(i + 1) * m + i] = beta[i]; }
+            jacobi_eigh(m, Tm, Q);
+            ccur.assign(m, 0.0);
+            for (int e = 0; e < m; ++e) {
+                double lam = Tm[(size_t)e * m + e], sq = lam > 0 ? std::sqrt(lam) : 0.0, q0 = Q[e];       // Q[0][e]
+                for (int i = 0; i < m; ++i) ccur[i] += wn * Q[(size_t)i * m + e] * sq * q0;
+            }
+            double diff = 0, nrm = 0;
+            for (int i = 0; i < m; ++i) { double d = ccur[i] - (i < (int)cprev.size() ? cprev[i] : 0.0); diff += d * d; nrm += ccur[i] * ccur[i]; }
+            cprev = ccur;
+            if (e_j > 0 && std::sqrt(diff) <= c->tol * std::sqrt(nrm)) converged = true;
+            else if (beta[e_j] <= 1e-7 * std::fabs(alpha[0])) converged = true;                          // invariant subspace
         }
-        alpha.push_back(c->h_scal[1 + 2 * j]);
-        beta.push_back(std::sqrt(c->h_scal[2 + 2 * j]));
-        m = j + 1;
-        // coefficient vector  c = |w| T^{1/2} e_1  of the m x m tridiagonal
-        std::vector<double> Tm((size_t)m * m, 0.0), Q;
-        for (int i = 0; i < m; ++i) { Tm[(size_t)i * m + i] = alpha[i]; if (i + 1 < m) Tm[(size_t)i * m + i + 1] = Tm[(size_t)(i + 1) * m + i] = beta[i]; }
-        jacobi_eigh(m, Tm, Q);
-        ccur.assign(m, 0.0);
-        for (int e = 0; e < m; ++e) {
-            double lam = Tm[(size_t)e * m + e], sq = lam > 0 ? std::sqrt(lam) : 0.0, q0 = Q[e];       // Q[0][e]
-            for (int i = 0; i < m; ++i) ccur[i] += wn * Q[(size_t)i * m + e] * sq * q0;
-        }
-        double diff = 0, nrm = 0;
-        for (int i = 0; i < m; ++i) { double d = ccur[i] - (i < (int)cprev.size() ? cprev[i] : 0.0); diff += d * d; nrm += ccur[i] * ccur[i]; }
-        cprev = ccur;
-        if (j > 0 && std::sqrt(diff) <= c->tol * std::sqrt(nrm)) { converged = true; break; }
-        if (beta[j] <= 1e-7 * std::fabs(alpha[0])) { converged = true; break; }          // invariant subspace
     }
+    c->last_lanczos_iters = m;
     std::vector<float> cf(ccur.begin(), ccur.end());
     PSE_TRY(upload_coefs(c, cf));
     { ScopedPhase ph(c, PSE_T_VECTOR);
@@ -310,14 +321,14 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     { ScopedPhase ph(c, PSE_T_VECTOR);
       k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(w, 0, 1, w, n4, c->d_scal); KERNEL_CHECK(c);
       k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V, w, c->d_scal, n4); KERNEL_CHECK(c); }
-    PSE_TRY(read_scalars(c, 1));
-    const double bnorm = std::sqrt(c->h_scal[0]);
+    double bnorm = 0;                                               // |b| arrives with the first read-back
     int m = 0;
     std::vector<double> H((size_t)(maxit + 1) * maxit, 0.0), cs(maxit, 0.0), sn(maxit, 0.0), g(maxit + 1, 0.0), y;
-    bool converged = !(bnorm > 0);
-    if (!converged) {
-        g[0] = bnorm;
-        for (int k = 0; k < maxit; ++k) {
+    bool converged = false;
+    {
+        const int first_check = std::max(0, c->last_gmres_iters - 2);     // see pse_lanczos_sqrt
+        int examined = 0;
+        for (int k = 0; k < maxit && !converged; ++k) {
             const int base = 1 + k * (k + 3) / 2;
             float4 *Zk = Z + (size_t)k * n4;
             PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH, PSE_IN_S | PSE_OUT_E));   // M_ES v_k: 5 grids in, 5 out
@@ -326,22 +337,32 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
               k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, Zk, n4, c->d_scal + base); KERNEL_CHECK(c);
               k_gs_update<<<vgrid((size_t)N), VT, 0, c->stream>>>(w, Zk, V, n4, k + 1, c->d_scal + base, N, c->d_scal + base + k + 1); KERNEL_CHECK(c);
               if (k + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V + (size_t)(k + 1) * n4, w, c->d_scal + base + k + 1, n4); KERNEL_CHECK(c); } }
-            PSE_TRY(read_scalars(c, base + k + 2));                  // one read-back per iteration
-            for (int j = 0; j <= k; ++j) H[(size_t)j * maxit + k] = c->h_scal[base + j];
-            const double hk1 = std::sqrt(c->h_scal[base + k + 1]);
-            H[(size_t)(k + 1) * maxit + k] = hk1;
-            for (int j = 0; j < k; ++j) {                        // apply previous Givens rotations to column k
-                double a = H[(size_t)j * maxit + k], b = H[(size_t)(j + 1) * maxit + k];
-                H[(size_t)j * maxit + k] = cs[j] * a + sn[j] * b; H[(size_t)(j + 1) * maxit + k] = -sn[j] * a + cs[j] * b;
+            if (k < first_check && k + 1 < maxit) continue;
+            PSE_TRY(read_scalars(c, base + k + 2));
+            if (examined == 0) {
+                bnorm = std::sqrt(c->h_scal[0]);
+                if (!(bnorm > 0)) { converged = true; break; }          // zero right-hand side: S = 0
+                g[0] = bnorm;
             }
-            double a = H[(size_t)k * maxit + k], b = H[(size_t)(k + 1) * maxit + k], r = std::hypot(a, b);
-            cs[k] = r > 0 ? a / r : 1.0; sn[k] = r > 0 ? b / r : 0.0;
-            H[(size_t)k * maxit + k] = r; H[(size_t)(k + 1) * maxit + k] = 0.0;
-            g[k + 1] = -sn[k] * g[k]; g[k] = cs[k] * g[k];
-            m = k + 1;
-            if (std::fabs(g[k + 1]) <= c->tol * bnorm) { converged = true; break; }
-            if (hk1 <= 1e-12 * bnorm) { converged = true; break; }
+            for (; examined <= k && !converged; ++examined) {
+                const int e = examined, eb = 1 + e * (e + 3) / 2;
+                for (int j = 0; j <= e; ++j) H[(size_t)j * maxit + e] = c->h_scal[eb + j];
+                const double hk1 = std::sqrt(c->h_scal[eb + e + 1]);
+                H[(size_t)(e + 1) * maxit + e] = hk1;
+                for (int j = 0; j < e; ++j) {                        // apply previous Givens rotations to column e
+                    double a = H[(size_t)j * maxit + e], b = H[(size_t)(j + 1) * maxit + e];
+                    H[(size_t)j * maxit + e] = cs[j] * a + sn[j] * b; H[(size_t)(j + 1) * maxit + e] = -sn[j] * a + cs[j] * b;
+                }
+                double a = H[(size_t)e * maxit + e], b = H[(size_t)(e + 1) * maxit + e], r = std::hypot(a, b);
+                cs[e] = r > 0 ? a / r : 1.0; sn[e] = r > 0 ? b / r : 0.0;
+                H[(size_t)e * maxit + e] = r; H[(size_t)(e + 1) * maxit + e] = 0.0;
+                g[e + 1] = -sn[e] * g[e]; g[e] = cs[e] * g[e];
+                m = e + 1;
+                if (std::fabs(g[e + 1]) <= c->tol * bnorm) converged = true;
+                else if (hk1 <= 1e-12 * bnorm) converged = true;
+            }
         }
+        c->last_gmres_iters = m;
         y.assign(m, 0.0);
         for (int i = m - 1; i >= 0; --i) {
             double s = g[i];

@@ -65,6 +65,7 @@ struct pse_ctx {
     double *d_scal = nullptr;                // device scalars (dots, norms)
     double *h_scal = nullptr;                // pinned mirror
     float *d_coef = nullptr;                 // small coefficient vector upload
+    int last_lanczos_iters = 0, last_gmres_iters = 0;   // iteration counts of the previous solves (when to start reading back)
     unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
     float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
     float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
