@@ -6,7 +6,10 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <cooperative_groups.h>
 #include "pse_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -115,23 +118,6 @@ __global__ void __launch_bounds__(VT) k_constraint_result(float4 *out, const flo
 // accumulated into, so an iteration needs one host read-back (for the tiny T / Hessenberg algebra and the stopping
 // test) instead of a read-back plus a coefficient upload per reduction. ----
 
-// Lanczos three-term update: u -= alpha v_j + beta_{j-1} v_{j-1};  *beta2_out += |u|^2
-__global__ void __launch_bounds__(VT) k_lanczos_update(float4 *u, const float4 *vj, const float4 *vjm1, const double *alpha,
-                                                       const double *beta2_prev, size_t n4, double *beta2_out) {
-    const float a = (float)*alpha, b = beta2_prev ? (float)sqrt(*beta2_prev) : 0.f;
-    double acc = 0;
-    for (size_t i = (size_t)blockIdx.x * VT + threadIdx.x; i < n4; i += (size_t)gridDim.x * VT) {
-        float4 x = u[i];
-        const float4 v = vj[i];
-        x.x -= a * v.x; x.y -= a * v.y; x.z -= a * v.z; x.w -= a * v.w;
-        if (vjm1) { const float4 p = vjm1[i]; x.x -= b * p.x; x.y -= b * p.y; x.z -= b * p.z; x.w -= b * p.w; }
-        u[i] = x;
-        acc += (double)(x.x * x.x + x.y * x.y) + (double)(x.z * x.z + x.w * x.w);
-    }
-    acc = block_sum(acc);
-    if (threadIdx.x == 0) atomicAdd(beta2_out, acc);
-}
-
 // dst = src / sqrt(*norm2)   (dst = 0 if the norm vanishes)
 __global__ void __launch_bounds__(VT) k_scale_dev(float4 *dst, const float4 *src, const double *norm2, size_t n4) {
     const double n2 = *norm2;
@@ -143,11 +129,71 @@ __global__ void __launch_bounds__(VT) k_scale_dev(float4 *dst, const float4 *src
     }
 }
 
-// Gram-Schmidt step of GMRES fused with the E-part embedding: w = Epart(Z) - sum_j h[j] V_j;  *norm2 += |w|^2
-__global__ void __launch_bounds__(VT) k_gs_update(float4 *w, const float4 *Z, const float4 *V, size_t stride4, int nvec, const double *h,
-                                                  int N, double *norm2) {
+// ---- one cooperative launch per Krylov iteration: the three dependent vector passes (dots, update + norm, scale)
+// are separated by grid barriers instead of kernel boundaries; the vectors (2 MB at N = 65536) stay in L2 ----
+
+// Lanczos:  alpha = <v_j, u>;  u -= alpha v_j + beta_{j-1} v_{j-1};  beta_j^2 = |u|^2;  v_{j+1} = u / beta_j
+__global__ void __launch_bounds__(VT) k_lanczos_step(float4 *u, const float4 *vj, const float4 *vjm1, float4 *vnext, double *alpha,
+                                                     const double *beta2_prev, double *beta2_out, size_t n4) {
+    cg::grid_group grid = cg::this_grid();
+    const size_t i0 = (size_t)blockIdx.x * VT + threadIdx.x, step = (size_t)gridDim.x * VT;
     double acc = 0;
-    for (int s = blockIdx.x * VT + threadIdx.x; s < N; s += gridDim.x * VT) {
+    for (size_t i = i0; i < n4; i += step) {
+        const float4 a = vj[i], b = u[i];
+        acc += (double)(a.x * b.x + a.y * b.y) + (double)(a.z * b.z + a.w * b.w);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) atomicAdd(alpha, acc);
+    grid.sync();
+    const float a = (float)*alpha, b = beta2_prev ? (float)sqrt(*beta2_prev) : 0.f;
+    acc = 0;
+    for (size_t i = i0; i < n4; i += step) {
+        float4 x = u[i];
+        const float4 v = vj[i];
+        x.x -= a * v.x; x.y -= a * v.y; x.z -= a * v.z; x.w -= a * v.w;
+        if (vjm1) { const float4 p = vjm1[i]; x.x -= b * p.x; x.y -= b * p.y; x.z -= b * p.z; x.w -= b * p.w; }
+        u[i] = x;
+        acc += (double)(x.x * x.x + x.y * x.y) + (double)(x.z * x.z + x.w * x.w);
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) atomicAdd(beta2_out, acc);
+    if (!vnext) return;                                       // uniform over the grid
+    grid.sync();
+    const double n2 = *beta2_out;
+    const float sc = n2 > 0 ? (float)(1.0 / sqrt(n2)) : 0.f;
+    for (size_t i = i0; i < n4; i += step) {
+        float4 x = u[i];                                      // this thread's own writes of the pass above
+        x.x *= sc; x.y *= sc; x.z *= sc; x.w *= sc;
+        vnext[i] = x;
+    }
+}
+
+// Arnoldi:  h_j = <V_j, Z> (j < nvec);  w = Epart(Z) - sum_j h_j V_j;  h_{nvec} = |w|^2;  V_{nvec} = w / |w|
+__global__ void __launch_bounds__(VT) k_arnoldi_step(float4 *w, const float4 *Z, const float4 *V, size_t stride4, int nvec, double *h,
+                                                     float4 *vnext, int N) {
+    cg::grid_group grid = cg::this_grid();
+    const int s0 = blockIdx.x * VT + threadIdx.x, step = gridDim.x * VT;
+    for (int j0 = 0; j0 < nvec; j0 += 4) {                   // four dots per pass over Z
+        double acc[4] = {0, 0, 0, 0};
+        for (int s = s0; s < N; s += step) {
+            const float4 za = Z[2 * s], zb = Z[2 * s + 1];
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                if (j0 + jj < nvec) {
+                    const float4 va = V[(size_t)(j0 + jj) * stride4 + 2 * s], vb = V[(size_t)(j0 + jj) * stride4 + 2 * s + 1];
+                    acc[jj] += (double)(va.x * za.x + va.y * za.y) + (double)(va.z * za.z + va.w * za.w)
+                             + (double)(vb.x * zb.x + vb.y * zb.y) + (double)(vb.z * zb.z + vb.w * zb.w);
+                }
+            }
+        }
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            if (j0 + jj < nvec) { const double r = block_sum(acc[jj]); if (threadIdx.x == 0) atomicAdd(h + j0 + jj, r); }
+        }
+    }
+    grid.sync();
+    double acc = 0;
+    for (int s = s0; s < N; s += step) {
         float4 a = Z[2 * s], b = Z[2 * s + 1];
         a.x = a.y = a.z = 0.f;
         for (int j = 0; j < nvec; ++j) {
@@ -159,7 +205,30 @@ __global__ void __launch_bounds__(VT) k_gs_update(float4 *w, const float4 *Z, co
         acc += (double)(a.w * a.w + b.x * b.x) + (double)(b.y * b.y + b.z * b.z) + (double)(b.w * b.w);
     }
     acc = block_sum(acc);
-    if (threadIdx.x == 0) atomicAdd(norm2, acc);
+    if (threadIdx.x == 0) atomicAdd(h + nvec, acc);
+    if (!vnext) return;
+    grid.sync();
+    const double n2 = h[nvec];
+    const float sc = n2 > 0 ? (float)(1.0 / sqrt(n2)) : 0.f;
+    for (int s = s0; s < N; s += step) {
+        float4 a = w[2 * s], b = w[2 * s + 1];
+        a.x *= sc; a.y *= sc; a.z *= sc; a.w *= sc; b.x *= sc; b.y *= sc; b.z *= sc; b.w *= sc;
+        vnext[2 * s] = a; vnext[2 * s + 1] = b;
+    }
+}
+
+// grid of a cooperative launch: every CTA must be resident
+template <typename K>
+int coop_grid(K kernel, size_t work_items) {
+    static int cap = 0;
+    if (!cap) {
+        int dev = 0, nsm = 0, per_sm = 0;
+        cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, VT, 0);
+        cap = nsm * std::max(1, per_sm);
+    }
+    const size_t b = (work_items + 2 * VT - 1) / (2 * VT);          // at least two items per thread: fewer CTAs at the barriers
+    return (int)std::max<size_t>(1, std::min<size_t>(b, (size_t)cap));
 }
 
 // cyclic Jacobi eigen-decomposition of a small symmetric matrix (n <= 51), fp64, host
@@ -258,10 +327,14 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
         float4 *vj = V + (size_t)j * n4;
         PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
         { ScopedPhase ph(c, PSE_T_VECTOR);
-          k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(vj, 0, 1, u, n4, c->d_scal + 1 + 2 * j); KERNEL_CHECK(c);
-          k_lanczos_update<<<vgrid(n4), VT, 0, c->stream>>>(u, vj, j ? vj - n4 : nullptr, c->d_scal + 1 + 2 * j, j ? c->d_scal + 2 * j : nullptr,
-                                                           n4, c->d_scal + 2 + 2 * j); KERNEL_CHECK(c);
-          if (j + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(vj + n4, u, c->d_scal + 2 + 2 * j, n4); KERNEL_CHECK(c); } }
+          const float4 *a_vj = vj, *a_vjm1 = j ? vj - n4 : nullptr;
+          float4 *a_u = u, *a_next = j + 1 < maxit ? vj + n4 : nullptr;
+          double *a_alpha = c->d_scal + 1 + 2 * j, *a_b2 = c->d_scal + 2 + 2 * j;
+          const double *a_b2prev = j ? c->d_scal + 2 * j : nullptr;
+          size_t a_n4 = n4;
+          void *args[] = {&a_u, &a_vj, &a_vjm1, &a_next, &a_alpha, &a_b2prev, &a_b2, &a_n4};
+          CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_lanczos_step, dim3(coop_grid(k_lanczos_step, n4)), dim3(VT), args, 0, c->stream));
+          KERNEL_CHECK(c); }
         if (j < first_check && j + 1 < maxit) continue;
         PSE_TRY(read_scalars(c, 3 + 2 * j));
         for (; examined <= j && !converged; ++examined) {
@@ -334,9 +407,13 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
             PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH, PSE_IN_S | PSE_OUT_E));   // M_ES v_k: 5 grids in, 5 out
             { ScopedPhase ph(c, PSE_T_VECTOR);
               // the velocity slots of every V_j are zero, so <V_j, Z_k> over all 8 components is the E-part product
-              k_multi_dot<<<vgrid(n4), VT, 0, c->stream>>>(V, n4, k + 1, Zk, n4, c->d_scal + base); KERNEL_CHECK(c);
-              k_gs_update<<<vgrid((size_t)N), VT, 0, c->stream>>>(w, Zk, V, n4, k + 1, c->d_scal + base, N, c->d_scal + base + k + 1); KERNEL_CHECK(c);
-              if (k + 1 < maxit) { k_scale_dev<<<vgrid(n4), VT, 0, c->stream>>>(V + (size_t)(k + 1) * n4, w, c->d_scal + base + k + 1, n4); KERNEL_CHECK(c); } }
+              float4 *a_w = w, *a_next = k + 1 < maxit ? V + (size_t)(k + 1) * n4 : nullptr;
+              const float4 *a_Z = Zk, *a_V = V;
+              size_t a_stride = n4; int a_nvec = k + 1, a_N = N;
+              double *a_h = c->d_scal + base;
+              void *args[] = {&a_w, &a_Z, &a_V, &a_stride, &a_nvec, &a_h, &a_next, &a_N};
+              CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_arnoldi_step, dim3(coop_grid(k_arnoldi_step, (size_t)N)), dim3(VT), args, 0, c->stream));
+              KERNEL_CHECK(c); }
             if (k < first_check && k + 1 < maxit) continue;
             PSE_TRY(read_scalars(c, base + k + 2));
             if (examined == 0) {

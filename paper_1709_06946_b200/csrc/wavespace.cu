@@ -20,7 +20,6 @@ namespace {
 
 constexpr int T = PSE_TILE;
 constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
-constexpr float TWO_PI = 6.283185307179586f;
 
 // support base (unwrapped, may be negative) and grid coordinate g = x/h   (reading R5)
 __device__ __forceinline__ int support_base(float g, int P) {
