@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
 constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32;
 
 __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
-                                                                   float L, float invL, float rc2, int *__restrict__ count,
+                                                                   float L, float invL, float rc2, float band, int *__restrict__ count,
                                                                    unsigned long long *__restrict__ off, int *__restrict__ idx,
                                                                    unsigned long long cap, unsigned long long *__restrict__ cursor,
                                                                    int *__restrict__ fallback) {
@@ -307,11 +307,18 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
         if (tid == 0) atomicExch(fallback, 1);
         return;
     }
+    // Screening: with >= 5 cells per edge every candidate has one periodic image within reach of the whole cell, so it is
+    // staged already shifted to that image and the test is a plain difference.  The decision itself stays the R16
+    // arithmetic: whenever the screened d^2 falls within `band` of r_c^2 (far wider than the rounding difference between
+    // the two forms) the pair is re-evaluated with dist2 on the unshifted position.
+    const bool fast = nc >= 5;
+    const float edge = L / (float)nc, mx = ((float)cx + 0.5f) * edge, my = ((float)cy + 0.5f) * edge, mz = ((float)cz + 0.5f) * edge;
     for (int c = tid; c < total; c += NS_THREADS) {
         int r = 0;
         while (run_cum[r + 1] <= c) ++r;
         const int j = run_lo[r] + c - run_cum[r];
         float4 q = pos[j];
+        if (fast) { q.x -= L * rintf((q.x - mx) * invL); q.y -= L * rintf((q.y - my) * invL); q.z -= L * rintf((q.z - mz) * invL); }
         q.w = __int_as_float(j);
         cpos[c] = q;
     }
@@ -323,8 +330,22 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
         int found = 0;
         for (int w = 0; w < nwords; ++w) {
             const int c = w * 32 + lane;
-            bool in = false;
-            if (c < total) { const float4 q = cpos[c]; in = (__float_as_int(q.w) != s) && dist2(p, q, L, invL) < rc2; }
+            bool in = false, exact = false;
+            float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+            int j = s;
+            if (c < total) { q = cpos[c]; j = __float_as_int(q.w); }
+            if (j != s) {
+                if (fast) {
+                    const float dx = p.x - q.x, dy = p.y - q.y, dz = p.z - q.z, d2 = dx * dx + dy * dy + dz * dz;
+                    in = d2 < rc2;
+                    exact = fabsf(d2 - rc2) <= band;
+                } else {
+                    exact = true;
+                }
+            }
+            if (__any_sync(0xffffffffu, exact)) {                // rare on the screened path: a real branch, not predication
+                if (exact) in = dist2(p, fast ? pos[j] : q, L, invL) < rc2;
+            }
             const unsigned m = __ballot_sync(0xffffffffu, in);
             if (lane == 0) masks[pi][w] = m;
             found += __popc(m);
@@ -346,16 +367,21 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     }
     __syncthreads();
     const unsigned long long base = base_s;
-    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks
+    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks, a lane per 32-candidate word
         const int s = first + pi;
         const unsigned long long o = base + (unsigned long long)loc[pi];
         if (lane == 0) { off[s] = o; count[s] = cnt[pi]; }
         if (o + (unsigned long long)cnt[pi] > cap) continue;  // overflow: the host re-runs with a larger index array
-        int found = 0;
-        for (int w = 0; w < nwords; ++w) {
-            const unsigned m = masks[pi][w];
-            if ((m >> lane) & 1u) idx[o + found + __popc(m & ((1u << lane) - 1))] = __float_as_int(cpos[w * 32 + lane].w);
-            found += __popc(m);
+        unsigned m = lane < nwords ? masks[pi][lane] : 0u;
+        const int mine = __popc(m);
+        int inc = mine;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        int *dst = idx + o + (inc - mine);
+        while (m) {                                           // ascending bit order keeps the list sorted by candidate
+            const int b = __ffs(m) - 1;
+            m &= m - 1;
+            *dst++ = __float_as_int(cpos[lane * 32 + b].w);
         }
     }
 }
@@ -413,6 +439,7 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     const int N = c->N, T = 256, nb = (N + T - 1) / T;
     const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
     const float rc = (float)c->rcut, rc2 = rc * rc;
+    const float band = 32.f * rc * L * 1.2e-7f;          // >> 2 r_c ulp(L): rounding gap between screened and R16 distances
     c->have_nbrs = false;
     CUDA_TRY(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
     CUDA_TRY(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
@@ -432,7 +459,7 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     bool done = false;
     for (int attempt = 0; attempt < 3 && !done; ++attempt) {
         CUDA_TRY(c, cudaMemsetAsync(c->d_nbr_ctl, 0, 2 * sizeof(unsigned long long), c->stream));
-        neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count, c->d_nbr_off,
+        neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
                                                                    c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
                                                                    reinterpret_cast<int *>(c->d_nbr_ctl + 1)); KERNEL_CHECK(c);
         CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));

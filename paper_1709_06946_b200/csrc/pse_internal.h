@@ -55,9 +55,14 @@ struct pse_ctx {
     int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]
-    cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
+    cufftComplex *d_spec = nullptr;          // [8][M][M][Mhp]
     cufftHandle plan_r2c[3] = {0, 0, 0}, plan_c2r[3] = {0, 0, 0};   // [0] all 8 grids, [1] planes 0-2 (F / U), [2] planes 3-7 (S / E)
     void *d_fft_work = nullptr; int nplans = 0;
+    bool own_fft = false;                    // fft.cu serves this grid size (else cuFFT)
+    float *d_fft_tw = nullptr;               // [M][2] twiddles exp(-2 pi i n / M)
+    void *d_fft_dev = nullptr;               // plan record of fft.cu
+    size_t fft_smem_plane = 0, fft_smem_x = 0;
+    int Mhp = 0;                             // row pitch of d_spec in complex entries (Mh, or padded to a multiple of 4 by fft.cu)
     // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
     float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
     float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]
@@ -136,6 +141,12 @@ void pse_wave_free(pse_ctx *c);
 pse_status pse_tile_bins(pse_ctx *c);
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp = nullptr, int mode = PSE_MODE_ALL);   // out (+)= M_w in
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
+// fft.cu
+pse_status pse_fft_init(pse_ctx *c);
+pse_status pse_fft_forward_planes(pse_ctx *c, int first, int ncomp);
+pse_status pse_fft_x_scale(pse_ctx *c, int mode);
+pse_status pse_fft_x_inverse(pse_ctx *c);
+pse_status pse_fft_inverse_planes(pse_ctx *c, int first, int ncomp);
 // krylov.cu
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted
 pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed);

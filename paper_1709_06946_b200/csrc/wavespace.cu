@@ -15,11 +15,11 @@
 #include <algorithm>
 #include <cuda_pipeline.h>
 #include "pse_internal.h"
+#include "wave_scale.cuh"
 
 namespace {
 
 constexpr int T = PSE_TILE;
-constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
 
 // support base (unwrapped, may be negative) and grid coordinate g = x/h   (reading R5)
 __device__ __forceinline__ int support_base(float g, int P) {
@@ -384,97 +384,12 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     }
 }
 
-struct ScaleParams {
-    int M, Mh;
-    float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
-    const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
-    int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
-};
-
-__device__ __forceinline__ float shape_s1(float x) {     // 3 (sin x - x cos x)/x^3, series below 0.5 (cancellation)
-    if (x < 0.5f) { float x2 = x * x; return 1.f - x2 * (0.1f - x2 * (1.f / 280.f - x2 * (1.f / 15120.f))); }
-    float s, c; sincosf(x, &s, &c);
-    return 3.f * (s - x * c) / (x * x * x);
-}
-
-// Wave vector of half-spectrum entry (ix,iy,iz); returns false for k = 0 and Nyquist modes (weight set to zero in
-// both the product and the Brownian factor, reading R8).
-__device__ __forceinline__ bool mode_k(const ScaleParams &sp, int ix, int iy, int iz, float &kx, float &ky, float &kz) {
-    const int M = sp.M, half = (M + 1) / 2;
-    const int nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M, nz = iz;
-    const bool nyq = !(M & 1) && (ix == M / 2 || iy == M / 2 || iz == M / 2);
-    kx = sp.two_pi_over_L * (float)nx; ky = sp.two_pi_over_L * (float)ny; kz = sp.two_pi_over_L * (float)nz;
-    return !(nyq || (nx == 0 && ny == 0 && nz == 0));
-}
-
-// Given uh (3 complex, already carrying B or sqrt(B) and the projector), write the 8 outputs of P^H (Eq. 41):
-//   Uh = s0 uh ;  Eh^q = i s1 (e^q k).uh
-__device__ __forceinline__ void write_outputs(cufftComplex *spec, size_t stride, size_t o, float s0, float s1,
-                                              float kx, float ky, float kz, float2 ux, float2 uy, float2 uz, int mode) {
-    if (mode & PSE_OUT_U) {
-        spec[o] = make_float2(s0 * ux.x, s0 * ux.y);
-        spec[stride + o] = make_float2(s0 * uy.x, s0 * uy.y);
-        spec[2 * stride + o] = make_float2(s0 * uz.x, s0 * uz.y);
-    }
-    if (!(mode & PSE_OUT_E)) return;
-    // i*s1*z = s1 * (-z.im, z.re)
-    float2 pxx = make_float2(kx * ux.x, kx * ux.y), pyy = make_float2(ky * uy.x, ky * uy.y), pzz = make_float2(kz * uz.x, kz * uz.y);
-    float2 d1 = make_float2((pxx.x - pyy.x) * RS2, (pxx.y - pyy.y) * RS2);
-    float2 d2 = make_float2((2.f * pzz.x - pxx.x - pyy.x) * RS6, (2.f * pzz.y - pxx.y - pyy.y) * RS6);
-    float2 d3 = make_float2((kx * uy.x + ky * ux.x) * RS2, (kx * uy.y + ky * ux.y) * RS2);
-    float2 d4 = make_float2((kx * uz.x + kz * ux.x) * RS2, (kx * uz.y + kz * ux.y) * RS2);
-    float2 d5 = make_float2((ky * uz.x + kz * uy.x) * RS2, (ky * uz.y + kz * uy.y) * RS2);
-    spec[3 * stride + o] = make_float2(-s1 * d1.y, s1 * d1.x);
-    spec[4 * stride + o] = make_float2(-s1 * d2.y, s1 * d2.x);
-    spec[5 * stride + o] = make_float2(-s1 * d3.y, s1 * d3.x);
-    spec[6 * stride + o] = make_float2(-s1 * d4.y, s1 * d4.x);
-    spec[7 * stride + o] = make_float2(-s1 * d5.y, s1 * d5.x);
-}
-
-// a5: fh = s0 Fh - i s1 (Sh.k);  uh = Bt(k) (I - kh kh) fh  with  Bt = c_mv (1+k^2/4xi^2) exp(-(1-eta_g) k^2/4xi^2)/(eta k^2)
+// a5 (cuFFT path): one thread per half-spectrum mode, in place
 __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScaleParams sp) {
     const size_t nmode = (size_t)sp.M * sp.M * sp.Mh, o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= nmode) return;
     const int iz = (int)(o % sp.Mh), iy = (int)((o / sp.Mh) % sp.M), ix = (int)(o / ((size_t)sp.Mh * sp.M));
-    float kx, ky, kz;
-    float2 zero = make_float2(0.f, 0.f);
-    if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
-#pragma unroll
-        for (int c = 0; c < 8; ++c)
-            if (sp.mode & (c < 3 ? PSE_OUT_U : PSE_OUT_E)) spec[c * nmode + o] = zero;
-        return;
-    }
-    const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
-    const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
-    const float q = k2 * sp.inv4xi2;
-    const float dw = __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);            // one window undone for spreading,
-    const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-q) / k2 * dw * dw;          // one for interpolation
-    float2 F[3], S[5];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) F[c] = (sp.mode & PSE_IN_F) ? spec[c * nmode + o] : zero;
-#pragma unroll
-    for (int c = 0; c < 5; ++c) S[c] = (sp.mode & PSE_IN_S) ? spec[(3 + c) * nmode + o] : zero;
-    // (S.k)_i from the 5 coordinates
-    float2 sk[3];
-#pragma unroll
-    for (int ri = 0; ri < 2; ++ri) {
-        float s1c = ri ? S[0].y : S[0].x, s2c = ri ? S[1].y : S[1].x, s3c = ri ? S[2].y : S[2].x, s4c = ri ? S[3].y : S[3].x,
-              s5c = ri ? S[4].y : S[4].x;
-        float sxx = s1c * RS2 - s2c * RS6, syy = -s1c * RS2 - s2c * RS6, szz = 2.f * s2c * RS6;
-        float sxy = s3c * RS2, sxz = s4c * RS2, syz = s5c * RS2;
-        float vx = sxx * kx + sxy * ky + sxz * kz, vy = sxy * kx + syy * ky + syz * kz, vz = sxz * kx + syz * ky + szz * kz;
-        if (ri) { sk[0].y = vx; sk[1].y = vy; sk[2].y = vz; } else { sk[0].x = vx; sk[1].x = vy; sk[2].x = vz; }
-    }
-    // fh = s0 F - i s1 sk = s0 F + s1 (sk.im, -sk.re)
-    float2 f[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) f[c] = make_float2(s0 * F[c].x + s1 * sk[c].y, s0 * F[c].y - s1 * sk[c].x);
-    const float ik2 = 1.f / k2;
-    const float2 kf = make_float2((kx * f[0].x + ky * f[1].x + kz * f[2].x) * ik2, (kx * f[0].y + ky * f[1].y + kz * f[2].y) * ik2);
-    const float2 ux = make_float2(Bt * (f[0].x - kx * kf.x), Bt * (f[0].y - kx * kf.y));
-    const float2 uy = make_float2(Bt * (f[1].x - ky * kf.x), Bt * (f[1].y - ky * kf.y));
-    const float2 uz = make_float2(Bt * (f[2].x - kz * kf.x), Bt * (f[2].y - kz * kf.y));
-    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, sp.mode);
+    scale_point(sp, ix, iy, iz, spec, nmode, o, spec, nmode, o);
 }
 
 // a5, Brownian flavour (Eq. 75): uh = c_br sqrt((1+k^2/4xi^2)/(eta k^2)) exp(-(1-eta_g) k^2/8xi^2) (I - kh kh) W(k),
@@ -487,9 +402,11 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const int iz = (int)(o % sp.Mh), iy = (int)((o / sp.Mh) % M), ix = (int)(o / ((size_t)sp.Mh * M));
     float kx, ky, kz;
     float2 zero = make_float2(0.f, 0.f);
+    // the noise buffer has the ABI's [M][M][Mh] layout; the spectrum rows may be padded to Mhp entries
+    const size_t oplane = (size_t)M * M * sp.Mhp, oo = ((size_t)ix * M + iy) * sp.Mhp + iz;
     if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) spec[c * nmode + o] = zero;
+        for (int c = 0; c < 8; ++c) spec[c * oplane + oo] = zero;
         return;
     }
     const int half = (M + 1) / 2, nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M;
@@ -498,7 +415,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float sgn = canon ? 1.f : -1.f;
     float2 W[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { float2 g = noise[c * nmode + src]; W[c] = make_float2(g.x * RS2, sgn * g.y * RS2); }
+    for (int c = 0; c < 3; ++c) { float2 g = noise[c * nmode + src]; W[c] = make_float2(g.x * WS_RS2, sgn * g.y * WS_RS2); }
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
     const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
     const float q = k2 * sp.inv4xi2;
@@ -508,7 +425,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float2 ux = make_float2(Bh * (W[0].x - kx * kw.x), Bh * (W[0].y - kx * kw.y));
     const float2 uy = make_float2(Bh * (W[1].x - ky * kw.x), Bh * (W[1].y - ky * kw.y));
     const float2 uz = make_float2(Bh * (W[2].x - kz * kw.x), Bh * (W[2].y - kz * kw.y));
-    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
+    write_outputs(spec, oplane, oo, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
 }
 
 }  // namespace
@@ -517,7 +434,8 @@ pse_status pse_wave_init(pse_ctx *c) {
     const int M = c->M;
     c->Mh = M / 2 + 1;
     c->nt = (M + T - 1) / T; c->ntile = c->nt * c->nt * c->nt;
-    const size_t M3 = (size_t)M * M * M, nmode = (size_t)M * M * c->Mh;
+    PSE_TRY(pse_fft_init(c));                          // decides own FFT vs cuFFT and with it the spectrum pitch
+    const size_t M3 = (size_t)M * M * M, nmode = (size_t)M * M * c->Mhp;
     CUDA_TRY(c, cudaMalloc(&c->d_grid, 8 * M3 * sizeof(float)));
     CUDA_TRY(c, cudaMalloc(&c->d_spec, 8 * nmode * sizeof(cufftComplex)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_count, (size_t)(c->ntile + 1) * sizeof(int)));
@@ -525,6 +443,7 @@ pse_status pse_wave_init(pse_ctx *c) {
     CUDA_TRY(c, cudaMalloc(&c->d_tile_fill, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
+    if (c->own_fft) return PSE_OK;                    // fft.cu serves this size: no cuFFT plans, no work area
     int n[3] = {M, M, M};
     const int batches[3] = {8, 3, 5};                 // all grids | planes 0-2 (F in, U out) | planes 3-7 (S in, E out)
     size_t w = 0;
@@ -546,7 +465,7 @@ pse_status pse_wave_init(pse_ctx *c) {
 
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
-    cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
+    cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work); cudaFree(c->d_fft_tw); cudaFree(c->d_fft_dev);
     cudaFree(c->d_tile_count); cudaFree(c->d_tile_start); cudaFree(c->d_tile_fill); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
 }
 
@@ -561,18 +480,6 @@ pse_status pse_tile_bins(pse_ctx *c) {
     return PSE_OK;
 }
 
-static ScaleParams make_scale_params(const pse_ctx *c, int mode = PSE_MODE_ALL) {
-    ScaleParams sp;
-    sp.mode = mode;
-    sp.M = c->M; sp.Mh = c->Mh;
-    sp.two_pi_over_L = (float)(2.0 * M_PI / c->L); sp.a = (float)c->a;
-    sp.inv4xi2 = (float)(1.0 / (4.0 * c->xi * c->xi)); sp.dec = c->d_dec;
-    const double V = c->L * c->L * c->L;
-    sp.c_mv = (float)(1.0 / V); sp.c_br = (float)(1.0 / std::sqrt(V));
-    sp.inv_eta = (float)(1.0 / c->eta);
-    return sp;
-}
-
 // plane range of a 2-bit component mask (bit 0: planes 0-2, bit 1: planes 3-7): plan index and first plane
 static inline void plane_range(int bits, int &plan, int &first) {
     plan = bits == 3 ? 0 : bits; first = bits == 2 ? 3 : 0;
@@ -584,7 +491,8 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
         int plan, first;
         plane_range((mode >> 2) & 3, plan, first);
         const size_t M3 = (size_t)c->M * c->M * c->M, nmode = (size_t)c->M * c->M * c->Mh;
-        CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++;
+        if (c->own_fft) PSE_TRY(pse_fft_inverse_planes(c, first, plan == 0 ? 8 : plan == 1 ? 3 : 5));
+        else { CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++; }
     }
     if (wait_ev) CUDA_TRY(c, cudaStreamWaitEvent(c->stream, wait_ev, 0));
     ScopedPhase ph(c, PSE_T_INTERP);
@@ -636,6 +544,11 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
         else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         KERNEL_CHECK(c);
     }
+    if (c->own_fft) {
+        { ScopedPhase ph(c, PSE_T_FFT_FWD); PSE_TRY(pse_fft_forward_planes(c, first, plan == 0 ? 8 : plan == 1 ? 3 : 5)); }
+        { ScopedPhase ph(c, PSE_T_SCALE); PSE_TRY(pse_fft_x_scale(c, mode)); }      // x transform, operator, inverse x transform
+        return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp, mode);
+    }
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[plan], c->d_grid + first * M3, c->d_spec + first * nmode)); c->launches++; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
@@ -651,6 +564,7 @@ pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out
         scale_brownian_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(
             c->d_spec, reinterpret_cast<const float2 *>(d_noise_wave), make_scale_params(c));
         KERNEL_CHECK(c);
+        if (c->own_fft) PSE_TRY(pse_fft_x_inverse(c));
     }
     return inverse_and_interpolate(c, d_out, accumulate);
 }
