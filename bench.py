@@ -27,7 +27,7 @@ WORKLOADS = {
     # name: N, phi, tol, xi, dt, relax sweeps          (BASELINE.json configs; xi is the free tuning knob)
     'tiny': dict(N=4096, phi=0.20, tol=1e-3, xi=0.5, dt=1e-3, relax=0),
     'config2': dict(N=4096, phi=0.20, tol=1e-4, xi=0.5, dt=1e-3, relax=0),
-    'config3': dict(N=65536, phi=0.30, tol=1e-3, xi=0.55, dt=1e-4, relax=2),
+    'config3': dict(N=65536, phi=0.30, tol=1e-3, xi=0.575, dt=1e-4, relax=2),   # largest xi that keeps the 100^3 grid
     'config4': dict(N=1048576, phi=0.10, tol=1e-3, xi=0.34, dt=1e-4, relax=0),
 }
 

@@ -43,6 +43,8 @@ def test_suggest_params_rules(pse):
     # above 64 the cheapest measured cuFFT size is taken (profiles/r1_cufft_sizes.md): 90 -> 90, 320 -> 343, 97 -> 100
     assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.5)[1] == 90
     assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.55)[1] == 100
+    assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.575)[1] == 100        # bench.py's config3
+    assert pse.pse_suggest_params(65536, 97.084, 1.0, 1e-3, 0.58)[1] == 108
     for tol, want in [(1e-2, 3), (1e-3, 4), (1e-4, 5)]:
         assert pse.pse_suggest_params(4096, 44.1, 1.0, tol, 0.5)[2] == want
     assert pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.3)[0] == pse.PSE_EINVAL      # rcut > L/2
