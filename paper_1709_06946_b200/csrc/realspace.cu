@@ -10,6 +10,7 @@
 // Tensor algebra per pair (rh = unit separation, f = rh.F, t = S rh, q = rh.t):
 //   U += F1 (F - rh f) + F2 rh f + Ga t - Gb rh q
 //   E += A S + sym(rh (x) w),  w = -Ga F + 2B t + (Gb f + D q) rh     (projected on e1..e5; trace terms drop out)
+#include <cstdlib>
 #include "pse_internal.h"
 
 namespace {
@@ -19,7 +20,7 @@ constexpr float RS6 = 0.40824829046386302f;   // 1/sqrt6
 
 // MODE = PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: terms of absent inputs / outputs are removed at compile time
 // (inside GMRES the operator is S -> E: no U accumulation, no F terms, and only the E-part table is read).
-template <int MODE>
+template <int MODE, int G>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
                   const unsigned long long *__restrict__ off, const int *__restrict__ cnt, const int *__restrict__ idx,
@@ -32,21 +33,26 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
     __syncthreads();
     constexpr bool INF = MODE & PSE_IN_F, INS = MODE & PSE_IN_S, OUTU = MODE & PSE_OUT_U, OUTE = MODE & PSE_OUT_E;
     constexpr bool NEED_TU = (OUTU) || (INF && OUTE), NEED_TE = INS && OUTE;
-    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
-    for (int s = blockIdx.x * wpb + (threadIdx.x >> 5); s < N; s += gridDim.x * wpb) {
-        const float4 p = pos[s];
+    // G lanes per particle (32 / G particles per warp): a list of ~51 entries fills 7 passes of 8 lanes to 91 %, two
+    // passes of 32 lanes only to 80 %
+    constexpr int PPW = 32 / G;
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5, gl = lane & (G - 1), grp = lane / G;
+    for (int ws = blockIdx.x * wpb + (threadIdx.x >> 5); ws * PPW < N; ws += gridDim.x * wpb) {
+        const int s = ws * PPW + grp;
+        const bool live = s < N;
+        const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
         float u0 = 0, u1 = 0, u2 = 0, e0 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
-        const unsigned long long lo = off[s], hi = lo + (unsigned long long)cnt[s];
+        const unsigned long long lo = live ? off[s] : 0ull, hi = lo + (unsigned long long)(live ? cnt[s] : 0);
         // software pipeline of depth one on the dependent chain idx -> pos: the next neighbour's index and position
         // are requested while the current pair is evaluated (ncu: 42 % of the stall samples sat on these two waits)
-        unsigned long long j = lo + lane;
+        unsigned long long j = lo + gl;
         int b = j < hi ? idx[j] : 0;
         float4 q4 = pos[b];
-        for (; j < hi; j += 32) {
+        for (; j < hi; j += G) {
             float4 a0 = in[2 * b], a1 = in[2 * b + 1];
             if (!INF) { a0.x = 0.f; a0.y = 0.f; a0.z = 0.f; }
             if (!INS) { a0.w = 0.f; a1 = make_float4(0.f, 0.f, 0.f, 0.f); }
-            const int bn = (j + 32 < hi) ? idx[j + 32] : b;
+            const int bn = (j + G < hi) ? idx[j + G] : b;
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
             const float r2 = dx * dx + dy * dy + dz * dz;
@@ -86,33 +92,62 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             b = bn;
             q4 = qn;
         }
-        // self term (r -> 0 limit: F1(0) F and A(0) S) added by lane 0 before the reduction
-        if (lane == 0) {
+        // self term (r -> 0 limit: F1(0) F and A(0) S) added by the group's first lane before the reduction
+        if (gl == 0 && live) {
             const float4 a0 = in[2 * s], a1 = in[2 * s + 1], t0 = tabU[0], t1 = tabE[0];
             if (INF && OUTU) { u0 += t0.x * a0.x; u1 += t0.x * a0.y; u2 += t0.x * a0.z; }
             if (INS && OUTE) { e0 += t1.x * a0.w; e1 += t1.x * a1.x; e2 += t1.x * a1.y; e3 += t1.x * a1.z; e4 += t1.x * a1.w; }
         }
         const float part[8] = {u0, u1, u2, e0, e1, e2, e3, e4};
-        int comp;
-        const float r = warp_reduce8(part, lane, comp);
-        if ((lane & 3) == 0) reinterpret_cast<float *>(out)[(size_t)s * 8 + comp] = r;
+        if (G == 32) {
+            int comp;
+            const float r = warp_reduce8(part, lane, comp);
+            if ((lane & 3) == 0 && live) reinterpret_cast<float *>(out)[(size_t)s * 8 + comp] = r;
+        } else {
+            // 8 sums over G lanes: every step halves the values a lane carries (4 + 2 + 1 shuffles for G = 8, where lane
+            // gl ends with component gl and the group stores 32 contiguous bytes)
+            constexpr int O1 = G / 2, O2 = G / 4;
+            const bool h1 = gl & O1, h2 = gl & O2;
+            float r4[4], r2[2];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) r4[c] = (h1 ? part[c + 4] : part[c]) + __shfl_xor_sync(0xffffffffu, h1 ? part[c] : part[c + 4], O1);
+#pragma unroll
+            for (int c = 0; c < 2; ++c) r2[c] = (h2 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h2 ? r4[c] : r4[c + 2], O2);
+            float *o = reinterpret_cast<float *>(out) + (size_t)s * 8 + (h1 ? 4 : 0) + (h2 ? 2 : 0);
+            if (G == 4) {
+                if (live) *reinterpret_cast<float2 *>(o) = make_float2(r2[0], r2[1]);
+            } else {
+                constexpr int O3 = G / 8;
+                const bool h3 = gl & O3;
+                float r = (h3 ? r2[1] : r2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? r2[0] : r2[1], O3);
+                if (G == 16) r += __shfl_xor_sync(0xffffffffu, r, 1);
+                if (live && (G == 8 || (gl & 1) == 0)) o[h3 ? 1 : 0] = r;
+            }
+        }
     }
 }
 
 }  // namespace
 
-template <int MODE>
-static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
+template <int MODE, int G>
+static pse_status launch_real_g(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
     static bool attr_set = false;
     if (!attr_set) {
-        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<MODE, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    real_pairs_kernel<MODE><<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
+    real_pairs_kernel<MODE, G><<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
                                                      c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
                                                      (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
     KERNEL_CHECK(c);
     return PSE_OK;
+}
+
+template <int MODE>
+static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
+    // measured (config 3 / config 4, us per launch): 32 lanes per particle 44.9 / 719, 16: 40.3 / 608, 8: 41.0 / 585, 4: 41.1 / 591
+    static const bool wide = getenv("PSE_PAIR_LANES") && atoi(getenv("PSE_PAIR_LANES")) == 32;
+    return wide ? launch_real_g<MODE, 32>(c, d_in, d_out, st, grid, smem) : launch_real_g<MODE, 8>(c, d_in, d_out, st, grid, smem);
 }
 
 pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int ctas_per_sm, int mode) {
