@@ -71,8 +71,25 @@ __global__ void scan_apply(const int *in, size_t n, const unsigned long long *bs
     if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = (OutT)bsum[nb];
 }
 
+// whole scan in one CTA for short inputs (cell and tile counts: a few thousand entries): one launch instead of three
+constexpr int SCAN1_THREADS = 1024, SCAN1_MAX = 1 << 14;
+template <typename OutT>
+__global__ void __launch_bounds__(SCAN1_THREADS) scan_single_cta(const int *in, int n, OutT *out) {
+    __shared__ unsigned long long tot;
+    const int per = (n + SCAN1_THREADS - 1) / SCAN1_THREADS, lo = threadIdx.x * per, hi = min(n, lo + per);
+    unsigned long long s = 0;
+    for (int i = lo; i < hi; ++i) s += (unsigned long long)in[i];
+    unsigned long long e = block_exclusive_scan(s, &tot);
+    for (int i = lo; i < hi; ++i) { out[i] = (OutT)e; e += (unsigned long long)in[i]; }
+    if (threadIdx.x == 0) out[n] = (OutT)tot;
+}
+
 template <typename OutT>
 pse_status scan_impl(pse_ctx *c, const int *d_in, OutT *d_out, size_t n) {
+    if (n <= (size_t)SCAN1_MAX && (const void *)d_in != (const void *)d_out) {
+        scan_single_cta<OutT><<<1, SCAN1_THREADS, 0, c->stream>>>(d_in, (int)n, d_out); KERNEL_CHECK(c);
+        return PSE_OK;
+    }
     size_t nb = (n + SCAN_CHUNK - 1) / SCAN_CHUNK;
     if (nb == 0) nb = 1;
     if (c->scan_tmp_n < nb + 1) {
@@ -399,26 +416,28 @@ __global__ void lists_to_original(const int *idx, const unsigned long long *off_
     for (unsigned long long j = lane; j < n; j += 32) out[dst + j] = order[idx[lo + j]];
 }
 
-// Heyes-Melrose overlap force (reading R12), warp per particle over the neighbour list, packed output.
+// Heyes-Melrose overlap force (reading R12), 8 lanes per particle over the neighbour list (as the pair kernel), packed output.
 __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off, const int *__restrict__ count,
                           const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out) {
-    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (s >= N) return;
-    float4 p = pos[s];
+    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, gl = threadIdx.x & 7;
+    const bool live = s < N;
+    const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
     float fx = 0, fy = 0, fz = 0;
-    for (unsigned long long j = off[s] + lane, hi = off[s] + (unsigned long long)count[s]; j < hi; j += 32) {
-        float4 q = pos[idx[j]];
-        float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
-        float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 < two_a * two_a && r2 > 0.f) {
-            float r = sqrtf(r2), g = coef * (two_a - r) / r;
-            fx += g * dx; fy += g * dy; fz += g * dz;
+    if (live) {
+        for (unsigned long long j = off[s] + gl, hi = off[s] + (unsigned long long)count[s]; j < hi; j += 8) {
+            float4 q = pos[idx[j]];
+            float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
+            float r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < two_a * two_a && r2 > 0.f) {
+                float r = sqrtf(r2), g = coef * (two_a - r) / r;
+                fx += g * dx; fy += g * dy; fz += g * dz;
+            }
         }
     }
-    for (int o = 16; o; o >>= 1) {
+    for (int o = 4; o; o >>= 1) {
         fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
     }
-    if (lane == 0) {
+    if (gl == 0 && live) {
         float4 *o4 = reinterpret_cast<float4 *>(out + (size_t)s * 8);
         o4[0] = make_float4(fx, fy, fz, 0.f); o4[1] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
@@ -517,7 +536,7 @@ pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {
     ScopedPhase ph(c, PSE_T_REAL);
     const int N = c->N, T = 256;
     float coef = (float)(3.0 * M_PI * c->eta * c->a / dt);
-    hs_forces<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, (float)c->L,
+    hs_forces<<<(unsigned)(((size_t)N * 8 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, (float)c->L,
                                                                             1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed);
     KERNEL_CHECK(c);
     return PSE_OK;
