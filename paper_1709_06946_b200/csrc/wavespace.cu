@@ -25,7 +25,8 @@ constexpr int T = PSE_TILE;
 __device__ __forceinline__ int support_base(float g, int P) {
     return (P & 1) ? (int)rintf(g) - (P - 1) / 2 : (int)floorf(g) - P / 2 + 1;
 }
-__device__ __forceinline__ int pmod(int i, int M) { int r = i % M; return r < 0 ? r + M : r; }
+// periodic index for arguments in [-M, 2M) (support bases and offsets never leave that range since P <= M): no division
+__device__ __forceinline__ int pmod(int i, int M) { i += i < 0 ? M : 0; return i >= M ? i - M : i; }
 
 // Exponent of the 1-D window at offset tt (grid units) from the particle.  wb == 0: the paper's Gaussian,
 // exp(-wa tt^2) with wa = 2 pi / P.  wb > 0: "exponential of semicircle" window
