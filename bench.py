@@ -330,6 +330,8 @@ def main():
         if name in ab:
             e['alg_GBps'] = ab[name] / (avg * 1e-3) / 1e9
             e['frac_of_hbm_peak'] = e['alg_GBps'] / peak
+        if name == 'real':                       # the pair kernel is not a streaming kernel: also report pair evaluations per second
+            e['pairs_per_sec'] = wl['N'] * r['nb_mean'] / (avg * 1e-3)
         phases[name] = e
     dom = max((p for p in phases if p in ab), key=lambda p: phases[p]['ms_per_step'])
     fft_share = (phases.get('fft_fwd', {}).get('ms_per_step', 0) + phases.get('fft_inv', {}).get('ms_per_step', 0)) / \

@@ -124,9 +124,7 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaMalloc(&c->d_order_tmp, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_tmp, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_cell_of, (size_t)N * sizeof(int)));
-    CUDA_TRY(c, cudaMalloc(&c->d_cell_count, (size_t)(c->ncell + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_cell_start, (size_t)(c->ncell + 1) * sizeof(int)));
-    CUDA_TRY(c, cudaMalloc(&c->d_cell_fill, (size_t)(c->ncell + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_count, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_off, (size_t)(N + 1) * sizeof(unsigned long long)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_ctl, 2 * sizeof(unsigned long long)));
@@ -139,6 +137,10 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
+    c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1);
+    CUDA_TRY(c, cudaMalloc(&c->d_bins, c->bins_n * sizeof(int)));
+    c->d_cell_count = c->d_bins; c->d_cell_fill = c->d_cell_count + c->ncell + 1;
+    c->d_tile_count = c->d_cell_fill + c->ncell + 1; c->d_tile_fill = c->d_tile_count + c->ntile + 1;
     {
         std::vector<float> dec;
         pse_window_table(c->win_kind, P, c->win_a, c->win_b, grid, dec);
@@ -161,7 +163,7 @@ pse_status pse_destroy(pse_ctx *c) {
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
-    cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_fill); cudaFree(c->d_nbr_count);
+    cudaFree(c->d_bins); cudaFree(c->d_cell_start); cudaFree(c->d_nbr_count);
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx); cudaFree(c->d_nbr_ctl);
     if (c->h_nbr_ctl) cudaFreeHost(c->h_nbr_ctl);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);

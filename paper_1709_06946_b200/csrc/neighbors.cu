@@ -84,6 +84,20 @@ __global__ void __launch_bounds__(SCAN1_THREADS) scan_single_cta(const int *in, 
     if (threadIdx.x == 0) out[n] = (OutT)tot;
 }
 
+// two short scans in one launch (cell counts and tile counts)
+__global__ void __launch_bounds__(SCAN1_THREADS) scan_two_ctas(const int *in0, int n0, int *out0, const int *in1, int n1, int *out1) {
+    __shared__ unsigned long long tot;
+    const int *in = blockIdx.x ? in1 : in0;
+    int *out = blockIdx.x ? out1 : out0;
+    const int n = blockIdx.x ? n1 : n0;
+    const int per = (n + SCAN1_THREADS - 1) / SCAN1_THREADS, lo = threadIdx.x * per, hi = min(n, lo + per);
+    unsigned long long s = 0;
+    for (int i = lo; i < hi; ++i) s += (unsigned long long)in[i];
+    unsigned long long e = block_exclusive_scan(s, &tot);
+    for (int i = lo; i < hi; ++i) { out[i] = (int)e; e += (unsigned long long)in[i]; }
+    if (threadIdx.x == 0) out[n] = (int)tot;
+}
+
 template <typename OutT>
 pse_status scan_impl(pse_ctx *c, const int *d_in, OutT *d_out, size_t n) {
     if (n <= (size_t)SCAN1_MAX && (const void *)d_in != (const void *)d_out) {
@@ -119,7 +133,7 @@ __device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL) 
 }
 
 __global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int nc, float cell_inv,
-                             float4 *posw, int *cell_of, int *cell_count) {
+                             float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     float4 p = pos[i];
@@ -129,6 +143,9 @@ __global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int 
     int cell = (cx * nc + cy) * nc + cz;
     cell_of[i] = cell;
     atomicAdd(&cell_count[cell], 1);
+    const int t = pse_tile_of(p, inv_h, M, P, nt);              // spread / interpolate tile bin of the same particle
+    tile_of[i] = t;
+    atomicAdd(&tile_count[t], 1);
 }
 
 __global__ void scatter_to_cells(const int *cell_of, int N, const int *cell_start, int *cell_fill, int *order) {
@@ -153,9 +170,14 @@ __global__ void rank_sort_segments(const int *__restrict__ seg_start, int nseg, 
     }
 }
 
-__global__ void gather_positions(const float4 *posw, const int *order, int N, float4 *pos_sorted) {
+// positions into cell-sorted numbering; the sorted index is appended to the particle's tile bin on the way
+__global__ void gather_positions(const float4 *posw, const int *order, int N, float4 *pos_sorted, const int *tile_of, const int *tile_start,
+                                 int *tile_fill, int *tile_list) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < N) pos_sorted[s] = posw[order[s]];
+    if (s >= N) return;
+    const int o = order[s], t = tile_of[o];
+    pos_sorted[s] = posw[o];
+    tile_list[tile_start[t] + atomicAdd(&tile_fill[t], 1)] = s;
 }
 
 // One warp per (sorted) particle; FILL=false counts, FILL=true writes the list.
@@ -460,14 +482,21 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     const float rc = (float)c->rcut, rc2 = rc * rc;
     const float band = 32.f * rc * L * 1.2e-7f;          // >> 2 r_c ulp(L): rounding gap between screened and R16 distances
     c->have_nbrs = false;
-    CUDA_TRY(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
-    CUDA_TRY(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)(c->ncell + 1) * sizeof(int), c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->d_bins, 0, c->bins_n * sizeof(int), c->stream));      // cell and tile counters, one memset
     wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
-                                           c->d_posw, c->d_cell_of, c->d_cell_count); KERNEL_CHECK(c);
-    PSE_TRY(pse_scan_i32(c, c->d_cell_count, c->d_cell_start, (size_t)c->ncell));
+                                           c->d_posw, c->d_cell_of, c->d_cell_count, (float)(1.0 / c->h), c->M, c->P, c->nt,
+                                           c->d_tile_of, c->d_tile_count); KERNEL_CHECK(c);
+    if (c->ncell <= SCAN1_MAX && c->ntile <= SCAN1_MAX) {
+        scan_two_ctas<<<2, SCAN1_THREADS, 0, c->stream>>>(c->d_cell_count, c->ncell, c->d_cell_start, c->d_tile_count, c->ntile, c->d_tile_start);
+        KERNEL_CHECK(c);
+    } else {
+        PSE_TRY(pse_scan_i32(c, c->d_cell_count, c->d_cell_start, (size_t)c->ncell));
+        PSE_TRY(pse_scan_i32(c, c->d_tile_count, c->d_tile_start, (size_t)c->ntile));
+    }
     scatter_to_cells<<<nb, T, 0, c->stream>>>(c->d_cell_of, N, c->d_cell_start, c->d_cell_fill, c->d_order_tmp); KERNEL_CHECK(c);
     pse_rank_sort(c, c->d_cell_start, c->ncell, c->d_order_tmp, c->d_order);
-    gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos); KERNEL_CHECK(c);
+    gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos, c->d_tile_of, c->d_tile_start, c->d_tile_fill, c->d_tile_tmp);
+    KERNEL_CHECK(c);
     PSE_TRY(pse_tile_bins(c));                       // independent of the list; enqueued first so it overlaps the read-back
     // ---- single-pass build into a cursor-allocated index array; grows and repeats if the array was too small ----
     if (!c->d_nbr_idx) {

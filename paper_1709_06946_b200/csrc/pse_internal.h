@@ -43,15 +43,16 @@ struct pse_ctx {
     int *d_order = nullptr;                  // [N] sorted -> original
     int *d_order_tmp = nullptr, *d_tile_tmp = nullptr;   // [N] unsorted scatter targets
     int *d_cell_of = nullptr;                // [N] cell of original particle
-    int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]
+    int *d_bins = nullptr; size_t bins_n = 0;   // one block cleared by a single memset: cell_count | cell_fill | tile_count | tile_fill
+    int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]; count and fill point into d_bins
     int *d_nbr_count = nullptr;              // [N]
     unsigned long long *d_nbr_off = nullptr; // [N+1]
     int *d_nbr_idx = nullptr; size_t nbr_cap = 0, nbr_total = 0;
     unsigned long long *d_nbr_ctl = nullptr, *h_nbr_ctl = nullptr;   // {allocation cursor, fallback flag}; pinned mirror
     // ---- FFT-grid tile bins ----
     int nt = 0, ntile = 0, Mh = 0;           // tiles per dimension, total, M/2+1
-    int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]
-    int *d_tile_of = nullptr;                // [N] tile of (sorted) particle's support base
+    int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]; count and fill point into d_bins
+    int *d_tile_of = nullptr;                // [N] tile of the particle's support base, original numbering
     int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]
@@ -103,6 +104,18 @@ struct ScopedPhase {
 };
 
 #ifdef __CUDACC__
+// support base (unwrapped, may be negative) of grid coordinate g = x/h   (reading R5)
+__device__ __forceinline__ int pse_support_base(float g, int P) {
+    return (P & 1) ? (int)rintf(g) - (P - 1) / 2 : (int)floorf(g) - P / 2 + 1;
+}
+// periodic index for arguments in [-M, 2M) (support bases and offsets never leave that range since P <= M): no division
+__device__ __forceinline__ int pse_pmod(int i, int M) { i += i < 0 ? M : 0; return i >= M ? i - M : i; }
+// spread / interpolate tile (edge PSE_TILE grid points) that holds the support base of a wrapped position
+__device__ __forceinline__ int pse_tile_of(float4 p, float inv_h, int M, int P, int nt) {
+    const int tx = pse_pmod(pse_support_base(p.x * inv_h, P), M) / PSE_TILE, ty = pse_pmod(pse_support_base(p.y * inv_h, P), M) / PSE_TILE,
+              tz = pse_pmod(pse_support_base(p.z * inv_h, P), M) / PSE_TILE;
+    return (tx * nt + ty) * nt + tz;
+}
 // Warp reduction of 8 per-lane partial sums with 9 shuffles instead of 40: each step halves the number of values a
 // lane carries.  On return the lanes with (lane & 3) == 0 hold the full sum of component
 // comp = 4*bit4(lane) + 2*bit3(lane) + bit2(lane).

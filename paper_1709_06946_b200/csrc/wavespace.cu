@@ -21,12 +21,8 @@ namespace {
 
 constexpr int T = PSE_TILE;
 
-// support base (unwrapped, may be negative) and grid coordinate g = x/h   (reading R5)
-__device__ __forceinline__ int support_base(float g, int P) {
-    return (P & 1) ? (int)rintf(g) - (P - 1) / 2 : (int)floorf(g) - P / 2 + 1;
-}
-// periodic index for arguments in [-M, 2M) (support bases and offsets never leave that range since P <= M): no division
-__device__ __forceinline__ int pmod(int i, int M) { i += i < 0 ? M : 0; return i >= M ? i - M : i; }
+__device__ __forceinline__ int support_base(float g, int P) { return pse_support_base(g, P); }
+__device__ __forceinline__ int pmod(int i, int M) { return pse_pmod(i, M); }
 
 // Exponent of the 1-D window at offset tt (grid units) from the particle.  wb == 0: the paper's Gaussian,
 // exp(-wa tt^2) with wa = 2 pi / P.  wb > 0: "exponential of semicircle" window
@@ -34,24 +30,6 @@ __device__ __forceinline__ int pmod(int i, int M) { i += i < 0 ? M : 0; return i
 // tolerance needs fewer points per dimension.  The branch is uniform across the grid.
 __device__ __forceinline__ float win_arg(float tt, float wa, float wb) {
     return wb > 0.f ? wb * (sqrtf(fmaxf(1.f - wa * tt * tt, 0.f)) - 1.f) : -wa * tt * tt;
-}
-
-__global__ void tile_of_particles(const float4 *pos, int N, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count) {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    float4 p = pos[s];
-    int tx = pmod(support_base(p.x * inv_h, P), M) / T, ty = pmod(support_base(p.y * inv_h, P), M) / T,
-        tz = pmod(support_base(p.z * inv_h, P), M) / T;
-    int t = (tx * nt + ty) * nt + tz;
-    tile_of[s] = t;
-    atomicAdd(&tile_count[t], 1);
-}
-
-__global__ void scatter_to_tiles(const int *tile_of, int N, const int *tile_start, int *tile_fill, int *tile_list) {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    int t = tile_of[s];
-    tile_list[tile_start[t] + atomicAdd(&tile_fill[t], 1)] = s;
 }
 
 // Tiles (along one axis) whose particles' supports can reach tile t: bases in [t*T-(P-1), t*T+T-1] mod M.
@@ -439,9 +417,7 @@ pse_status pse_wave_init(pse_ctx *c) {
     const size_t M3 = (size_t)M * M * M, nmode = (size_t)M * M * c->Mhp;
     CUDA_TRY(c, cudaMalloc(&c->d_grid, 8 * M3 * sizeof(float)));
     CUDA_TRY(c, cudaMalloc(&c->d_spec, 8 * nmode * sizeof(cufftComplex)));
-    CUDA_TRY(c, cudaMalloc(&c->d_tile_count, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_start, (size_t)(c->ntile + 1) * sizeof(int)));
-    CUDA_TRY(c, cudaMalloc(&c->d_tile_fill, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
     if (c->own_fft) return PSE_OK;                    // fft.cu serves this size: no cuFFT plans, no work area
@@ -467,18 +443,13 @@ pse_status pse_wave_init(pse_ctx *c) {
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work); cudaFree(c->d_fft_tw); cudaFree(c->d_fft_dev);
-    cudaFree(c->d_tile_count); cudaFree(c->d_tile_start); cudaFree(c->d_tile_fill); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
+    cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
 }
 
+// Tile bins: counted in wrap_and_bin, scanned with the cell counts, scattered in gather_positions (neighbors.cu);
+// what is left is the deterministic order inside every tile.
 pse_status pse_tile_bins(pse_ctx *c) {
-    const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
-    CUDA_TRY(c, cudaMemsetAsync(c->d_tile_count, 0, (size_t)(c->ntile + 1) * sizeof(int), c->stream));
-    CUDA_TRY(c, cudaMemsetAsync(c->d_tile_fill, 0, (size_t)(c->ntile + 1) * sizeof(int), c->stream));
-    tile_of_particles<<<nb, TB, 0, c->stream>>>(c->d_pos, N, (float)(1.0 / c->h), c->M, c->P, c->nt, c->d_tile_of, c->d_tile_count); KERNEL_CHECK(c);
-    PSE_TRY(pse_scan_i32(c, c->d_tile_count, c->d_tile_start, (size_t)c->ntile));
-    scatter_to_tiles<<<nb, TB, 0, c->stream>>>(c->d_tile_of, N, c->d_tile_start, c->d_tile_fill, c->d_tile_tmp); KERNEL_CHECK(c);
-    PSE_TRY(pse_rank_sort(c, c->d_tile_start, c->ntile, c->d_tile_tmp, c->d_tile_list));
-    return PSE_OK;
+    return pse_rank_sort(c, c->d_tile_start, c->ntile, c->d_tile_tmp, c->d_tile_list);
 }
 
 // plane range of a 2-bit component mask (bit 0: planes 0-2, bit 1: planes 3-7): plan index and first plane
