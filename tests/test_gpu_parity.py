@@ -383,3 +383,52 @@ def test_own_fft_path_matches_oracle_and_cufft(grid, monkeypatch):
     assert rel(out['own'][1], amp * np.hstack([Uw, Ew])) < tol
     assert rel(out['own'][0], out['cufft'][0]) < 2e-5
     assert rel(out['own'][1], out['cufft'][1]) < 2e-5
+
+
+@pytest.mark.parametrize('N,sep', [(1, None), (2, 1.6), (2, 2.5), (3, 9.0)])
+def test_degenerate_sizes_against_oracle(N, sep):
+    """One particle (only self terms and its own periodic images: the Hasimoto lattice), an overlapping pair (r < 2a,
+    the regularised branch of the real-space functions), a separated pair, and three particles none of
+    which has a neighbour inside r_cut (empty lists): product and Brownian sample against the oracle."""
+    import paper_1709_06946_b200 as pse
+    L, xi, tol, grid, P = 16.0, 0.6, 1e-3, 36, 8
+    _, _, _, rcut = pse.pse_suggest_params(max(N, 2), L, A, tol, xi)
+    rng = np.random.default_rng(N)
+    x = np.zeros((N, 3))
+    x[0] = rng.uniform(0, L, 3)
+    for i in range(1, N):
+        d = rng.standard_normal(3)
+        x[i] = x[i - 1] + sep * d / np.linalg.norm(d)
+    x32 = x.astype(np.float32)
+    xd = x32.astype(np.float64)
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    sets = nbr_sets_from_gpu(ctx)
+    ref = nbo.neighbor_sets(x32, L, rcut)
+    assert all(np.array_equal(a, b) for a, b in zip(sets, ref))
+    if N == 3:
+        assert all(len(s) == 0 for s in sets)
+    F, S = synth.gaussian_inputs(N, 7)
+    U, E = gpu_apply(ctx, F, S, 3)
+    Uo, Eo = mob.mobility_apply(xd, L, A, ETA, xi, F, S, eps=1e-12)
+    assert rel(np.hstack([U, E]), np.hstack([Uo, Eo])) < bar(tol)
+    w1, w2 = synth.brownian_noise(N, grid, 9)
+    UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_brownian(1e-3, dev(w1.reshape(N, 8)), dev(w2), UB, EB)
+    torch.cuda.synchronize()
+    Ub, Eb = brn.brownian(xd, L, A, ETA, KT, xi, 1e-3, grid, w1, w2, eps=1e-12)
+    assert rel(np.hstack([UB.cpu().numpy(), EB.cpu().numpy()]), np.hstack([Ub, Eb])) < bar(tol)
+    ctx.close()
+
+
+def test_calls_before_neighbors_fail_with_not_ready():
+    import paper_1709_06946_b200 as pse
+    N, L, xi, tol = 8, 16.0, 0.6, 1e-3
+    _, _, _, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    ctx = make_ctx(N, L, xi, 32, 8, rcut, tol)
+    F, S = synth.gaussian_inputs(N, 0)
+    U, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    with pytest.raises(pse.PSEError) as ei:
+        ctx.pse_mobility_apply(dev(F), dev(S), U, E, 3)
+    assert 'ENOTREADY' in str(ei.value) or ei.value.status == 5
+    ctx.close()
