@@ -77,7 +77,7 @@ class ClockSampler:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/r1_traffic.md), default workload only; other workloads report null.
-NCU_TRAFFIC = {'config3': {'real': 17376000, 'spread': 3478272, 'interp': 23429888, 'scale': 20025856, 'neighbors': 1096960}}
+NCU_TRAFFIC = {'config3': {'real': 17375744, 'spread': 3477760, 'interp': 23429376, 'scale': 20025088, 'neighbors': 1099776}}
 
 
 def max_over_ranks(ms, device=None):
