@@ -314,52 +314,55 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int P2 = P * P, EE = E * Ez;
     float *outf = reinterpret_cast<float *>(out);
-    // lane <-> (j,k) column of the support; the loop over i walks x with a uniform weight, so the inner loop is
-    // two 16-byte shared loads and 8 FMAs, no index arithmetic and no shuffles except the broadcast of wx[i].
-    const int mycomp = ((lane & 16) ? 4 : 0) + ((lane & 8) ? 2 : 0) + ((lane & 4) ? 1 : 0);   // component this lane ends up holding
-    const bool writer = (lane & 3) == 0 && (mode & (mycomp < 3 ? PSE_OUT_U : PSE_OUT_E));
-    int s_next = wid < np ? tile_list[first + wid] : 0;
-    float4 p_next = pos[s_next];
-    for (int pi = wid; pi < np; pi += nw) {
-        const int s = s_next;
-        const float4 p = p_next;
-        if (pi + nw < np) { s_next = tile_list[first + pi + nw]; p_next = pos[s_next]; }       // next particle in flight
-        const float prev = (writer && accumulate) ? outf[(size_t)s * 8 + mycomp] : 0.f;         // read-modify-write operand early
+    // Eight lanes per particle, four particles per warp.  A lane owns the (j,k) columns jk = gl, gl + 8, ... of the
+    // support and walks each along x: two 16-byte shared loads and 8 FMAs per point, the x weights in registers.  The
+    // fixed cost per particle (support base, weights, reduction, read-modify-write) is paid by 8 lanes instead of 32,
+    // and the 8-lane reduction leaves component gl in lane gl: one 32-byte store per particle.
+    constexpr int NP = PT ? PT : PSE_MAXP;
+    const int gl = lane & 7, grp = lane >> 3, gbase = lane & 24;
+    const bool mine = mode & (gl < 3 ? PSE_OUT_U : PSE_OUT_E);
+    for (int pi0 = wid * 4; pi0 < np; pi0 += nw * 4) {                  // uniform over the warp (shuffles inside)
+        const int pi = pi0 + grp;
+        const bool live = pi < np;
+        const int s = live ? tile_list[first + pi] : 0;
+        const float4 p = pos[s];
+        const float prev = (live && mine && accumulate) ? outf[(size_t)s * 8 + gl] : 0.f;       // read-modify-write operand early
         const float gx = p.x * inv_h, gy = p.y * inv_h, gz = p.z * inv_h;
         const int b0 = support_base(gx, P), b1 = support_base(gy, P), b2 = support_base(gz, P);
         const int r0 = pmod(b0, M) - t0 * T, r1 = pmod(b1, M) - t1 * T, r2 = pmod(b2, M) - t2 * T;
-        const float tx = (float)(b0 + lane) - gx;
-        const float wxr = lane < P ? __expf(win_arg(tx, wa, wb)) : 0.f;
+        // x weights: lane gl evaluates i = gl (and gl + 8 for supports wider than 8), the group shares them by shuffle
+        const float wxa = gl < P ? __expf(win_arg((float)(b0 + gl) - gx, wa, wb)) : 0.f;
+        const float wxb = (NP > 8 && gl + 8 < P) ? __expf(win_arg((float)(b0 + gl + 8) - gx, wa, wb)) : 0.f;
+        float wx[NP];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) wx[i] = __shfl_sync(0xffffffffu, i < 8 ? wxa : wxb, gbase + (i & 7));
         float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        // lanes <-> (g, j, k): when P^2 <= 16 the warp holds nI = 32 / P^2 copies of the (j,k) face and copy g walks
-        // x = g, g + nI, ...; otherwise one copy, and faces larger than 32 columns take several passes.
-        const int nI = P2 <= 16 ? 32 / P2 : 1;
-        for (int jk0 = 0; jk0 < P2; jk0 += 32) {
-            const int g = nI > 1 ? lane / P2 : 0, jk = nI > 1 ? lane - g * P2 : jk0 + lane;
-            const bool ok = jk < P2 && g < nI;
-            const int j = ok ? jk / P : 0, k = ok ? jk % P : 0;
-            const float ty = (float)(b1 + j) - gy, tz = (float)(b2 + k) - gz;
-            const float wyz = ok ? __expf(win_arg(ty, wa, wb) + win_arg(tz, wa, wb)) : 0.f;
-            int sidx = ((r0 + (ok ? g : 0)) * E + r1 + j) * Ez + r2 + k;
+        const int ncol = live ? P2 : 0;
+        for (int jk = gl; jk < ncol; jk += 8) {
+            const int j = jk / P, k = jk - j * P;
+            const float wyz = __expf(win_arg((float)(b1 + j) - gy, wa, wb) + win_arg((float)(b2 + k) - gz, wa, wb));
+            int sidx = (r0 * E + r1 + j) * Ez + r2 + k;
             float tsum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #pragma unroll
-            for (int i0 = 0; i0 < (PT ? PT : PSE_MAXP); ++i0) {
-                const int i = i0 * nI + g;                          // uniform trip count: every lane runs ceil(P / nI) rounds
-                if (i0 * nI >= P) break;
-                const float wx = __shfl_sync(0xffffffffu, wxr, i < P ? i : 0);
-                if (i < P) {
-                    const float4 v0 = lo[sidx], v1 = hi[sidx];
-                    tsum[0] += wx * v0.x; tsum[1] += wx * v0.y; tsum[2] += wx * v0.z; tsum[3] += wx * v0.w;
-                    tsum[4] += wx * v1.x; tsum[5] += wx * v1.y; tsum[6] += wx * v1.z; tsum[7] += wx * v1.w;
-                }
-                sidx += nI * EE;
+            for (int i = 0; i < NP; ++i) {
+                if (i >= P) break;
+                const float4 v0 = lo[sidx], v1 = hi[sidx];
+                tsum[0] += wx[i] * v0.x; tsum[1] += wx[i] * v0.y; tsum[2] += wx[i] * v0.z; tsum[3] += wx[i] * v0.w;
+                tsum[4] += wx[i] * v1.x; tsum[5] += wx[i] * v1.y; tsum[6] += wx[i] * v1.z; tsum[7] += wx[i] * v1.w;
+                sidx += EE;
             }
 #pragma unroll
             for (int c = 0; c < 8; ++c) acc[c] += wyz * tsum[c];
         }
-        int comp;
-        const float r = warp_reduce8(acc, lane, comp);
-        if (writer) outf[(size_t)s * 8 + mycomp] = r + prev;
+        // 8 sums over 8 lanes in 4 + 2 + 1 shuffles: every step halves the values a lane carries
+        const bool h4 = gl & 4, h2 = gl & 2, h1 = gl & 1;
+        float r4[4], r2s[2];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) r4[c] = (h4 ? acc[c + 4] : acc[c]) + __shfl_xor_sync(0xffffffffu, h4 ? acc[c] : acc[c + 4], 4);
+#pragma unroll
+        for (int c = 0; c < 2; ++c) r2s[c] = (h2 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h2 ? r4[c] : r4[c + 2], 2);
+        const float r = (h1 ? r2s[1] : r2s[0]) + __shfl_xor_sync(0xffffffffu, h1 ? r2s[0] : r2s[1], 1);
+        if (live && mine) outf[(size_t)s * 8 + gl] = r + prev;
     }
 }
 
