@@ -534,6 +534,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
 
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {
     const size_t nmode = (size_t)c->M * c->M * c->Mh;
+    if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
         scale_brownian_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(

@@ -432,3 +432,32 @@ def test_calls_before_neighbors_fail_with_not_ready():
         ctx.pse_mobility_apply(dev(F), dev(S), U, E, 3)
     assert 'ENOTREADY' in str(ei.value) or ei.value.status == 5
     ctx.close()
+
+
+def test_host_buffer_entry_points_match_device_ones():
+    """pse_step_host / pse_mobility_apply_host (the end-to-end calls bench.py times: host buffers, copies inside the
+    call, wave noise uploaded on a second stream) against pse_step / pse_mobility_apply on the same inputs, two
+    consecutive steps so that the staging buffers are reused while the previous step may still be reading them."""
+    import paper_1709_06946_b200 as pse
+    N, tol, xi, dt = 2000, 1e-3, 0.5, 1e-3
+    x, L = synth.rsa(N, 0.20, seed=31)
+    x32 = x.astype(np.float32)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    noises = [synth.brownian_noise(N, grid, 40 + i) for i in range(2)]
+    ctx_d, ctx_h = make_ctx(N, L, xi, grid, P, rcut, tol), make_ctx(N, L, xi, grid, P, rcut, tol)
+    pos_d = dev(pos4(x32))
+    pos_h = torch.from_numpy(pos4(x32)).pin_memory()
+    for w1, w2 in noises:
+        ctx_d.pse_step(pos_d, dt, dev(w1.reshape(N, 8)), dev(w2))
+        ctx_h.pse_step_host(pos_h, dt, torch.from_numpy(np.ascontiguousarray(w1.reshape(N, 8), dtype=np.float32)).pin_memory(),
+                            torch.from_numpy(np.ascontiguousarray(w2, dtype=np.float32)).pin_memory())
+    torch.cuda.synchronize()
+    assert np.array_equal(pos_d.cpu().numpy(), pos_h.numpy())
+    F, S = synth.gaussian_inputs(N, 3)
+    ctx_d.pse_neighbors(pos_d)
+    Ud, Ed = gpu_apply(ctx_d, F, S, 3)
+    Uh, Eh = torch.empty(N, 3).pin_memory(), torch.empty(N, 5).pin_memory()
+    ctx_h.pse_mobility_apply_host(pos_h, torch.from_numpy(F.astype(np.float32)).pin_memory(), torch.from_numpy(S.astype(np.float32)).pin_memory(), Uh, Eh)
+    assert np.array_equal(Ud, Uh.numpy()) and np.array_equal(Ed, Eh.numpy())
+    ctx_d.close(); ctx_h.close()
