@@ -29,6 +29,8 @@ WORKLOADS = {
     'config2': dict(N=4096, phi=0.20, tol=1e-4, xi=0.5, dt=1e-3, relax=0),
     'config3': dict(N=65536, phi=0.30, tol=1e-3, xi=0.575, dt=1e-4, relax=2),   # largest xi that keeps the 100^3 grid
     'config4': dict(N=1048576, phi=0.10, tol=1e-3, xi=0.34, dt=1e-4, relax=0),
+    # fractal aggregates (d_f ~ 1.8, 32-sphere clusters); tol and xi are swept with --tol / --xi
+    'config5': dict(N=262144, phi=0.05, tol=1e-3, xi=0.28, dt=1e-4, relax=0, fractal=True),
 }
 
 
@@ -98,6 +100,8 @@ def replica_throughput(steps, world, ms_max):
 
 def make_suspension(wl, seed):
     import synth
+    if wl.get('fractal'):
+        return synth.fractal_aggregates(wl['N'], wl['phi'], seed=seed)
     x, L = synth.rsa(wl['N'], wl['phi'], seed=seed)
     if wl['relax']:
         x = synth.relax_overlaps(x, L, sweeps=wl['relax'], seed=seed)
@@ -279,12 +283,15 @@ def main():
     ap.add_argument('--impl', default='ours', choices=['ours', 'reference'])
     ap.add_argument('--no-cpu-baseline', action='store_true')
     ap.add_argument('--xi', type=float, default=None, help='override the splitting parameter (tuning knob, PAPER.md:154)')
+    ap.add_argument('--tol', type=float, default=None, help='override the Ewald tolerance of the workload')
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
     if args.xi:
         wl['xi'] = args.xi
+    if args.tol:
+        wl['tol'] = args.tol
     rank, world = int(os.environ.get('RANK', 0)), int(os.environ.get('WORLD_SIZE', 1))
-    config = {'workload': f'{args.workload}: N={wl["N"]} hard spheres, phi={wl["phi"]}, Ewald tol={wl["tol"]}, xi={wl["xi"]}, '
+    config = {'workload': f'{args.workload}: N={wl["N"]} {"spheres in 32-sphere fractal aggregates" if wl.get("fractal") else "hard spheres"}, phi={wl["phi"]}, Ewald tol={wl["tol"]}, xi={wl["xi"]}, '
                           f'dt={wl["dt"]}, kT=1, RSA placement' + (f' + {wl["relax"]} relax sweeps' if wl['relax'] else ''),
               'N': wl['N'], 'phi': wl['phi'], 'tol': wl['tol'], 'xi': wl['xi']}
     base = {'metric': 'constrained_bd_steps_per_sec', 'unit': 'steps/s', 'n_gpus': args.gpus, 'steps': args.steps, 'warmup': args.warmup,
@@ -347,7 +354,7 @@ def main():
     line['e2e'] = {'value': 1e3 / r['e2e_ms'], 'unit': 'steps/s', 'h2d_bytes_per_step': r['h2d'], 'd2h_bytes_per_step': r['d2h'],
                    'api': 'pse_step_host (pinned host buffers, copies inside the timed call)', 'steps': r['e2e_steps']}
     line['roofline'] = {'bound': 'hbm', 'kernel': dom, 'achieved': phases[dom]['alg_GBps'], 'peak': peak, 'unit': 'GB/s',
-                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not args.xi else None, 'peak_source': peak_src,
+                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not (args.xi or args.tol) else None, 'peak_source': peak_src,
                         'note': 'algorithmic bytes per launch / mean launch duration from CUDA events inside the library over '
                                 f'{r["profiled_steps"]} profiled steps; at this size the grids are L2-resident (see DESIGN.md §5)'}
     line['phases'] = phases

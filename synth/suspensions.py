@@ -141,7 +141,7 @@ def fractal_aggregates(N, phi, seed=0, a=1.0, cluster_size=32, pool=32, max_trie
     x = np.empty((N, 3))
     n = 0
     dmin = 2.0 * a * (1.0 + 1e-9)
-    tree = None
+    tree, n_tree = None, 0                       # k-d tree over x[:n_tree]; x[n_tree:n] is checked directly until the next rebuild
     for _ in range(max_tries):
         if n >= N:
             break
@@ -150,9 +150,15 @@ def fractal_aggregates(N, phi, seed=0, a=1.0, cluster_size=32, pool=32, max_trie
             d, _ = tree.query(P, k=1, distance_upper_bound=dmin)
             if not np.all(np.isinf(d)):
                 continue
+        if n > n_tree:
+            dd = P[:, None, :] - x[None, n_tree:n, :]
+            dd -= L * np.round(dd / L)
+            if np.einsum('ijk,ijk->ij', dd, dd).min() < dmin * dmin:
+                continue
         x[n:n + cluster_size] = P
         n += cluster_size
-        tree = cKDTree(x[:n], boxsize=L)
+        if n - n_tree >= max(cluster_size, n_tree // 16):
+            tree, n_tree = cKDTree(x[:n], boxsize=L), n
     if n < N:
         raise RuntimeError(f'aggregate placement stalled at {n}/{N}')
     return x, L
