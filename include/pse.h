@@ -83,8 +83,17 @@ pse_status pse_constrained_solve(pse_ctx *ctx, const float *d_F, const float *d_
  * DESIGN.md reading R12): F_i = sum_{j: r_ij<2a} 3 pi eta a (2a - r_ij)/dt rhat_ij.  d_F [N][3] out. */
 pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);
 
+/* Bonds with the pair potential U(r) = k |r - r0| of the paper's equilibrium test (its Boltzmann
+ * distribution of r is Eq. (80)).  h_pairs: HOST array [n_bonds][2] of particle indices (copied);
+ * n_bonds = 0 removes all bonds.  pse_step adds the bond forces, evaluated at x_{k+1/2} with the minimum image, to F^P.
+ * Synchronises the stream.  PSE_EINVAL: index out of range, i == j, r0 < 0. */
+pse_status pse_set_bonds(pse_ctx *ctx, const int *h_pairs, int n_bonds, double k, double r0);
+/* Bond forces at the positions of the last pse_neighbors call: F_i = -k sign(r - r0) rhat_ij, F_j = -F_i,
+ * rhat_ij = (x_i - x_j)/r.  d_F [N][3] out (overwritten; zero without bonds).  Asynchronous. */
+pse_status pse_bond_forces(pse_ctx *ctx, float *d_F);
+
 /* One mid-point step of the constrained overdamped Langevin dynamics, Eqs. (76)-(79):
- * neighbours(x_k); Brownian slip; x_{k+1/2} = x_k + dt/2 U^B; neighbours(x_{k+1/2}); hard-sphere forces;
+ * neighbours(x_k); Brownian slip; x_{k+1/2} = x_k + dt/2 U^B; neighbours(x_{k+1/2}); hard-sphere (+ bond) forces;
  * constrained solve; x_{k+1} = x_k + dt U_{k+1/2} (wrapped into [0,L)).  d_pos [N][4] in/out.
  * On return the context's neighbour structures refer to x_{k+1/2}; call pse_neighbors before further products. */
 pse_status pse_step(pse_ctx *ctx, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave,

@@ -105,6 +105,28 @@ def heyes_melrose(x, L, a, eta, dt):
     return np.einsum('ab,abi->ai', coef, d)
 
 
+def bond_forces(x, L, pairs, k, r0):
+    """Forces of the pair potential of the paper's equilibrium test, U(r) = k |r - r0|, on the bonded
+    pairs `pairs` (n,2): F_i = -dU/dx_i = -k sign(r - r0) rhat_ij, F_j = -F_i, rhat_ij = (x_i - x_j)/r (minimum image)."""
+    x = np.asarray(x, dtype=np.float64)
+    F = np.zeros_like(x)
+    for i, j in np.asarray(pairs, dtype=np.int64).reshape(-1, 2):
+        d = x[i] - x[j]
+        d -= L * np.round(d / L)
+        r = np.linalg.norm(d)
+        f = -k * np.sign(r - r0) * d / r
+        F[i] += f
+        F[j] -= f
+    return F
+
+
+def pair_distance_pdf(r, kt, r0):
+    """Eq. (80): Boltzmann density of the centre-to-centre distance of a pair bound by U = k|r - r0|,
+    f(r) = kt^3 / (2 (2 + kt^2 r0^2)) r^2 exp(-kt |r - r0|),  kt = k / kT."""
+    r = np.asarray(r, dtype=np.float64)
+    return kt ** 3 / (2.0 * (2.0 + kt ** 2 * r0 ** 2)) * r ** 2 * np.exp(-kt * np.abs(r - r0))
+
+
 def constrained_solve(M, N, UB, EB, FP):
     """Eqs. (36)-(38), (78) with deterministic forces (reading R12):
     solve M_ES S = -(E^B + M_EF F^P), then U = U^B + M_UF F^P + M_US S.  M is the dense 8N x 8N matrix."""
@@ -116,13 +138,17 @@ def constrained_solve(M, N, UB, EB, FP):
     return U.reshape(N, 3), S.reshape(N, 5)
 
 
-def step(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14):
-    """One mid-point step, Eqs. (76)-(79).  Returns x_{k+1} (not wrapped), U_{k+1/2}, S."""
+def step(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14, bonds=None):
+    """One mid-point step, Eqs. (76)-(79).  Returns x_{k+1} (not wrapped), U_{k+1/2}, S.
+    bonds = (pairs, k, r0) adds the forces of U = k|r - r0| at the mid-point to F^P."""
     x = np.asarray(x, dtype=np.float64)
     N = x.shape[0]
     UB, EB = brownian(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps)          # (76)
     xh = x + 0.5 * dt * UB                                                   # (77)
     xh -= L * np.floor(xh / L)
     M = mob.dense(xh, L, a, eta, xi, 'both', eps)
-    U, S = constrained_solve(M, N, UB, EB, heyes_melrose(xh, L, a, eta, dt))  # (78)
+    FP = heyes_melrose(xh, L, a, eta, dt)
+    if bonds is not None:
+        FP = FP + bond_forces(xh, L, *bonds)
+    U, S = constrained_solve(M, N, UB, EB, FP)                               # (78)
     return x + dt * U, U, S                                                  # (79)

@@ -18,7 +18,7 @@ _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PS
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
 EXPORTS = ('pse_suggest_params', 'pse_create', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
-           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
 
@@ -42,6 +42,8 @@ def load_library():
     lib.pse_brownian.argtypes = [vp, dbl, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
+    lib.pse_set_bonds.argtypes = [vp, vp, i32, dbl, dbl]
+    lib.pse_bond_forces.argtypes = [vp, vp]
     lib.pse_step.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pse_mobility_apply_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.pse_step_host.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
@@ -139,6 +141,15 @@ class Context:
 
     def pse_hard_sphere_forces(self, dt, F):
         self._check(_lib.pse_hard_sphere_forces(self._h, dt, _ptr(F, (self.N, 3))))
+
+    def pse_set_bonds(self, pairs, k, r0):
+        """pairs: host int32 array-like (n, 2)."""
+        import numpy as np
+        p = np.ascontiguousarray(np.asarray(pairs, dtype=np.int32).reshape(-1, 2))
+        self._check(_lib.pse_set_bonds(self._h, p.ctypes.data_as(C.c_void_p) if len(p) else None, len(p), float(k), float(r0)))
+
+    def pse_bond_forces(self, F):
+        self._check(_lib.pse_bond_forces(self._h, _ptr(F, (self.N, 3))))
 
     def pse_step(self, pos, dt, noise_real, noise_wave):
         N, M = self.N, self.grid

@@ -169,7 +169,7 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx); cudaFree(c->d_nbr_ctl);
     if (c->h_nbr_ctl) cudaFreeHost(c->h_nbr_ctl);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
-    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec);
+    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec); cudaFree(c->d_bonds);
     cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     delete c;
@@ -214,6 +214,27 @@ pse_status pse_hard_sphere_forces(pse_ctx *c, double dt, float *d_F) {
     return pse_unpack(c, c->d_vecA, 1.f, d_F, nullptr);
 }
 
+pse_status pse_set_bonds(pse_ctx *c, const int *h_pairs, int n_bonds, double k, double r0) {
+    if (!c || n_bonds < 0 || (n_bonds > 0 && (!h_pairs || !(r0 >= 0)))) return PSE_EINVAL;
+    for (int b = 0; b < 2 * n_bonds; ++b)
+        if (h_pairs[b] < 0 || h_pairs[b] >= c->N) { c->err = "pse_set_bonds: particle index out of range"; return PSE_EINVAL; }
+    for (int b = 0; b < n_bonds; ++b)
+        if (h_pairs[2 * b] == h_pairs[2 * b + 1]) { c->err = "pse_set_bonds: bond of a particle with itself"; return PSE_EINVAL; }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->d_bonds); c->d_bonds = nullptr; c->n_bonds = 0;
+    if (n_bonds == 0) return PSE_OK;
+    CUDA_TRY(c, cudaMalloc(&c->d_bonds, (size_t)n_bonds * sizeof(int2)));
+    CUDA_TRY(c, cudaMemcpy(c->d_bonds, h_pairs, (size_t)n_bonds * sizeof(int2), cudaMemcpyHostToDevice));
+    c->n_bonds = n_bonds; c->bond_k = k; c->bond_r0 = r0;
+    return PSE_OK;
+}
+
+pse_status pse_bond_forces(pse_ctx *c, float *d_F) {
+    if (!c || !d_F) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_bond_forces before pse_neighbors"; return PSE_ENOTREADY; }
+    return pse_bond_forces_orig(c, d_F);
+}
+
 pse_status pse_constrained_solve(pse_ctx *c, const float *d_F, const float *d_UB, const float *d_EB, float *d_U, float *d_S, int *gmres_iters) {
     if (!c || !d_U || !d_S) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_constrained_solve before pse_neighbors"; return PSE_ENOTREADY; }
@@ -241,6 +262,11 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
     // (78) constrained solve at the mid-point with hard-sphere forces (reading R12)
     PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+    if (c->n_bonds) {                                                  // F^P += bond forces (d_vecC, d_out: free until the solve)
+        PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
+        PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
+        PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+    }
     PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
     st = pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
     if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;

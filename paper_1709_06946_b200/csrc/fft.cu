@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 2) fft_fwd_plane_kernel(const flo
     const FftDev &f = *sm.f;
     float2 *A = sm.A, *B = A + f.bufsz;
     const int M = f.M, Mh = f.Mh, x = blockIdx.x, c = first + blockIdx.y;
-    const float *g = grid + ((size_t)c * M + x) * M * M;
+    const float *g = grid + (size_t)c * pse_plane_stride(M) + (size_t)x * M * M;
     // two real rows per complex line (two-for-one): one conflict-free 8-byte shared store per pair of coalesced loads
     for (int idx = tid; idx < f.NP * M; idx += FFT_THREADS) {
         const int p = f.divM.div(idx), z = idx - p * M;
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 2) fft_inv_plane_kernel(const flo
     __syncthreads();
     { float2 *t = A; A = B; B = t; }
     fft_lines<true, FFT_THREADS>(A, B, f, 0, f.NP, f.divNP, f.Pz, 1, sm.tw, tid);
-    float *g = grid + ((size_t)c * M + x) * M * M;
+    float *g = grid + (size_t)c * pse_plane_stride(M) + (size_t)x * M * M;
     for (int idx = tid; idx < f.NP * M; idx += FFT_THREADS) {
         const int p = f.divM.div(idx), z = idx - p * M;
         const float2 v = A[p * f.Pz + z];

@@ -465,7 +465,33 @@ __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned 
     }
 }
 
+// Forces of the bond potential U(r) = k |r - r0| of the paper's equilibrium test: a thread per bond,
+// positions and output in original numbering, F_i -= k sign(r - r0) rhat_ij, F_j += the same (out is zeroed beforehand).
+__global__ void bond_forces(const float4 *__restrict__ posw, const int2 *__restrict__ bonds, int nb, float L, float invL, float k, float r0,
+                            float *__restrict__ out) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nb) return;
+    const int2 ij = bonds[b];
+    const float4 p = posw[ij.x], q = posw[ij.y];
+    const float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
+    const float r = sqrtf(dx * dx + dy * dy + dz * dz);
+    if (!(r > 0.f) || r == r0) return;
+    const float g = (r > r0 ? -k : k) / r;
+    atomicAdd(out + 3 * (size_t)ij.x, g * dx); atomicAdd(out + 3 * (size_t)ij.x + 1, g * dy); atomicAdd(out + 3 * (size_t)ij.x + 2, g * dz);
+    atomicAdd(out + 3 * (size_t)ij.y, -g * dx); atomicAdd(out + 3 * (size_t)ij.y + 1, -g * dy); atomicAdd(out + 3 * (size_t)ij.y + 2, -g * dz);
+}
+
 }  // namespace
+
+pse_status pse_bond_forces_orig(pse_ctx *c, float *d_F) {
+    ScopedPhase ph(c, PSE_T_REAL);
+    CUDA_TRY(c, cudaMemsetAsync(d_F, 0, (size_t)3 * c->N * sizeof(float), c->stream));
+    if (c->n_bonds == 0) return PSE_OK;
+    bond_forces<<<(c->n_bonds + 127) / 128, 128, 0, c->stream>>>(c->d_posw, c->d_bonds, c->n_bonds, (float)c->L, 1.0f / (float)c->L,
+                                                                 (float)c->bond_k, (float)c->bond_r0, d_F);
+    KERNEL_CHECK(c);
+    return PSE_OK;
+}
 
 pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *in, int *out) {
     rank_sort_segments<<<(unsigned)(((size_t)nseg * 32 + 255) / 256), 256, 0, c->stream>>>(seg_start, nseg, in, out); KERNEL_CHECK(c);

@@ -76,6 +76,8 @@ struct pse_ctx {
     unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
     float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
     float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
+    // ---- bonds of the equilibrium test potential U = k |r - r0|, original numbering ----
+    int2 *d_bonds = nullptr; int n_bonds = 0; double bond_k = 0, bond_r0 = 0;
     // ---- staging for the host-buffer entry points ----
     float *d_stage_pos = nullptr, *d_stage_a = nullptr, *d_stage_b = nullptr, *d_stage_noise = nullptr;
     // ---- profiling ----
@@ -103,6 +105,13 @@ struct ScopedPhase {
     }
     ~ScopedPhase() { if (idx >= 0) cudaEventRecord(c->timers[idx].b, c->stream); }
 };
+
+// Distance in floats between two of the 8 real grids: M^3 rounded up to a multiple of 4, so that every plane starts
+// 16-byte aligned (cuFFT rejects a real batch pointer that is only 4-byte aligned: odd M, odd first plane).
+#ifdef __CUDACC__
+__host__ __device__
+#endif
+inline size_t pse_plane_stride(int M) { return ((size_t)M * M * M + 3) & ~(size_t)3; }
 
 #ifdef __CUDACC__
 // support base (unwrapped, may be negative) of grid coordinate g = x/h   (reading R5)
@@ -147,6 +156,7 @@ pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n);
 pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *in, int *out);
 pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total);
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
+pse_status pse_bond_forces_orig(pse_ctx *c, float *d_F);   // [N][3], original numbering, overwritten
 // realspace.cu
 pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st = nullptr, int ctas_per_sm = 2, int mode = PSE_MODE_ALL);   // out = M_r in
 // wavespace.cu

@@ -200,7 +200,7 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
         nh = left;
     }
     const int gx = g0[0] + a, gz = g0[2] + cc;
-    const size_t M3 = (size_t)M * M * M;
+    const size_t M3 = pse_plane_stride(M);
     if (gx < M && gz < M) {
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
@@ -231,7 +231,7 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
         float tt = (d < 3) ? (float)(base[d] + i) - g[d] : 0.f;
         wr[h] = (d < 3) ? __expf(win_arg(tt, wa, wb)) : 0.f;
     }
-    const size_t M3 = (size_t)M * M * M;
+    const size_t M3 = pse_plane_stride(M);
     float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     const int P2 = P * P, P3 = P2 * P;
     for (int pt0 = 0; pt0 < P3; pt0 += 32) {
@@ -279,7 +279,7 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int first = tile_start[t], np = tile_start[t + 1] - first;
     if (np == 0) return;
-    const size_t M3 = (size_t)M * M * M;
+    const size_t M3 = pse_plane_stride(M);
     {   // stage row by row: a half-warp (E <= 16) or a warp per (ix,iy) row, lanes along z; wrap by subtraction
         const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
         const int rpi = E <= 16 ? 2 : 1, lz = E <= 16 ? (lane & 15) : lane, sub = E <= 16 ? (lane >> 4) : 0;
@@ -417,7 +417,7 @@ pse_status pse_wave_init(pse_ctx *c) {
     c->Mh = M / 2 + 1;
     c->nt = (M + T - 1) / T; c->ntile = c->nt * c->nt * c->nt;
     PSE_TRY(pse_fft_init(c));                          // decides own FFT vs cuFFT and with it the spectrum pitch
-    const size_t M3 = (size_t)M * M * M, nmode = (size_t)M * M * c->Mhp;
+    const size_t M3 = pse_plane_stride(M), nmode = (size_t)M * M * c->Mhp;
     CUDA_TRY(c, cudaMalloc(&c->d_grid, 8 * M3 * sizeof(float)));
     CUDA_TRY(c, cudaMalloc(&c->d_spec, 8 * nmode * sizeof(cufftComplex)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_start, (size_t)(c->ntile + 1) * sizeof(int)));
@@ -431,8 +431,14 @@ pse_status pse_wave_init(pse_ctx *c) {
         size_t w1 = 0, w2 = 0;
         CUFFT_TRY(c, cufftCreate(&c->plan_r2c[i])); CUFFT_TRY(c, cufftCreate(&c->plan_c2r[i])); c->nplans = i + 1;
         CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_r2c[i], 0)); CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_c2r[i], 0));
-        CUFFT_TRY(c, cufftMakePlanMany(c->plan_r2c[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, batches[i], &w1));
-        CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, batches[i], &w2));
+        if (M3 == (size_t)M * M * M) {                // even M: packed planes, basic layout
+            CUFFT_TRY(c, cufftMakePlanMany(c->plan_r2c[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, batches[i], &w1));
+            CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r[i], 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, batches[i], &w2));
+        } else {                                      // odd M: real planes pse_plane_stride(M) apart
+            int nr[3] = {M, M, M}, ncx[3] = {M, M, c->Mh};
+            CUFFT_TRY(c, cufftMakePlanMany(c->plan_r2c[i], 3, n, nr, 1, (int)M3, ncx, 1, M * M * c->Mh, CUFFT_R2C, batches[i], &w1));
+            CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r[i], 3, n, ncx, 1, M * M * c->Mh, nr, 1, (int)M3, CUFFT_C2R, batches[i], &w2));
+        }
         w = std::max(w, std::max(w1, w2));
     }
     if (w) CUDA_TRY(c, cudaMalloc(&c->d_fft_work, w));
@@ -465,7 +471,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
         ScopedPhase ph(c, PSE_T_FFT_INV);
         int plan, first;
         plane_range((mode >> 2) & 3, plan, first);
-        const size_t M3 = (size_t)c->M * c->M * c->M, nmode = (size_t)c->M * c->M * c->Mh;
+        const size_t M3 = pse_plane_stride(c->M), nmode = (size_t)c->M * c->M * c->Mh;
         if (c->own_fft) PSE_TRY(pse_fft_inverse_planes(c, first, plan == 0 ? 8 : plan == 1 ? 3 : 5));
         else { CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++; }
     }
@@ -506,7 +512,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
 }
 
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp, int mode) {
-    const size_t nmode = (size_t)c->M * c->M * c->Mh, M3 = (size_t)c->M * c->M * c->M;
+    const size_t nmode = (size_t)c->M * c->M * c->Mh, M3 = pse_plane_stride(c->M);
     if (!(mode & (PSE_IN_F | PSE_IN_S)) || !(mode & (PSE_OUT_U | PSE_OUT_E))) { c->err = "pse_wave_apply: empty component mask"; return PSE_EINVAL; }
     int plan, first;
     plane_range(mode & 3, plan, first);

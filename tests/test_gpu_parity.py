@@ -245,6 +245,35 @@ def test_product_mid_size_sampled_rows(N, phi, tol, xi, seed):
     assert rel(U[rows], Uo) < bar(tol) and rel(E[rows], Eo) < bar(tol)
 
 
+@pytest.mark.parametrize('grid', [35, 45])
+def test_odd_grid_component_masks(grid):
+    """Odd M: M^3 is odd, so the S / E planes (first plane 3) of a packed [8][M^3] array would start 4-byte aligned only
+    and cuFFT rejects them; the planes are pse_plane_stride(M) apart instead.  S -> E, F -> U and full products."""
+    N, xi, tol = 400, 0.5, 1e-3
+    x, L = synth.rsa(N, 0.15, seed=41)
+    x32 = x.astype(np.float32)
+    rcut = np.sqrt(-np.log(tol)) / xi + 1.0
+    ctx = make_ctx(N, L, xi, grid, 6, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    F, S = synth.gaussian_inputs(N, 41)
+    k = brn.grid_modes(grid, L)
+    k2 = np.einsum('ki,ki->k', k, k)
+    w = fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2)
+    Ug, Eg = mob.wave_apply_modes(x32.astype(np.float64), L, A, ETA, k, w, F, S)
+    U, E = gpu_apply(ctx, F, S, 2)
+    assert rel(U, Ug) < 1e-3 and rel(E, Eg) < 1e-3
+    Us, Es = mob.wave_apply_modes(x32.astype(np.float64), L, A, ETA, k, w, np.zeros_like(F), S)
+    E2 = torch.empty(N, 5, device='cuda')
+    ctx.pse_mobility_apply(None, dev(S), None, E2, 2)         # S -> E: planes 3-7 both ways
+    assert rel(E2.cpu().numpy(), Es) < 1e-3
+    Uf, Ef = mob.wave_apply_modes(x32.astype(np.float64), L, A, ETA, k, w, F, np.zeros_like(S))
+    U2 = torch.empty(N, 3, device='cuda')
+    ctx.pse_mobility_apply(dev(F), None, U2, None, 2)         # F -> U: planes 0-2
+    assert rel(U2.cpu().numpy(), Uf) < 1e-3
+    ctx.pse_mobility_apply(dev(F), None, None, E2, 2)         # F -> E: planes 0-2 in, 3-7 out
+    assert rel(E2.cpu().numpy(), Ef) < 1e-3
+
+
 def test_large_support_uses_global_interpolation_path():
     """P = 14 exceeds the shared-memory staging budget of the tiled interpolation: fallback kernel, same result."""
     x, L = synth.rsa(200, 0.10, seed=31)

@@ -176,3 +176,63 @@ def test_P12_schur_complement_solve():
     Mc = M[np.ix_(iu, iu)] - M[np.ix_(iu, ie)] @ np.linalg.solve(M[np.ix_(ie, ie)], M[np.ix_(ie, iu)])
     assert np.abs(Mc - Mc.T).max() < 1e-13
     assert np.linalg.eigvalsh(Mc).min() > 0 and np.linalg.eigvalsh(M[np.ix_(iu, iu)] - Mc).min() > -1e-13
+
+
+def test_P13_bond_force_is_minus_gradient_of_the_test_potential():
+    """U(r) = k |r - r0|: F = -grad U by central differences, including a bond through the periodic
+    boundary and particles in several bonds; the forces of a bond sum to zero."""
+    L, k, r0 = 9.0, 2.5, 3.0
+    x = np.array([[0.5, 0.6, 0.7], [8.6, 1.0, 0.9], [1.1, 4.0, 5.5], [2.0, 2.0, 2.3], [5.0, 5.5, 2.0]])
+    pairs = np.array([[0, 1], [2, 3], [3, 0], [4, 2]])
+
+    def energy(y):
+        d = y[pairs[:, 0]] - y[pairs[:, 1]]
+        d -= L * np.round(d / L)
+        return k * np.abs(np.linalg.norm(d, axis=1) - r0).sum()
+    F = brn.bond_forces(x, L, pairs, k, r0)
+    h = 1e-6
+    for i in range(5):
+        for c in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, c] += h
+            xm[i, c] -= h
+            assert abs(F[i, c] + (energy(xp) - energy(xm)) / (2 * h)) < 1e-8
+    assert np.abs(F.sum(axis=0)).max() < 1e-14
+    # bond 0-1 passes through the boundary (minimum-image distance 1.97 < r0: repulsive, 0 pushed towards +x)
+    F01 = brn.bond_forces(x, L, pairs[:1], k, r0)
+    assert F01[0, 0] > 0 and np.isclose(np.linalg.norm(F01[0]), k)
+
+
+def test_P14_eq80_is_the_normalised_boltzmann_density_of_the_pair_distance():
+    """Eq. (80) as printed: integrates to one and equals r^2 exp(-U/kT) up to that constant."""
+    for kt, r0 in [(3.0, 5.0), (1.0, 2.5), (6.0, 4.0)]:
+        r = np.linspace(0.0, r0 + 60.0 / kt, 400001)
+        f = brn.pair_distance_pdf(r, kt, r0)
+        tail = np.exp(-kt * r0) * (2 / kt**3 - 0)      # part of the r^2 e^{-kt|r-r0|} integral that a formula on (-inf, inf) would add
+        assert abs(np.trapezoid(f, r) - 1.0) < 2e-3 + tail
+        w = r[1:]**2 * np.exp(-kt * np.abs(r[1:] - r0))
+        assert np.allclose(f[1:] / w, f[1000] / (r[1000]**2 * np.exp(-kt * abs(r[1000] - r0))), rtol=1e-12)
+
+
+def test_P15_oracle_midpoint_steps_sample_eq80():
+    """Two bonded spheres, 1 500 oracle mid-point steps (Eqs. 76-79) with fresh noise: <|r - r0|> of Eq. (80) within the
+    statistical error of ~35 independent samples (a wrong noise amplitude or a missing factor 2 in kT fails it; the
+    sharp version of this test runs on the GPU, tests/test_gpu_equilibrium.py)."""
+    L, xi, Mg, dt, k, r0, kT = 12.0, 0.3, 8, 4e-3, 6.0, 4.0, 1.0
+    x = np.array([[4.0, 4.0, 4.0], [8.0, 4.0, 4.0]])
+    g = np.random.Generator(np.random.Philox(7))
+    bonds = (np.array([[0, 1]]), k, r0)
+    rs = []
+    for s in range(1500):
+        w1, w2 = g.standard_normal(16), g.standard_normal((3, Mg, Mg, Mg // 2 + 1, 2))
+        x, _, _ = brn.step(x, L, A, ETA, kT, xi, dt, Mg, w1, w2, eps=1e-6, bonds=bonds)
+        d = x[0] - x[1]
+        d -= L * np.round(d / L)
+        rs.append(np.linalg.norm(d))
+    rs = np.array(rs[60:])
+    r = np.linspace(0.0, L / 2, 60001)
+    f = brn.pair_distance_pdf(r, k / kT, r0)
+    want = np.trapezoid(f * np.abs(r - r0), r)
+    got = np.abs(rs - r0).mean()
+    assert 0.6 * want < got < 1.5 * want, (got, want)
+    assert abs(rs.mean() - np.trapezoid(f * r, r)) < 0.12
