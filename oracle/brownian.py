@@ -138,6 +138,33 @@ def constrained_solve(M, N, UB, EB, FP):
     return U.reshape(N, 3), S.reshape(N, 5)
 
 
+def constrained_mobility(M, N):
+    """R_FU^{-1} = M_UF - M_US M_ES^{-1} M_EF (Eq. B15), the 3N x 3N mobility of rigid spheres, from the
+    dense 8N x 8N grand mobility."""
+    iu = (8 * np.arange(N)[:, None] + np.arange(3)[None, :]).ravel()
+    ie = (8 * np.arange(N)[:, None] + 3 + np.arange(5)[None, :]).ravel()
+    return M[np.ix_(iu, iu)] - M[np.ix_(iu, ie)] @ np.linalg.solve(M[np.ix_(ie, ie)], M[np.ix_(ie, iu)])
+
+
+def constrained_mobility_divergence(x, L, a, eta, xi, h=1e-4, eps=1e-12):
+    """(div R_FU^{-1})_i = sum_l d/dx_l (R_FU^{-1})_{il}, the drift of Eq. (B12) per unit kT dt, by central
+    differences of the dense matrix.  Returns (div R_FU^{-1}, div M_UF), each (3N,); the second is zero."""
+    x = np.asarray(x, dtype=np.float64)
+    N = x.shape[0]
+    iu = (8 * np.arange(N)[:, None] + np.arange(3)[None, :]).ravel()
+    div_c, div_uf = np.zeros(3 * N), np.zeros(3 * N)
+    for l in range(3 * N):
+        cols = []
+        for sgn in (1.0, -1.0):
+            y = x.copy().ravel()
+            y[l] += sgn * h
+            M = mob.dense(y.reshape(N, 3), L, a, eta, xi, 'both', eps)
+            cols.append((constrained_mobility(M, N)[:, l], M[np.ix_(iu, iu)][:, l]))
+        div_c += (cols[0][0] - cols[1][0]) / (2 * h)
+        div_uf += (cols[0][1] - cols[1][1]) / (2 * h)
+    return div_c, div_uf
+
+
 def step(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14, bonds=None):
     """One mid-point step, Eqs. (76)-(79).  Returns x_{k+1} (not wrapped), U_{k+1/2}, S.
     bonds = (pairs, k, r0) adds the forces of U = k|r - r0| at the mid-point to F^P."""

@@ -236,3 +236,20 @@ def test_P15_oracle_midpoint_steps_sample_eq80():
     got = np.abs(rs - r0).mean()
     assert 0.6 * want < got < 1.5 * want, (got, want)
     assert abs(rs.mean() - np.trapezoid(f * r, r)) < 0.12
+
+
+def test_P16_divergence_of_M_UF_vanishes_and_constrained_drift_is_antisymmetric():
+    """'because div M_UF = 0': the RPY block of the periodic grand mobility is divergence-free, also for an
+    overlapping pair; the divergence of the constrained mobility R_FU^-1 (the drift of Eq. B12) is not,
+    and for two spheres it is equal and opposite along the line of centres."""
+    L, xi = 16.0, 0.5
+    for r in (1.7, 2.5):
+        x = np.array([[4.0, 4.0, 4.0], [4.0 + r, 4.0, 4.0]])
+        div_c, div_uf = brn.constrained_mobility_divergence(x, L, A, ETA, xi)
+        assert np.abs(div_uf).max() < 2e-9
+        assert abs(div_c[0]) > 5e-3 and abs(div_c[0] + div_c[3]) < 1e-9
+        assert np.abs(div_c[[1, 2, 4, 5]]).max() < 1e-9
+    M = mob.dense(x, L, A, ETA, xi)
+    Mc = brn.constrained_mobility(M, 2)
+    U, _ = brn.constrained_solve(M, 2, np.zeros((2, 3)), np.zeros((2, 5)), np.eye(6)[2].reshape(2, 3))
+    assert np.abs(Mc[:, 2] - U.ravel()).max() < 1e-14
