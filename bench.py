@@ -79,7 +79,7 @@ class ClockSampler:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/r1_traffic.md), default workload only; other workloads report null.
-NCU_TRAFFIC = {'config3': {'real': 17375744, 'spread': 3477760, 'interp': 23429376, 'scale': 20025088, 'neighbors': 1099776}}
+NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 3478528, 'interp': 23429120, 'scale': 20024832, 'neighbors': 1098240}}
 
 
 def max_over_ranks(ms, device=None):
@@ -356,7 +356,9 @@ def main():
     line['roofline'] = {'bound': 'hbm', 'kernel': dom, 'achieved': phases[dom]['alg_GBps'], 'peak': peak, 'unit': 'GB/s',
                         'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not (args.xi or args.tol) else None, 'peak_source': peak_src,
                         'note': 'algorithmic bytes per launch / mean launch duration from CUDA events inside the library over '
-                                f'{r["profiled_steps"]} profiled steps; at this size the grids are L2-resident (see DESIGN.md §5)'}
+                                f'{r["profiled_steps"]} profiled steps; ' + (
+                                    'at this size the grids are L2-resident (see DESIGN.md §5)' if 64 * r['grid']**3 < 100e6 else
+                                    'the 8 real + 8 spectral grids exceed the L2 (see DESIGN.md §5)')}
     line['phases'] = phases
     line['cufft_share_of_step'] = fft_share
     if not args.no_cpu_baseline:

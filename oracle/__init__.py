@@ -13,13 +13,16 @@ It is a plain, slow, obviously-correct statement of what the path computes:
                    and row-sampled application for larger N.
 * ``brownian``   – Eq. (71)/(74)/(76) sample: principal square root of the dense
                    real-space matrix plus the direct non-uniform sum of the wave-space factor over the
-                   grid's wave vectors; the mid-point step Eqs. (76)-(79).
+                   grid's wave vectors; the mid-point step Eqs. (76)-(79); the bond force of
+                   the equilibrium test potential U = k|r - r0| and Eq. (80); the constrained
+                   mobility R_FU^-1 of Eq. (B15) and its divergence, the drift of Eq. (B12).
 * ``neighbors``  – brute-force fp32 neighbour sets.
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): Hasimoto periodic self-mobility, xi-independence of
 M_r + M_w, symmetry and positive-definiteness of M, M_r, M_w, textbook RPY / RPY-overlap free-space
 limits, printed closed forms F1, F2 of Appendix A, exact covariance identity
-A_w A_w^T = M_w(grid modes), Schur-complement constraint solve.
+A_w A_w^T = M_w(grid modes), Schur-complement constraint solve, bond force = -grad U, Eq. (80) normalised
+Boltzmann density, a short two-sphere run against Eq. (80), div M_UF = 0.
 
 Parity unpinned (not in the paper): the Heyes-Melrose hard-sphere force (reading R12 in DESIGN.md).
 """
