@@ -302,7 +302,7 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
 // order); only the placement of whole cells in the index array depends on scheduling, which no consumer sees
 // (they go through off[s], count[s]).  Cells too large for the mask store (> NB_MAXP particles or > NS_CHUNK
 // candidates) set *fallback and are handled by the two-pass kernels above.
-constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32;
+constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32, NB_PB = 4;
 
 __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
                                                                    float L, float invL, float rc2, float band, int *__restrict__ count,
@@ -314,6 +314,7 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     __shared__ int cnt[NB_MAXP], loc[NB_MAXP];
     __shared__ int run_lo[18], run_cum[19];
     __shared__ unsigned long long base_s;
+    __shared__ int self_s;
     const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int first = cell_start[cell], np = cell_start[cell + 1] - first;
     if (np == 0) return;
@@ -352,44 +353,65 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     // the two forms) the pair is re-evaluated with dist2 on the unshifted position.
     const bool fast = nc >= 5;
     const float edge = L / (float)nc, mx = ((float)cx + 0.5f) * edge, my = ((float)cy + 0.5f) * edge, mz = ((float)cz + 0.5f) * edge;
-    for (int c = tid; c < total; c += NS_THREADS) {
-        int r = 0;
-        while (run_cum[r + 1] <= c) ++r;
-        const int j = run_lo[r] + c - run_cum[r];
-        float4 q = pos[j];
-        if (fast) { q.x -= L * rintf((q.x - mx) * invL); q.y -= L * rintf((q.y - my) * invL); q.z -= L * rintf((q.z - mz) * invL); }
-        q.w = __int_as_float(j);
-        cpos[c] = q;
-    }
-    __syncthreads();
     const int nwords = (total + 31) >> 5;
-    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass A: distance tests, masks, counts
-        const int s = first + pi;
-        const float4 p = pos[s];
-        int found = 0;
+    for (int r = wid; r < 18; r += NS_THREADS / 32) {            // staging: a warp per run, no search for the run of a candidate
+        const int lo = run_lo[r], c0 = run_cum[r], len = run_cum[r + 1] - c0;
+        if (first >= lo && first < lo + len && lane == 0) self_s = c0 + first - lo;     // where the cell's own particles sit
+        for (int i = lane; i < len; i += 32) {
+            float4 q = pos[lo + i];
+            if (fast) { q.x -= L * rintf((q.x - mx) * invL); q.y -= L * rintf((q.y - my) * invL); q.z -= L * rintf((q.z - mz) * invL); }
+            q.w = __int_as_float(lo + i);
+            cpos[c0 + i] = q;
+        }
+    }
+    // padding of the last word: infinitely far, index -1 (d^2 = inf: neither a hit nor inside the band)
+    if (tid < nwords * 32 - total) cpos[total + tid] = make_float4(3e37f, 3e37f, 3e37f, __int_as_float(-1));
+    __syncthreads();
+    const int self0 = self_s;
+    // pass A: distance tests, masks, counts.  A warp takes NB_PB particles at a time so that one staged candidate
+    // (one LDS.128 per lane) is tested against all of them; the particle's own entry (d^2 = 0, always a hit) is
+    // cleared afterwards instead of being tested for in the loop.
+    for (int pi0 = wid * NB_PB; pi0 < np; pi0 += (NS_THREADS / 32) * NB_PB) {
+        float4 p[NB_PB];
+        int found[NB_PB];
+#pragma unroll
+        for (int b = 0; b < NB_PB; ++b) { p[b] = pos[first + min(pi0 + b, np - 1)]; found[b] = 0; }
         for (int w = 0; w < nwords; ++w) {
-            const int c = w * 32 + lane;
-            bool in = false, exact = false;
-            float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
-            int j = s;
-            if (c < total) { q = cpos[c]; j = __float_as_int(q.w); }
-            if (j != s) {
-                if (fast) {
-                    const float dx = p.x - q.x, dy = p.y - q.y, dz = p.z - q.z, d2 = dx * dx + dy * dy + dz * dz;
-                    in = d2 < rc2;
-                    exact = fabsf(d2 - rc2) <= band;
-                } else {
-                    exact = true;
+            const float4 q = cpos[w * 32 + lane];
+            bool in[NB_PB], anyex = false;
+#pragma unroll
+            for (int b = 0; b < NB_PB; ++b) {
+                const float dx = p[b].x - q.x, dy = p[b].y - q.y, dz = p[b].z - q.z, d2 = dx * dx + dy * dy + dz * dz;
+                in[b] = d2 < rc2;
+                anyex = anyex || !(fabsf(d2 - rc2) > band);
+            }
+            if (__any_sync(0xffffffffu, anyex || !fast)) {       // rare on the screened path: a real branch, not predication
+                const int j = __float_as_int(q.w);
+                if (j >= 0) {
+                    const float4 qe = fast ? pos[j] : q;
+#pragma unroll
+                    for (int b = 0; b < NB_PB; ++b) {
+                        const float dx = p[b].x - q.x, dy = p[b].y - q.y, dz = p[b].z - q.z, d2 = dx * dx + dy * dy + dz * dz;
+                        if (!fast || !(fabsf(d2 - rc2) > band)) in[b] = dist2(p[b], qe, L, invL) < rc2;
+                    }
                 }
             }
-            if (__any_sync(0xffffffffu, exact)) {                // rare on the screened path: a real branch, not predication
-                if (exact) in = dist2(p, fast ? pos[j] : q, L, invL) < rc2;
+#pragma unroll
+            for (int b = 0; b < NB_PB; ++b) {
+                const unsigned m = __ballot_sync(0xffffffffu, in[b]);
+                if (lane == 0 && pi0 + b < np) masks[pi0 + b][w] = m;
+                found[b] += __popc(m);
             }
-            const unsigned m = __ballot_sync(0xffffffffu, in);
-            if (lane == 0) masks[pi][w] = m;
-            found += __popc(m);
         }
-        if (lane == 0) cnt[pi] = found;
+        if (lane == 0) {
+#pragma unroll
+            for (int b = 0; b < NB_PB; ++b)
+                if (pi0 + b < np) {
+                    const int sc = self0 + pi0 + b;
+                    masks[pi0 + b][sc >> 5] &= ~(1u << (sc & 31));
+                    cnt[pi0 + b] = found[b] - 1;
+                }
+        }
     }
     __syncthreads();
     if (tid < 32) {                                           // exclusive prefix of the <= 64 counts, one reservation
@@ -406,21 +428,17 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     }
     __syncthreads();
     const unsigned long long base = base_s;
-    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks, a lane per 32-candidate word
+    for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks word by word, a lane per candidate
         const int s = first + pi;
         const unsigned long long o = base + (unsigned long long)loc[pi];
         if (lane == 0) { off[s] = o; count[s] = cnt[pi]; }
         if (o + (unsigned long long)cnt[pi] > cap) continue;  // overflow: the host re-runs with a larger index array
-        unsigned m = lane < nwords ? masks[pi][lane] : 0u;
-        const int mine = __popc(m);
-        int inc = mine;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-        int *dst = idx + o + (inc - mine);
-        while (m) {                                           // ascending bit order keeps the list sorted by candidate
-            const int b = __ffs(m) - 1;
-            m &= m - 1;
-            *dst++ = __float_as_int(cpos[lane * 32 + b].w);
+        int *dst = idx + o;
+        const unsigned lt = (1u << lane) - 1u;
+        for (int w = 0; w < nwords; ++w) {                    // ascending candidate order; consecutive hits, consecutive addresses
+            const unsigned m = masks[pi][w];
+            if ((m >> lane) & 1u) dst[__popc(m & lt)] = __float_as_int(cpos[w * 32 + lane].w);
+            dst += __popc(m);
         }
     }
 }
