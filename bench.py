@@ -79,6 +79,11 @@ class ClockSampler:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/r1_traffic.md), default workload only; other workloads report null.
+# fp32 operations per pair evaluation of real_pairs_kernel (ncu: fadd + fmul + 2 ffma predicated-on thread instructions / pairs,
+# profiles/r1_ncu_kernels.md): 161 for the full 8 x 8 product (Lanczos iterations), 128 for S -> E (GMRES iterations); a step runs
+# seven of each plus two mixed products, so their mean is used
+FLOP_PER_PAIR = 0.5 * (161.0 + 128.0)
+N_SM, FP32_LANES_PER_SM = 148, 128                # B200: 4 sub-partitions x 32 fp32 lanes per SM (blackwell guide), FMA = 2 flop
 NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 3478528, 'interp': 23429120, 'scale': 20024832, 'neighbors': 1098240}}
 
 
@@ -359,6 +364,17 @@ def main():
                                 f'{r["profiled_steps"]} profiled steps; ' + (
                                     'at this size the grids are L2-resident (see DESIGN.md §5)' if 64 * r['grid']**3 < 100e6 else
                                     'the 8 real + 8 spectral grids exceed the L2 (see DESIGN.md §5)')}
+    if dom == 'real':
+        # the pair kernel moves few bytes per flop (its gathers are served by L1/L2): the binding roofline is fp32 issue, not HBM
+        hbm_view = {k: line['roofline'][k] for k in ('achieved', 'peak', 'unit', 'frac')}
+        clock_ghz = (r['clocks'].get('sm_mhz') or r['clocks'].get('sm_max_mhz') or 1965.0) / 1e3
+        peak_tf = N_SM * FP32_LANES_PER_SM * 2 * clock_ghz / 1e3
+        tf = phases['real']['pairs_per_sec'] * FLOP_PER_PAIR / 1e12
+        line['roofline'].update({'bound': 'alu', 'achieved': tf, 'peak': peak_tf, 'unit': 'TFLOP/s', 'frac': tf / peak_tf, 'hbm_view': hbm_view,
+                                 'peak_source': f'{N_SM} SMs x {FP32_LANES_PER_SM} fp32 lanes x 2 flop x {clock_ghz:.3f} GHz (median SM clock under load in this run)',
+                                 'note': f'pair evaluations/s x {FLOP_PER_PAIR:.1f} fp32 operations per pair (ncu count, profiles/r1_ncu_kernels.md); the kernel is '
+                                         'bound by gather latency and instruction issue (ncu: issue slots 50 % busy, FMA pipe 32 %), its DRAM traffic '
+                                         '(traffic, bytes per launch) is the neighbour list; hbm_view = algorithmic bytes / launch time against the measured HBM peak'})
     line['phases'] = phases
     line['cufft_share_of_step'] = fft_share
     if not args.no_cpu_baseline:
