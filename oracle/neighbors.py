@@ -19,14 +19,14 @@ def wrap32(pos, L):
     return w
 
 
-def neighbor_sets(pos, L, rcut):
-    """List (length N) of sorted int arrays: all beta != alpha with minimum-image fp32 r2 < rcut^2."""
+def neighbor_sets(pos, L, rcut, rows=None):
+    """List (length N, or len(rows)) of sorted int arrays: all beta != alpha with minimum-image fp32 r2 < rcut^2."""
     x = wrap32(pos, L)
     L32 = f32(L)
     invL = f32(1.0) / L32
     rc2 = f32(rcut) * f32(rcut)
     out = []
-    for a in range(x.shape[0]):
+    for a in (range(x.shape[0]) if rows is None else rows):
         d = (x[a][None, :] - x).astype(f32)
         d = (d - (L32 * np.rint((d * invL).astype(f32)).astype(f32)).astype(f32)).astype(f32)
         sq = (d * d).astype(f32)

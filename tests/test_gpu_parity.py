@@ -245,6 +245,46 @@ def test_product_mid_size_sampled_rows(N, phi, tol, xi, seed):
     assert rel(U[rows], Uo) < bar(tol) and rel(E[rows], Eo) < bar(tol)
 
 
+def test_config4_full_size_sampled_neighbors_rows_and_properties():
+    """BASELINE.json configs[3] (N=1 048 576, phi=0.10, tol=1e-3) with bench.py's parameters (xi=0.34, grid 216, P=4).  The
+    O(N^2) oracle cannot finish here, so: (i) neighbour sets of sampled particles bit-exact against the fp32 brute force;
+    (ii) the real-space product exactly on sampled rows; (iii) the full product independent of xi (0.34 against 0.42:
+    other r_cut, grid, tables) and symmetric."""
+    import paper_1709_06946_b200 as pse
+    N, phi, tol = 1048576, 0.10, 1e-3
+    x, L = synth.rsa(N, phi, seed=4)
+    x32 = x.astype(np.float32)
+    F, S = synth.gaussian_inputs(N, 1)
+    F2, S2 = synth.gaussian_inputs(N, 2)
+    rows = np.sort(np.random.default_rng(4).choice(N, 12, replace=False))
+    res = {}
+    for xi in (0.34, 0.42):
+        st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+        assert st == 0 and (xi != 0.34 or (grid, P) == (216, 4))
+        ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+        ctx.pse_neighbors(dev(pos4(x32)))
+        if xi == 0.34:
+            count, index = ctx.pse_get_neighbors()
+            count = count.cpu().numpy()
+            off = np.concatenate([[0], np.cumsum(count)])
+            want = nbo.neighbor_sets(pos4(x32), L, rcut, rows=rows)
+            for r, w in zip(rows, want):
+                got = np.sort(index[off[r]:off[r + 1]].cpu().numpy())
+                assert np.array_equal(got, w)
+            assert abs(count.mean() - 65.9) < 1.0
+        res[xi] = dict(full=np.hstack(gpu_apply(ctx, F, S, 3)), real=np.hstack(gpu_apply(ctx, F, S, 1)), rcut=rcut,
+                       full2=np.hstack(gpu_apply(ctx, F2, S2, 3)))
+        ctx.close()
+    assert rel(res[0.34]['full'], res[0.42]['full']) < bar(tol)
+    v1, v2 = np.hstack([F, S]).astype(np.float64), np.hstack([F2, S2]).astype(np.float64)
+    a, b = res[0.34]['full'].astype(np.float64), res[0.34]['full2'].astype(np.float64)
+    d12, d21 = float((v1 * b).sum()), float((v2 * a).sum())
+    assert abs(d12 - d21) < bar(tol) * np.sqrt(float((v1 * a).sum()) * float((v2 * b).sum()))
+    assert float((v1 * a).sum()) > 0
+    Ur, Er = mob.real_apply(x32.astype(np.float64), L, A, ETA, 0.34, F, S, rows=rows[:6], rcut=res[0.34]['rcut'])
+    assert rel(res[0.34]['real'][rows[:6]], np.hstack([Ur, Er])) < 2e-5
+
+
 @pytest.mark.parametrize('grid', [35, 45])
 def test_odd_grid_component_masks(grid):
     """Odd M: M^3 is odd, so the S / E planes (first plane 3) of a packed [8][M^3] array would start 4-byte aligned only
