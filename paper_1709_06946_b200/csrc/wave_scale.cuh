@@ -15,10 +15,13 @@ struct ScaleParams {
     int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
 };
 
-__device__ __forceinline__ float shape_s1(float x) {     // 3 (sin x - x cos x)/x^3, series below 0.5 (cancellation)
-    if (x < 0.5f) { float x2 = x * x; return 1.f - x2 * (0.1f - x2 * (1.f / 280.f - x2 * (1.f / 15120.f))); }
+// s0 = sin x / x and s1 = 3 (sin x - x cos x)/x^3 (series below 0.5: cancellation) from one sincosf, x > 0
+__device__ __forceinline__ void shape_factors(float x, float &s0, float &s1) {
     float s, c; sincosf(x, &s, &c);
-    return 3.f * (s - x * c) / (x * x * x);
+    const float ix = 1.f / x;
+    s0 = s * ix;
+    if (x < 0.5f) { const float x2 = x * x; s1 = 1.f - x2 * (0.1f - x2 * (1.f / 280.f - x2 * (1.f / 15120.f))); }
+    else s1 = 3.f * (s - x * c) * (ix * ix * ix);
 }
 
 // Wave vector of half-spectrum entry (ix,iy,iz); returns false for k = 0 and Nyquist modes (weight set to zero in
@@ -69,7 +72,8 @@ __device__ __forceinline__ void scale_point(const ScaleParams &sp, int ix, int i
         return;
     }
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
-    const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
+    float s0, s1;
+    shape_factors(ka, s0, s1);
     const float q = k2 * sp.inv4xi2;
     const float dw = __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);            // one window undone for spreading,
     const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-q) / k2 * dw * dw;          // one for interpolation

@@ -367,10 +367,12 @@ interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_
 }
 
 // a5 (cuFFT path): one thread per half-spectrum mode, in place
+// (grid.y = ix, grid.x covers the (iy, iz) plane: 32-bit index arithmetic, no 64-bit division per thread)
 __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScaleParams sp) {
-    const size_t nmode = (size_t)sp.M * sp.M * sp.Mh, o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= nmode) return;
-    const int iz = (int)(o % sp.Mh), iy = (int)((o / sp.Mh) % sp.M), ix = (int)(o / ((size_t)sp.Mh * sp.M));
+    const unsigned plane = (unsigned)sp.M * (unsigned)sp.Mh, rem = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rem >= plane) return;
+    const int ix = (int)blockIdx.y, iy = (int)(rem / (unsigned)sp.Mh), iz = (int)(rem - (unsigned)iy * (unsigned)sp.Mh);
+    const size_t nmode = (size_t)plane * sp.M, o = (size_t)ix * plane + rem;
     scale_point(sp, ix, iy, iz, spec, nmode, o, spec, nmode, o);
 }
 
@@ -378,10 +380,11 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
 // W(k) = (g_re + i g_im)/sqrt2 from the noise buffer; in the plane kz = 0 the non-canonical member of each +-k
 // pair takes the conjugate of its partner's entry (reading R8) so that the C2R transform sees a Hermitian field.
 __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec, const float2 *__restrict__ noise, ScaleParams sp) {
-    const size_t nmode = (size_t)sp.M * sp.M * sp.Mh, o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= nmode) return;
     const int M = sp.M;
-    const int iz = (int)(o % sp.Mh), iy = (int)((o / sp.Mh) % M), ix = (int)(o / ((size_t)sp.Mh * M));
+    const unsigned plane = (unsigned)M * (unsigned)sp.Mh, rem = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rem >= plane) return;
+    const int ix = (int)blockIdx.y, iy = (int)(rem / (unsigned)sp.Mh), iz = (int)(rem - (unsigned)iy * (unsigned)sp.Mh);
+    const size_t nmode = (size_t)plane * M, o = (size_t)ix * plane + rem;
     float kx, ky, kz;
     float2 zero = make_float2(0.f, 0.f);
     // the noise buffer has the ABI's [M][M][Mh] layout; the spectrum rows may be padded to Mhp entries
@@ -399,7 +402,8 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
 #pragma unroll
     for (int c = 0; c < 3; ++c) { float2 g = noise[c * nmode + src]; W[c] = make_float2(g.x * WS_RS2, sgn * g.y * WS_RS2); }
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
-    const float s0 = sinf(ka) / ka, s1 = shape_s1(ka);
+    float s0, s1;
+    shape_factors(ka, s0, s1);
     const float q = k2 * sp.inv4xi2;
     const float Bh = sp.c_br * sqrtf(sp.inv_eta * (1.f + q) / k2) * __expf(-0.5f * q) * __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);
     const float ik2 = 1.f / k2;
@@ -533,7 +537,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[plan], c->d_grid + first * M3, c->d_spec + first * nmode)); c->launches++; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
-        scale_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c, mode)); KERNEL_CHECK(c);
+        scale_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c, mode)); KERNEL_CHECK(c);
     }
     return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp, mode);
 }
@@ -543,7 +547,7 @@ pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out
     if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
-        scale_brownian_kernel<<<(unsigned)((nmode + 255) / 256), 256, 0, c->stream>>>(
+        scale_brownian_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(
             c->d_spec, reinterpret_cast<const float2 *>(d_noise_wave), make_scale_params(c));
         KERNEL_CHECK(c);
         if (c->own_fft) PSE_TRY(pse_fft_x_inverse(c));
