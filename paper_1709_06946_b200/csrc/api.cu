@@ -151,6 +151,7 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_real, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise, cudaEventDisableTiming));
+    CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise_r, cudaEventDisableTiming));
     if (const char *e = getenv("PSE_OVERLAP")) c->overlap = (e[0] != '0');
     return PSE_OK;
 }
@@ -162,6 +163,7 @@ pse_status pse_destroy(pse_ctx *c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_real) cudaEventDestroy(c->ev_real);
     if (c->ev_noise) cudaEventDestroy(c->ev_noise);
+    if (c->ev_noise_r) cudaEventDestroy(c->ev_noise_r);
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
@@ -199,6 +201,7 @@ pse_status pse_mobility_apply(pse_ctx *c, const float *d_F, const float *d_S, fl
 pse_status pse_brownian(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters) {
     if (!c || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_brownian before pse_neighbors"; return PSE_ENOTREADY; }
+    if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
     PSE_TRY(pse_pack8(c, d_noise_real, c->d_in));
     pse_status st = pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters);
     if (st != PSE_OK && st != PSE_ENOCONV) return st;
@@ -307,16 +310,20 @@ pse_status pse_step_host(pse_ctx *c, float *h_pos, double dt, const float *h_noi
     PSE_TRY(ensure_stage(c, true));
     const size_t N = (size_t)c->N, nw = (size_t)6 * c->M * c->M * c->Mh;
     CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_pos, h_pos, N * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_a, h_noise_real, N * 8 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    // the wave-space noise (the bulk of the input: 24 bytes per half-spectrum mode) is first needed after the neighbour
-    // build and the Lanczos iteration: its copy runs on the second stream and pse_wave_brownian waits for it
-    CUDA_TRY(c, cudaEventRecord(c->ev_fork, c->stream));                         // the previous call's use of the buffer is over
+    // only the positions are needed at once (neighbour build).  The real-space noise is first read by the Lanczos start and
+    // the wave-space noise (the bulk of the input: 24 bytes per half-spectrum mode) after the Lanczos iteration: both
+    // copies run on the second stream, in that order, and pse_brownian / pse_wave_brownian wait for them
+    CUDA_TRY(c, cudaEventRecord(c->ev_fork, c->stream));                         // the previous call's use of the buffers is over
     CUDA_TRY(c, cudaStreamWaitEvent(c->stream2, c->ev_fork, 0));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_a, h_noise_real, N * 8 * sizeof(float), cudaMemcpyHostToDevice, c->stream2));
+    CUDA_TRY(c, cudaEventRecord(c->ev_noise_r, c->stream2));
+    c->noise_r_pending = true;
     CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_noise, h_noise_wave, nw * sizeof(float), cudaMemcpyHostToDevice, c->stream2));
     CUDA_TRY(c, cudaEventRecord(c->ev_noise, c->stream2));
     c->noise_pending = true;
     pse_status st = pse_step(c, c->d_stage_pos, dt, c->d_stage_a, c->d_stage_noise, gmres_iters, lanczos_iters);
-    if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }   // step failed early
+    if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }   // step failed early
+    if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
     if (st != PSE_OK && st != PSE_ENOCONV) return st;
     CUDA_TRY(c, cudaMemcpyAsync(h_pos, c->d_stage_pos, N * 4 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));

@@ -29,7 +29,8 @@ struct pse_ctx {
     float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index
     cudaStream_t stream = nullptr;
     cudaStream_t stream2 = nullptr;          // real-space half of a full product runs here, concurrently with the wave half
-    cudaEvent_t ev_fork = nullptr, ev_real = nullptr, ev_noise = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_real = nullptr, ev_noise = nullptr, ev_noise_r = nullptr;
+    bool noise_r_pending = false;            // pse_step_host: the real-space noise upload on stream2 has not been waited for yet
     bool noise_pending = false;              // pse_step_host: the wave-noise upload on stream2 has not been waited for yet
     bool overlap = false;                    // measured neutral (1M) to slightly slower (65k): off unless PSE_OVERLAP=1
     std::string err;
