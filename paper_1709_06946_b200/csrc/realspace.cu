@@ -29,10 +29,15 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
     // all eight 16-byte bank groups; the interleaved 32-byte rows reached only four (ncu: 17 wavefronts per LDS.128)
     extern __shared__ float4 tab[];               // tabU[PSE_NTAB] then tabE[PSE_NTAB]
     float4 *tabU = tab, *tabE = tab + PSE_NTAB;
-    for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) { tabU[i] = table[2 * i]; tabE[i] = table[2 * i + 1]; }
-    __syncthreads();
     constexpr bool INF = MODE & PSE_IN_F, INS = MODE & PSE_IN_S, OUTU = MODE & PSE_OUT_U, OUTE = MODE & PSE_OUT_E;
     constexpr bool NEED_TU = (OUTU) || (INF && OUTE), NEED_TE = INS && OUTE;
+    // only the half of the table the component mask reads is staged (32 KB per CTA less for S -> E); row 0 of both halves
+    // is always there for the self term
+    for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) {
+        if (NEED_TU || i == 0) tabU[i] = table[2 * i];
+        if (NEED_TE || i == 0) tabE[i] = table[2 * i + 1];
+    }
+    __syncthreads();
     // G lanes per particle (32 / G particles per warp): a list of ~51 entries fills 7 passes of 8 lanes to 91 %, two
     // passes of 32 lanes only to 80 %
     constexpr int PPW = 32 / G;
