@@ -289,12 +289,15 @@ def main():
     ap.add_argument('--no-cpu-baseline', action='store_true')
     ap.add_argument('--xi', type=float, default=None, help='override the splitting parameter (tuning knob, PAPER.md:154)')
     ap.add_argument('--tol', type=float, default=None, help='override the Ewald tolerance of the workload')
+    ap.add_argument('--particles', type=int, default=None, help='override N of the workload (size sweep; phi, tol and xi are kept)')
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
     if args.xi:
         wl['xi'] = args.xi
     if args.tol:
         wl['tol'] = args.tol
+    if args.particles:
+        wl['N'] = args.particles
     rank, world = int(os.environ.get('RANK', 0)), int(os.environ.get('WORLD_SIZE', 1))
     config = {'workload': f'{args.workload}: N={wl["N"]} {"spheres in 32-sphere fractal aggregates" if wl.get("fractal") else "hard spheres"}, phi={wl["phi"]}, Ewald tol={wl["tol"]}, xi={wl["xi"]}, '
                           f'dt={wl["dt"]}, kT=1, RSA placement' + (f' + {wl["relax"]} relax sweeps' if wl['relax'] else ''),
@@ -359,7 +362,7 @@ def main():
     line['e2e'] = {'value': 1e3 / r['e2e_ms'], 'unit': 'steps/s', 'h2d_bytes_per_step': r['h2d'], 'd2h_bytes_per_step': r['d2h'],
                    'api': 'pse_step_host (pinned host buffers, copies inside the timed call)', 'steps': r['e2e_steps']}
     line['roofline'] = {'bound': 'hbm', 'kernel': dom, 'achieved': phases[dom]['alg_GBps'], 'peak': peak, 'unit': 'GB/s',
-                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not (args.xi or args.tol) else None, 'peak_source': peak_src,
+                        'frac': phases[dom]['alg_GBps'] / peak, 'traffic': NCU_TRAFFIC.get(args.workload, {}).get(dom) if not (args.xi or args.tol or args.particles) else None, 'peak_source': peak_src,
                         'note': 'algorithmic bytes per launch / mean launch duration from CUDA events inside the library over '
                                 f'{r["profiled_steps"]} profiled steps; ' + (
                                     'at this size the grids are L2-resident (see DESIGN.md §5)' if 64 * r['grid']**3 < 100e6 else
