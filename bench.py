@@ -84,7 +84,8 @@ class ClockSampler:
 # seven of each plus two mixed products, so their mean is used
 FLOP_PER_PAIR = 0.5 * (161.0 + 128.0)
 N_SM, FP32_LANES_PER_SM = 148, 128                # B200: 4 sub-partitions x 32 fp32 lanes per SM (blackwell guide), FMA = 2 flop
-NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 3478528, 'interp': 23429376, 'scale': 20020224, 'neighbors': 1101056}}
+NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 3478528, 'interp': 23429376, 'scale': 20020224, 'neighbors': 1101056},
+               'config4': {'real': 374564352, 'spread': 327781888, 'interp': 288555520, 'scale': 347489536, 'neighbors': 251551488}}   # profiles/r1_config4.md
 
 
 def max_over_ranks(ms, device=None):
