@@ -20,6 +20,14 @@ constexpr float RS6 = 0.40824829046386302f;   // 1/sqrt6
 
 // MODE = PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: terms of absent inputs / outputs are removed at compile time
 // (inside GMRES the operator is S -> E: no U accumulation, no F terms, and only the E-part table is read).
+// The packed input of a particle ([8] floats, 32-byte aligned = one sector) in ONE 256-bit load (LDG.E.256, new on sm_100)
+// instead of two 128-bit ones: a third fewer load instructions and L1 requests per pair.
+__device__ __forceinline__ void load_packed8(const float4 *in, int b, float4 &a0, float4 &a1) {
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(a0.x), "=f"(a0.y), "=f"(a0.z), "=f"(a0.w), "=f"(a1.x), "=f"(a1.y), "=f"(a1.z), "=f"(a1.w)
+                 : "l"(in + 2 * (size_t)b));
+}
+
 template <int MODE, int G>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
@@ -54,9 +62,10 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
         int b = j < hi ? idx[j] : 0;
         float4 q4 = pos[b];
         for (; j < hi; j += G) {
-            float4 a0 = in[2 * b], a1 = in[2 * b + 1];
+            float4 a0, a1;
+            if (INS) load_packed8(in, b, a0, a1);
+            else { a0 = in[2 * b]; a0.w = 0.f; a1 = make_float4(0.f, 0.f, 0.f, 0.f); }
             if (!INF) { a0.x = 0.f; a0.y = 0.f; a0.z = 0.f; }
-            if (!INS) { a0.w = 0.f; a1 = make_float4(0.f, 0.f, 0.f, 0.f); }
             const int bn = (j + G < hi) ? idx[j + G] : b;
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
