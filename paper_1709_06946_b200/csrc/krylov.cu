@@ -321,7 +321,8 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     // synchronisation that idles the GPU) is skipped until one iteration before the count the previous call needed;
     // the skipped iterations are then examined in order and the first converged one is taken — same result as
     // checking every time.
-    const int first_check = std::max(0, c->last_lanczos_iters - 2);
+    // (once the count has repeated, only the iteration it is expected to end in is read back: one synchronisation per solve)
+    const int first_check = std::max(0, c->last_lanczos_iters - (c->lanczos_repeats >= 2 ? 1 : 2));
     int examined = 0;
     for (int j = 0; j < maxit && !converged; ++j) {
         float4 *vj = V + (size_t)j * n4;
@@ -362,6 +363,7 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
             else if (beta[e_j] <= 1e-7 * std::fabs(alpha[0])) converged = true;                          // invariant subspace
         }
     }
+    c->lanczos_repeats = (m == c->last_lanczos_iters) ? c->lanczos_repeats + 1 : 0;
     c->last_lanczos_iters = m;
     std::vector<float> cf(ccur.begin(), ccur.end());
     PSE_TRY(upload_coefs(c, cf));
@@ -399,7 +401,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     std::vector<double> H((size_t)(maxit + 1) * maxit, 0.0), cs(maxit, 0.0), sn(maxit, 0.0), g(maxit + 1, 0.0), y;
     bool converged = false;
     {
-        const int first_check = std::max(0, c->last_gmres_iters - 2);     // see pse_lanczos_sqrt
+        const int first_check = std::max(0, c->last_gmres_iters - (c->gmres_repeats >= 2 ? 1 : 2));     // see pse_lanczos_sqrt
         int examined = 0;
         for (int k = 0; k < maxit && !converged; ++k) {
             const int base = 1 + k * (k + 3) / 2;
@@ -439,6 +441,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
                 else if (hk1 <= 1e-12 * bnorm) converged = true;
             }
         }
+        c->gmres_repeats = (m == c->last_gmres_iters) ? c->gmres_repeats + 1 : 0;
         c->last_gmres_iters = m;
         y.assign(m, 0.0);
         for (int i = m - 1; i >= 0; --i) {

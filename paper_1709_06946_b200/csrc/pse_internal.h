@@ -74,6 +74,7 @@ struct pse_ctx {
     double *h_scal = nullptr;                // pinned mirror
     float *d_coef = nullptr;                 // small coefficient vector upload
     int last_lanczos_iters = 0, last_gmres_iters = 0;   // iteration counts of the previous solves (when to start reading back)
+    int lanczos_repeats = 0, gmres_repeats = 0;         // how many solves in a row ended with that same count
     unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
     float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
     float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
