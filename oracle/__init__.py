@@ -17,12 +17,19 @@ It is a plain, slow, obviously-correct statement of what the path computes:
                    the equilibrium test potential U = k|r - r0| and Eq. (80); the constrained
                    mobility R_FU^-1 of Eq. (B15) and its divergence, the drift of Eq. (B12).
 * ``neighbors``  – brute-force fp32 neighbour sets.
+* ``pse_reference`` (+ ``pse_ref.c``, ``krylov``) – second tier: the paper's own fast scheme in fp64 (linked-cell pair sum,
+                   Gaussian NUFFT of Eq. 42 with scipy's FFT, textbook Lanczos / GMRES), pinned against the direct sums at
+                   N <= 4 096; the parity reference at N >= 65 536 and bench.py's second timed CPU baseline.
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): Hasimoto periodic self-mobility, xi-independence of
 M_r + M_w, symmetry and positive-definiteness of M, M_r, M_w, textbook RPY / RPY-overlap free-space
 limits, printed closed forms F1, F2 of Appendix A, exact covariance identity
 A_w A_w^T = M_w(grid modes), Schur-complement constraint solve, bond force = -grad U, Eq. (80) normalised
-Boltzmann density, a short two-sphere run against Eq. (80), div M_UF = 0.
+Boltzmann density, a short two-sphere run against Eq. (80), div M_UF = 0, printed K3 / G1 (r > 2a) / (A12)
+(PAPER.md:670, 723, 737, 744), the mid-point step written out by hand from the dense matrices, the Brownian amplitude
+against its dense factors, and the Heyes-Melrose force (not in the paper; reading R12) by the property that defines it:
+a free-draining pair ends at contact after one dt.  The PSE reference is pinned in tests/test_pse_reference.py.
 
-Parity unpinned (not in the paper): the Heyes-Melrose hard-sphere force (reading R12 in DESIGN.md).
+Parity unpinned: none of the functions on the timed path; the RSA / aggregate generators live in synth/ (no method
+arithmetic) and are checked only for "no overlaps".
 """

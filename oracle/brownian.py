@@ -37,12 +37,15 @@ def grid_modes(Mg, L):
     return 2 * np.pi * np.concatenate([n, -n]) / L
 
 
-def wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, chunk=None):
+def wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, chunk=None, rows=None):
     """A_w w2.  wbuf: real array [3][Mg][Mg][Mg/2+1][2] of i.i.d. N(0,1).  For each canonical mode
     W(k) = (g_re + i g_im)/sqrt2, W(-k) = conj W(k), so the pair contributes 2 Re[...]:
         uh = sqrt(H/(eta V k^2)) (I - kh kh) W ;  U_a = sum_k e^{ik.x_a} s0 uh ;  E^q_a = sum_k e^{ik.x_a} i s1 (e^q k).uh
+    rows restricts the particles a the sum is evaluated at (the noise field does not depend on the particles).
     """
     x = np.asarray(x, dtype=np.float64)
+    if rows is not None:
+        x = x[np.asarray(rows)]
     N = x.shape[0]
     wbuf = np.asarray(wbuf, dtype=np.float64).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
     idx, n = canonical_modes(Mg)
@@ -93,7 +96,8 @@ def brownian(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14):
 
 
 def heyes_melrose(x, L, a, eta, dt):
-    """Hard-sphere overlap force, reading R12 (named by BASELINE.json, not in the paper — parity unpinned):
+    """Hard-sphere overlap force, reading R12 (named by BASELINE.json, not in the paper; pinned by the property that defines it:
+    a free-draining pair moved by it for one dt ends exactly at contact, tests/test_oracle_pins.py):
     F_i = sum_{j: r_ij < 2a} 3 pi eta a (2a - r_ij)/dt rhat_ij,  rhat_ij = (x_i - x_j)/r_ij (minimum image)."""
     x = np.asarray(x, dtype=np.float64)
     d = x[:, None, :] - x[None, :, :]

@@ -1,0 +1,361 @@
+"""fp64 CPU PSE reference: the paper's own fast scheme, step by step, in double precision.  Test infrastructure only.
+
+    M = M_r + M_w,   M_w = sigma Q^T F^H P^H B P F Q        (Eq. 42)
+    M_r: cut-off pair sum over linked cells
+
+This is the second tier of the oracle (SURVEY.md 8(c) "two-tier oracle"): the O(N^2) direct sums of
+``oracle.mobility`` cannot finish at N >= 65 536, this can.  It is pinned against the direct sums at N <= 4 096
+(tests/test_pse_reference.py) and is then (i) the reference of the full-size GPU parity tests on sampled rows and
+(ii) the second timed CPU baseline of bench.py.  It shares no code with the CUDA path: Gaussian window exactly as
+the paper states it (eta_g = (h P xi/m)^2 with m = sqrt(pi P)), scipy's FFT for the
+bare transform, real-space functions from ``oracle.functions`` (free-space closed form minus quadrature of the
+Gaussian-damped wave integral).  The three particle loops are plain C + OpenMP (oracle/pse_ref.c, compiled on
+first use with gcc); everything else is numpy.
+
+Steps of the wave-space product, in the paper's order (constants: DESIGN.md reading R4):
+    1. Q    spread the 8 components with K(r) = (2 xi^2/(pi eta_g))^{3/2} exp(-2 xi^2 r^2/eta_g), P^3 points
+    2. F    un-normalised real-to-complex 3-D FFT of every grid
+    3. P^H B P   fh = s0 Fh - i s1 Sh.k ;  uh = (h^3/V) H(k) exp(+eta_g k^2/4xi^2)/(eta k^2) (I - kh kh) fh ;
+                 Uh = s0 uh ; Eh^q = i s1 (e^q k).uh                                             (Eqs. 40-41)
+    4. F^H  un-normalised complex-to-real inverse FFT
+    5. sigma Q^T  interpolate with weight h^3 K
+The k = 0 mode is dropped and the Nyquist planes of an even grid carry zero weight (reading R8).
+"""
+import ctypes
+import functools
+import os
+import subprocess
+
+import numpy as np
+import scipy.fft as sfft
+from scipy.interpolate import CubicSpline
+from scipy.spatial import cKDTree
+
+from . import functions as fn
+from . import mobility as mob
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, 'pse_ref.c')
+_LIB = os.path.join(_HERE, 'libpse_ref.so')
+_lib = None
+
+
+def build(force=False):
+    """Compile oracle/pse_ref.c -> oracle/libpse_ref.so (gcc -O2 -fopenmp; no fast-math, no contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f'.{os.getpid()}.tmp'
+        subprocess.run(['gcc', '-O2', '-ffp-contract=off', '-fopenmp', '-fPIC', '-shared', _SRC, '-o', tmp, '-lm'], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        h = ctypes.CDLL(build())
+        dp, lp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_long)
+        h.ref_threads.restype = ctypes.c_int
+        h.ref_spread.argtypes = [ctypes.c_int, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, dp]
+        h.ref_interp.argtypes = [ctypes.c_int, lp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, dp, dp]
+        h.ref_pairs.argtypes = [ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                dp, ctypes.c_int, ctypes.c_double, ctypes.c_int, lp, dp, dp]
+        for f in (h.ref_spread, h.ref_interp, h.ref_pairs):
+            f.restype = None
+        _lib = h
+    return _lib
+
+
+def threads():
+    return int(lib().ref_threads())
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _lp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_long))
+
+
+def _c(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def gaussian_support(tol):
+    """Smallest P with 10 (e^{-pi P/2} + erfc sqrt(pi P/2)) <= tol: the paper's quadrature bound for m = sqrt(pi P)
+    (Eq. 55 with lambda_max = 1; P = 5 at 1e-3 in Table I) with a safety factor 10 because
+    the strain-rate rows carry an extra factor k."""
+    from scipy.special import erfc
+    P = 2
+    while 10.0 * (np.exp(-np.pi * P / 2) + erfc(np.sqrt(np.pi * P / 2))) > tol:
+        P += 1
+    return P
+
+
+@functools.lru_cache(maxsize=8)
+def _wave_table(xi, a, rcut, table_nodes, fine_nodes):
+    """Gaussian-damped wave integrals W_X(r) (smooth in r): exact quadrature on table_nodes, cubic spline, fine linear table
+    [fine_nodes][7] on [0, rcut] for the C pair loop.  Memoised: a step builds several PSEReference objects with one xi."""
+    rn = np.linspace(0.0, rcut, table_nodes)
+    W = fn.wave_integrals(rn, xi, a)
+    rf = np.linspace(0.0, rcut, fine_nodes)
+    return _c(np.stack([CubicSpline(rn, W[n])(rf) for n in fn.NAMES], axis=1)), float(rf[1] - rf[0])
+
+
+class PSEReference:
+    """fp64 PSE for N equal spheres of radius a in a cubic periodic box L, viscosity eta, splitting parameter xi.
+
+    tol sets every truncation: r_cut = sqrt(-ln tol)/xi + 2a (functions decay like exp(-xi^2 (r-2a)^2)),
+    grid M >= 1.1 * 2 xi sqrt(-ln tol) L/pi (even, FFT-friendly), Gaussian support P = gaussian_support(tol).
+    Any of rcut, M, P can be given instead (bench.py's timing leg uses the GPU run's xi, grid and r_cut)."""
+
+    def __init__(self, L, a, eta, xi, tol=1e-8, M=None, P=None, rcut=None, table_nodes=4097, fine_nodes=(1 << 17) + 1):
+        s = np.sqrt(-np.log(tol))
+        self.L, self.a, self.eta, self.xi, self.tol = float(L), float(a), float(eta), float(xi), float(tol)
+        self.rcut = float(rcut) if rcut is not None else s / xi + 2.0 * a
+        if self.rcut > 0.5 * L:
+            raise ValueError(f'PSEReference: r_cut {self.rcut:.3f} > L/2 = {0.5 * L:.3f} (minimum-image pair sum); raise xi')
+        if M is None:
+            M = int(np.ceil(1.1 * 2.0 * xi * s * L / np.pi))
+            M = max(8, M + (M & 1))
+            while sfft.next_fast_len(M, real=True) != M or (M & 1):
+                M += 1
+        self.M = int(M)
+        self.P = int(P) if P is not None else gaussian_support(tol)
+        if self.P > min(self.M, 64):
+            raise ValueError('PSEReference: support P exceeds the grid (or 64)')
+        self.h = self.L / self.M
+        self.eta_g = (self.h * self.P * xi) ** 2 / (np.pi * self.P)          # (h P xi/m)^2, m^2 = pi P
+        if not self.eta_g < 1.0:
+            raise ValueError(f'PSEReference: eta_g = {self.eta_g:.3f} >= 1 (grid too coarse for this xi and P)')
+        self.pref = 1.0 / (6.0 * np.pi * eta * a)
+        self.wtab, self.dr = _wave_table(float(xi), float(a), self.rcut, int(table_nodes), int(fine_nodes))
+
+    # ---- real space -------------------------------------------------------------------------------------------
+    def real_apply(self, x, F, S5, rows=None, exact=False):
+        """[U;E]_rows = M_r [F;S] truncated at r_cut.  exact=True evaluates the scalar functions of every pair by
+        quadrature (oracle.functions, no table) with pairs from a periodic k-d tree; default: linked cells + fine table
+        of the smooth wave integrals (oracle/pse_ref.c)."""
+        x = _c(np.asarray(x, dtype=np.float64) % self.L)
+        N = x.shape[0]
+        rows = np.arange(N, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        F, S5 = _c(F), _c(S5)
+        if exact:
+            return self._real_exact(x, F, S5, rows)
+        U, E = np.empty((rows.size, 3)), np.empty((rows.size, 5))
+        lib().ref_pairs(N, _dp(x), _dp(F), _dp(S5), self.L, self.a, self.rcut, self.pref, _dp(self.wtab), self.wtab.shape[0], self.dr,
+                        rows.size, _lp(rows), _dp(U), _dp(E))
+        return U, E
+
+    def _real_exact(self, x, F, S5, rows):
+        tree = cKDTree(x, boxsize=self.L)
+        nb = tree.query_ball_point(x[rows], self.rcut)
+        ia = np.concatenate([np.full(len(b), i, dtype=np.int64) for i, b in enumerate(nb)])
+        ib = np.concatenate([np.asarray(b, dtype=np.int64) for b in nb])
+        keep = rows[ia] != ib
+        ia, ib = ia[keep], ib[keep]
+        rv = x[rows[ia]] - x[ib]
+        rv -= self.L * np.round(rv / self.L)
+        r = np.linalg.norm(rv, axis=1)
+        m = r < self.rcut
+        ia, ib, rv, r = ia[m], ib[m], rv[m], r[m]
+        R = fn.real_space_functions(r, self.xi, self.a)
+        Up, Ep = mob.pair_apply(rv, F[ib], fn.to_tensor(S5[ib]), R, self.pref)
+        U, E = np.zeros((rows.size, 3)), np.zeros((rows.size, 5))
+        np.add.at(U, ia, Up)
+        np.add.at(E, ia, fn.to_coords(Ep))
+        R0 = fn.real_space_functions(np.zeros(1), self.xi, self.a)                 # self term
+        U += self.pref * R0['F1'][0] * F[rows]
+        E += self.pref * R0['Z0'][0] / 5.0 * S5[rows]
+        return U, E
+
+    # ---- wave space -------------------------------------------------------------------------------------------
+    def _kvec(self):
+        M, L = self.M, self.L
+        k1 = 2.0 * np.pi * sfft.fftfreq(M, d=1.0 / M) / L
+        kz = 2.0 * np.pi * np.arange(M // 2 + 1) / L
+        kx, ky, kz = np.meshgrid(k1, k1, kz, indexing='ij', sparse=True)
+        live = np.ones((M, M, M // 2 + 1), bool)
+        live[0, 0, 0] = False
+        if M % 2 == 0:
+            live[M // 2, :, :] = False; live[:, M // 2, :] = False; live[:, :, M // 2] = False
+        return kx, ky, kz, live
+
+    def spread(self, x, q):
+        """Step 1: q (N, C) -> grids (C, M, M, M) = sum_beta K(x_n - x_beta) q_beta."""
+        x, q = _c(x), _c(q)
+        C = q.shape[1]
+        g = np.empty((C, self.M, self.M, self.M))
+        lib().ref_spread(x.shape[0], _dp(x), _dp(q), C, self.M, self.P, self.L, _dp(g))
+        return g * (2.0 * self.xi ** 2 / (np.pi * self.eta_g)) ** 1.5
+
+    def interpolate(self, x, grids, rows):
+        """Step 5: h^3 sum_n K(x_n - x_alpha) grid_c(x_n) at the particles `rows`."""
+        x, grids = _c(x), _c(grids)
+        C = grids.shape[0]
+        out = np.empty((rows.size, C))
+        lib().ref_interp(rows.size, _lp(rows), _dp(x), C, self.M, self.P, self.L, _dp(grids), _dp(out))
+        return out * self.h ** 3 * (2.0 * self.xi ** 2 / (np.pi * self.eta_g)) ** 1.5
+
+    def _outputs(self, uh, kx, ky, kz, c0, c1):
+        """P^H of Eq. (41): Uh = s0 uh, Eh^q = i s1 (e^q k).uh, as 8 half spectra."""
+        e = fn.basis()
+        kk = (kx, ky, kz)
+        out = [c0 * uh[i] for i in range(3)]
+        for q in range(5):
+            acc = 0.0
+            for i in range(3):
+                for j in range(3):
+                    if e[q, i, j] != 0.0:
+                        acc = acc + e[q, i, j] * kk[j] * uh[i]
+            out.append(1j * c1 * acc)
+        return out
+
+    def wave_apply(self, x, F, S5, rows=None):
+        """[U;E]_rows = M_w [F;S] by the five steps of the module docstring."""
+        x = _c(np.asarray(x, dtype=np.float64) % self.L)
+        N = x.shape[0]
+        rows = np.arange(N, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        M, V = self.M, self.L ** 3
+        nw = os.cpu_count() or 1
+        g = self.spread(x, np.hstack([_c(F), _c(S5)]))                                   # 1
+        gh = sfft.rfftn(g, axes=(1, 2, 3), workers=nw)                                   # 2
+        del g
+        kx, ky, kz, live = self._kvec()                                                  # 3
+        k2 = kx * kx + ky * ky + kz * kz
+        k2 = np.where(k2 > 0, k2, 1.0)
+        kn = np.sqrt(k2)
+        c0, c1 = fn.s0(kn * self.a), fn.s1(kn * self.a)
+        e = fn.basis()
+        kk = (kx, ky, kz)
+        fh = []
+        for i in range(3):
+            Sk = 0.0
+            for q in range(5):
+                for j in range(3):
+                    if e[q, i, j] != 0.0:
+                        Sk = Sk + e[q, i, j] * kk[j] * gh[3 + q]
+            fh.append(c0 * gh[i] - 1j * c1 * Sk)
+        del gh
+        Bt = np.where(live, (self.h ** 3 / V) * fn.hasimoto_H(kn, self.xi) * np.exp(self.eta_g * k2 / (4.0 * self.xi ** 2)) / (self.eta * k2), 0.0)
+        kf = (kx * fh[0] + ky * fh[1] + kz * fh[2]) / k2
+        uh = [Bt * (fh[i] - kk[i] * kf) for i in range(3)]
+        del fh
+        oh = np.stack(self._outputs(uh, kx, ky, kz, c0, c1))
+        del uh
+        go = sfft.irfftn(oh, s=(M, M, M), axes=(1, 2, 3), workers=nw) * float(M) ** 3   # 4 (un-normalised)
+        del oh
+        out = self.interpolate(x, go, rows)                                              # 5
+        return out[:, :3], out[:, 3:]
+
+    def apply(self, x, F, S5, rows=None, exact_real=False):
+        """[U;E]_rows = (M_r + M_w) [F;S]  (Eq. 30)."""
+        Ur, Er = self.real_apply(x, F, S5, rows, exact=exact_real)
+        Uw, Ew = self.wave_apply(x, F, S5, rows)
+        return Ur + Uw, Er + Ew
+
+    def wave_sqrt_apply(self, x, Mg, wbuf, rows=None):
+        """A_w w2 of Eq. (75) for the noise buffer of an Mg^3 grid (reading R8), evaluated on THIS object's
+        finer grid: the factor sqrt(H/(eta V k^2)) (I - kh kh) W(k) of the Mg-grid's modes is placed in the spectrum of the
+        M-grid (M >= Mg; all other modes zero), the Gaussian of the interpolation is divided out, and steps 4-5 follow."""
+        from . import brownian as brn
+        if self.M < Mg:
+            raise ValueError('wave_sqrt_apply: reference grid coarser than the noise grid')
+        x = _c(np.asarray(x, dtype=np.float64) % self.L)
+        N = x.shape[0]
+        rows = np.arange(N, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        M, V = self.M, self.L ** 3
+        wbuf = np.asarray(wbuf, dtype=np.float64).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
+        idx, n = brn.canonical_modes(Mg)
+        k = 2.0 * np.pi * n / self.L
+        W = (wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 0] + 1j * wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 1]).T / np.sqrt(2.0)
+        k2 = np.einsum('ki,ki->k', k, k)
+        kn = np.sqrt(k2)
+        kh = k / kn[:, None]
+        uh = np.sqrt(fn.hasimoto_H(kn, self.xi) / (self.eta * V * k2))[:, None] * (W - kh * np.einsum('ki,ki->k', kh, W)[:, None])
+        uh = uh * np.exp(self.eta_g * k2 / (8.0 * self.xi ** 2))[:, None]                 # undo the interpolation Gaussian
+        c0, c1 = fn.s0(kn * self.a), fn.s1(kn * self.a)
+        outs = self._outputs([uh[:, 0], uh[:, 1], uh[:, 2]], k[:, 0], k[:, 1], k[:, 2], c0, c1)
+        oh = np.zeros((8, M, M, M // 2 + 1), dtype=complex)
+        # canonical modes have n_z >= 0: they and (for n_z = 0) their conjugate partners fill the half spectrum
+        jx, jy, jz = n[:, 0] % M, n[:, 1] % M, n[:, 2]
+        for c in range(8):
+            oh[c, jx, jy, jz] = outs[c]
+            z0 = jz == 0
+            oh[c, (-n[z0, 0]) % M, (-n[z0, 1]) % M, 0] = np.conj(outs[c][z0])
+        go = sfft.irfftn(oh, s=(M, M, M), axes=(1, 2, 3), workers=os.cpu_count() or 1) * float(M) ** 3
+        out = self.interpolate(x, go, rows)
+        return out[:, :3], out[:, 3:]
+
+
+# ---- Brownian sample and mid-point step on the fast operators (the tier for N = 4 096 and up) -----
+
+def brownian(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, tol=1e-8, krylov_tol=1e-10, rows=None, params=None):
+    """Eq. (76): sqrt(2kT/dt) ( M_r^{1/2} w1 + A_w w2 ).  M_r^{1/2} w1 by fp64 Lanczos on the
+    cut-off pair sum (r_cut from `tol`: the truncated tail is below tol); A_w w2 over exactly the modes of the Mg^3 noise
+    grid (Eq. 75).  Returns (U^B, E^B, Lanczos iterations); rows restricts the OUTPUT rows.  params = dict(M, P, rcut)
+    replaces the parameters derived from tol (bench.py's timing leg runs with the GPU run's grid and cutoff)."""
+    from . import krylov
+    x = np.asarray(x, dtype=np.float64)
+    N = x.shape[0]
+    ref = PSEReference(L, a, eta, xi, tol, **(params or {}))
+
+    def mr(v):
+        v = v.reshape(N, 8)
+        U, E = ref.real_apply(x, v[:, :3], v[:, 3:])
+        return np.hstack([U, E]).ravel()
+
+    y, its = krylov.lanczos_sqrt(mr, np.asarray(w1, dtype=np.float64).ravel(), krylov_tol)
+    y = y.reshape(N, 8)
+    if ref.M < Mg:
+        ref = PSEReference(L, a, eta, xi, tol, **dict(params or {}, M=Mg + (Mg & 1)))
+    Uw, Ew = ref.wave_sqrt_apply(x, Mg, wbuf)
+    amp = np.sqrt(2.0 * kT / dt)
+    U, E = amp * (y[:, :3] + Uw), amp * (y[:, 3:] + Ew)
+    return (U, E, its) if rows is None else (U[rows], E[rows], its)
+
+
+def constrained_solve(x, L, a, eta, xi, UB, EB, FP, tol=1e-8, krylov_tol=1e-10, params=None):
+    """Eqs. (36)-(38), (78): M_ES S = -(E^B + M_EF F^P) by fp64 GMRES on the reference product,
+    then U = U^B + M_UF F^P + M_US S.  Returns (U, S, GMRES iterations)."""
+    from . import krylov
+    x = np.asarray(x, dtype=np.float64)
+    N = x.shape[0]
+    ref = PSEReference(L, a, eta, xi, tol, **(params or {}))
+    zF, zS = np.zeros((N, 3)), np.zeros((N, 5))
+    _, Ef = ref.apply(x, FP, zS)
+    S, its = krylov.gmres(lambda s: ref.apply(x, zF, s.reshape(N, 5))[1].ravel(), -(np.asarray(EB, float) + Ef).ravel(), krylov_tol)
+    S = S.reshape(N, 5)
+    Uf, _ = ref.apply(x, FP, S)
+    return np.asarray(UB, float) + Uf, S, its
+
+
+def step(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, tol=1e-8, krylov_tol=1e-10, bonds=None, params=None):
+    """One mid-point step, Eqs. (76)-(79), on the fast fp64 operators; the counterpart of
+    oracle.brownian.step for sizes its dense matrices cannot reach.  Returns x_{k+1} (not wrapped), U_{k+1/2}, S, (Lanczos, GMRES)."""
+    from . import brownian as brn
+    x = np.asarray(x, dtype=np.float64)
+    UB, EB, li = brownian(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, tol, krylov_tol, params=params)   # (76)
+    xh = x + 0.5 * dt * UB                                                                   # (77)
+    xh -= L * np.floor(xh / L)
+    FP = heyes_melrose(xh, L, a, eta, dt)
+    if bonds is not None:
+        FP = FP + brn.bond_forces(xh, L, *bonds)
+    U, S, gi = constrained_solve(xh, L, a, eta, xi, UB, EB, FP, tol, krylov_tol, params)     # (78)
+    return x + dt * U, U, S, (li, gi)                                                        # (79)
+
+
+def heyes_melrose(x, L, a, eta, dt):
+    """oracle.brownian.heyes_melrose (reading R12) with the overlapping pairs from a periodic k-d tree instead of the dense
+    N x N distance matrix, for sizes that one cannot hold."""
+    x = np.asarray(x, dtype=np.float64) % L
+    pairs = cKDTree(x, boxsize=L).query_pairs(2.0 * a, output_type='ndarray')
+    F = np.zeros_like(x)
+    if len(pairs):
+        d = x[pairs[:, 0]] - x[pairs[:, 1]]
+        d -= L * np.round(d / L)
+        r = np.linalg.norm(d, axis=1)
+        f = (3.0 * np.pi * eta * a * (2.0 * a - r) / dt / r)[:, None] * d
+        np.add.at(F, pairs[:, 0], f)
+        np.add.at(F, pairs[:, 1], -f)
+    return F

@@ -253,3 +253,76 @@ def test_P16_divergence_of_M_UF_vanishes_and_constrained_drift_is_antisymmetric(
     Mc = brn.constrained_mobility(M, 2)
     U, _ = brn.constrained_solve(M, 2, np.zeros((2, 3)), np.zeros((2, 5)), np.eye(6)[2].reshape(2, 3))
     assert np.abs(Mc[:, 2] - U.ravel()).max() < 1e-14
+
+
+@pytest.mark.parametrize('xi', [0.3, 0.45, 0.8])
+def test_P6_printed_closed_forms_of_the_dipole_couplings(xi):
+    """The other printed forms of Appendix A that survive the extraction (SURVEY.md 8(c) errata): K3 in both cases
+     pins (Z2 + Z4)/7, G1 for r > 2a pins G1 (printed = -2 R_G1 at a = 1), and the self term
+    (A12) pins Z0(0)/5 = -3 x its bracket."""
+    r = np.array([0.6, 1.7, 1.999, 2.001, 2.6, 4.5])
+    R = fn.real_space_functions(r, xi, A)
+    _, _, C, _ = fn.rank4_combinations(R)
+    for i, ri in enumerate(r):
+        assert abs(C[i] - app.K3(ri, A, xi)) < 1e-10
+        if ri > 2 * A:
+            assert abs(-2 * R['G1'][i] - app.G1_case1(ri, A, xi)) < 1e-10
+    R0 = fn.real_space_functions(np.zeros(1), xi, A)
+    assert abs(R0['Z0'][0] / 5 + 3 * app.self_DC_bracket(A, xi)) < 1e-12
+
+
+def test_heyes_melrose_moves_a_free_draining_pair_exactly_to_contact():
+    """What the force is FOR (reading R12): a free-draining pair (mobility 1/(6 pi eta a) each) at separation r < 2a
+    moved for one dt by its Heyes-Melrose forces ends at r = 2a exactly; separated pairs feel nothing; pairs through the
+    periodic boundary are found; forces sum to zero."""
+    L, dt = 11.0, 3e-3
+    for a, eta in [(1.0, ETA), (0.7, 0.31)]:
+        for r in (1.2 * a, 1.7 * a, 1.999 * a):
+            d = np.array([0.3, -0.5, 0.81]); d *= r / np.linalg.norm(d)
+            x = np.array([[10.8, 0.2, 5.0], [10.8, 0.2, 5.0] + d]) % L            # pair straddles the boundary
+            F = brn.heyes_melrose(x, L, a, eta, dt)
+            xn = x + dt * F / (6 * np.pi * eta * a)
+            dn = xn[0] - xn[1]
+            dn -= L * np.round(dn / L)
+            assert abs(np.linalg.norm(dn) - 2 * a) < 1e-13 and np.abs(F.sum(axis=0)).max() < 1e-12
+    x = np.array([[1.0, 1.0, 1.0], [3.001, 1.0, 1.0], [1.0, 2.5, 1.0]])            # 0-1 apart, 0-2 overlapping
+    F = brn.heyes_melrose(x, L, 1.0, ETA, dt)
+    assert np.all(F[1] == 0) and F[0, 1] < 0 < F[2, 1] and F[0, 0] == 0
+
+
+def test_brownian_amplitude_and_composition_against_its_dense_factors():
+    """oracle.brownian.brownian = sqrt(2kT/dt) (sqrtm(M_r) w1 + A_w w2) with exactly that amplitude (Eq. B4) and
+    the per-particle (U, e1..e5) ordering of w1."""
+    x, L, xi, Mg, kT, dt = X4[:3], 7.0, 0.6, 6, 1.7, 0.02
+    g = np.random.default_rng(3)
+    w1, w2 = g.standard_normal(24), g.standard_normal((3, Mg, Mg, Mg // 2 + 1, 2))
+    U, E = brn.brownian(x, L, A, ETA, kT, xi, dt, Mg, w1, w2)
+    want = np.sqrt(2 * kT / dt) * (brn.sqrtm_psd(mob.dense_real(x, L, A, ETA, xi)) @ w1 + brn.wave_sqrt_dense(x, L, A, ETA, xi, Mg) @ w2.ravel())
+    assert np.abs(np.hstack([U, E]).ravel() - want).max() < 1e-11
+    U4, _ = brn.brownian(x, L, A, ETA, 4 * kT, xi, dt / 4, Mg, w1, w2)
+    assert np.allclose(U4, 4 * U, rtol=1e-13)
+
+
+def test_midpoint_step_structure_written_out_by_hand():
+    """Eqs. (76)-(79) for two spheres with a fixed noise vector, every line written out from the dense
+    matrices: the half step uses dt/2 (Eq. 77), the matrix of the solve is the one at x_{k+1/2} (Eq. 78), the full step
+    starts again from x_k (Eq. 79), and E = 0 holds for the returned S."""
+    L, xi, Mg, kT, dt = 9.0, 0.6, 6, 1.0, 0.05
+    x = np.array([[3.0, 3.0, 3.0], [5.3, 3.4, 2.8]])
+    g = np.random.default_rng(11)
+    w1, w2 = g.standard_normal(16), g.standard_normal((3, Mg, Mg, Mg // 2 + 1, 2))
+    xn, U, S = brn.step(x, L, A, ETA, kT, xi, dt, Mg, w1, w2)
+    ub = (np.sqrt(2 * kT / dt) * (brn.sqrtm_psd(mob.dense_real(x, L, A, ETA, xi)) @ w1
+                                  + brn.wave_sqrt_dense(x, L, A, ETA, xi, Mg) @ w2.ravel())).reshape(2, 8)
+    xh = x + 0.5 * dt * ub[:, :3]                                         # (77)
+    Mh = mob.dense(xh, L, A, ETA, xi)                                     # matrix at the mid-point
+    iu, ie = np.array([0, 1, 2, 8, 9, 10]), np.array([3, 4, 5, 6, 7, 11, 12, 13, 14, 15])
+    Sh = np.linalg.solve(Mh[np.ix_(ie, ie)], -ub[:, 3:].ravel())          # (78) with F^P = 0 (no overlap, no bonds)
+    Uh = ub[:, :3].ravel() + Mh[np.ix_(iu, ie)] @ Sh
+    assert np.abs(brn.heyes_melrose(xh, L, A, ETA, dt)).max() == 0
+    assert np.abs(U.ravel() - Uh).max() < 1e-12 and np.abs(S.ravel() - Sh).max() < 1e-11
+    assert np.abs(xn - (x + dt * Uh.reshape(2, 3))).max() < 1e-13       # (79)
+    # a full-dt half step, or the matrix at x_k, is a different (wrong) scheme and is told apart
+    Mk = mob.dense(x, L, A, ETA, xi)
+    Uk = ub[:, :3].ravel() + Mk[np.ix_(iu, ie)] @ np.linalg.solve(Mk[np.ix_(ie, ie)], -ub[:, 3:].ravel())
+    assert np.abs(Uk - Uh).max() > 1e-4
