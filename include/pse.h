@@ -5,8 +5,9 @@
  * Conventions
  *   - Pointers prefixed d_ are DEVICE pointers owned by the caller (e.g. torch tensors); h_ are HOST pointers.
  *     The library never frees or reallocates caller buffers.  All internal buffers belong to the context.
- *   - All work is enqueued on the CUDA stream given at pse_create (NULL = legacy default stream).  Calls that
- *     return iteration counts or need host-side convergence decisions synchronise that stream.
+ *   - All work is enqueued on the CUDA stream given at pse_create (NULL = legacy default stream), on the device that was
+ *     current at pse_create.  Calls that return iteration counts or need host-side convergence decisions synchronise that
+ *     stream.  Callers that produce inputs on another stream must order that stream before the call themselves.
  *   - fp32 on the device.  Per-particle vectors: positions [N][4] (x,y,z,unused); forces/velocities [N][3];
  *     stresslets / rates of strain [N][5] as coordinates in the orthonormal basis of symmetric traceless tensors
  *       e1=(xx-yy)/sqrt2, e2=(2zz-xx-yy)/sqrt6, e3=(xy+yx)/sqrt2, e4=(xz+zx)/sqrt2, e5=(yz+zy)/sqrt2
@@ -31,6 +32,15 @@ typedef enum {
 /* which half of the Ewald sum pse_mobility_apply evaluates (Eq. 30) */
 enum { PSE_REAL = 1, PSE_WAVE = 2, PSE_BOTH = 3 };
 
+/* Window of the spreading / interpolation operators Q, Q^T of Eq. (42) on its P^3-point support:
+ *   PSE_WINDOW_GAUSS  the paper's truncated Gaussian, exp(-2 xi^2 r^2/eta_g) with eta_g = (h P xi/m)^2, m = sqrt(pi P)
+ *                     (PAPER.md:263, 306, 334); needs eta_g < 1;
+ *   PSE_WINDOW_ES     "exponential of semicircle" exp(beta (sqrt(1 - (2t/P)^2) - 1)), beta = 2.2 P, t = offset in grid
+ *                     spacings: same support, reaches a given tolerance with fewer points (R3, R6).  Default.
+ * The window is divided out exactly in wave space (R4), so the operator is the same; only the quadrature
+ * error for a given P differs.  P from pse_suggest_params* fits the window it was asked for. */
+enum { PSE_WINDOW_GAUSS = 0, PSE_WINDOW_ES = 1 };
+
 /* phases reported by pse_get_timings */
 enum { PSE_T_NEIGHBORS = 0, PSE_T_REAL = 1, PSE_T_SPREAD = 2, PSE_T_FFT_FWD = 3, PSE_T_SCALE = 4, PSE_T_FFT_INV = 5,
        PSE_T_INTERP = 6, PSE_T_VECTOR = 7, PSE_T_PACK = 8, PSE_T_COUNT = 9 };
@@ -38,23 +48,30 @@ enum { PSE_T_NEIGHBORS = 0, PSE_T_REAL = 1, PSE_T_SPREAD = 2, PSE_T_FFT_FWD = 3,
 /* Parameter derivation from a tolerance (reading R6; paper: eps_r ~ exp(-xi^2 rcut^2) PAPER.md:207,
  * quadrature bound Eq. (55) with m = sqrt(pi P) PAPER.md:308, 334).  Host only, no GPU needed.
  *   in : N, L, a, tol, xi
- *   out: *grid (FFT points per dimension, 2^a 3^b 5^c 7^d), *P (Gaussian support, points per dimension),
- *        *rcut (real-space cutoff).  Returns PSE_EINVAL if no valid choice exists (rcut > L/2). */
+ *   out: *grid (FFT points per dimension, 2^a 3^b 5^c 7^d), *P (window support, points per dimension: 3/4/5 at
+ *        tol = 1e-2/1e-3/1e-4 for PSE_WINDOW_ES, 5/6/8 for PSE_WINDOW_GAUSS), *rcut (real-space cutoff).
+ *   Returns PSE_EINVAL if no valid choice exists (rcut > L/2).  pse_suggest_params = the default window. */
 pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, int *grid, int *P, double *rcut);
+pse_status pse_suggest_params_window(int N, double L, double a, double tol, double xi, int window, int *grid, int *P, double *rcut);
 
 /* Create a context for N equal spheres of radius a in a cubic periodic box of edge L, viscosity eta, thermal
- * energy kT, splitting parameter xi (Eq. 28), FFT grid `grid`^3, Gaussian support P^3 grid points
+ * energy kT, splitting parameter xi (Eq. 28), FFT grid `grid`^3, window support P^3 grid points
  * (PAPER.md:227), real-space cutoff rcut, Krylov tolerance tol.  Builds the
- * real-space tables (Eqs. 25-27 PAPER.md:127-143 via DESIGN.md §3), cuFFT plans and workspaces.
- * PSE_EINVAL: non-positive sizes, rcut > L/2, rcut < 2a, P > grid, P > 16, Gaussian parameter eta_g >= 1. */
+ * real-space tables (Eqs. 25-27 PAPER.md:127-143 via DESIGN.md §3), cuFFT plans and workspaces on the current device.
+ * pse_create uses PSE_WINDOW_ES; pse_create_window takes the window explicitly (no environment variable is read anywhere).
+ * PSE_EINVAL: non-positive sizes, rcut > L/2, rcut < 2a, P > grid, P > 16, unknown window, and for PSE_WINDOW_GAUSS a
+ * shape parameter eta_g >= 1.  *out is set even on failure so that pse_last_error works; destroy it. */
 pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
                       int grid, int P, double rcut, double tol, void *cuda_stream);
+pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
+                             int grid, int P, double rcut, double tol, int window, void *cuda_stream);
 pse_status pse_destroy(pse_ctx *ctx);
 
 /* Bin the particles (positions may be unwrapped; they are wrapped into [0,L)) into linked cells of edge >= rcut
  * and build the full neighbour list {beta != alpha : |x_alpha - x_beta|_min-image^2 < rcut^2}, plus
  * the FFT-grid tile bins used by spread/interpolate.  Must be re-called whenever positions change.
- * d_pos: [N][4] float, device.  Asynchronous except for one size read-back. */
+ * d_pos: [N][4] float, device.  Synchronises once (the list size comes back to the host; inside pse_step the builds are
+ * only enqueued and that read-back is examined after the Krylov solve that follows). */
 pse_status pse_neighbors(pse_ctx *ctx, const float *d_pos);
 
 /* [U;E] = M [F;S]  (Eqs. 30-31): real-space pair sum over the neighbour list with tabulated

@@ -6,4 +6,4 @@ include/pse.h; this package is its thin ctypes binding.  Importing it requires t
 """
 from .binding import (Context, PSEError, pse_create, pse_suggest_params, pse_version, EXPORTS, LIB_PATH, PHASES,  # noqa: F401
                       PSE_OK, PSE_EINVAL, PSE_ENOMEM, PSE_ECUDA, PSE_ECUFFT, PSE_ENOTREADY, PSE_ENOCONV, PSE_EOVERFLOW,
-                      PSE_REAL, PSE_WAVE, PSE_BOTH)
+                      PSE_REAL, PSE_WAVE, PSE_BOTH, PSE_WINDOW_GAUSS, PSE_WINDOW_ES)

@@ -13,11 +13,12 @@ LIB_PATH = os.path.join(_HERE, 'libpse.so')
 
 PSE_OK, PSE_EINVAL, PSE_ENOMEM, PSE_ECUDA, PSE_ECUFFT, PSE_ENOTREADY, PSE_ENOCONV, PSE_EOVERFLOW = range(8)
 PSE_REAL, PSE_WAVE, PSE_BOTH = 1, 2, 3
+PSE_WINDOW_GAUSS, PSE_WINDOW_ES = 0, 1
 PHASES = ('neighbors', 'real', 'spread', 'fft_fwd', 'scale', 'fft_inv', 'interp', 'vector', 'pack')
 _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PSE_ECUFFT', 5: 'PSE_ENOTREADY',
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
-EXPORTS = ('pse_suggest_params', 'pse_create', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
+EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
            'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
@@ -36,6 +37,8 @@ def load_library():
     vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
     lib.pse_suggest_params.argtypes = [i32, dbl, dbl, dbl, dbl, C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
     lib.pse_create.argtypes = [C.POINTER(vp), i32, dbl, dbl, dbl, dbl, dbl, i32, i32, dbl, dbl, vp]
+    lib.pse_suggest_params_window.argtypes = [i32, dbl, dbl, dbl, dbl, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
+    lib.pse_create_window.argtypes = [C.POINTER(vp), i32, dbl, dbl, dbl, dbl, dbl, i32, i32, dbl, dbl, i32, vp]
     lib.pse_destroy.argtypes = [vp]
     lib.pse_neighbors.argtypes = [vp, vp]
     lib.pse_mobility_apply.argtypes = [vp, vp, vp, vp, vp, i32]
@@ -62,11 +65,13 @@ def load_library():
 _lib = load_library()
 
 
-def _ptr(t, shape=None):
+def _ptr(t, shape=None, dtype=torch.float32):
     if t is None:
         return None
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
         raise TypeError('expected a contiguous CUDA tensor')
+    if t.dtype != dtype:
+        raise TypeError(f'expected dtype {dtype}, got {t.dtype}')
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise ValueError(f'expected shape {tuple(shape)}, got {tuple(t.shape)}')
     return C.c_void_p(t.data_ptr())
@@ -84,21 +89,23 @@ def pse_version():
     return _lib.pse_version().decode()
 
 
-def pse_suggest_params(N, L, a, tol, xi):
-    """-> (status, grid, P, rcut); see include/pse.h."""
+def pse_suggest_params(N, L, a, tol, xi, window=PSE_WINDOW_ES):
+    """-> (status, grid, P, rcut); see include/pse.h (pse_suggest_params_window)."""
     g, p, rc = C.c_int(), C.c_int(), C.c_double()
-    st = _lib.pse_suggest_params(N, L, a, tol, xi, C.byref(g), C.byref(p), C.byref(rc))
+    st = _lib.pse_suggest_params_window(N, L, a, tol, xi, window, C.byref(g), C.byref(p), C.byref(rc))
     return st, g.value, p.value, rc.value
 
 
 class Context:
     """Owns a pse_ctx*.  Methods are one-to-one with the C calls of the same name."""
 
-    def __init__(self, N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None):
+    def __init__(self, N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None, window=PSE_WINDOW_ES):
         self.N, self.L, self.grid, self.P = int(N), float(L), int(grid), int(P)
         self._h = C.c_void_p()
+        # the library enqueues on this stream (NULL = legacy default stream, which torch's default stream is ordered with);
+        # inputs produced on another torch stream must be ordered before the calls by the caller
         sp = C.c_void_p(stream.cuda_stream) if stream is not None else None
-        st = _lib.pse_create(C.byref(self._h), N, L, a, eta, kT, xi, grid, P, rcut, tol, sp)
+        st = _lib.pse_create_window(C.byref(self._h), N, L, a, eta, kT, xi, grid, P, rcut, tol, window, sp)
         if st != PSE_OK:
             msg = _lib.pse_last_error(self._h).decode() if self._h else 'allocation failed'
             if self._h:
@@ -175,9 +182,9 @@ class Context:
         """-> (count [N] int32 tensor, index [total] int32 tensor) in original particle numbering."""
         total = C.c_size_t()
         count = torch.empty(self.N, dtype=torch.int32, device='cuda')
-        self._check(_lib.pse_get_neighbors(self._h, _ptr(count), None, 0, C.byref(total)))
+        self._check(_lib.pse_get_neighbors(self._h, _ptr(count, dtype=torch.int32), None, 0, C.byref(total)))
         index = torch.empty(max(total.value, 1), dtype=torch.int32, device='cuda')
-        self._check(_lib.pse_get_neighbors(self._h, _ptr(count), _ptr(index), index.numel(), C.byref(total)))
+        self._check(_lib.pse_get_neighbors(self._h, _ptr(count, dtype=torch.int32), _ptr(index, dtype=torch.int32), index.numel(), C.byref(total)))
         return count, index[:total.value]
 
     def pse_set_profiling(self, on):
@@ -201,5 +208,5 @@ class Context:
         return tab, dr.value
 
 
-def pse_create(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None):
-    return Context(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream)
+def pse_create(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream=None, window=PSE_WINDOW_ES):
+    return Context(N, L, a, eta, kT, xi, grid, P, rcut, tol, stream, window)

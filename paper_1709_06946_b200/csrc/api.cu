@@ -1,7 +1,6 @@
 // C-ABI entry points of libpse (include/pse.h).
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <new>
 #include "pse_internal.h"
 
@@ -54,6 +53,11 @@ const char *pse_last_error(const pse_ctx *c) { return c ? c->err.c_str() : "null
 long long pse_kernel_launches(const pse_ctx *c) { return c ? c->launches : 0; }
 
 pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, int *grid, int *P, double *rcut) {
+    return pse_suggest_params_window(N, L, a, tol, xi, PSE_WINDOW_ES, grid, P, rcut);
+}
+
+pse_status pse_suggest_params_window(int N, double L, double a, double tol, double xi, int window, int *grid, int *P, double *rcut) {
+    if (window != PSE_WINDOW_GAUSS && window != PSE_WINDOW_ES) return PSE_EINVAL;
     if (N <= 0 || !(L > 0) || !(a > 0) || !(tol > 0 && tol < 1) || !(xi > 0)) return PSE_EINVAL;
     const double s = std::sqrt(-std::log(tol));
     // C1: functions decay like exp(-xi^2 (r-2a)^2), so the paper's estimate r = s/xi
@@ -66,12 +70,12 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
     if (M > 64) M = choose_grid(M); else while (!smooth7(M)) ++M;
     // C3: support size.  Default window = exponential of semicircle with beta = 2.2 P: measured against
     // the oracle it reaches the tolerance with P = 3, 4, 5 points at tol = 1e-2, 1e-3, 1e-4, i.e. P = ceil(-log10 tol) + 1.
-    // PSE_WINDOW=gauss selects the paper's Gaussian: its quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1,
+    // PSE_WINDOW_GAUSS selects the paper's Gaussian: its quadrature bound with m = sqrt(pi P) (Eq. 55 with lambda_max = 1,
     // PAPER.md:308, 334), e^{-pi P/2} + erfc(sqrt(pi P/2)), gives P = 5 at 1e-3 as in Table I, but the
     // measured relative L2 error of the strain-rate rows is 10-20x that bound, so it is required to be <= tol/10:
     // P = 5, 6, 8 (R6).
     int p = 2;
-    if (pse_window_kind_from_env() == 0) {
+    if (window == PSE_WINDOW_GAUSS) {
         while (p < PSE_MAXP && 10.0 * (std::exp(-M_PI * p / 2.0) + std::erfc(std::sqrt(M_PI * p / 2.0))) > tol) ++p;
     } else {
         p = std::min(PSE_MAXP, std::max(3, (int)std::ceil(-std::log10(tol) - 1e-9) + 1));
@@ -85,6 +89,11 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
 
 pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
                       int grid, int P, double rcut, double tol, void *cuda_stream) {
+    return pse_create_window(out, N, L, a, eta, kT, xi, grid, P, rcut, tol, PSE_WINDOW_ES, cuda_stream);
+}
+
+pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
+                             int grid, int P, double rcut, double tol, int window, void *cuda_stream) {
     if (!out) return PSE_EINVAL;
     *out = nullptr;
     pse_ctx *c = new (std::nothrow) pse_ctx;
@@ -97,18 +106,25 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     if (rcut > 0.5 * L) { c->err = "pse_create: rcut > L/2 (minimum-image real-space sum)"; return PSE_EINVAL; }
     if (rcut < 2.0 * a) { c->err = "pse_create: rcut < 2a (overlap forces need contact pairs)"; return PSE_EINVAL; }
     if (P > grid || P > PSE_MAXP) { c->err = "pse_create: P > grid or P > 16"; return PSE_EINVAL; }
+    if (window != PSE_WINDOW_GAUSS && window != PSE_WINDOW_ES) { c->err = "pse_create: unknown window"; return PSE_EINVAL; }
     c->N = N; c->L = L; c->a = a; c->eta = eta; c->kT = kT; c->xi = xi; c->M = grid; c->P = P; c->rcut = rcut; c->tol = tol;
     c->h = L / grid;
-    c->win_kind = pse_window_kind_from_env();
+    c->win_kind = window;
     if (c->win_kind == 0) {
         c->eta_g = (c->h * P * xi) * (c->h * P * xi) / (M_PI * P);     // (h P xi/m)^2, m^2 = pi P
         if (!(c->eta_g < 1.0)) { c->err = "pse_create: Gaussian shape parameter eta_g >= 1 (grid too coarse for this xi and P)"; return PSE_EINVAL; }
         c->win_a = 2.0 * M_PI / P; c->win_b = 0.0;
     } else {
-        c->win_a = 4.0 / ((double)P * P); c->win_b = pse_es_beta_from_env(P);
+        c->win_a = 4.0 / ((double)P * P); c->win_b = pse_es_beta(P);
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { c->err = "no CUDA device (libpse has no CPU fallback)"; return PSE_ECUDA; }
+    // the context lives on the device that is current now; its kernel attributes (dynamic shared memory opt-in, cooperative
+    // grid cap) are set for THIS device on every create, so several contexts on several GPUs of one process are fine
+    CUDA_TRY(c, cudaGetDevice(&c->device));
+    CUDA_TRY(c, cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, c->device));
+    PSE_TRY(pse_real_init(c));
+    PSE_TRY(pse_krylov_init(c));
     // real-space table
     std::vector<float> tab;
     pse_build_table(a, eta, xi, rcut, PSE_NTAB, tab, &c->tab_dr);
@@ -149,10 +165,9 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
     }
     CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-    CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_real, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise_r, cudaEventDisableTiming));
-    if (const char *e = getenv("PSE_OVERLAP")) c->overlap = (e[0] != '0');
+    CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_nbr, cudaEventDisableTiming));
     return PSE_OK;
 }
 
@@ -161,9 +176,9 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaStreamSynchronize(c->stream);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
-    if (c->ev_real) cudaEventDestroy(c->ev_real);
     if (c->ev_noise) cudaEventDestroy(c->ev_noise);
     if (c->ev_noise_r) cudaEventDestroy(c->ev_noise_r);
+    if (c->ev_nbr) cudaEventDestroy(c->ev_nbr);
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
@@ -180,7 +195,7 @@ pse_status pse_destroy(pse_ctx *c) {
 
 pse_status pse_neighbors(pse_ctx *c, const float *d_pos) {
     if (!c || !d_pos) return PSE_EINVAL;
-    return pse_neighbors_impl(c, d_pos);
+    return pse_neighbors_sync(c, d_pos);
 }
 
 pse_status pse_get_neighbors(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total) {
@@ -256,23 +271,39 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     float *UB = c->d_vecD, *EB = c->d_vecD + (size_t)3 * N;           // original numbering: [N][3] then [N][5]
     float4 *xh = reinterpret_cast<float4 *>(c->d_zu);                  // scratch for x_{k+1/2}; d_zu is rewritten by GMRES afterwards
     pse_status soft = PSE_OK;
+    // The neighbour builds are only enqueued; what they report (list size, overflow, oversized cell) is examined after the
+    // Krylov solve that follows has synchronised the stream anyway.  In the rare case that a build must be repeated (first
+    // step of a context, or a list that grew by more than 25 % since the last step) the phase that consumed it is redone.
+    pse_status st = PSE_OK;
+    bool redo = true;
     // (76) Brownian slip at x_k
-    PSE_TRY(pse_neighbors_impl(c, d_pos));
-    pse_status st = pse_brownian(c, dt, d_noise_real, d_noise_wave, UB, EB, lanczos_iters);
-    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
-    // (77) mid-point
-    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
-    PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
-    // (78) constrained solve at the mid-point with hard-sphere forces (reading R12)
-    PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
-    if (c->n_bonds) {                                                  // F^P += bond forces (d_vecC, d_out: free until the solve)
-        PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
-        PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
-        PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+    for (int attempt = 0; redo && attempt < 4; ++attempt) {
+        PSE_TRY(pse_neighbors_impl(c, d_pos));
+        st = pse_brownian(c, dt, d_noise_real, d_noise_wave, UB, EB, lanczos_iters);
+        if (st != PSE_OK && st != PSE_ENOCONV) return st;
+        PSE_TRY(pse_neighbors_settle(c, &redo));
     }
-    PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
-    st = pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
-    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
+    if (redo) { c->err = "neighbour build did not settle"; return PSE_EOVERFLOW; }
+    if (st == PSE_ENOCONV) soft = st;
+    redo = true;
+    for (int attempt = 0; redo && attempt < 4; ++attempt) {
+        // (77) mid-point
+        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+        PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
+        // (78) constrained solve at the mid-point with hard-sphere forces (reading R12)
+        PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+        if (c->n_bonds) {                                              // F^P += bond forces (d_vecC, d_out: free until the solve)
+            PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
+            PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
+            PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+        }
+        PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
+        st = pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
+        if (st != PSE_OK && st != PSE_ENOCONV) return st;
+        PSE_TRY(pse_neighbors_settle(c, &redo));
+    }
+    if (redo) { c->err = "neighbour build did not settle"; return PSE_EOVERFLOW; }
+    if (st == PSE_ENOCONV) soft = st;
     PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));     // U_{k+1/2}, original numbering [N][3]
     // (79) full step from x_k
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
@@ -297,7 +328,7 @@ pse_status pse_mobility_apply_host(pse_ctx *c, const float *h_pos, const float *
     CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_pos, h_pos, N * 4 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(dF, h_F, N * 3 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(dS, h_S, N * 5 * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    PSE_TRY(pse_neighbors_impl(c, c->d_stage_pos));
+    PSE_TRY(pse_neighbors_sync(c, c->d_stage_pos));
     PSE_TRY(pse_mobility_apply(c, dF, dS, dU, dE, PSE_BOTH));
     CUDA_TRY(c, cudaMemcpyAsync(h_U, dU, N * 3 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(h_E, dE, N * 5 * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
@@ -360,21 +391,11 @@ pse_status pse_get_table(pse_ctx *c, float *h_table, int cap_nodes, int *n_nodes
 }  // extern "C"
 
 pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode) {
-    if (which == PSE_BOTH && c->overlap && !c->profiling && c->stream2) {
-        // the two halves of the Ewald sum are independent: the pair kernel (one CTA per SM, so that it leaves half of
-        // every SM's registers free) runs on a second stream while spread / FFT / scale / FFT run on the main one;
-        // the interpolation, which accumulates into the same output, waits for it.
-        CUDA_TRY(c, cudaEventRecord(c->ev_fork, c->stream));
-        CUDA_TRY(c, cudaStreamWaitEvent(c->stream2, c->ev_fork, 0));
-        PSE_TRY(pse_real_apply(c, d_in, d_out, c->stream2, 1, mode));
-        CUDA_TRY(c, cudaEventRecord(c->ev_real, c->stream2));
-        return pse_wave_apply(c, d_in, d_out, true, c->ev_real, mode);
-    }
-    if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out, nullptr, 2, mode));
+    if (which & PSE_REAL) PSE_TRY(pse_real_apply(c, d_in, d_out, mode));
     if (which & PSE_WAVE) {
         // wave-only products start from zero: the interpolation of a masked product writes only the requested planes
         if (!(which & PSE_REAL) && mode != PSE_MODE_ALL) CUDA_TRY(c, cudaMemsetAsync(d_out, 0, (size_t)c->N * 8 * sizeof(float), c->stream));
-        PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0, nullptr, mode));
+        PSE_TRY(pse_wave_apply(c, d_in, d_out, (which & PSE_REAL) != 0, mode));
     }
     return PSE_OK;
 }

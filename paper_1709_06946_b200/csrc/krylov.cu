@@ -217,18 +217,10 @@ __global__ void __launch_bounds__(VT) k_arnoldi_step(float4 *w, const float4 *Z,
     }
 }
 
-// grid of a cooperative launch: every CTA must be resident
-template <typename K>
-int coop_grid(K kernel, size_t work_items) {
-    static int cap = 0;
-    if (!cap) {
-        int dev = 0, nsm = 0, per_sm = 0;
-        cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, VT, 0);
-        cap = nsm * std::max(1, per_sm);
-    }
+// grid of a cooperative launch: every CTA must be resident (cap computed per device in pse_krylov_init)
+int coop_grid(const pse_ctx *c, size_t work_items) {
     const size_t b = (work_items + 2 * VT - 1) / (2 * VT);          // at least two items per thread: fewer CTAs at the barriers
-    return (int)std::max<size_t>(1, std::min<size_t>(b, (size_t)cap));
+    return (int)std::max<size_t>(1, std::min<size_t>(b, (size_t)c->coop_cap));
 }
 
 // cyclic Jacobi eigen-decomposition of a small symmetric matrix (n <= 51), fp64, host
@@ -277,6 +269,16 @@ pse_status upload_coefs(pse_ctx *c, const std::vector<float> &v) {
 }
 
 }  // namespace
+
+pse_status pse_krylov_init(pse_ctx *c) {
+    int a = 0, b = 0, coop = 0;
+    CUDA_TRY(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
+    if (!coop) { c->err = "device does not support cooperative launches (Krylov step kernels)"; return PSE_ECUDA; }
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_lanczos_step, VT, 0));
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_arnoldi_step, VT, 0));
+    c->coop_cap = c->nsm * std::max(1, std::min(a, b));
+    return PSE_OK;
+}
 
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed) {
     ScopedPhase ph(c, PSE_T_PACK);
@@ -334,7 +336,7 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
           const double *a_b2prev = j ? c->d_scal + 2 * j : nullptr;
           size_t a_n4 = n4;
           void *args[] = {&a_u, &a_vj, &a_vjm1, &a_next, &a_alpha, &a_b2prev, &a_b2, &a_n4};
-          CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_lanczos_step, dim3(coop_grid(k_lanczos_step, n4)), dim3(VT), args, 0, c->stream));
+          CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_lanczos_step, dim3(coop_grid(c, n4)), dim3(VT), args, 0, c->stream));
           KERNEL_CHECK(c); }
         if (j < first_check && j + 1 < maxit) continue;
         PSE_TRY(read_scalars(c, 3 + 2 * j));
@@ -414,7 +416,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
               size_t a_stride = n4; int a_nvec = k + 1, a_N = N;
               double *a_h = c->d_scal + base;
               void *args[] = {&a_w, &a_Z, &a_V, &a_stride, &a_nvec, &a_h, &a_next, &a_N};
-              CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_arnoldi_step, dim3(coop_grid(k_arnoldi_step, (size_t)N)), dim3(VT), args, 0, c->stream));
+              CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_arnoldi_step, dim3(coop_grid(c, (size_t)N)), dim3(VT), args, 0, c->stream));
               KERNEL_CHECK(c); }
             if (k < first_check && k + 1 < maxit) continue;
             PSE_TRY(read_scalars(c, base + k + 2));

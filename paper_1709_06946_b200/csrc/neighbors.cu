@@ -1,10 +1,14 @@
 // Cell list + full neighbour list (step a1; "linked-cell lists ... sub-cells of size r_cut").
 //
-// Design (sm_100a, not a translation of HOOMD's lists): counting sort of particles by cell (deterministic:
-// each cell's members are re-sorted by original index), positions gathered into cell order so that the pair
-// kernel's gathers hit 9 contiguous runs, then a warp-per-particle sweep of the 27-cell stencil with ballot
-// compaction, once to count and once to fill a CSR list.  The in/out decision is taken in fp32 with the exact
-// operation order of DESIGN.md reading R16 (no FMA contraction), so the sets are bit-identical to the oracle's.
+// Design (sm_100a, not a translation of HOOMD's lists): counting sort of particles by cell (deterministic: each cell's
+// members are re-sorted by original index), positions gathered into cell order, then ONE pass with a CTA per cell
+// (neighbor_build_cell): the <= 18 contiguous candidate runs of the cell are staged in shared memory, every
+// (particle, candidate) pair is tested once with the hits kept as bit masks, the cell reserves its segment of the index
+// array with one atomicAdd on a cursor and expands the masks into it.  Cells too large for the mask store take a two-pass
+// count / scan / fill path (neighbor_sweep_cell), remembered per context.  The in/out decision is taken in fp32 with the
+// exact operation order of DESIGN.md reading R16 (no FMA contraction), so the sets are bit-identical to the oracle's.
+// The host never waits for the build: the list size and the overflow / fallback flags come back asynchronously and are
+// examined at the next point where the stream is synchronised anyway (pse_neighbors_settle).
 #include "pse_internal.h"
 
 namespace {
@@ -180,45 +184,7 @@ __global__ void gather_positions(const float4 *posw, const int *order, int N, fl
     tile_list[tile_start[t] + atomicAdd(&tile_fill[t], 1)] = s;
 }
 
-// One warp per (sorted) particle; FILL=false counts, FILL=true writes the list.
-template <bool FILL>
-__global__ void __launch_bounds__(256) neighbor_sweep(const float4 *__restrict__ pos, int N, const int *__restrict__ cell_start,
-                                                      int nc, float cell_inv, float L, float invL, float rc2,
-                                                      int *__restrict__ count, const unsigned long long *__restrict__ off,
-                                                      int *__restrict__ idx) {
-    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (s >= N) return;
-    float4 p = pos[s];
-    int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
-    const int span = nc >= 3 ? 3 : nc;             // fewer than 3 cells per side: visit each cell once
-    int found = 0;
-    const unsigned long long base = FILL ? off[s] : 0ull;
-    for (int ix = 0; ix < span; ++ix) for (int iy = 0; iy < span; ++iy) {
-        int ccx = ix, ccy = iy;
-        if (nc >= 3) { ccx = cx + ix - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + iy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
-        const int col = (ccx * nc + ccy) * nc;
-        // cells cz-1..cz+1 of one (x,y) column are contiguous in the sorted order: one run, or two when z wraps
-        int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
-        int seg_lo[2], seg_hi[2], nseg = 1;
-        if (z0 < 0) { seg_lo[0] = cell_start[col]; seg_hi[0] = cell_start[col + z1 + 1]; seg_lo[1] = cell_start[col + nc - 1]; seg_hi[1] = cell_start[col + nc]; nseg = 2; }
-        else if (z1 >= nc) { seg_lo[0] = cell_start[col]; seg_hi[0] = cell_start[col + 1]; seg_lo[1] = cell_start[col + z0]; seg_hi[1] = cell_start[col + nc]; nseg = 2; }
-        else { seg_lo[0] = cell_start[col + z0]; seg_hi[0] = cell_start[col + z1 + 1]; }
-        for (int sg = 0; sg < nseg; ++sg) {
-            const int lo = seg_lo[sg], hi = seg_hi[sg];
-            for (int j0 = lo; j0 < hi; j0 += 32) {
-                const int j = j0 + lane;
-                bool in = false;
-                if (j < hi && j != s) in = dist2(p, pos[j], L, invL) < rc2;
-                const unsigned m = __ballot_sync(0xffffffffu, in);
-                if (FILL && in) idx[base + found + __popc(m & ((1u << lane) - 1))] = j;
-                found += __popc(m);
-            }
-        }
-    }
-    if (!FILL && lane == 0) count[s] = found;
-}
-
-// Neighbour sweep, CTA per cell (default path).  The candidates of a cell are the same for all of its particles:
+// Neighbour sweep, CTA per cell, two passes (fallback for oversized cells).  The candidates of a cell are the same for all of its particles:
 // up to 18 contiguous runs of the cell-sorted order (9 (x,y) columns, z-1..z+1 contiguous, split where z wraps).
 // They are staged once in shared memory in chunks of NS_CHUNK; each warp then takes particles of the cell and tests
 // 32 staged candidates per iteration with full lanes.  FILL=false accumulates counts, FILL=true writes the CSR
@@ -431,8 +397,10 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     for (int pi = wid; pi < np; pi += NS_THREADS / 32) {     // pass B: expand the masks word by word, a lane per candidate
         const int s = first + pi;
         const unsigned long long o = base + (unsigned long long)loc[pi];
-        if (lane == 0) { off[s] = o; count[s] = cnt[pi]; }
-        if (o + (unsigned long long)cnt[pi] > cap) continue;  // overflow: the host re-runs with a larger index array
+        const bool fits = o + (unsigned long long)cnt[pi] <= cap;
+        if (lane == 0) { off[s] = fits ? o : 0ull; count[s] = fits ? cnt[pi] : 0; }
+        if (!fits) continue;                                  // overflow: empty list here (nothing reads past the array); the
+                                                              // host sees cursor > cap later and re-runs with a larger array
         int *dst = idx + o;
         const unsigned lt = (1u << lane) - 1u;
         for (int w = 0; w < nwords; ++w) {                    // ascending candidate order; consecutive hits, consecutive addresses
@@ -542,29 +510,22 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos, c->d_tile_of, c->d_tile_start, c->d_tile_fill, c->d_tile_tmp);
     KERNEL_CHECK(c);
     PSE_TRY(pse_tile_bins(c));                       // independent of the list; enqueued first so it overlaps the read-back
-    // ---- single-pass build into a cursor-allocated index array; grows and repeats if the array was too small ----
     if (!c->d_nbr_idx) {
         const size_t cap = (size_t)N * 48 + 1024;
         if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
         c->nbr_cap = cap;
     }
-    bool done = false;
-    for (int attempt = 0; attempt < 3 && !done; ++attempt) {
+    if (!c->nbr_two_pass) {
+        // single-pass build into a cursor-allocated index array; {cursor, fallback flag} travel to the pinned mirror behind
+        // the kernel and are looked at by pse_neighbors_settle, never here
         CUDA_TRY(c, cudaMemsetAsync(c->d_nbr_ctl, 0, 2 * sizeof(unsigned long long), c->stream));
         neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
                                                                    c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
                                                                    reinterpret_cast<int *>(c->d_nbr_ctl + 1)); KERNEL_CHECK(c);
         CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->h_nbr_ctl[1] != 0) break;                            // a cell exceeds the mask store: two-pass path below
-        const unsigned long long total = c->h_nbr_ctl[0];
-        if (total <= c->nbr_cap) { c->nbr_total = (size_t)total; done = true; break; }
-        cudaFree(c->d_nbr_idx); c->d_nbr_idx = nullptr; c->nbr_cap = 0;
-        const size_t cap = (size_t)(total * 1.25) + 1024;
-        if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
-        c->nbr_cap = cap;
-    }
-    if (!done) {                                                     // general two-pass path (count, scan, fill)
+        CUDA_TRY(c, cudaEventRecord(c->ev_nbr, c->stream));
+        c->nbr_pending = true;
+    } else {                                                         // general two-pass path (count, scan, fill); synchronises
         neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
                                                                             nullptr, nullptr); KERNEL_CHECK(c);
         PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
@@ -581,9 +542,44 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         c->nbr_total = (size_t)total;
         neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
                                                                            c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
+        c->nbr_pending = false;
     }
     c->have_nbrs = true;
     return PSE_OK;
+}
+
+// Look at what the last single-pass build reported.  *redo = true: the index array was too small (it has been enlarged) or
+// a cell exceeded the mask store (the context now takes the two-pass path); the caller must build again and recompute
+// whatever consumed the list since (overflowed particles had empty lists, so nothing read out of bounds).  Waits only for
+// the build itself; called right after a stream synchronisation it does not wait at all.
+pse_status pse_neighbors_settle(pse_ctx *c, bool *redo) {
+    *redo = false;
+    if (!c->nbr_pending) return PSE_OK;
+    CUDA_TRY(c, cudaEventSynchronize(c->ev_nbr));
+    c->nbr_pending = false;
+    if (c->h_nbr_ctl[1] != 0) { c->nbr_two_pass = true; c->have_nbrs = false; *redo = true; return PSE_OK; }
+    const unsigned long long total = c->h_nbr_ctl[0];
+    if (total > c->nbr_cap) {
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));               // kernels still reading the old array
+        cudaFree(c->d_nbr_idx); c->d_nbr_idx = nullptr; c->nbr_cap = 0;
+        const size_t cap = (size_t)(total * 1.25) + 1024;
+        if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }
+        c->nbr_cap = cap; c->have_nbrs = false; *redo = true;
+        return PSE_OK;
+    }
+    c->nbr_total = (size_t)total;
+    return PSE_OK;
+}
+
+// build + settle until the list is complete (the public pse_neighbors and everything outside pse_step)
+pse_status pse_neighbors_sync(pse_ctx *c, const float *d_pos) {
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        bool redo = false;
+        PSE_TRY(pse_neighbors_impl(c, d_pos));
+        PSE_TRY(pse_neighbors_settle(c, &redo));
+        if (!redo) return PSE_OK;
+    }
+    c->err = "neighbour build did not settle"; return PSE_EOVERFLOW;
 }
 
 pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total) {
@@ -593,16 +589,21 @@ pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t
     if (d_count) { counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, d_count); KERNEL_CHECK(c); }
     if (!d_index) return PSE_OK;
     if (cap < c->nbr_total) { c->err = "pse_get_neighbors: index buffer too small"; return PSE_EOVERFLOW; }
-    int *cnt = nullptr; unsigned long long *off = nullptr;
-    CUDA_TRY(c, cudaMalloc(&cnt, (size_t)N * sizeof(int)));
-    CUDA_TRY(c, cudaMalloc(&off, (size_t)(N + 1) * sizeof(unsigned long long)));
-    counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, cnt); KERNEL_CHECK(c);
-    PSE_TRY(pse_scan_u64(c, cnt, off, (size_t)N));
-    lists_to_original<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_nbr_idx, c->d_nbr_off, c->d_nbr_count, c->d_order, N, off, d_index);
-    KERNEL_CHECK(c);
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    int *cnt = nullptr; unsigned long long *off = nullptr;                    // temporaries released on every path
+    pse_status st = PSE_OK;
+    if (cudaMalloc(&cnt, (size_t)N * sizeof(int)) != cudaSuccess || cudaMalloc(&off, (size_t)(N + 1) * sizeof(unsigned long long)) != cudaSuccess) {
+        c->err = "out of memory (pse_get_neighbors)"; st = PSE_ENOMEM;
+    }
+    if (st == PSE_OK) { counts_to_original<<<(N + T - 1) / T, T, 0, c->stream>>>(c->d_nbr_count, c->d_order, N, cnt); c->launches++; }
+    if (st == PSE_OK) st = pse_scan_u64(c, cnt, off, (size_t)N);
+    if (st == PSE_OK) {
+        lists_to_original<<<(unsigned)(((size_t)N * 32 + T - 1) / T), T, 0, c->stream>>>(c->d_nbr_idx, c->d_nbr_off, c->d_nbr_count, c->d_order, N, off, d_index);
+        c->launches++;
+        const cudaError_t e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) { c->err = std::string("pse_get_neighbors: ") + cudaGetErrorString(e); st = PSE_ECUDA; }
+    }
     cudaFree(cnt); cudaFree(off);
-    return PSE_OK;
+    return st;
 }
 
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {

@@ -28,11 +28,12 @@ struct pse_ctx {
     double win_a = 0, win_b = 0;             // window parameters handed to the kernels (see win_arg in wavespace.cu)
     float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index
     cudaStream_t stream = nullptr;
-    cudaStream_t stream2 = nullptr;          // real-space half of a full product runs here, concurrently with the wave half
-    cudaEvent_t ev_fork = nullptr, ev_real = nullptr, ev_noise = nullptr, ev_noise_r = nullptr;
+    int device = 0, nsm = 0;                 // device the context lives on (recorded at pse_create), its SM count
+    int coop_cap = 0;                        // largest cooperative grid of the Krylov step kernels on that device
+    cudaStream_t stream2 = nullptr;          // pse_step_host uploads the noise here while the step starts on `stream`
+    cudaEvent_t ev_fork = nullptr, ev_noise = nullptr, ev_noise_r = nullptr;
     bool noise_r_pending = false;            // pse_step_host: the real-space noise upload on stream2 has not been waited for yet
     bool noise_pending = false;              // pse_step_host: the wave-noise upload on stream2 has not been waited for yet
-    bool overlap = false;                    // measured neutral (1M) to slightly slower (65k): off unless PSE_OVERLAP=1
     std::string err;
     long long launches = 0;
     // ---- real-space table ----
@@ -51,6 +52,9 @@ struct pse_ctx {
     unsigned long long *d_nbr_off = nullptr; // [N+1]
     int *d_nbr_idx = nullptr; size_t nbr_cap = 0, nbr_total = 0;
     unsigned long long *d_nbr_ctl = nullptr, *h_nbr_ctl = nullptr;   // {allocation cursor, fallback flag}; pinned mirror
+    cudaEvent_t ev_nbr = nullptr;            // recorded behind the build's read-back
+    bool nbr_pending = false;                // the last build's size / flags have not been examined yet (pse_neighbors_settle)
+    bool nbr_two_pass = false;               // a cell once exceeded the mask store: this context takes the two-pass path
     // ---- FFT-grid tile bins ----
     int nt = 0, ntile = 0, Mh = 0;           // tiles per dimension, total, M/2+1
     int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]; count and fill point into d_bins
@@ -58,14 +62,9 @@ struct pse_ctx {
     int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]
-    cufftComplex *d_spec = nullptr;          // [8][M][M][Mhp]
+    cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
     cufftHandle plan_r2c[3] = {0, 0, 0}, plan_c2r[3] = {0, 0, 0};   // [0] all 8 grids, [1] planes 0-2 (F / U), [2] planes 3-7 (S / E)
     void *d_fft_work = nullptr; int nplans = 0;
-    bool own_fft = false;                    // fft.cu serves this grid size (else cuFFT)
-    float *d_fft_tw = nullptr;               // [M][2] twiddles exp(-2 pi i n / M)
-    void *d_fft_dev = nullptr;               // plan record of fft.cu
-    size_t fft_smem_plane = 0, fft_smem_x = 0;
-    int Mhp = 0;                             // row pitch of d_spec in complex entries (Mh, or padded to a multiple of 4 by fft.cu)
     // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
     float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
     float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]
@@ -149,10 +148,11 @@ __device__ __forceinline__ float warp_reduce8(const float (&a)[8], int lane, int
 // tables.cu
 void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr);
 void pse_window_table(int kind, int P, double wa, double wb, int M, std::vector<float> &dec);
-int pse_window_kind_from_env();
-double pse_es_beta_from_env(int P);
+double pse_es_beta(int P);
 // neighbors.cu
-pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);
+pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);    // enqueue only
+pse_status pse_neighbors_settle(pse_ctx *c, bool *redo);
+pse_status pse_neighbors_sync(pse_ctx *c, const float *d_pos);    // build + settle, repeated until complete
 pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n);   // exclusive, n+1 outputs
 pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n);
 pse_status pse_rank_sort(pse_ctx *c, const int *seg_start, int nseg, const int *in, int *out);
@@ -160,20 +160,16 @@ pse_status pse_get_neighbors_impl(pse_ctx *c, int *d_count, int *d_index, size_t
 pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed);
 pse_status pse_bond_forces_orig(pse_ctx *c, float *d_F);   // [N][3], original numbering, overwritten
 // realspace.cu
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st = nullptr, int ctas_per_sm = 2, int mode = PSE_MODE_ALL);   // out = M_r in
+pse_status pse_real_init(pse_ctx *c);     // per-device kernel attributes (dynamic shared memory opt-in)
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode = PSE_MODE_ALL);   // out = M_r in
 // wavespace.cu
 pse_status pse_wave_init(pse_ctx *c);
 void pse_wave_free(pse_ctx *c);
 pse_status pse_tile_bins(pse_ctx *c);
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp = nullptr, int mode = PSE_MODE_ALL);   // out (+)= M_w in
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode = PSE_MODE_ALL);   // out (+)= M_w in
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
-// fft.cu
-pse_status pse_fft_init(pse_ctx *c);
-pse_status pse_fft_forward_planes(pse_ctx *c, int first, int ncomp);
-pse_status pse_fft_x_scale(pse_ctx *c, int mode);
-pse_status pse_fft_x_inverse(pse_ctx *c);
-pse_status pse_fft_inverse_planes(pse_ctx *c, int first, int ncomp);
 // krylov.cu
+pse_status pse_krylov_init(pse_ctx *c);   // cooperative-grid cap of the step kernels on the context's device
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted
 pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed);
 pse_status pse_unpack(pse_ctx *c, const float *d_packed, float scale, float *d_U, float *d_E);

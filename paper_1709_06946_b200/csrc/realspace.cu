@@ -1,16 +1,16 @@
 // Real-space pair kernel (step a2): [U;E]_alpha = sum_beta M^(r)(x_alpha - x_beta) [F;S]_beta + self term
 // (Eqs. 25-27; self terms Eqs. A4/A12), over the neighbour list.
 //
-// Design: persistent CTAs (grid = 2 x #SM), the 64 KB table of (F1,F2,Ga,Gb | A,B,D,-) staged once per CTA in
-// shared memory, one warp per particle, lanes stride the CSR neighbour list, float4 gathers of the neighbour's
-// position and its two float4 of packed input, linear interpolation of the table in r, warp-shuffle reduction
-// of the 8 outputs.  The paper kept its tables in texture memory on a K40; shared memory gives
-// conflict-tolerant 16-byte reads with no L1 pressure on the gathers.
+// Design: persistent CTAs (2 per SM), the table of (F1,F2,Ga,Gb | A,B,D,-) staged once per CTA in shared memory as two
+// planar float4 arrays, EIGHT lanes per particle (four particles per warp, four independent idx -> pos -> input chains in
+// flight), lanes stride the CSR neighbour list, one 128-bit gather of the neighbour's position and one 256-bit gather of its
+// packed input, linear interpolation of the table in r, 7-shuffle reduction of the 8 outputs over the 8 lanes and one
+// 32-byte store per particle.  Templated on the component mask of the product.  The paper kept its tables in texture memory
+// on a K40; shared memory gives conflict-tolerant 16-byte reads with no L1 pressure on the gathers.
 //
 // Tensor algebra per pair (rh = unit separation, f = rh.F, t = S rh, q = rh.t):
 //   U += F1 (F - rh f) + F2 rh f + Ga t - Gb rh q
 //   E += A S + sym(rh (x) w),  w = -Ga F + 2B t + (Gb f + D q) rh     (projected on e1..e5; trace terms drop out)
-#include <cstdlib>
 #include "pse_internal.h"
 
 namespace {
@@ -28,7 +28,7 @@ __device__ __forceinline__ void load_packed8(const float4 *in, int b, float4 &a0
                  : "l"(in + 2 * (size_t)b));
 }
 
-template <int MODE, int G>
+template <int MODE>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
                   const unsigned long long *__restrict__ off, const int *__restrict__ cnt, const int *__restrict__ idx,
@@ -46,9 +46,9 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
         if (NEED_TE || i == 0) tabE[i] = table[2 * i + 1];
     }
     __syncthreads();
-    // G lanes per particle (32 / G particles per warp): a list of ~51 entries fills 7 passes of 8 lanes to 91 %, two
-    // passes of 32 lanes only to 80 %
-    constexpr int PPW = 32 / G;
+    // G = 8 lanes per particle (4 particles per warp): a list of ~51 entries fills 7 passes of 8 lanes to 91 %, two passes
+    // of 32 lanes only to 80 % (measured, config 3 / config 4, us per launch: 32 lanes 44.9 / 719, 16: 40.3 / 608, 8: 41.0 / 585)
+    constexpr int G = 8, PPW = 32 / G;
     const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5, gl = lane & (G - 1), grp = lane / G;
     for (int ws = blockIdx.x * wpb + (threadIdx.x >> 5); ws * PPW < N; ws += gridDim.x * wpb) {
         const int s = ws * PPW + grp;
@@ -113,73 +113,52 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             if (INS && OUTE) { e0 += t1.x * a0.w; e1 += t1.x * a1.x; e2 += t1.x * a1.y; e3 += t1.x * a1.z; e4 += t1.x * a1.w; }
         }
         const float part[8] = {u0, u1, u2, e0, e1, e2, e3, e4};
-        if (G == 32) {
-            int comp;
-            const float r = warp_reduce8(part, lane, comp);
-            if ((lane & 3) == 0 && live) reinterpret_cast<float *>(out)[(size_t)s * 8 + comp] = r;
-        } else {
-            // 8 sums over G lanes: every step halves the values a lane carries (4 + 2 + 1 shuffles for G = 8, where lane
-            // gl ends with component gl and the group stores 32 contiguous bytes)
-            constexpr int O1 = G / 2, O2 = G / 4;
-            const bool h1 = gl & O1, h2 = gl & O2;
-            float r4[4], r2[2];
+        // 8 sums over 8 lanes in 4 + 2 + 1 shuffles: every step halves the values a lane carries; lane gl ends with component gl
+        const bool h1 = gl & 4, h2 = gl & 2, h3 = gl & 1;
+        float r4[4], r2[2];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) r4[c] = (h1 ? part[c + 4] : part[c]) + __shfl_xor_sync(0xffffffffu, h1 ? part[c] : part[c + 4], O1);
+        for (int c = 0; c < 4; ++c) r4[c] = (h1 ? part[c + 4] : part[c]) + __shfl_xor_sync(0xffffffffu, h1 ? part[c] : part[c + 4], 4);
 #pragma unroll
-            for (int c = 0; c < 2; ++c) r2[c] = (h2 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h2 ? r4[c] : r4[c + 2], O2);
-            float *o = reinterpret_cast<float *>(out) + (size_t)s * 8 + (h1 ? 4 : 0) + (h2 ? 2 : 0);
-            if (G == 4) {
-                if (live) *reinterpret_cast<float2 *>(o) = make_float2(r2[0], r2[1]);
-            } else {
-                constexpr int O3 = G / 8;
-                const bool h3 = gl & O3;
-                float r = (h3 ? r2[1] : r2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? r2[0] : r2[1], O3);
-                if (G == 16) r += __shfl_xor_sync(0xffffffffu, r, 1);
-                if (live && (G == 8 || (gl & 1) == 0)) o[h3 ? 1 : 0] = r;
-            }
-        }
+        for (int c = 0; c < 2; ++c) r2[c] = (h2 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h2 ? r4[c] : r4[c + 2], 2);
+        const float r = (h3 ? r2[1] : r2[0]) + __shfl_xor_sync(0xffffffffu, h3 ? r2[0] : r2[1], 1);
+        if (live) reinterpret_cast<float *>(out)[(size_t)s * 8 + gl] = r;
     }
 }
 
 }  // namespace
 
-template <int MODE, int G>
-static pse_status launch_real_g(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<MODE, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
-    real_pairs_kernel<MODE, G><<<grid, 512, smem, st>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
-                                                     c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
-                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
+constexpr size_t REAL_SMEM = (size_t)PSE_NTAB * 2 * sizeof(float4);
+
+template <int MODE>
+static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, int grid) {
+    real_pairs_kernel<MODE><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
+                                                               c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
+                                                               (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
     KERNEL_CHECK(c);
     return PSE_OK;
 }
 
-template <int MODE>
-static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int grid, size_t smem) {
-    // measured (config 3 / config 4, us per launch): 32 lanes per particle 44.9 / 719, 16: 40.3 / 608, 8: 41.0 / 585, 4: 41.1 / 591
-    static const bool wide = getenv("PSE_PAIR_LANES") && atoi(getenv("PSE_PAIR_LANES")) == 32;
-    return wide ? launch_real_g<MODE, 32>(c, d_in, d_out, st, grid, smem) : launch_real_g<MODE, 8>(c, d_in, d_out, st, grid, smem);
+// dynamic shared-memory opt-in of every instantiation on the context's device (called by pse_create)
+pse_status pse_real_init(pse_ctx *c) {
+#define PSE_REAL_ATTR(M) CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REAL_SMEM))
+    PSE_REAL_ATTR(PSE_IN_S | PSE_OUT_E); PSE_REAL_ATTR(PSE_IN_F | PSE_OUT_E); PSE_REAL_ATTR(PSE_IN_F | PSE_IN_S | PSE_OUT_U);
+    PSE_REAL_ATTR(PSE_IN_S | PSE_OUT_U); PSE_REAL_ATTR(PSE_IN_F | PSE_OUT_U); PSE_REAL_ATTR(PSE_MODE_ALL);
+#undef PSE_REAL_ATTR
+    return PSE_OK;
 }
 
-pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, cudaStream_t st, int ctas_per_sm, int mode) {
-    const bool own = (st == nullptr);
-    if (own) st = c->stream;
-    ScopedPhase ph(c, own ? PSE_T_REAL : -1);
-    static int nsm = 0;
-    if (!nsm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
-    const size_t smem = (size_t)PSE_NTAB * 2 * sizeof(float4);
-    int grid = ctas_per_sm * nsm, wpb = 512 / 32;
-    if ((long long)grid * wpb > c->N) grid = (c->N + wpb - 1) / wpb;
+pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode) {
+    ScopedPhase ph(c, PSE_T_REAL);
+    int grid = 2 * c->nsm;
+    const int wpb = 512 / 32;
+    if ((long long)grid * wpb * 4 > c->N) grid = (c->N + wpb * 4 - 1) / (wpb * 4);
     // unrequested outputs are written as zeros; absent inputs must be zero in d_in (they are skipped, not read as data)
     switch (mode) {
-        case PSE_IN_S | PSE_OUT_E: return launch_real<PSE_IN_S | PSE_OUT_E>(c, d_in, d_out, st, grid, smem);
-        case PSE_IN_F | PSE_OUT_E: return launch_real<PSE_IN_F | PSE_OUT_E>(c, d_in, d_out, st, grid, smem);
-        case PSE_IN_F | PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
-        case PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
-        case PSE_IN_F | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_OUT_U>(c, d_in, d_out, st, grid, smem);
-        default: return launch_real<PSE_MODE_ALL>(c, d_in, d_out, st, grid, smem);
+        case PSE_IN_S | PSE_OUT_E: return launch_real<PSE_IN_S | PSE_OUT_E>(c, d_in, d_out, grid);
+        case PSE_IN_F | PSE_OUT_E: return launch_real<PSE_IN_F | PSE_OUT_E>(c, d_in, d_out, grid);
+        case PSE_IN_F | PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid);
+        case PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid);
+        case PSE_IN_F | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_OUT_U>(c, d_in, d_out, grid);
+        default: return launch_real<PSE_MODE_ALL>(c, d_in, d_out, grid);
     }
 }

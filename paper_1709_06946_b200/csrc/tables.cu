@@ -9,7 +9,6 @@
 // by 1/(6 pi eta a):  (F1, F2, G1+G2, G1+4G2, A, B, D, 0)  at r_i = i * dr, i = 0..ntab-1, dr = rcut/(ntab-2).
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <vector>
 #include "pse_internal.h"
 
@@ -136,14 +135,5 @@ void pse_window_table(int kind, int P, double wa, double wb, int M, std::vector<
     }
 }
 
-int pse_window_kind_from_env() {
-    const char *e = getenv("PSE_WINDOW");
-    return (e && (e[0] == 'g' || e[0] == 'G')) ? 0 : 1;
-}
-
-// shape parameter of the exponential-of-semicircle window; PSE_ES_BETA (a multiple of P) overrides the default
-double pse_es_beta_from_env(int P) {
-    const char *e = getenv("PSE_ES_BETA");
-    const double per_point = e ? atof(e) : 2.2;
-    return per_point * P;
-}
+// shape parameter of the exponential-of-semicircle window: beta = 2.2 P (calibrated against the oracle, R3/R6)
+double pse_es_beta(int P) { return 2.2 * P; }

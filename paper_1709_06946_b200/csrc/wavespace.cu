@@ -387,8 +387,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const size_t nmode = (size_t)plane * M, o = (size_t)ix * plane + rem;
     float kx, ky, kz;
     float2 zero = make_float2(0.f, 0.f);
-    // the noise buffer has the ABI's [M][M][Mh] layout; the spectrum rows may be padded to Mhp entries
-    const size_t oplane = (size_t)M * M * sp.Mhp, oo = ((size_t)ix * M + iy) * sp.Mhp + iz;
+    const size_t oplane = nmode, oo = o;
     if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
 #pragma unroll
         for (int c = 0; c < 8; ++c) spec[c * oplane + oo] = zero;
@@ -420,14 +419,12 @@ pse_status pse_wave_init(pse_ctx *c) {
     const int M = c->M;
     c->Mh = M / 2 + 1;
     c->nt = (M + T - 1) / T; c->ntile = c->nt * c->nt * c->nt;
-    PSE_TRY(pse_fft_init(c));                          // decides own FFT vs cuFFT and with it the spectrum pitch
-    const size_t M3 = pse_plane_stride(M), nmode = (size_t)M * M * c->Mhp;
+    const size_t M3 = pse_plane_stride(M), nmode = (size_t)M * M * c->Mh;
     CUDA_TRY(c, cudaMalloc(&c->d_grid, 8 * M3 * sizeof(float)));
     CUDA_TRY(c, cudaMalloc(&c->d_spec, 8 * nmode * sizeof(cufftComplex)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_start, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
-    if (c->own_fft) return PSE_OK;                    // fft.cu serves this size: no cuFFT plans, no work area
     int n[3] = {M, M, M};
     const int batches[3] = {8, 3, 5};                 // all grids | planes 0-2 (F in, U out) | planes 3-7 (S in, E out)
     size_t w = 0;
@@ -455,7 +452,7 @@ pse_status pse_wave_init(pse_ctx *c) {
 
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
-    cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work); cudaFree(c->d_fft_tw); cudaFree(c->d_fft_dev);
+    cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
     cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
 }
 
@@ -470,16 +467,14 @@ static inline void plane_range(int bits, int &plan, int &first) {
     plan = bits == 3 ? 0 : bits; first = bits == 2 ? 3 : 0;
 }
 
-static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, cudaEvent_t wait_ev = nullptr, int mode = PSE_MODE_ALL) {
+static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, int mode = PSE_MODE_ALL) {
     {
         ScopedPhase ph(c, PSE_T_FFT_INV);
         int plan, first;
         plane_range((mode >> 2) & 3, plan, first);
         const size_t M3 = pse_plane_stride(c->M), nmode = (size_t)c->M * c->M * c->Mh;
-        if (c->own_fft) PSE_TRY(pse_fft_inverse_planes(c, first, plan == 0 ? 8 : plan == 1 ? 3 : 5));
-        else { CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++; }
+        CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++;
     }
-    if (wait_ev) CUDA_TRY(c, cudaStreamWaitEvent(c->stream, wait_ev, 0));
     ScopedPhase ph(c, PSE_T_INTERP);
     const int TB = 256, E = T + c->P - 1;
     const int Ez = E + ((c->P - E) & 7);
@@ -515,7 +510,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     return PSE_OK;
 }
 
-pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, cudaEvent_t wait_before_interp, int mode) {
+pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode) {
     const size_t nmode = (size_t)c->M * c->M * c->Mh, M3 = pse_plane_stride(c->M);
     if (!(mode & (PSE_IN_F | PSE_IN_S)) || !(mode & (PSE_OUT_U | PSE_OUT_E))) { c->err = "pse_wave_apply: empty component mask"; return PSE_EINVAL; }
     int plan, first;
@@ -529,17 +524,12 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
         else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         KERNEL_CHECK(c);
     }
-    if (c->own_fft) {
-        { ScopedPhase ph(c, PSE_T_FFT_FWD); PSE_TRY(pse_fft_forward_planes(c, first, plan == 0 ? 8 : plan == 1 ? 3 : 5)); }
-        { ScopedPhase ph(c, PSE_T_SCALE); PSE_TRY(pse_fft_x_scale(c, mode)); }      // x transform, operator, inverse x transform
-        return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp, mode);
-    }
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[plan], c->d_grid + first * M3, c->d_spec + first * nmode)); c->launches++; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
         scale_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(c->d_spec, make_scale_params(c, mode)); KERNEL_CHECK(c);
     }
-    return inverse_and_interpolate(c, d_out, accumulate, wait_before_interp, mode);
+    return inverse_and_interpolate(c, d_out, accumulate, mode);
 }
 
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {
@@ -550,7 +540,6 @@ pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out
         scale_brownian_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(
             c->d_spec, reinterpret_cast<const float2 *>(d_noise_wave), make_scale_params(c));
         KERNEL_CHECK(c);
-        if (c->own_fft) PSE_TRY(pse_fft_x_inverse(c));
     }
     return inverse_and_interpolate(c, d_out, accumulate);
 }

@@ -433,41 +433,6 @@ def test_config3_full_size_properties_and_sampled_rows():
     assert rel(res[0.5]['real'][rows], np.hstack([Ur, Er])) < 2e-5
 
 
-@pytest.mark.parametrize('grid', [32, 36, 40, 45, 48, 50, 54, 60])
-def test_own_fft_path_matches_oracle_and_cufft(grid, monkeypatch):
-    """PSE_FFT=own (csrc/fft.cu: plane transforms + x pass fused with the k-space operator) against the oracle's direct
-    sum over the same grid modes, and against the default cuFFT path, for grids whose sizes exercise every radix
-    (32 = 16*2, 36 = 12*3, 40 = 10*4, 45 = 9*5 (odd), 48 = 16*3, 50 = 10*5, 54 = 9*6, 60 = 12*5)."""
-    import paper_1709_06946_b200 as pse
-    N, tol, xi, P = 64, 1e-3, 0.6, 8
-    x, L = synth.rsa(N, 0.10, seed=5)
-    x32 = x.astype(np.float32)
-    _, _, _, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
-    F, S = synth.gaussian_inputs(N, 2)
-    _, w2 = synth.brownian_noise(N, grid, 4)
-    out = {}
-    for name in ('cufft', 'own'):
-        monkeypatch.setenv('PSE_FFT', name)
-        ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
-        ctx.pse_neighbors(dev(pos4(x32)))
-        U, E = gpu_apply(ctx, F, S, 2)
-        UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
-        ctx.pse_brownian(0.5, torch.zeros(N, 8, device='cuda'), dev(w2), UB, EB)
-        torch.cuda.synchronize()
-        out[name] = (np.hstack([U, E]), np.hstack([UB.cpu().numpy(), EB.cpu().numpy()]))
-    xd = x32.astype(np.float64)
-    k = brn.grid_modes(grid, L)
-    k2 = np.einsum('ki,ki->k', k, k)
-    w = fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2)
-    Ug, Eg = mob.wave_apply_modes(xd, L, A, ETA, k, w, F, S)
-    Uw, Ew = brn.wave_sqrt_apply(xd, L, A, ETA, xi, grid, w2)
-    amp = np.sqrt(2 * KT / 0.5)
-    assert rel(out['own'][0], np.hstack([Ug, Eg])) < tol
-    assert rel(out['own'][1], amp * np.hstack([Uw, Ew])) < tol
-    assert rel(out['own'][0], out['cufft'][0]) < 2e-5
-    assert rel(out['own'][1], out['cufft'][1]) < 2e-5
-
-
 @pytest.mark.parametrize('N,sep', [(1, None), (2, 1.6), (2, 2.5), (3, 9.0)])
 def test_degenerate_sizes_against_oracle(N, sep):
     """One particle (only self terms and its own periodic images: the Hasimoto lattice), an overlapping pair (r < 2a,
