@@ -106,6 +106,7 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     if (rcut > 0.5 * L) { c->err = "pse_create: rcut > L/2 (minimum-image real-space sum)"; return PSE_EINVAL; }
     if (rcut < 2.0 * a) { c->err = "pse_create: rcut < 2a (overlap forces need contact pairs)"; return PSE_EINVAL; }
     if (P > grid || P > PSE_MAXP) { c->err = "pse_create: P > grid or P > 16"; return PSE_EINVAL; }
+    if (grid > 1024) { c->err = "pse_create: grid > 1024 points per dimension (support bases are packed in 10 bits)"; return PSE_EINVAL; }
     if (window != PSE_WINDOW_GAUSS && window != PSE_WINDOW_ES) { c->err = "pse_create: unknown window"; return PSE_EINVAL; }
     c->N = N; c->L = L; c->a = a; c->eta = eta; c->kT = kT; c->xi = xi; c->M = grid; c->P = P; c->rcut = rcut; c->tol = tol;
     c->h = L / grid;
@@ -153,10 +154,11 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
-    c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1);
+    c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1) + (size_t)(2 * c->ntile + 1);
     CUDA_TRY(c, cudaMalloc(&c->d_bins, c->bins_n * sizeof(int)));
     c->d_cell_count = c->d_bins; c->d_cell_fill = c->d_cell_count + c->ncell + 1;
     c->d_tile_count = c->d_cell_fill + c->ncell + 1; c->d_tile_fill = c->d_tile_count + c->ntile + 1;
+    c->d_half_count = c->d_tile_fill + c->ntile + 1;
     {
         std::vector<float> dec;
         pse_window_table(c->win_kind, P, c->win_a, c->win_b, grid, dec);

@@ -509,7 +509,8 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     pse_rank_sort(c, c->d_cell_start, c->ncell, c->d_order_tmp, c->d_order);
     gather_positions<<<nb, T, 0, c->stream>>>(c->d_posw, c->d_order, N, c->d_pos, c->d_tile_of, c->d_tile_start, c->d_tile_fill, c->d_tile_tmp);
     KERNEL_CHECK(c);
-    PSE_TRY(pse_tile_bins(c));                       // independent of the list; enqueued first so it overlaps the read-back
+    PSE_TRY(pse_tile_bins(c));
+    PSE_TRY(pse_particle_windows(c));
     if (!c->d_nbr_idx) {
         const size_t cap = (size_t)N * 48 + 1024;
         if (cudaMalloc(&c->d_nbr_idx, cap * sizeof(int)) != cudaSuccess) { c->err = "out of memory (neighbour list)"; return PSE_ENOMEM; }

@@ -1,5 +1,6 @@
 // Internal declarations of libpse (not part of the ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <cstdint>
@@ -46,7 +47,7 @@ struct pse_ctx {
     int *d_order = nullptr;                  // [N] sorted -> original
     int *d_order_tmp = nullptr, *d_tile_tmp = nullptr;   // [N] unsorted scatter targets
     int *d_cell_of = nullptr;                // [N] cell of original particle
-    int *d_bins = nullptr; size_t bins_n = 0;   // one block cleared by a single memset: cell_count | cell_fill | tile_count | tile_fill
+    int *d_bins = nullptr; size_t bins_n = 0;   // one block cleared by a single memset: cell_count | cell_fill | tile_count | tile_fill | half_count
     int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]; count and fill point into d_bins
     int *d_nbr_count = nullptr;              // [N]
     unsigned long long *d_nbr_off = nullptr; // [N+1]
@@ -60,11 +61,22 @@ struct pse_ctx {
     int *d_tile_count = nullptr, *d_tile_start = nullptr, *d_tile_fill = nullptr;   // [ntile+1]; count and fill point into d_bins
     int *d_tile_of = nullptr;                // [N] tile of the particle's support base, original numbering
     int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
+    // ---- per-particle window data, computed once per pse_neighbors and shared by every spread / interpolation of that
+    //      configuration (a step runs ~25 of them on two configurations) ----
+    int *d_pbase = nullptr;                  // [N] wrapped support base, packed bx | by << 10 | bz << 20 (sorted numbering)
+    float *d_pw = nullptr;                   // [N][3][PP] window values at the P support points per dimension, PP = P rounded up to 4
+    int PP = 0;
+    // particles that reach each half tile (4 x 8 x 8 grid points, one warp of the spread kernel): CSR, built in pse_neighbors
+    int *d_half_count = nullptr;             // [2 ntile + 1], inside d_bins
+    int *d_half_start = nullptr, *d_half_list = nullptr;
+    size_t half_cap = 0;
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]
     cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
     cufftHandle plan_r2c[3] = {0, 0, 0}, plan_c2r[3] = {0, 0, 0};   // [0] all 8 grids, [1] planes 0-2 (F / U), [2] planes 3-7 (S / E)
     void *d_fft_work = nullptr; int nplans = 0;
+    CUtensorMap tmap_grid[9];                // TMA descriptor of d_grid as a [8][M][M][M] tensor with the (T+P-1)^3 box of this P (index P)
+    bool tma_ok = false;                     // descriptor valid (needs M % 4 == 0)
     // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
     float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
     float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]
@@ -166,6 +178,7 @@ pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode 
 pse_status pse_wave_init(pse_ctx *c);
 void pse_wave_free(pse_ctx *c);
 pse_status pse_tile_bins(pse_ctx *c);
+pse_status pse_particle_windows(pse_ctx *c);   // d_pbase, d_pw from d_pos (after the cell sort)
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode = PSE_MODE_ALL);   // out (+)= M_w in
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
 // krylov.cu

@@ -214,6 +214,203 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
     }
 }
 
+// ---- per-particle window data -------------------------------------------------------------------------------------------
+// Positions are fixed between two pse_neighbors calls while ~25 spreads / interpolations run on them, so the P window values
+// per dimension (a sqrt and an exp each for the default window) and the wrapped support base are computed once here.
+__global__ void particle_window_kernel(const float4 *__restrict__ pos, int N, int M, int P, int PP, float inv_h, float wa, float wb,
+                                       int *__restrict__ pbase, float *__restrict__ pw) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float4 p = pos[s];
+    const float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
+    int packed = 0;
+    for (int d = 0; d < 3; ++d) {
+        const int base = support_base(g[d], P);
+        packed |= pmod(base, M) << (10 * d);
+        for (int i = 0; i < PP; ++i)
+            pw[((size_t)s * 3 + d) * PP + i] = i < P ? __expf(win_arg((float)(base + i) - g[d], wa, wb)) : 0.f;
+    }
+    pbase[s] = packed;
+}
+
+// ---- lists of the particles that reach each half tile (built once per pse_neighbors, used by every spread) -----------------
+// A "half" is the 4 x 8 x 8 block of grid points one warp of the spread kernel owns: half index = (tile index) * 2 + (x half).
+// One warp per half walks the particles binned in the tiles that can reach it (two per dimension, three next to a partial last
+// tile), 32 at a time, keeps those whose support overlaps the half and appends them in candidate order with a ballot: no
+// atomics, deterministic.  WRITE = false counts (the offsets come from a scan in between), WRITE = true writes.
+template <bool WRITE>
+__global__ void __launch_bounds__(128)
+half_lists_kernel(const int *__restrict__ pbase, const int *__restrict__ tile_start, const int *__restrict__ tile_list, int M, int P, int nt,
+                  int nhalf, int *__restrict__ half_count, const int *__restrict__ half_start, int *__restrict__ half_list) {
+    __shared__ int s_lo[4][32], s_cum[4][33], s_reach[4][3][4], s_nreach[4][3];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, h = blockIdx.x * 4 + w;
+    if (h >= nhalf) return;
+    const int t = h >> 1, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
+    const int lo[3] = {t0 * T + 4 * (h & 1), t1 * T, t2 * T};
+    if (lane < 3) s_nreach[w][lane] = reach_tiles(lane == 0 ? t0 : (lane == 1 ? t1 : t2), M, P, nt, s_reach[w][lane]);
+    __syncwarp();
+    const int ny = s_nreach[w][1], nz = s_nreach[w][2], n = s_nreach[w][0] * ny * nz;      // n <= 27 for P <= 8
+    int cnt = 0, first = 0;
+    if (lane < n) {
+        const int i = lane / (ny * nz), j = (lane / nz) % ny, k = lane % nz;
+        const int tb = (s_reach[w][0][i] * nt + s_reach[w][1][j]) * nt + s_reach[w][2][k];
+        first = tile_start[tb];
+        cnt = tile_start[tb + 1] - first;
+    }
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    s_lo[w][lane] = first; s_cum[w][lane + 1] = inc;
+    if (lane == 0) s_cum[w][0] = 0;
+    const int total = __shfl_sync(0xffffffffu, inc, 31);
+    __syncwarp();
+    const int halfM = M >> 1;
+    int found = 0;
+    int *dst = WRITE ? half_list + half_start[h] : nullptr;
+    for (int c0 = 0; c0 < total; c0 += 32) {
+        const int ci = c0 + lane;
+        bool hit = false;
+        int s = 0;
+        if (ci < total) {
+            int k = 0;
+            for (int q = 1; q < n; ++q) k += (s_cum[w][q] <= ci);
+            s = tile_list[s_lo[w][k] + ci - s_cum[w][k]];
+            const int b = pbase[s];
+            hit = true;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                int so = lo[d] - ((b >> (10 * d)) & 1023);                  // offset of the half's origin from the support base
+                so += so < -halfM ? M : 0;
+                so -= so > halfM ? M : 0;
+                hit = hit && so > -(d == 0 ? 4 : 8) && so < P;
+            }
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, hit);
+        if (WRITE && hit) dst[found + __popc(bal & ((1u << lane) - 1u))] = s;
+        found += __popc(bal);
+    }
+    if (!WRITE && lane == 0) half_count[h] = found;
+}
+
+// ---- spread (a3), default path for P <= 8 ---------------------------------------------------------------------------------
+// Gather form with REGISTER accumulators, as before, but with the lane footprint matched to the support: a lane owns a
+// 2 x 2 x 2 block of grid points (8 points x NC components in registers), a warp a 4 x 8 x 8 half of an 8^3 tile, and a lane
+// evaluates a particle only if the particle's P^3 support really overlaps its block: (P/(P+1))^3 = 51 % of its FMAs are then
+// useful at P = 4, against 17 % when a half-warp owned a whole 8 x 8 face (ncu, round 1).  Per warp, with no CTA barrier:
+//   1. the particles that reach the warp's half come from the list built in pse_neighbors, 32 at a time, one per lane: the
+//      lane stages its particle in shared memory (inputs, zero-padded window rows, the offset of the half's origin from the
+//      support base, and a 10-bit code of the blocks the support overlaps per dimension);
+//   2. every lane builds a 64-bit mask of the staged particles whose code covers its own block (one AND + compare each);
+//   3. every lane walks its own mask: 6 window values, 12 products, 8 x NC FMAs per entry.
+// No atomics, no memset, each grid value written once (8-byte stores), summation in list order (deterministic).
+template <int P, int C0, int NC>
+__global__ void __launch_bounds__(64)
+spread_blocks_kernel(const int *__restrict__ pbase, const float *__restrict__ pw, const float4 *__restrict__ in,
+                     const int *__restrict__ half_start, const int *__restrict__ half_list, float *__restrict__ grid, int M, int nt) {
+    constexpr int CAP = 64, PP = (P + 3) & ~3, WR = P + 2;
+    __shared__ __align__(16) unsigned s_code[2][CAP];
+    __shared__ unsigned s_off[2][CAP];
+    __shared__ float4 s_q[2][CAP][2];
+    __shared__ float s_w[2][CAP][3 * WR];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
+    const int lo[3] = {t0 * T + 4 * w, t1 * T, t2 * T};            // origin of the warp's half: 4 x 8 x 8 points
+    const int first = half_start[2 * t + w], total = half_start[2 * t + w + 1] - first;
+    const int rxl = lane >> 4, ryl = (lane >> 2) & 3, rzl = lane & 3;            // my block inside the half: 2 x 4 x 4 blocks
+    const unsigned mymask = (1u << rxl) | (1u << (2 + ryl)) | (1u << (6 + rzl));
+    const int cx = 2 * rxl + 1 - 16, cy = 2 * ryl + 1 - 16, cz = 2 * rzl + 1 - 16;
+    const int halfM = M >> 1;
+    float acc[8][NC];
+#pragma unroll
+    for (int m = 0; m < 8; ++m)
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[m][c] = 0.f;
+    for (int c0 = 0; c0 < total; c0 += CAP) {
+        const int nb = min(CAP, total - c0);
+        // 1. stage up to CAP particles of the list, one per lane and pass
+#pragma unroll
+        for (int pass = 0; pass < CAP / 32; ++pass) {
+            const int slot = pass * 32 + lane;
+            if (slot < nb) {
+                const int s = half_list[first + c0 + slot];
+                const int b = pbase[s];
+                unsigned code = 0, off = 0;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const int nblk = d == 0 ? 2 : 4, sh = d == 0 ? 0 : (d == 1 ? 2 : 6);
+                    int so = lo[d] - ((b >> (10 * d)) & 1023);                  // offset of the half's origin from the support base,
+                    so += so < -halfM ? M : 0;                                  // minimum image: -len < so < P for a listed particle
+                    so -= so > halfM ? M : 0;
+                    const int rmin = max(0, (-so) >> 1), rmax = min(nblk - 1, (P - 1 - so) >> 1);      // blocks r with -1-2r <= so <= P-1-2r
+                    code |= (((2u << rmax) - 1u) & ~((1u << rmin) - 1u)) << sh;
+                    off |= (unsigned)((so + 16) & 255) << (8 * d);
+                }
+                s_code[w][slot] = code; s_off[w][slot] = off;
+                s_q[w][slot][0] = in[2 * s]; s_q[w][slot][1] = in[2 * s + 1];
+                const float4 *src = reinterpret_cast<const float4 *>(pw + (size_t)s * 3 * PP);
+                float *dst = s_w[w][slot];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    float v[PP];
+#pragma unroll
+                    for (int i4 = 0; i4 < PP / 4; ++i4) { const float4 x = src[d * (PP / 4) + i4]; v[4 * i4] = x.x; v[4 * i4 + 1] = x.y; v[4 * i4 + 2] = x.z; v[4 * i4 + 3] = x.w; }
+                    dst[d * WR] = 0.f;
+#pragma unroll
+                    for (int i = 0; i < P; ++i) dst[d * WR + 1 + i] = v[i];
+                    dst[d * WR + P + 1] = 0.f;
+                }
+            } else if (slot < ((nb + 3) & ~3)) s_code[w][slot] = 0u;            // padding of the last group of four codes
+        }
+        __syncwarp();
+        // 2. my particles of this batch as a bit mask (four codes per 16-byte shared load)
+        unsigned mlo = 0u, mhi = 0u;
+#pragma unroll
+        for (int i4 = 0; i4 < CAP / 4; ++i4) {
+            if (4 * i4 < nb) {
+                const uint4 cd = *reinterpret_cast<const uint4 *>(&s_code[w][4 * i4]);
+                const unsigned bits = ((cd.x & mymask) == mymask ? 1u : 0u) | ((cd.y & mymask) == mymask ? 2u : 0u) |
+                                      ((cd.z & mymask) == mymask ? 4u : 0u) | ((cd.w & mymask) == mymask ? 8u : 0u);
+                if (i4 < 8) mlo |= bits << (4 * i4); else mhi |= bits << (4 * (i4 - 8));
+            }
+        }
+        unsigned long long m = ((unsigned long long)mhi << 32) | mlo;
+        // 3. walk the mask
+        while (m) {
+            const int i = __ffsll((long long)m) - 1;
+            m &= m - 1ull;
+            const unsigned off = s_off[w][i];
+            const float *wr = s_w[w][i];
+            const int ix = (int)(off & 255u) + cx, iy = (int)((off >> 8) & 255u) + cy, iz = (int)((off >> 16) & 255u) + cz;
+            const float wx0 = wr[ix], wx1 = wr[ix + 1], wy0 = wr[WR + iy], wy1 = wr[WR + iy + 1], wz0 = wr[2 * WR + iz], wz1 = wr[2 * WR + iz + 1];
+            const float4 q0 = s_q[w][i][0], q1 = s_q[w][i][1];
+            const float qv[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+            const float wxy[4] = {wx0 * wy0, wx0 * wy1, wx1 * wy0, wx1 * wy1};
+#pragma unroll
+            for (int ab = 0; ab < 4; ++ab) {
+                const float w0 = wxy[ab] * wz0, w1 = wxy[ab] * wz1;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) { acc[2 * ab][c] += w0 * qv[C0 + c]; acc[2 * ab + 1][c] += w1 * qv[C0 + c]; }
+            }
+        }
+        __syncwarp();
+    }
+    const size_t M3 = pse_plane_stride(M);
+    const int gz = lo[2] + 2 * rzl;
+    const bool pair_ok = !(M & 1) && gz + 1 < M;                     // even M: rows start 8-byte aligned
+#pragma unroll
+    for (int ab = 0; ab < 4; ++ab) {
+        const int gx = lo[0] + 2 * rxl + (ab >> 1), gy = lo[1] + 2 * ryl + (ab & 1);
+        if (gx >= M || gy >= M || gz >= M) continue;
+        const size_t o = ((size_t)gx * M + gy) * M + gz;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            float *dst = grid + (C0 + c) * M3 + o;
+            if (pair_ok) *reinterpret_cast<float2 *>(dst) = make_float2(acc[2 * ab][c], acc[2 * ab + 1][c]);
+            else { dst[0] = acc[2 * ab][c]; if (gz + 1 < M) dst[1] = acc[2 * ab + 1][c]; }
+        }
+    }
+}
+
 // Interpolation (a7): warp per particle (visited in tile order for L1/L2 locality), lanes over the P^3 support.
 __global__ void __launch_bounds__(256)
 interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list, const float *__restrict__ grid,
@@ -263,106 +460,126 @@ interp_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list,
     }
 }
 
-// Interpolation, tile-staged (default path): one CTA per tile bin.  The (T+P-1)^3 block of all 8 grids that the
-// bin's particles can touch is staged once in shared memory with coalesced loads (periodic wrap resolved while
-// loading), then each warp takes particles of the bin, lanes over the P^3 support, reading only shared memory.
-// Every particle belongs to exactly one bin, so the output is written once, with no atomics.
-template <int PT>                                  // PT > 0: support size known at compile time (no integer divisions)
+// Interpolation (a7), default path for P <= 8: one CTA per tile bin (every particle belongs to exactly one bin, so the output is
+// written once, no atomics).  The (T+P-1)^3 block of the requested planes that the bin's particles can touch is staged in
+// shared memory, planar, [plane][ix][iy][iz]:
+//   * tiles whose block does not cross the periodic seam: ONE TMA box copy per plane (cp.async.bulk.tensor.4d on the
+//     [8][M][M][M] grid array, completion on an mbarrier) issued by one thread: no staging instructions at all;
+//   * seam tiles, or grids whose row pitch is not a multiple of 16 bytes (M % 4 != 0, which TMA cannot address): 4-byte
+//     cp.async copies with the wrap resolved per row.
+// Only the planes the product asks for are staged (3, 5 or 8), so more CTAs are resident.  Then eight lanes per particle, four
+// particles per warp: a lane owns (j,k) columns of the support and walks them along x; the window values come from the
+// per-particle table of pse_neighbors (no exp / sqrt here); 7-shuffle reduction leaves component gl in lane gl.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <int PT> struct InterpGeom {
+    static constexpr int E = T + PT - 1, EP = (E + 3) & ~3, PL = ((E * E * EP * 4 + 127) / 128 * 128) / 4;   // floats per staged plane
+};
+
+template <int PT, int C0, int NC>
 __global__ void __launch_bounds__(256)
-interp_tile_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_start, const int *__restrict__ tile_list,
-                   const float *__restrict__ grid, float4 *__restrict__ out, int M, int Prt, int nt, float inv_h, float wa, float wb,
-                   int accumulate, int mode) {
-    extern __shared__ float4 sm[];
-    const int P = PT ? PT : Prt;
-    const int E = T + P - 1, Ez = E + ((P - E) & 7), E3 = E * E * Ez;   // z-rows padded so that Ez = P (mod 8): the
-    float4 *lo = sm, *hi = sm + E3;                                      // 16-byte chunks of a (j,k) lane set never collide
+interp_planes_kernel(const __grid_constant__ CUtensorMap tmap, const int *__restrict__ pbase, const float *__restrict__ pw,
+                     const int *__restrict__ tile_start, const int *__restrict__ tile_list, const float *__restrict__ grid,
+                     float *__restrict__ out, int M, int nt, int accumulate, int use_tma) {
+    constexpr int P = PT, E = InterpGeom<PT>::E, EP = InterpGeom<PT>::EP, PL = InterpGeom<PT>::PL, PP = (P + 3) & ~3, EE = E * EP;
+    extern __shared__ __align__(128) float sm[];                    // [NC][PL]
+    __shared__ __align__(8) unsigned long long bar;
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int first = tile_start[t], np = tile_start[t + 1] - first;
     if (np == 0) return;
-    const size_t M3 = pse_plane_stride(M);
-    {   // stage row by row: a half-warp (E <= 16) or a warp per (ix,iy) row, lanes along z; wrap by subtraction
-        const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-        const int rpi = E <= 16 ? 2 : 1, lz = E <= 16 ? (lane & 15) : lane, sub = E <= 16 ? (lane >> 4) : 0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const bool seam = t0 * T + E > M || t1 * T + E > M || t2 * T + E > M;
+    if (use_tma && !seam) {
+        if (threadIdx.x == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar)));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bar)), "r"(NC * E * E * EP * 4) : "memory");
+#pragma unroll
+            for (int c = 0; c < NC; ++c)
+                asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                             ::"r"(smem_u32(sm + c * PL)), "l"(&tmap), "r"(t2 * T), "r"(t1 * T), "r"(t0 * T), "r"(C0 + c), "r"(smem_u32(&bar))
+                             : "memory");
+        }
+        unsigned done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(smem_u32(&bar)) : "memory");
+    } else {
+        const size_t M3 = pse_plane_stride(M);
+        // a half-warp (E <= 16) per (ix,iy) row, lanes along z; wrap by subtraction; all copies in flight at once
+        const int lz = lane & 15, sub = lane >> 4;
         int gz = t2 * T + lz;
-        while (gz >= M) gz -= M;
-        for (int row = wid * rpi + sub; row < E * E; row += nw * rpi) {
+        gz -= gz >= M ? M : 0;
+        for (int row = wid * 2 + sub; row < E * E; row += nw * 2) {
             const int ix = row / E, iy = row - ix * E;
             int gx = t0 * T + ix, gy = t1 * T + iy;
-            while (gx >= M) gx -= M;
-            while (gy >= M) gy -= M;
+            gx -= gx >= M ? M : 0;
+            gy -= gy >= M ? M : 0;
             if (lz < E) {
-                const size_t o = ((size_t)gx * M + gy) * M + gz;
-                const int idx = row * Ez + lz;
-                // asynchronous 4-byte copies global -> shared (cp.async, LDGSTS): all rows of the block are in flight
-                // at once instead of one L2 round trip per row; planes the caller did not ask for are zero-filled
-                float *dlo = reinterpret_cast<float *>(lo + idx), *dhi = reinterpret_cast<float *>(hi + idx);
-                if (mode & PSE_OUT_U) {
-                    __pipeline_memcpy_async(dlo, grid + o, 4); __pipeline_memcpy_async(dlo + 1, grid + M3 + o, 4);
-                    __pipeline_memcpy_async(dlo + 2, grid + 2 * M3 + o, 4);
-                } else { dlo[0] = 0.f; dlo[1] = 0.f; dlo[2] = 0.f; }
-                if (mode & PSE_OUT_E) {
-                    __pipeline_memcpy_async(dlo + 3, grid + 3 * M3 + o, 4);
-                    __pipeline_memcpy_async(dhi, grid + 4 * M3 + o, 4); __pipeline_memcpy_async(dhi + 1, grid + 5 * M3 + o, 4);
-                    __pipeline_memcpy_async(dhi + 2, grid + 6 * M3 + o, 4); __pipeline_memcpy_async(dhi + 3, grid + 7 * M3 + o, 4);
-                } else { dlo[3] = 0.f; hi[idx] = make_float4(0.f, 0.f, 0.f, 0.f); }
+                const float *src = grid + C0 * M3 + ((size_t)gx * M + gy) * M + gz;
+                float *dst = sm + row * EP + lz;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) __pipeline_memcpy_async(dst + c * PL, src + c * M3, 4);
             }
         }
         __pipeline_commit();
         __pipeline_wait_prior(0);
+        __syncthreads();
     }
-    __syncthreads();
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    const int P2 = P * P, EE = E * Ez;
-    float *outf = reinterpret_cast<float *>(out);
-    // Eight lanes per particle, four particles per warp.  A lane owns the (j,k) columns jk = gl, gl + 8, ... of the
-    // support and walks each along x: two 16-byte shared loads and 8 FMAs per point, the x weights in registers.  The
-    // fixed cost per particle (support base, weights, reduction, read-modify-write) is paid by 8 lanes instead of 32,
-    // and the 8-lane reduction leaves component gl in lane gl: one 32-byte store per particle.
-    constexpr int NP = PT ? PT : PSE_MAXP;
-    const int gl = lane & 7, grp = lane >> 3, gbase = lane & 24;
-    const bool mine = mode & (gl < 3 ? PSE_OUT_U : PSE_OUT_E);
+    const int gl = lane & 7, grp = lane >> 3;
     for (int pi0 = wid * 4; pi0 < np; pi0 += nw * 4) {                  // uniform over the warp (shuffles inside)
         const int pi = pi0 + grp;
         const bool live = pi < np;
-        const int s = live ? tile_list[first + pi] : 0;
-        const float4 p = pos[s];
-        const float prev = (live && mine && accumulate) ? outf[(size_t)s * 8 + gl] : 0.f;       // read-modify-write operand early
-        const float gx = p.x * inv_h, gy = p.y * inv_h, gz = p.z * inv_h;
-        const int b0 = support_base(gx, P), b1 = support_base(gy, P), b2 = support_base(gz, P);
-        const int r0 = pmod(b0, M) - t0 * T, r1 = pmod(b1, M) - t1 * T, r2 = pmod(b2, M) - t2 * T;
-        // x weights: lane gl evaluates i = gl (and gl + 8 for supports wider than 8), the group shares them by shuffle
-        const float wxa = gl < P ? __expf(win_arg((float)(b0 + gl) - gx, wa, wb)) : 0.f;
-        const float wxb = (NP > 8 && gl + 8 < P) ? __expf(win_arg((float)(b0 + gl + 8) - gx, wa, wb)) : 0.f;
-        float wx[NP];
+        const int s = tile_list[first + (live ? pi : 0)];
+        const int b = pbase[s];
+        const bool mine = gl >= C0 && gl < C0 + NC;
+        const float prev = (live && mine && accumulate) ? out[(size_t)s * 8 + gl] : 0.f;         // read-modify-write operand early
+        const int r0 = (b & 1023) - t0 * T, r1 = ((b >> 10) & 1023) - t1 * T, r2 = ((b >> 20) & 1023) - t2 * T;   // 0..7: binned by base
+        const float *wrow = pw + (size_t)s * 3 * PP;
+        float wx[P];
 #pragma unroll
-        for (int i = 0; i < NP; ++i) wx[i] = __shfl_sync(0xffffffffu, i < 8 ? wxa : wxb, gbase + (i & 7));
-        float acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        const int ncol = live ? P2 : 0;
-        for (int jk = gl; jk < ncol; jk += 8) {
-            const int j = jk / P, k = jk - j * P;
-            const float wyz = __expf(win_arg((float)(b1 + j) - gy, wa, wb) + win_arg((float)(b2 + k) - gz, wa, wb));
-            int sidx = (r0 * E + r1 + j) * Ez + r2 + k;
-            float tsum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#pragma unroll
-            for (int i = 0; i < NP; ++i) {
-                if (i >= P) break;
-                const float4 v0 = lo[sidx], v1 = hi[sidx];
-                tsum[0] += wx[i] * v0.x; tsum[1] += wx[i] * v0.y; tsum[2] += wx[i] * v0.z; tsum[3] += wx[i] * v0.w;
-                tsum[4] += wx[i] * v1.x; tsum[5] += wx[i] * v1.y; tsum[6] += wx[i] * v1.z; tsum[7] += wx[i] * v1.w;
-                sidx += EE;
-            }
-#pragma unroll
-            for (int c = 0; c < 8; ++c) acc[c] += wyz * tsum[c];
+        for (int i4 = 0; i4 < PP / 4; ++i4) {
+            const float4 v = reinterpret_cast<const float4 *>(wrow)[i4];
+            if (4 * i4 < P) wx[4 * i4] = v.x;
+            if (4 * i4 + 1 < P) wx[4 * i4 + 1] = v.y;
+            if (4 * i4 + 2 < P) wx[4 * i4 + 2] = v.z;
+            if (4 * i4 + 3 < P) wx[4 * i4 + 3] = v.w;
         }
+        float acc[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[c] = 0.f;
+        if (live) {
+#pragma unroll
+            for (int jk = gl; jk < P * P; jk += 8) {                   // jk - gl is a compile-time constant: j, k from one division
+                const int j = jk / P, k = jk - j * P;
+                const float wyz = wrow[PP + j] * wrow[2 * PP + k];
+                const float *col = sm + (r0 * E + r1 + j) * EP + r2 + k;
+                float ts[NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) ts[c] = 0.f;
+#pragma unroll
+                for (int i = 0; i < P; ++i)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) ts[c] += wx[i] * col[c * PL + i * EE];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] += wyz * ts[c];
+            }
+        }
+        float full[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) full[c] = (c >= C0 && c < C0 + NC) ? acc[c - C0] : 0.f;
         // 8 sums over 8 lanes in 4 + 2 + 1 shuffles: every step halves the values a lane carries
         const bool h4 = gl & 4, h2 = gl & 2, h1 = gl & 1;
         float r4[4], r2s[2];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) r4[c] = (h4 ? acc[c + 4] : acc[c]) + __shfl_xor_sync(0xffffffffu, h4 ? acc[c] : acc[c + 4], 4);
+        for (int c = 0; c < 4; ++c) r4[c] = (h4 ? full[c + 4] : full[c]) + __shfl_xor_sync(0xffffffffu, h4 ? full[c] : full[c + 4], 4);
 #pragma unroll
         for (int c = 0; c < 2; ++c) r2s[c] = (h2 ? r4[c + 2] : r4[c]) + __shfl_xor_sync(0xffffffffu, h2 ? r4[c] : r4[c + 2], 2);
         const float r = (h1 ? r2s[1] : r2s[0]) + __shfl_xor_sync(0xffffffffu, h1 ? r2s[0] : r2s[1], 1);
-        if (live && mine) outf[(size_t)s * 8 + gl] = r + prev;
+        if (live && mine) out[(size_t)s * 8 + gl] = r + prev;
     }
 }
 
@@ -415,6 +632,51 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
 
 }  // namespace
 
+template <int PT, int C0, int NC>
+static pse_status launch_interp_planes(pse_ctx *c, float *d_out, bool accumulate) {
+    const size_t smem = (size_t)NC * InterpGeom<PT>::PL * sizeof(float);
+    interp_planes_kernel<PT, C0, NC><<<c->ntile, 256, smem, c->stream>>>(c->tmap_grid[PT], c->d_pbase, c->d_pw, c->d_tile_start, c->d_tile_list, c->d_grid,
+                                                                        d_out, c->M, c->nt, accumulate ? 1 : 0, c->tma_ok ? 1 : 0);
+    return PSE_OK;
+}
+template <int PT>
+static pse_status launch_interp(pse_ctx *c, int oplan, float *d_out, bool accumulate) {
+    return oplan == 3 ? launch_interp_planes<PT, 0, 8>(c, d_out, accumulate)
+         : oplan == 1 ? launch_interp_planes<PT, 0, 3>(c, d_out, accumulate) : launch_interp_planes<PT, 3, 5>(c, d_out, accumulate);
+}
+
+// dynamic shared-memory opt-in of the interpolation kernels and the TMA descriptor of the grid array for this context's P
+template <int PT>
+static pse_status init_interp(pse_ctx *c) {
+#define PSE_INTERP_ATTR(C0, NC) CUDA_TRY(c, cudaFuncSetAttribute(interp_planes_kernel<PT, C0, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                                                 (int)((size_t)NC * InterpGeom<PT>::PL * sizeof(float))))
+    PSE_INTERP_ATTR(0, 8); PSE_INTERP_ATTR(0, 3); PSE_INTERP_ATTR(3, 5);
+#undef PSE_INTERP_ATTR
+    c->tma_ok = false;
+    if (c->M % 4 != 0) return PSE_OK;                 // row pitch not a multiple of 16 bytes: TMA cannot address the grid
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+        cudaGetLastError();
+        return PSE_OK;                                // driver without tensor maps: cp.async staging everywhere
+    }
+    const cuuint64_t M = (cuuint64_t)c->M;
+    const cuuint64_t dims[4] = {M, M, M, 8};
+    const cuuint64_t strides[3] = {M * 4, M * M * 4, (cuuint64_t)pse_plane_stride(c->M) * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)InterpGeom<PT>::EP, (cuuint32_t)InterpGeom<PT>::E, (cuuint32_t)InterpGeom<PT>::E, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = ((encode_fn)fn)(&c->tmap_grid[PT], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->d_grid, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    c->tma_ok = (r == CUDA_SUCCESS);
+    return PSE_OK;
+}
+
+// the block-owning spread serves supports up to 8 points on grids of at least two tiles per dimension; anything else takes
+// the generic gather kernel
+static bool use_block_spread(const pse_ctx *c) { return c->P <= 8 && c->P != 7 && c->M >= 2 * T && c->M >= 2 * c->P; }
+
 pse_status pse_wave_init(pse_ctx *c) {
     const int M = c->M;
     c->Mh = M / 2 + 1;
@@ -425,6 +687,35 @@ pse_status pse_wave_init(pse_ctx *c) {
     CUDA_TRY(c, cudaMalloc(&c->d_tile_start, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
+    switch (c->P) {
+        case 2: PSE_TRY(init_interp<2>(c)); break;
+        case 3: PSE_TRY(init_interp<3>(c)); break;
+        case 4: PSE_TRY(init_interp<4>(c)); break;
+        case 5: PSE_TRY(init_interp<5>(c)); break;
+        case 6: PSE_TRY(init_interp<6>(c)); break;
+        case 7: PSE_TRY(init_interp<7>(c)); break;
+        case 8: PSE_TRY(init_interp<8>(c)); break;
+        default: break;
+    }
+    c->PP = (c->P + 3) & ~3;
+    CUDA_TRY(c, cudaMalloc(&c->d_pbase, (size_t)c->N * sizeof(int)));
+    CUDA_TRY(c, cudaMalloc(&c->d_pw, (size_t)c->N * 3 * c->PP * sizeof(float)));
+    if (use_block_spread(c)) {
+        // exact bound of the halves one particle can reach for this (P, M): units touched per dimension, maximised over the base
+        auto max_units = [&](int UW) {
+            int best = 1;
+            for (int b = 0; b < M; ++b) {
+                int u[4], n = 0;
+                for (int i = 0; i < c->P; ++i) { const int unit = ((b + i) % M) / UW; bool seen = false; for (int q = 0; q < n; ++q) seen |= u[q] == unit; if (!seen && n < 4) u[n++] = unit; }
+                best = std::max(best, n);
+            }
+            return best;
+        };
+        const int my = max_units(T);
+        c->half_cap = (size_t)c->N * max_units(T / 2) * my * my;
+        CUDA_TRY(c, cudaMalloc(&c->d_half_start, (size_t)(2 * c->ntile + 1) * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&c->d_half_list, c->half_cap * sizeof(int)));
+    }
     int n[3] = {M, M, M};
     const int batches[3] = {8, 3, 5};                 // all grids | planes 0-2 (F in, U out) | planes 3-7 (S in, E out)
     size_t w = 0;
@@ -453,13 +744,34 @@ pse_status pse_wave_init(pse_ctx *c) {
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
-    cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list);
+    cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list); cudaFree(c->d_pbase); cudaFree(c->d_pw);
+    cudaFree(c->d_half_start); cudaFree(c->d_half_list);
 }
 
 // Tile bins: counted in wrap_and_bin, scanned with the cell counts, scattered in gather_positions (neighbors.cu);
 // what is left is the deterministic order inside every tile.
 pse_status pse_tile_bins(pse_ctx *c) {
     return pse_rank_sort(c, c->d_tile_start, c->ntile, c->d_tile_tmp, c->d_tile_list);
+}
+
+pse_status pse_particle_windows(pse_ctx *c) {
+    particle_window_kernel<<<(c->N + 255) / 256, 256, 0, c->stream>>>(c->d_pos, c->N, c->M, c->P, c->PP, (float)(1.0 / c->h), (float)c->win_a,
+                                                                     (float)c->win_b, c->d_pbase, c->d_pw);
+    KERNEL_CHECK(c);
+    if (!use_block_spread(c)) return PSE_OK;
+    // lists of the particles that reach every half tile: count, scan, write
+    const int nhalf = 2 * c->ntile, nbk = (nhalf + 3) / 4;
+    half_lists_kernel<false><<<nbk, 128, 0, c->stream>>>(c->d_pbase, c->d_tile_start, c->d_tile_list, c->M, c->P, c->nt, nhalf, c->d_half_count, nullptr, nullptr); KERNEL_CHECK(c);
+    PSE_TRY(pse_scan_i32(c, c->d_half_count, c->d_half_start, (size_t)nhalf));
+    half_lists_kernel<true><<<nbk, 128, 0, c->stream>>>(c->d_pbase, c->d_tile_start, c->d_tile_list, c->M, c->P, c->nt, nhalf, nullptr, c->d_half_start, c->d_half_list); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
+template <int P>
+static void launch_spread_blocks(pse_ctx *c, int plan, const float4 *in4) {
+    if (plan == 0) spread_blocks_kernel<P, 0, 8><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
+    else if (plan == 1) spread_blocks_kernel<P, 0, 3><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
+    else spread_blocks_kernel<P, 3, 5><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
 }
 
 // plane range of a 2-bit component mask (bit 0: planes 0-2, bit 1: planes 3-7): plan index and first plane
@@ -476,31 +788,17 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
         CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++;
     }
     ScopedPhase ph(c, PSE_T_INTERP);
-    const int TB = 256, E = T + c->P - 1;
-    const int Ez = E + ((c->P - E) & 7);
-    const size_t smem = (size_t)2 * E * E * Ez * sizeof(float4);
-    if (smem <= 200 * 1024) {
-#define PSE_LAUNCH_INTERP(PT)                                                                                              \
-    do {                                                                                                                   \
-        static size_t smem_set = 0;                                                                                        \
-        if (smem > smem_set) {                                                                                             \
-            CUDA_TRY(c, cudaFuncSetAttribute(interp_tile_kernel<PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-            smem_set = smem;                                                                                               \
-        }                                                                                                                  \
-        interp_tile_kernel<PT><<<c->ntile, TB, smem, c->stream>>>(c->d_pos, c->d_tile_start, c->d_tile_list, c->d_grid,       \
-            reinterpret_cast<float4 *>(d_out), c->M, c->P, c->nt, (float)(1.0 / c->h), (float)c->win_a, (float)c->win_b, \
-            accumulate ? 1 : 0, mode);                                                                                     \
-    } while (0)
+    const int TB = 256, oplan = (mode >> 2) & 3;
+    if (c->P <= 8) {
         switch (c->P) {
-            case 3: PSE_LAUNCH_INTERP(3); break;
-            case 4: PSE_LAUNCH_INTERP(4); break;
-            case 5: PSE_LAUNCH_INTERP(5); break;
-            case 6: PSE_LAUNCH_INTERP(6); break;
-            case 7: PSE_LAUNCH_INTERP(7); break;
-            case 8: PSE_LAUNCH_INTERP(8); break;
-            default: PSE_LAUNCH_INTERP(0); break;
+            case 2: PSE_TRY(launch_interp<2>(c, oplan, d_out, accumulate)); break;
+            case 3: PSE_TRY(launch_interp<3>(c, oplan, d_out, accumulate)); break;
+            case 4: PSE_TRY(launch_interp<4>(c, oplan, d_out, accumulate)); break;
+            case 5: PSE_TRY(launch_interp<5>(c, oplan, d_out, accumulate)); break;
+            case 6: PSE_TRY(launch_interp<6>(c, oplan, d_out, accumulate)); break;
+            case 7: PSE_TRY(launch_interp<7>(c, oplan, d_out, accumulate)); break;
+            default: PSE_TRY(launch_interp<8>(c, oplan, d_out, accumulate)); break;
         }
-#undef PSE_LAUNCH_INTERP
     } else {
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
@@ -519,7 +817,16 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
         ScopedPhase ph(c, PSE_T_SPREAD);
         const float4 *in4 = reinterpret_cast<const float4 *>(d_in);
         const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
-        if (plan == 0) spread_kernel<0, 8><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
+        if (use_block_spread(c)) {
+            switch (c->P) {
+                case 2: launch_spread_blocks<2>(c, plan, in4); break;
+                case 3: launch_spread_blocks<3>(c, plan, in4); break;
+                case 4: launch_spread_blocks<4>(c, plan, in4); break;
+                case 5: launch_spread_blocks<5>(c, plan, in4); break;
+                case 6: launch_spread_blocks<6>(c, plan, in4); break;
+                default: launch_spread_blocks<8>(c, plan, in4); break;
+            }
+        } else if (plan == 0) spread_kernel<0, 8><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         else if (plan == 1) spread_kernel<0, 3><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
         KERNEL_CHECK(c);
