@@ -154,11 +154,11 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
-    c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1) + (size_t)(2 * c->ntile + 1);
+    c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1) + 1;
     CUDA_TRY(c, cudaMalloc(&c->d_bins, c->bins_n * sizeof(int)));
     c->d_cell_count = c->d_bins; c->d_cell_fill = c->d_cell_count + c->ncell + 1;
     c->d_tile_count = c->d_cell_fill + c->ncell + 1; c->d_tile_fill = c->d_tile_count + c->ntile + 1;
-    c->d_half_count = c->d_tile_fill + c->ntile + 1;
+    c->d_half_cursor = c->d_tile_fill + c->ntile + 1;
     {
         std::vector<float> dec;
         pse_window_table(c->win_kind, P, c->win_a, c->win_b, grid, dec);

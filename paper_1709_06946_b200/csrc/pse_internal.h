@@ -47,7 +47,7 @@ struct pse_ctx {
     int *d_order = nullptr;                  // [N] sorted -> original
     int *d_order_tmp = nullptr, *d_tile_tmp = nullptr;   // [N] unsorted scatter targets
     int *d_cell_of = nullptr;                // [N] cell of original particle
-    int *d_bins = nullptr; size_t bins_n = 0;   // one block cleared by a single memset: cell_count | cell_fill | tile_count | tile_fill | half_count
+    int *d_bins = nullptr; size_t bins_n = 0;   // one block cleared by a single memset: cell_count | cell_fill | tile_count | tile_fill | half_cursor
     int *d_cell_count = nullptr, *d_cell_start = nullptr, *d_cell_fill = nullptr;   // [ncell+1]; count and fill point into d_bins
     int *d_nbr_count = nullptr;              // [N]
     unsigned long long *d_nbr_off = nullptr; // [N+1]
@@ -63,12 +63,12 @@ struct pse_ctx {
     int *d_tile_list = nullptr;              // [N] sorted-particle indices grouped by tile
     // ---- per-particle window data, computed once per pse_neighbors and shared by every spread / interpolation of that
     //      configuration (a step runs ~25 of them on two configurations) ----
-    int *d_pbase = nullptr;                  // [N] wrapped support base, packed bx | by << 10 | bz << 20 (sorted numbering)
-    float *d_pw = nullptr;                   // [N][3][PP] window values at the P support points per dimension, PP = P rounded up to 4
+    int *d_pbase = nullptr;                  // [N] wrapped support base, packed bx | by << 10 | bz << 20; TILE ORDER: entry i is particle d_tile_list[i]
+    float *d_pw = nullptr;                   // [N][3][PP] (tile order) window values at the P support points per dimension, PP = P rounded up to 4
     int PP = 0;
     // particles that reach each half tile (4 x 8 x 8 grid points, one warp of the spread kernel): CSR, built in pse_neighbors
-    int *d_half_count = nullptr;             // [2 ntile + 1], inside d_bins
-    int *d_half_start = nullptr, *d_half_list = nullptr;
+    int *d_half_cursor = nullptr;            // allocation cursor of d_half_list, inside d_bins (cleared by its memset)
+    int *d_half_start = nullptr, *d_half_count = nullptr, *d_half_list = nullptr;   // [2 ntile] segment start / length; entries = tile-order indices
     size_t half_cap = 0;
     // ---- grids ----
     float *d_grid = nullptr;                 // [8][M][M][M]

@@ -216,80 +216,91 @@ spread_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, con
 
 // ---- per-particle window data -------------------------------------------------------------------------------------------
 // Positions are fixed between two pse_neighbors calls while ~25 spreads / interpolations run on them, so the P window values
-// per dimension (a sqrt and an exp each for the default window) and the wrapped support base are computed once here.
-__global__ void particle_window_kernel(const float4 *__restrict__ pos, int N, int M, int P, int PP, float inv_h, float wa, float wb,
-                                       int *__restrict__ pbase, float *__restrict__ pw) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    const float4 p = pos[s];
+// per dimension (a sqrt and an exp each for the default window) and the wrapped support base are computed once here.  Both
+// arrays are in TILE ORDER (entry i belongs to particle tile_list[i]): the particles of a tile bin are contiguous, so spread
+// and interpolation read them without an indirection.
+template <int PP>
+__global__ void particle_window_kernel(const float4 *__restrict__ pos, const int *__restrict__ tile_list, int N, int M, int P, float inv_h,
+                                       float wa, float wb, int *__restrict__ pbase, float4 *__restrict__ pw) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const float4 p = pos[tile_list[i]];
     const float g[3] = {p.x * inv_h, p.y * inv_h, p.z * inv_h};
     int packed = 0;
+#pragma unroll
     for (int d = 0; d < 3; ++d) {
         const int base = support_base(g[d], P);
         packed |= pmod(base, M) << (10 * d);
-        for (int i = 0; i < PP; ++i)
-            pw[((size_t)s * 3 + d) * PP + i] = i < P ? __expf(win_arg((float)(base + i) - g[d], wa, wb)) : 0.f;
+        float v[PP];
+#pragma unroll
+        for (int k = 0; k < PP; ++k) v[k] = k < P ? __expf(win_arg((float)(base + k) - g[d], wa, wb)) : 0.f;
+#pragma unroll
+        for (int k4 = 0; k4 < PP / 4; ++k4) pw[((size_t)i * 3 + d) * (PP / 4) + k4] = make_float4(v[4 * k4], v[4 * k4 + 1], v[4 * k4 + 2], v[4 * k4 + 3]);
     }
-    pbase[s] = packed;
+    pbase[i] = packed;
 }
 
 // ---- lists of the particles that reach each half tile (built once per pse_neighbors, used by every spread) -----------------
 // A "half" is the 4 x 8 x 8 block of grid points one warp of the spread kernel owns: half index = (tile index) * 2 + (x half).
-// One warp per half walks the particles binned in the tiles that can reach it (two per dimension, three next to a partial last
-// tile), 32 at a time, keeps those whose support overlaps the half and appends them in candidate order with a ballot: no
-// atomics, deterministic.  WRITE = false counts (the offsets come from a scan in between), WRITE = true writes.
-template <bool WRITE>
-__global__ void __launch_bounds__(128)
-half_lists_kernel(const int *__restrict__ pbase, const int *__restrict__ tile_start, const int *__restrict__ tile_list, int M, int P, int nt,
-                  int nhalf, int *__restrict__ half_count, const int *__restrict__ half_start, int *__restrict__ half_list) {
-    __shared__ int s_lo[4][32], s_cum[4][33], s_reach[4][3][4], s_nreach[4][3];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, h = blockIdx.x * 4 + w;
+// One warp per half walks the tile bins that can reach it (two per dimension, three next to a partial last tile), 32 entries
+// at a time, keeps the particles whose support overlaps the half and collects them in bin order with a ballot (no atomics per
+// particle, deterministic content).  The warp then reserves its segment of the list array with ONE atomicAdd on a cursor (the
+// placement of whole segments depends on scheduling, which no consumer sees: they go through half_start / half_count) and
+// copies the collected entries out.  Entries are tile-order indices (see particle_window_kernel).
+constexpr int HL_WARPS = 4, HL_CAP = 512;
+
+__global__ void __launch_bounds__(HL_WARPS * 32)
+half_lists_kernel(const int *__restrict__ pbase, const int *__restrict__ tile_start, int M, int P, int nt, int nhalf,
+                  int *__restrict__ half_start, int *__restrict__ half_count, int *__restrict__ half_list, int *__restrict__ cursor) {
+    __shared__ int s_hits[HL_WARPS][HL_CAP];
+    __shared__ int s_reach[HL_WARPS][3][4], s_nreach[HL_WARPS][3];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, h = blockIdx.x * HL_WARPS + w;
     if (h >= nhalf) return;
     const int t = h >> 1, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int lo[3] = {t0 * T + 4 * (h & 1), t1 * T, t2 * T};
     if (lane < 3) s_nreach[w][lane] = reach_tiles(lane == 0 ? t0 : (lane == 1 ? t1 : t2), M, P, nt, s_reach[w][lane]);
     __syncwarp();
-    const int ny = s_nreach[w][1], nz = s_nreach[w][2], n = s_nreach[w][0] * ny * nz;      // n <= 27 for P <= 8
-    int cnt = 0, first = 0;
-    if (lane < n) {
-        const int i = lane / (ny * nz), j = (lane / nz) % ny, k = lane % nz;
-        const int tb = (s_reach[w][0][i] * nt + s_reach[w][1][j]) * nt + s_reach[w][2][k];
-        first = tile_start[tb];
-        cnt = tile_start[tb + 1] - first;
-    }
-    int inc = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-    s_lo[w][lane] = first; s_cum[w][lane + 1] = inc;
-    if (lane == 0) s_cum[w][0] = 0;
-    const int total = __shfl_sync(0xffffffffu, inc, 31);
-    __syncwarp();
+    const int nx = s_nreach[w][0], ny = s_nreach[w][1], nz = s_nreach[w][2];
     const int halfM = M >> 1;
-    int found = 0;
-    int *dst = WRITE ? half_list + half_start[h] : nullptr;
-    for (int c0 = 0; c0 < total; c0 += 32) {
-        const int ci = c0 + lane;
-        bool hit = false;
-        int s = 0;
-        if (ci < total) {
-            int k = 0;
-            for (int q = 1; q < n; ++q) k += (s_cum[w][q] <= ci);
-            s = tile_list[s_lo[w][k] + ci - s_cum[w][k]];
-            const int b = pbase[s];
-            hit = true;
+    int found = 0, base_out = 0;
+    // pass 0 collects in shared memory (and counts); only if the half holds more than HL_CAP particles a second pass writes the rest
+    for (int pass = 0; pass < 2; ++pass) {
+        int seen = 0;
+        for (int bi = 0; bi < nx * ny * nz; ++bi) {
+            const int i = bi / (ny * nz), j = (bi / nz) % ny, k = bi % nz;
+            const int tb = (s_reach[w][0][i] * nt + s_reach[w][1][j]) * nt + s_reach[w][2][k];
+            const int first = tile_start[tb], cnt = tile_start[tb + 1] - first;
+            for (int c0 = 0; c0 < cnt; c0 += 32) {
+                const int e = first + c0 + lane;
+                bool hit = c0 + lane < cnt;
+                if (hit) {
+                    const int b = pbase[e];
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                int so = lo[d] - ((b >> (10 * d)) & 1023);                  // offset of the half's origin from the support base
-                so += so < -halfM ? M : 0;
-                so -= so > halfM ? M : 0;
-                hit = hit && so > -(d == 0 ? 4 : 8) && so < P;
+                    for (int d = 0; d < 3; ++d) {
+                        int so = lo[d] - ((b >> (10 * d)) & 1023);                  // offset of the half's origin from the support base
+                        so += so < -halfM ? M : 0;
+                        so -= so > halfM ? M : 0;
+                        hit = hit && so > -(d == 0 ? 4 : 8) && so < P;
+                    }
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, hit);
+                const int at = seen + __popc(bal & ((1u << lane) - 1u));
+                if (hit) {
+                    if (pass == 0) { if (at < HL_CAP) s_hits[w][at] = e; }
+                    else if (at >= HL_CAP) half_list[base_out + at] = e;
+                }
+                seen += __popc(bal);
             }
         }
-        const unsigned bal = __ballot_sync(0xffffffffu, hit);
-        if (WRITE && hit) dst[found + __popc(bal & ((1u << lane) - 1u))] = s;
-        found += __popc(bal);
+        if (pass == 0) {
+            found = seen;
+            if (lane == 0) { base_out = atomicAdd(cursor, found); half_start[h] = base_out; half_count[h] = found; }
+            base_out = __shfl_sync(0xffffffffu, base_out, 0);
+            __syncwarp();
+            for (int q = lane; q < min(found, HL_CAP); q += 32) half_list[base_out + q] = s_hits[w][q];
+            if (found <= HL_CAP) break;
+        }
     }
-    if (!WRITE && lane == 0) half_count[h] = found;
 }
 
 // ---- spread (a3), default path for P <= 8 ---------------------------------------------------------------------------------
@@ -305,17 +316,18 @@ half_lists_kernel(const int *__restrict__ pbase, const int *__restrict__ tile_st
 // No atomics, no memset, each grid value written once (8-byte stores), summation in list order (deterministic).
 template <int P, int C0, int NC>
 __global__ void __launch_bounds__(64)
-spread_blocks_kernel(const int *__restrict__ pbase, const float *__restrict__ pw, const float4 *__restrict__ in,
-                     const int *__restrict__ half_start, const int *__restrict__ half_list, float *__restrict__ grid, int M, int nt) {
-    constexpr int CAP = 64, PP = (P + 3) & ~3, WR = P + 2;
-    __shared__ __align__(16) unsigned s_code[2][CAP];
+spread_blocks_kernel(const int *__restrict__ pbase, const float *__restrict__ pw, const int *__restrict__ tile_list, const float4 *__restrict__ in,
+                     const int *__restrict__ half_start, const int *__restrict__ half_count, const int *__restrict__ half_list,
+                     float *__restrict__ grid, int M, int nt) {
+    constexpr int CAP = 64, PP = (P + 3) & ~3, WR = P + 2, WROW = (3 * WR) | 1, QROW = 3;     // odd row pitch (words) / 48-byte rows:
+    __shared__ __align__(16) unsigned s_code[2][CAP];                                         // lanes on different rows, different banks
     __shared__ unsigned s_off[2][CAP];
-    __shared__ float4 s_q[2][CAP][2];
-    __shared__ float s_w[2][CAP][3 * WR];
+    __shared__ float4 s_q[2][CAP][QROW];
+    __shared__ float s_w[2][CAP][WROW];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int t = blockIdx.x, t0 = t / (nt * nt), t1 = (t / nt) % nt, t2 = t % nt;
     const int lo[3] = {t0 * T + 4 * w, t1 * T, t2 * T};            // origin of the warp's half: 4 x 8 x 8 points
-    const int first = half_start[2 * t + w], total = half_start[2 * t + w + 1] - first;
+    const int first = half_start[2 * t + w], total = half_count[2 * t + w];
     const int rxl = lane >> 4, ryl = (lane >> 2) & 3, rzl = lane & 3;            // my block inside the half: 2 x 4 x 4 blocks
     const unsigned mymask = (1u << rxl) | (1u << (2 + ryl)) | (1u << (6 + rzl));
     const int cx = 2 * rxl + 1 - 16, cy = 2 * ryl + 1 - 16, cz = 2 * rzl + 1 - 16;
@@ -332,8 +344,8 @@ spread_blocks_kernel(const int *__restrict__ pbase, const float *__restrict__ pw
         for (int pass = 0; pass < CAP / 32; ++pass) {
             const int slot = pass * 32 + lane;
             if (slot < nb) {
-                const int s = half_list[first + c0 + slot];
-                const int b = pbase[s];
+                const int e = half_list[first + c0 + slot];          // tile-order index: window data contiguous per tile
+                const int b = pbase[e], s = tile_list[e];
                 unsigned code = 0, off = 0;
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
@@ -347,7 +359,7 @@ spread_blocks_kernel(const int *__restrict__ pbase, const float *__restrict__ pw
                 }
                 s_code[w][slot] = code; s_off[w][slot] = off;
                 s_q[w][slot][0] = in[2 * s]; s_q[w][slot][1] = in[2 * s + 1];
-                const float4 *src = reinterpret_cast<const float4 *>(pw + (size_t)s * 3 * PP);
+                const float4 *src = reinterpret_cast<const float4 *>(pw + (size_t)e * 3 * PP);
                 float *dst = s_w[w][slot];
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
@@ -489,6 +501,7 @@ interp_planes_kernel(const __grid_constant__ CUtensorMap tmap, const int *__rest
     if (np == 0) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const bool seam = t0 * T + E > M || t1 * T + E > M || t2 * T + E > M;
+    bool staged = !(use_tma && !seam);             // TMA path: every thread waits on the mbarrier itself, after its own first loads
     if (use_tma && !seam) {
         if (threadIdx.x == 0) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar)));
@@ -503,10 +516,6 @@ interp_planes_kernel(const __grid_constant__ CUtensorMap tmap, const int *__rest
                              ::"r"(smem_u32(sm + c * PL)), "l"(&tmap), "r"(t2 * T), "r"(t1 * T), "r"(t0 * T), "r"(C0 + c), "r"(smem_u32(&bar))
                              : "memory");
         }
-        unsigned done = 0;
-        while (!done)
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                         : "=r"(done) : "r"(smem_u32(&bar)) : "memory");
     } else {
         const size_t M3 = pse_plane_stride(M);
         // a half-warp (E <= 16) per (ix,iy) row, lanes along z; wrap by subtraction; all copies in flight at once
@@ -533,12 +542,13 @@ interp_planes_kernel(const __grid_constant__ CUtensorMap tmap, const int *__rest
     for (int pi0 = wid * 4; pi0 < np; pi0 += nw * 4) {                  // uniform over the warp (shuffles inside)
         const int pi = pi0 + grp;
         const bool live = pi < np;
-        const int s = tile_list[first + (live ? pi : 0)];
-        const int b = pbase[s];
+        const int e = first + (live ? pi : 0);                          // tile-order index: base and window rows are contiguous per tile
+        const int b = pbase[e];
+        const int s = tile_list[e];
         const bool mine = gl >= C0 && gl < C0 + NC;
         const float prev = (live && mine && accumulate) ? out[(size_t)s * 8 + gl] : 0.f;         // read-modify-write operand early
         const int r0 = (b & 1023) - t0 * T, r1 = ((b >> 10) & 1023) - t1 * T, r2 = ((b >> 20) & 1023) - t2 * T;   // 0..7: binned by base
-        const float *wrow = pw + (size_t)s * 3 * PP;
+        const float *wrow = pw + (size_t)e * 3 * PP;
         float wx[P];
 #pragma unroll
         for (int i4 = 0; i4 < PP / 4; ++i4) {
@@ -548,24 +558,41 @@ interp_planes_kernel(const __grid_constant__ CUtensorMap tmap, const int *__rest
             if (4 * i4 + 2 < P) wx[4 * i4 + 2] = v.z;
             if (4 * i4 + 3 < P) wx[4 * i4 + 3] = v.w;
         }
+        // the window products of this lane's columns, before the staged block is needed
+        constexpr int NCOL = (P * P + 7) / 8;
+        float wyz[NCOL];
+#pragma unroll
+        for (int m = 0; m < NCOL; ++m) {
+            const int jk = gl + 8 * m, j = jk / P, k = jk - j * P;
+            wyz[m] = jk < P * P ? wrow[PP + j] * wrow[2 * PP + k] : 0.f;
+        }
+        if (!staged) {                                                  // first pass of the TMA path: the loads above are in flight
+            unsigned done = 0;
+            while (!done)
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(done) : "r"(smem_u32(&bar)) : "memory");
+            staged = true;
+        }
         float acc[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[c] = 0.f;
         if (live) {
 #pragma unroll
-            for (int jk = gl; jk < P * P; jk += 8) {                   // jk - gl is a compile-time constant: j, k from one division
-                const int j = jk / P, k = jk - j * P;
-                const float wyz = wrow[PP + j] * wrow[2 * PP + k];
-                const float *col = sm + (r0 * E + r1 + j) * EP + r2 + k;
-                float ts[NC];
+            for (int m = 0; m < NCOL; ++m) {
+                const int jk = gl + 8 * m;
+                if (jk < P * P) {
+                    const int j = jk / P, k = jk - j * P;
+                    const float *col = sm + (r0 * E + r1 + j) * EP + r2 + k;
+                    float ts[NC];
 #pragma unroll
-                for (int c = 0; c < NC; ++c) ts[c] = 0.f;
+                    for (int c = 0; c < NC; ++c) ts[c] = 0.f;
 #pragma unroll
-                for (int i = 0; i < P; ++i)
+                    for (int i = 0; i < P; ++i)
 #pragma unroll
-                    for (int c = 0; c < NC; ++c) ts[c] += wx[i] * col[c * PL + i * EE];
+                        for (int c = 0; c < NC; ++c) ts[c] += wx[i] * col[c * PL + i * EE];
 #pragma unroll
-                for (int c = 0; c < NC; ++c) acc[c] += wyz * ts[c];
+                    for (int c = 0; c < NC; ++c) acc[c] += wyz[m] * ts[c];
+                }
             }
         }
         float full[8];
@@ -714,6 +741,7 @@ pse_status pse_wave_init(pse_ctx *c) {
         const int my = max_units(T);
         c->half_cap = (size_t)c->N * max_units(T / 2) * my * my;
         CUDA_TRY(c, cudaMalloc(&c->d_half_start, (size_t)(2 * c->ntile + 1) * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&c->d_half_count, (size_t)(2 * c->ntile + 1) * sizeof(int)));
         CUDA_TRY(c, cudaMalloc(&c->d_half_list, c->half_cap * sizeof(int)));
     }
     int n[3] = {M, M, M};
@@ -745,7 +773,7 @@ void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
     cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list); cudaFree(c->d_pbase); cudaFree(c->d_pw);
-    cudaFree(c->d_half_start); cudaFree(c->d_half_list);
+    cudaFree(c->d_half_start); cudaFree(c->d_half_count); cudaFree(c->d_half_list);
 }
 
 // Tile bins: counted in wrap_and_bin, scanned with the cell counts, scattered in gather_positions (neighbors.cu);
@@ -755,23 +783,31 @@ pse_status pse_tile_bins(pse_ctx *c) {
 }
 
 pse_status pse_particle_windows(pse_ctx *c) {
-    particle_window_kernel<<<(c->N + 255) / 256, 256, 0, c->stream>>>(c->d_pos, c->N, c->M, c->P, c->PP, (float)(1.0 / c->h), (float)c->win_a,
-                                                                     (float)c->win_b, c->d_pbase, c->d_pw);
+    const float4 *pos = c->d_pos;
+    float4 *pw4 = reinterpret_cast<float4 *>(c->d_pw);
+    const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
+    const int nb = (c->N + 127) / 128;
+    switch (c->PP) {
+        case 4: particle_window_kernel<4><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
+        case 8: particle_window_kernel<8><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
+        case 12: particle_window_kernel<12><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
+        default: particle_window_kernel<16><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
+    }
     KERNEL_CHECK(c);
     if (!use_block_spread(c)) return PSE_OK;
-    // lists of the particles that reach every half tile: count, scan, write
-    const int nhalf = 2 * c->ntile, nbk = (nhalf + 3) / 4;
-    half_lists_kernel<false><<<nbk, 128, 0, c->stream>>>(c->d_pbase, c->d_tile_start, c->d_tile_list, c->M, c->P, c->nt, nhalf, c->d_half_count, nullptr, nullptr); KERNEL_CHECK(c);
-    PSE_TRY(pse_scan_i32(c, c->d_half_count, c->d_half_start, (size_t)nhalf));
-    half_lists_kernel<true><<<nbk, 128, 0, c->stream>>>(c->d_pbase, c->d_tile_start, c->d_tile_list, c->M, c->P, c->nt, nhalf, nullptr, c->d_half_start, c->d_half_list); KERNEL_CHECK(c);
+    // lists of the particles that reach every half tile: one pass, segments reserved on a cursor (cleared with the bin counters)
+    const int nhalf = 2 * c->ntile;
+    half_lists_kernel<<<(nhalf + HL_WARPS - 1) / HL_WARPS, HL_WARPS * 32, 0, c->stream>>>(c->d_pbase, c->d_tile_start, c->M, c->P, c->nt, nhalf,
+                                                                                        c->d_half_start, c->d_half_count, c->d_half_list, c->d_half_cursor);
+    KERNEL_CHECK(c);
     return PSE_OK;
 }
 
 template <int P>
 static void launch_spread_blocks(pse_ctx *c, int plan, const float4 *in4) {
-    if (plan == 0) spread_blocks_kernel<P, 0, 8><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
-    else if (plan == 1) spread_blocks_kernel<P, 0, 3><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
-    else spread_blocks_kernel<P, 3, 5><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, in4, c->d_half_start, c->d_half_list, c->d_grid, c->M, c->nt);
+    if (plan == 0) spread_blocks_kernel<P, 0, 8><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, c->d_tile_list, in4, c->d_half_start, c->d_half_count, c->d_half_list, c->d_grid, c->M, c->nt);
+    else if (plan == 1) spread_blocks_kernel<P, 0, 3><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, c->d_tile_list, in4, c->d_half_start, c->d_half_count, c->d_half_list, c->d_grid, c->M, c->nt);
+    else spread_blocks_kernel<P, 3, 5><<<c->ntile, 64, 0, c->stream>>>(c->d_pbase, c->d_pw, c->d_tile_list, in4, c->d_half_start, c->d_half_count, c->d_half_list, c->d_grid, c->M, c->nt);
 }
 
 // plane range of a 2-bit component mask (bit 0: planes 0-2, bit 1: planes 3-7): plan index and first plane
