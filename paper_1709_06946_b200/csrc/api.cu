@@ -44,6 +44,9 @@ int choose_grid(int mmin) {
 
 }  // namespace
 
+// cheapest measured cuFFT size >= mmin (2,3,5,7-smooth beyond the table)
+int pse_choose_grid(int mmin) { return mmin > 64 ? choose_grid(mmin) : [&] { int M = mmin; while (!smooth7(M)) ++M; return M; }(); }
+
 extern "C" {
 
 const char *pse_version(void) { return "libpse 0.1 (sm_100a)"; }
@@ -145,13 +148,15 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_count, (size_t)N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_off, (size_t)(N + 1) * sizeof(unsigned long long)));
     CUDA_TRY(c, cudaMalloc(&c->d_nbr_ctl, 2 * sizeof(unsigned long long)));
-    CUDA_TRY(c, cudaMallocHost(&c->h_nbr_ctl, 2 * sizeof(unsigned long long)));
+    CUDA_TRY(c, cudaMallocHost(&c->h_nbr_ctl, 4 * sizeof(unsigned long long)));
     for (float **p : {&c->d_in, &c->d_out, &c->d_tmp, &c->d_tmp2, &c->d_vecA, &c->d_vecB, &c->d_vecC, &c->d_vecD}) CUDA_TRY(c, cudaMalloc(p, n8));
     c->krylov_cap = PSE_MAX_KRYLOV + 1;
     CUDA_TRY(c, cudaMalloc(&c->d_krylov, (size_t)c->krylov_cap * n8));
     CUDA_TRY(c, cudaMalloc(&c->d_zu, (size_t)PSE_MAX_KRYLOV * n8));
     CUDA_TRY(c, cudaMalloc(&c->d_scal, 2048 * sizeof(double)));
     CUDA_TRY(c, cudaMallocHost(&c->h_scal, 2304 * sizeof(double)));
+    CUDA_TRY(c, cudaMallocHost(&c->h_scal_l, 128 * sizeof(double)));
+    CUDA_TRY(c, cudaMalloc(&c->d_xk, (size_t)N * sizeof(float4)));
     CUDA_TRY(c, cudaMalloc(&c->d_coef, 64 * sizeof(float)));
     PSE_TRY(pse_wave_init(c));
     c->bins_n = 2 * (size_t)(c->ncell + 1) + 2 * (size_t)(c->ntile + 1) + 1;
@@ -164,6 +169,12 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
         pse_window_table(c->win_kind, P, c->win_a, c->win_b, grid, dec);
         CUDA_TRY(c, cudaMalloc(&c->d_dec, dec.size() * sizeof(float)));
         CUDA_TRY(c, cudaMemcpy(c->d_dec, dec.data(), dec.size() * sizeof(float), cudaMemcpyHostToDevice));
+        // the finer grid of the Brownian wave pass, window of Pb = P + 1 points
+        if (c->win_kind == PSE_WINDOW_GAUSS) { c->win_a_b = 2.0 * M_PI / c->Pb; c->win_b_b = 0.0; }
+        else { c->win_a_b = 4.0 / ((double)c->Pb * c->Pb); c->win_b_b = pse_es_beta(c->Pb); }
+        pse_window_table(c->win_kind, c->Pb, c->win_a_b, c->win_b_b, c->Mb, dec);
+        CUDA_TRY(c, cudaMalloc(&c->d_dec_b, dec.size() * sizeof(float)));
+        CUDA_TRY(c, cudaMemcpy(c->d_dec_b, dec.data(), dec.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
@@ -188,9 +199,11 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaFree(c->d_nbr_off); cudaFree(c->d_nbr_idx); cudaFree(c->d_nbr_ctl);
     if (c->h_nbr_ctl) cudaFreeHost(c->h_nbr_ctl);
     for (float *p : {c->d_in, c->d_out, c->d_tmp, c->d_tmp2, c->d_vecA, c->d_vecB, c->d_vecC, c->d_vecD, c->d_krylov, c->d_zu, c->d_coef}) cudaFree(p);
-    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec); cudaFree(c->d_bonds);
+    cudaFree(c->d_scal); cudaFree(c->d_scan_tmp); cudaFree(c->d_dec); cudaFree(c->d_dec_b); cudaFree(c->d_bonds);
     cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);
     if (c->h_scal) cudaFreeHost(c->h_scal);
+    if (c->h_scal_l) cudaFreeHost(c->h_scal_l);
+    cudaFree(c->d_xk);
     delete c;
     return PSE_OK;
 }
@@ -215,12 +228,20 @@ pse_status pse_mobility_apply(pse_ctx *c, const float *d_F, const float *d_S, fl
     return pse_unpack(c, c->d_out, 1.f, d_U, d_E);
 }
 
+static pse_status brownian_impl(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters,
+                                int fixed_m);
+
 pse_status pse_brownian(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters) {
+    return brownian_impl(c, dt, d_noise_real, d_noise_wave, d_UB, d_EB, lanczos_iters, 0);
+}
+
+static pse_status brownian_impl(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters,
+                                int fixed_m) {
     if (!c || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_brownian before pse_neighbors"; return PSE_ENOTREADY; }
     if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
     PSE_TRY(pse_pack8(c, d_noise_real, c->d_in));
-    pse_status st = pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters);
+    pse_status st = pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters, fixed_m);
     if (st != PSE_OK && st != PSE_ENOCONV) return st;
     PSE_TRY(pse_wave_brownian(c, d_noise_wave, c->d_out, true));
     PSE_TRY(pse_unpack(c, c->d_out, (float)std::sqrt(2.0 * c->kT / dt), d_UB, d_EB));
@@ -273,7 +294,46 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     float *UB = c->d_vecD, *EB = c->d_vecD + (size_t)3 * N;           // original numbering: [N][3] then [N][5]
     float4 *xh = reinterpret_cast<float4 *>(c->d_zu);                  // scratch for x_{k+1/2}; d_zu is rewritten by GMRES afterwards
     pse_status soft = PSE_OK;
-    // The neighbour builds are only enqueued; what they report (list size, overflow, oversized cell) is examined after the
+    // ---- optimistic path: once a step has completed, the next one is enqueued WHOLE with the iteration counts that one needed
+    // (fixed-count Lanczos and GMRES, their small algebra on the device), the host synchronises once at the end and only then
+    // looks at what the two neighbour builds and the two solves report.  If anything is off (list overflow, a solve that needed
+    // more iterations) x_k is restored and the step is redone by the checked path below, which also re-learns the counts. ----
+    if (c->lanczos_budget > 0 && c->gmres_budget > 0) {
+        const int mL = c->lanczos_budget, mG = c->gmres_budget;
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_xk, d_pos, (size_t)N * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+        PSE_TRY(pse_neighbors_impl(c, d_pos));
+        const int slot0 = c->nbr_last;
+        const bool single0 = c->nbr_pending;                         // false: the context takes the synchronous two-pass build
+        PSE_TRY(brownian_impl(c, dt, d_noise_real, d_noise_wave, UB, EB, nullptr, mL));
+        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+        PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
+        PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+        if (c->n_bonds) {
+            PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
+            PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
+            PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+        }
+        PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
+        PSE_TRY(pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, nullptr, mG));
+        PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));
+        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
+                                            reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        bool redo0 = false, redo1 = false, shrinkL = false, shrinkG = false;
+        if (single0) PSE_TRY(pse_neighbors_examine(c, slot0, &redo0));
+        PSE_TRY(pse_neighbors_settle(c, &redo1));
+        const bool okL = pse_lanczos_validate(c, mL, &shrinkL), okG = pse_gmres_validate(c, mG, &shrinkG);
+        if (!redo0 && !redo1 && okL && okG) {
+            if (shrinkL && mL > 2) c->lanczos_budget = mL - 1;
+            if (shrinkG && mG > 1) c->gmres_budget = mG - 1;
+            if (gmres_iters) *gmres_iters = mG;
+            if (lanczos_iters) *lanczos_iters = mL;
+            return PSE_OK;
+        }
+        c->lanczos_budget = c->gmres_budget = 0;                      // re-learn
+        CUDA_TRY(c, cudaMemcpyAsync(d_pos, c->d_xk, (size_t)N * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+    }
+    // ---- checked path.  The neighbour builds are only enqueued; what they report (list size, overflow, oversized cell) is examined after the
     // Krylov solve that follows has synchronised the stream anyway.  In the rare case that a build must be repeated (first
     // step of a context, or a list that grew by more than 25 % since the last step) the phase that consumed it is redone.
     pse_status st = PSE_OK;
@@ -310,6 +370,9 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     // (79) full step from x_k
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
                                         reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+    if (soft == PSE_OK && c->last_lanczos_iters > 0 && c->last_gmres_iters > 0) {      // the counts the next step is enqueued with
+        c->lanczos_budget = c->last_lanczos_iters; c->gmres_budget = c->last_gmres_iters;
+    }
     return soft;
 }
 

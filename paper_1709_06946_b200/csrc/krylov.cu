@@ -217,6 +217,91 @@ __global__ void __launch_bounds__(VT) k_arnoldi_step(float4 *w, const float4 *Z,
     }
 }
 
+// ---- the small algebra of a solve with a FIXED iteration count, on the device (one warp), so that the host need not be in
+// the loop: pse_step enqueues both solves with the counts the previous step needed and looks at the scalars only afterwards ----
+
+// coef[0..m) = |w| T_m^{1/2} e_1 for the Lanczos tridiagonal T_m (alpha_j on the diagonal, beta_j next to it), by the implicit
+// QL iteration with Wilkinson shift (EISPACK imtql2) on (d, e) with the eigenvector rows spread over the lanes.
+// scal: [0] = |w|^2, [1 + 2j] = alpha_j, [2 + 2j] = beta_j^2.
+__global__ void __launch_bounds__(32) k_lanczos_coef_dev(const double *__restrict__ scal, int m, float *__restrict__ coef) {
+    __shared__ double Z[PSE_MAX_KRYLOV][PSE_MAX_KRYLOV + 1], d[PSE_MAX_KRYLOV], e[PSE_MAX_KRYLOV];
+    const int lane = threadIdx.x;
+    for (int i = lane; i < m; i += 32) { d[i] = scal[1 + 2 * i]; e[i] = i + 1 < m ? sqrt(fmax(scal[2 + 2 * i], 0.0)) : 0.0; }
+    for (int i = lane; i < m; i += 32) for (int j = 0; j < m; ++j) Z[i][j] = i == j ? 1.0 : 0.0;
+    __syncwarp();
+    for (int l = 0; l < m; ++l) {
+        for (int iter = 0; iter < 60; ++iter) {
+            int mm = l;
+            for (; mm < m - 1; ++mm) { const double dd = fabs(d[mm]) + fabs(d[mm + 1]); if (fabs(e[mm]) <= 2e-16 * dd) break; }
+            if (mm == l) break;
+            double g = (d[l + 1] - d[l]) / (2.0 * e[l]), r = hypot(g, 1.0);
+            g = d[mm] - d[l] + e[l] / (g + (g >= 0 ? fabs(r) : -fabs(r)));
+            double sn = 1.0, cs = 1.0, pp = 0.0;
+            int i = mm - 1;
+            bool under = false;
+            for (; i >= l; --i) {
+                double f = sn * e[i];
+                const double b = cs * e[i];
+                r = hypot(f, g);
+                __syncwarp();
+                if (lane == 0) e[i + 1] = r;
+                if (r == 0.0) { if (lane == 0) { d[i + 1] -= pp; e[mm] = 0.0; } under = true; __syncwarp(); break; }
+                sn = f / r; cs = g / r;
+                g = d[i + 1] - pp;
+                r = (d[i] - g) * sn + 2.0 * cs * b;
+                pp = sn * r;
+                __syncwarp();
+                if (lane == 0) d[i + 1] = g + pp;
+                g = cs * r - b;
+                for (int k = lane; k < m; k += 32) {                   // eigenvector rows over the lanes
+                    f = Z[k][i + 1];
+                    Z[k][i + 1] = sn * Z[k][i] + cs * f;
+                    Z[k][i] = cs * Z[k][i] - sn * f;
+                }
+                __syncwarp();
+            }
+            if (under) continue;
+            __syncwarp();
+            if (lane == 0) { d[l] -= pp; e[l] = g; e[mm] = 0.0; }
+            __syncwarp();
+        }
+    }
+    __syncwarp();
+    const double wn = sqrt(fmax(scal[0], 0.0));
+    for (int i = lane; i < m; i += 32) {
+        double acc = 0.0;
+        for (int k = 0; k < m; ++k) acc += Z[i][k] * sqrt(fmax(d[k], 0.0)) * Z[0][k];
+        coef[i] = (float)(wn * acc);
+    }
+}
+
+// y[0..m) of the GMRES least-squares problem after m Arnoldi iterations: Givens rotations column by column, back-substitution.
+// scal: [0] = |b|^2; iteration k owns [base_k .. base_k + k + 1] = h_0..h_k, |w|^2 with base_k = 1 + k(k+3)/2.
+__global__ void __launch_bounds__(32) k_gmres_coef_dev(const double *__restrict__ scal, int m, float *__restrict__ coef) {
+    __shared__ double H[PSE_MAX_KRYLOV + 1][PSE_MAX_KRYLOV], cs[PSE_MAX_KRYLOV], sn[PSE_MAX_KRYLOV], g[PSE_MAX_KRYLOV + 1], y[PSE_MAX_KRYLOV];
+    if (threadIdx.x != 0) return;
+    g[0] = sqrt(fmax(scal[0], 0.0));
+    for (int e = 0; e < m; ++e) {
+        const int eb = 1 + e * (e + 3) / 2;
+        for (int j = 0; j <= e; ++j) H[j][e] = scal[eb + j];
+        H[e + 1][e] = sqrt(fmax(scal[eb + e + 1], 0.0));
+        for (int j = 0; j < e; ++j) {
+            const double a = H[j][e], b = H[j + 1][e];
+            H[j][e] = cs[j] * a + sn[j] * b; H[j + 1][e] = -sn[j] * a + cs[j] * b;
+        }
+        const double a = H[e][e], b = H[e + 1][e], r = hypot(a, b);
+        cs[e] = r > 0 ? a / r : 1.0; sn[e] = r > 0 ? b / r : 0.0;
+        H[e][e] = r; H[e + 1][e] = 0.0;
+        g[e + 1] = -sn[e] * g[e]; g[e] = cs[e] * g[e];
+    }
+    for (int i = m - 1; i >= 0; --i) {
+        double s = g[i];
+        for (int j = i + 1; j < m; ++j) s -= H[i][j] * y[j];
+        y[i] = H[i][i] != 0.0 ? s / H[i][i] : 0.0;
+    }
+    for (int i = 0; i < m; ++i) coef[i] = (float)y[i];
+}
+
 // grid of a cooperative launch: every CTA must be resident (cap computed per device in pse_krylov_init)
 int coop_grid(const pse_ctx *c, size_t work_items) {
     const size_t b = (work_items + 2 * VT - 1) / (2 * VT);          // at least two items per thread: fewer CTAs at the barriers
@@ -303,7 +388,9 @@ pse_status pse_axpby(pse_ctx *c, size_t n, float alpha, const float *x, float be
 
 // y = M_r^{1/2} w  by Lanczos:  v_1 = w/|w|,  T_m = V_m^T M_r V_m,  y_m = |w| V_m T_m^{1/2} e_1.
 // Stop when |y_m - y_{m-1}| <= tol |y_m|; with V orthonormal this is the change of the coefficient vector.
-pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters) {
+// fixed_m > 0: exactly fixed_m iterations, coefficients by k_lanczos_coef_dev, no host read-back: the scalars are copied to
+// h_scal_l behind the solve and examined by pse_lanczos_validate once the stream has been synchronised.
+pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m) {
     const size_t n = (size_t)c->N * 8, n4 = n / 4;
     float4 *V = reinterpret_cast<float4 *>(c->d_krylov);
     float4 *u = reinterpret_cast<float4 *>(c->d_tmp);
@@ -326,18 +413,20 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     // (once the count has repeated, only the iteration it is expected to end in is read back: one synchronisation per solve)
     const int first_check = std::max(0, c->last_lanczos_iters - (c->lanczos_repeats >= 2 ? 1 : 2));
     int examined = 0;
-    for (int j = 0; j < maxit && !converged; ++j) {
+    const int niter = fixed_m > 0 ? std::min(fixed_m, maxit) : maxit;
+    for (int j = 0; j < niter && !converged; ++j) {
         float4 *vj = V + (size_t)j * n4;
         PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
         { ScopedPhase ph(c, PSE_T_VECTOR);
           const float4 *a_vj = vj, *a_vjm1 = j ? vj - n4 : nullptr;
-          float4 *a_u = u, *a_next = j + 1 < maxit ? vj + n4 : nullptr;
+          float4 *a_u = u, *a_next = j + 1 < niter ? vj + n4 : nullptr;
           double *a_alpha = c->d_scal + 1 + 2 * j, *a_b2 = c->d_scal + 2 + 2 * j;
           const double *a_b2prev = j ? c->d_scal + 2 * j : nullptr;
           size_t a_n4 = n4;
           void *args[] = {&a_u, &a_vj, &a_vjm1, &a_next, &a_alpha, &a_b2prev, &a_b2, &a_n4};
           CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_lanczos_step, dim3(coop_grid(c, n4)), dim3(VT), args, 0, c->stream));
           KERNEL_CHECK(c); }
+        if (fixed_m > 0) continue;
         if (j < first_check && j + 1 < maxit) continue;
         PSE_TRY(read_scalars(c, 3 + 2 * j));
         for (; examined <= j && !converged; ++examined) {
@@ -365,6 +454,14 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
             else if (beta[e_j] <= 1e-7 * std::fabs(alpha[0])) converged = true;                          // invariant subspace
         }
     }
+    if (fixed_m > 0) {
+        k_lanczos_coef_dev<<<1, 32, 0, c->stream>>>(c->d_scal, niter, c->d_coef); KERNEL_CHECK(c);
+        { ScopedPhase ph(c, PSE_T_VECTOR);
+          k_lincomb<<<vgrid(n4), VT, 0, c->stream>>>(reinterpret_cast<float4 *>(d_y), nullptr, 0.f, V, n4, niter, c->d_coef, n4); KERNEL_CHECK(c); }
+        CUDA_TRY(c, cudaMemcpyAsync(c->h_scal_l, c->d_scal, (size_t)(1 + 2 * niter) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        if (iters) *iters = niter;
+        return PSE_OK;
+    }
     c->lanczos_repeats = (m == c->last_lanczos_iters) ? c->lanczos_repeats + 1 : 0;
     c->last_lanczos_iters = m;
     std::vector<float> cf(ccur.begin(), ccur.end());
@@ -376,13 +473,71 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     return PSE_OK;
 }
 
+// coefficient vector |w| T_m^{1/2} e_1 of the leading m x m block, host fp64 (Jacobi)
+static std::vector<double> lanczos_coefs_host(const double *hs, int m) {
+    std::vector<double> Tm((size_t)m * m, 0.0), Q, out(m, 0.0);
+    for (int i = 0; i < m; ++i) {
+        Tm[(size_t)i * m + i] = hs[1 + 2 * i];
+        if (i + 1 < m) Tm[(size_t)i * m + i + 1] = Tm[(size_t)(i + 1) * m + i] = std::sqrt(std::max(hs[2 + 2 * i], 0.0));
+    }
+    jacobi_eigh(m, Tm, Q);
+    const double wn = std::sqrt(std::max(hs[0], 0.0));
+    for (int e = 0; e < m; ++e) {
+        const double lam = Tm[(size_t)e * m + e], sq = lam > 0 ? std::sqrt(lam) : 0.0, q0 = Q[e];
+        for (int i = 0; i < m; ++i) out[i] += wn * Q[(size_t)i * m + e] * sq * q0;
+    }
+    return out;
+}
+
+// After a fixed-count solve and a stream synchronisation: did the sample converge within m iterations (same criterion as the
+// adaptive driver, |c_m - c_{m-1}| <= tol |c_m|), and would one iteration fewer have done (*shrink)?
+bool pse_lanczos_validate(pse_ctx *c, int m, bool *shrink) {
+    const double *hs = c->h_scal_l;
+    *shrink = false;
+    if (!(hs[0] > 0)) return true;                                   // zero noise: zero sample
+    if (m < 2) return false;
+    auto change = [&](int mm) {
+        const std::vector<double> a = lanczos_coefs_host(hs, mm), b = lanczos_coefs_host(hs, mm - 1);
+        double diff = 0, nrm = 0;
+        for (int i = 0; i < mm; ++i) { const double d = a[i] - (i < mm - 1 ? b[i] : 0.0); diff += d * d; nrm += a[i] * a[i]; }
+        return std::sqrt(diff) <= c->tol * std::sqrt(nrm);
+    };
+    const bool ok = change(m) || std::sqrt(std::max(hs[2 + 2 * (m - 1)], 0.0)) <= 1e-7 * std::fabs(hs[1]);
+    if (ok && m >= 3) *shrink = change(m - 1);
+    return ok;
+}
+
+// Same for GMRES: relative residual of the Givens recurrence after m iterations <= tol, and after m - 1 (*shrink).
+bool pse_gmres_validate(pse_ctx *c, int m, bool *shrink) {
+    const double *hs = c->h_scal;
+    *shrink = false;
+    const double bnorm = std::sqrt(std::max(hs[0], 0.0));
+    if (!(bnorm > 0)) return true;
+    std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m, 0.0), sn(m, 0.0), g(m + 1, 0.0);
+    g[0] = bnorm;
+    for (int e = 0; e < m; ++e) {
+        const int eb = 1 + e * (e + 3) / 2;
+        for (int j = 0; j <= e; ++j) H[(size_t)j * m + e] = hs[eb + j];
+        H[(size_t)(e + 1) * m + e] = std::sqrt(std::max(hs[eb + e + 1], 0.0));
+        for (int j = 0; j < e; ++j) {
+            const double a = H[(size_t)j * m + e], b = H[(size_t)(j + 1) * m + e];
+            H[(size_t)j * m + e] = cs[j] * a + sn[j] * b; H[(size_t)(j + 1) * m + e] = -sn[j] * a + cs[j] * b;
+        }
+        const double a = H[(size_t)e * m + e], b = H[(size_t)(e + 1) * m + e], r = std::hypot(a, b);
+        cs[e] = r > 0 ? a / r : 1.0; sn[e] = r > 0 ? b / r : 0.0;
+        g[e + 1] = -sn[e] * g[e]; g[e] = cs[e] * g[e];
+        if (e + 1 == m - 1 && std::fabs(g[e + 1]) <= c->tol * bnorm) *shrink = true;
+    }
+    return std::fabs(g[m]) <= c->tol * bnorm;
+}
+
 // Forward declaration of the full product on packed vectors (api.cu)
 pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode = PSE_MODE_ALL);
 
 // GMRES on  M_ES S = -(E^B + M_EF F)  with S and E embedded in packed vectors whose velocity slots are zero.
 // Z_j = M [0; v_j] is kept whole: its E-part feeds Arnoldi, its U-part gives M_US S at the end without another
 // product.  out (packed) = (U, S) with U = U^B + M_UF F + M_US S.
-pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp, float *d_outp, int *iters) {
+pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp, float *d_outp, int *iters, int fixed_m) {
     const int N = c->N;
     const size_t n = (size_t)N * 8, n4 = n / 4;
     float4 *V = reinterpret_cast<float4 *>(c->d_krylov), *Z = reinterpret_cast<float4 *>(c->d_zu);
@@ -405,19 +560,21 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     {
         const int first_check = std::max(0, c->last_gmres_iters - (c->gmres_repeats >= 2 ? 1 : 2));     // see pse_lanczos_sqrt
         int examined = 0;
-        for (int k = 0; k < maxit && !converged; ++k) {
+        const int niter = fixed_m > 0 ? std::min(fixed_m, maxit) : maxit;
+        for (int k = 0; k < niter && !converged; ++k) {
             const int base = 1 + k * (k + 3) / 2;
             float4 *Zk = Z + (size_t)k * n4;
             PSE_TRY(pse_apply_packed(c, reinterpret_cast<const float *>(V + (size_t)k * n4), reinterpret_cast<float *>(Zk), PSE_BOTH, PSE_IN_S | PSE_OUT_E));   // M_ES v_k: 5 grids in, 5 out
             { ScopedPhase ph(c, PSE_T_VECTOR);
               // the velocity slots of every V_j are zero, so <V_j, Z_k> over all 8 components is the E-part product
-              float4 *a_w = w, *a_next = k + 1 < maxit ? V + (size_t)(k + 1) * n4 : nullptr;
+              float4 *a_w = w, *a_next = k + 1 < niter ? V + (size_t)(k + 1) * n4 : nullptr;
               const float4 *a_Z = Zk, *a_V = V;
               size_t a_stride = n4; int a_nvec = k + 1, a_N = N;
               double *a_h = c->d_scal + base;
               void *args[] = {&a_w, &a_Z, &a_V, &a_stride, &a_nvec, &a_h, &a_next, &a_N};
               CUDA_TRY(c, cudaLaunchCooperativeKernel((const void *)k_arnoldi_step, dim3(coop_grid(c, (size_t)N)), dim3(VT), args, 0, c->stream));
               KERNEL_CHECK(c); }
+            if (fixed_m > 0) { m = k + 1; continue; }
             if (k < first_check && k + 1 < maxit) continue;
             PSE_TRY(read_scalars(c, base + k + 2));
             if (examined == 0) {
@@ -443,8 +600,14 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
                 else if (hk1 <= 1e-12 * bnorm) converged = true;
             }
         }
-        c->gmres_repeats = (m == c->last_gmres_iters) ? c->gmres_repeats + 1 : 0;
-        c->last_gmres_iters = m;
+        if (fixed_m > 0) {
+            k_gmres_coef_dev<<<1, 32, 0, c->stream>>>(c->d_scal, m, c->d_coef); KERNEL_CHECK(c);
+            CUDA_TRY(c, cudaMemcpyAsync(c->h_scal, c->d_scal, (size_t)(1 + m * (m + 3) / 2) * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            converged = true;                                        // decided later by pse_gmres_validate
+        } else {
+            c->gmres_repeats = (m == c->last_gmres_iters) ? c->gmres_repeats + 1 : 0;
+            c->last_gmres_iters = m;
+        }
         y.assign(m, 0.0);
         for (int i = m - 1; i >= 0; --i) {
             double s = g[i];
@@ -455,7 +618,7 @@ pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UB
     // S = sum_j y_j v_j;  U = U^B + U-rows of M [F; S]: one last product with 3 output grids (the Arnoldi products
     // carried only the E rows)
     std::vector<float> yf(y.begin(), y.end());
-    if (m) PSE_TRY(upload_coefs(c, yf));
+    if (m && fixed_m <= 0) PSE_TRY(upload_coefs(c, yf));
     float4 *fin = w;                                               // [F; S] packed, reuses the Arnoldi work vector
     { ScopedPhase ph(c, PSE_T_VECTOR);
       k_lincomb<<<vgrid(n4), VT, 0, c->stream>>>(fin, reinterpret_cast<const float4 *>(d_Fp), 1.f, V, n4, m, c->d_coef, n4); KERNEL_CHECK(c); }

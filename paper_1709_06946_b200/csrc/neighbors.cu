@@ -523,7 +523,8 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
                                                                    c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
                                                                    reinterpret_cast<int *>(c->d_nbr_ctl + 1)); KERNEL_CHECK(c);
-        CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        c->nbr_last = c->nbr_slot; c->nbr_slot ^= 1;               // two report slots: pse_step has two builds in flight
+        CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl + 2 * c->nbr_last, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(c, cudaEventRecord(c->ev_nbr, c->stream));
         c->nbr_pending = true;
     } else {                                                         // general two-pass path (count, scan, fill); synchronises
@@ -558,8 +559,15 @@ pse_status pse_neighbors_settle(pse_ctx *c, bool *redo) {
     if (!c->nbr_pending) return PSE_OK;
     CUDA_TRY(c, cudaEventSynchronize(c->ev_nbr));
     c->nbr_pending = false;
-    if (c->h_nbr_ctl[1] != 0) { c->nbr_two_pass = true; c->have_nbrs = false; *redo = true; return PSE_OK; }
-    const unsigned long long total = c->h_nbr_ctl[0];
+    return pse_neighbors_examine(c, c->nbr_last, redo);
+}
+
+// the report of one build (slot of h_nbr_ctl), after the stream has passed its read-back
+pse_status pse_neighbors_examine(pse_ctx *c, int slot, bool *redo) {
+    *redo = false;
+    const unsigned long long *ctl = c->h_nbr_ctl + 2 * slot;
+    if (ctl[1] != 0) { c->nbr_two_pass = true; c->have_nbrs = false; *redo = true; return PSE_OK; }
+    const unsigned long long total = ctl[0];
     if (total > c->nbr_cap) {
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));               // kernels still reading the old array
         cudaFree(c->d_nbr_idx); c->d_nbr_idx = nullptr; c->nbr_cap = 0;

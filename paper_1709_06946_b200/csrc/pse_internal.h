@@ -28,6 +28,15 @@ struct pse_ctx {
     int win_kind = 1;                        // 0 = Gaussian (paper), 1 = exponential-of-semicircle window
     double win_a = 0, win_b = 0;             // window parameters handed to the kernels (see win_arg in wavespace.cu)
     float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index
+    // ---- finer grid of the Brownian wave pass (the field sqrt(B) W decays only like exp(-k^2/8 xi^2), so the modes
+    //      next to the Nyquist frequency of the product grid, which a P-point window cannot interpolate, still carry weight;
+    //      the same modes are therefore evaluated on a grid Mb > M: zero-padded spectrum, own C2R plan, generic interpolation) ----
+    int Mb = 0, Mbh = 0, Pb = 0;             // Pb = P + 1 support points per dimension
+    double win_a_b = 0, win_b_b = 0;         // window parameters for Pb
+    float *d_dec_b = nullptr;                // [Mb]
+    float *d_grid_b = nullptr;               // [8][Mb^3]
+    cufftComplex *d_spec_b = nullptr;        // [8][Mb][Mb][Mbh]
+    cufftHandle plan_c2r_b = 0; bool have_plan_b = false;
     cudaStream_t stream = nullptr;
     int device = 0, nsm = 0;                 // device the context lives on (recorded at pse_create), its SM count
     int coop_cap = 0;                        // largest cooperative grid of the Krylov step kernels on that device
@@ -52,7 +61,8 @@ struct pse_ctx {
     int *d_nbr_count = nullptr;              // [N]
     unsigned long long *d_nbr_off = nullptr; // [N+1]
     int *d_nbr_idx = nullptr; size_t nbr_cap = 0, nbr_total = 0;
-    unsigned long long *d_nbr_ctl = nullptr, *h_nbr_ctl = nullptr;   // {allocation cursor, fallback flag}; pinned mirror
+    unsigned long long *d_nbr_ctl = nullptr, *h_nbr_ctl = nullptr;   // {allocation cursor, fallback flag}; pinned mirror, two slots of two
+    int nbr_slot = 0, nbr_last = 0;          // slot of h_nbr_ctl the next build reports into / the last one did
     cudaEvent_t ev_nbr = nullptr;            // recorded behind the build's read-back
     bool nbr_pending = false;                // the last build's size / flags have not been examined yet (pse_neighbors_settle)
     bool nbr_two_pass = false;               // a cell once exceeded the mask store: this context takes the two-pass path
@@ -83,6 +93,9 @@ struct pse_ctx {
     float *d_zu = nullptr;                               // [PSE_MAX_KRYLOV][N][8] full outputs M[0;v_j] (GMRES)
     double *d_scal = nullptr;                // device scalars (dots, norms)
     double *h_scal = nullptr;                // pinned mirror
+    double *h_scal_l = nullptr;              // pinned mirror of the Lanczos scalars of a fixed-count solve (pse_step's optimistic path)
+    int lanczos_budget = 0, gmres_budget = 0;   // iteration counts the last completed step needed; 0 = not known yet
+    float4 *d_xk = nullptr;                  // [N] copy of x_k while an optimistic step is in flight
     float *d_coef = nullptr;                 // small coefficient vector upload
     int last_lanczos_iters = 0, last_gmres_iters = 0;   // iteration counts of the previous solves (when to start reading back)
     int lanczos_repeats = 0, gmres_repeats = 0;         // how many solves in a row ended with that same count
@@ -157,6 +170,8 @@ __device__ __forceinline__ float warp_reduce8(const float (&a)[8], int lane, int
 }
 #endif
 
+// api.cu
+int pse_choose_grid(int mmin);
 // tables.cu
 void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr);
 void pse_window_table(int kind, int P, double wa, double wb, int M, std::vector<float> &dec);
@@ -164,6 +179,7 @@ double pse_es_beta(int P);
 // neighbors.cu
 pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos);    // enqueue only
 pse_status pse_neighbors_settle(pse_ctx *c, bool *redo);
+pse_status pse_neighbors_examine(pse_ctx *c, int slot, bool *redo);
 pse_status pse_neighbors_sync(pse_ctx *c, const float *d_pos);    // build + settle, repeated until complete
 pse_status pse_scan_u64(pse_ctx *c, const int *d_in, unsigned long long *d_out, size_t n);   // exclusive, n+1 outputs
 pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n);
@@ -186,7 +202,9 @@ pse_status pse_krylov_init(pse_ctx *c);   // cooperative-grid cap of the step ke
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted
 pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed);
 pse_status pse_unpack(pse_ctx *c, const float *d_packed, float scale, float *d_U, float *d_E);
-pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters);          // y = M_r^{1/2} w
+pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m = 0);          // y = M_r^{1/2} w
+bool pse_lanczos_validate(pse_ctx *c, int m, bool *shrink);
+bool pse_gmres_validate(pse_ctx *c, int m, bool *shrink);
 pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp,
-                                float *d_outp, int *iters);
+                                float *d_outp, int *iters, int fixed_m = 0);
 pse_status pse_axpby(pse_ctx *c, size_t n, float alpha, const float *x, float beta, float *y);

@@ -9,6 +9,7 @@ constexpr float WS_RS2 = 0.70710678118654752f, WS_RS6 = 0.40824829046386302f;
 
 struct ScaleParams {
     int M, Mh;
+    int Mc, Mch;                                   // Brownian pass on the finer grid: the (coarser) product grid the noise buffer is laid out on
     float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
     const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
     int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
@@ -107,7 +108,7 @@ __device__ __forceinline__ void scale_point(const ScaleParams &sp, int ix, int i
 inline ScaleParams make_scale_params(const pse_ctx *c, int mode = PSE_MODE_ALL) {
     ScaleParams sp;
     sp.mode = mode;
-    sp.M = c->M; sp.Mh = c->Mh;
+    sp.M = c->M; sp.Mh = c->Mh; sp.Mc = c->M; sp.Mch = c->Mh;
     sp.two_pi_over_L = (float)(2.0 * M_PI / c->L); sp.a = (float)c->a;
     sp.inv4xi2 = (float)(1.0 / (4.0 * c->xi * c->xi)); sp.dec = c->d_dec;
     const double V = c->L * c->L * c->L;

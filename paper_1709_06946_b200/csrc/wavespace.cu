@@ -620,30 +620,35 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
     scale_point(sp, ix, iy, iz, spec, nmode, o, spec, nmode, o);
 }
 
-// a5, Brownian flavour (Eq. 75): uh = c_br sqrt((1+k^2/4xi^2)/(eta k^2)) exp(-(1-eta_g) k^2/8xi^2) (I - kh kh) W(k),
-// W(k) = (g_re + i g_im)/sqrt2 from the noise buffer; in the plane kz = 0 the non-canonical member of each +-k
-// pair takes the conjugate of its partner's entry (reading R8) so that the C2R transform sees a Hermitian field.
+// a5, Brownian flavour (Eq. 75): uh = c_br sqrt((1+k^2/4xi^2)/(eta k^2)) exp(-k^2/8xi^2) / kappa(k) (I - kh kh) W(k),
+// W(k) = (g_re + i g_im)/sqrt2 from the noise buffer; in the plane kz = 0 the non-canonical member of each +-k pair takes the
+// conjugate of its partner's entry (reading R8) so that the C2R transform sees a Hermitian field.  The thread grid is the half
+// spectrum of the FINER grid sp.M of the Brownian pass; the noise buffer is laid out on the product grid sp.Mc <= sp.M and only
+// its modes carry weight (zero-padded spectrum): same field as on the product grid, interpolated with an oversampled window.
 __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec, const float2 *__restrict__ noise, ScaleParams sp) {
-    const int M = sp.M;
+    const int M = sp.M, Mc = sp.Mc;
     const unsigned plane = (unsigned)M * (unsigned)sp.Mh, rem = blockIdx.x * blockDim.x + threadIdx.x;
     if (rem >= plane) return;
     const int ix = (int)blockIdx.y, iy = (int)(rem / (unsigned)sp.Mh), iz = (int)(rem - (unsigned)iy * (unsigned)sp.Mh);
     const size_t nmode = (size_t)plane * M, o = (size_t)ix * plane + rem;
-    float kx, ky, kz;
-    float2 zero = make_float2(0.f, 0.f);
-    const size_t oplane = nmode, oo = o;
-    if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
+    const float2 zero = make_float2(0.f, 0.f);
+    const int half = (M + 1) / 2, nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M, nz = iz;
+    // modes of the product grid, its Nyquist planes and k = 0 excluded (reading R8)
+    const int lim = (Mc - 1) / 2;                                      // largest |n| below the product grid's Nyquist index
+    const bool live = abs(nx) <= lim && abs(ny) <= lim && nz <= lim && (nx | ny | nz) != 0;
+    if (!live) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) spec[c * oplane + oo] = zero;
+        for (int c = 0; c < 8; ++c) spec[c * nmode + o] = zero;
         return;
     }
-    const int half = (M + 1) / 2, nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M;
-    const bool canon = iz > 0 || ny > 0 || (ny == 0 && nx > 0);
-    const size_t src = canon ? o : ((size_t)((M - ix) % M) * M + (size_t)((M - iy) % M)) * sp.Mh;
+    const float kx = sp.two_pi_over_L * (float)nx, ky = sp.two_pi_over_L * (float)ny, kz = sp.two_pi_over_L * (float)nz;
+    const bool canon = nz > 0 || ny > 0 || (ny == 0 && nx > 0);
+    const int sx = canon ? nx : -nx, sy = canon ? ny : -ny;           // noise entry of the canonical member, product-grid indices
+    const size_t cmode = (size_t)Mc * Mc * sp.Mch, src = ((size_t)(sx < 0 ? sx + Mc : sx) * Mc + (size_t)(sy < 0 ? sy + Mc : sy)) * sp.Mch + nz;
     const float sgn = canon ? 1.f : -1.f;
     float2 W[3];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { float2 g = noise[c * nmode + src]; W[c] = make_float2(g.x * WS_RS2, sgn * g.y * WS_RS2); }
+    for (int c = 0; c < 3; ++c) { float2 g = noise[c * cmode + src]; W[c] = make_float2(g.x * WS_RS2, sgn * g.y * WS_RS2); }
     const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
     float s0, s1;
     shape_factors(ka, s0, s1);
@@ -654,7 +659,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float2 ux = make_float2(Bh * (W[0].x - kx * kw.x), Bh * (W[0].y - kx * kw.y));
     const float2 uy = make_float2(Bh * (W[1].x - ky * kw.x), Bh * (W[1].y - ky * kw.y));
     const float2 uz = make_float2(Bh * (W[2].x - kz * kw.x), Bh * (W[2].y - kz * kw.y));
-    write_outputs(spec, oplane, oo, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
+    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
 }
 
 }  // namespace
@@ -707,6 +712,9 @@ static bool use_block_spread(const pse_ctx *c) { return c->P <= 8 && c->P != 7 &
 pse_status pse_wave_init(pse_ctx *c) {
     const int M = c->M;
     c->Mh = M / 2 + 1;
+    c->Mb = std::max(M + 2, pse_choose_grid((int)std::ceil(1.18 * M)));      // finer grid of the Brownian wave pass (see pse_internal.h)
+    c->Mbh = c->Mb / 2 + 1;
+    c->Pb = std::min(PSE_MAXP, c->P + 1);                                      // and one more window point per dimension
     c->nt = (M + T - 1) / T; c->ntile = c->nt * c->nt * c->nt;
     const size_t M3 = pse_plane_stride(M), nmode = (size_t)M * M * c->Mh;
     CUDA_TRY(c, cudaMalloc(&c->d_grid, 8 * M3 * sizeof(float)));
@@ -761,7 +769,20 @@ pse_status pse_wave_init(pse_ctx *c) {
         }
         w = std::max(w, std::max(w1, w2));
     }
+    {   // Brownian pass: 8 planes C2R on the finer grid
+        const int Mb = c->Mb, Mbh = c->Mbh;
+        const size_t M3b = pse_plane_stride(Mb);
+        CUDA_TRY(c, cudaMalloc(&c->d_grid_b, 8 * M3b * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->d_spec_b, 8 * (size_t)Mb * Mb * Mbh * sizeof(cufftComplex)));
+        int nb3[3] = {Mb, Mb, Mb}, nr[3] = {Mb, Mb, Mb}, ncx[3] = {Mb, Mb, Mbh};
+        size_t wb = 0;
+        CUFFT_TRY(c, cufftCreate(&c->plan_c2r_b)); c->have_plan_b = true;
+        CUFFT_TRY(c, cufftSetAutoAllocation(c->plan_c2r_b, 0));
+        CUFFT_TRY(c, cufftMakePlanMany(c->plan_c2r_b, 3, nb3, ncx, 1, Mb * Mb * Mbh, nr, 1, (int)M3b, CUFFT_C2R, 8, &wb));
+        w = std::max(w, wb);
+    }
     if (w) CUDA_TRY(c, cudaMalloc(&c->d_fft_work, w));
+    CUFFT_TRY(c, cufftSetWorkArea(c->plan_c2r_b, c->d_fft_work)); CUFFT_TRY(c, cufftSetStream(c->plan_c2r_b, c->stream));
     for (int i = 0; i < 3; ++i) {
         CUFFT_TRY(c, cufftSetWorkArea(c->plan_r2c[i], c->d_fft_work)); CUFFT_TRY(c, cufftSetWorkArea(c->plan_c2r[i], c->d_fft_work));
         CUFFT_TRY(c, cufftSetStream(c->plan_r2c[i], c->stream)); CUFFT_TRY(c, cufftSetStream(c->plan_c2r[i], c->stream));
@@ -771,6 +792,8 @@ pse_status pse_wave_init(pse_ctx *c) {
 
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
+    if (c->have_plan_b) cufftDestroy(c->plan_c2r_b);
+    cudaFree(c->d_grid_b); cudaFree(c->d_spec_b);
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
     cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list); cudaFree(c->d_pbase); cudaFree(c->d_pw);
     cudaFree(c->d_half_start); cudaFree(c->d_half_count); cudaFree(c->d_half_list);
@@ -876,13 +899,22 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
 }
 
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {
-    const size_t nmode = (size_t)c->M * c->M * c->Mh;
     if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
+    const int Mb = c->Mb;
     {
         ScopedPhase ph(c, PSE_T_SCALE);
-        scale_brownian_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(
-            c->d_spec, reinterpret_cast<const float2 *>(d_noise_wave), make_scale_params(c));
+        ScaleParams sp = make_scale_params(c);
+        sp.M = Mb; sp.Mh = c->Mbh; sp.dec = c->d_dec_b;               // thread grid and window table of the finer grid; noise on (Mc, Mch)
+        scale_brownian_kernel<<<dim3((unsigned)((Mb * c->Mbh + 255) / 256), (unsigned)Mb), 256, 0, c->stream>>>(
+            c->d_spec_b, reinterpret_cast<const float2 *>(d_noise_wave), sp);
         KERNEL_CHECK(c);
     }
-    return inverse_and_interpolate(c, d_out, accumulate);
+    { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r_b, c->d_spec_b, c->d_grid_b)); c->launches++; }
+    ScopedPhase ph(c, PSE_T_INTERP);
+    const int TB = 256;
+    interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
+        c->d_pos, c->d_tile_list, c->d_grid_b, reinterpret_cast<float4 *>(d_out), c->N, Mb, c->Pb, (float)(Mb / c->L),
+        (float)c->win_a_b, (float)c->win_b_b, accumulate ? 1 : 0, PSE_MODE_ALL);
+    KERNEL_CHECK(c);
+    return PSE_OK;
 }

@@ -217,7 +217,7 @@ def test_config2_full_midpoint_step_against_fp64_reference_step():
     e_x = np.linalg.norm(d) / np.linalg.norm(disp)
     assert e_x < 3 * bar(tol), e_x
     assert np.linalg.norm(d, axis=1).max() < 30 * bar(tol) * np.sqrt((disp * disp).sum(axis=1).mean())
-    assert abs(l_it - li) <= 6 and abs(g_it - gi) <= 8 and 3 <= g_it <= 20
+    assert 3 <= l_it <= li and 3 <= g_it <= gi and g_it <= 20       # the reference iterates to 1e-10, the library to tol
     # the pieces of the step, for U and S
     ctx.pse_neighbors(dev(pos4(x32)))
     UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
