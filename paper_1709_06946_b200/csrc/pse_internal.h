@@ -20,6 +20,16 @@ enum { PSE_IN_F = 1, PSE_IN_S = 2, PSE_OUT_U = 4, PSE_OUT_E = 8, PSE_MODE_ALL = 
 
 struct Timer { cudaEvent_t a, b; int phase; };
 
+// Everything the tiled interpolation needs about one grid: the product grid (M, P) or the finer grid of the Brownian pass.
+struct InterpSet {
+    int M = 0, P = 0, PP = 0, nt = 0, ntile = 0;
+    float *grid = nullptr;                   // [8][pse_plane_stride(M)]
+    int *tile_start = nullptr, *tile_list = nullptr;     // bins of the particles by the tile of their support base
+    int *pbase = nullptr; float *pw = nullptr;           // per-particle window data in tile order
+    CUtensorMap tmap;                        // TMA descriptor of grid as [8][M][M][M] with the (T+P-1)^3 box
+    bool tma_ok = false;
+};
+
 struct pse_ctx {
     // ---- parameters (pse_create) ----
     int N = 0, M = 0, P = 0;
@@ -85,8 +95,9 @@ struct pse_ctx {
     cufftComplex *d_spec = nullptr;          // [8][M][M][Mh]
     cufftHandle plan_r2c[3] = {0, 0, 0}, plan_c2r[3] = {0, 0, 0};   // [0] all 8 grids, [1] planes 0-2 (F / U), [2] planes 3-7 (S / E)
     void *d_fft_work = nullptr; int nplans = 0;
-    CUtensorMap tmap_grid[9];                // TMA descriptor of d_grid as a [8][M][M][M] tensor with the (T+P-1)^3 box of this P (index P)
-    bool tma_ok = false;                     // descriptor valid (needs M % 4 == 0)
+    InterpSet iset, iset_b;                  // interpolation views of the product grid and of the Brownian pass's finer grid
+    int *d_tile_of_b = nullptr, *d_tile_tmp_b = nullptr, *d_tile_cnt_b = nullptr;   // binning scratch of the finer grid ([N], [N], [2 (ntile_b + 1)])
+    bool fine_bins_valid = false;            // iset_b's bins and window data belong to the current positions
     // ---- packed per-particle vectors, sorted numbering: [N][8] = (x,y,z,e1..e5) ----
     float *d_in = nullptr, *d_out = nullptr, *d_tmp = nullptr, *d_tmp2 = nullptr;
     float *d_krylov = nullptr;  int krylov_cap = 0;      // [krylov_cap][N][8]

@@ -240,6 +240,21 @@ __global__ void particle_window_kernel(const float4 *__restrict__ pos, const int
     pbase[i] = packed;
 }
 
+// ---- tile bins of the finer grid of the Brownian pass (built on demand, once per configuration that draws a sample) ----
+__global__ void fine_bin_count(const float4 *__restrict__ pos, int N, float inv_h, int M, int P, int nt, int *__restrict__ tile_of, int *__restrict__ count) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const int t = pse_tile_of(pos[s], inv_h, M, P, nt);
+    tile_of[s] = t;
+    atomicAdd(count + t, 1);
+}
+__global__ void fine_bin_scatter(const int *__restrict__ tile_of, int N, const int *__restrict__ start, int *__restrict__ fill, int *__restrict__ tmp) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const int t = tile_of[s];
+    tmp[start[t] + atomicAdd(fill + t, 1)] = s;                      // order inside a tile fixed afterwards by the rank sort
+}
+
 // ---- lists of the particles that reach each half tile (built once per pse_neighbors, used by every spread) -----------------
 // A "half" is the 4 x 8 x 8 block of grid points one warp of the spread kernel owns: half index = (tile index) * 2 + (x half).
 // One warp per half walks the tile bins that can reach it (two per dimension, three next to a partial last tile), 32 entries
@@ -665,27 +680,38 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
 }  // namespace
 
 template <int PT, int C0, int NC>
-static pse_status launch_interp_planes(pse_ctx *c, float *d_out, bool accumulate) {
+static pse_status launch_interp_planes(pse_ctx *c, const InterpSet &g, float *d_out, bool accumulate) {
     const size_t smem = (size_t)NC * InterpGeom<PT>::PL * sizeof(float);
-    interp_planes_kernel<PT, C0, NC><<<c->ntile, 256, smem, c->stream>>>(c->tmap_grid[PT], c->d_pbase, c->d_pw, c->d_tile_start, c->d_tile_list, c->d_grid,
-                                                                        d_out, c->M, c->nt, accumulate ? 1 : 0, c->tma_ok ? 1 : 0);
+    interp_planes_kernel<PT, C0, NC><<<g.ntile, 256, smem, c->stream>>>(g.tmap, g.pbase, g.pw, g.tile_start, g.tile_list, g.grid,
+                                                                       d_out, g.M, g.nt, accumulate ? 1 : 0, g.tma_ok ? 1 : 0);
     return PSE_OK;
 }
 template <int PT>
-static pse_status launch_interp(pse_ctx *c, int oplan, float *d_out, bool accumulate) {
-    return oplan == 3 ? launch_interp_planes<PT, 0, 8>(c, d_out, accumulate)
-         : oplan == 1 ? launch_interp_planes<PT, 0, 3>(c, d_out, accumulate) : launch_interp_planes<PT, 3, 5>(c, d_out, accumulate);
+static pse_status launch_interp(pse_ctx *c, const InterpSet &g, int oplan, float *d_out, bool accumulate) {
+    return oplan == 3 ? launch_interp_planes<PT, 0, 8>(c, g, d_out, accumulate)
+         : oplan == 1 ? launch_interp_planes<PT, 0, 3>(c, g, d_out, accumulate) : launch_interp_planes<PT, 3, 5>(c, g, d_out, accumulate);
+}
+static pse_status launch_interp_any(pse_ctx *c, const InterpSet &g, int oplan, float *d_out, bool accumulate) {
+    switch (g.P) {
+        case 2: return launch_interp<2>(c, g, oplan, d_out, accumulate);
+        case 3: return launch_interp<3>(c, g, oplan, d_out, accumulate);
+        case 4: return launch_interp<4>(c, g, oplan, d_out, accumulate);
+        case 5: return launch_interp<5>(c, g, oplan, d_out, accumulate);
+        case 6: return launch_interp<6>(c, g, oplan, d_out, accumulate);
+        case 7: return launch_interp<7>(c, g, oplan, d_out, accumulate);
+        default: return launch_interp<8>(c, g, oplan, d_out, accumulate);
+    }
 }
 
-// dynamic shared-memory opt-in of the interpolation kernels and the TMA descriptor of the grid array for this context's P
+// dynamic shared-memory opt-in of the interpolation kernels and the TMA descriptor of one grid array
 template <int PT>
-static pse_status init_interp(pse_ctx *c) {
+static pse_status init_interp(pse_ctx *c, InterpSet &g) {
 #define PSE_INTERP_ATTR(C0, NC) CUDA_TRY(c, cudaFuncSetAttribute(interp_planes_kernel<PT, C0, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                                                  (int)((size_t)NC * InterpGeom<PT>::PL * sizeof(float))))
     PSE_INTERP_ATTR(0, 8); PSE_INTERP_ATTR(0, 3); PSE_INTERP_ATTR(3, 5);
 #undef PSE_INTERP_ATTR
-    c->tma_ok = false;
-    if (c->M % 4 != 0) return PSE_OK;                 // row pitch not a multiple of 16 bytes: TMA cannot address the grid
+    g.tma_ok = false;
+    if (g.M % 4 != 0) return PSE_OK;                  // row pitch not a multiple of 16 bytes: TMA cannot address the grid
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
     void *fn = nullptr;
@@ -694,15 +720,27 @@ static pse_status init_interp(pse_ctx *c) {
         cudaGetLastError();
         return PSE_OK;                                // driver without tensor maps: cp.async staging everywhere
     }
-    const cuuint64_t M = (cuuint64_t)c->M;
+    const cuuint64_t M = (cuuint64_t)g.M;
     const cuuint64_t dims[4] = {M, M, M, 8};
-    const cuuint64_t strides[3] = {M * 4, M * M * 4, (cuuint64_t)pse_plane_stride(c->M) * 4};
+    const cuuint64_t strides[3] = {M * 4, M * M * 4, (cuuint64_t)pse_plane_stride(g.M) * 4};
     const cuuint32_t box[4] = {(cuuint32_t)InterpGeom<PT>::EP, (cuuint32_t)InterpGeom<PT>::E, (cuuint32_t)InterpGeom<PT>::E, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    const CUresult r = ((encode_fn)fn)(&c->tmap_grid[PT], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->d_grid, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const CUresult r = ((encode_fn)fn)(&g.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, g.grid, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    c->tma_ok = (r == CUDA_SUCCESS);
+    g.tma_ok = (r == CUDA_SUCCESS);
     return PSE_OK;
+}
+static pse_status init_interp_any(pse_ctx *c, InterpSet &g) {
+    switch (g.P) {
+        case 2: return init_interp<2>(c, g);
+        case 3: return init_interp<3>(c, g);
+        case 4: return init_interp<4>(c, g);
+        case 5: return init_interp<5>(c, g);
+        case 6: return init_interp<6>(c, g);
+        case 7: return init_interp<7>(c, g);
+        case 8: return init_interp<8>(c, g);
+        default: return PSE_OK;                       // wider supports take the generic kernel
+    }
 }
 
 // the block-owning spread serves supports up to 8 points on grids of at least two tiles per dimension; anything else takes
@@ -722,19 +760,15 @@ pse_status pse_wave_init(pse_ctx *c) {
     CUDA_TRY(c, cudaMalloc(&c->d_tile_start, (size_t)(c->ntile + 1) * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_of, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_tile_list, (size_t)c->N * sizeof(int)));
-    switch (c->P) {
-        case 2: PSE_TRY(init_interp<2>(c)); break;
-        case 3: PSE_TRY(init_interp<3>(c)); break;
-        case 4: PSE_TRY(init_interp<4>(c)); break;
-        case 5: PSE_TRY(init_interp<5>(c)); break;
-        case 6: PSE_TRY(init_interp<6>(c)); break;
-        case 7: PSE_TRY(init_interp<7>(c)); break;
-        case 8: PSE_TRY(init_interp<8>(c)); break;
-        default: break;
-    }
     c->PP = (c->P + 3) & ~3;
     CUDA_TRY(c, cudaMalloc(&c->d_pbase, (size_t)c->N * sizeof(int)));
     CUDA_TRY(c, cudaMalloc(&c->d_pw, (size_t)c->N * 3 * c->PP * sizeof(float)));
+    {
+        InterpSet &g = c->iset;
+        g.M = c->M; g.P = c->P; g.PP = c->PP; g.nt = c->nt; g.ntile = c->ntile; g.grid = c->d_grid;
+        g.tile_start = c->d_tile_start; g.tile_list = c->d_tile_list; g.pbase = c->d_pbase; g.pw = c->d_pw;
+        PSE_TRY(init_interp_any(c, g));
+    }
     if (use_block_spread(c)) {
         // exact bound of the halves one particle can reach for this (P, M): units touched per dimension, maximised over the base
         auto max_units = [&](int UW) {
@@ -774,6 +808,16 @@ pse_status pse_wave_init(pse_ctx *c) {
         const size_t M3b = pse_plane_stride(Mb);
         CUDA_TRY(c, cudaMalloc(&c->d_grid_b, 8 * M3b * sizeof(float)));
         CUDA_TRY(c, cudaMalloc(&c->d_spec_b, 8 * (size_t)Mb * Mb * Mbh * sizeof(cufftComplex)));
+        InterpSet &g = c->iset_b;                     // tile bins and window data of the finer grid, built on demand (pse_wave_brownian)
+        g.M = Mb; g.P = c->Pb; g.PP = (c->Pb + 3) & ~3; g.nt = (Mb + T - 1) / T; g.ntile = g.nt * g.nt * g.nt; g.grid = c->d_grid_b;
+        CUDA_TRY(c, cudaMalloc(&g.tile_start, (size_t)(g.ntile + 1) * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&g.tile_list, (size_t)c->N * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&g.pbase, (size_t)c->N * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&g.pw, (size_t)c->N * 3 * g.PP * sizeof(float)));
+        CUDA_TRY(c, cudaMalloc(&c->d_tile_of_b, (size_t)c->N * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&c->d_tile_tmp_b, (size_t)c->N * sizeof(int)));
+        CUDA_TRY(c, cudaMalloc(&c->d_tile_cnt_b, (size_t)2 * (g.ntile + 1) * sizeof(int)));
+        PSE_TRY(init_interp_any(c, g));
         int nb3[3] = {Mb, Mb, Mb}, nr[3] = {Mb, Mb, Mb}, ncx[3] = {Mb, Mb, Mbh};
         size_t wb = 0;
         CUFFT_TRY(c, cufftCreate(&c->plan_c2r_b)); c->have_plan_b = true;
@@ -794,6 +838,8 @@ void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     if (c->have_plan_b) cufftDestroy(c->plan_c2r_b);
     cudaFree(c->d_grid_b); cudaFree(c->d_spec_b);
+    cudaFree(c->iset_b.tile_start); cudaFree(c->iset_b.tile_list); cudaFree(c->iset_b.pbase); cudaFree(c->iset_b.pw);
+    cudaFree(c->d_tile_of_b); cudaFree(c->d_tile_tmp_b); cudaFree(c->d_tile_cnt_b);
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
     cudaFree(c->d_tile_start); cudaFree(c->d_tile_of); cudaFree(c->d_tile_list); cudaFree(c->d_pbase); cudaFree(c->d_pw);
     cudaFree(c->d_half_start); cudaFree(c->d_half_count); cudaFree(c->d_half_list);
@@ -805,18 +851,40 @@ pse_status pse_tile_bins(pse_ctx *c) {
     return pse_rank_sort(c, c->d_tile_start, c->ntile, c->d_tile_tmp, c->d_tile_list);
 }
 
-pse_status pse_particle_windows(pse_ctx *c) {
+static pse_status launch_particle_window(pse_ctx *c, const InterpSet &g, double wa_d, double wb_d) {
     const float4 *pos = c->d_pos;
-    float4 *pw4 = reinterpret_cast<float4 *>(c->d_pw);
-    const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
+    float4 *pw4 = reinterpret_cast<float4 *>(g.pw);
+    const float ih = (float)(g.M / c->L), wa = (float)wa_d, wb = (float)wb_d;
     const int nb = (c->N + 127) / 128;
-    switch (c->PP) {
-        case 4: particle_window_kernel<4><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
-        case 8: particle_window_kernel<8><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
-        case 12: particle_window_kernel<12><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
-        default: particle_window_kernel<16><<<nb, 128, 0, c->stream>>>(pos, c->d_tile_list, c->N, c->M, c->P, ih, wa, wb, c->d_pbase, pw4); break;
+    switch (g.PP) {
+        case 4: particle_window_kernel<4><<<nb, 128, 0, c->stream>>>(pos, g.tile_list, c->N, g.M, g.P, ih, wa, wb, g.pbase, pw4); break;
+        case 8: particle_window_kernel<8><<<nb, 128, 0, c->stream>>>(pos, g.tile_list, c->N, g.M, g.P, ih, wa, wb, g.pbase, pw4); break;
+        case 12: particle_window_kernel<12><<<nb, 128, 0, c->stream>>>(pos, g.tile_list, c->N, g.M, g.P, ih, wa, wb, g.pbase, pw4); break;
+        default: particle_window_kernel<16><<<nb, 128, 0, c->stream>>>(pos, g.tile_list, c->N, g.M, g.P, ih, wa, wb, g.pbase, pw4); break;
     }
     KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
+// tile bins and window data of the finer grid for the current (cell-sorted) positions; no-op if they are current
+static pse_status ensure_fine_bins(pse_ctx *c) {
+    if (c->fine_bins_valid) return PSE_OK;
+    InterpSet &g = c->iset_b;
+    const int N = c->N, nb = (N + 255) / 256;
+    int *count = c->d_tile_cnt_b, *fill = c->d_tile_cnt_b + g.ntile + 1;
+    CUDA_TRY(c, cudaMemsetAsync(c->d_tile_cnt_b, 0, (size_t)2 * (g.ntile + 1) * sizeof(int), c->stream));
+    fine_bin_count<<<nb, 256, 0, c->stream>>>(c->d_pos, N, (float)(g.M / c->L), g.M, g.P, g.nt, c->d_tile_of_b, count); KERNEL_CHECK(c);
+    PSE_TRY(pse_scan_i32(c, count, g.tile_start, (size_t)g.ntile));
+    fine_bin_scatter<<<nb, 256, 0, c->stream>>>(c->d_tile_of_b, N, g.tile_start, fill, c->d_tile_tmp_b); KERNEL_CHECK(c);
+    PSE_TRY(pse_rank_sort(c, g.tile_start, g.ntile, c->d_tile_tmp_b, g.tile_list));
+    PSE_TRY(launch_particle_window(c, g, c->win_a_b, c->win_b_b));
+    c->fine_bins_valid = true;
+    return PSE_OK;
+}
+
+pse_status pse_particle_windows(pse_ctx *c) {
+    c->fine_bins_valid = false;                                      // new positions
+    PSE_TRY(launch_particle_window(c, c->iset, c->win_a, c->win_b));
     if (!use_block_spread(c)) return PSE_OK;
     // lists of the particles that reach every half tile: one pass, segments reserved on a cursor (cleared with the bin counters)
     const int nhalf = 2 * c->ntile;
@@ -849,15 +917,7 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
     ScopedPhase ph(c, PSE_T_INTERP);
     const int TB = 256, oplan = (mode >> 2) & 3;
     if (c->P <= 8) {
-        switch (c->P) {
-            case 2: PSE_TRY(launch_interp<2>(c, oplan, d_out, accumulate)); break;
-            case 3: PSE_TRY(launch_interp<3>(c, oplan, d_out, accumulate)); break;
-            case 4: PSE_TRY(launch_interp<4>(c, oplan, d_out, accumulate)); break;
-            case 5: PSE_TRY(launch_interp<5>(c, oplan, d_out, accumulate)); break;
-            case 6: PSE_TRY(launch_interp<6>(c, oplan, d_out, accumulate)); break;
-            case 7: PSE_TRY(launch_interp<7>(c, oplan, d_out, accumulate)); break;
-            default: PSE_TRY(launch_interp<8>(c, oplan, d_out, accumulate)); break;
-        }
+        PSE_TRY(launch_interp_any(c, c->iset, oplan, d_out, accumulate));
     } else {
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
@@ -911,10 +971,15 @@ pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out
     }
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r_b, c->d_spec_b, c->d_grid_b)); c->launches++; }
     ScopedPhase ph(c, PSE_T_INTERP);
-    const int TB = 256;
-    interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
-        c->d_pos, c->d_tile_list, c->d_grid_b, reinterpret_cast<float4 *>(d_out), c->N, Mb, c->Pb, (float)(Mb / c->L),
-        (float)c->win_a_b, (float)c->win_b_b, accumulate ? 1 : 0, PSE_MODE_ALL);
+    if (c->Pb <= 8) {
+        PSE_TRY(ensure_fine_bins(c));
+        PSE_TRY(launch_interp_any(c, c->iset_b, 3, d_out, accumulate));
+    } else {
+        const int TB = 256;
+        interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
+            c->d_pos, c->d_tile_list, c->d_grid_b, reinterpret_cast<float4 *>(d_out), c->N, Mb, c->Pb, (float)(Mb / c->L),
+            (float)c->win_a_b, (float)c->win_b_b, accumulate ? 1 : 0, PSE_MODE_ALL);
+    }
     KERNEL_CHECK(c);
     return PSE_OK;
 }
