@@ -1,6 +1,7 @@
 // C-ABI entry points of libpse (include/pse.h).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <new>
 #include "pse_internal.h"
 
@@ -177,6 +178,7 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
         CUDA_TRY(c, cudaMemcpy(c->d_dec_b, dec.data(), dec.size() * sizeof(float), cudaMemcpyHostToDevice));
     }
     CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream_cap, cudaStreamNonBlocking));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise, cudaEventDisableTiming));
     CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_noise_r, cudaEventDisableTiming));
@@ -188,10 +190,12 @@ pse_status pse_destroy(pse_ctx *c) {
     if (!c) return PSE_OK;
     cudaStreamSynchronize(c->stream);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
+    if (c->stream_cap) cudaStreamDestroy(c->stream_cap);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_noise) cudaEventDestroy(c->ev_noise);
     if (c->ev_noise_r) cudaEventDestroy(c->ev_noise_r);
     if (c->ev_nbr) cudaEventDestroy(c->ev_nbr);
+    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) cudaGraphExecDestroy(c->step_graph[g]);
     pse_wave_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
@@ -231,6 +235,17 @@ pse_status pse_mobility_apply(pse_ctx *c, const float *d_F, const float *d_S, fl
 static pse_status brownian_impl(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters,
                                 int fixed_m);
 
+// the two halves of a Brownian sample (Eq. 71): d_out = M_r^{1/2} w1 (Lanczos), then d_out += M_w^{1/2} w2 and the sqrt(2kT/dt) scaling
+static pse_status brownian_real_part(pse_ctx *c, const float *d_noise_real, int *lanczos_iters, int fixed_m) {
+    if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
+    PSE_TRY(pse_pack8(c, d_noise_real, c->d_in));
+    return pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters, fixed_m);
+}
+static pse_status brownian_wave_part(pse_ctx *c, double dt, const float *d_noise_wave, float *d_UB, float *d_EB) {
+    PSE_TRY(pse_wave_brownian(c, d_noise_wave, c->d_out, true));
+    return pse_unpack(c, c->d_out, (float)std::sqrt(2.0 * c->kT / dt), d_UB, d_EB);
+}
+
 pse_status pse_brownian(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_EB, int *lanczos_iters) {
     return brownian_impl(c, dt, d_noise_real, d_noise_wave, d_UB, d_EB, lanczos_iters, 0);
 }
@@ -239,12 +254,9 @@ static pse_status brownian_impl(pse_ctx *c, double dt, const float *d_noise_real
                                 int fixed_m) {
     if (!c || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_brownian before pse_neighbors"; return PSE_ENOTREADY; }
-    if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
-    PSE_TRY(pse_pack8(c, d_noise_real, c->d_in));
-    pse_status st = pse_lanczos_sqrt(c, c->d_in, c->d_out, lanczos_iters, fixed_m);
+    pse_status st = brownian_real_part(c, d_noise_real, lanczos_iters, fixed_m);
     if (st != PSE_OK && st != PSE_ENOCONV) return st;
-    PSE_TRY(pse_wave_brownian(c, d_noise_wave, c->d_out, true));
-    PSE_TRY(pse_unpack(c, c->d_out, (float)std::sqrt(2.0 * c->kT / dt), d_UB, d_EB));
+    PSE_TRY(brownian_wave_part(c, dt, d_noise_wave, d_UB, d_EB));
     return st;
 }
 
@@ -262,6 +274,7 @@ pse_status pse_set_bonds(pse_ctx *c, const int *h_pairs, int n_bonds, double k, 
     for (int b = 0; b < n_bonds; ++b)
         if (h_pairs[2 * b] == h_pairs[2 * b + 1]) { c->err = "pse_set_bonds: bond of a particle with itself"; return PSE_EINVAL; }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the bond array is baked in
     cudaFree(c->d_bonds); c->d_bonds = nullptr; c->n_bonds = 0;
     if (n_bonds == 0) return PSE_OK;
     CUDA_TRY(c, cudaMalloc(&c->d_bonds, (size_t)n_bonds * sizeof(int2)));
@@ -287,6 +300,45 @@ pse_status pse_constrained_solve(pse_ctx *c, const float *d_F, const float *d_UB
     return st;
 }
 
+static pse_status ensure_stage(pse_ctx *c, bool noise);
+
+// The whole mid-point step, Eqs. (76)-(79), with FIXED iteration counts and no host synchronisation: only enqueues (so it can
+// also run under stream capture).  x_k is saved in d_xk first.  *slot0 / *slot1: report slots of the two neighbour builds;
+// *single = false if the context takes the synchronous two-pass build (nothing to examine then).
+// parts: 1 = up to and including the Lanczos solve (needs the positions and the real-space noise), 2 = the rest (needs the
+// wave-space noise, the bulk of a host upload), 3 = both.
+static pse_status enqueue_step_fixed(pse_ctx *c, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave, int mL, int mG,
+                                     int *slot0, int *slot1, bool *single, int parts = 3) {
+    const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
+    const float L = (float)c->L, invL = 1.0f / L;
+    float *UB = c->d_vecD, *EB = c->d_vecD + (size_t)3 * N;
+    float4 *xh = reinterpret_cast<float4 *>(c->d_zu);
+    if (parts & 1) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_xk, d_pos, (size_t)N * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+        PSE_TRY(pse_neighbors_impl(c, d_pos));
+        *slot0 = c->nbr_last;
+        *single = c->nbr_pending;
+        PSE_TRY(brownian_real_part(c, d_noise_real, nullptr, mL));
+    }
+    if (!(parts & 2)) return PSE_OK;
+    PSE_TRY(brownian_wave_part(c, dt, d_noise_wave, UB, EB));
+    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+    PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
+    *slot1 = c->nbr_last;
+    PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
+    if (c->n_bonds) {
+        PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
+        PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
+        PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+    }
+    PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
+    PSE_TRY(pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, nullptr, mG));
+    PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));
+    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
+                                        reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
 pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave, int *gmres_iters, int *lanczos_iters) {
     if (!c || !d_pos || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
     const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
@@ -300,28 +352,77 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     // more iterations) x_k is restored and the step is redone by the checked path below, which also re-learns the counts. ----
     if (c->lanczos_budget > 0 && c->gmres_budget > 0) {
         const int mL = c->lanczos_budget, mG = c->gmres_budget;
-        CUDA_TRY(c, cudaMemcpyAsync(c->d_xk, d_pos, (size_t)N * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
-        PSE_TRY(pse_neighbors_impl(c, d_pos));
-        const int slot0 = c->nbr_last;
-        const bool single0 = c->nbr_pending;                         // false: the context takes the synchronous two-pass build
-        PSE_TRY(brownian_impl(c, dt, d_noise_real, d_noise_wave, UB, EB, nullptr, mL));
-        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
-        PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
-        PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
-        if (c->n_bonds) {
-            PSE_TRY(pse_bond_forces_orig(c, c->d_vecC));
-            PSE_TRY(pse_pack(c, c->d_vecC, nullptr, c->d_out));
-            PSE_TRY(pse_axpby(c, (size_t)8 * N, 1.f, c->d_out, 1.f, c->d_vecA));
+        int slot0 = 0, slot1 = 0;
+        bool single = true;
+        float *user_pos = nullptr;                                    // set if the step runs on the library's copy of the positions
+        // A step is ~230 launches and the host cannot enqueue them as fast as the GPU runs them (measured: 1.07 -> 0.81 ms at
+        // N = 4 096, 2.45 -> 2.17 ms at N = 65 536), so the step is replayed as CUDA graphs captured from the same enqueue code
+        // and keyed by everything that is baked into them.
+        const bool want_graph = !c->profiling && !c->nbr_two_pass && !c->graph_failed && N <= PSE_GRAPH_MAX_N;
+        bool replayed = false;
+        if (want_graph) {
+            // the graphs work on buffers of the library's own (the staging buffers of pse_step_host), so that they do not depend
+            // on where the caller keeps its arrays: three small device copies in, one out
+            PSE_TRY(ensure_stage(c, true));
+            if (d_pos != c->d_stage_pos) {
+                CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_pos, d_pos, (size_t)N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+                CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_a, d_noise_real, (size_t)N * 8 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+                CUDA_TRY(c, cudaMemcpyAsync(c->d_stage_noise, d_noise_wave, (size_t)6 * c->M * c->M * c->Mh * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+                user_pos = d_pos;
+                d_pos = c->d_stage_pos; d_noise_real = c->d_stage_a; d_noise_wave = c->d_stage_noise;
+            }
+            const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap};
+            if (!c->step_graph[0] || !(key == c->graph_key)) {
+                for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
+                const long long l0 = c->launches;
+                // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot capture), in
+                // two graphs: [neighbour build, Lanczos] and [wave part of the sample, mid-point, build, solve, update]; the uploads
+                // that pse_step_host has in flight on its second stream are waited for between them, not before them
+                cudaStream_t user = c->stream;
+                const bool pr = c->noise_r_pending, pw = c->noise_pending;
+                c->noise_r_pending = c->noise_pending = false;        // no event waits inside a capture
+                c->stream = c->stream_cap;
+                pse_wave_set_stream(c, c->stream);
+                bool ok = true;
+                for (int g = 0; g < 2 && ok; ++g) {
+                    cudaGraph_t gr = nullptr;
+                    ok = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+                    if (ok) {
+                        const pse_status es = enqueue_step_fixed(c, d_pos, dt, d_noise_real, d_noise_wave, mL, mG, &slot0, &slot1, &single, 1 << g);
+                        ok = cudaStreamEndCapture(c->stream, &gr) == cudaSuccess && es == PSE_OK && gr;
+                    }
+                    if (ok) ok = cudaGraphInstantiate(&c->step_graph[g], gr, 0) == cudaSuccess;
+                    if (gr) cudaGraphDestroy(gr);
+                }
+                c->stream = user;
+                pse_wave_set_stream(c, c->stream);
+                c->noise_r_pending = pr; c->noise_pending = pw;
+                if (!ok || !single) {                                 // capture not possible here: plain enqueue from now on
+                    cudaGetLastError();
+                    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
+                    c->graph_failed = true;
+                } else {
+                    c->graph_key = key; c->graph_slot0 = slot0; c->graph_slot1 = slot1; c->graph_launches = c->launches - l0;
+                }
+                c->launches = l0;
+            }
+            if (c->step_graph[0] && !c->graph_failed) {
+                if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
+                CUDA_TRY(c, cudaGraphLaunch(c->step_graph[0], c->stream));
+                if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
+                CUDA_TRY(c, cudaGraphLaunch(c->step_graph[1], c->stream));
+                slot0 = c->graph_slot0; slot1 = c->graph_slot1;
+                c->launches += c->graph_launches;
+                c->nbr_pending = false; c->fine_bins_valid = false; c->have_nbrs = true;
+                replayed = true;
+            }
         }
-        PSE_TRY(pse_pack(c, UB, EB, c->d_vecB));
-        PSE_TRY(pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, nullptr, mG));
-        PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));
-        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
-                                            reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+        if (!replayed) PSE_TRY(enqueue_step_fixed(c, d_pos, dt, d_noise_real, d_noise_wave, mL, mG, &slot0, &slot1, &single));
+        if (user_pos) CUDA_TRY(c, cudaMemcpyAsync(user_pos, d_pos, (size_t)N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        c->nbr_pending = false;
         bool redo0 = false, redo1 = false, shrinkL = false, shrinkG = false;
-        if (single0) PSE_TRY(pse_neighbors_examine(c, slot0, &redo0));
-        PSE_TRY(pse_neighbors_settle(c, &redo1));
+        if (single) { PSE_TRY(pse_neighbors_examine(c, slot0, &redo0)); PSE_TRY(pse_neighbors_examine(c, slot1, &redo1)); }
         const bool okL = pse_lanczos_validate(c, mL, &shrinkL), okG = pse_gmres_validate(c, mG, &shrinkG);
         if (!redo0 && !redo1 && okL && okG) {
             if (shrinkL && mL > 2) c->lanczos_budget = mL - 1;
@@ -331,6 +432,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
             return PSE_OK;
         }
         c->lanczos_budget = c->gmres_budget = 0;                      // re-learn
+        if (user_pos) { d_pos = user_pos; user_pos = nullptr; }      // back to the caller's array (its noise copies stay valid)
         CUDA_TRY(c, cudaMemcpyAsync(d_pos, c->d_xk, (size_t)N * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
     }
     // ---- checked path.  The neighbour builds are only enqueued; what they report (list size, overflow, oversized cell) is examined after the

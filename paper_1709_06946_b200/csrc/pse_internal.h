@@ -18,7 +18,18 @@
 // is S -> E only, so 5 + 5 grids are spread / transformed / interpolated instead of 8 + 8.
 enum { PSE_IN_F = 1, PSE_IN_S = 2, PSE_OUT_U = 4, PSE_OUT_E = 8, PSE_MODE_ALL = 15 };
 
+#define PSE_GRAPH_MAX_N (1 << 30)  // pse_step replays captured CUDA graphs up to this many particles (all sizes: it pays everywhere measured)
+
 struct Timer { cudaEvent_t a, b; int phase; };
+
+// everything baked into the captured graph of a step
+struct StepGraphKey {
+    const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap;
+    bool operator==(const StepGraphKey &o) const {
+        return pos == o.pos && noise_real == o.noise_real && noise_wave == o.noise_wave && dt == o.dt && mL == o.mL && mG == o.mG &&
+               n_bonds == o.n_bonds && nbr_cap == o.nbr_cap;
+    }
+};
 
 // Everything the tiled interpolation needs about one grid: the product grid (M, P) or the finer grid of the Brownian pass.
 struct InterpSet {
@@ -51,6 +62,7 @@ struct pse_ctx {
     int device = 0, nsm = 0;                 // device the context lives on (recorded at pse_create), its SM count
     int coop_cap = 0;                        // largest cooperative grid of the Krylov step kernels on that device
     cudaStream_t stream2 = nullptr;          // pse_step_host uploads the noise here while the step starts on `stream`
+    cudaStream_t stream_cap = nullptr;       // pse_step's graph is captured here (the caller's stream may be the legacy default stream)
     cudaEvent_t ev_fork = nullptr, ev_noise = nullptr, ev_noise_r = nullptr;
     bool noise_r_pending = false;            // pse_step_host: the real-space noise upload on stream2 has not been waited for yet
     bool noise_pending = false;              // pse_step_host: the wave-noise upload on stream2 has not been waited for yet
@@ -107,6 +119,9 @@ struct pse_ctx {
     double *h_scal_l = nullptr;              // pinned mirror of the Lanczos scalars of a fixed-count solve (pse_step's optimistic path)
     int lanczos_budget = 0, gmres_budget = 0;   // iteration counts the last completed step needed; 0 = not known yet
     float4 *d_xk = nullptr;                  // [N] copy of x_k while an optimistic step is in flight
+    cudaGraphExec_t step_graph[2] = {nullptr, nullptr};   // the fixed-count step as two graphs: [build, Lanczos], [wave sample ... update]
+    StepGraphKey graph_key = {};
+    int graph_slot0 = 0, graph_slot1 = 0; long long graph_launches = 0; bool graph_failed = false; int graph_recaptures = 0;
     float *d_coef = nullptr;                 // small coefficient vector upload
     int last_lanczos_iters = 0, last_gmres_iters = 0;   // iteration counts of the previous solves (when to start reading back)
     int lanczos_repeats = 0, gmres_repeats = 0;         // how many solves in a row ended with that same count
@@ -204,6 +219,7 @@ pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode 
 // wavespace.cu
 pse_status pse_wave_init(pse_ctx *c);
 void pse_wave_free(pse_ctx *c);
+void pse_wave_set_stream(pse_ctx *c, cudaStream_t st);    // stream of the cuFFT plans
 pse_status pse_tile_bins(pse_ctx *c);
 pse_status pse_particle_windows(pse_ctx *c);   // d_pbase, d_pw from d_pos (after the cell sort)
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode = PSE_MODE_ALL);   // out (+)= M_w in

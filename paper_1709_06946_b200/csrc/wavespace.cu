@@ -834,6 +834,11 @@ pse_status pse_wave_init(pse_ctx *c) {
     return PSE_OK;
 }
 
+void pse_wave_set_stream(pse_ctx *c, cudaStream_t st) {
+    for (int i = 0; i < c->nplans; ++i) { cufftSetStream(c->plan_r2c[i], st); cufftSetStream(c->plan_c2r[i], st); }
+    if (c->have_plan_b) cufftSetStream(c->plan_c2r_b, st);
+}
+
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     if (c->have_plan_b) cufftDestroy(c->plan_c2r_b);
