@@ -509,3 +509,43 @@ def test_host_buffer_entry_points_match_device_ones():
     ctx_h.pse_mobility_apply_host(pos_h, torch.from_numpy(F.astype(np.float32)).pin_memory(), torch.from_numpy(S.astype(np.float32)).pin_memory(), Uh, Eh)
     assert np.array_equal(Ud, Uh.numpy()) and np.array_equal(Ed, Eh.numpy())
     ctx_d.close(); ctx_h.close()
+
+
+def test_bitwise_reproducible_across_contexts_and_repeats():
+    """Stand-in for a race detector (compute-sanitizer is closed on this GPU pool): every kernel on the path has a fixed summation
+    order (gather-form spread, ballot-ordered lists, 8-lane shuffle reductions), so two fresh contexts and repeated calls must
+    agree BITWISE on the neighbour lists as sets, every masked product, the Brownian sample and three consecutive steps (checked
+    path, then the fixed-count path replayed as CUDA graphs).  A shared-memory race or an atomics-ordered sum would break this."""
+    import paper_1709_06946_b200 as pse
+    N, tol, xi, dt = 20000, 1e-3, 0.55, 1e-4
+    x, L = synth.rsa(N, 0.30, seed=61)
+    x32 = x.astype(np.float32)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    F, S = synth.gaussian_inputs(N, 6)
+    w1, w2 = synth.brownian_noise(N, grid, 6)
+    outs = []
+    for rep in range(2):
+        ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+        pos = dev(pos4(x32))
+        ctx.pse_neighbors(pos)
+        o = {'sets': [s.tobytes() for s in nbr_sets_from_gpu(ctx)[:200]]}
+        for name, (f, s_, u, e) in {'all': (1, 1, 1, 1), 'se': (0, 1, 0, 1), 'fe': (1, 0, 0, 1), 'fsu': (1, 1, 1, 0)}.items():
+            U, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+            for _ in range(2):                      # repeated call on the same context
+                ctx.pse_mobility_apply(dev(F) if f else None, dev(S) if s_ else None, U if u else None, E if e else None, 3)
+                key = name + str(_)
+                o[key] = (U.cpu().numpy().tobytes() if u else b'') + (E.cpu().numpy().tobytes() if e else b'')
+            assert o[name + '0'] == o[name + '1']
+        UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+        ctx.pse_brownian(dt, dev(w1.reshape(N, 8)), dev(w2), UB, EB)
+        o['brownian'] = UB.cpu().numpy().tobytes() + EB.cpu().numpy().tobytes()
+        its = []
+        for k in range(3):
+            its.append(ctx.pse_step(pos, dt, dev(w1.reshape(N, 8)), dev(w2)))
+        o['steps'] = pos.cpu().numpy().tobytes()
+        o['its'] = its
+        outs.append(o)
+        ctx.close()
+    for key in outs[0]:
+        assert outs[0][key] == outs[1][key], key
