@@ -221,56 +221,55 @@ __global__ void __launch_bounds__(VT) k_arnoldi_step(float4 *w, const float4 *Z,
 // the loop: pse_step enqueues both solves with the counts the previous step needed and looks at the scalars only afterwards ----
 
 // coef[0..m) = |w| T_m^{1/2} e_1 for the Lanczos tridiagonal T_m (alpha_j on the diagonal, beta_j next to it), by the implicit
-// QL iteration with Wilkinson shift (EISPACK imtql2) on (d, e) with the eigenvector rows spread over the lanes.
+// QL iteration with Wilkinson shift (EISPACK imtql2).  Every lane carries its own copy of (d, e) and runs the scalar recurrence
+// redundantly (identical values, no exchange, no barrier); lane k accumulates row k (and k + 32) of the eigenvector matrix.
 // scal: [0] = |w|^2, [1 + 2j] = alpha_j, [2 + 2j] = beta_j^2.
 __global__ void __launch_bounds__(32) k_lanczos_coef_dev(const double *__restrict__ scal, int m, float *__restrict__ coef) {
-    __shared__ double Z[PSE_MAX_KRYLOV][PSE_MAX_KRYLOV + 1], d[PSE_MAX_KRYLOV], e[PSE_MAX_KRYLOV];
+    __shared__ double z0[PSE_MAX_KRYLOV];                 // row 0 of the eigenvector matrix (first components), for the last step
+    double d[PSE_MAX_KRYLOV], e[PSE_MAX_KRYLOV], za[PSE_MAX_KRYLOV], zb[PSE_MAX_KRYLOV];
     const int lane = threadIdx.x;
-    for (int i = lane; i < m; i += 32) { d[i] = scal[1 + 2 * i]; e[i] = i + 1 < m ? sqrt(fmax(scal[2 + 2 * i], 0.0)) : 0.0; }
-    for (int i = lane; i < m; i += 32) for (int j = 0; j < m; ++j) Z[i][j] = i == j ? 1.0 : 0.0;
-    __syncwarp();
+    for (int i = 0; i < m; ++i) {
+        d[i] = scal[1 + 2 * i]; e[i] = i + 1 < m ? sqrt(fmax(scal[2 + 2 * i], 0.0)) : 0.0;
+        za[i] = i == lane ? 1.0 : 0.0; zb[i] = i == lane + 32 ? 1.0 : 0.0;
+    }
     for (int l = 0; l < m; ++l) {
         for (int iter = 0; iter < 60; ++iter) {
             int mm = l;
             for (; mm < m - 1; ++mm) { const double dd = fabs(d[mm]) + fabs(d[mm + 1]); if (fabs(e[mm]) <= 2e-16 * dd) break; }
             if (mm == l) break;
-            double g = (d[l + 1] - d[l]) / (2.0 * e[l]), r = hypot(g, 1.0);
-            g = d[mm] - d[l] + e[l] / (g + (g >= 0 ? fabs(r) : -fabs(r)));
+            double g = (d[l + 1] - d[l]) / (2.0 * e[l]), r = sqrt(g * g + 1.0);
+            g = d[mm] - d[l] + e[l] / (g + (g >= 0 ? r : -r));
             double sn = 1.0, cs = 1.0, pp = 0.0;
             int i = mm - 1;
             bool under = false;
             for (; i >= l; --i) {
                 double f = sn * e[i];
                 const double b = cs * e[i];
-                r = hypot(f, g);
-                __syncwarp();
-                if (lane == 0) e[i + 1] = r;
-                if (r == 0.0) { if (lane == 0) { d[i + 1] -= pp; e[mm] = 0.0; } under = true; __syncwarp(); break; }
-                sn = f / r; cs = g / r;
+                r = sqrt(f * f + g * g);
+                e[i + 1] = r;
+                if (r == 0.0) { d[i + 1] -= pp; e[mm] = 0.0; under = true; break; }
+                const double ir = 1.0 / r;
+                sn = f * ir; cs = g * ir;
                 g = d[i + 1] - pp;
                 r = (d[i] - g) * sn + 2.0 * cs * b;
                 pp = sn * r;
-                __syncwarp();
-                if (lane == 0) d[i + 1] = g + pp;
+                d[i + 1] = g + pp;
                 g = cs * r - b;
-                for (int k = lane; k < m; k += 32) {                   // eigenvector rows over the lanes
-                    f = Z[k][i + 1];
-                    Z[k][i + 1] = sn * Z[k][i] + cs * f;
-                    Z[k][i] = cs * Z[k][i] - sn * f;
-                }
-                __syncwarp();
+                f = za[i + 1]; za[i + 1] = sn * za[i] + cs * f; za[i] = cs * za[i] - sn * f;        // my rows of the eigenvectors
+                if (m > 32) { f = zb[i + 1]; zb[i + 1] = sn * zb[i] + cs * f; zb[i] = cs * zb[i] - sn * f; }
             }
             if (under) continue;
-            __syncwarp();
-            if (lane == 0) { d[l] -= pp; e[l] = g; e[mm] = 0.0; }
-            __syncwarp();
+            d[l] -= pp; e[l] = g; e[mm] = 0.0;
         }
     }
+    if (lane == 0) for (int k = 0; k < m; ++k) z0[k] = za[k];
     __syncwarp();
     const double wn = sqrt(fmax(scal[0], 0.0));
-    for (int i = lane; i < m; i += 32) {
+    for (int half = 0; half < 2; ++half) {
+        const int i = lane + 32 * half;
+        if (i >= m) break;
         double acc = 0.0;
-        for (int k = 0; k < m; ++k) acc += Z[i][k] * sqrt(fmax(d[k], 0.0)) * Z[0][k];
+        for (int k = 0; k < m; ++k) acc += (half ? zb[k] : za[k]) * sqrt(fmax(d[k], 0.0)) * z0[k];
         coef[i] = (float)(wn * acc);
     }
 }
