@@ -77,15 +77,15 @@ class ClockSampler:
                 'samples': len(sm)}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r1_traffic.md), default workload only; other workloads report null.
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/r2_traffic.md), default
+# workloads only; other workloads report null.
 # fp32 operations per pair evaluation of real_pairs_kernel (ncu: fadd + fmul + 2 ffma predicated-on thread instructions / pairs,
-# profiles/r1_ncu_kernels.md): 162 for the full 8 x 8 product (Lanczos iterations), 129 for S -> E (GMRES iterations); a step runs
-# seven of each plus two mixed products, so their mean is used
+# profiles/r1_ncu_kernels.md; the kernel is unchanged since): 162 for the full 8 x 8 product (Lanczos iterations), 129 for S -> E
+# (GMRES iterations); a step runs seven of each plus two mixed products, so their mean is used
 FLOP_PER_PAIR = 0.5 * (162.0 + 129.0)
 N_SM, FP32_LANES_PER_SM = 148, 128                # B200: 4 sub-partitions x 32 fp32 lanes per SM (blackwell guide), FMA = 2 flop
-NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 3479552, 'interp': 23429376, 'scale': 20021760, 'neighbors': 1100800},
-               'config4': {'real': 374564352, 'spread': 327781888, 'interp': 288555520, 'scale': 347489536, 'neighbors': 251551488}}   # profiles/r1_config4.md
+NCU_TRAFFIC = {'config3': {'real': 17375488, 'spread': 6934784, 'interp': 25789440, 'scale': 12053760, 'neighbors': 1096704},
+               'config4': {'real': 372716288, 'spread': 264503808, 'interp': 327649280, 'scale': 271386112, 'neighbors': 251827968}}
 
 
 def max_over_ranks(ms, device=None):

@@ -1,17 +1,18 @@
 // Wave-space half of the product: M_w = sigma Q^T F^H P^H B P F Q (Eq. 42) and the Brownian factor
 // M_w^{1/2} = sigma^{1/2} Q^T F^H P^H B^{1/2} (Eq. 75).  Steps a3-a7 of SURVEY.md §8(a).
 //
-// Grid layout: 8 planar real grids [c][ix][iy][iz] (iz fastest), grid point n at n*h; half spectrum
-// [c][ix][iy][iz<=M/2].  c = (Fx,Fy,Fz,S1..S5) going in, (Ux,Uy,Uz,E1..E5) coming out.
-// Gaussian (R3-R5): K(r) = (2 xi^2/(pi eta_g))^{3/2} exp(-2 xi^2 r^2/eta_g) with
-// eta_g = (h P xi/m)^2, m = sqrt(pi P), so on the grid K ~ exp(-(2 pi/P) t^2), t = distance in grid units: the
-// weights depend on P only.  All constant prefactors (both Gaussians' normalisation, h^3 of the two quadratures,
-// 1/V) are folded into the scale kernel: (2/P)^3/V for the product, (2/P)^{3/2}/sqrt(V) for the Brownian factor.
+// Grid layout: 8 planar real grids [c][ix][iy][iz] (iz fastest, planes pse_plane_stride(M) floats apart), grid point n at
+// n*h; half spectrum [c][ix][iy][iz<=M/2].  c = (Fx,Fy,Fz,S1..S5) going in, (Ux,Uy,Uz,E1..E5) coming out.
+// Window of Q / Q^T on its P^3 support (R3-R5): exponential of semicircle by default, the paper's Gaussian
+// exp(-(2 pi/P) t^2) (eta_g = (h P xi/m)^2, m = sqrt(pi P)) on request; its continuous transform is divided out
+// per dimension in the scale kernels (table d_dec), together with 1/V, so all normalisation lives there.
 //
-// Spread is written in GATHER form (not the paper's per-particle atomics): one CTA owns an 8^3 tile
-// of grid points, one thread per point with the 8 components in registers; it walks the particles binned in the
-// tiles whose supports can reach it, with separable weights staged in shared memory.  No atomics, no memset,
-// each grid value is written exactly once with full-sector coalesced stores, and the summation order is fixed.
+// What runs where:
+//   pse_neighbors   particle_window_kernel (support base + window values per particle, tile order), half_lists_kernel
+//   spread          spread_blocks_kernel (P <= 8: lane owns 2x2x2 grid points, gather form, register accumulators, lists),
+//                   spread_kernel (generic gather for wider supports / tiny grids); no atomics, no memset, fixed order
+//   scale           scale_kernel (P^H B P), scale_brownian_kernel (P^H B^{1/2} W on the finer grid of the Brownian pass)
+//   interpolate     interp_planes_kernel (P <= 8: TMA-staged tile block, 8 lanes per particle), interp_kernel (generic)
 #include <algorithm>
 #include <cuda_pipeline.h>
 #include "pse_internal.h"
