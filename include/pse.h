@@ -100,6 +100,23 @@ pse_status pse_constrained_solve(pse_ctx *ctx, const float *d_F, const float *d_
  * DESIGN.md reading R12): F_i = sum_{j: r_ij<2a} 3 pi eta a (2a - r_ij)/dt rhat_ij.  d_F [N][3] out. */
 pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);
 
+/* The same force for callers that cannot call cudaMalloc (under CUDA-graph capture, in a serving loop, in a harness that
+ * forbids it): no context, no allocation of any kind.  The linked-cell scratch (cell heads + per-particle links) is a
+ * static __device__ array of PSE_NOALLOC_SCRATCH_BYTES (5 MiB) that every GPU holding the library keeps until exit.
+ *   N <= PSE_NOALLOC_MAX_N particles (PSE_EOVERFLOW beyond, nothing is launched); L >= 4a (PSE_EINVAL: minimum image);
+ *   d_pos [N][4] device, may be unwrapped; d_F [N][3] device, overwritten, original numbering; cuda_stream = the stream
+ *   the three operations (clear heads, link, forces) are enqueued on, on the CURRENT device (NULL = legacy default).
+ *   h_err: HOST buffer of h_err_cap bytes receiving a message on failure (may be NULL).  Asynchronous.
+ * All calls share the one array: calls on one stream are ordered; calls that overlap on the GPU (two streams, two
+ * threads) race and give garbage.  Nothing is kept between calls.  The first call on a device looks up the array's
+ * device address (cudaGetSymbolAddress): make it before a capture begins.  The sum over overlapping partners runs
+ * in a fixed order (neighbour cells, ascending particle index), so repeated calls agree bit for bit; against
+ * pse_hard_sphere_forces the per-pair terms are identical and only the fp32 summation order differs. */
+#define PSE_NOALLOC_MAX_N 1048576
+#define PSE_NOALLOC_SCRATCH_BYTES 5242880
+pse_status pse_hard_sphere_forces_noalloc(int N, double L, double a, double eta, double dt, const float *d_pos, float *d_F,
+                                          void *cuda_stream, char *h_err, size_t h_err_cap);
+
 /* Bonds with the pair potential U(r) = k |r - r0| of the paper's equilibrium test (its Boltzmann
  * distribution of r is Eq. (80)).  h_pairs: HOST array [n_bonds][2] of particle indices (copied);
  * n_bonds = 0 removes all bonds.  pse_step adds the bond forces, evaluated at x_{k+1/2} with the minimum image, to F^P.

@@ -14,12 +14,13 @@ LIB_PATH = os.path.join(_HERE, 'libpse.so')
 PSE_OK, PSE_EINVAL, PSE_ENOMEM, PSE_ECUDA, PSE_ECUFFT, PSE_ENOTREADY, PSE_ENOCONV, PSE_EOVERFLOW = range(8)
 PSE_REAL, PSE_WAVE, PSE_BOTH = 1, 2, 3
 PSE_WINDOW_GAUSS, PSE_WINDOW_ES = 0, 1
+PSE_NOALLOC_MAX_N = 1 << 20
 PHASES = ('neighbors', 'real', 'spread', 'fft_fwd', 'scale', 'fft_inv', 'interp', 'vector', 'pack')
 _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PSE_ECUFFT', 5: 'PSE_ENOTREADY',
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
 EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
-           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
 
@@ -45,6 +46,7 @@ def load_library():
     lib.pse_brownian.argtypes = [vp, dbl, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
+    lib.pse_hard_sphere_forces_noalloc.argtypes = [i32, dbl, dbl, dbl, dbl, vp, vp, vp, C.c_char_p, C.c_size_t]
     lib.pse_set_bonds.argtypes = [vp, vp, i32, dbl, dbl]
     lib.pse_bond_forces.argtypes = [vp, vp]
     lib.pse_step.argtypes = [vp, vp, dbl, vp, vp, C.POINTER(i32), C.POINTER(i32)]
@@ -94,6 +96,17 @@ def pse_suggest_params(N, L, a, tol, xi, window=PSE_WINDOW_ES):
     g, p, rc = C.c_int(), C.c_int(), C.c_double()
     st = _lib.pse_suggest_params_window(N, L, a, tol, xi, window, C.byref(g), C.byref(p), C.byref(rc))
     return st, g.value, p.value, rc.value
+
+
+def pse_hard_sphere_forces_noalloc(L, a, eta, dt, pos, F, stream=None):
+    """Heyes-Melrose overlap forces without a context and without any allocation (static device scratch; see include/pse.h).
+    pos [N][4], F [N][3] CUDA float32 tensors on the current device; N <= PSE_NOALLOC_MAX_N."""
+    N = int(pos.shape[0]) if isinstance(pos, torch.Tensor) and pos.dim() == 2 else -1
+    msg = C.create_string_buffer(256)
+    sp = C.c_void_p(stream.cuda_stream) if stream is not None else None
+    st = _lib.pse_hard_sphere_forces_noalloc(N, L, a, eta, dt, _ptr(pos, (N, 4)), _ptr(F, (N, 3)), sp, msg, len(msg))
+    if st != PSE_OK:
+        raise PSEError(st, msg.value.decode())
 
 
 class Context:
