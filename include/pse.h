@@ -96,6 +96,26 @@ pse_status pse_brownian(pse_ctx *ctx, double dt, const float *d_noise_real, cons
 pse_status pse_constrained_solve(pse_ctx *ctx, const float *d_F, const float *d_UB, const float *d_EB,
                                  float *d_U, float *d_S, int *gmres_iters);
 
+/* The full couplet of Eq. (31): [U; Omega; E] = M [F; L; S] with the torque L and the angular velocity Omega
+ * of Eqs. (32), (34) beside force, stresslet, velocity and rate of strain.  Conventions (reading R21:
+ * the paper's index order in Eqs. (4)/(8)/(16) and the sign of Eq. (32) disagree with each other, so the
+ * physics decides): a torque acts on the fluid as the force density (1/2) curl(L delta), Omega is the sphere average of
+ * (1/2) curl u, both with the couplet shape factor 3 j1(ka)/ka: an isolated sphere turns with L/(8 pi eta a^3),
+ * a torque on beta moves alpha with L x r/(8 pi eta r^3), r = x_alpha - x_beta > 2a.  The matrix stays symmetric positive
+ * semi-definite; its force / stresslet block is pse_mobility_apply's.
+ * d_F [N][3], d_L [N][3], d_S [N][5] in (any may be NULL = 0, not all); d_U [N][3], d_W [N][3] (Omega), d_E [N][5] out (any may
+ * be NULL, not all).  which = PSE_REAL | PSE_WAVE | PSE_BOTH.  The first call allocates the torque planes (3 spectra, 3 packed
+ * vectors, one table) and synchronises once; later calls are asynchronous.  PSE_ENOTREADY before pse_neighbors. */
+pse_status pse_mobility_apply_full(pse_ctx *ctx, const float *d_F, const float *d_L, const float *d_S,
+                                   float *d_U, float *d_W, float *d_E, int which);
+
+/* pse_constrained_solve with torques (Eqs. 36-38, with script-F = [F; L], script-U = [U; Omega]):
+ * M_ES S = -(E^B + M_EF F + M_EL L) by GMRES, then U = U^B + M_UF F + M_UL L + M_US S and Omega = M_OF F + M_OL L + M_OS S.
+ * d_F, d_L, d_UB, d_EB may be NULL (= 0); d_U [N][3], d_S [N][5] out; d_W [N][3] out, may be NULL (one product less).
+ * No Brownian angular velocity enters: orientations of spheres are not tracked (R21). */
+pse_status pse_constrained_solve_full(pse_ctx *ctx, const float *d_F, const float *d_L, const float *d_UB, const float *d_EB,
+                                      float *d_U, float *d_W, float *d_S, int *gmres_iters);
+
 /* Heyes-Melrose hard-sphere overlap force at the current positions (named by BASELINE.json, not the paper;
  * DESIGN.md reading R12): F_i = sum_{j: r_ij<2a} 3 pi eta a (2a - r_ij)/dt rhat_ij.  d_F [N][3] out. */
 pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);

@@ -20,7 +20,7 @@ _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PS
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
 EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
-           'pse_constrained_solve', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_constrained_solve', 'pse_mobility_apply_full', 'pse_constrained_solve_full', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
 
@@ -46,6 +46,8 @@ def load_library():
     lib.pse_brownian.argtypes = [vp, dbl, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
+    lib.pse_mobility_apply_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32]
+    lib.pse_constrained_solve_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces_noalloc.argtypes = [i32, dbl, dbl, dbl, dbl, vp, vp, vp, C.c_char_p, C.c_size_t]
     lib.pse_set_bonds.argtypes = [vp, vp, i32, dbl, dbl]
     lib.pse_bond_forces.argtypes = [vp, vp]
@@ -157,6 +159,19 @@ class Context:
         it = C.c_int()
         self._check(_lib.pse_constrained_solve(self._h, _ptr(F, (N, 3)), _ptr(UB, (N, 3)), _ptr(EB, (N, 5)),
                                                _ptr(U, (N, 3)), _ptr(S, (N, 5)), C.byref(it)))
+        return it.value
+
+    def pse_mobility_apply_full(self, F, Lq, S, U, W, E, which=PSE_BOTH):
+        """[U; Omega; E] = M [F; L; S] (torque Lq [N][3] in, angular velocity W [N][3] out); any tensor may be None."""
+        N = self.N
+        self._check(_lib.pse_mobility_apply_full(self._h, _ptr(F, (N, 3)), _ptr(Lq, (N, 3)), _ptr(S, (N, 5)),
+                                                 _ptr(U, (N, 3)), _ptr(W, (N, 3)), _ptr(E, (N, 5)), which))
+
+    def pse_constrained_solve_full(self, F, Lq, UB, EB, U, W, S):
+        N = self.N
+        it = C.c_int()
+        self._check(_lib.pse_constrained_solve_full(self._h, _ptr(F, (N, 3)), _ptr(Lq, (N, 3)), _ptr(UB, (N, 3)), _ptr(EB, (N, 5)),
+                                                    _ptr(U, (N, 3)), _ptr(W, (N, 3)), _ptr(S, (N, 5)), C.byref(it)))
         return it.value
 
     def pse_hard_sphere_forces(self, dt, F):

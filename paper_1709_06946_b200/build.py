@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, 'csrc')
 LIB = os.path.join(HERE, 'libpse.so')
-SOURCES = ['tables.cu', 'neighbors.cu', 'realspace.cu', 'wavespace.cu', 'krylov.cu', 'api.cu', 'noalloc.cu']
+SOURCES = ['tables.cu', 'neighbors.cu', 'realspace.cu', 'wavespace.cu', 'krylov.cu', 'api.cu', 'couplet.cu', 'noalloc.cu']
 CUDA_HOME = os.environ.get('CUDA_HOME', '/usr/local/cuda')
 
 

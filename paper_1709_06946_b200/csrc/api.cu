@@ -197,6 +197,7 @@ pse_status pse_destroy(pse_ctx *c) {
     if (c->ev_nbr) cudaEventDestroy(c->ev_nbr);
     for (int g = 0; g < 2; ++g) if (c->step_graph[g]) cudaGraphExecDestroy(c->step_graph[g]);
     pse_wave_free(c);
+    pse_couplet_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     cudaFree(c->d_table); cudaFree(c->d_pos); cudaFree(c->d_posw); cudaFree(c->d_order); cudaFree(c->d_order_tmp); cudaFree(c->d_tile_tmp); cudaFree(c->d_cell_of);
     cudaFree(c->d_bins); cudaFree(c->d_cell_start); cudaFree(c->d_nbr_count);

@@ -1,0 +1,265 @@
+// Full couplet: [U; Omega; E] = M [F; L; S], Eq. (31) with the decomposition of Eqs. (32)-(35)
+// (PAPER.md:175-185).  The force / stresslet block is the tuned 8-component path; this file adds the torque and
+// angular-velocity rows around it without touching it (reading R21 fixes the conventions by the physics:
+// a torque acts on the fluid as (1/2) curl(L delta), the angular velocity is the sphere average of (1/2) curl u, both
+// with the couplet shape factor s1 = 3 j1(ka)/ka of PAPER.md:111):
+//
+//   wave space   fh = s0 Fh + (i/2) s1 k x Lh - i s1 Sh.k ;  uh = B (I - kh kh) fh ;
+//                Uh = s0 uh ;  Omega_h = (i/2) s1 k x uh ;  Eh^q = i s1 (e^q k).uh
+//                -> the torque is spread on 3 planes of its own and transformed into c->d_spec_rot, ONE scaling kernel reads the
+//                   11 spectra and writes 11, the three Omega planes come back through the same 3-plane transform and interpolation.
+//   real space   U     += T' L x rh
+//                Omega += T' F x rh + Y0 L + Y2 (rh rh.L - L/3) + 2 Y2 (S rh) x rh
+//                E     += 2 Y2 sym[ rh (x) (rh x L) ]
+//                with (T', Y0, Y2) = (T/2, Z0/6, Z2/4)/(6 pi eta a), T = G1 - G2 (the antisymmetric part of Eq. 26), from a
+//                table of their own at the nodes of the main table (tables.cu).  A second sweep over the neighbour list, eight
+//                lanes per particle as in the pair kernel; it adds to the 8-component result and writes Omega.
+#include <algorithm>
+#include <cmath>
+#include "pse_internal.h"
+#include "wave_scale.cuh"
+
+pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode);
+
+namespace {
+
+constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
+
+__global__ void __launch_bounds__(256)
+real_rot_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, const float4 *__restrict__ inL, float *__restrict__ out8,
+                float *__restrict__ outW, int N, const unsigned long long *__restrict__ off, const int *__restrict__ cnt,
+                const int *__restrict__ idx, const float4 *__restrict__ table, float inv_dr, float L, float invL) {
+    __shared__ float4 tab[PSE_NTAB];
+    for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) tab[i] = table[i];
+    __syncthreads();
+    const int gl = threadIdx.x & 7, grp = (threadIdx.x & 31) >> 3, wpb = blockDim.x >> 5;
+    for (int ws = blockIdx.x * wpb + (threadIdx.x >> 5); ws * 4 < N; ws += gridDim.x * wpb) {     // warp = four particles
+        const int s = ws * 4 + grp;
+        const bool live = s < N;
+        const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float acc[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};          // dU (3), dE (5), Omega (3)
+        const unsigned long long lo = live ? off[s] : 0ull, hi = lo + (unsigned long long)(live ? cnt[s] : 0);
+        for (unsigned long long j = lo + gl; j < hi; j += 8) {
+            const int b = idx[j];
+            const float4 q4 = pos[b], a0 = in8[2 * b], a1 = in8[2 * b + 1], l4 = inL[2 * b];
+            float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
+            dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float rinv = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * rinv;
+            const float rx = dx * rinv, ry = dy * rinv, rz = dz * rinv;
+            const float tt = r * inv_dr;
+            const int it = min((int)tt, PSE_NTAB - 2);
+            const float w1 = tt - (float)it, w0 = 1.f - w1;
+            const float4 ta = tab[it], tb = tab[it + 1];
+            const float Tq = w0 * ta.x + w1 * tb.x, Y0 = w0 * ta.y + w1 * tb.y, Y2 = w0 * ta.z + w1 * tb.z;
+            // L x rh, F x rh
+            const float cx = l4.y * rz - l4.z * ry, cy = l4.z * rx - l4.x * rz, cz = l4.x * ry - l4.y * rx;
+            const float gx = a0.y * rz - a0.z * ry, gy = a0.z * rx - a0.x * rz, gz = a0.x * ry - a0.y * rx;
+            acc[0] += Tq * cx; acc[1] += Tq * cy; acc[2] += Tq * cz;
+            // t = S rh from the 5 coordinates
+            const float sxx = a0.w * RS2 - a1.x * RS6, syy = -a0.w * RS2 - a1.x * RS6, szz = 2.f * a1.x * RS6;
+            const float sxy = a1.y * RS2, sxz = a1.z * RS2, syz = a1.w * RS2;
+            const float tx = sxx * rx + sxy * ry + sxz * rz, ty = sxy * rx + syy * ry + syz * rz, tz = sxz * rx + syz * ry + szz * rz;
+            const float rl = rx * l4.x + ry * l4.y + rz * l4.z, Y22 = 2.f * Y2, third = 1.f / 3.f;
+            acc[8] += Tq * gx + Y0 * l4.x + Y2 * (rx * rl - third * l4.x) + Y22 * (ty * rz - tz * ry);
+            acc[9] += Tq * gy + Y0 * l4.y + Y2 * (ry * rl - third * l4.y) + Y22 * (tz * rx - tx * rz);
+            acc[10] += Tq * gz + Y0 * l4.z + Y2 * (rz * rl - third * l4.z) + Y22 * (tx * ry - ty * rx);
+            // E += sym[rh (x) w], w = 2 Y2 (rh x L) = -2 Y2 (L x rh)
+            const float wx = -Y22 * cx, wy = -Y22 * cy, wz = -Y22 * cz;
+            const float pxx = rx * wx, pyy = ry * wy, pzz = rz * wz;
+            acc[3] += (pxx - pyy) * RS2;
+            acc[4] += (2.f * pzz - pxx - pyy) * RS6;
+            acc[5] += (rx * wy + ry * wx) * RS2;
+            acc[6] += (rx * wz + rz * wx) * RS2;
+            acc[7] += (ry * wz + rz * wy) * RS2;
+        }
+        if (gl == 0 && live) {                                       // self term: Omega += Z0(0)/6 L  (r -> 0, rh := 0)
+            const float4 l4 = inL[2 * s];
+            const float y0 = tab[0].y;
+            acc[8] += y0 * l4.x; acc[9] += y0 * l4.y; acc[10] += y0 * l4.z;
+        }
+#pragma unroll
+        for (int c = 0; c < 11; ++c)
+            for (int o = 4; o; o >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], o);
+        if (live) {
+            float mine = acc[0], w = acc[8];
+#pragma unroll
+            for (int c = 1; c < 8; ++c) mine = gl == c ? acc[c] : mine;
+            w = gl == 1 ? acc[9] : (gl == 2 ? acc[10] : w);
+            out8[(size_t)s * 8 + gl] += mine;
+            outW[(size_t)s * 8 + gl] = gl < 3 ? w : 0.f;
+        }
+    }
+}
+
+// a5 for the full couplet: the 8 spectra of (F, S) in `spec`, the 3 of L in `rot`; all 11 are overwritten with (U, E) and Omega
+__global__ void __launch_bounds__(256) scale_full_kernel(cufftComplex *spec, cufftComplex *rot, ScaleParams sp) {
+    const unsigned plane = (unsigned)sp.M * (unsigned)sp.Mh, rem = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rem >= plane) return;
+    const int ix = (int)blockIdx.y, iy = (int)(rem / (unsigned)sp.Mh), iz = (int)(rem - (unsigned)iy * (unsigned)sp.Mh);
+    const size_t nmode = (size_t)plane * sp.M, o = (size_t)ix * plane + rem;
+    const float2 zero = make_float2(0.f, 0.f);
+    float kx, ky, kz;
+    if (!mode_k(sp, ix, iy, iz, kx, ky, kz)) {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) spec[c * nmode + o] = zero;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) rot[c * nmode + o] = zero;
+        return;
+    }
+    const float k2 = kx * kx + ky * ky + kz * kz, kn = sqrtf(k2), ka = kn * sp.a;
+    float s0, s1;
+    shape_factors(ka, s0, s1);
+    const float q = k2 * sp.inv4xi2;
+    const float dw = __ldg(sp.dec + ix) * __ldg(sp.dec + iy) * __ldg(sp.dec + iz);
+    const float Bt = sp.c_mv * sp.inv_eta * (1.f + q) * __expf(-q) / k2 * dw * dw;
+    float2 F[3], S[5], Lh[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { F[c] = spec[c * nmode + o]; Lh[c] = rot[c * nmode + o]; }
+#pragma unroll
+    for (int c = 0; c < 5; ++c) S[c] = spec[(3 + c) * nmode + o];
+    float2 sk[3], kl[3];                                             // S.k and k x L, real and imaginary parts
+#pragma unroll
+    for (int ri = 0; ri < 2; ++ri) {
+        const float s1c = ri ? S[0].y : S[0].x, s2c = ri ? S[1].y : S[1].x, s3c = ri ? S[2].y : S[2].x, s4c = ri ? S[3].y : S[3].x,
+                    s5c = ri ? S[4].y : S[4].x;
+        const float sxx = s1c * WS_RS2 - s2c * WS_RS6, syy = -s1c * WS_RS2 - s2c * WS_RS6, szz = 2.f * s2c * WS_RS6;
+        const float sxy = s3c * WS_RS2, sxz = s4c * WS_RS2, syz = s5c * WS_RS2;
+        const float vx = sxx * kx + sxy * ky + sxz * kz, vy = sxy * kx + syy * ky + syz * kz, vz = sxz * kx + syz * ky + szz * kz;
+        const float lx = ri ? Lh[0].y : Lh[0].x, ly = ri ? Lh[1].y : Lh[1].x, lz = ri ? Lh[2].y : Lh[2].x;
+        const float cx = ky * lz - kz * ly, cy = kz * lx - kx * lz, cz = kx * ly - ky * lx;
+        if (ri) { sk[0].y = vx; sk[1].y = vy; sk[2].y = vz; kl[0].y = cx; kl[1].y = cy; kl[2].y = cz; }
+        else { sk[0].x = vx; sk[1].x = vy; sk[2].x = vz; kl[0].x = cx; kl[1].x = cy; kl[2].x = cz; }
+    }
+    // fh = s0 F - i s1 sk + (i/2) s1 kl :   -i z = (z.im, -z.re),  i z = (-z.im, z.re)
+    const float h1 = 0.5f * s1;
+    float2 f[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) f[c] = make_float2(s0 * F[c].x + s1 * sk[c].y - h1 * kl[c].y, s0 * F[c].y - s1 * sk[c].x + h1 * kl[c].x);
+    const float ik2 = 1.f / k2;
+    const float2 kf = make_float2((kx * f[0].x + ky * f[1].x + kz * f[2].x) * ik2, (kx * f[0].y + ky * f[1].y + kz * f[2].y) * ik2);
+    const float2 ux = make_float2(Bt * (f[0].x - kx * kf.x), Bt * (f[0].y - kx * kf.y));
+    const float2 uy = make_float2(Bt * (f[1].x - ky * kf.x), Bt * (f[1].y - ky * kf.y));
+    const float2 uz = make_float2(Bt * (f[2].x - kz * kf.x), Bt * (f[2].y - kz * kf.y));
+    write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
+    // Omega_h = (i/2) s1 k x uh
+    const float2 wx = make_float2(ky * uz.x - kz * uy.x, ky * uz.y - kz * uy.y);
+    const float2 wy = make_float2(kz * ux.x - kx * uz.x, kz * ux.y - kx * uz.y);
+    const float2 wz = make_float2(kx * uy.x - ky * ux.x, kx * uy.y - ky * ux.y);
+    rot[o] = make_float2(-h1 * wx.y, h1 * wx.x);
+    rot[nmode + o] = make_float2(-h1 * wy.y, h1 * wy.x);
+    rot[2 * nmode + o] = make_float2(-h1 * wz.y, h1 * wz.x);
+}
+
+// in8 = (F of a | S of b): the force slots of one packed vector, the stresslet slots of another (a may be NULL = 0)
+__global__ void k_merge_force_stresslet(const float4 *a, const float4 *b, int N, float4 *out) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float4 f = a ? a[2 * s] : make_float4(0.f, 0.f, 0.f, 0.f), b0 = b[2 * s];
+    out[2 * s] = make_float4(f.x, f.y, f.z, b0.w);
+    out[2 * s + 1] = b[2 * s + 1];
+}
+
+}  // namespace
+
+void pse_couplet_free(pse_ctx *c) {
+    cudaFree(c->d_rot_table); cudaFree(c->d_spec_rot); cudaFree(c->d_rot_in); cudaFree(c->d_rot_out); cudaFree(c->d_rot_tmp);
+    c->d_rot_table = nullptr; c->d_spec_rot = nullptr; c->d_rot_in = c->d_rot_out = c->d_rot_tmp = nullptr;
+}
+
+// table, spectrum and packed vectors of the torque rows: made by the first call that needs them (synchronises once)
+static pse_status ensure_couplet(pse_ctx *c) {
+    if (c->d_rot_table) return PSE_OK;
+    std::vector<float> tab;
+    pse_build_rot_table(c->a, c->eta, c->xi, c->rcut, PSE_NTAB, tab);
+    const size_t nmode = (size_t)c->M * c->M * c->Mh, vec = (size_t)c->N * 8 * sizeof(float);
+    if (cudaMalloc(&c->d_spec_rot, 3 * nmode * sizeof(cufftComplex)) != cudaSuccess || cudaMalloc(&c->d_rot_in, vec) != cudaSuccess ||
+        cudaMalloc(&c->d_rot_out, vec) != cudaSuccess || cudaMalloc(&c->d_rot_tmp, vec) != cudaSuccess ||
+        cudaMalloc(&c->d_rot_table, tab.size() * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        pse_couplet_free(c);
+        c->err = "out of memory (full-couplet buffers)"; return PSE_ENOMEM;
+    }
+    CUDA_TRY(c, cudaMemcpy(c->d_rot_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    return PSE_OK;
+}
+
+// out8 (U, E) and outW (Omega in slots 0-2) = M [in8 (F, S); inL (L in slots 0-2)], packed vectors in sorted numbering
+static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *inL, float *out8, float *outW, int which) {
+    const size_t vec = (size_t)c->N * 8 * sizeof(float);
+    if (which & PSE_REAL) {
+        PSE_TRY(pse_real_apply(c, in8, out8, PSE_MODE_ALL));
+        ScopedPhase ph(c, PSE_T_REAL);
+        const int wpb = 256 / 32;
+        int grid = 4 * c->nsm;
+        if ((long long)grid * wpb * 4 > c->N) grid = (c->N + wpb * 4 - 1) / (wpb * 4);
+        real_rot_kernel<<<grid, 256, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(in8), reinterpret_cast<const float4 *>(inL), out8, outW,
+                                                     c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_rot_table),
+                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
+        KERNEL_CHECK(c);
+    } else {
+        CUDA_TRY(c, cudaMemsetAsync(out8, 0, vec, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(outW, 0, vec, c->stream));
+    }
+    if (!(which & PSE_WAVE)) return PSE_OK;
+    const size_t nmode = (size_t)c->M * c->M * c->Mh;
+    // torque planes first (they pass through planes 0-2 of the grid array), then the eight planes of (F, S)
+    PSE_TRY(pse_wave_spread(c, inL, 1));
+    { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[1], c->d_grid, c->d_spec_rot)); c->launches++; }
+    PSE_TRY(pse_wave_spread(c, in8, 0));
+    { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[0], c->d_grid, c->d_spec)); c->launches++; }
+    {
+        ScopedPhase ph(c, PSE_T_SCALE);
+        scale_full_kernel<<<dim3((unsigned)((c->M * c->Mh + 255) / 256), (unsigned)c->M), 256, 0, c->stream>>>(c->d_spec, c->d_spec_rot, make_scale_params(c));
+        KERNEL_CHECK(c);
+    }
+    { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[0], c->d_spec, c->d_grid)); c->launches++; }
+    PSE_TRY(pse_wave_interp(c, out8, true, 3));
+    { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[1], c->d_spec_rot, c->d_grid)); c->launches++; }
+    (void)nmode;
+    return pse_wave_interp(c, outW, true, 1);
+}
+
+extern "C" {
+
+pse_status pse_mobility_apply_full(pse_ctx *c, const float *d_F, const float *d_L, const float *d_S, float *d_U, float *d_W, float *d_E, int which) {
+    if (!c || !(which & PSE_BOTH) || (!d_F && !d_L && !d_S) || (!d_U && !d_W && !d_E)) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_mobility_apply_full before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(ensure_couplet(c));
+    PSE_TRY(pse_pack(c, d_F, d_S, c->d_in));
+    PSE_TRY(pse_pack(c, d_L, nullptr, c->d_rot_in));
+    PSE_TRY(apply_full_packed(c, c->d_in, c->d_rot_in, c->d_out, c->d_rot_out, which));
+    if (d_U || d_E) PSE_TRY(pse_unpack(c, c->d_out, 1.f, d_U, d_E));
+    if (d_W) PSE_TRY(pse_unpack(c, c->d_rot_out, 1.f, d_W, nullptr));
+    return PSE_OK;
+}
+
+pse_status pse_constrained_solve_full(pse_ctx *c, const float *d_F, const float *d_L, const float *d_UB, const float *d_EB,
+                                      float *d_U, float *d_W, float *d_S, int *gmres_iters) {
+    if (!c || !d_U || !d_S) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_constrained_solve_full before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(ensure_couplet(c));
+    const size_t vec = (size_t)c->N * 8 * sizeof(float);
+    PSE_TRY(pse_pack(c, d_UB, d_EB, c->d_vecB));
+    PSE_TRY(pse_pack(c, d_L, nullptr, c->d_rot_in));
+    if (d_L) {
+        // what the torques alone do: (U_L, E_L) joins the Brownian slip on the right-hand side of Eq. (38)
+        CUDA_TRY(c, cudaMemsetAsync(c->d_in, 0, vec, c->stream));
+        PSE_TRY(apply_full_packed(c, c->d_in, c->d_rot_in, c->d_rot_tmp, c->d_rot_out, PSE_BOTH));
+        PSE_TRY(pse_axpby(c, (size_t)c->N * 8, 1.f, c->d_rot_tmp, 1.f, c->d_vecB));
+    }
+    if (d_F) PSE_TRY(pse_pack(c, d_F, nullptr, c->d_vecA));
+    pse_status st = pse_gmres_constraint(c, d_F ? c->d_vecA : nullptr, c->d_vecB, c->d_vecB, c->d_vecC, gmres_iters);
+    if (st != PSE_OK && st != PSE_ENOCONV) return st;
+    PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, d_U, d_S));
+    if (d_W) {                                                       // Omega = M_OF F + M_OL L + M_OS S: the Omega rows of one more full product
+        k_merge_force_stresslet<<<(c->N + 255) / 256, 256, 0, c->stream>>>(d_F ? reinterpret_cast<const float4 *>(c->d_vecA) : nullptr,
+                                                                           reinterpret_cast<const float4 *>(c->d_vecC), c->N, reinterpret_cast<float4 *>(c->d_in));
+        KERNEL_CHECK(c);
+        PSE_TRY(apply_full_packed(c, c->d_in, c->d_rot_in, c->d_out, c->d_rot_out, PSE_BOTH));
+        PSE_TRY(pse_unpack(c, c->d_rot_out, 1.f, d_W, nullptr));
+    }
+    return st;
+}
+
+}  // extern "C"

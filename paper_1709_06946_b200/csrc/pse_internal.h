@@ -128,6 +128,10 @@ struct pse_ctx {
     unsigned long long *d_scan_tmp = nullptr; size_t scan_tmp_n = 0;
     float4 *d_posw = nullptr;                // [N] wrapped positions, original numbering
     float *d_vecA = nullptr, *d_vecB = nullptr, *d_vecC = nullptr, *d_vecD = nullptr;   // [N][8] scratch for pse_step
+    // ---- full couplet (torque in, angular velocity out; couplet.cu), allocated by the first call that needs them ----
+    float *d_rot_table = nullptr;            // [PSE_NTAB][4] = (T/2, Z0/6, Z2/4, 0)/(6 pi eta a) at the nodes of d_table
+    cufftComplex *d_spec_rot = nullptr;      // [3][M][M][Mh] spectrum of the torque planes in, of the angular-velocity planes out
+    float *d_rot_in = nullptr, *d_rot_out = nullptr, *d_rot_tmp = nullptr;   // [N][8] packed: (Lx,Ly,Lz,0..), (Ox,Oy,Oz,0..), scratch
     // ---- bonds of the equilibrium test potential U = k |r - r0|, original numbering ----
     int2 *d_bonds = nullptr; int n_bonds = 0; double bond_k = 0, bond_r0 = 0;
     // ---- staging for the host-buffer entry points ----
@@ -223,7 +227,12 @@ void pse_wave_set_stream(pse_ctx *c, cudaStream_t st);    // stream of the cuFFT
 pse_status pse_tile_bins(pse_ctx *c);
 pse_status pse_particle_windows(pse_ctx *c);   // d_pbase, d_pw from d_pos (after the cell sort)
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode = PSE_MODE_ALL);   // out (+)= M_w in
+pse_status pse_wave_spread(pse_ctx *c, const float *d_in, int plan);                    // packed vector -> c->d_grid, planes of plan 0 / 1 / 2
+pse_status pse_wave_interp(pse_ctx *c, float *d_out, bool accumulate, int oplan);      // c->d_grid -> packed vector, planes of oplan 3 / 1 / 2
 pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
+// couplet.cu (torque / angular-velocity rows, NEXT-3)
+void pse_couplet_free(pse_ctx *c);
+void pse_build_rot_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab);   // tables.cu
 // krylov.cu
 pse_status pse_krylov_init(pse_ctx *c);   // cooperative-grid cap of the step kernels on the context's device
 pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_packed);      // original -> sorted

@@ -69,7 +69,8 @@ void free_space(double r, double a, double f[7]) {   // F1 F2 G1 G2 Z0 Z2 Z4
 
 }  // namespace
 
-void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr_out) {
+// R_X(r_i) = Free_X - W_X at the table nodes r_i = i dr, X = F1 F2 G1 G2 Z0 Z2 Z4, in units of 1/(6 pi eta a)
+static void real_space_nodes(double a, double xi, double rcut, int ntab, std::vector<double> &R, double *dr_out) {
     const double dr = rcut / (ntab - 2);         // node ntab-2 sits at rcut; one guard node beyond
     const double kmax = 2.0 * xi * std::sqrt(48.0);
     const int npanel = (int)std::ceil(kmax * (rcut + dr + 2 * a) / M_PI) + 8;
@@ -87,8 +88,8 @@ void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std
             int n = p * 16 + i;
             k[n] = kk; c00[n] = w * H * s0 * s0; c01[n] = w * H * kk * s0 * s1; c11[n] = w * H * kk * kk * s1 * s1;
         }
-    const double pref = 3.0 * a / M_PI, unit = 1.0 / (6.0 * M_PI * eta * a);
-    tab.assign((size_t)ntab * 8, 0.f);
+    const double pref = 3.0 * a / M_PI;
+    R.assign((size_t)ntab * 7, 0.0);
     for (int i = 0; i < ntab; ++i) {
         double r = i * dr, W[7] = {0, 0, 0, 0, 0, 0, 0};
         for (int n = 0; n < nq; ++n) {
@@ -99,7 +100,18 @@ void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std
             W[4] += c11[n] * j[0];           W[5] += c11[n] * j[2];          W[6] += c11[n] * j[4];
         }
         double f[7]; free_space(r, a, f);
-        double R[7]; for (int m = 0; m < 7; ++m) R[m] = f[m] - pref * W[m];
+        for (int m = 0; m < 7; ++m) R[(size_t)i * 7 + m] = f[m] - pref * W[m];
+    }
+    *dr_out = dr;
+}
+
+void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab, double *dr_out) {
+    std::vector<double> Rn;
+    real_space_nodes(a, xi, rcut, ntab, Rn, dr_out);
+    const double unit = 1.0 / (6.0 * M_PI * eta * a);
+    tab.assign((size_t)ntab * 8, 0.f);
+    for (int i = 0; i < ntab; ++i) {
+        const double *R = &Rn[(size_t)i * 7];
         double j1x = (R[4] + R[5]) / 3, j3x = (R[5] + R[6]) / 7, j2xx = (j1x + j3x) / 5;
         float *t = &tab[(size_t)i * 8];
         t[0] = (float)(unit * R[0]);                 t[1] = (float)(unit * R[1]);
@@ -107,7 +119,22 @@ void pse_build_table(double a, double eta, double xi, double rcut, int ntab, std
         t[4] = (float)(unit * (j1x - 2 * j2xx));     t[5] = (float)(unit * (2 * j3x - R[5] / 2));
         t[6] = (float)(unit * (-R[6]));              t[7] = 0.f;
     }
-    *dr_out = dr;
+}
+
+// Scalar functions of the rotational couplings (torque in, angular velocity out; reading R21) at the same nodes:
+// (T/2, Z0/6, Z2/4, 0) with T = G1 - G2, times 1/(6 pi eta a).  The antisymmetric part of Eq. (26) contracts to G1 - G2, and the
+// L / Omega couplings carry the weight k^2 s1^2 of Z0, Z2: no new integral.
+void pse_build_rot_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab) {
+    std::vector<double> Rn;
+    double dr;
+    real_space_nodes(a, xi, rcut, ntab, Rn, &dr);
+    const double unit = 1.0 / (6.0 * M_PI * eta * a);
+    tab.assign((size_t)ntab * 4, 0.f);
+    for (int i = 0; i < ntab; ++i) {
+        const double *R = &Rn[(size_t)i * 7];
+        float *t = &tab[(size_t)i * 4];
+        t[0] = (float)(unit * 0.5 * (R[2] - R[3])); t[1] = (float)(unit * R[4] / 6.0); t[2] = (float)(unit * R[5] / 4.0); t[3] = 0.f;
+    }
 }
 
 // ---- spreading / interpolation window and its transform ----

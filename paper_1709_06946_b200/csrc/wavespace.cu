@@ -912,6 +912,21 @@ static inline void plane_range(int bits, int &plan, int &first) {
     plan = bits == 3 ? 0 : bits; first = bits == 2 ? 3 : 0;
 }
 
+// interpolation of the planes of one output plan from c->d_grid (oplan bit 0: planes 0-2, bit 1: planes 3-7)
+pse_status pse_wave_interp(pse_ctx *c, float *d_out, bool accumulate, int oplan) {
+    ScopedPhase ph(c, PSE_T_INTERP);
+    const int TB = 256;
+    if (c->P <= 8) {
+        PSE_TRY(launch_interp_any(c, c->iset, oplan, d_out, accumulate));
+    } else {
+        interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
+            c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
+            (float)c->win_a, (float)c->win_b, accumulate ? 1 : 0, oplan << 2);
+    }
+    KERNEL_CHECK(c);
+    return PSE_OK;
+}
+
 static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumulate, int mode = PSE_MODE_ALL) {
     {
         ScopedPhase ph(c, PSE_T_FFT_INV);
@@ -920,15 +935,26 @@ static pse_status inverse_and_interpolate(pse_ctx *c, float *d_out, bool accumul
         const size_t M3 = pse_plane_stride(c->M), nmode = (size_t)c->M * c->M * c->Mh;
         CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[plan], c->d_spec + first * nmode, c->d_grid + first * M3)); c->launches++;
     }
-    ScopedPhase ph(c, PSE_T_INTERP);
-    const int TB = 256, oplan = (mode >> 2) & 3;
-    if (c->P <= 8) {
-        PSE_TRY(launch_interp_any(c, c->iset, oplan, d_out, accumulate));
-    } else {
-        interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
-            c->d_pos, c->d_tile_list, c->d_grid, reinterpret_cast<float4 *>(d_out), c->N, c->M, c->P, (float)(1.0 / c->h),
-            (float)c->win_a, (float)c->win_b, accumulate ? 1 : 0, mode);
-    }
+    return pse_wave_interp(c, d_out, accumulate, (mode >> 2) & 3);
+}
+
+// spread of the planes of one input plan (0: all 8, 1: planes 0-2, 2: planes 3-7) of the packed vector d_in into c->d_grid
+pse_status pse_wave_spread(pse_ctx *c, const float *d_in, int plan) {
+    ScopedPhase ph(c, PSE_T_SPREAD);
+    const float4 *in4 = reinterpret_cast<const float4 *>(d_in);
+    const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
+    if (use_block_spread(c)) {
+        switch (c->P) {
+            case 2: launch_spread_blocks<2>(c, plan, in4); break;
+            case 3: launch_spread_blocks<3>(c, plan, in4); break;
+            case 4: launch_spread_blocks<4>(c, plan, in4); break;
+            case 5: launch_spread_blocks<5>(c, plan, in4); break;
+            case 6: launch_spread_blocks<6>(c, plan, in4); break;
+            default: launch_spread_blocks<8>(c, plan, in4); break;
+        }
+    } else if (plan == 0) spread_kernel<0, 8><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
+    else if (plan == 1) spread_kernel<0, 3><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
+    else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
     KERNEL_CHECK(c);
     return PSE_OK;
 }
@@ -938,24 +964,7 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     if (!(mode & (PSE_IN_F | PSE_IN_S)) || !(mode & (PSE_OUT_U | PSE_OUT_E))) { c->err = "pse_wave_apply: empty component mask"; return PSE_EINVAL; }
     int plan, first;
     plane_range(mode & 3, plan, first);
-    {
-        ScopedPhase ph(c, PSE_T_SPREAD);
-        const float4 *in4 = reinterpret_cast<const float4 *>(d_in);
-        const float ih = (float)(1.0 / c->h), wa = (float)c->win_a, wb = (float)c->win_b;
-        if (use_block_spread(c)) {
-            switch (c->P) {
-                case 2: launch_spread_blocks<2>(c, plan, in4); break;
-                case 3: launch_spread_blocks<3>(c, plan, in4); break;
-                case 4: launch_spread_blocks<4>(c, plan, in4); break;
-                case 5: launch_spread_blocks<5>(c, plan, in4); break;
-                case 6: launch_spread_blocks<6>(c, plan, in4); break;
-                default: launch_spread_blocks<8>(c, plan, in4); break;
-            }
-        } else if (plan == 0) spread_kernel<0, 8><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
-        else if (plan == 1) spread_kernel<0, 3><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
-        else spread_kernel<3, 5><<<c->ntile, SPREAD_THREADS, 0, c->stream>>>(c->d_pos, in4, c->d_tile_start, c->d_tile_list, c->d_grid, c->M, c->P, c->nt, ih, wa, wb);
-        KERNEL_CHECK(c);
-    }
+    PSE_TRY(pse_wave_spread(c, d_in, plan));
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[plan], c->d_grid + first * M3, c->d_spec + first * nmode)); c->launches++; }
     {
         ScopedPhase ph(c, PSE_T_SCALE);

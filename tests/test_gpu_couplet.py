@@ -1,0 +1,140 @@
+"""GPU parity of the full couplet: pse_mobility_apply_full / pse_constrained_solve_full through the C ABI
+against oracle/couplet.py (direct Ewald sums, fp64) on the same seeded inputs.  Bar: relative L2 error max(2 tol, 1e-5) per output
+block (U, Omega, E), as for the force / stresslet product (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+import synth
+from oracle import couplet as cpl
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip('torch')
+
+A, ETA, KT = 1.0, 1.0 / (6.0 * np.pi), 1.0
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / np.linalg.norm(np.asarray(b, float)))
+
+
+def bar(tol):
+    return max(2 * tol, 1e-5)
+
+
+def dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x), dtype=torch.float32).cuda().contiguous()
+
+
+def pos4(x):
+    p = np.zeros((x.shape[0], 4), np.float32)
+    p[:, :3] = x
+    return p
+
+
+def inputs(N, seed):
+    rng = np.random.default_rng(seed)
+    F, S = synth.gaussian_inputs(N, seed)
+    return F.astype(np.float64), rng.standard_normal((N, 3)), S.astype(np.float64)
+
+
+def gpu_full(ctx, F, Lq, S, which=3):
+    N = ctx.N
+    U, W, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_mobility_apply_full(None if F is None else dev(F), None if Lq is None else dev(Lq), None if S is None else dev(S), U, W, E, which)
+    torch.cuda.synchronize()
+    return U.cpu().numpy(), W.cpu().numpy(), E.cpu().numpy()
+
+
+def make(N, phi, xi, tol, seed, grid=None, P=None, squeeze=1.0):
+    import paper_1709_06946_b200 as pse
+    x, L = synth.rsa(N, phi, seed=seed)
+    x, L = x * squeeze, L * squeeze
+    x32 = x.astype(np.float32)
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0
+    ctx = pse.pse_create(N, L, A, ETA, KT, xi, grid or g, P or p, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    return ctx, x32.astype(np.float64), L
+
+
+def test_full_couplet_config1_every_block_and_both_halves():
+    """BASELINE.json configs[0] (N = 64, grid 32, P = 8, tol 1e-3) with a torque on every particle: all inputs together, every input
+    block alone (a wrong sign in one coupling cannot hide in the total), and the real and wave halves separately."""
+    xi, tol = 0.6, 1e-3
+    ctx, x, L = make(64, 0.10, xi, tol, seed=1, grid=32, P=8)
+    F, Lq, S = inputs(64, 0)
+    want = cpl.mobility_apply_full(x, L, A, ETA, xi, F, Lq, S, eps=1e-10)
+    got = gpu_full(ctx, F, Lq, S)
+    for g, w, name in zip(got, want, 'UWE'):
+        assert rel(g, w) < bar(tol), (name, rel(g, w))
+    z3, z5 = np.zeros((64, 3)), np.zeros((64, 5))
+    for Fi, Li, Si, name in ((F, None, None, 'F'), (None, Lq, None, 'L'), (None, None, S, 'S')):
+        want = cpl.mobility_apply_full(x, L, A, ETA, xi, z3 if Fi is None else Fi, z3 if Li is None else Li, z5 if Si is None else Si, eps=1e-10)
+        got = gpu_full(ctx, Fi, Li, Si)
+        scale = max(np.linalg.norm(w) for w in want)
+        for g, w, out in zip(got, want, 'UWE'):
+            assert np.linalg.norm(g - w) < bar(tol) * scale, (name, out, np.linalg.norm(g - w) / scale)
+    for which, part in ((1, 'real'), (2, 'wave')):
+        want = cpl.mobility_apply_full(x, L, A, ETA, xi, F, Lq, S, eps=1e-10, part=part)
+        got = gpu_full(ctx, F, Lq, S, which)
+        tot = cpl.mobility_apply_full(x, L, A, ETA, xi, F, Lq, S, eps=1e-10)
+        for g, w, t, out in zip(got, want, tot, 'UWE'):
+            assert np.linalg.norm(g - w) < bar(tol) * np.linalg.norm(t), (part, out)
+    # without a torque, U and E are those of the 8-component product
+    U8, E8 = torch.empty(64, 3, device='cuda'), torch.empty(64, 5, device='cuda')
+    ctx.pse_mobility_apply(dev(F), dev(S), U8, E8)
+    U, W, E = gpu_full(ctx, F, None, S)
+    assert rel(U, U8.cpu().numpy()) < 2e-6 and rel(E, E8.cpu().numpy()) < 2e-6
+
+
+@pytest.mark.parametrize('tol', [1e-3, 1e-4])
+def test_full_couplet_sampled_rows_with_overlaps(tol):
+    """N = 1 500 at phi = 0.25, compressed 6 % (overlapping pairs: the regularised branch of every function), parameters from
+    pse_suggest_params, 12 sampled particles against the direct sums."""
+    N, xi = 1500, 0.55
+    ctx, x, L = make(N, 0.25, xi, tol, seed=4, squeeze=0.94)
+    F, Lq, S = inputs(N, 5)
+    rows = np.sort(np.random.default_rng(2).choice(N, 12, replace=False))
+    want = cpl.mobility_apply_full(x, L, A, ETA, xi, F, Lq, S, rows=rows, eps=1e-9)
+    got = gpu_full(ctx, F, Lq, S)
+    for g, w, name in zip(got, want, 'UWE'):
+        assert rel(g[rows], w) < bar(tol), (name, rel(g[rows], w))
+    # torque only: the couplings that exist only in the new rows
+    z3, z5 = np.zeros((N, 3)), np.zeros((N, 5))
+    want = cpl.mobility_apply_full(x, L, A, ETA, xi, z3, Lq, z5, rows=rows, eps=1e-9)
+    got = gpu_full(ctx, None, Lq, None)
+    for g, w, name in zip(got, want, 'UWE'):
+        assert rel(g[rows], w) < 2 * bar(tol), (name, rel(g[rows], w))
+
+
+def test_full_couplet_is_symmetric_on_the_gpu():
+    """v . M w = w . M v for random 11N vectors (Eq. 31's matrix is symmetric): a transposed coupling fails this."""
+    N, xi, tol = 600, 0.6, 1e-3
+    ctx, x, L = make(N, 0.15, xi, tol, seed=8)
+    v, w = inputs(N, 1), inputs(N, 2)
+    Mv, Mw = gpu_full(ctx, *v), gpu_full(ctx, *w)
+    dot = lambda a, b: float(sum((p.astype(np.float64) * q).sum() for p, q in zip(a, b)))
+    vMw, wMv = dot((v[0], v[1], v[2]), Mw), dot((w[0], w[1], w[2]), Mv)
+    assert abs(vMw - wMv) < 2 * tol * max(abs(vMw), abs(wMv), 1.0), (vMw, wMv)
+    assert dot((v[0], v[1], v[2]), Mv) > 0
+
+
+def test_constrained_solve_with_torques_against_dense_oracle():
+    N, xi, tol = 48, 0.85, 1e-4
+    ctx, x, L = make(N, 0.20, xi, tol, seed=3)
+    M = cpl.dense_full(x, L, A, ETA, xi, eps=1e-10)
+    rng = np.random.default_rng(9)
+    F, Lq = rng.standard_normal((N, 3)), rng.standard_normal((N, 3))
+    UB, EB = rng.standard_normal((N, 3)), rng.standard_normal((N, 5))
+    Uo, Wo, So = cpl.constrained_solve_full(M, N, UB, np.zeros((N, 3)), EB, F, Lq)
+    U, W, S = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    it = ctx.pse_constrained_solve_full(dev(F), dev(Lq), dev(UB), dev(EB), U, W, S)
+    assert 2 <= it <= 30
+    assert rel(S.cpu().numpy(), So) < 5 * bar(tol) and rel(U.cpu().numpy(), Uo) < 3 * bar(tol) and rel(W.cpu().numpy(), Wo) < 3 * bar(tol), \
+        (rel(S.cpu().numpy(), So), rel(U.cpu().numpy(), Uo), rel(W.cpu().numpy(), Wo))
+    # no torque, no Omega asked for: the 8-component solve
+    U2, S2 = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_constrained_solve_full(dev(F), None, dev(UB), dev(EB), U2, None, S2)
+    U3, S3 = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_constrained_solve(dev(F), dev(UB), dev(EB), U3, S3)
+    assert torch.equal(U2, U3) and torch.equal(S2, S3)
