@@ -254,6 +254,83 @@ class PSEReference:
         Uw, Ew = self.wave_apply(x, F, S5, rows)
         return Ur + Uw, Er + Ew
 
+    # ---- full couplet: torque in, angular velocity out (SURVEY.md 8(f) NEXT-3; conventions: oracle/couplet.py) ------------
+    def real_apply_full(self, x, F, Lq, S5, rows=None):
+        """[U;Omega;E]_rows = M_r [F;L;S] truncated at r_cut: pairs from a periodic k-d tree, scalar functions of every pair by
+        quadrature (oracle.functions), tensor forms of oracle.couplet.pair_apply_full; self terms F1(0) F, Z0(0)/6 L, Z0(0)/5 S."""
+        from . import couplet as cpl
+        x = _c(np.asarray(x, dtype=np.float64) % self.L)
+        N = x.shape[0]
+        rows = np.arange(N, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        F, Lq, S5 = _c(F), _c(Lq), _c(S5)
+        nb = cKDTree(x, boxsize=self.L).query_ball_point(x[rows], self.rcut)
+        ia = np.concatenate([np.full(len(b), i, dtype=np.int64) for i, b in enumerate(nb)])
+        ib = np.concatenate([np.asarray(b, dtype=np.int64) for b in nb])
+        keep = rows[ia] != ib
+        ia, ib = ia[keep], ib[keep]
+        rv = x[rows[ia]] - x[ib]
+        rv -= self.L * np.round(rv / self.L)
+        r = np.linalg.norm(rv, axis=1)
+        m = r < self.rcut
+        ia, ib, rv, r = ia[m], ib[m], rv[m], r[m]
+        R = fn.real_space_functions(r, self.xi, self.a)
+        Up, Wp, Ep = cpl.pair_apply_full(rv, F[ib], Lq[ib], fn.to_tensor(S5[ib]), R, self.pref)
+        U, W, E = np.zeros((rows.size, 3)), np.zeros((rows.size, 3)), np.zeros((rows.size, 5))
+        np.add.at(U, ia, Up)
+        np.add.at(W, ia, Wp)
+        np.add.at(E, ia, fn.to_coords(Ep))
+        R0 = fn.real_space_functions(np.zeros(1), self.xi, self.a)
+        U += self.pref * R0['F1'][0] * F[rows]
+        W += self.pref * R0['Z0'][0] / 6.0 * Lq[rows]
+        E += self.pref * R0['Z0'][0] / 5.0 * S5[rows]
+        return U, W, E
+
+    def wave_apply_full(self, x, F, Lq, S5, rows=None):
+        """[U;Omega;E]_rows = M_w [F;L;S]: the five steps of the module docstring on 11 grids, with
+        fh = s0 Fh + (i/2) s1 k x Lh - i s1 Sh.k in step 3 and the extra output Omega_h = (i/2) s1 k x uh."""
+        x = _c(np.asarray(x, dtype=np.float64) % self.L)
+        N = x.shape[0]
+        rows = np.arange(N, dtype=np.int64) if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+        M, V = self.M, self.L ** 3
+        nw = os.cpu_count() or 1
+        g = self.spread(x, np.hstack([_c(F), _c(Lq), _c(S5)]))                           # 1: planes 0-2 F, 3-5 L, 6-10 S
+        gh = sfft.rfftn(g, axes=(1, 2, 3), workers=nw)                                   # 2
+        del g
+        kx, ky, kz, live = self._kvec()                                                  # 3
+        k2 = kx * kx + ky * ky + kz * kz
+        k2 = np.where(k2 > 0, k2, 1.0)
+        kn = np.sqrt(k2)
+        c0, c1 = fn.s0(kn * self.a), fn.s1(kn * self.a)
+        e = fn.basis()
+        kk = (kx, ky, kz)
+        kxL = (ky * gh[5] - kz * gh[4], kz * gh[3] - kx * gh[5], kx * gh[4] - ky * gh[3])
+        fh = []
+        for i in range(3):
+            Sk = 0.0
+            for q in range(5):
+                for j in range(3):
+                    if e[q, i, j] != 0.0:
+                        Sk = Sk + e[q, i, j] * kk[j] * gh[6 + q]
+            fh.append(c0 * gh[i] + 0.5j * c1 * kxL[i] - 1j * c1 * Sk)
+        del gh, kxL
+        Bt = np.where(live, (self.h ** 3 / V) * fn.hasimoto_H(kn, self.xi) * np.exp(self.eta_g * k2 / (4.0 * self.xi ** 2)) / (self.eta * k2), 0.0)
+        kf = (kx * fh[0] + ky * fh[1] + kz * fh[2]) / k2
+        uh = [Bt * (fh[i] - kk[i] * kf) for i in range(3)]
+        del fh
+        o8 = self._outputs(uh, kx, ky, kz, c0, c1)
+        wh = [0.5j * c1 * (ky * uh[2] - kz * uh[1]), 0.5j * c1 * (kz * uh[0] - kx * uh[2]), 0.5j * c1 * (kx * uh[1] - ky * uh[0])]
+        oh = np.stack(o8[:3] + wh + o8[3:])
+        del uh, o8, wh
+        go = sfft.irfftn(oh, s=(M, M, M), axes=(1, 2, 3), workers=nw) * float(M) ** 3   # 4 (un-normalised)
+        del oh
+        out = self.interpolate(x, go, rows)                                              # 5
+        return out[:, :3], out[:, 3:6], out[:, 6:]
+
+    def apply_full(self, x, F, Lq, S5, rows=None):
+        """[U;Omega;E]_rows = (M_r + M_w) [F;L;S]  (Eq. 31, PAPER.md:175)."""
+        a_, b_ = self.real_apply_full(x, F, Lq, S5, rows), self.wave_apply_full(x, F, Lq, S5, rows)
+        return tuple(u + v for u, v in zip(a_, b_))
+
     def wave_sqrt_apply(self, x, Mg, wbuf, rows=None):
         """A_w w2 of Eq. (75) for the noise buffer of an Mg^3 grid (reading R8), evaluated on THIS object's
         finer grid: the factor sqrt(H/(eta V k^2)) (I - kh kh) W(k) of the Mg-grid's modes is placed in the spectrum of the

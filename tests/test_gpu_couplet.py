@@ -138,3 +138,20 @@ def test_constrained_solve_with_torques_against_dense_oracle():
     U3, S3 = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
     ctx.pse_constrained_solve(dev(F), dev(UB), dev(EB), U3, S3)
     assert torch.equal(U2, U3) and torch.equal(S2, S3)
+
+
+def test_full_couplet_at_config3_size_against_pse_reference():
+    """bench.py's default workload (N = 65 536, phi = 0.30, tol = 1e-3, xi = 0.575, grid 100, P = 4) with torques: U, Omega and E on
+    128 sampled particles against the fp64 reference tier (its own xi = 0.40, tol = 1e-7; pinned against the direct sums in
+    tests/test_pse_reference.py), plus the worst sampled particle as in tests/test_gpu_reference.py."""
+    from oracle import pse_reference as pr
+    N, tol, xi = 65536, 1e-3, 0.575
+    ctx, x, L = make(N, 0.30, xi, tol, seed=100)
+    assert (ctx.grid, ctx.P) == (100, 4)
+    F, Lq, S = inputs(N, 1)
+    rows = np.sort(np.random.default_rng(5).choice(N, 128, replace=False))
+    want = pr.PSEReference(L, A, ETA, 0.40, tol=1e-7).apply_full(x, F, Lq, S, rows=rows)
+    got = gpu_full(ctx, F, Lq, S)
+    for g, w, name in zip(got, want, 'UWE'):
+        worst = float(np.linalg.norm(g[rows] - w, axis=1).max() / np.sqrt((w * w).sum(axis=1).mean()))
+        assert rel(g[rows], w) < bar(tol) and worst < 10 * bar(tol), (name, rel(g[rows], w), worst)
