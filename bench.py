@@ -233,6 +233,19 @@ def run_ours(args, wl, rank, world):
         torch.cuda.synchronize()
         mv += e0.elapsed_time(e1)
     out['matvec_ms'] = mv / nmv
+    # the same with torques and angular velocities (Eq. 31's full couplet, 11 components)
+    Lq, W = torch.randn(N, 3, device=dev, generator=gen), torch.empty(N, 3, device=dev)
+    for _ in range(3):
+        ctx.pse_mobility_apply_full(F, Lq, S, U, W, E)
+    mv = 0.0
+    for _ in range(nmv):
+        flush.fill_(1.0)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); ctx.pse_mobility_apply_full(F, Lq, S, U, W, E); e1.record()
+        torch.cuda.synchronize()
+        mv += e0.elapsed_time(e1)
+    out['matvec_full_ms'] = mv / nmv
     # ---- end to end through the C ABI with host buffers ----
     hpos = pos.cpu().pin_memory()
     hnr = torch.randn(N, 8).pin_memory(); hnw = torch.randn(nshape).pin_memory()
@@ -360,6 +373,7 @@ def assemble(name, wl, r, K, world, overridden):
                   'lanczos_iters': r['lanczos'], 'parallelism': f'replicas x{world}' if world > 1 else 'single GPU',
                   'l2': 'flushed (256 MiB write) between timed steps; each step bracketed by its own CUDA events'}
     out['matvecs_per_sec'] = 1e3 / r['matvec_ms']
+    out['matvecs_full_couplet_per_sec'] = 1e3 / r['matvec_full_ms']      # [U;Omega;E] = M [F;L;S], 11 components
     out['ptps'] = value * wl['N']
     out['clocks'] = r['clocks']
     out['gpu_launches'] = int(r['launches'])
