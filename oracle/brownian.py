@@ -37,11 +37,13 @@ def grid_modes(Mg, L):
     return 2 * np.pi * np.concatenate([n, -n]) / L
 
 
-def wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, chunk=None, rows=None):
+def wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, chunk=None, rows=None, A=None):
     """A_w w2.  wbuf: real array [3][Mg][Mg][Mg/2+1][2] of i.i.d. N(0,1).  For each canonical mode
     W(k) = (g_re + i g_im)/sqrt2, W(-k) = conj W(k), so the pair contributes 2 Re[...]:
         uh = sqrt(H/(eta V k^2)) (I - kh kh) W ;  U_a = sum_k e^{ik.x_a} s0 uh ;  E^q_a = sum_k e^{ik.x_a} i s1 (e^q k).uh
     rows restricts the particles a the sum is evaluated at (the noise field does not depend on the particles).
+    A (3x3, det 1): deformed lattice with vectors = columns of L A; the mode of integer indices n is then
+    k = (2 pi/L) A^{-T} n instead of 2 pi n/L, everything else unchanged (V = L^3).
     """
     x = np.asarray(x, dtype=np.float64)
     if rows is not None:
@@ -49,7 +51,7 @@ def wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, chunk=None, rows=None):
     N = x.shape[0]
     wbuf = np.asarray(wbuf, dtype=np.float64).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
     idx, n = canonical_modes(Mg)
-    k = 2 * np.pi * n / L
+    k = 2 * np.pi * n / L if A is None else 2 * np.pi * (n @ np.linalg.inv(np.asarray(A, dtype=np.float64))) / L
     W = (wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 0] + 1j * wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 1]).T / np.sqrt(2)
     e = fn.basis()
     U, E = np.zeros((N, 3)), np.zeros((N, 5))
