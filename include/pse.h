@@ -53,6 +53,11 @@ enum { PSE_T_NEIGHBORS = 0, PSE_T_REAL = 1, PSE_T_SPREAD = 2, PSE_T_FFT_FWD = 3,
  *   Returns PSE_EINVAL if no valid choice exists (rcut > L/2).  pse_suggest_params = the default window. */
 pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, int *grid, int *P, double *rcut);
 pse_status pse_suggest_params_window(int N, double L, double a, double tol, double xi, int window, int *grid, int *P, double *rcut);
+/* The same for a deformed lattice A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]] (see pse_set_lattice): the grid grows by the largest
+ * column norm of A (the index range that still holds every |k| <= k_cut), P does not change (the window acts on lattice
+ * coordinates), and PSE_EINVAL also if rcut * (largest row norm of A^-1) > L/2 or det A != 1. */
+pse_status pse_suggest_params_lattice(int N, double L, double a, double tol, double xi, int window, double a11, double a12, double a22,
+                                      int *grid, int *P, double *rcut);
 
 /* Create a context for N equal spheres of radius a in a cubic periodic box of edge L, viscosity eta, thermal
  * energy kT, splitting parameter xi (Eq. 28), FFT grid `grid`^3, window support P^3 grid points
@@ -66,6 +71,17 @@ pse_status pse_create(pse_ctx **out, int N, double L, double a, double eta, doub
 pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double eta, double kT, double xi,
                              int grid, int P, double rcut, double tol, int window, void *cuda_stream);
 pse_status pse_destroy(pse_ctx *ctx);
+
+/* Deformed periodic lattice: the periodic cell is the cube of edge L mapped by the volume-preserving
+ * A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]], i.e. the lattice vectors are the columns of L A.  Simple shear (Lees-Edwards,
+ * Eq. 56): a11 = a22 = 1, a12 = gamma; planar extension (Kraynik-Reinelt, Eq. 58): a11 = epsilon,
+ * a22 = 1/epsilon, a12 = 0.  Positions, forces, velocities stay PHYSICAL (Cartesian) vectors; any periodic image of a position is
+ * accepted.  Inside, particles are carried in lattice coordinates s = A^-1 x, so cells, spreading and interpolation are those of
+ * the cube, separations are r = A d and wave vectors k = (2 pi/L) A^-T n (reading R22): P is that of the cube, the grid
+ * must be pse_suggest_params_lattice's.  Call before pse_neighbors; the neighbour structures are invalidated; pse_step then leaves
+ * positions unwrapped.  (1, 0, 1) restores the cube.  Synchronises the stream.
+ * PSE_EINVAL: a11 <= 0, a22 <= 0, a11 a22 != 1, or rcut * (largest row norm of A^-1) > L/2. */
+pse_status pse_set_lattice(pse_ctx *ctx, double a11, double a12, double a22);
 
 /* Bin the particles (positions may be unwrapped; they are wrapped into [0,L)) into linked cells of edge >= rcut
  * and build the full neighbour list {beta != alpha : |x_alpha - x_beta|_min-image^2 < rcut^2}, plus

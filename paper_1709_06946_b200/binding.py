@@ -19,7 +19,7 @@ PHASES = ('neighbors', 'real', 'spread', 'fft_fwd', 'scale', 'fft_inv', 'interp'
 _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PSE_ECUFFT', 5: 'PSE_ENOTREADY',
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
-EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
+EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_suggest_params_lattice', 'pse_set_lattice', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
            'pse_constrained_solve', 'pse_mobility_apply_full', 'pse_constrained_solve_full', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
@@ -40,6 +40,8 @@ def load_library():
     lib.pse_create.argtypes = [C.POINTER(vp), i32, dbl, dbl, dbl, dbl, dbl, i32, i32, dbl, dbl, vp]
     lib.pse_suggest_params_window.argtypes = [i32, dbl, dbl, dbl, dbl, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
     lib.pse_create_window.argtypes = [C.POINTER(vp), i32, dbl, dbl, dbl, dbl, dbl, i32, i32, dbl, dbl, i32, vp]
+    lib.pse_suggest_params_lattice.argtypes = [i32, dbl, dbl, dbl, dbl, i32, dbl, dbl, dbl, C.POINTER(i32), C.POINTER(i32), C.POINTER(dbl)]
+    lib.pse_set_lattice.argtypes = [vp, dbl, dbl, dbl]
     lib.pse_destroy.argtypes = [vp]
     lib.pse_neighbors.argtypes = [vp, vp]
     lib.pse_mobility_apply.argtypes = [vp, vp, vp, vp, vp, i32]
@@ -93,10 +95,10 @@ def pse_version():
     return _lib.pse_version().decode()
 
 
-def pse_suggest_params(N, L, a, tol, xi, window=PSE_WINDOW_ES):
-    """-> (status, grid, P, rcut); see include/pse.h (pse_suggest_params_window)."""
+def pse_suggest_params(N, L, a, tol, xi, window=PSE_WINDOW_ES, lattice=(1.0, 0.0, 1.0)):
+    """-> (status, grid, P, rcut); see include/pse.h (pse_suggest_params_window / _lattice).  lattice = (a11, a12, a22)."""
     g, p, rc = C.c_int(), C.c_int(), C.c_double()
-    st = _lib.pse_suggest_params_window(N, L, a, tol, xi, window, C.byref(g), C.byref(p), C.byref(rc))
+    st = _lib.pse_suggest_params_lattice(N, L, a, tol, xi, window, lattice[0], lattice[1], lattice[2], C.byref(g), C.byref(p), C.byref(rc))
     return st, g.value, p.value, rc.value
 
 
@@ -139,6 +141,10 @@ class Context:
             self._h = C.c_void_p()
 
     __del__ = close
+
+    def pse_set_lattice(self, a11, a12, a22):
+        """Deformed lattice A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]] (simple shear: (1, gamma, 1); extension: (eps, 0, 1/eps))."""
+        self._check(_lib.pse_set_lattice(self._h, float(a11), float(a12), float(a22)))
 
     def pse_neighbors(self, pos):
         self._check(_lib.pse_neighbors(self._h, _ptr(pos, (self.N, 4))))

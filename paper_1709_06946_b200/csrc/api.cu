@@ -60,9 +60,27 @@ pse_status pse_suggest_params(int N, double L, double a, double tol, double xi, 
     return pse_suggest_params_window(N, L, a, tol, xi, PSE_WINDOW_ES, grid, P, rcut);
 }
 
+// what a lattice A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]] asks of the grid and of the cutoff (reading R22):
+//   grid_factor = max_i ||col_i(A)||   the index range that holds |k| <= k_cut, k = (2 pi/L) A^-T n, is |n_i| <= k_cut L ||col_i A||/2 pi
+//   reach       = max_i ||row_i(A^-1)|| a separation |r| < r_cut has lattice-coordinate components |d_i| <= reach r_cut
+static bool lattice_factors(double a11, double a12, double a22, double *grid_factor, double *reach) {
+    if (!(a11 > 0) || !(a22 > 0) || !std::isfinite(a12) || std::fabs(a11 * a22 - 1.0) > 1e-9) return false;     // volume preserving
+    const double i11 = 1.0 / a11, i12 = -a12 / (a11 * a22), i22 = 1.0 / a22;
+    *grid_factor = std::max(std::max(a11, std::sqrt(a12 * a12 + a22 * a22)), 1.0);
+    *reach = std::max(std::max(std::sqrt(i11 * i11 + i12 * i12), i22), 1.0);
+    return true;
+}
+
 pse_status pse_suggest_params_window(int N, double L, double a, double tol, double xi, int window, int *grid, int *P, double *rcut) {
+    return pse_suggest_params_lattice(N, L, a, tol, xi, window, 1.0, 0.0, 1.0, grid, P, rcut);
+}
+
+pse_status pse_suggest_params_lattice(int N, double L, double a, double tol, double xi, int window, double a11, double a12, double a22,
+                                      int *grid, int *P, double *rcut) {
     if (window != PSE_WINDOW_GAUSS && window != PSE_WINDOW_ES) return PSE_EINVAL;
     if (N <= 0 || !(L > 0) || !(a > 0) || !(tol > 0 && tol < 1) || !(xi > 0)) return PSE_EINVAL;
+    double gfac = 1.0, reach = 1.0;
+    if (!lattice_factors(a11, a12, a22, &gfac, &reach)) return PSE_EINVAL;
     const double s = std::sqrt(-std::log(tol));
     // C1: functions decay like exp(-xi^2 (r-2a)^2), so the paper's estimate r = s/xi
     // is optimistic; the shift of one radius is calibrated against the oracle (R6: truncation error
@@ -70,7 +88,7 @@ pse_status pse_suggest_params_window(int N, double L, double a, double tol, doub
     double rc = s / xi + 1.0 * a;
     // C2: wave cutoff k_cut = 2 xi s (H(k) ~ exp(-k^2/4 xi^2)); M >= 1.07 k_cut L / pi (the strain-rate rows carry an
     // extra factor k, so the bare estimate leaves their truncation error at ~tol), then the cheapest measured cuFFT size >= that (2,3,5,7-smooth below 64)
-    int M = std::max(8, (int)std::ceil(1.07 * 2.0 * xi * s * L / M_PI));
+    int M = std::max(8, (int)std::ceil(1.07 * 2.0 * xi * s * L / M_PI * gfac));      // gfac = 1 on the cube
     if (M > 64) M = choose_grid(M); else while (!smooth7(M)) ++M;
     // C3: support size.  Default window = exponential of semicircle with beta = 2.2 P: measured against
     // the oracle it reaches the tolerance with P = 3, 4, 5 points at tol = 1e-2, 1e-3, 1e-4, i.e. P = ceil(-log10 tol) + 1.
@@ -87,7 +105,7 @@ pse_status pse_suggest_params_window(int N, double L, double a, double tol, doub
     if (grid) *grid = M;
     if (P) *P = p;
     if (rcut) *rcut = rc;
-    if (rc > 0.5 * L || p > M) return PSE_EINVAL;
+    if (rc * reach > 0.5 * L || p > M) return PSE_EINVAL;
     return PSE_OK;
 }
 
@@ -218,6 +236,24 @@ pse_status pse_neighbors(pse_ctx *c, const float *d_pos) {
     return pse_neighbors_sync(c, d_pos);
 }
 
+pse_status pse_set_lattice(pse_ctx *c, double a11, double a12, double a22) {
+    if (!c) return PSE_EINVAL;
+    double gfac, reach;
+    if (!lattice_factors(a11, a12, a22, &gfac, &reach)) { c->err = "pse_set_lattice: A must have a11, a22 > 0 and det A = a11 a22 = 1"; return PSE_EINVAL; }
+    if (c->rcut * reach > 0.5 * c->L) {
+        c->err = "pse_set_lattice: rcut * max row norm of A^-1 > L/2 (the minimum image in lattice coordinates would miss pairs)"; return PSE_EINVAL;
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the lattice is baked in
+    c->lat_a11 = a11; c->lat_a12 = a12; c->lat_a22 = a22;
+    c->deformed = !(a11 == 1.0 && a12 == 0.0 && a22 == 1.0);
+    // cells of lattice-coordinate edge >= reach * rcut (never more cells than pse_create made room for: reach >= 1)
+    c->nc = std::max(1, (int)std::floor(c->L / (c->rcut * 1.0001 * reach)));
+    c->ncell = c->nc * c->nc * c->nc;
+    c->have_nbrs = false; c->nbr_pending = false; c->fine_bins_valid = false;
+    return PSE_OK;
+}
+
 pse_status pse_get_neighbors(pse_ctx *c, int *d_count, int *d_index, size_t cap, size_t *total) {
     if (!c) return PSE_EINVAL;
     return pse_get_neighbors_impl(c, d_count, d_index, cap, total);
@@ -323,7 +359,7 @@ static pse_status enqueue_step_fixed(pse_ctx *c, float *d_pos, double dt, const 
     }
     if (!(parts & 2)) return PSE_OK;
     PSE_TRY(brownian_wave_part(c, dt, d_noise_wave, UB, EB));
-    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+    k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, c->deformed ? 0 : 1); KERNEL_CHECK(c);
     PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
     *slot1 = c->nbr_last;
     PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
@@ -336,7 +372,7 @@ static pse_status enqueue_step_fixed(pse_ctx *c, float *d_pos, double dt, const 
     PSE_TRY(pse_gmres_constraint(c, c->d_vecA, c->d_vecB, c->d_vecB, c->d_vecC, nullptr, mG));
     PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
-                                        reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+                                        reinterpret_cast<float4 *>(d_pos), c->deformed ? 0 : 1); KERNEL_CHECK(c);
     return PSE_OK;
 }
 
@@ -453,7 +489,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     redo = true;
     for (int attempt = 0; redo && attempt < 4; ++attempt) {
         // (77) mid-point
-        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, 1); KERNEL_CHECK(c);
+        k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, c->deformed ? 0 : 1); KERNEL_CHECK(c);
         PSE_TRY(pse_neighbors_impl(c, reinterpret_cast<const float *>(xh)));
         // (78) constrained solve at the mid-point with hard-sphere forces (reading R12)
         PSE_TRY(pse_hs_forces_packed(c, dt, c->d_vecA));
@@ -472,7 +508,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
     PSE_TRY(pse_unpack(c, c->d_vecC, 1.f, c->d_vecA, nullptr));     // U_{k+1/2}, original numbering [N][3]
     // (79) full step from x_k
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), c->d_vecA, (float)dt, L, invL, N,
-                                        reinterpret_cast<float4 *>(d_pos), 1); KERNEL_CHECK(c);
+                                        reinterpret_cast<float4 *>(d_pos), c->deformed ? 0 : 1); KERNEL_CHECK(c);
     if (soft == PSE_OK && c->last_lanczos_iters > 0 && c->last_gmres_iters > 0) {      // the counts the next step is enqueued with
         c->lanczos_budget = c->last_lanczos_iters; c->gmres_budget = c->last_gmres_iters;
     }

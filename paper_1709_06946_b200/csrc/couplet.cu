@@ -28,7 +28,7 @@ constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
 __global__ void __launch_bounds__(256)
 real_rot_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, const float4 *__restrict__ inL, float *__restrict__ out8,
                 float *__restrict__ outW, int N, const unsigned long long *__restrict__ off, const int *__restrict__ cnt,
-                const int *__restrict__ idx, const float4 *__restrict__ table, float inv_dr, float L, float invL) {
+                const int *__restrict__ idx, const float4 *__restrict__ table, float inv_dr, float L, float invL, Lat lat) {
     __shared__ float4 tab[PSE_NTAB];
     for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) tab[i] = table[i];
     __syncthreads();
@@ -44,6 +44,7 @@ real_rot_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, 
             const float4 q4 = pos[b], a0 = in8[2 * b], a1 = in8[2 * b + 1], l4 = inL[2 * b];
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
+            dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy;                 // r = A d on a deformed lattice (identity on the cube)
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float rinv = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * rinv;
             const float rx = dx * rinv, ry = dy * rinv, rz = dz * rinv;
@@ -195,7 +196,7 @@ static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *i
         if ((long long)grid * wpb * 4 > c->N) grid = (c->N + wpb * 4 - 1) / (wpb * 4);
         real_rot_kernel<<<grid, 256, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(in8), reinterpret_cast<const float4 *>(inL), out8, outW,
                                                      c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_rot_table),
-                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
+                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L, pse_lat(c));
         KERNEL_CHECK(c);
     } else {
         CUDA_TRY(c, cudaMemsetAsync(out8, 0, vec, c->stream));

@@ -9,6 +9,7 @@
 // exact operation order of DESIGN.md reading R16 (no FMA contraction), so the sets are bit-identical to the oracle's.
 // The host never waits for the build: the list size and the overflow / fallback flags come back asynchronously and are
 // examined at the next point where the stream is synchronised anyway (pse_neighbors_settle).
+#include <cmath>
 #include "pse_internal.h"
 
 namespace {
@@ -129,18 +130,22 @@ __device__ __forceinline__ float wrap_coord(float x, float L, float invL) {
 __device__ __forceinline__ float min_image(float d, float L, float invL) {
     return __fsub_rn(d, __fmul_rn(L, rintf(__fmul_rn(d, invL))));
 }
-__device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL) {
+// a, b: lattice coordinates; the physical separation is r = A d (reading R22).  On the cube (a11 = a22 = 1, a12 = 0) the
+// extra products and the sum are exact, so the value is bit for bit that of the plain R16 form.
+__device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL, Lat lat) {
     float dx = min_image(__fsub_rn(a.x, b.x), L, invL);
     float dy = min_image(__fsub_rn(a.y, b.y), L, invL);
     float dz = min_image(__fsub_rn(a.z, b.z), L, invL);
-    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    const float rx = __fadd_rn(__fmul_rn(lat.a11, dx), __fmul_rn(lat.a12, dy)), ry = __fmul_rn(lat.a22, dy);
+    return __fadd_rn(__fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)), __fmul_rn(dz, dz));
 }
 
 __global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int nc, float cell_inv,
-                             float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count) {
+                             float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count, Lat lat) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     float4 p = pos[i];
+    p.x = __fadd_rn(__fmul_rn(lat.i11, p.x), __fmul_rn(lat.i12, p.y)); p.y = __fmul_rn(lat.i22, p.y);     // s = A^-1 x (exact on the cube)
     p.x = wrap_coord(p.x, L, invL); p.y = wrap_coord(p.y, L, invL); p.z = wrap_coord(p.z, L, invL); p.w = 0.f;
     posw[i] = p;
     int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
@@ -194,7 +199,7 @@ constexpr int NS_CHUNK = 1024, NS_THREADS = 128;
 template <bool FILL>
 __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start,
                                                                    int nc, float L, float invL, float rc2, int *__restrict__ cursor,
-                                                                   const unsigned long long *__restrict__ off, int *__restrict__ idx) {
+                                                                   const unsigned long long *__restrict__ off, int *__restrict__ idx, Lat lat) {
     __shared__ float4 cpos[NS_CHUNK];
     __shared__ int run_lo[18], run_cum[19];
     const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -249,7 +254,7 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
                 if (c < nchunk) {
                     const float4 q = cpos[c];
                     j = __float_as_int(q.w);
-                    in = (j != s) && dist2(p, q, L, invL) < rc2;
+                    in = (j != s) && dist2(p, q, L, invL, lat) < rc2;
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, in);
                 if (FILL && in) idx[base + found + __popc(m & ((1u << lane) - 1))] = j;
@@ -270,11 +275,12 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
 // candidates) set *fallback and are handled by the two-pass kernels above.
 constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32, NB_PB = 4;
 
+template <bool DEF>                                           // DEF: deformed lattice, the screened separation is mapped by A as well
 __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
                                                                    float L, float invL, float rc2, float band, int *__restrict__ count,
                                                                    unsigned long long *__restrict__ off, int *__restrict__ idx,
                                                                    unsigned long long cap, unsigned long long *__restrict__ cursor,
-                                                                   int *__restrict__ fallback) {
+                                                                   int *__restrict__ fallback, Lat lat) {
     __shared__ float4 cpos[NS_CHUNK];
     __shared__ unsigned masks[NB_MAXP][NB_WORDS];
     __shared__ int cnt[NB_MAXP], loc[NB_MAXP];
@@ -347,7 +353,10 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
             bool in[NB_PB], anyex = false;
 #pragma unroll
             for (int b = 0; b < NB_PB; ++b) {
-                const float dx = p[b].x - q.x, dy = p[b].y - q.y, dz = p[b].z - q.z, d2 = dx * dx + dy * dy + dz * dz;
+                float dx = p[b].x - q.x, dy = p[b].y - q.y;
+                const float dz = p[b].z - q.z;
+                if (DEF) { dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy; }
+                const float d2 = dx * dx + dy * dy + dz * dz;
                 in[b] = d2 < rc2;
                 anyex = anyex || !(fabsf(d2 - rc2) > band);
             }
@@ -357,8 +366,11 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
                     const float4 qe = fast ? pos[j] : q;
 #pragma unroll
                     for (int b = 0; b < NB_PB; ++b) {
-                        const float dx = p[b].x - q.x, dy = p[b].y - q.y, dz = p[b].z - q.z, d2 = dx * dx + dy * dy + dz * dz;
-                        if (!fast || !(fabsf(d2 - rc2) > band)) in[b] = dist2(p[b], qe, L, invL) < rc2;
+                        float dx = p[b].x - q.x, dy = p[b].y - q.y;
+                        const float dz = p[b].z - q.z;
+                        if (DEF) { dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy; }
+                        const float d2 = dx * dx + dy * dy + dz * dz;
+                        if (!fast || !(fabsf(d2 - rc2) > band)) in[b] = dist2(p[b], qe, L, invL, lat) < rc2;
                     }
                 }
             }
@@ -426,7 +438,7 @@ __global__ void lists_to_original(const int *idx, const unsigned long long *off_
 
 // Heyes-Melrose overlap force (reading R12), 8 lanes per particle over the neighbour list (as the pair kernel), packed output.
 __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off, const int *__restrict__ count,
-                          const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out) {
+                          const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out, Lat lat) {
     const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, gl = threadIdx.x & 7;
     const bool live = s < N;
     const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -435,6 +447,7 @@ __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned 
         for (unsigned long long j = off[s] + gl, hi = off[s] + (unsigned long long)count[s]; j < hi; j += 8) {
             float4 q = pos[idx[j]];
             float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
+            dx = __fadd_rn(__fmul_rn(lat.a11, dx), __fmul_rn(lat.a12, dy)); dy = __fmul_rn(lat.a22, dy);     // r = A d (exact on the cube)
             float r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < two_a * two_a && r2 > 0.f) {
                 float r = sqrtf(r2), g = coef * (two_a - r) / r;
@@ -454,12 +467,14 @@ __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned 
 // Forces of the bond potential U(r) = k |r - r0| of the paper's equilibrium test: a thread per bond,
 // positions and output in original numbering, F_i -= k sign(r - r0) rhat_ij, F_j += the same (out is zeroed beforehand).
 __global__ void bond_forces(const float4 *__restrict__ posw, const int2 *__restrict__ bonds, int nb, float L, float invL, float k, float r0,
-                            float *__restrict__ out) {
+                            float *__restrict__ out, Lat lat) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nb) return;
     const int2 ij = bonds[b];
     const float4 p = posw[ij.x], q = posw[ij.y];
-    const float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL), dz = min_image(p.z - q.z, L, invL);
+    float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL);
+    const float dz = min_image(p.z - q.z, L, invL);
+    dx = __fadd_rn(__fmul_rn(lat.a11, dx), __fmul_rn(lat.a12, dy)); dy = __fmul_rn(lat.a22, dy);
     const float r = sqrtf(dx * dx + dy * dy + dz * dz);
     if (!(r > 0.f) || r == r0) return;
     const float g = (r > r0 ? -k : k) / r;
@@ -474,7 +489,7 @@ pse_status pse_bond_forces_orig(pse_ctx *c, float *d_F) {
     CUDA_TRY(c, cudaMemsetAsync(d_F, 0, (size_t)3 * c->N * sizeof(float), c->stream));
     if (c->n_bonds == 0) return PSE_OK;
     bond_forces<<<(c->n_bonds + 127) / 128, 128, 0, c->stream>>>(c->d_posw, c->d_bonds, c->n_bonds, (float)c->L, 1.0f / (float)c->L,
-                                                                 (float)c->bond_k, (float)c->bond_r0, d_F);
+                                                                 (float)c->bond_k, (float)c->bond_r0, d_F, pse_lat(c));
     KERNEL_CHECK(c);
     return PSE_OK;
 }
@@ -492,12 +507,14 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     const int N = c->N, T = 256, nb = (N + T - 1) / T;
     const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
     const float rc = (float)c->rcut, rc2 = rc * rc;
-    const float band = 32.f * rc * L * 1.2e-7f;          // >> 2 r_c ulp(L): rounding gap between screened and R16 distances
+    const Lat lat = pse_lat(c);
+    // >> 2 r_c ulp(L): rounding gap between screened and R16 distances (the map by A adds a few more roundings of the same size)
+    const float band = 32.f * rc * L * 1.2e-7f * (c->deformed ? 4.f * (float)(std::fabs(c->lat_a11) + std::fabs(c->lat_a12) + std::fabs(c->lat_a22)) : 1.f);
     c->have_nbrs = false;
     CUDA_TRY(c, cudaMemsetAsync(c->d_bins, 0, c->bins_n * sizeof(int), c->stream));      // cell and tile counters, one memset
     wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
                                            c->d_posw, c->d_cell_of, c->d_cell_count, (float)(1.0 / c->h), c->M, c->P, c->nt,
-                                           c->d_tile_of, c->d_tile_count); KERNEL_CHECK(c);
+                                           c->d_tile_of, c->d_tile_count, lat); KERNEL_CHECK(c);
     if (c->ncell <= SCAN1_MAX && c->ntile <= SCAN1_MAX) {
         scan_two_ctas<<<2, SCAN1_THREADS, 0, c->stream>>>(c->d_cell_count, c->ncell, c->d_cell_start, c->d_tile_count, c->ntile, c->d_tile_start);
         KERNEL_CHECK(c);
@@ -520,16 +537,22 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         // single-pass build into a cursor-allocated index array; {cursor, fallback flag} travel to the pinned mirror behind
         // the kernel and are looked at by pse_neighbors_settle, never here
         CUDA_TRY(c, cudaMemsetAsync(c->d_nbr_ctl, 0, 2 * sizeof(unsigned long long), c->stream));
-        neighbor_build_cell<<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
-                                                                   c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
-                                                                   reinterpret_cast<int *>(c->d_nbr_ctl + 1)); KERNEL_CHECK(c);
+        if (c->deformed)
+            neighbor_build_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
+                                                                             c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
+                                                                             reinterpret_cast<int *>(c->d_nbr_ctl + 1), lat);
+        else
+            neighbor_build_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
+                                                                              c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
+                                                                              reinterpret_cast<int *>(c->d_nbr_ctl + 1), lat);
+        KERNEL_CHECK(c);
         c->nbr_last = c->nbr_slot; c->nbr_slot ^= 1;               // two report slots: pse_step has two builds in flight
         CUDA_TRY(c, cudaMemcpyAsync(c->h_nbr_ctl + 2 * c->nbr_last, c->d_nbr_ctl, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(c, cudaEventRecord(c->ev_nbr, c->stream));
         c->nbr_pending = true;
     } else {                                                         // general two-pass path (count, scan, fill); synchronises
         neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
-                                                                            nullptr, nullptr); KERNEL_CHECK(c);
+                                                                            nullptr, nullptr, lat); KERNEL_CHECK(c);
         PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
         unsigned long long total = 0;
         CUDA_TRY(c, cudaMemcpyAsync(&total, c->d_nbr_off + N, sizeof(total), cudaMemcpyDeviceToHost, c->stream));
@@ -543,7 +566,7 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         }
         c->nbr_total = (size_t)total;
         neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
-                                                                           c->d_nbr_off, c->d_nbr_idx); KERNEL_CHECK(c);
+                                                                           c->d_nbr_off, c->d_nbr_idx, lat); KERNEL_CHECK(c);
         c->nbr_pending = false;
     }
     c->have_nbrs = true;
@@ -620,7 +643,7 @@ pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {
     const int N = c->N, T = 256;
     float coef = (float)(3.0 * M_PI * c->eta * c->a / dt);
     hs_forces<<<(unsigned)(((size_t)N * 8 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, (float)c->L,
-                                                                            1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed);
+                                                                            1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed, pse_lat(c));
     KERNEL_CHECK(c);
     return PSE_OK;
 }

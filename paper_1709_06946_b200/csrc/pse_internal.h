@@ -22,6 +22,13 @@ enum { PSE_IN_F = 1, PSE_IN_S = 2, PSE_OUT_U = 4, PSE_OUT_E = 8, PSE_MODE_ALL = 
 
 struct Timer { cudaEvent_t a, b; int phase; };
 
+// Deformed periodic lattice (NEXT-4; Eqs. 56, 58): lattice vectors = columns of L A with
+// A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]], det A = 1 (simple shear: a12 = gamma; planar extension: a11 = 1/a22 = epsilon).
+// Inside the library positions are LATTICE coordinates s = A^-1 x wrapped into [0, L)^3, so binning, spreading and interpolation
+// are those of the cube; physical separations r = A d (d = minimum image of s_a - s_b) and wave vectors k = (2 pi/L) A^-T n
+// appear only where distances and the Green's function are evaluated (reading R22).  i** = entries of A^-1.
+struct Lat { float a11, a12, a22, i11, i12, i22; };
+
 // everything baked into the captured graph of a step
 struct StepGraphKey {
     const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap;
@@ -46,6 +53,8 @@ struct pse_ctx {
     int N = 0, M = 0, P = 0;
     double L = 0, a = 0, eta = 0, kT = 0, xi = 0, rcut = 0, tol = 0;
     double h = 0, eta_g = 0;                 // grid spacing, Gaussian shape parameter
+    double lat_a11 = 1, lat_a12 = 0, lat_a22 = 1;   // the lattice deformation A (pse_set_lattice); identity = the cubic box
+    bool deformed = false;
     int win_kind = 1;                        // 0 = Gaussian (paper), 1 = exponential-of-semicircle window
     double win_a = 0, win_b = 0;             // window parameters handed to the kernels (see win_arg in wavespace.cu)
     float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index
@@ -199,6 +208,13 @@ __device__ __forceinline__ float warp_reduce8(const float (&a)[8], int lane, int
     return r;
 }
 #endif
+
+inline Lat pse_lat(const pse_ctx *c) {
+    Lat l;
+    l.a11 = (float)c->lat_a11; l.a12 = (float)c->lat_a12; l.a22 = (float)c->lat_a22;
+    l.i11 = (float)(1.0 / c->lat_a11); l.i12 = (float)(-c->lat_a12 / (c->lat_a11 * c->lat_a22)); l.i22 = (float)(1.0 / c->lat_a22);
+    return l;
+}
 
 // api.cu
 int pse_choose_grid(int mmin);

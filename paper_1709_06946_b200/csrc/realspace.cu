@@ -28,11 +28,12 @@ __device__ __forceinline__ void load_packed8(const float4 *in, int b, float4 &a0
                  : "l"(in + 2 * (size_t)b));
 }
 
-template <int MODE>
+// DEF: deformed lattice (reading R22): pos holds lattice coordinates, the physical separation is r = A d, three more FMAs per pair.
+template <int MODE, bool DEF>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
                   const unsigned long long *__restrict__ off, const int *__restrict__ cnt, const int *__restrict__ idx,
-                  const float4 *__restrict__ table, float inv_dr, float L, float invL) {
+                  const float4 *__restrict__ table, float inv_dr, float L, float invL, Lat lat) {
     // two planar float4 arrays (U-part functions, E-part functions): a 16-byte row stride spreads random rows over
     // all eight 16-byte bank groups; the interleaved 32-byte rows reached only four (ncu: 17 wavefronts per LDS.128)
     extern __shared__ float4 tab[];               // tabU[PSE_NTAB] then tabE[PSE_NTAB]
@@ -69,6 +70,7 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
             const int bn = (j + G < hi) ? idx[j + G] : b;
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
+            if (DEF) { dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy; }
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float rinv = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * rinv;
             const float rx = dx * rinv, ry = dy * rinv, rz = dz * rinv;
@@ -131,16 +133,23 @@ constexpr size_t REAL_SMEM = (size_t)PSE_NTAB * 2 * sizeof(float4);
 
 template <int MODE>
 static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, int grid) {
-    real_pairs_kernel<MODE><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(d_in), reinterpret_cast<float4 *>(d_out), c->N,
-                                                               c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_table),
-                                                               (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L);
+    const float4 *in4 = reinterpret_cast<const float4 *>(d_in), *tab = reinterpret_cast<const float4 *>(c->d_table);
+    float4 *out4 = reinterpret_cast<float4 *>(d_out);
+    const float inv_dr = (float)(1.0 / c->tab_dr), L = (float)c->L, invL = 1.0f / (float)c->L;
+    if (c->deformed)
+        real_pairs_kernel<MODE, true><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
+                                                                         inv_dr, L, invL, pse_lat(c));
+    else
+        real_pairs_kernel<MODE, false><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
+                                                                          inv_dr, L, invL, pse_lat(c));
     KERNEL_CHECK(c);
     return PSE_OK;
 }
 
 // dynamic shared-memory opt-in of every instantiation on the context's device (called by pse_create)
 pse_status pse_real_init(pse_ctx *c) {
-#define PSE_REAL_ATTR(M) CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REAL_SMEM))
+#define PSE_REAL_ATTR(M) CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<M, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REAL_SMEM)); \
+                         CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_kernel<M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REAL_SMEM))
     PSE_REAL_ATTR(PSE_IN_S | PSE_OUT_E); PSE_REAL_ATTR(PSE_IN_F | PSE_OUT_E); PSE_REAL_ATTR(PSE_IN_F | PSE_IN_S | PSE_OUT_U);
     PSE_REAL_ATTR(PSE_IN_S | PSE_OUT_U); PSE_REAL_ATTR(PSE_IN_F | PSE_OUT_U); PSE_REAL_ATTR(PSE_MODE_ALL);
 #undef PSE_REAL_ATTR

@@ -13,6 +13,7 @@ struct ScaleParams {
     float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
     const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
     int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
+    float ki11, ki12, ki22;                        // k = (2 pi/L) A^-T n: kx = ki11 nx, ky = ki22 ny + ki12 nx (entries of A^-1; 1, 0, 1 on the cube)
 };
 
 // s0 = sin x / x and s1 = 3 (sin x - x cos x)/x^3 (series below 0.5: cancellation) from one sincosf, x > 0
@@ -30,7 +31,7 @@ __device__ __forceinline__ bool mode_k(const ScaleParams &sp, int ix, int iy, in
     const int M = sp.M, half = (M + 1) / 2;
     const int nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M, nz = iz;
     const bool nyq = !(M & 1) && (ix == M / 2 || iy == M / 2 || iz == M / 2);
-    kx = sp.two_pi_over_L * (float)nx; ky = sp.two_pi_over_L * (float)ny; kz = sp.two_pi_over_L * (float)nz;
+    kx = sp.two_pi_over_L * (sp.ki11 * (float)nx); ky = sp.two_pi_over_L * (sp.ki22 * (float)ny + sp.ki12 * (float)nx); kz = sp.two_pi_over_L * (float)nz;
     return !(nyq || (nx == 0 && ny == 0 && nz == 0));
 }
 
@@ -114,6 +115,8 @@ inline ScaleParams make_scale_params(const pse_ctx *c, int mode = PSE_MODE_ALL) 
     const double V = c->L * c->L * c->L;
     sp.c_mv = (float)(1.0 / V); sp.c_br = (float)(1.0 / std::sqrt(V));
     sp.inv_eta = (float)(1.0 / c->eta);
+    const Lat l = pse_lat(c);
+    sp.ki11 = l.i11; sp.ki12 = l.i12; sp.ki22 = l.i22;
     return sp;
 }
 

@@ -51,6 +51,21 @@ def test_suggest_params_rules(pse):
     assert pse.pse_suggest_params(0, 13.892, 1.0, 1e-3, 0.6)[0] == pse.PSE_EINVAL
 
 
+def test_suggest_params_on_deformed_lattices(pse):
+    """pse_suggest_params_lattice (host only): the grid grows by the largest column norm of A, P stays, and the cutoff must fit the
+    deformed cell in lattice coordinates (reading R22)."""
+    base = pse.pse_suggest_params(4096, 44.1, 1.0, 1e-3, 0.5)
+    assert pse.pse_suggest_params(4096, 44.1, 1.0, 1e-3, 0.5, lattice=(1.0, 0.0, 1.0)) == base
+    st, grid, P, rcut = pse.pse_suggest_params(4096, 44.1, 1.0, 1e-3, 0.5, lattice=(1.0, 0.5, 1.0))
+    assert st == 0 and P == base[2] and rcut == base[3]
+    need = 1.07 * 2 * 0.5 * np.sqrt(-np.log(1e-3)) * 44.1 / np.pi
+    assert grid >= need * np.sqrt(1.25) > base[1] * 0.999 and grid > base[1]
+    st, grid2, _, _ = pse.pse_suggest_params(4096, 44.1, 1.0, 1e-3, 0.5, lattice=(1.25, 0.0, 0.8))
+    assert st == 0 and grid2 >= need * 1.25
+    assert pse.pse_suggest_params(4096, 44.1, 1.0, 1e-3, 0.5, lattice=(1.0, 0.0, 1.2))[0] == pse.PSE_EINVAL      # det A != 1
+    assert pse.pse_suggest_params(64, 13.892, 1.0, 1e-3, 0.6, lattice=(1.0, 1.0, 1.0))[0] == pse.PSE_EINVAL      # 5.38 * sqrt2 > L/2
+
+
 def test_create_validates_arguments_and_fails_loudly_without_gpu(pse):
     import torch
     eta = 1 / (6 * np.pi)

@@ -1,0 +1,198 @@
+"""GPU parity on deformed lattices: pse_set_lattice + the existing calls against
+oracle/lattice.py (direct Ewald sums with lattice vectors L A and k = (2 pi/L) A^-T n).  Bars as on the cube: neighbour sets bit-exact,
+products and samples within max(2 tol, 1e-5) relative L2."""
+import numpy as np
+import pytest
+
+import synth
+from oracle import lattice as lat
+from oracle import mobility as mob
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip('torch')
+
+A, ETA, KT = 1.0, 1.0 / (6.0 * np.pi), 1.0
+SHEAR, EXT = (1.0, 0.5, 1.0), (1.25, 0.0, 0.8)
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, float) - np.asarray(b, float)) / np.linalg.norm(np.asarray(b, float)))
+
+
+def bar(tol):
+    return max(2 * tol, 1e-5)
+
+
+def dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x), dtype=torch.float32).cuda().contiguous()
+
+
+def pos4(x):
+    p = np.zeros((x.shape[0], 4), np.float32)
+    p[:, :3] = x
+    return p
+
+
+def matrix(l3):
+    return np.array([[l3[0], l3[1], 0.0], [0.0, l3[2], 0.0], [0.0, 0.0, 1.0]])
+
+
+def deformed_suspension(N, phi, l3, seed, images=True):
+    """A seeded hard-sphere suspension of the cube carried along by the deformation (x = A s: what Lees-Edwards / Kraynik-Reinelt
+    boxes hold after straining), then every particle moved to a random periodic image (lattice vectors = columns of L A)."""
+    s, L = synth.rsa(N, phi, seed=seed)
+    Am = matrix(l3)
+    x = s @ Am.T
+    if images:
+        n = np.random.default_rng(seed).integers(-1, 2, size=(N, 3))
+        x = x + L * (n @ Am.T)
+    return x.astype(np.float32), L
+
+
+def make(N, L, xi, tol, l3, x32):
+    import paper_1709_06946_b200 as pse
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi, lattice=l3)
+    assert st == 0, 'rcut does not fit the deformed cell'
+    ctx = pse.pse_create(N, L, A, ETA, KT, xi, g, p, rcut, tol)
+    ctx.pse_set_lattice(*l3)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    return ctx, rcut
+
+
+def gpu_apply(ctx, F, S, which=3):
+    N = ctx.N
+    U, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_mobility_apply(dev(F), dev(S), U, E, which)
+    torch.cuda.synchronize()
+    return U.cpu().numpy(), E.cpu().numpy()
+
+
+def nbr_sets(ctx):
+    count, index = ctx.pse_get_neighbors()
+    count, index = count.cpu().numpy(), index.cpu().numpy()
+    off = np.concatenate([[0], np.cumsum(count)])
+    return [np.sort(index[off[i]:off[i + 1]]) for i in range(len(count))]
+
+
+@pytest.mark.parametrize('l3', [SHEAR, EXT, (1.0, -0.3, 1.0)])
+def test_neighbour_sets_bit_exact_on_deformed_lattices(l3):
+    N = 3000
+    x32, L = deformed_suspension(N, 0.25, l3, seed=3)
+    ctx, rcut = make(N, L, 0.6, 1e-3, l3, x32)
+    got = nbr_sets(ctx)
+    want = lat.neighbor_sets(x32, L, *l3, rcut)
+    assert sum(len(w) for w in want) > 20 * N
+    assert all(np.array_equal(g, w) for g, w in zip(got, want))
+
+
+def test_identity_lattice_is_the_cube_bit_for_bit():
+    import paper_1709_06946_b200 as pse
+    N, xi, tol = 2000, 0.6, 1e-3
+    x, L = synth.rsa(N, 0.2, seed=2)
+    x32 = x.astype(np.float32)
+    F, S = synth.gaussian_inputs(N, 1)
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert pse.pse_suggest_params(N, L, A, tol, xi, lattice=(1.0, 0.0, 1.0)) == (st, g, p, rcut)
+    outs = []
+    for set_it in (False, True):
+        ctx = pse.pse_create(N, L, A, ETA, KT, xi, g, p, rcut, tol)
+        if set_it:
+            ctx.pse_set_lattice(1.0, 0.7, 1.0)
+            ctx.pse_set_lattice(1.0, 0.0, 1.0)
+        ctx.pse_neighbors(dev(pos4(x32)))
+        outs.append(gpu_apply(ctx, F, S))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+@pytest.mark.parametrize('l3,tol', [(SHEAR, 1e-3), (SHEAR, 1e-4), (EXT, 1e-3)])
+def test_product_on_deformed_lattice_against_direct_sums(l3, tol):
+    """N = 400 all rows: total, and the real and wave halves separately (relative to the total)."""
+    N, xi = 400, 0.55
+    x32, L = deformed_suspension(N, 0.20, l3, seed=7)
+    ctx, _ = make(N, L, xi, tol, l3, x32)
+    F, S = synth.gaussian_inputs(N, 3)
+    x = x32.astype(np.float64)
+    Uo, Eo = lat.mobility_apply(x, L, matrix(l3), A, ETA, xi, F, S, eps=1e-10)
+    U, E = gpu_apply(ctx, F, S)
+    assert rel(U, Uo) < bar(tol) and rel(E, Eo) < bar(tol), (rel(U, Uo), rel(E, Eo))
+    for which, part in ((1, 'real'), (2, 'wave')):
+        Up, Ep = lat.mobility_apply(x, L, matrix(l3), A, ETA, xi, F, S, eps=1e-10, part=part)
+        Ug, Eg = gpu_apply(ctx, F, S, which)
+        assert np.linalg.norm(Ug - Up) < bar(tol) * np.linalg.norm(Uo) and np.linalg.norm(Eg - Ep) < bar(tol) * np.linalg.norm(Eo), part
+    # the cube's operator is a different one: the deformation is really in the numbers
+    Uc, Ec = mob.mobility_apply(x, L, A, ETA, xi, F, S, eps=1e-8)
+    assert rel(U, Uc) > 50 * bar(tol)
+
+
+def test_product_sampled_rows_mid_size_sheared():
+    N, xi, tol, l3 = 2000, 0.5, 1e-3, (1.0, 0.4, 1.0)
+    x32, L = deformed_suspension(N, 0.25, l3, seed=11)
+    ctx, _ = make(N, L, xi, tol, l3, x32)
+    F, S = synth.gaussian_inputs(N, 4)
+    rows = np.sort(np.random.default_rng(3).choice(N, 12, replace=False))
+    Uo, Eo = lat.mobility_apply(x32.astype(np.float64), L, matrix(l3), A, ETA, xi, F, S, rows=rows, eps=1e-9)
+    U, E = gpu_apply(ctx, F, S)
+    assert rel(U[rows], Uo) < bar(tol) and rel(E[rows], Eo) < bar(tol), (rel(U[rows], Uo), rel(E[rows], Eo))
+
+
+def test_a_shear_by_a_whole_lattice_vector_is_the_same_lattice_on_the_gpu():
+    """gamma and gamma - 1 describe the same lattice: the same physical positions give the same product."""
+    N, xi, tol = 800, 0.6, 1e-3
+    x32, L = deformed_suspension(N, 0.2, (1.0, 0.3, 1.0), seed=5)
+    F, S = synth.gaussian_inputs(N, 5)
+    ctx_a, _ = make(N, L, xi, tol, (1.0, 0.3, 1.0), x32)
+    ctx_b, _ = make(N, L, xi, tol, (1.0, -0.7, 1.0), x32)
+    Ua, Ea = gpu_apply(ctx_a, F, S)
+    Ub, Eb = gpu_apply(ctx_b, F, S)
+    assert rel(Ub, Ua) < bar(tol) and rel(Eb, Ea) < bar(tol)
+
+
+def test_brownian_sample_constrained_solve_and_overlap_forces_on_a_sheared_lattice():
+    N, xi, tol, l3, dt = 150, 0.7, 1e-3, (1.0, 0.4, 1.0), 1e-3
+    x32, L = deformed_suspension(N, 0.25, l3, seed=9)
+    ctx, rcut = make(N, L, xi, tol, l3, x32)
+    x, Am = x32.astype(np.float64), matrix(l3)
+    w1, w2 = synth.brownian_noise(N, ctx.grid, 4)
+    UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_brownian(dt, dev(w1.reshape(N, 8)), dev(w2), UB, EB)
+    Uo, Eo = lat.brownian(x, L, Am, A, ETA, KT, xi, dt, ctx.grid, w1, w2, eps=1e-10)
+    assert rel(UB.cpu().numpy(), Uo) < bar(tol) and rel(EB.cpu().numpy(), Eo) < bar(tol), (rel(UB.cpu().numpy(), Uo), rel(EB.cpu().numpy(), Eo))
+    # overlap forces: pairs closer than 2a from the oracle's image search
+    ia, ib, rv = lat.real_pairs(x, L, Am, 2.0 * A)
+    keep = ia != ib
+    ia, rv = ia[keep], rv[keep]
+    r = np.linalg.norm(rv, axis=1)
+    Fo = np.zeros((N, 3))
+    np.add.at(Fo, ia, (3 * np.pi * ETA * A * (2 * A - r) / dt / r)[:, None] * rv)
+    assert np.abs(Fo).max() > 0
+    Fp = torch.empty(N, 3, device='cuda')
+    ctx.pse_hard_sphere_forces(dt, Fp)
+    assert rel(Fp.cpu().numpy(), Fo) < 1e-4
+    # constrained solve against the dense matrix of the deformed lattice
+    from oracle import brownian as brn
+    M = lat.dense(x, L, Am, A, ETA, xi, eps=1e-10)
+    rng = np.random.default_rng(2)
+    F, UBh, EBh = rng.standard_normal((N, 3)), rng.standard_normal((N, 3)), rng.standard_normal((N, 5))
+    Us, Ss = brn.constrained_solve(M, N, UBh, EBh, F)
+    U, S = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_constrained_solve(dev(F), dev(UBh), dev(EBh), U, S)
+    assert rel(U.cpu().numpy(), Us) < 3 * bar(tol) and rel(S.cpu().numpy(), Ss) < 5 * bar(tol)
+    # a step runs on the deformed lattice (positions stay unwrapped) and repeats bit for bit
+    pos = dev(pos4(x32))
+    p1, p2 = pos.clone(), pos.clone()
+    ctx.pse_step(p1, dt, dev(w1.reshape(N, 8)), dev(w2))
+    ctx.pse_step(p2, dt, dev(w1.reshape(N, 8)), dev(w2))
+    assert torch.isfinite(p1).all() and torch.equal(p1, p2) and float((p1 - pos).abs().max()) > 0
+
+
+def test_set_lattice_rejects_what_it_cannot_do():
+    import paper_1709_06946_b200 as pse
+    N = 64
+    x, L = synth.rsa(N, 0.10, seed=1)
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, 1e-3, 0.6)
+    ctx = pse.pse_create(N, L, A, ETA, KT, 0.6, g, p, rcut, 1e-3)
+    for bad in ((1.0, 0.0, 1.1), (-1.0, 0.0, -1.0), (2.0, 0.0, 0.5)):       # not volume preserving; negative; rcut no longer fits
+        with pytest.raises(pse.PSEError) as e:
+            ctx.pse_set_lattice(*bad)
+        assert e.value.status == pse.PSE_EINVAL
+    assert pse.pse_suggest_params(N, L, A, 1e-3, 0.6, lattice=(2.0, 0.0, 0.5))[0] == pse.PSE_EINVAL
