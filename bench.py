@@ -117,7 +117,7 @@ def make_suspension(wl, seed):
 def choose_params(wl, L, need_gpu_lib=True):
     """grid, P, r_cut of the run from pse_suggest_params (host-only entry point of libpse.so: parameter arithmetic, no kernels)."""
     import paper_1709_06946_b200 as pse
-    st, grid, P, rcut = pse.pse_suggest_params(wl['N'], L, A, wl['tol'], wl['xi'])
+    st, grid, P, rcut = pse.pse_suggest_params(wl['N'], L, A, wl['tol'], wl['xi'], lattice=(1.0, wl.get('shear', 0.0), 1.0))
     if st != 0:
         raise RuntimeError(f'no valid PSE parameters for {wl}')
     return grid, P, rcut
@@ -158,6 +158,10 @@ def run_ours(args, wl, rank, world):
     x, L = make_suspension(wl, seed=100 + rank)
     grid, P, rcut = choose_params(wl, L)
     ctx = pse.pse_create(N, L, A, ETA, KT, wl['xi'], grid, P, rcut, wl['tol'])
+    if wl.get('shear'):                              # Lees-Edwards cell of strain gamma (Eq. 56): the suspension is carried along, x = A s
+        ctx.pse_set_lattice(1.0, wl['shear'], 1.0)
+        x = x.copy()
+        x[:, 0] += wl['shear'] * x[:, 1]
     pos = torch.zeros(N, 4, device=dev)
     pos[:, :3] = torch.from_numpy(x.astype(np.float32)).to(dev)
     gen = torch.Generator(device=dev); gen.manual_seed(1234 + rank)
@@ -369,6 +373,8 @@ def assemble(name, wl, r, K, world, overridden):
     out = {'value': value, 'ms_per_step': ms_step}
     out['config'] = {'workload': describe(name, wl), 'N': wl['N'], 'phi': wl['phi'], 'tol': wl['tol'], 'xi': wl['xi'], 'dt': wl['dt'],
                      'grid': r['grid'], 'rcut': round(r['rcut'], 4), 'L': round(r['L'], 4)}
+    if wl.get('shear'):
+        out['config']['lattice'] = f"simple shear, strain {wl['shear']} (Eq. 56): lattice vectors = columns of L [[1, {wl['shear']}, 0], [0, 1, 0], [0, 0, 1]]"
     out['run'] = {'window': 'exponential of semicircle', 'P': r['P'], 'mean_neighbors': round(r['nb_mean'], 2), 'gmres_iters': r['gmres'],
                   'lanczos_iters': r['lanczos'], 'parallelism': f'replicas x{world}' if world > 1 else 'single GPU',
                   'l2': 'flushed (256 MiB write) between timed steps; each step bracketed by its own CUDA events'}
@@ -414,9 +420,16 @@ def main():
     ap.add_argument('--xi', type=float, default=None, help='override the splitting parameter (tuning knob, PAPER.md:154)')
     ap.add_argument('--tol', type=float, default=None, help='override the Ewald tolerance of the workload')
     ap.add_argument('--particles', type=int, default=None, help='override N of the workload (size sweep; phi, tol and xi are kept)')
+    ap.add_argument('--shear', type=float, default=None, help='run the workload in a sheared periodic cell of this strain (Eq. 56, PAPER.md:318); '
+                                                               'implies --no-cpu-baseline (the reference tier is cubic)')
     args = ap.parse_args()
     wl = dict(WORKLOADS[args.workload])
-    overridden = bool(args.xi or args.tol or args.particles)
+    overridden = bool(args.xi or args.tol or args.particles or args.shear)
+    if args.shear:
+        if args.impl == 'reference':
+            raise SystemExit('bench.py: --shear has no reference arm (oracle/pse_reference.py is cubic)')
+        wl['shear'] = args.shear
+        args.no_cpu_baseline = True
     if args.xi:
         wl['xi'] = args.xi
     if args.tol:
