@@ -45,13 +45,18 @@ def pair_apply_full(rvec, F, Lq, S, R, pref):
     return U, W, E
 
 
-def real_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14, rcut=None):
-    """[U;Omega;E]_rows = M^(r) [F;L;S]: direct lattice sum incl. self term and periodic images (as oracle.mobility.real_apply)."""
+def real_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14, rcut=None, A=None):
+    """[U;Omega;E]_rows = M^(r) [F;L;S]: direct lattice sum incl. self term and periodic images (as oracle.mobility.real_apply).
+    A (3x3, det 1): deformed lattice, image vectors L A n (oracle.lattice)."""
     x = np.asarray(x, dtype=np.float64)
     N = x.shape[0]
     rows = np.arange(N) if rows is None else np.asarray(rows)
     rmax = mob.real_cutoff(xi, a, eps) if rcut is None else rcut
-    ia, ib, rv = mob.real_pairs(x, L, rmax, rows)
+    if A is None:
+        ia, ib, rv = mob.real_pairs(x, L, rmax, rows)
+    else:
+        from . import lattice as lat
+        ia, ib, rv = lat.real_pairs(x, L, A, rmax, rows)
     if rcut is not None:
         keep = np.einsum('ni,ni->n', rv, rv) < rcut * rcut
         ia, ib, rv = ia[keep], ib[keep], rv[keep]
@@ -95,19 +100,23 @@ def wave_apply_modes_full(x, a, k, weight, F, Lq, S5, rows=None, chunk=None):
     return U, W, E
 
 
-def wave_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14):
-    k = mob.wave_vectors(L, mob.wave_cutoff(xi, eps))
+def wave_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14, A=None):
+    if A is None:
+        k = mob.wave_vectors(L, mob.wave_cutoff(xi, eps))
+    else:
+        from . import lattice as lat
+        k = lat.wave_vectors(L, A, mob.wave_cutoff(xi, eps))
     k2 = np.einsum('ki,ki->k', k, k)
     return wave_apply_modes_full(x, a, k, fn.hasimoto_H(np.sqrt(k2), xi) / (eta * L**3 * k2), F, Lq, S5, rows)
 
 
-def mobility_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14, part='both'):
-    """[U;Omega;E]_rows = (M^(r) + M^(w)) [F;L;S]  (Eqs. 30-31, PAPER.md:167-175)."""
+def mobility_apply_full(x, L, a, eta, xi, F, Lq, S5, rows=None, eps=1e-14, part='both', A=None):
+    """[U;Omega;E]_rows = (M^(r) + M^(w)) [F;L;S]  (Eqs. 30-31); A: deformed lattice (oracle.lattice)."""
     out = [0.0, 0.0, 0.0]
     if part in ('both', 'real'):
-        out = [o + v for o, v in zip(out, real_apply_full(x, L, a, eta, xi, F, Lq, S5, rows, eps))]
+        out = [o + v for o, v in zip(out, real_apply_full(x, L, a, eta, xi, F, Lq, S5, rows, eps, A=A))]
     if part in ('both', 'wave'):
-        out = [o + v for o, v in zip(out, wave_apply_full(x, L, a, eta, xi, F, Lq, S5, rows, eps))]
+        out = [o + v for o, v in zip(out, wave_apply_full(x, L, a, eta, xi, F, Lq, S5, rows, eps, A=A))]
     return tuple(out)
 
 

@@ -196,3 +196,25 @@ def test_set_lattice_rejects_what_it_cannot_do():
             ctx.pse_set_lattice(*bad)
         assert e.value.status == pse.PSE_EINVAL
     assert pse.pse_suggest_params(N, L, A, 1e-3, 0.6, lattice=(2.0, 0.0, 0.5))[0] == pse.PSE_EINVAL
+
+
+def test_full_couplet_and_paper_window_on_a_sheared_lattice():
+    """The torque / angular-velocity rows (pse_mobility_apply_full) and the paper's Gaussian window, both on a sheared cell."""
+    import paper_1709_06946_b200 as pse
+    from oracle import couplet as cpl
+    N, xi, tol, l3 = 400, 0.55, 1e-3, (1.0, 0.4, 1.0)
+    x32, L = deformed_suspension(N, 0.20, l3, seed=13)
+    x, Am = x32.astype(np.float64), matrix(l3)
+    F, S = synth.gaussian_inputs(N, 6)
+    Lq = np.random.default_rng(6).standard_normal((N, 3))
+    want = cpl.mobility_apply_full(x, L, A, ETA, xi, F, Lq, S, eps=1e-10, A=Am)
+    for window in (pse.PSE_WINDOW_ES, pse.PSE_WINDOW_GAUSS):
+        st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi, window, lattice=l3)
+        assert st == 0
+        ctx = pse.pse_create(N, L, A, ETA, KT, xi, g, p, rcut, tol, window=window)
+        ctx.pse_set_lattice(*l3)
+        ctx.pse_neighbors(dev(pos4(x32)))
+        U, W, E = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+        ctx.pse_mobility_apply_full(dev(F), dev(Lq), dev(S), U, W, E)
+        for got, w, name in zip((U, W, E), want, 'UWE'):
+            assert rel(got.cpu().numpy(), w) < bar(tol), (window, name, rel(got.cpu().numpy(), w))

@@ -151,3 +151,17 @@ def test_C6_constrained_solve_with_torques_leaves_no_rate_of_strain():
     U0, W0, S0 = cpl.constrained_solve_full(M, 4, UB, WB, EB, F, 0 * Lq)
     U8, S8 = brn.constrained_solve(mob.dense(x, L, A, ETA, 0.7), 4, UB, EB, F)
     assert rel(U0, U8) < 1e-11 and rel(S0, S8) < 1e-11
+
+
+def test_C7_full_couplet_on_a_deformed_lattice_split_independence_and_lattice_equivalence():
+    """The torque rows on a sheared cell (oracle.lattice): xi-independence, and gamma -> gamma - 1 is the same lattice."""
+    from oracle import lattice as lat
+    x, L = cluster()
+    rng = np.random.default_rng(6)
+    F, Lq, S = rng.standard_normal((5, 3)), rng.standard_normal((5, 3)), rng.standard_normal((5, 5))
+    a_ = np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S, A=lat.shear(0.4)))
+    b_ = np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.9, F, Lq, S, A=lat.shear(0.4)))
+    c_ = np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S, A=lat.shear(-0.6)))
+    assert rel(b_, a_) < 1e-11 and rel(c_, a_) < 1e-11
+    cube = np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S))
+    assert rel(np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S, A=np.eye(3))), cube) < 1e-13 and rel(a_, cube) > 1e-3
