@@ -125,10 +125,19 @@ pse_status pse_constrained_solve(pse_ctx *ctx, const float *d_F, const float *d_
 pse_status pse_mobility_apply_full(pse_ctx *ctx, const float *d_F, const float *d_L, const float *d_S,
                                    float *d_U, float *d_W, float *d_E, int which);
 
+/* The Brownian slip of the full couplet, script-U^B = [U^B; Omega^B] and E^B (Eq. 76 with the 11 components of Eq. 31; the paper's
+ * "11" grids): sqrt(2 kT/dt) ( M_r^{1/2} w1 + M_w^{1/2} w2 ) with the 11N x 11N matrices.  The wave half draws the
+ * SAME random fluid velocity field as pse_brownian from the same d_noise_wave and reads three more moments of it
+ * (Omega_h = (i/2) s1 k x uh); the real half is a Lanczos iteration on the 11-component pair sum.
+ * d_noise_real: [N][11] i.i.d. N(0,1), per particle (Ux,Uy,Uz, Ox,Oy,Oz, e1..e5); d_noise_wave as in pse_brownian.
+ * d_UB [N][3], d_WB [N][3], d_EB [N][5] out (any may be NULL).  Synchronises the stream (every Lanczos iteration). */
+pse_status pse_brownian_full(pse_ctx *ctx, double dt, const float *d_noise_real, const float *d_noise_wave,
+                             float *d_UB, float *d_WB, float *d_EB, int *lanczos_iters);
+
 /* pse_constrained_solve with torques (Eqs. 36-38, with script-F = [F; L], script-U = [U; Omega]):
  * M_ES S = -(E^B + M_EF F + M_EL L) by GMRES, then U = U^B + M_UF F + M_UL L + M_US S and Omega = M_OF F + M_OL L + M_OS S.
  * d_F, d_L, d_UB, d_EB may be NULL (= 0); d_U [N][3], d_S [N][5] out; d_W [N][3] out, may be NULL (one product less).
- * No Brownian angular velocity enters: orientations of spheres are not tracked (R21). */
+ * Omega^B of pse_brownian_full, if wanted, is added by the caller (it does not enter the constraint). */
 pse_status pse_constrained_solve_full(pse_ctx *ctx, const float *d_F, const float *d_L, const float *d_UB, const float *d_EB,
                                       float *d_U, float *d_W, float *d_S, int *gmres_iters);
 

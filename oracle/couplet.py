@@ -152,3 +152,44 @@ def constrained_solve_full(M, N, UB, WB, EB, F, Lq):
     UW = np.concatenate([np.asarray(UB, float), np.asarray(WB, float)], axis=1).ravel() + M[np.ix_(iu, iu)] @ FL + M[np.ix_(iu, ie)] @ S
     UW = UW.reshape(N, 6)
     return UW[:, :3], UW[:, 3:], S.reshape(N, 5)
+
+
+def wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf, rows=None, A=None):
+    """A_w w2 of Eq. (75) with the angular-velocity rows: the random field uh = sqrt(H/(eta V k^2)) (I - kh kh) W(k)
+    over the modes of the Mg^3 grid is that of oracle.brownian.wave_sqrt_apply (same noise buffer, reading R8); here its moments are
+    U = s0 uh, Omega = (i/2) s1 k x uh, E^q = i s1 (e^q k).uh.  Returns U, Omega, E at the particles (rows)."""
+    from . import brownian as brn
+    x = np.asarray(x, dtype=np.float64)
+    if rows is not None:
+        x = x[np.asarray(rows)]
+    N = x.shape[0]
+    wbuf = np.asarray(wbuf, dtype=np.float64).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
+    idx, n = brn.canonical_modes(Mg)
+    k = 2 * np.pi * n / L if A is None else 2 * np.pi * (n @ np.linalg.inv(np.asarray(A, dtype=np.float64))) / L
+    Wn = (wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 0] + 1j * wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 1]).T / np.sqrt(2)
+    e = fn.basis()
+    U, W, E = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5))
+    chunk = max(1, 4_000_000 // max(N, 1))
+    for lo in range(0, k.shape[0], chunk):
+        kk, Wk = k[lo:lo + chunk], Wn[lo:lo + chunk]
+        k2 = np.einsum('ki,ki->k', kk, kk)
+        kn = np.sqrt(k2)
+        kh = kk / kn[:, None]
+        uh = np.sqrt(fn.hasimoto_H(kn, xi) / (eta * L**3 * k2))[:, None] * (Wk - kh * np.einsum('ki,ki->k', kh, Wk)[:, None])
+        pa = np.exp(1j * (kk @ x.T))
+        c0, c1 = fn.s0(kn * a), fn.s1(kn * a)
+        U += 2 * np.real(np.einsum('ka,ki->ai', pa, c0[:, None] * uh))
+        W += 2 * np.real(np.einsum('ka,ki->ai', pa, 0.5j * c1[:, None] * np.cross(kk, uh)))
+        E += 2 * np.real(np.einsum('ka,kq->aq', pa, 1j * c1[:, None] * np.einsum('qij,kj,ki->kq', e, kk, uh)))
+    return U, W, E
+
+
+def brownian_full(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14):
+    """Eq. (76) for the 11 components: sqrt(2kT/dt) ( M_r^{1/2} w1 + A_w w2 ), M_r the dense 11N x 11N real-space
+    matrix (principal root), w1 (N, 11) in the (U, Omega, E) ordering.  Returns U^B, Omega^B, E^B."""
+    from . import brownian as brn
+    N = np.asarray(x).shape[0]
+    yr = (brn.sqrtm_psd(dense_full(x, L, a, eta, xi, part='real', eps=eps)) @ np.asarray(w1, dtype=np.float64).ravel()).reshape(N, 11)
+    Uw, Ww, Ew = wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf)
+    amp = np.sqrt(2.0 * kT / dt)
+    return amp * (yr[:, :3] + Uw), amp * (yr[:, 3:6] + Ww), amp * (yr[:, 6:] + Ew)

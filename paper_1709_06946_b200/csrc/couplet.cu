@@ -161,11 +161,24 @@ __global__ void k_merge_force_stresslet(const float4 *a, const float4 *b, int N,
     out[2 * s + 1] = b[2 * s + 1];
 }
 
+// noise [N][11] = (Ux,Uy,Uz, Ox,Oy,Oz, e1..e5) per particle, original numbering -> wide packed vector [2][N][8], sorted numbering
+__global__ void k_pack11(const float *v11, const int *order, int N, float4 *wide) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float *v = v11 + 11 * (size_t)order[s];
+    wide[2 * s] = make_float4(v[0], v[1], v[2], v[6]);
+    wide[2 * s + 1] = make_float4(v[7], v[8], v[9], v[10]);
+    wide[2 * (size_t)N + 2 * s] = make_float4(v[3], v[4], v[5], 0.f);
+    wide[2 * (size_t)N + 2 * s + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
 }  // namespace
 
 void pse_couplet_free(pse_ctx *c) {
     cudaFree(c->d_rot_table); cudaFree(c->d_spec_rot); cudaFree(c->d_rot_in); cudaFree(c->d_rot_out); cudaFree(c->d_rot_tmp);
+    cudaFree(c->d_rot_w); cudaFree(c->d_rot_y); cudaFree(c->d_rot_u);
     c->d_rot_table = nullptr; c->d_spec_rot = nullptr; c->d_rot_in = c->d_rot_out = c->d_rot_tmp = nullptr;
+    c->d_rot_w = c->d_rot_y = c->d_rot_u = nullptr;
 }
 
 // table, spectrum and packed vectors of the torque rows: made by the first call that needs them (synchronises once)
@@ -176,6 +189,7 @@ static pse_status ensure_couplet(pse_ctx *c) {
     const size_t nmode = (size_t)c->M * c->M * c->Mh, vec = (size_t)c->N * 8 * sizeof(float);
     if (cudaMalloc(&c->d_spec_rot, 3 * nmode * sizeof(cufftComplex)) != cudaSuccess || cudaMalloc(&c->d_rot_in, vec) != cudaSuccess ||
         cudaMalloc(&c->d_rot_out, vec) != cudaSuccess || cudaMalloc(&c->d_rot_tmp, vec) != cudaSuccess ||
+        cudaMalloc(&c->d_rot_w, 2 * vec) != cudaSuccess || cudaMalloc(&c->d_rot_y, 2 * vec) != cudaSuccess || cudaMalloc(&c->d_rot_u, 2 * vec) != cudaSuccess ||
         cudaMalloc(&c->d_rot_table, tab.size() * sizeof(float)) != cudaSuccess) {
         cudaGetLastError();
         pse_couplet_free(c);
@@ -221,7 +235,29 @@ static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *i
     return pse_wave_interp(c, outW, true, 1);
 }
 
+// the real-space half on a wide vector [2][N][8]: (U, E | Omega) = M_r (F, S | L)
+static pse_status real_full_wide(pse_ctx *c, const float *d_in, float *d_out) {
+    const size_t half = (size_t)c->N * 8;
+    return apply_full_packed(c, d_in, d_in + half, d_out, d_out + half, PSE_REAL);
+}
+
 extern "C" {
+
+pse_status pse_brownian_full(pse_ctx *c, double dt, const float *d_noise_real, const float *d_noise_wave, float *d_UB, float *d_WB, float *d_EB,
+                             int *lanczos_iters) {
+    if (!c || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
+    if (!c->have_nbrs) { c->err = "pse_brownian_full before pse_neighbors"; return PSE_ENOTREADY; }
+    PSE_TRY(ensure_couplet(c));
+    const size_t half = (size_t)c->N * 8;
+    k_pack11<<<(c->N + 255) / 256, 256, 0, c->stream>>>(d_noise_real, c->d_order, c->N, reinterpret_cast<float4 *>(c->d_rot_w)); KERNEL_CHECK(c);
+    pse_status st = pse_lanczos_sqrt_wide(c, c->d_rot_w, c->d_rot_y, lanczos_iters, 2, real_full_wide, c->d_rot_u);
+    if (st != PSE_OK && st != PSE_ENOCONV) return st;
+    PSE_TRY(pse_wave_brownian(c, d_noise_wave, c->d_rot_y, true, c->d_rot_y + half));
+    const float amp = (float)std::sqrt(2.0 * c->kT / dt);
+    if (d_UB || d_EB) PSE_TRY(pse_unpack(c, c->d_rot_y, amp, d_UB, d_EB));
+    if (d_WB) PSE_TRY(pse_unpack(c, c->d_rot_y + half, amp, d_WB, nullptr));
+    return st;
+}
 
 pse_status pse_mobility_apply_full(pse_ctx *c, const float *d_F, const float *d_L, const float *d_S, float *d_U, float *d_W, float *d_E, int which) {
     if (!c || !(which & PSE_BOTH) || (!d_F && !d_L && !d_S) || (!d_U && !d_W && !d_E)) return PSE_EINVAL;

@@ -389,11 +389,21 @@ pse_status pse_axpby(pse_ctx *c, size_t n, float alpha, const float *x, float be
 // Stop when |y_m - y_{m-1}| <= tol |y_m|; with V orthonormal this is the change of the coefficient vector.
 // fixed_m > 0: exactly fixed_m iterations, coefficients by k_lanczos_coef_dev, no host read-back: the scalars are copied to
 // h_scal_l behind the solve and examined by pse_lanczos_validate once the stream has been synchronised.
+static pse_status real_apply_all(pse_ctx *c, const float *d_in, float *d_out) { return pse_real_apply(c, d_in, d_out); }
+static pse_status lanczos_impl(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m, int width, pse_matvec_fn op, float *d_u);
+
 pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m) {
-    const size_t n = (size_t)c->N * 8, n4 = n / 4;
+    return lanczos_impl(c, d_w, d_y, iters, fixed_m, 1, real_apply_all, c->d_tmp);
+}
+pse_status pse_lanczos_sqrt_wide(pse_ctx *c, const float *d_w, float *d_y, int *iters, int width, pse_matvec_fn op, float *d_u) {
+    return lanczos_impl(c, d_w, d_y, iters, 0, width, op, d_u);
+}
+
+static pse_status lanczos_impl(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m, int width, pse_matvec_fn op, float *d_u) {
+    const size_t n = (size_t)c->N * 8 * width, n4 = n / 4;
     float4 *V = reinterpret_cast<float4 *>(c->d_krylov);
-    float4 *u = reinterpret_cast<float4 *>(c->d_tmp);
-    const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap - 1);
+    float4 *u = reinterpret_cast<float4 *>(d_u);
+    const int maxit = std::min(PSE_MAX_KRYLOV, c->krylov_cap / width - 1);
     // slots: [0] = |w|^2, [1+2j] = alpha_j, [2+2j] = beta_j^2
     const int nslots = 1 + 2 * maxit;
     PSE_TRY(zero_scalars(c, nslots));
@@ -410,12 +420,12 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
     // the skipped iterations are then examined in order and the first converged one is taken — same result as
     // checking every time.
     // (once the count has repeated, only the iteration it is expected to end in is read back: one synchronisation per solve)
-    const int first_check = std::max(0, c->last_lanczos_iters - (c->lanczos_repeats >= 2 ? 1 : 2));
+    const int first_check = width > 1 ? 0 : std::max(0, c->last_lanczos_iters - (c->lanczos_repeats >= 2 ? 1 : 2));
     int examined = 0;
     const int niter = fixed_m > 0 ? std::min(fixed_m, maxit) : maxit;
     for (int j = 0; j < niter && !converged; ++j) {
         float4 *vj = V + (size_t)j * n4;
-        PSE_TRY(pse_real_apply(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
+        PSE_TRY(op(c, reinterpret_cast<const float *>(vj), reinterpret_cast<float *>(u)));
         { ScopedPhase ph(c, PSE_T_VECTOR);
           const float4 *a_vj = vj, *a_vjm1 = j ? vj - n4 : nullptr;
           float4 *a_u = u, *a_next = j + 1 < niter ? vj + n4 : nullptr;
@@ -461,8 +471,10 @@ pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters
         if (iters) *iters = niter;
         return PSE_OK;
     }
-    c->lanczos_repeats = (m == c->last_lanczos_iters) ? c->lanczos_repeats + 1 : 0;
-    c->last_lanczos_iters = m;
+    if (width == 1) {
+        c->lanczos_repeats = (m == c->last_lanczos_iters) ? c->lanczos_repeats + 1 : 0;
+        c->last_lanczos_iters = m;
+    }
     std::vector<float> cf(ccur.begin(), ccur.end());
     PSE_TRY(upload_coefs(c, cf));
     { ScopedPhase ph(c, PSE_T_VECTOR);

@@ -141,6 +141,9 @@ struct pse_ctx {
     float *d_rot_table = nullptr;            // [PSE_NTAB][4] = (T/2, Z0/6, Z2/4, 0)/(6 pi eta a) at the nodes of d_table
     cufftComplex *d_spec_rot = nullptr;      // [3][M][M][Mh] spectrum of the torque planes in, of the angular-velocity planes out
     float *d_rot_in = nullptr, *d_rot_out = nullptr, *d_rot_tmp = nullptr;   // [N][8] packed: (Lx,Ly,Lz,0..), (Ox,Oy,Oz,0..), scratch
+    float *d_rot_w = nullptr, *d_rot_y = nullptr, *d_rot_u = nullptr;        // [2][N][8] each: 11-component Lanczos input, result, work vector
+    cufftComplex *d_spec_rot_b = nullptr;    // [3][Mb][Mb][Mbh] angular-velocity spectra of the Brownian pass (finer grid)
+    cufftHandle plan_c2r_rot_b = 0; bool have_plan_rot_b = false;
     // ---- bonds of the equilibrium test potential U = k |r - r0|, original numbering ----
     int2 *d_bonds = nullptr; int n_bonds = 0; double bond_k = 0, bond_r0 = 0;
     // ---- staging for the host-buffer entry points ----
@@ -245,7 +248,7 @@ pse_status pse_particle_windows(pse_ctx *c);   // d_pbase, d_pw from d_pos (afte
 pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accumulate, int mode = PSE_MODE_ALL);   // out (+)= M_w in
 pse_status pse_wave_spread(pse_ctx *c, const float *d_in, int plan);                    // packed vector -> c->d_grid, planes of plan 0 / 1 / 2
 pse_status pse_wave_interp(pse_ctx *c, float *d_out, bool accumulate, int oplan);      // c->d_grid -> packed vector, planes of oplan 3 / 1 / 2
-pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate);
+pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate, float *d_outW = nullptr);
 // couplet.cu (torque / angular-velocity rows, NEXT-3)
 void pse_couplet_free(pse_ctx *c);
 void pse_build_rot_table(double a, double eta, double xi, double rcut, int ntab, std::vector<float> &tab);   // tables.cu
@@ -255,6 +258,10 @@ pse_status pse_pack(pse_ctx *c, const float *d_F, const float *d_S, float *d_pac
 pse_status pse_pack8(pse_ctx *c, const float *d_v8, float *d_packed);
 pse_status pse_unpack(pse_ctx *c, const float *d_packed, float scale, float *d_U, float *d_E);
 pse_status pse_lanczos_sqrt(pse_ctx *c, const float *d_w, float *d_y, int *iters, int fixed_m = 0);          // y = M_r^{1/2} w
+// the same iteration on vectors of `width` packed arrays ([width][N][8], width = 2: force/stresslet slots then torque slots) with
+// any operator out = A in and work vector d_u of that size; checks convergence every iteration, leaves the iteration history alone
+typedef pse_status (*pse_matvec_fn)(pse_ctx *c, const float *d_in, float *d_out);
+pse_status pse_lanczos_sqrt_wide(pse_ctx *c, const float *d_w, float *d_y, int *iters, int width, pse_matvec_fn op, float *d_u);
 bool pse_lanczos_validate(pse_ctx *c, int m, bool *shrink);
 bool pse_gmres_validate(pse_ctx *c, int m, bool *shrink);
 pse_status pse_gmres_constraint(pse_ctx *c, const float *d_Fp, const float *d_UBp, const float *d_EBp,

@@ -641,7 +641,8 @@ __global__ void __launch_bounds__(256) scale_kernel(cufftComplex *spec, ScalePar
 // conjugate of its partner's entry (reading R8) so that the C2R transform sees a Hermitian field.  The thread grid is the half
 // spectrum of the FINER grid sp.M of the Brownian pass; the noise buffer is laid out on the product grid sp.Mc <= sp.M and only
 // its modes carry weight (zero-padded spectrum): same field as on the product grid, interpolated with an oversampled window.
-__global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec, const float2 *__restrict__ noise, ScaleParams sp) {
+// rot != nullptr: the angular-velocity planes Omega_h = (i/2) s1 k x uh of the same random field go to rot[3][modes] (full couplet, R21).
+__global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec, const float2 *__restrict__ noise, ScaleParams sp, cufftComplex *rot) {
     const int M = sp.M, Mc = sp.Mc;
     const unsigned plane = (unsigned)M * (unsigned)sp.Mh, rem = blockIdx.x * blockDim.x + threadIdx.x;
     if (rem >= plane) return;
@@ -655,6 +656,7 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     if (!live) {
 #pragma unroll
         for (int c = 0; c < 8; ++c) spec[c * nmode + o] = zero;
+        if (rot) { rot[o] = zero; rot[nmode + o] = zero; rot[2 * nmode + o] = zero; }
         return;
     }
     const float kx = sp.two_pi_over_L * (sp.ki11 * (float)nx), ky = sp.two_pi_over_L * (sp.ki22 * (float)ny + sp.ki12 * (float)nx), kz = sp.two_pi_over_L * (float)nz;
@@ -676,6 +678,15 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
     const float2 uy = make_float2(Bh * (W[1].x - ky * kw.x), Bh * (W[1].y - ky * kw.y));
     const float2 uz = make_float2(Bh * (W[2].x - kz * kw.x), Bh * (W[2].y - kz * kw.y));
     write_outputs(spec, nmode, o, s0, s1, kx, ky, kz, ux, uy, uz, PSE_OUT_U | PSE_OUT_E);
+    if (rot) {
+        const float h1 = 0.5f * s1;
+        const float2 wx = make_float2(ky * uz.x - kz * uy.x, ky * uz.y - kz * uy.y);
+        const float2 wy = make_float2(kz * ux.x - kx * uz.x, kz * ux.y - kx * uz.y);
+        const float2 wz = make_float2(kx * uy.x - ky * ux.x, kx * uy.y - ky * ux.y);
+        rot[o] = make_float2(-h1 * wx.y, h1 * wx.x);
+        rot[nmode + o] = make_float2(-h1 * wy.y, h1 * wy.x);
+        rot[2 * nmode + o] = make_float2(-h1 * wz.y, h1 * wz.x);
+    }
 }
 
 }  // namespace
@@ -838,12 +849,14 @@ pse_status pse_wave_init(pse_ctx *c) {
 void pse_wave_set_stream(pse_ctx *c, cudaStream_t st) {
     for (int i = 0; i < c->nplans; ++i) { cufftSetStream(c->plan_r2c[i], st); cufftSetStream(c->plan_c2r[i], st); }
     if (c->have_plan_b) cufftSetStream(c->plan_c2r_b, st);
+    if (c->have_plan_rot_b) cufftSetStream(c->plan_c2r_rot_b, st);
 }
 
 void pse_wave_free(pse_ctx *c) {
     for (int i = 0; i < c->nplans; ++i) { cufftDestroy(c->plan_r2c[i]); cufftDestroy(c->plan_c2r[i]); }
     if (c->have_plan_b) cufftDestroy(c->plan_c2r_b);
-    cudaFree(c->d_grid_b); cudaFree(c->d_spec_b);
+    if (c->have_plan_rot_b) cufftDestroy(c->plan_c2r_rot_b);
+    cudaFree(c->d_grid_b); cudaFree(c->d_spec_b); cudaFree(c->d_spec_rot_b);
     cudaFree(c->iset_b.tile_start); cudaFree(c->iset_b.tile_list); cudaFree(c->iset_b.pbase); cudaFree(c->iset_b.pw);
     cudaFree(c->d_tile_of_b); cudaFree(c->d_tile_tmp_b); cudaFree(c->d_tile_cnt_b);
     cudaFree(c->d_grid); cudaFree(c->d_spec); cudaFree(c->d_fft_work);
@@ -973,15 +986,26 @@ pse_status pse_wave_apply(pse_ctx *c, const float *d_in, float *d_out, bool accu
     return inverse_and_interpolate(c, d_out, accumulate, mode);
 }
 
-pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate) {
+// d_outW != nullptr (full couplet): the angular velocities of the same field are ADDED to slots 0-2 of the packed vector d_outW;
+// three more spectra and a 3-plane C2R plan on the finer grid are made by the first such call.
+pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out, bool accumulate, float *d_outW) {
     if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
     const int Mb = c->Mb;
+    if (d_outW && !c->d_spec_rot_b) {
+        const size_t M3b = pse_plane_stride(Mb);
+        if (cudaMalloc(&c->d_spec_rot_b, 3 * (size_t)Mb * Mb * c->Mbh * sizeof(cufftComplex)) != cudaSuccess) {
+            cudaGetLastError(); c->d_spec_rot_b = nullptr; c->err = "out of memory (angular-velocity spectra of the Brownian pass)"; return PSE_ENOMEM;
+        }
+        int nb3[3] = {Mb, Mb, Mb}, nr[3] = {Mb, Mb, Mb}, ncx[3] = {Mb, Mb, c->Mbh};
+        CUFFT_TRY(c, cufftPlanMany(&c->plan_c2r_rot_b, 3, nb3, ncx, 1, Mb * Mb * c->Mbh, nr, 1, (int)M3b, CUFFT_C2R, 3)); c->have_plan_rot_b = true;
+        CUFFT_TRY(c, cufftSetStream(c->plan_c2r_rot_b, c->stream));
+    }
     {
         ScopedPhase ph(c, PSE_T_SCALE);
         ScaleParams sp = make_scale_params(c);
         sp.M = Mb; sp.Mh = c->Mbh; sp.dec = c->d_dec_b;               // thread grid and window table of the finer grid; noise on (Mc, Mch)
         scale_brownian_kernel<<<dim3((unsigned)((Mb * c->Mbh + 255) / 256), (unsigned)Mb), 256, 0, c->stream>>>(
-            c->d_spec_b, reinterpret_cast<const float2 *>(d_noise_wave), sp);
+            c->d_spec_b, reinterpret_cast<const float2 *>(d_noise_wave), sp, d_outW ? c->d_spec_rot_b : nullptr);
         KERNEL_CHECK(c);
     }
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r_b, c->d_spec_b, c->d_grid_b)); c->launches++; }
@@ -994,6 +1018,18 @@ pse_status pse_wave_brownian(pse_ctx *c, const float *d_noise_wave, float *d_out
         interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
             c->d_pos, c->d_tile_list, c->d_grid_b, reinterpret_cast<float4 *>(d_out), c->N, Mb, c->Pb, (float)(Mb / c->L),
             (float)c->win_a_b, (float)c->win_b_b, accumulate ? 1 : 0, PSE_MODE_ALL);
+    }
+    KERNEL_CHECK(c);
+    if (!d_outW) return PSE_OK;
+    // the three angular-velocity planes pass through planes 0-2 of the finer grid array
+    CUFFT_TRY(c, cufftExecC2R(c->plan_c2r_rot_b, c->d_spec_rot_b, c->d_grid_b)); c->launches++;
+    if (c->Pb <= 8) {
+        PSE_TRY(launch_interp_any(c, c->iset_b, 1, d_outW, true));
+    } else {
+        const int TB = 256;
+        interp_kernel<<<(unsigned)(((size_t)c->N * 32 + TB - 1) / TB), TB, 0, c->stream>>>(
+            c->d_pos, c->d_tile_list, c->d_grid_b, reinterpret_cast<float4 *>(d_outW), c->N, Mb, c->Pb, (float)(Mb / c->L),
+            (float)c->win_a_b, (float)c->win_b_b, 1, PSE_OUT_U);
     }
     KERNEL_CHECK(c);
     return PSE_OK;

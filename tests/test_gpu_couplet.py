@@ -155,3 +155,27 @@ def test_full_couplet_at_config3_size_against_pse_reference():
     for g, w, name in zip(got, want, 'UWE'):
         worst = float(np.linalg.norm(g[rows] - w, axis=1).max() / np.sqrt((w * w).sum(axis=1).mean()))
         assert rel(g[rows], w) < bar(tol) and worst < 10 * bar(tol), (name, rel(g[rows], w), worst)
+
+
+@pytest.mark.parametrize('tol', [1e-3, 1e-4])
+def test_brownian_sample_of_the_full_couplet_against_dense_oracle(tol):
+    """pse_brownian_full at N = 300 (dense 3 300 x 3 300 principal root), U^B, Omega^B and E^B separately; the same wave noise through
+    pse_brownian gives a U^B, E^B whose WAVE half is identical (same random fluid field)."""
+    N, xi, dt = 300, 0.7, 1e-3
+    ctx, x, L = make(N, 0.20, xi, tol, seed=6)
+    _, w2 = synth.brownian_noise(N, ctx.grid, 7)
+    w1 = np.random.default_rng(7).standard_normal((N, 11))
+    UB, WB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    it = ctx.pse_brownian_full(dt, dev(w1), dev(w2), UB, WB, EB)
+    assert 3 <= it <= 40
+    Uo, Wo, Eo = cpl.brownian_full(x, L, A, ETA, KT, xi, dt, ctx.grid, w1, w2, eps=1e-10)
+    for g, w, name in zip((UB, WB, EB), (Uo, Wo, Eo), 'UWE'):
+        assert rel(g.cpu().numpy(), w) < bar(tol), (name, rel(g.cpu().numpy(), w))
+    # wave half alone (zero real-space noise): the 8-component call sees the same field
+    U1, W1, E1 = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_brownian_full(dt, torch.zeros(N, 11, device='cuda'), dev(w2), U1, W1, E1)
+    U2, E2 = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_brownian(dt, torch.zeros(N, 8, device='cuda'), dev(w2), U2, E2)
+    assert torch.equal(U1, U2) and torch.equal(E1, E2)
+    Uw, Ww, Ew = cpl.wave_sqrt_apply_full(x, L, A, ETA, xi, ctx.grid, w2)
+    assert rel(W1.cpu().numpy(), np.sqrt(2 * KT / dt) * Ww) < bar(tol)

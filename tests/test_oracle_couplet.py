@@ -165,3 +165,46 @@ def test_C7_full_couplet_on_a_deformed_lattice_split_independence_and_lattice_eq
     assert rel(b_, a_) < 1e-11 and rel(c_, a_) < 1e-11
     cube = np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S))
     assert rel(np.hstack(cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S, A=np.eye(3))), cube) < 1e-13 and rel(a_, cube) > 1e-3
+
+
+def test_C8_wave_factor_of_the_full_couplet_has_the_covariance_of_its_matrix():
+    """A_w A_w^T = M_w summed over exactly the modes of the noise grid (the identity of pin P9, now with the Omega rows), built one unit
+    noise entry at a time on a 4^3 and a 5^3 grid; the U and E rows are those of oracle.brownian.wave_sqrt_apply."""
+    from oracle import brownian as brn
+    x, L = cluster(N=3, L=7.0, seed=11)
+    xi = 0.8
+    for Mg in (4, 5):
+        ncol = 3 * Mg * Mg * (Mg // 2 + 1) * 2
+        Aw = np.zeros((33, ncol))
+        for c in range(ncol):
+            w = np.zeros(ncol); w[c] = 1.0
+            Aw[:, c] = np.concatenate(cpl.wave_sqrt_apply_full(x, L, A, ETA, xi, Mg, w), axis=1).ravel()
+        k = brn.grid_modes(Mg, L)
+        k2 = np.einsum('ki,ki->k', k, k)
+        wt = fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2)
+        M = np.zeros((33, 33))
+        for col in range(33):
+            v = np.zeros((3, 11)); v[col // 11, col % 11] = 1.0
+            M[:, col] = np.concatenate(cpl.wave_apply_modes_full(x, A, k, wt, v[:, :3], v[:, 3:6], v[:, 6:]), axis=1).ravel()
+        assert np.abs(Aw @ Aw.T - M).max() < 1e-13 * np.abs(M).max()
+        w2 = np.random.default_rng(Mg).standard_normal(ncol)
+        U, W, E = cpl.wave_sqrt_apply_full(x, L, A, ETA, xi, Mg, w2)
+        U8, E8 = brn.wave_sqrt_apply(x, L, A, ETA, xi, Mg, w2)
+        assert np.abs(U - U8).max() < 1e-14 and np.abs(E - E8).max() < 1e-14
+
+
+def test_C9_brownian_full_amplitude_and_real_part():
+    """brownian_full against its dense factors: zero wave noise leaves sqrt(2kT/dt) sqrtm(M_r) w1, whose square is M_r; without the
+    Omega rows of the noise and with the torque-free block it is NOT the 8-component sample (the principal root of a bordered matrix
+    differs), but both have the covariance of their matrix -- only the latter is asserted."""
+    from oracle import brownian as brn
+    x, L = cluster(N=3, L=7.0, seed=12)
+    xi, dt, kT, Mg = 0.8, 1e-3, 0.7, 4
+    w1 = np.random.default_rng(1).standard_normal((3, 11))
+    zero = np.zeros(3 * Mg * Mg * (Mg // 2 + 1) * 2)
+    U, W, E = cpl.brownian_full(x, L, A, ETA, kT, xi, dt, Mg, w1, zero)
+    Mr = cpl.dense_full(x, L, A, ETA, xi, part='real')
+    R = brn.sqrtm_psd(Mr)
+    assert np.abs(R @ R - Mr).max() < 1e-12 * np.abs(Mr).max()
+    want = np.sqrt(2 * kT / dt) * (R @ w1.ravel())
+    assert rel(np.concatenate([U, W, E], axis=1).ravel(), want) < 1e-12
