@@ -183,3 +183,101 @@ def brownian(x, L, A, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14):
     Uw, Ew = brn.wave_sqrt_apply(x, L, a, eta, xi, Mg, wbuf, A=A)
     amp = np.sqrt(2.0 * kT / dt)
     return amp * (yr[:, :3] + Uw), amp * (yr[:, 3:] + Ew)
+
+
+class LatticeReference:
+    """Second tier on a deformed lattice, for sizes the direct sums cannot reach (pinned against them in
+    tests/test_oracle_lattice.py): the fp64 NUFFT of oracle.pse_reference carried out in LATTICE coordinates s = A^-1 x, where the
+    cell is the cube, with the Green's function at the physical wave vector k = (2 pi/L) A^-T n; the Gaussian of the quadrature then
+    is one of the lattice coordinates and its transform exp(-eta_g kappa^2/4 xi^2), kappa = 2 pi n/L, is what is divided out.
+    Real space: pairs from a periodic k-d tree in lattice coordinates within ||A^-1|| r_cut, kept if |A d| < r_cut, scalar
+    functions by quadrature."""
+
+    def __init__(self, L, A, a, eta, xi, tol=1e-8):
+        import scipy.fft as sfft
+        from . import pse_reference as pr
+        self.A = np.asarray(A, dtype=np.float64)
+        self.Ai = np.linalg.inv(self.A)
+        s = np.sqrt(-np.log(tol))
+        rcut = s / xi + 2.0 * a
+        self.reach = float(np.linalg.norm(self.Ai, 2))
+        if rcut * self.reach > 0.5 * L:
+            raise ValueError('LatticeReference: r_cut ||A^-1|| > L/2; raise xi')
+        gfac = max(np.linalg.norm(self.A[:, i]) for i in range(3))
+        M = int(np.ceil(1.1 * 2.0 * xi * s * L / np.pi * gfac))
+        M = max(8, M + (M & 1))
+        while sfft.next_fast_len(M, real=True) != M or (M & 1):
+            M += 1
+        self.ref = pr.PSEReference(L, a, eta, xi, tol, M=M, rcut=rcut)
+        self.L, self.a, self.eta, self.xi, self.rcut = float(L), float(a), float(eta), float(xi), rcut
+
+    def real_apply(self, x, F, S5, rows):
+        from scipy.spatial import cKDTree
+        s = to_lattice(x, self.A) % self.L
+        rows = np.asarray(rows, dtype=np.int64)
+        F, S5 = np.asarray(F, float), np.asarray(S5, float)
+        nb = cKDTree(s, boxsize=self.L).query_ball_point(s[rows], self.reach * self.rcut)
+        ia = np.concatenate([np.full(len(b), i, dtype=np.int64) for i, b in enumerate(nb)])
+        ib = np.concatenate([np.asarray(b, dtype=np.int64) for b in nb])
+        keep = rows[ia] != ib
+        ia, ib = ia[keep], ib[keep]
+        d = s[rows[ia]] - s[ib]
+        d -= self.L * np.round(d / self.L)
+        rv = d @ self.A.T
+        r = np.linalg.norm(rv, axis=1)
+        m = r < self.rcut
+        ia, ib, rv, r = ia[m], ib[m], rv[m], r[m]
+        R = fn.real_space_functions(r, self.xi, self.a)
+        pref = 1.0 / (6 * np.pi * self.eta * self.a)
+        Up, Ep = mob.pair_apply(rv, F[ib], fn.to_tensor(S5[ib]), R, pref)
+        U, E = np.zeros((rows.size, 3)), np.zeros((rows.size, 5))
+        np.add.at(U, ia, Up)
+        np.add.at(E, ia, fn.to_coords(Ep))
+        R0 = fn.real_space_functions(np.zeros(1), self.xi, self.a)
+        return U + pref * R0['F1'][0] * F[rows], E + pref * R0['Z0'][0] / 5.0 * S5[rows]
+
+    def wave_apply(self, x, F, S5, rows):
+        import os
+        import scipy.fft as sfft
+        ref = self.ref
+        s = to_lattice(x, self.A) % self.L
+        rows = np.ascontiguousarray(rows, dtype=np.int64)
+        M, V = ref.M, self.L ** 3
+        nw = os.cpu_count() or 1
+        gh = sfft.rfftn(ref.spread(s, np.hstack([np.asarray(F, float), np.asarray(S5, float)])), axes=(1, 2, 3), workers=nw)
+        qx, qy, qz, live = ref._kvec()                                  # kappa = 2 pi n/L, the wave vector of the cube
+        kap2 = qx * qx + qy * qy + qz * qz
+        Ai = self.Ai                                                    # k_i = sum_j kappa_j (A^-1)_ji
+        kx = qx * Ai[0, 0] + qy * Ai[1, 0] + qz * Ai[2, 0]
+        ky = qx * Ai[0, 1] + qy * Ai[1, 1] + qz * Ai[2, 1]
+        kz = qx * Ai[0, 2] + qy * Ai[1, 2] + qz * Ai[2, 2]
+        k2 = kx * kx + ky * ky + kz * kz
+        k2 = np.where(k2 > 0, k2, 1.0)
+        kn = np.sqrt(k2)
+        c0, c1 = fn.s0(kn * self.a), fn.s1(kn * self.a)
+        e = fn.basis()
+        kk = (kx, ky, kz)
+        fh = []
+        for i in range(3):
+            Sk = 0.0
+            for q in range(5):
+                for j in range(3):
+                    if e[q, i, j] != 0.0:
+                        Sk = Sk + e[q, i, j] * kk[j] * gh[3 + q]
+            fh.append(c0 * gh[i] - 1j * c1 * Sk)
+        del gh
+        Bt = np.where(live, (ref.h ** 3 / V) * fn.hasimoto_H(kn, self.xi) * np.exp(ref.eta_g * kap2 / (4.0 * self.xi ** 2)) / (self.eta * k2), 0.0)
+        kf = (kx * fh[0] + ky * fh[1] + kz * fh[2]) / k2
+        uh = [Bt * (fh[i] - kk[i] * kf) for i in range(3)]
+        del fh
+        oh = np.stack(ref._outputs(uh, kx, ky, kz, c0, c1))
+        del uh
+        go = sfft.irfftn(oh, s=(M, M, M), axes=(1, 2, 3), workers=nw) * float(M) ** 3
+        del oh
+        out = ref.interpolate(s, go, rows)
+        return out[:, :3], out[:, 3:]
+
+    def apply(self, x, F, S5, rows):
+        Ur, Er = self.real_apply(x, F, S5, rows)
+        Uw, Ew = self.wave_apply(x, F, S5, rows)
+        return Ur + Uw, Er + Ew

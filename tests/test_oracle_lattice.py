@@ -121,3 +121,22 @@ def test_L6_fp32_neighbour_sets_reduce_to_the_cubic_ones_and_follow_the_lattice(
         assert inside <= set(sets[al].tolist())
         ia2, ib2, _ = lat.real_pairs(x.astype(np.float64), L, lat.shear(g), rc * (1 + 1e-5), rows=[al])
         assert set(sets[al].tolist()) <= set(ib2[ib2 != al].tolist())
+
+
+def test_L7_lattice_reference_tier_against_direct_sums():
+    """The NUFFT tier in lattice coordinates (oracle.lattice.LatticeReference) against the direct sums on a sheared and an extended
+    cell, at ANOTHER xi, N = 300 with an overlapping pair, sampled rows; wave half separately at the same xi."""
+    import synth
+    s, L = synth.rsa(300, 0.20, seed=3)
+    F, S = synth.gaussian_inputs(300, 1)
+    rows = np.array([0, 3, 7, 150, 299])
+    for A in (lat.shear(0.4), lat.extension(1.2)):
+        x = s @ A.T
+        x[7] = x[3] + np.array([1.1, 0.9, 0.6])
+        want = lat.mobility_apply(x, L, A, A_, ETA, 0.8, F, S, rows=rows, eps=1e-12)
+        ref = lat.LatticeReference(L, A, A_, ETA, 1.0, tol=1e-8)
+        got = ref.apply(x, F, S, rows)
+        assert rel(got[0], want[0]) < 1e-7 and rel(got[1], want[1]) < 1e-7
+        ww = lat.mobility_apply(x, L, A, A_, ETA, 1.0, F, S, rows=rows, eps=1e-12, part='wave')
+        gw = ref.wave_apply(x, F, S, rows)
+        assert np.linalg.norm(gw[0] - ww[0]) < 1e-7 * np.linalg.norm(want[0]) and np.linalg.norm(gw[1] - ww[1]) < 1e-7 * np.linalg.norm(want[1])
