@@ -26,19 +26,20 @@ def test_L1_lambda_max_formulas_and_the_printed_table():
     extraction).  The printed supports at 1e-3 (5, 6, 7, 8 and 5, 6, 10) lie between 5 sqrt(lambda_max) and that + 1; Eq. (55) with
     C = 1 and m = sqrt(pi P) gives 5, 5, 8, 12 and 5, 6, 19 instead: the table is not reproducible from the bound as printed
     (reading R22), so only the bracket is asserted."""
-    for g, printed, P in ((0.0, 1.00, 5), (0.1, 1.11, 6), (0.5, 1.64, 7), (1.0, 2.62, 8)):
+    from golden import paper_table1 as tab
+    for g, printed, P in tab.SHEAR_ROWS:
         assert abs(lat.lambda_max(lat.shear(g)) - lat.lambda_max_shear(g)) < 1e-13
         assert abs(lat.lambda_max_shear(g) - printed) < 0.006
         assert 5 * np.sqrt(lat.lambda_max_shear(g)) - 0.1 <= P <= 5 * np.sqrt(lat.lambda_max_shear(g)) + 1
-    for e, printed, P in ((1.0, 1.00, 5), (1.1, 1.21, 6), (1.5, 2.25, None), (2.0, 4.00, 10), (0.5, 4.00, 10)):
+    for e, printed, P in tab.EXTENSION_ROWS + ((0.5, 4.00, 10),):
         assert abs(lat.lambda_max(lat.extension(e)) - lat.lambda_max_extension(e)) < 1e-13
         assert abs(lat.lambda_max_extension(e) - printed) < 0.006
         if P:
             assert 5 * np.sqrt(lat.lambda_max_extension(e)) - 0.1 <= P <= 5 * np.sqrt(lat.lambda_max_extension(e)) + 1
     # Eq. (55): lambda_max = 1 is Lindbo & Tornberg's bound; the paper's worked numbers "0.015 for simple shear and 0.046 for planar
     # extension" at gamma = epsilon = 0.5 ... are (1e-3)^(1/lambda_max) (PAPER.md:334)
-    assert abs((1e-3) ** (1 / lat.lambda_max_shear(0.5)) - 0.015) < 5e-4
-    assert abs((1e-3) ** (1 / 2.25) - 0.046) < 5e-4
+    assert abs((1e-3) ** (1 / lat.lambda_max_shear(0.5)) - tab.EXPECTED_ERROR_SHEAR_G05) < 5e-4
+    assert abs((1e-3) ** (1 / lat.lambda_max_extension(1.5)) - tab.EXPECTED_ERROR_EXT) < 5e-4
     assert lat.quadrature_bound(5, 1.0) < 1e-3 < lat.quadrature_bound(4, 1.0)          # P = 5 at 1e-3 on the orthorhombic grid (Table I)
     want = {1.0: 5, 1.105: 5, 1.21: 6, 1.64: 8, 2.618: 12, 4.0: 19}                    # Eq. (55), C = 1: what the bound itself asks for
     for lam, P in want.items():
