@@ -19,8 +19,6 @@
 #include "pse_internal.h"
 #include "wave_scale.cuh"
 
-pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int which, int mode);
-
 namespace {
 
 constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
@@ -217,7 +215,6 @@ static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *i
         CUDA_TRY(c, cudaMemsetAsync(outW, 0, vec, c->stream));
     }
     if (!(which & PSE_WAVE)) return PSE_OK;
-    const size_t nmode = (size_t)c->M * c->M * c->Mh;
     // torque planes first (they pass through planes 0-2 of the grid array), then the eight planes of (F, S)
     PSE_TRY(pse_wave_spread(c, inL, 1));
     { ScopedPhase ph(c, PSE_T_FFT_FWD); CUFFT_TRY(c, cufftExecR2C(c->plan_r2c[1], c->d_grid, c->d_spec_rot)); c->launches++; }
@@ -231,7 +228,6 @@ static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *i
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[0], c->d_spec, c->d_grid)); c->launches++; }
     PSE_TRY(pse_wave_interp(c, out8, true, 3));
     { ScopedPhase ph(c, PSE_T_FFT_INV); CUFFT_TRY(c, cufftExecC2R(c->plan_c2r[1], c->d_spec_rot, c->d_grid)); c->launches++; }
-    (void)nmode;
     return pse_wave_interp(c, outW, true, 1);
 }
 
@@ -262,6 +258,7 @@ pse_status pse_brownian_full(pse_ctx *c, double dt, const float *d_noise_real, c
 pse_status pse_mobility_apply_full(pse_ctx *c, const float *d_F, const float *d_L, const float *d_S, float *d_U, float *d_W, float *d_E, int which) {
     if (!c || !(which & PSE_BOTH) || (!d_F && !d_L && !d_S) || (!d_U && !d_W && !d_E)) return PSE_EINVAL;
     if (!c->have_nbrs) { c->err = "pse_mobility_apply_full before pse_neighbors"; return PSE_ENOTREADY; }
+    if (!d_L && !d_W) return pse_mobility_apply(c, d_F, d_S, d_U, d_E, which);       // no torque in, no angular velocity out: the 8-component path
     PSE_TRY(ensure_couplet(c));
     PSE_TRY(pse_pack(c, d_F, d_S, c->d_in));
     PSE_TRY(pse_pack(c, d_L, nullptr, c->d_rot_in));
