@@ -213,7 +213,7 @@ pse_status pse_destroy(pse_ctx *c) {
     if (c->ev_noise) cudaEventDestroy(c->ev_noise);
     if (c->ev_noise_r) cudaEventDestroy(c->ev_noise_r);
     if (c->ev_nbr) cudaEventDestroy(c->ev_nbr);
-    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) cudaGraphExecDestroy(c->step_graph[g]);
+    for (int g = 0; g < 3; ++g) if (c->step_graph[g]) cudaGraphExecDestroy(c->step_graph[g]);
     pse_wave_free(c);
     pse_couplet_free(c);
     for (Timer &t : c->timers) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
@@ -244,7 +244,7 @@ pse_status pse_set_lattice(pse_ctx *c, double a11, double a12, double a22) {
         c->err = "pse_set_lattice: rcut * max row norm of A^-1 > L/2 (the minimum image in lattice coordinates would miss pairs)"; return PSE_EINVAL;
     }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the lattice is baked in
+    for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the lattice is baked in
     c->lat_a11 = a11; c->lat_a12 = a12; c->lat_a22 = a22;
     c->deformed = !(a11 == 1.0 && a12 == 0.0 && a22 == 1.0);
     // cells of lattice-coordinate edge >= reach * rcut (never more cells than pse_create made room for: reach >= 1)
@@ -311,7 +311,7 @@ pse_status pse_set_bonds(pse_ctx *c, const int *h_pairs, int n_bonds, double k, 
     for (int b = 0; b < n_bonds; ++b)
         if (h_pairs[2 * b] == h_pairs[2 * b + 1]) { c->err = "pse_set_bonds: bond of a particle with itself"; return PSE_EINVAL; }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the bond array is baked in
+    for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the bond array is baked in
     cudaFree(c->d_bonds); c->d_bonds = nullptr; c->n_bonds = 0;
     if (n_bonds == 0) return PSE_OK;
     CUDA_TRY(c, cudaMalloc(&c->d_bonds, (size_t)n_bonds * sizeof(int2)));
@@ -342,10 +342,10 @@ static pse_status ensure_stage(pse_ctx *c, bool noise);
 // The whole mid-point step, Eqs. (76)-(79), with FIXED iteration counts and no host synchronisation: only enqueues (so it can
 // also run under stream capture).  x_k is saved in d_xk first.  *slot0 / *slot1: report slots of the two neighbour builds;
 // *single = false if the context takes the synchronous two-pass build (nothing to examine then).
-// parts: 1 = up to and including the Lanczos solve (needs the positions and the real-space noise), 2 = the rest (needs the
-// wave-space noise, the bulk of a host upload), 3 = both.
+// parts (bit mask): 1 = the first neighbour build (needs the positions only), 4 = the Lanczos solve (needs the real-space noise),
+// 2 = the rest (needs the wave-space noise, the bulk of a host upload); 7 = all.
 static pse_status enqueue_step_fixed(pse_ctx *c, float *d_pos, double dt, const float *d_noise_real, const float *d_noise_wave, int mL, int mG,
-                                     int *slot0, int *slot1, bool *single, int parts = 3) {
+                                     int *slot0, int *slot1, bool *single, int parts = 7) {
     const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
     const float L = (float)c->L, invL = 1.0f / L;
     float *UB = c->d_vecD, *EB = c->d_vecD + (size_t)3 * N;
@@ -355,8 +355,8 @@ static pse_status enqueue_step_fixed(pse_ctx *c, float *d_pos, double dt, const 
         PSE_TRY(pse_neighbors_impl(c, d_pos));
         *slot0 = c->nbr_last;
         *single = c->nbr_pending;
-        PSE_TRY(brownian_real_part(c, d_noise_real, nullptr, mL));
     }
+    if (parts & 4) PSE_TRY(brownian_real_part(c, d_noise_real, nullptr, mL));
     if (!(parts & 2)) return PSE_OK;
     PSE_TRY(brownian_wave_part(c, dt, d_noise_wave, UB, EB));
     k_advance<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, c->deformed ? 0 : 1); KERNEL_CHECK(c);
@@ -410,10 +410,10 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
             }
             const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap};
             if (!c->step_graph[0] || !(key == c->graph_key)) {
-                for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
+                for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
                 const long long l0 = c->launches;
                 // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot capture), in
-                // two graphs: [neighbour build, Lanczos] and [wave part of the sample, mid-point, build, solve, update]; the uploads
+                // three graphs: [neighbour build], [Lanczos] and [wave part of the sample, mid-point, build, solve, update]; the uploads
                 // that pse_step_host has in flight on its second stream are waited for between them, not before them
                 cudaStream_t user = c->stream;
                 const bool pr = c->noise_r_pending, pw = c->noise_pending;
@@ -421,11 +421,12 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
                 c->stream = c->stream_cap;
                 pse_wave_set_stream(c, c->stream);
                 bool ok = true;
-                for (int g = 0; g < 2 && ok; ++g) {
+                const int part_of[3] = {1, 4, 2};
+                for (int g = 0; g < 3 && ok; ++g) {
                     cudaGraph_t gr = nullptr;
                     ok = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess;
                     if (ok) {
-                        const pse_status es = enqueue_step_fixed(c, d_pos, dt, d_noise_real, d_noise_wave, mL, mG, &slot0, &slot1, &single, 1 << g);
+                        const pse_status es = enqueue_step_fixed(c, d_pos, dt, d_noise_real, d_noise_wave, mL, mG, &slot0, &slot1, &single, part_of[g]);
                         ok = cudaStreamEndCapture(c->stream, &gr) == cudaSuccess && es == PSE_OK && gr;
                     }
                     if (ok) ok = cudaGraphInstantiate(&c->step_graph[g], gr, 0) == cudaSuccess;
@@ -436,7 +437,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
                 c->noise_r_pending = pr; c->noise_pending = pw;
                 if (!ok || !single) {                                 // capture not possible here: plain enqueue from now on
                     cudaGetLastError();
-                    for (int g = 0; g < 2; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
+                    for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
                     c->graph_failed = true;
                 } else {
                     c->graph_key = key; c->graph_slot0 = slot0; c->graph_slot1 = slot1; c->graph_launches = c->launches - l0;
@@ -444,10 +445,11 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
                 c->launches = l0;
             }
             if (c->step_graph[0] && !c->graph_failed) {
+                CUDA_TRY(c, cudaGraphLaunch(c->step_graph[0], c->stream));          // the build runs while the noise is still on its way
                 if (c->noise_r_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise_r, 0)); c->noise_r_pending = false; }
-                CUDA_TRY(c, cudaGraphLaunch(c->step_graph[0], c->stream));
-                if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
                 CUDA_TRY(c, cudaGraphLaunch(c->step_graph[1], c->stream));
+                if (c->noise_pending) { CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->ev_noise, 0)); c->noise_pending = false; }
+                CUDA_TRY(c, cudaGraphLaunch(c->step_graph[2], c->stream));
                 slot0 = c->graph_slot0; slot1 = c->graph_slot1;
                 c->launches += c->graph_launches;
                 c->nbr_pending = false; c->fine_bins_valid = false; c->have_nbrs = true;

@@ -128,7 +128,7 @@ struct pse_ctx {
     double *h_scal_l = nullptr;              // pinned mirror of the Lanczos scalars of a fixed-count solve (pse_step's optimistic path)
     int lanczos_budget = 0, gmres_budget = 0;   // iteration counts the last completed step needed; 0 = not known yet
     float4 *d_xk = nullptr;                  // [N] copy of x_k while an optimistic step is in flight
-    cudaGraphExec_t step_graph[2] = {nullptr, nullptr};   // the fixed-count step as two graphs: [build, Lanczos], [wave sample ... update]
+    cudaGraphExec_t step_graph[3] = {nullptr, nullptr, nullptr};   // the fixed-count step as three graphs: [build], [Lanczos], [wave sample ... update]
     StepGraphKey graph_key = {};
     int graph_slot0 = 0, graph_slot1 = 0; long long graph_launches = 0; bool graph_failed = false; int graph_recaptures = 0;
     float *d_coef = nullptr;                 // small coefficient vector upload
