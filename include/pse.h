@@ -141,6 +141,14 @@ pse_status pse_brownian_full(pse_ctx *ctx, double dt, const float *d_noise_real,
 pse_status pse_constrained_solve_full(pse_ctx *ctx, const float *d_F, const float *d_L, const float *d_UB, const float *d_EB,
                                       float *d_U, float *d_W, float *d_S, int *gmres_iters);
 
+/* pse_step with external torques: one mid-point step of Eqs. (76)-(79) in which script-F = [F^P; L] carries the torques d_L [N][3]
+ * (may be NULL) beside the overlap / bond forces, and script-U = [U; Omega] is returned: positions advance with U_{k+1/2}, the
+ * angular velocities Omega_{k+1/2} = M_OF F + M_OL L + M_OS S go to d_W [N][3] (may be NULL) for the caller's own orientation
+ * update.  The Brownian slip is pse_brownian's (no Brownian angular velocity is added; pse_brownian_full has it).  Runs the checked
+ * path (synchronous builds, per-iteration convergence checks), not the graph replay of pse_step. */
+pse_status pse_step_full(pse_ctx *ctx, float *d_pos, double dt, const float *d_L, const float *d_noise_real, const float *d_noise_wave,
+                         float *d_W, int *gmres_iters, int *lanczos_iters);
+
 /* Heyes-Melrose hard-sphere overlap force at the current positions (named by BASELINE.json, not the paper;
  * DESIGN.md reading R12): F_i = sum_{j: r_ij<2a} 3 pi eta a (2a - r_ij)/dt rhat_ij.  d_F [N][3] out. */
 pse_status pse_hard_sphere_forces(pse_ctx *ctx, double dt, float *d_F);

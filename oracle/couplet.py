@@ -193,3 +193,19 @@ def brownian_full(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps=1e-14):
     Uw, Ww, Ew = wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf)
     amp = np.sqrt(2.0 * kT / dt)
     return amp * (yr[:, :3] + Uw), amp * (yr[:, 3:6] + Ww), amp * (yr[:, 6:] + Ew)
+
+
+def step_full(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, Lq, eps=1e-14):
+    """One mid-point step, Eqs. (76)-(79), with external torques Lq in script-F = [F^P; L]: the Brownian slip of
+    oracle.brownian.brownian at x_k, the overlap forces, torques and the dense 11N x 11N matrix at x_{k+1/2}.
+    Returns x_{k+1} (not wrapped), U_{k+1/2}, Omega_{k+1/2}, S."""
+    from . import brownian as brn
+    x = np.asarray(x, dtype=np.float64)
+    N = x.shape[0]
+    UB, EB = brn.brownian(x, L, a, eta, kT, xi, dt, Mg, w1, wbuf, eps)          # (76)
+    xh = x + 0.5 * dt * UB                                                   # (77)
+    xh -= L * np.floor(xh / L)
+    M = dense_full(xh, L, a, eta, xi, eps=eps)
+    FP = brn.heyes_melrose(xh, L, a, eta, dt)
+    U, W, S = constrained_solve_full(M, N, UB, np.zeros((N, 3)), EB, FP, Lq)   # (78)
+    return x + dt * U, U, W, S                                               # (79)

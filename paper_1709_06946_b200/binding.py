@@ -20,7 +20,7 @@ _STATUS = {0: 'PSE_OK', 1: 'PSE_EINVAL', 2: 'PSE_ENOMEM', 3: 'PSE_ECUDA', 4: 'PS
            6: 'PSE_ENOCONV', 7: 'PSE_EOVERFLOW'}
 
 EXPORTS = ('pse_suggest_params', 'pse_suggest_params_window', 'pse_suggest_params_lattice', 'pse_set_lattice', 'pse_create', 'pse_create_window', 'pse_destroy', 'pse_neighbors', 'pse_mobility_apply', 'pse_brownian',
-           'pse_constrained_solve', 'pse_mobility_apply_full', 'pse_constrained_solve_full', 'pse_brownian_full', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
+           'pse_constrained_solve', 'pse_mobility_apply_full', 'pse_constrained_solve_full', 'pse_brownian_full', 'pse_step_full', 'pse_hard_sphere_forces', 'pse_hard_sphere_forces_noalloc', 'pse_set_bonds', 'pse_bond_forces', 'pse_step', 'pse_mobility_apply_host', 'pse_step_host', 'pse_get_neighbors', 'pse_set_profiling',
            'pse_get_timings', 'pse_kernel_launches', 'pse_get_table', 'pse_last_error', 'pse_version')
 
 
@@ -49,6 +49,7 @@ def load_library():
     lib.pse_constrained_solve.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces.argtypes = [vp, dbl, vp]
     lib.pse_mobility_apply_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32]
+    lib.pse_step_full.argtypes = [vp, vp, dbl, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pse_brownian_full.argtypes = [vp, dbl, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_constrained_solve_full.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i32)]
     lib.pse_hard_sphere_forces_noalloc.argtypes = [i32, dbl, dbl, dbl, dbl, vp, vp, vp, C.c_char_p, C.c_size_t]
@@ -173,6 +174,14 @@ class Context:
         N = self.N
         self._check(_lib.pse_mobility_apply_full(self._h, _ptr(F, (N, 3)), _ptr(Lq, (N, 3)), _ptr(S, (N, 5)),
                                                  _ptr(U, (N, 3)), _ptr(W, (N, 3)), _ptr(E, (N, 5)), which))
+
+    def pse_step_full(self, pos, dt, Lq, noise_real, noise_wave, W=None):
+        """pse_step with external torques Lq [N][3] (or None); angular velocities to W [N][3] (or None).  -> (gmres, lanczos) iterations."""
+        N, M = self.N, self.grid
+        gi, li = C.c_int(), C.c_int()
+        self._check(_lib.pse_step_full(self._h, _ptr(pos, (N, 4)), dt, _ptr(Lq, (N, 3)), _ptr(noise_real, (N, 8)),
+                                       _ptr(noise_wave, (3, M, M, M // 2 + 1, 2)), _ptr(W, (N, 3)), C.byref(gi), C.byref(li)))
+        return gi.value, li.value
 
     def pse_brownian_full(self, dt, noise_real, noise_wave, UB, WB, EB):
         """11-component Brownian slip: noise_real [N][11] (Ux..Uz, Ox..Oz, e1..e5), outputs UB, WB (Omega^B), EB."""

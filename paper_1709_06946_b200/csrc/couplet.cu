@@ -170,6 +170,22 @@ __global__ void k_pack11(const float *v11, const int *order, int N, float4 *wide
     wide[2 * (size_t)N + 2 * s + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
+// x_out = x_in + dt U (original numbering), wrapped into [0, L) per component on the cube only (on a deformed lattice that is not
+// a lattice translation; pse_neighbors takes any image)
+__global__ void k_advance_full(const float4 *pos_in, const float *U, float dt, float L, float invL, int N, float4 *pos_out, int wrap) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float4 p = pos_in[i];
+    p.x += dt * U[3 * i]; p.y += dt * U[3 * i + 1]; p.z += dt * U[3 * i + 2];
+    if (wrap) {
+        p.x -= L * floorf(p.x * invL); p.y -= L * floorf(p.y * invL); p.z -= L * floorf(p.z * invL);
+        if (p.x >= L || p.x < 0.f) p.x = 0.f;
+        if (p.y >= L || p.y < 0.f) p.y = 0.f;
+        if (p.z >= L || p.z < 0.f) p.z = 0.f;
+    }
+    pos_out[i] = p;
+}
+
 }  // namespace
 
 void pse_couplet_free(pse_ctx *c) {
@@ -253,6 +269,38 @@ pse_status pse_brownian_full(pse_ctx *c, double dt, const float *d_noise_real, c
     if (d_UB || d_EB) PSE_TRY(pse_unpack(c, c->d_rot_y, amp, d_UB, d_EB));
     if (d_WB) PSE_TRY(pse_unpack(c, c->d_rot_y + half, amp, d_WB, nullptr));
     return st;
+}
+
+pse_status pse_step_full(pse_ctx *c, float *d_pos, double dt, const float *d_L, const float *d_noise_real, const float *d_noise_wave,
+                         float *d_W, int *gmres_iters, int *lanczos_iters) {
+    if (!c || !d_pos || !(dt > 0) || !d_noise_real || !d_noise_wave) return PSE_EINVAL;
+    PSE_TRY(ensure_couplet(c));
+    const int N = c->N, TB = 256, nb = (N + TB - 1) / TB;
+    const float L = (float)c->L, invL = 1.0f / L;
+    // [N][3] / [N][5] vectors in original numbering, carved out of the wide Lanczos vectors (idle outside pse_brownian_full)
+    float *UB = c->d_rot_w, *EB = UB + (size_t)3 * N, *FP = UB + (size_t)8 * N, *U = UB + (size_t)11 * N;
+    float *S = c->d_rot_u, *FB = S + (size_t)8 * N;
+    float4 *xh = reinterpret_cast<float4 *>(c->d_rot_y);
+    pse_status soft = PSE_OK;
+    // (76) Brownian slip at x_k
+    PSE_TRY(pse_neighbors(c, d_pos));
+    pse_status st = pse_brownian(c, dt, d_noise_real, d_noise_wave, UB, EB, lanczos_iters);
+    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
+    // (77) mid-point
+    k_advance_full<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), UB, (float)(0.5 * dt), L, invL, N, xh, c->deformed ? 0 : 1); KERNEL_CHECK(c);
+    PSE_TRY(pse_neighbors(c, reinterpret_cast<const float *>(xh)));
+    // (78) F^P (overlap + bond forces) and the torques at the mid-point; stresslet-constrained [U; Omega]
+    PSE_TRY(pse_hard_sphere_forces(c, dt, FP));
+    if (c->n_bonds) {
+        PSE_TRY(pse_bond_forces(c, FB));
+        PSE_TRY(pse_axpby(c, (size_t)3 * N, 1.f, FB, 1.f, FP));
+    }
+    st = pse_constrained_solve_full(c, FP, d_L, UB, EB, U, d_W, S, gmres_iters);
+    if (st == PSE_ENOCONV) soft = st; else if (st != PSE_OK) return st;
+    // (79) full step from x_k
+    k_advance_full<<<nb, TB, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos), U, (float)dt, L, invL, N, reinterpret_cast<float4 *>(d_pos),
+                                             c->deformed ? 0 : 1); KERNEL_CHECK(c);
+    return soft;
 }
 
 pse_status pse_mobility_apply_full(pse_ctx *c, const float *d_F, const float *d_L, const float *d_S, float *d_U, float *d_W, float *d_E, int which) {

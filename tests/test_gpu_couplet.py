@@ -179,3 +179,28 @@ def test_brownian_sample_of_the_full_couplet_against_dense_oracle(tol):
     assert torch.equal(U1, U2) and torch.equal(E1, E2)
     Uw, Ww, Ew = cpl.wave_sqrt_apply_full(x, L, A, ETA, xi, ctx.grid, w2)
     assert rel(W1.cpu().numpy(), np.sqrt(2 * KT / dt) * Ww) < bar(tol)
+
+
+def test_step_with_external_torques_against_dense_oracle():
+    """pse_step_full at N = 48, tol 1e-4: displacement and angular velocities against oracle.couplet.step_full (dense matrices), with
+    overlapping pairs (F^P != 0) and a torque on every sphere; without torques the displacement is pse_step's."""
+    N, xi, tol, dt = 48, 0.85, 1e-4, 1e-3
+    ctx, x, L = make(N, 0.20, xi, tol, seed=3, squeeze=0.93)
+    w1, w2 = synth.brownian_noise(N, ctx.grid, 2)
+    Lq = 20.0 * np.random.default_rng(5).standard_normal((N, 3))
+    xo, Uo, Wo, So = cpl.step_full(x, L, A, ETA, KT, xi, dt, ctx.grid, w1, w2, Lq, eps=1e-10)
+    pos = dev(pos4(x.astype(np.float32)))
+    W = torch.empty(N, 3, device='cuda')
+    gi, li = ctx.pse_step_full(pos, dt, dev(Lq), dev(w1.reshape(N, 8)), dev(w2), W)
+    assert 2 <= gi <= 30 and 2 <= li <= 40
+    d = pos[:, :3].cpu().numpy().astype(np.float64) - x
+    d -= L * np.round(d / L)                                        # the library wraps into [0, L)
+    assert rel(d, xo - x) < 3 * bar(tol) and rel(W.cpu().numpy(), Wo) < 3 * bar(tol), (rel(d, xo - x), rel(W.cpu().numpy(), Wo))
+    # the torques really moved the spheres, and without them the step is pse_step's
+    p0, p1 = dev(pos4(x.astype(np.float32))), dev(pos4(x.astype(np.float32)))
+    ctx.pse_step_full(p0, dt, None, dev(w1.reshape(N, 8)), dev(w2))
+    ctx.pse_step(p1, dt, dev(w1.reshape(N, 8)), dev(w2))
+    d0 = (p0 - dev(pos4(x.astype(np.float32))))[:, :3].cpu().numpy()
+    d1 = (p1 - dev(pos4(x.astype(np.float32))))[:, :3].cpu().numpy()
+    d0 -= L * np.round(d0 / L); d1 -= L * np.round(d1 / L)
+    assert rel(d0, d1) < 3 * bar(tol) and rel(d, d0) > 10 * bar(tol)

@@ -208,3 +208,25 @@ def test_C9_brownian_full_amplitude_and_real_part():
     assert np.abs(R @ R - Mr).max() < 1e-12 * np.abs(Mr).max()
     want = np.sqrt(2 * kT / dt) * (R @ w1.ravel())
     assert rel(np.concatenate([U, W, E], axis=1).ravel(), want) < 1e-12
+
+
+def test_C10_step_with_torques_reduces_to_the_pinned_step_and_turns_the_spheres():
+    """step_full with L = 0 is oracle.brownian.step (pinned by hand in tests/test_oracle_pins.py); with a torque on one sphere every
+    translational velocity changes by exactly the constrained response to that torque at the SAME mid-point."""
+    from oracle import brownian as brn
+    import synth
+    N, xi, dt, Mg, L = 6, 0.9, 1e-3, 6, 7.5
+    rng = np.random.default_rng(3)
+    x = rng.uniform(0, L, (N, 3))
+    x[1] = x[0] + np.array([1.0, 0.9, 0.7])
+    w1, w2 = synth.brownian_noise(N, Mg, 1)
+    x0, U0, S0 = brn.step(x, L, A, ETA, 1.0, xi, dt, Mg, w1, w2, eps=1e-12)
+    x1, U1, W1, S1 = cpl.step_full(x, L, A, ETA, 1.0, xi, dt, Mg, w1, w2, np.zeros((N, 3)), eps=1e-12)
+    assert rel(x1 - x, x0 - x) < 1e-11 and rel(S1, S0) < 1e-11 and np.abs(W1).max() > 0
+    Lq = np.zeros((N, 3)); Lq[2] = (0.0, 0.0, 5.0)
+    x2, U2, W2, S2 = cpl.step_full(x, L, A, ETA, 1.0, xi, dt, Mg, w1, w2, Lq, eps=1e-12)
+    UB, EB = brn.brownian(x, L, A, ETA, 1.0, xi, dt, Mg, w1, w2, 1e-12)
+    xh = (x + 0.5 * dt * UB) % L
+    M = cpl.dense_full(xh, L, A, ETA, xi, eps=1e-12)
+    dU, dW, dS = cpl.constrained_solve_full(M, N, np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5)), np.zeros((N, 3)), Lq)
+    assert rel(U2 - U1, dU) < 1e-9 and rel(W2 - W1, dW) < 1e-9 and dW[2, 2] > 0
