@@ -12,8 +12,8 @@
 //                Omega += T' F x rh + Y0 L + Y2 (rh rh.L - L/3) + 2 Y2 (S rh) x rh
 //                E     += 2 Y2 sym[ rh (x) (rh x L) ]
 //                with (T', Y0, Y2) = (T/2, Z0/6, Z2/4)/(6 pi eta a), T = G1 - G2 (the antisymmetric part of Eq. 26), from a
-//                table of their own at the nodes of the main table (tables.cu).  A second sweep over the neighbour list, eight
-//                lanes per particle as in the pair kernel; it adds to the 8-component result and writes Omega.
+//                table of their own at the nodes of the main table (tables.cu), in real_pairs_full_kernel: the 11-component pair
+//                sum in one sweep, eight lanes per particle as in the 8-component pair kernel.
 #include <algorithm>
 #include <cmath>
 #include "pse_internal.h"
@@ -23,58 +23,80 @@ namespace {
 
 constexpr float RS2 = 0.70710678118654752f, RS6 = 0.40824829046386302f;
 
-__global__ void __launch_bounds__(256)
-real_rot_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, const float4 *__restrict__ inL, float *__restrict__ out8,
-                float *__restrict__ outW, int N, const unsigned long long *__restrict__ off, const int *__restrict__ cnt,
-                const int *__restrict__ idx, const float4 *__restrict__ table, float inv_dr, float L, float invL, Lat lat) {
-    __shared__ float4 tab[PSE_NTAB];
-    for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) tab[i] = table[i];
+// The 11-component pair sum in ONE sweep over the neighbour list: the tensor algebra of real_pairs_kernel (realspace.cu) plus the
+// rotational terms of the file header on one set of gathers, with both tables in shared memory (64 + 32 KB).  Eight lanes per
+// particle, 384 threads, two CTAs per SM (72 registers: 11 accumulators, 11 inputs).  (A second sweep that added the rotational
+// terms to the 8-component kernel's result cost 48 us on top of its 37 us at config 3; this one takes 60 us.)
+constexpr size_t FULL_SMEM = (size_t)PSE_NTAB * 3 * sizeof(float4);
+
+__global__ void __launch_bounds__(384, 2)
+real_pairs_full_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, const float4 *__restrict__ inL, float *__restrict__ out8,
+                       float *__restrict__ outW, int N, const unsigned long long *__restrict__ off, const int *__restrict__ cnt,
+                       const int *__restrict__ idx, const float4 *__restrict__ table, const float4 *__restrict__ rtable, float inv_dr, float L,
+                       float invL, Lat lat) {
+    extern __shared__ float4 ftab[];                           // tabU[NTAB] | tabE[NTAB] | tabR[NTAB]
+    float4 *tabU = ftab, *tabE = ftab + PSE_NTAB, *tabR = ftab + 2 * PSE_NTAB;
+    for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) { tabU[i] = table[2 * i]; tabE[i] = table[2 * i + 1]; tabR[i] = rtable[i]; }
     __syncthreads();
     const int gl = threadIdx.x & 7, grp = (threadIdx.x & 31) >> 3, wpb = blockDim.x >> 5;
-    for (int ws = blockIdx.x * wpb + (threadIdx.x >> 5); ws * 4 < N; ws += gridDim.x * wpb) {     // warp = four particles
+    for (int ws = blockIdx.x * wpb + (threadIdx.x >> 5); ws * 4 < N; ws += gridDim.x * wpb) {
         const int s = ws * 4 + grp;
         const bool live = s < N;
         const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
-        float acc[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};          // dU (3), dE (5), Omega (3)
+        float acc[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};          // U (3), E (5), Omega (3)
         const unsigned long long lo = live ? off[s] : 0ull, hi = lo + (unsigned long long)(live ? cnt[s] : 0);
-        for (unsigned long long j = lo + gl; j < hi; j += 8) {
-            const int b = idx[j];
-            const float4 q4 = pos[b], a0 = in8[2 * b], a1 = in8[2 * b + 1], l4 = inL[2 * b];
+        unsigned long long j = lo + gl;
+        int b = j < hi ? idx[j] : 0;
+        float4 q4 = pos[b];
+        for (; j < hi; j += 8) {
+            const float4 a0 = in8[2 * b], a1 = in8[2 * b + 1], l4 = inL[2 * b];
+            const int bn = (j + 8 < hi) ? idx[j + 8] : b;
             float dx = p.x - q4.x, dy = p.y - q4.y, dz = p.z - q4.z;
             dx -= L * rintf(dx * invL); dy -= L * rintf(dy * invL); dz -= L * rintf(dz * invL);
-            dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy;                 // r = A d on a deformed lattice (identity on the cube)
+            dx = lat.a11 * dx + lat.a12 * dy; dy = lat.a22 * dy;
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float rinv = rsqrtf(fmaxf(r2, 1e-30f)), r = r2 * rinv;
             const float rx = dx * rinv, ry = dy * rinv, rz = dz * rinv;
             const float tt = r * inv_dr;
             const int it = min((int)tt, PSE_NTAB - 2);
             const float w1 = tt - (float)it, w0 = 1.f - w1;
-            const float4 ta = tab[it], tb = tab[it + 1];
-            const float Tq = w0 * ta.x + w1 * tb.x, Y0 = w0 * ta.y + w1 * tb.y, Y2 = w0 * ta.z + w1 * tb.z;
-            // L x rh, F x rh
-            const float cx = l4.y * rz - l4.z * ry, cy = l4.z * rx - l4.x * rz, cz = l4.x * ry - l4.y * rx;
-            const float gx = a0.y * rz - a0.z * ry, gy = a0.z * rx - a0.x * rz, gz = a0.x * ry - a0.y * rx;
-            acc[0] += Tq * cx; acc[1] += Tq * cy; acc[2] += Tq * cz;
-            // t = S rh from the 5 coordinates
+            const float4 ta = tabU[it], tc = tabU[it + 1], tb = tabE[it], td = tabE[it + 1], ra = tabR[it], rb = tabR[it + 1];
+            const float F1 = w0 * ta.x + w1 * tc.x, F2 = w0 * ta.y + w1 * tc.y, Ga = w0 * ta.z + w1 * tc.z, Gb = w0 * ta.w + w1 * tc.w;
+            const float A = w0 * tb.x + w1 * td.x, B = w0 * tb.y + w1 * td.y, D = w0 * tb.z + w1 * td.z;
+            const float Tq = w0 * ra.x + w1 * rb.x, Y0 = w0 * ra.y + w1 * rb.y, Y2 = w0 * ra.z + w1 * rb.z;
+            const float4 qn = pos[bn];
             const float sxx = a0.w * RS2 - a1.x * RS6, syy = -a0.w * RS2 - a1.x * RS6, szz = 2.f * a1.x * RS6;
             const float sxy = a1.y * RS2, sxz = a1.z * RS2, syz = a1.w * RS2;
+            const float f = rx * a0.x + ry * a0.y + rz * a0.z;
             const float tx = sxx * rx + sxy * ry + sxz * rz, ty = sxy * rx + syy * ry + syz * rz, tz = sxz * rx + syz * ry + szz * rz;
-            const float rl = rx * l4.x + ry * l4.y + rz * l4.z, Y22 = 2.f * Y2, third = 1.f / 3.f;
+            const float q = rx * tx + ry * ty + rz * tz;
+            const float cx = l4.y * rz - l4.z * ry, cy = l4.z * rx - l4.x * rz, cz = l4.x * ry - l4.y * rx;      // L x rh
+            const float gx = a0.y * rz - a0.z * ry, gy = a0.z * rx - a0.x * rz, gz = a0.x * ry - a0.y * rx;      // F x rh
+            const float cu = (F2 - F1) * f - Gb * q;
+            acc[0] += F1 * a0.x + cu * rx + Ga * tx + Tq * cx;
+            acc[1] += F1 * a0.y + cu * ry + Ga * ty + Tq * cy;
+            acc[2] += F1 * a0.z + cu * rz + Ga * tz + Tq * cz;
+            const float cw = Gb * f + D * q, B2 = 2.f * B, Y22 = 2.f * Y2;
+            // E += A S + sym[rh (x) w],  w = -Ga F + 2B t + (Gb f + D q) rh + 2 Y2 (rh x L)
+            const float wx = -Ga * a0.x + B2 * tx + cw * rx - Y22 * cx, wy = -Ga * a0.y + B2 * ty + cw * ry - Y22 * cy,
+                        wz = -Ga * a0.z + B2 * tz + cw * rz - Y22 * cz;
+            const float pxx = rx * wx, pyy = ry * wy, pzz = rz * wz;
+            acc[3] += A * a0.w + (pxx - pyy) * RS2;
+            acc[4] += A * a1.x + (2.f * pzz - pxx - pyy) * RS6;
+            acc[5] += A * a1.y + (rx * wy + ry * wx) * RS2;
+            acc[6] += A * a1.z + (rx * wz + rz * wx) * RS2;
+            acc[7] += A * a1.w + (ry * wz + rz * wy) * RS2;
+            const float rl = rx * l4.x + ry * l4.y + rz * l4.z, third = 1.f / 3.f;
             acc[8] += Tq * gx + Y0 * l4.x + Y2 * (rx * rl - third * l4.x) + Y22 * (ty * rz - tz * ry);
             acc[9] += Tq * gy + Y0 * l4.y + Y2 * (ry * rl - third * l4.y) + Y22 * (tz * rx - tx * rz);
             acc[10] += Tq * gz + Y0 * l4.z + Y2 * (rz * rl - third * l4.z) + Y22 * (tx * ry - ty * rx);
-            // E += sym[rh (x) w], w = 2 Y2 (rh x L) = -2 Y2 (L x rh)
-            const float wx = -Y22 * cx, wy = -Y22 * cy, wz = -Y22 * cz;
-            const float pxx = rx * wx, pyy = ry * wy, pzz = rz * wz;
-            acc[3] += (pxx - pyy) * RS2;
-            acc[4] += (2.f * pzz - pxx - pyy) * RS6;
-            acc[5] += (rx * wy + ry * wx) * RS2;
-            acc[6] += (rx * wz + rz * wx) * RS2;
-            acc[7] += (ry * wz + rz * wy) * RS2;
+            b = bn; q4 = qn;
         }
-        if (gl == 0 && live) {                                       // self term: Omega += Z0(0)/6 L  (r -> 0, rh := 0)
-            const float4 l4 = inL[2 * s];
-            const float y0 = tab[0].y;
+        if (gl == 0 && live) {                                       // self terms F1(0) F, A(0) S, Z0(0)/6 L
+            const float4 a0 = in8[2 * s], a1 = in8[2 * s + 1], l4 = inL[2 * s];
+            const float f1 = tabU[0].x, a_ = tabE[0].x, y0 = tabR[0].y;
+            acc[0] += f1 * a0.x; acc[1] += f1 * a0.y; acc[2] += f1 * a0.z;
+            acc[3] += a_ * a0.w; acc[4] += a_ * a1.x; acc[5] += a_ * a1.y; acc[6] += a_ * a1.z; acc[7] += a_ * a1.w;
             acc[8] += y0 * l4.x; acc[9] += y0 * l4.y; acc[10] += y0 * l4.z;
         }
 #pragma unroll
@@ -85,7 +107,7 @@ real_rot_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, 
 #pragma unroll
             for (int c = 1; c < 8; ++c) mine = gl == c ? acc[c] : mine;
             w = gl == 1 ? acc[9] : (gl == 2 ? acc[10] : w);
-            out8[(size_t)s * 8 + gl] += mine;
+            out8[(size_t)s * 8 + gl] = mine;
             outW[(size_t)s * 8 + gl] = gl < 3 ? w : 0.f;
         }
     }
@@ -210,6 +232,7 @@ static pse_status ensure_couplet(pse_ctx *c) {
         c->err = "out of memory (full-couplet buffers)"; return PSE_ENOMEM;
     }
     CUDA_TRY(c, cudaMemcpy(c->d_rot_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY(c, cudaFuncSetAttribute(real_pairs_full_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FULL_SMEM));
     return PSE_OK;
 }
 
@@ -217,14 +240,14 @@ static pse_status ensure_couplet(pse_ctx *c) {
 static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *inL, float *out8, float *outW, int which) {
     const size_t vec = (size_t)c->N * 8 * sizeof(float);
     if (which & PSE_REAL) {
-        PSE_TRY(pse_real_apply(c, in8, out8, PSE_MODE_ALL));
         ScopedPhase ph(c, PSE_T_REAL);
-        const int wpb = 256 / 32;
-        int grid = 4 * c->nsm;
+        const int wpb = 384 / 32;
+        int grid = 2 * c->nsm;
         if ((long long)grid * wpb * 4 > c->N) grid = (c->N + wpb * 4 - 1) / (wpb * 4);
-        real_rot_kernel<<<grid, 256, 0, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(in8), reinterpret_cast<const float4 *>(inL), out8, outW,
-                                                     c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, reinterpret_cast<const float4 *>(c->d_rot_table),
-                                                     (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L, pse_lat(c));
+        real_pairs_full_kernel<<<grid, 384, FULL_SMEM, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(in8), reinterpret_cast<const float4 *>(inL),
+                                                                    out8, outW, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx,
+                                                                    reinterpret_cast<const float4 *>(c->d_table), reinterpret_cast<const float4 *>(c->d_rot_table),
+                                                                    (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L, pse_lat(c));
         KERNEL_CHECK(c);
     } else {
         CUDA_TRY(c, cudaMemsetAsync(out8, 0, vec, c->stream));
