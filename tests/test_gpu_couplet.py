@@ -204,3 +204,41 @@ def test_step_with_external_torques_against_dense_oracle():
     d1 = (p1 - dev(pos4(x.astype(np.float32))))[:, :3].cpu().numpy()
     d0 -= L * np.round(d0 / L); d1 -= L * np.round(d1 / L)
     assert rel(d0, d1) < 3 * bar(tol) and rel(d, d0) > 10 * bar(tol)
+
+
+def test_edge_cases_single_sphere_odd_grid_and_bitwise_repeats():
+    """(1) One sphere: the GPU reproduces the exact periodic rotational self-mobility Omega = L/(8 pi eta a^3) (1 - (4 pi/3)(a/L)^3)
+    (pin C1 of the oracle) within the bar; (2) an odd grid (planes padded to 16-byte starts, no TMA) with an odd support;
+    (3) two contexts and repeated calls agree bit for bit (every kernel of the full-couplet path has a fixed summation order)."""
+    import paper_1709_06946_b200 as pse
+    # (1)
+    L, xi, tol = 12.0, 0.7, 1e-4
+    st, g, p, rcut = pse.pse_suggest_params(1, L, A, tol, xi)
+    ctx = pse.pse_create(1, L, A, ETA, KT, xi, g, p, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(np.array([[0.3, 11.9, 5.5]], np.float32))))
+    Lq = np.array([[0.2, -1.0, 0.5]])
+    U, W, E = gpu_full(ctx, None, Lq, None)
+    want = Lq / (8 * np.pi * ETA * A**3) * (1.0 - 4 * np.pi / 3 * (A / L)**3)
+    assert rel(W, want) < bar(tol) and np.abs(U).max() < bar(tol) * np.abs(want).max() and np.abs(E).max() < bar(tol) * np.abs(want).max()
+    # (2)
+    N, xi, tol = 120, 0.6, 1e-3
+    x, L = synth.rsa(N, 0.15, seed=17)
+    x32 = x.astype(np.float32)
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    outs = []
+    for rep in range(2):
+        ctx = pse.pse_create(N, L, A, ETA, KT, xi, 27, 5, rcut, tol)          # 27^3: odd, not a multiple of 4
+        ctx.pse_neighbors(dev(pos4(x32)))
+        F, Lq, S = inputs(N, 9)
+        a_ = gpu_full(ctx, F, Lq, S)
+        b_ = gpu_full(ctx, F, Lq, S)
+        w1 = np.random.default_rng(3).standard_normal((N, 11))
+        _, w2 = synth.brownian_noise(N, 27, 3)
+        UB, WB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+        ctx.pse_brownian_full(1e-3, dev(w1), dev(w2), UB, WB, EB)
+        assert all(np.array_equal(u, v) for u, v in zip(a_, b_))
+        outs.append(a_ + (UB.cpu().numpy(), WB.cpu().numpy(), EB.cpu().numpy()))
+    assert all(np.array_equal(u, v) for u, v in zip(*outs))
+    want = cpl.mobility_apply_full(x32.astype(np.float64), L, A, ETA, xi, F, Lq, S, eps=1e-9)
+    for g_, w_, name in zip(outs[0][:3], want, 'UWE'):
+        assert rel(g_, w_) < bar(tol), (name, rel(g_, w_))
