@@ -258,3 +258,34 @@ def test_sedimentation_velocity_error_on_a_sheared_grid_tracks_the_tolerance():
     for xi, tol, P, grid, err in rows:
         assert P == {1e-2: 3, 1e-3: 4, 1e-4: 5}[tol] and err < bar(tol), (xi, tol, err)
     assert all(rows[i + 1][4] < rows[i][4] for i in (0, 1, 3, 4))          # and it falls with the tolerance at fixed xi
+
+
+def test_lattice_edge_cases_pair_across_the_sheared_boundary_compression_and_repeats():
+    """(1) Two spheres that are neighbours only through the sheared image (x1 = x0 + d + the lattice vector (gamma L, L, 0)): each is in
+    the other's list and the product matches the direct sums; (2) a cell compressed along x (epsilon < 1); (3) bit-identical repeats."""
+    import paper_1709_06946_b200 as pse
+    L, xi, tol, g = 14.0, 0.7, 1e-3, 0.5
+    x = np.array([[1.0, 0.3, 4.0], [1.0 + 1.5 + g * L, 0.3 + 1.2 + L, 4.5], [7.0, 7.0, 7.0]])
+    x32 = x.astype(np.float32)
+    ctx, rcut = make(3, L, xi, tol, (1.0, g, 1.0), x32)
+    sets = nbr_sets(ctx)
+    assert 1 in sets[0] and 0 in sets[1]
+    F, S = synth.gaussian_inputs(3, 2)
+    Uo, Eo = lat.mobility_apply(x32.astype(np.float64), L, lat.shear(g), A, ETA, xi, F, S, eps=1e-10)
+    U, E = gpu_apply(ctx, F, S)
+    assert rel(U, Uo) < bar(tol) and rel(E, Eo) < bar(tol)
+    # the same pair in the cube would not interact through that image
+    cube = lat.neighbor_sets(x32, L, 1.0, 0.0, 1.0, rcut)
+    assert 1 not in cube[0]
+    # (2), (3)
+    l3 = (0.8, 0.0, 1.25)
+    N = 300
+    xs, Ls = deformed_suspension(N, 0.2, l3, seed=31)
+    F, S = synth.gaussian_inputs(N, 3)
+    outs = []
+    for rep in range(2):
+        ctx, _ = make(N, Ls, 0.6, 1e-3, l3, xs)
+        outs.append(gpu_apply(ctx, F, S) + gpu_apply(ctx, F, S))
+    assert all(np.array_equal(outs[0][0], o) for o in (outs[0][2], outs[1][0], outs[1][2]))
+    Uo, Eo = lat.mobility_apply(xs.astype(np.float64), Ls, matrix(l3), A, ETA, 0.6, F, S, eps=1e-9)
+    assert rel(outs[0][0], Uo) < bar(1e-3) and rel(outs[0][1], Eo) < bar(1e-3)
