@@ -492,6 +492,12 @@ def main():
         blk.update(steps=a4.steps, warmup=a4.warmup)
         blk['hbm_fraction_per_kernel'] = {k: round(v['frac_of_hbm_peak'], 4) for k, v in blk['phases'].items() if 'frac_of_hbm_peak' in v}
         line['config4'] = blk
+        # the headline workload once more in a sheared periodic cell (NEXT-4; Eq. 56 at strain 0.5, the largest a Lees-Edwards cell reaches)
+        wls = dict(wl, shear=0.5)
+        rsh = run_ours(a4, wls, rank, world)
+        line['sheared_cell'] = {'strain': 0.5, 'value': replica_throughput(a4.steps, world, rsh['ms']), 'unit': 'steps/s', 'ms_per_step': rsh['ms'] / a4.steps,
+                                'grid': rsh['grid'], 'P': rsh['P'], 'matvecs_per_sec': 1e3 / rsh['matvec_ms'], 'e2e_steps_per_sec': 1e3 / rsh['e2e_ms'],
+                                'steps': a4.steps, 'warmup': a4.warmup}
     if not args.no_cpu_baseline:
         rs = ReferenceStepper(wl)
         sec, its = rs.step()
