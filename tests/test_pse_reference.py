@@ -121,7 +121,7 @@ def test_tree_based_overlap_force_equals_the_dense_one():
 
 def test_full_couplet_reference_against_direct_sums(small):
     """Torque in, angular velocity out (oracle/couplet.py) through the reference's NUFFT and cut-off pair sum: every output block
-    against the direct Ewald sums at another xi, all rows at N = 300 (one overlapping pair) and sampled rows at N = 1 000."""
+    against the direct Ewald sums at another xi, all rows at N = 300 (one overlapping pair) and sampled rows at N = 600."""
     from oracle import couplet as cpl
     x, L, F, S = small
     Lq = np.random.default_rng(8).standard_normal((300, 3))
@@ -133,11 +133,11 @@ def test_full_couplet_reference_against_direct_sums(small):
     wr = cpl.mobility_apply_full(x, L, A, ETA, 0.9, F, Lq, S, eps=1e-12, part='wave')
     for g, w, t in zip(ref.wave_apply_full(x, F, Lq, S), wr, want):
         assert np.linalg.norm(g - w) < 1e-7 * np.linalg.norm(t)
-    x, L = synth.rsa(1000, 0.30, seed=22)
-    F, S = synth.gaussian_inputs(1000, 22)
-    Lq = np.random.default_rng(9).standard_normal((1000, 3))
-    rows = np.sort(np.random.default_rng(1).choice(1000, 8, replace=False))
-    want = cpl.mobility_apply_full(x, L, A, ETA, 0.6, F, Lq, S, rows=rows, eps=1e-11)
-    got = pr.PSEReference(L, A, ETA, 0.5, tol=1e-8).apply_full(x, F, Lq, S, rows=rows)
+    x, L = synth.rsa(600, 0.30, seed=22)
+    F, S = synth.gaussian_inputs(600, 22)
+    Lq = np.random.default_rng(9).standard_normal((600, 3))
+    rows = np.sort(np.random.default_rng(1).choice(600, 8, replace=False))
+    want = cpl.mobility_apply_full(x, L, A, ETA, 0.75, F, Lq, S, rows=rows, eps=1e-11)
+    got = pr.PSEReference(L, A, ETA, 0.6, tol=1e-8).apply_full(x, F, Lq, S, rows=rows)
     for g, w in zip(got, want):
         assert rel(g, w) < 1e-7
