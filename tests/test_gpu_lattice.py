@@ -242,22 +242,24 @@ def test_sedimentation_velocity_error_on_a_sheared_grid_tracks_the_tolerance():
     with the orthorhombic bound miss the tolerance by an order of magnitude; here the window acts on lattice coordinates (reading
     R22), so the cube's P = 3, 4, 5 must meet the bar on the sheared grid as well.  Reference: direct sums of oracle.lattice."""
     N, l3 = 500, SHEAR
-    x32, L = deformed_suspension(N, 0.15, l3, seed=21)
-    x, Am = x32.astype(np.float64), matrix(l3)
     F = np.tile(np.array([0.0, 0.0, -1.0]), (N, 1))
     S = np.zeros((N, 5))
-    Uo, _ = lat.mobility_apply(x, L, Am, A, ETA, 0.6, F, S, eps=1e-10)
     rows = []
-    for xi in (0.5, 0.65):
-        for tol in (1e-2, 1e-3, 1e-4):
-            ctx, _ = make(N, L, xi, tol, l3, x32)
-            U, _ = gpu_apply(ctx, F, S)
-            rows.append((xi, tol, ctx.P, ctx.grid, rel(U, Uo)))
-            ctx.close()
-    print('\n'.join(f'xi={r[0]} tol={r[1]:g} P={r[2]} grid={r[3]} err={r[4]:.2e}' for r in rows))
-    for xi, tol, P, grid, err in rows:
-        assert P == {1e-2: 3, 1e-3: 4, 1e-4: 5}[tol] and err < bar(tol), (xi, tol, err)
-    assert all(rows[i + 1][4] < rows[i][4] for i in (0, 1, 3, 4))          # and it falls with the tolerance at fixed xi
+    for cell in ((1.0, 0.0, 1.0), l3):                        # the same suspension in the cube and carried along by the shear
+        x32, L = deformed_suspension(N, 0.15, cell, seed=21)
+        Uo, _ = lat.mobility_apply(x32.astype(np.float64), L, matrix(cell), A, ETA, 0.6, F, S, eps=1e-10)
+        for xi in (0.5, 0.65):
+            for tol in (1e-2, 1e-3, 1e-4):
+                ctx, _ = make(N, L, xi, tol, cell, x32)
+                U, _ = gpu_apply(ctx, F, S)
+                rows.append((cell[1], xi, tol, ctx.P, ctx.grid, rel(U, Uo)))
+                ctx.close()
+    print('\n'.join(f'gamma={r[0]} xi={r[1]} tol={r[2]:g} P={r[3]} grid={r[4]} err={r[5]:.2e}' for r in rows))
+    cube, sheared = rows[:6], rows[6:]
+    for (_, xi, tol, P, grid, err), (_, _, _, Pc, gridc, errc) in zip(sheared, cube):
+        assert P == Pc == {1e-2: 3, 1e-3: 4, 1e-4: 5}[tol] and grid >= gridc and err < bar(tol), (xi, tol, err)
+        assert err < 1.3 * errc + 0.2 * tol, (xi, tol, err, errc)          # the sheared grid is as accurate as the cube's
+    assert all(sheared[i + 1][5] < sheared[i][5] for i in (0, 1, 3, 4))    # and the error falls with the tolerance at fixed xi
 
 
 def test_lattice_edge_cases_pair_across_the_sheared_boundary_compression_and_repeats():
