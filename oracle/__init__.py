@@ -21,6 +21,16 @@ It is a plain, slow, obviously-correct statement of what the path computes:
                    Gaussian NUFFT of Eq. 42 with scipy's FFT, textbook Lanczos / GMRES), pinned against the direct sums at
                    N <= 4 096; the parity reference at N >= 65 536 and bench.py's second timed CPU baseline.
 
+* ``couplet``    – the full couplet of Eq. (31): torque in, angular velocity out, 11N x 11N matrix, constrained
+                   solve and mid-point step with torques, 11-component Brownian sample (reading R21).  Pins C1-C10
+                   (tests/test_oracle_couplet.py): exact periodic rotational self-mobility, textbook pair forms incl. overlap,
+                   xi-independence per block, SPD, covariance identity of the wave factor, reduction to the 8-component step.
+* ``lattice``    – deformed periodic cells (reading R22): Eqs. (55)-(59), direct sums with lattice vectors L A,
+                   fp32 neighbour sets, Brownian sample, and ``LatticeReference``, the NUFFT tier in lattice coordinates.
+                   Pins L1-L8 (tests/test_oracle_lattice.py): Table I as printed (tests/golden/paper_table1.py), identity
+                   lattice, lattice equivalence gamma -> gamma +- 1, a rectangular box written out by hand, xi-independence, SPD,
+                   covariance identity of the sheared wave factor, the reference tier against the direct sums.
+
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): Hasimoto periodic self-mobility, xi-independence of
 M_r + M_w, symmetry and positive-definiteness of M, M_r, M_w, textbook RPY / RPY-overlap free-space
 limits, printed closed forms F1, F2 of Appendix A, exact covariance identity

@@ -141,3 +141,29 @@ def test_L7_lattice_reference_tier_against_direct_sums():
         ww = lat.mobility_apply(x, L, A, A_, ETA, 1.0, F, S, rows=rows, eps=1e-12, part='wave')
         gw = ref.wave_apply(x, F, S, rows)
         assert np.linalg.norm(gw[0] - ww[0]) < 1e-7 * np.linalg.norm(want[0]) and np.linalg.norm(gw[1] - ww[1]) < 1e-7 * np.linalg.norm(want[1])
+
+
+def test_L8_brownian_wave_factor_on_a_sheared_lattice_has_the_covariance_of_its_matrix():
+    """oracle.brownian.wave_sqrt_apply with the lattice argument (used by oracle.lattice.brownian): A_w A_w^T equals the wave-space
+    matrix summed over exactly the modes k = (2 pi/L) A^-T n of the noise grid (pin P9 carried to a sheared cell), and
+    lattice.brownian with zero wave noise is sqrt(2kT/dt) sqrtm(M_r) w1 of the sheared real-space matrix."""
+    from oracle import brownian as brn
+    from oracle import functions as fn
+    x, L, _, _ = cluster(N=3, L=7.0, seed=4)
+    A, xi, Mg = lat.shear(0.3), 0.8, 4
+    ncol = 3 * Mg * Mg * (Mg // 2 + 1) * 2
+    Aw = np.zeros((24, ncol))
+    for c in range(ncol):
+        w = np.zeros(ncol); w[c] = 1.0
+        Aw[:, c] = np.concatenate(brn.wave_sqrt_apply(x, L, A_, ETA, xi, Mg, w, A=A), axis=1).ravel()
+    _, n = brn.canonical_modes(Mg)
+    k = 2 * np.pi * (np.concatenate([n, -n]) @ np.linalg.inv(A)) / L
+    k2 = np.einsum('ki,ki->k', k, k)
+    M = mob.dense_wave_modes(x, A_, k, fn.hasimoto_H(np.sqrt(k2), xi) / (ETA * L**3 * k2))
+    assert np.abs(Aw @ Aw.T - M).max() < 1e-13 * np.abs(M).max()
+    assert np.abs(Aw - np.column_stack([np.concatenate(brn.wave_sqrt_apply(x, L, A_, ETA, xi, Mg, np.eye(ncol)[c]), axis=1).ravel()
+                                        for c in range(ncol)])).max() > 1e-3 * np.abs(Aw).max()        # and it is not the cube's factor
+    w1 = np.random.default_rng(2).standard_normal((3, 8))
+    U, E = lat.brownian(x, L, A, A_, ETA, 0.7, xi, 1e-3, Mg, w1, np.zeros(ncol))
+    R = brn.sqrtm_psd(lat.dense(x, L, A, A_, ETA, xi, part='real'))
+    assert rel(np.hstack([U, E]).ravel(), np.sqrt(2 * 0.7 / 1e-3) * (R @ w1.ravel())) < 1e-12
