@@ -154,7 +154,7 @@ def constrained_solve_full(M, N, UB, WB, EB, F, Lq):
     return UW[:, :3], UW[:, 3:], S.reshape(N, 5)
 
 
-def wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf, rows=None, A=None):
+def wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf, rows=None):
     """A_w w2 of Eq. (75) with the angular-velocity rows: the random field uh = sqrt(H/(eta V k^2)) (I - kh kh) W(k)
     over the modes of the Mg^3 grid is that of oracle.brownian.wave_sqrt_apply (same noise buffer, reading R8); here its moments are
     U = s0 uh, Omega = (i/2) s1 k x uh, E^q = i s1 (e^q k).uh.  Returns U, Omega, E at the particles (rows)."""
@@ -165,7 +165,7 @@ def wave_sqrt_apply_full(x, L, a, eta, xi, Mg, wbuf, rows=None, A=None):
     N = x.shape[0]
     wbuf = np.asarray(wbuf, dtype=np.float64).reshape(3, Mg, Mg, Mg // 2 + 1, 2)
     idx, n = brn.canonical_modes(Mg)
-    k = 2 * np.pi * n / L if A is None else 2 * np.pi * (n @ np.linalg.inv(np.asarray(A, dtype=np.float64))) / L
+    k = 2 * np.pi * n / L
     Wn = (wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 0] + 1j * wbuf[:, idx[:, 0], idx[:, 1], idx[:, 2], 1]).T / np.sqrt(2)
     e = fn.basis()
     U, W, E = np.zeros((N, 3)), np.zeros((N, 3)), np.zeros((N, 5))
