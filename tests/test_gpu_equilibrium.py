@@ -77,17 +77,22 @@ def test_step_with_bonds_against_dense_oracle():
     assert np.linalg.norm(d) / np.linalg.norm(disp) < 5 * tol
 
 
-def test_pair_distance_distribution_matches_eq80():
+@pytest.mark.parametrize('gamma', [0.0, 0.3], ids=['cube', 'sheared_cell'])
+def test_pair_distance_distribution_matches_eq80(gamma):
     """64 bonded pairs in a dilute periodic box (phi = 0.002), 40 000 mid-point steps: the histogram of the
     centre-to-centre distance and its first moments against Eq. (80).  The bond keeps r > 2a with
-    probability 1 - 1e-4 (r0 = 5a, k = 3 kT/a), so the hard-sphere force plays no role inside a pair."""
+    probability 1 - 1e-4 (r0 = 5a, k = 3 kT/a), so the hard-sphere force plays no role inside a pair.
+    Second case: the same in a cell sheared to gamma = 0.3 (pse_set_lattice, NEXT-4): the equilibrium distribution does not
+    know about the lattice, so the whole deformed-lattice step path (graphs included) must reproduce it as well."""
     import paper_1709_06946_b200 as pse
     npair, k, r0, dt, tol, xi = 64, 3.0, 5.0, 2.5e-3, 1e-3, 0.3
     nsteps, burn, every = 40000, 1000, 4
     N, L = 2 * npair, 64.0
-    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi, lattice=(1.0, gamma, 1.0))
     assert st == 0
     ctx = pse.pse_create(N, L, A, ETA, KT, xi, grid, P, rcut, tol)
+    if gamma:
+        ctx.pse_set_lattice(1.0, gamma, 1.0)
     c = (np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing='ij'), -1).reshape(-1, 3) + 0.5) * (L / 4)    # 4^3 pair centres
     x = np.empty((N, 3))
     x[0::2] = c - [r0 / 2, 0, 0]
@@ -106,7 +111,9 @@ def test_pair_distance_distribution_matches_eq80():
         ctx.pse_step(pos, dt, w1, w2)
         if s >= burn and s % every == 0:
             d = pos[0::2, :3] - pos[1::2, :3]
+            d[:, 0] -= gamma * d[:, 1]                        # minimum image in lattice coordinates s = A^-1 x, back to x = A s
             d = d - L * torch.round(d / L)
+            d[:, 0] += gamma * d[:, 1]
             samples.append(d.norm(dim=1))
     r = torch.cat(samples).double().cpu().numpy()
     # Eq. (80) by quadrature
