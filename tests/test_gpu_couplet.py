@@ -242,3 +242,36 @@ def test_edge_cases_single_sphere_odd_grid_and_bitwise_repeats():
     want = cpl.mobility_apply_full(x32.astype(np.float64), L, A, ETA, xi, F, Lq, S, eps=1e-9)
     for g_, w_, name in zip(outs[0][:3], want, 'UWE'):
         assert rel(g_, w_) < bar(tol), (name, rel(g_, w_))
+
+
+def test_translational_rotational_brownian_covariance():
+    """<[U^B; Omega^B][U^B; Omega^B]^T> = (2 kT/dt) M_{script-U script-F} (Eq. 71 for the 11-component sample): two spheres
+    at r = 2.5a, 8 000 draws of pse_brownian_full with fresh device noise, against the 12 x 12 block of the oracle's dense matrix
+    (which contains the translation-rotation coupling of the pair)."""
+    import paper_1709_06946_b200 as pse
+    N, L, xi, tol, dt, ndraw = 2, 16.0, 0.5, 1e-3, 1e-2, 8000
+    x = np.array([[4.0, 4.0, 4.0], [6.0, 5.5, 4.0]])
+    st, g, p, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    ctx = pse.pse_create(N, L, A, ETA, KT, xi, g, p, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x.astype(np.float32))))
+    gen = torch.Generator(device='cuda')
+    gen.manual_seed(7)
+    w1 = torch.empty(N, 11, device='cuda')
+    w2 = torch.empty(3, g, g, g // 2 + 1, 2, device='cuda')
+    UB, WB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    acc = torch.zeros(12, 12, device='cuda', dtype=torch.float64)
+    for _ in range(ndraw):
+        w1.normal_(generator=gen)
+        w2.normal_(generator=gen)
+        ctx.pse_brownian_full(dt, w1, w2, UB, WB, EB)
+        v = torch.cat([UB, WB], dim=1).reshape(-1).double()
+        acc += torch.outer(v, v)
+    C = (acc / ndraw).cpu().numpy() * dt / (2 * KT)
+    M = cpl.dense_full(x, L, A, ETA, xi, eps=1e-10)
+    keep = np.array([11 * i + c for i in range(N) for c in range(6)])
+    Mo = M[np.ix_(keep, keep)]
+    err = np.linalg.norm(C - Mo) / np.linalg.norm(Mo)
+    tr_block = np.abs(Mo[:3, 9:12]).max()                            # U_1 <- L_2: the rotlet coupling, must be resolved
+    print(f'brownian_full covariance: rel Frobenius error {err:.3f}, max |C - M| {np.abs(C - Mo).max():.4f}, rotlet block {tr_block:.4f}')
+    assert err < 0.05
+    assert np.abs(C[:3, 9:12] - Mo[:3, 9:12]).max() < 0.5 * tr_block + 4 * np.sqrt(Mo[0, 0] * Mo[9, 9] / ndraw)
