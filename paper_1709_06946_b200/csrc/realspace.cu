@@ -132,15 +132,15 @@ real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in,
 constexpr size_t REAL_SMEM = (size_t)PSE_NTAB * 2 * sizeof(float4);
 
 template <int MODE>
-static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, int grid) {
+static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, int grid, int threads) {
     const float4 *in4 = reinterpret_cast<const float4 *>(d_in), *tab = reinterpret_cast<const float4 *>(c->d_table);
     float4 *out4 = reinterpret_cast<float4 *>(d_out);
     const float inv_dr = (float)(1.0 / c->tab_dr), L = (float)c->L, invL = 1.0f / (float)c->L;
     if (c->deformed)
-        real_pairs_kernel<MODE, true><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
+        real_pairs_kernel<MODE, true><<<grid, threads, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
                                                                          inv_dr, L, invL, pse_lat(c));
     else
-        real_pairs_kernel<MODE, false><<<grid, 512, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
+        real_pairs_kernel<MODE, false><<<grid, threads, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
                                                                           inv_dr, L, invL, pse_lat(c));
     KERNEL_CHECK(c);
     return PSE_OK;
@@ -158,16 +158,28 @@ pse_status pse_real_init(pse_ctx *c) {
 
 pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode) {
     ScopedPhase ph(c, PSE_T_REAL);
-    int grid = 2 * c->nsm;
-    const int wpb = 512 / 32;
-    if ((long long)grid * wpb * 4 > c->N) grid = (c->N + wpb * 4 - 1) / (wpb * 4);
+    int grid = 2 * c->nsm, wpb = 512 / 32;
+    const long long tasks = ((long long)c->N + 3) / 4;           // one warp pass = 4 particles
+    if ((long long)grid * wpb >= tasks) grid = (int)((tasks + wpb - 1) / wpb);
+    else {
+        // The persistent warps take whole tasks round-robin, so a launch lasts ceil(tasks / warps) rounds and the last one may be
+        // nearly empty (config 3: 3.46 rounds of 16-warp CTAs).  A round costs about in proportion to the warps that share an SM's L1,
+        // so narrower CTAs whose last round is full win: 14 warps at config 3 (3.95 rounds), 33.5 -> 31.2 us per launch; taken only
+        // where the model promises 8 % (measured: about half of what it promises); large N keeps 16 warps.
+        auto cost = [&](int w) { return ((tasks + (long long)grid * w - 1) / ((long long)grid * w)) * w; };
+        const long long c16 = cost(16);
+        long long best = c16;
+        for (int w = 15; w >= 12; --w)
+            if (cost(w) < best && cost(w) * 100 <= c16 * 92) { best = cost(w); wpb = w; }
+    }
+    const int threads = wpb * 32;
     // unrequested outputs are written as zeros; absent inputs must be zero in d_in (they are skipped, not read as data)
     switch (mode) {
-        case PSE_IN_S | PSE_OUT_E: return launch_real<PSE_IN_S | PSE_OUT_E>(c, d_in, d_out, grid);
-        case PSE_IN_F | PSE_OUT_E: return launch_real<PSE_IN_F | PSE_OUT_E>(c, d_in, d_out, grid);
-        case PSE_IN_F | PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid);
-        case PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid);
-        case PSE_IN_F | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_OUT_U>(c, d_in, d_out, grid);
-        default: return launch_real<PSE_MODE_ALL>(c, d_in, d_out, grid);
+        case PSE_IN_S | PSE_OUT_E: return launch_real<PSE_IN_S | PSE_OUT_E>(c, d_in, d_out, grid, threads);
+        case PSE_IN_F | PSE_OUT_E: return launch_real<PSE_IN_F | PSE_OUT_E>(c, d_in, d_out, grid, threads);
+        case PSE_IN_F | PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid, threads);
+        case PSE_IN_S | PSE_OUT_U: return launch_real<PSE_IN_S | PSE_OUT_U>(c, d_in, d_out, grid, threads);
+        case PSE_IN_F | PSE_OUT_U: return launch_real<PSE_IN_F | PSE_OUT_U>(c, d_in, d_out, grid, threads);
+        default: return launch_real<PSE_MODE_ALL>(c, d_in, d_out, grid, threads);
     }
 }
