@@ -1,7 +1,7 @@
 // Real-space pair kernel (step a2): [U;E]_alpha = sum_beta M^(r)(x_alpha - x_beta) [F;S]_beta + self term
 // (Eqs. 25-27; self terms Eqs. A4/A12), over the neighbour list.
 //
-// Design: persistent CTAs (2 per SM), the table of (F1,F2,Ga,Gb | A,B,D,-) staged once per CTA in shared memory as two
+// Design: persistent CTAs (2 per SM, 16 warps each or fewer where that fills the last round: pse_real_apply), the table of (F1,F2,Ga,Gb | A,B,D,-) staged once per CTA in shared memory as two
 // planar float4 arrays, EIGHT lanes per particle (four particles per warp, four independent idx -> pos -> input chains in
 // flight), lanes stride the CSR neighbour list, one 128-bit gather of the neighbour's position and one 256-bit gather of its
 // packed input, linear interpolation of the table in r, 7-shuffle reduction of the 8 outputs over the 8 lanes and one
