@@ -79,7 +79,9 @@ pse_status pse_destroy(pse_ctx *ctx);
  * accepted.  Inside, particles are carried in lattice coordinates s = A^-1 x, so cells, spreading and interpolation are those of
  * the cube, separations are r = A d and wave vectors k = (2 pi/L) A^-T n (reading R22): P is that of the cube, the grid
  * must be pse_suggest_params_lattice's.  Call before pse_neighbors; the neighbour structures are invalidated; pse_step then leaves
- * positions unwrapped.  (1, 0, 1) restores the cube.  Synchronises the stream.
+ * positions unwrapped.  (1, 0, 1) restores the cube.  Synchronises the stream.  Cheap enough to call before every step of a flowing
+ * suspension (grid taken for the largest strain): the kernels read A from device memory, so the captured graphs of pse_step survive
+ * the call and are rebuilt only when the cell count of the neighbour search changes or the lattice becomes / stops being the cube.
  * PSE_EINVAL: a11 <= 0, a22 <= 0, a11 a22 != 1, or rcut * (largest row norm of A^-1) > L/2. */
 pse_status pse_set_lattice(pse_ctx *ctx, double a11, double a12, double a22);
 

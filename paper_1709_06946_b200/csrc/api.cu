@@ -9,6 +9,8 @@ pse_status pse_apply_packed(pse_ctx *c, const float *d_in, float *d_out, int whi
 
 namespace {
 
+__global__ void k_set_lat(Lat *dst, Lat v) { *dst = v; }
+
 __global__ void k_advance(const float4 *pos_in, const float *U, float dt, float L, float invL, int N, float4 *pos_out, int wrap) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -153,6 +155,7 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     pse_build_table(a, eta, xi, rcut, PSE_NTAB, tab, &c->tab_dr);
     CUDA_TRY(c, cudaMalloc(&c->d_table, tab.size() * sizeof(float)));
     CUDA_TRY(c, cudaMemcpy(c->d_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    { const Lat id = pse_lat(c); CUDA_TRY(c, cudaMalloc(&c->d_lat, sizeof(Lat))); CUDA_TRY(c, cudaMemcpy(c->d_lat, &id, sizeof(Lat), cudaMemcpyHostToDevice)); }
     // cells: edge >= rcut with a relative margin far above fp32 rounding of the binning
     c->nc = std::max(1, (int)std::floor(L / (rcut * 1.0001)));
     c->ncell = c->nc * c->nc * c->nc;
@@ -226,7 +229,7 @@ pse_status pse_destroy(pse_ctx *c) {
     cudaFree(c->d_stage_pos); cudaFree(c->d_stage_a); cudaFree(c->d_stage_b); cudaFree(c->d_stage_noise);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     if (c->h_scal_l) cudaFreeHost(c->h_scal_l);
-    cudaFree(c->d_xk);
+    cudaFree(c->d_xk); cudaFree(c->d_lat);
     delete c;
     return PSE_OK;
 }
@@ -244,9 +247,11 @@ pse_status pse_set_lattice(pse_ctx *c, double a11, double a12, double a22) {
         c->err = "pse_set_lattice: rcut * max row norm of A^-1 > L/2 (the minimum image in lattice coordinates would miss pairs)"; return PSE_EINVAL;
     }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }   // the lattice is baked in
     c->lat_a11 = a11; c->lat_a12 = a12; c->lat_a22 = a22;
     c->deformed = !(a11 == 1.0 && a12 == 0.0 && a22 == 1.0);
+    // The kernels read A from device memory, so the captured graphs of pse_step stay valid while the strain advances step by step
+    // (a flowing suspension); they are keyed by the cell count and by cube / deformed, which select grids and instantiations.
+    k_set_lat<<<1, 1, 0, c->stream>>>(c->d_lat, pse_lat(c)); KERNEL_CHECK(c);
     // cells of lattice-coordinate edge >= reach * rcut (never more cells than pse_create made room for: reach >= 1)
     c->nc = std::max(1, (int)std::floor(c->L / (c->rcut * 1.0001 * reach)));
     c->ncell = c->nc * c->nc * c->nc;
@@ -408,7 +413,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
                 user_pos = d_pos;
                 d_pos = c->d_stage_pos; d_noise_real = c->d_stage_a; d_noise_wave = c->d_stage_noise;
             }
-            const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap};
+            const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap, c->nc, c->deformed};
             if (!c->step_graph[0] || !(key == c->graph_key)) {
                 for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
                 const long long l0 = c->launches;

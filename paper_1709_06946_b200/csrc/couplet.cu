@@ -33,7 +33,8 @@ __global__ void __launch_bounds__(384, 2)
 real_pairs_full_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in8, const float4 *__restrict__ inL, float *__restrict__ out8,
                        float *__restrict__ outW, int N, const unsigned long long *__restrict__ off, const int *__restrict__ cnt,
                        const int *__restrict__ idx, const float4 *__restrict__ table, const float4 *__restrict__ rtable, float inv_dr, float L,
-                       float invL, Lat lat) {
+                       float invL, const Lat *__restrict__ latp) {
+    const Lat lat = *latp;
     extern __shared__ float4 ftab[];                           // tabU[NTAB] | tabE[NTAB] | tabR[NTAB]
     float4 *tabU = ftab, *tabE = ftab + PSE_NTAB, *tabR = ftab + 2 * PSE_NTAB;
     for (int i = threadIdx.x; i < PSE_NTAB; i += blockDim.x) { tabU[i] = table[2 * i]; tabE[i] = table[2 * i + 1]; tabR[i] = rtable[i]; }
@@ -247,7 +248,7 @@ static pse_status apply_full_packed(pse_ctx *c, const float *in8, const float *i
         real_pairs_full_kernel<<<grid, 384, FULL_SMEM, c->stream>>>(c->d_pos, reinterpret_cast<const float4 *>(in8), reinterpret_cast<const float4 *>(inL),
                                                                     out8, outW, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx,
                                                                     reinterpret_cast<const float4 *>(c->d_table), reinterpret_cast<const float4 *>(c->d_rot_table),
-                                                                    (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L, pse_lat(c));
+                                                                    (float)(1.0 / c->tab_dr), (float)c->L, 1.0f / (float)c->L, c->d_lat);
         KERNEL_CHECK(c);
     } else {
         CUDA_TRY(c, cudaMemsetAsync(out8, 0, vec, c->stream));

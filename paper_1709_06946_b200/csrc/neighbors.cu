@@ -141,9 +141,10 @@ __device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL, 
 }
 
 __global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int nc, float cell_inv,
-                             float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count, Lat lat) {
+                             float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count, const Lat *__restrict__ latp) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    const Lat lat = *latp;
     float4 p = pos[i];
     p.x = __fadd_rn(__fmul_rn(lat.i11, p.x), __fmul_rn(lat.i12, p.y)); p.y = __fmul_rn(lat.i22, p.y);     // s = A^-1 x (exact on the cube)
     p.x = wrap_coord(p.x, L, invL); p.y = wrap_coord(p.y, L, invL); p.z = wrap_coord(p.z, L, invL); p.w = 0.f;
@@ -199,9 +200,10 @@ constexpr int NS_CHUNK = 1024, NS_THREADS = 128;
 template <bool FILL>
 __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start,
                                                                    int nc, float L, float invL, float rc2, int *__restrict__ cursor,
-                                                                   const unsigned long long *__restrict__ off, int *__restrict__ idx, Lat lat) {
+                                                                   const unsigned long long *__restrict__ off, int *__restrict__ idx, const Lat *__restrict__ latp) {
     __shared__ float4 cpos[NS_CHUNK];
     __shared__ int run_lo[18], run_cum[19];
+    const Lat lat = *latp;
     const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int first = cell_start[cell], np = cell_start[cell + 1] - first;
     if (np == 0) return;
@@ -277,10 +279,13 @@ constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32, NB_PB = 4;
 
 template <bool DEF>                                           // DEF: deformed lattice, the screened separation is mapped by A as well
 __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
-                                                                   float L, float invL, float rc2, float band, int *__restrict__ count,
+                                                                   float L, float invL, float rc2, float band0, int *__restrict__ count,
                                                                    unsigned long long *__restrict__ off, int *__restrict__ idx,
                                                                    unsigned long long cap, unsigned long long *__restrict__ cursor,
-                                                                   int *__restrict__ fallback, Lat lat) {
+                                                                   int *__restrict__ fallback, const Lat *__restrict__ latp) {
+    // the lattice is read from device memory so that a captured step stays valid while the strain advances (pse_set_lattice)
+    const Lat lat = DEF ? *latp : Lat{1.f, 0.f, 1.f, 1.f, 0.f, 1.f};
+    const float band = DEF ? band0 * 4.f * (fabsf(lat.a11) + fabsf(lat.a12) + fabsf(lat.a22)) : band0;
     __shared__ float4 cpos[NS_CHUNK];
     __shared__ unsigned masks[NB_MAXP][NB_WORDS];
     __shared__ int cnt[NB_MAXP], loc[NB_MAXP];
@@ -438,7 +443,8 @@ __global__ void lists_to_original(const int *idx, const unsigned long long *off_
 
 // Heyes-Melrose overlap force (reading R12), 8 lanes per particle over the neighbour list (as the pair kernel), packed output.
 __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned long long *__restrict__ off, const int *__restrict__ count,
-                          const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out, Lat lat) {
+                          const int *__restrict__ idx, float L, float invL, float two_a, float coef, float *__restrict__ out, const Lat *__restrict__ latp) {
+    const Lat lat = *latp;
     const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 3, gl = threadIdx.x & 7;
     const bool live = s < N;
     const float4 p = live ? pos[s] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -467,9 +473,10 @@ __global__ void hs_forces(const float4 *__restrict__ pos, int N, const unsigned 
 // Forces of the bond potential U(r) = k |r - r0| of the paper's equilibrium test: a thread per bond,
 // positions and output in original numbering, F_i -= k sign(r - r0) rhat_ij, F_j += the same (out is zeroed beforehand).
 __global__ void bond_forces(const float4 *__restrict__ posw, const int2 *__restrict__ bonds, int nb, float L, float invL, float k, float r0,
-                            float *__restrict__ out, Lat lat) {
+                            float *__restrict__ out, const Lat *__restrict__ latp) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= nb) return;
+    const Lat lat = *latp;
     const int2 ij = bonds[b];
     const float4 p = posw[ij.x], q = posw[ij.y];
     float dx = min_image(p.x - q.x, L, invL), dy = min_image(p.y - q.y, L, invL);
@@ -489,7 +496,7 @@ pse_status pse_bond_forces_orig(pse_ctx *c, float *d_F) {
     CUDA_TRY(c, cudaMemsetAsync(d_F, 0, (size_t)3 * c->N * sizeof(float), c->stream));
     if (c->n_bonds == 0) return PSE_OK;
     bond_forces<<<(c->n_bonds + 127) / 128, 128, 0, c->stream>>>(c->d_posw, c->d_bonds, c->n_bonds, (float)c->L, 1.0f / (float)c->L,
-                                                                 (float)c->bond_k, (float)c->bond_r0, d_F, pse_lat(c));
+                                                                 (float)c->bond_k, (float)c->bond_r0, d_F, c->d_lat);
     KERNEL_CHECK(c);
     return PSE_OK;
 }
@@ -507,9 +514,9 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     const int N = c->N, T = 256, nb = (N + T - 1) / T;
     const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
     const float rc = (float)c->rcut, rc2 = rc * rc;
-    const Lat lat = pse_lat(c);
+    const Lat *lat = c->d_lat;
     // >> 2 r_c ulp(L): rounding gap between screened and R16 distances (the map by A adds a few more roundings of the same size)
-    const float band = 32.f * rc * L * 1.2e-7f * (c->deformed ? 4.f * (float)(std::fabs(c->lat_a11) + std::fabs(c->lat_a12) + std::fabs(c->lat_a22)) : 1.f);
+    const float band = 32.f * rc * L * 1.2e-7f;      // the kernel widens it by 4 (|a11| + |a12| + |a22|) on a deformed lattice
     c->have_nbrs = false;
     CUDA_TRY(c, cudaMemsetAsync(c->d_bins, 0, c->bins_n * sizeof(int), c->stream));      // cell and tile counters, one memset
     wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
@@ -643,7 +650,7 @@ pse_status pse_hs_forces_packed(pse_ctx *c, double dt, float *d_out_packed) {
     const int N = c->N, T = 256;
     float coef = (float)(3.0 * M_PI * c->eta * c->a / dt);
     hs_forces<<<(unsigned)(((size_t)N * 8 + T - 1) / T), T, 0, c->stream>>>(c->d_pos, N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, (float)c->L,
-                                                                            1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed, pse_lat(c));
+                                                                            1.0f / (float)c->L, (float)(2 * c->a), coef, d_out_packed, c->d_lat);
     KERNEL_CHECK(c);
     return PSE_OK;
 }

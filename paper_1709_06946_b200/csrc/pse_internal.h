@@ -31,10 +31,10 @@ struct Lat { float a11, a12, a22, i11, i12, i22; };
 
 // everything baked into the captured graph of a step
 struct StepGraphKey {
-    const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap;
+    const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap; int nc; bool deformed;
     bool operator==(const StepGraphKey &o) const {
         return pos == o.pos && noise_real == o.noise_real && noise_wave == o.noise_wave && dt == o.dt && mL == o.mL && mG == o.mG &&
-               n_bonds == o.n_bonds && nbr_cap == o.nbr_cap;
+               n_bonds == o.n_bonds && nbr_cap == o.nbr_cap && nc == o.nc && deformed == o.deformed;
     }
 };
 
@@ -55,6 +55,7 @@ struct pse_ctx {
     double h = 0, eta_g = 0;                 // grid spacing, Gaussian shape parameter
     double lat_a11 = 1, lat_a12 = 0, lat_a22 = 1;   // the lattice deformation A (pse_set_lattice); identity = the cubic box
     bool deformed = false;
+    Lat *d_lat = nullptr;                    // A and A^-1 in device memory: what the kernels read, so that a captured step outlives a change of strain
     int win_kind = 1;                        // 0 = Gaussian (paper), 1 = exponential-of-semicircle window
     double win_a = 0, win_b = 0;             // window parameters handed to the kernels (see win_arg in wavespace.cu)
     float *d_dec = nullptr;                  // [M] inverse 1-D window transform per FFT index

@@ -33,7 +33,8 @@ template <int MODE, bool DEF>
 __global__ void __launch_bounds__(512, 2)
 real_pairs_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ in, float4 *__restrict__ out, int N,
                   const unsigned long long *__restrict__ off, const int *__restrict__ cnt, const int *__restrict__ idx,
-                  const float4 *__restrict__ table, float inv_dr, float L, float invL, Lat lat) {
+                  const float4 *__restrict__ table, float inv_dr, float L, float invL, const Lat *__restrict__ latp) {
+    const Lat lat = DEF ? *latp : Lat{1.f, 0.f, 1.f, 1.f, 0.f, 1.f};   // device memory: a captured step survives pse_set_lattice
     // two planar float4 arrays (U-part functions, E-part functions): a 16-byte row stride spreads random rows over
     // all eight 16-byte bank groups; the interleaved 32-byte rows reached only four (ncu: 17 wavefronts per LDS.128)
     extern __shared__ float4 tab[];               // tabU[PSE_NTAB] then tabE[PSE_NTAB]
@@ -138,10 +139,10 @@ static pse_status launch_real(pse_ctx *c, const float *d_in, float *d_out, int g
     const float inv_dr = (float)(1.0 / c->tab_dr), L = (float)c->L, invL = 1.0f / (float)c->L;
     if (c->deformed)
         real_pairs_kernel<MODE, true><<<grid, threads, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
-                                                                         inv_dr, L, invL, pse_lat(c));
+                                                                         inv_dr, L, invL, c->d_lat);
     else
         real_pairs_kernel<MODE, false><<<grid, threads, REAL_SMEM, c->stream>>>(c->d_pos, in4, out4, c->N, c->d_nbr_off, c->d_nbr_count, c->d_nbr_idx, tab,
-                                                                          inv_dr, L, invL, pse_lat(c));
+                                                                          inv_dr, L, invL, c->d_lat);
     KERNEL_CHECK(c);
     return PSE_OK;
 }

@@ -13,7 +13,8 @@ struct ScaleParams {
     float two_pi_over_L, a, inv4xi2, c_mv, c_br, inv_eta;
     const float *dec;                              // [M] 1/kappa(k_n): inverse 1-D window transform per FFT index
     int mode;                                      // PSE_IN_F | PSE_IN_S | PSE_OUT_U | PSE_OUT_E: which planes are read / written
-    float ki11, ki12, ki22;                        // k = (2 pi/L) A^-T n: kx = ki11 nx, ky = ki22 ny + ki12 nx (entries of A^-1; 1, 0, 1 on the cube)
+    const Lat *lat;                                // k = (2 pi/L) A^-T n: kx = i11 nx, ky = i22 ny + i12 nx (entries of A^-1; 1, 0, 1 on the cube), read from
+                                                   // device memory so that a captured step stays valid while the strain advances
 };
 
 // s0 = sin x / x and s1 = 3 (sin x - x cos x)/x^3 (series below 0.5: cancellation) from one sincosf, x > 0
@@ -31,7 +32,8 @@ __device__ __forceinline__ bool mode_k(const ScaleParams &sp, int ix, int iy, in
     const int M = sp.M, half = (M + 1) / 2;
     const int nx = ix < half ? ix : ix - M, ny = iy < half ? iy : iy - M, nz = iz;
     const bool nyq = !(M & 1) && (ix == M / 2 || iy == M / 2 || iz == M / 2);
-    kx = sp.two_pi_over_L * (sp.ki11 * (float)nx); ky = sp.two_pi_over_L * (sp.ki22 * (float)ny + sp.ki12 * (float)nx); kz = sp.two_pi_over_L * (float)nz;
+    const float ki11 = __ldg(&sp.lat->i11), ki12 = __ldg(&sp.lat->i12), ki22 = __ldg(&sp.lat->i22);
+    kx = sp.two_pi_over_L * (ki11 * (float)nx); ky = sp.two_pi_over_L * (ki22 * (float)ny + ki12 * (float)nx); kz = sp.two_pi_over_L * (float)nz;
     return !(nyq || (nx == 0 && ny == 0 && nz == 0));
 }
 
@@ -115,8 +117,7 @@ inline ScaleParams make_scale_params(const pse_ctx *c, int mode = PSE_MODE_ALL) 
     const double V = c->L * c->L * c->L;
     sp.c_mv = (float)(1.0 / V); sp.c_br = (float)(1.0 / std::sqrt(V));
     sp.inv_eta = (float)(1.0 / c->eta);
-    const Lat l = pse_lat(c);
-    sp.ki11 = l.i11; sp.ki12 = l.i12; sp.ki22 = l.i22;
+    sp.lat = c->d_lat;
     return sp;
 }
 

@@ -659,7 +659,8 @@ __global__ void __launch_bounds__(256) scale_brownian_kernel(cufftComplex *spec,
         if (rot) { rot[o] = zero; rot[nmode + o] = zero; rot[2 * nmode + o] = zero; }
         return;
     }
-    const float kx = sp.two_pi_over_L * (sp.ki11 * (float)nx), ky = sp.two_pi_over_L * (sp.ki22 * (float)ny + sp.ki12 * (float)nx), kz = sp.two_pi_over_L * (float)nz;
+    const float ki11 = __ldg(&sp.lat->i11), ki12 = __ldg(&sp.lat->i12), ki22 = __ldg(&sp.lat->i22);
+    const float kx = sp.two_pi_over_L * (ki11 * (float)nx), ky = sp.two_pi_over_L * (ki22 * (float)ny + ki12 * (float)nx), kz = sp.two_pi_over_L * (float)nz;
     const bool canon = nz > 0 || ny > 0 || (ny == 0 && nx > 0);
     const int sx = canon ? nx : -nx, sy = canon ? ny : -ny;           // noise entry of the canonical member, product-grid indices
     const size_t cmode = (size_t)Mc * Mc * sp.Mch, src = ((size_t)(sx < 0 ? sx + Mc : sx) * Mc + (size_t)(sy < 0 ? sy + Mc : sy)) * sp.Mch + nz;

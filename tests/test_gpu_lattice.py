@@ -291,3 +291,49 @@ def test_lattice_edge_cases_pair_across_the_sheared_boundary_compression_and_rep
     assert all(np.array_equal(outs[0][0], o) for o in (outs[0][2], outs[1][0], outs[1][2]))
     Uo, Eo = lat.mobility_apply(xs.astype(np.float64), Ls, matrix(l3), A, ETA, 0.6, F, S, eps=1e-9)
     assert rel(outs[0][0], Uo) < bar(1e-3) and rel(outs[0][1], Eo) < bar(1e-3)
+
+
+def test_strain_advanced_every_step_on_one_context_matches_fresh_contexts():
+    """A flowing suspension ("the periodic lattice must deform"): pse_set_lattice before every pse_step on ONE context, whose
+    captured step graphs stay alive because the kernels read A from device memory.  Each step must agree with a fresh context that is
+    given that step's lattice (checked path, nothing captured), within the solver tolerance; a context left on the PREVIOUS strain
+    must not (the check that this test can see a stale lattice at all)."""
+    import paper_1709_06946_b200 as pse
+    N, phi, xi, tol, dt = 4000, 0.2, 0.6, 1e-3, 1e-4
+    s, L = synth.rsa(N, phi, seed=77)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi, lattice=SHEAR)
+    assert st == 0
+    strains = [0.10, 0.20, 0.30, 0.35, 0.40, 0.45, 0.50, 0.10]            # jumps large enough that a stale lattice shows; back down at the end
+
+    def fresh_step(x32, gamma, w1, w2):
+        c = pse.pse_create(N, L, A, ETA, KT, xi, grid, P, rcut, tol)
+        c.pse_set_lattice(1.0, gamma, 1.0)
+        p = dev(pos4(x32))
+        c.pse_step(p, dt, dev(w1.reshape(N, 8)), dev(w2))
+        out = p.cpu().numpy()[:, :3].copy()
+        c.close()
+        return out
+
+    ctx = pse.pse_create(N, L, A, ETA, KT, xi, grid, P, rcut, tol)
+    x32 = (s @ matrix((1.0, strains[0], 1.0)).T).astype(np.float32)
+    worst, stale_seen = 0.0, 0.0
+    for k, gamma in enumerate(strains):
+        if k:                                                              # carry the suspension along: same lattice coordinates, new A
+            sl = x32.astype(np.float64) @ np.linalg.inv(matrix((1.0, strains[k - 1], 1.0))).T
+            x32 = (sl @ matrix((1.0, gamma, 1.0)).T).astype(np.float32)
+        w1, w2 = synth.brownian_noise(N, grid, 100 + k)
+        ctx.pse_set_lattice(1.0, gamma, 1.0)
+        p = dev(pos4(x32))
+        ctx.pse_step(p, dt, dev(w1.reshape(N, 8)), dev(w2))
+        got = p.cpu().numpy()[:, :3]
+        want = fresh_step(x32, gamma, w1, w2)
+        e = rel(got - x32, want - x32)
+        worst = max(worst, e)
+        assert e < 5 * tol, (k, gamma, e)
+        if k in (3, 7):
+            stale = fresh_step(x32, strains[k - 1], w1, w2)
+            stale_seen = max(stale_seen, rel(stale - x32, want - x32))
+        x32 = got.astype(np.float32).copy()
+    ctx.close()
+    print('worst displacement difference', worst, 'a stale lattice would give', stale_seen)
+    assert stale_seen > 20 * tol
