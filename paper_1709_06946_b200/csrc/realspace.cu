@@ -164,14 +164,18 @@ pse_status pse_real_apply(pse_ctx *c, const float *d_in, float *d_out, int mode)
     if ((long long)grid * wpb >= tasks) grid = (int)((tasks + wpb - 1) / wpb);
     else {
         // The persistent warps take whole tasks round-robin, so a launch lasts ceil(tasks / warps) rounds and the last one may be
-        // nearly empty (config 3: 3.46 rounds of 16-warp CTAs).  A round costs about in proportion to the warps that share an SM's L1,
-        // so narrower CTAs whose last round is full win: 14 warps at config 3 (3.95 rounds), 33.5 -> 31.2 us per launch; taken only
-        // where the model promises 8 % (measured: about half of what it promises); large N keeps 16 warps.
-        auto cost = [&](int w) { return ((tasks + (long long)grid * w - 1) / ((long long)grid * w)) * w; };
-        const long long c16 = cost(16);
-        long long best = c16;
+        // nearly empty (config 3: 3.46 rounds of 16-warp CTAs).  Measured (S -> E against N at config 3's density, 12 to 16 warps):
+        // time = 7.3 us + 0.44 us x cost, where a full round costs the number of warps that share an SM's L1 and a last round filled
+        // to a fraction f costs about min(1, 0.45 + 1.2 f) of a full one (its dependent loads are paid whatever f is).  Narrower
+        // CTAs whose last round is full win where that model says so by 5 %: 14 warps at config 3 (3.95 rounds), 33.5 -> 31.3 us
+        // per launch; a launch barely over one round (N = 20 000) and large N keep 16 warps.
+        auto cost = [&](int w) {
+            const double R = (double)tasks / ((double)grid * w), full = std::floor(R), f = R - full;
+            return w * (full + (f > 0 ? std::min(1.0, 0.45 + 1.2 * f) : 0.0));
+        };
+        double best = 0.95 * cost(16);
         for (int w = 15; w >= 12; --w)
-            if (cost(w) < best && cost(w) * 100 <= c16 * 92) { best = cost(w); wpb = w; }
+            if (cost(w) < best) { best = cost(w); wpb = w; }
     }
     const int threads = wpb * 32;
     // unrequested outputs are written as zeros; absent inputs must be zero in d_in (they are skipped, not read as data)
