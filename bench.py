@@ -498,7 +498,7 @@ def main():
         line['sheared_cell'] = {'strain': 0.5, 'value': replica_throughput(a4.steps, world, rsh['ms']), 'unit': 'steps/s', 'ms_per_step': rsh['ms'] / a4.steps,
                                 'grid': rsh['grid'], 'P': rsh['P'], 'matvecs_per_sec': 1e3 / rsh['matvec_ms'], 'e2e_steps_per_sec': 1e3 / rsh['e2e_ms'],
                                 'steps': a4.steps, 'warmup': a4.warmup}
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:          # the CPU baseline is reported at N = 1 only
         rs = ReferenceStepper(wl)
         sec, its = rs.step()
         if sec > 40.0:
