@@ -157,8 +157,7 @@ pse_status pse_create_window(pse_ctx **out, int N, double L, double a, double et
     CUDA_TRY(c, cudaMemcpy(c->d_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
     { const Lat id = pse_lat(c); CUDA_TRY(c, cudaMalloc(&c->d_lat, sizeof(Lat))); CUDA_TRY(c, cudaMemcpy(c->d_lat, &id, sizeof(Lat), cudaMemcpyHostToDevice)); }
     // cells: edge >= rcut with a relative margin far above fp32 rounding of the binning
-    c->nc = std::max(1, (int)std::floor(L / (rcut * 1.0001)));
-    c->ncell = c->nc * c->nc * c->nc;
+    { const int n = std::max(1, (int)std::floor(L / (rcut * 1.0001))); c->nc = Cells{n, n, n}; c->ncell = c->ncell_cap = n * n * n; }
     const size_t n8 = (size_t)N * 8 * sizeof(float);
     CUDA_TRY(c, cudaMalloc(&c->d_pos, (size_t)N * sizeof(float4)));
     CUDA_TRY(c, cudaMalloc(&c->d_posw, (size_t)N * sizeof(float4)));
@@ -252,9 +251,21 @@ pse_status pse_set_lattice(pse_ctx *c, double a11, double a12, double a22) {
     // The kernels read A from device memory, so the captured graphs of pse_step stay valid while the strain advances step by step
     // (a flowing suspension); they are keyed by the cell count and by cube / deformed, which select grids and instantiations.
     k_set_lat<<<1, 1, 0, c->stream>>>(c->d_lat, pse_lat(c)); KERNEL_CHECK(c);
-    // cells of lattice-coordinate edge >= reach * rcut (never more cells than pse_create made room for: reach >= 1)
-    c->nc = std::max(1, (int)std::floor(c->L / (c->rcut * 1.0001 * reach)));
-    c->ncell = c->nc * c->nc * c->nc;
+    // cells per lattice direction i of edge >= rcut * |row i of A^-1| (a separation |r| < rcut has |d_i| <= |row_i| |r|): a sheared
+    // cell is searched with bricks that are longer along x only, not with cubes sized for its worst direction.  Never more cells
+    // than pse_create made room for (the cube's count): the longest direction gives way first.
+    {
+        const double i11 = 1.0 / a11, i12 = -a12 / (a11 * a22), i22 = 1.0 / a22;
+        const double rows[3] = {std::sqrt(i11 * i11 + i12 * i12), std::fabs(i22), 1.0};
+        int n[3];
+        for (int i = 0; i < 3; ++i) n[i] = std::max(1, (int)std::floor(c->L / (c->rcut * 1.0001 * rows[i])));
+        while ((long long)n[0] * n[1] * n[2] > (long long)c->ncell_cap) {
+            int big = 0;
+            for (int i = 1; i < 3; ++i) if (n[i] > n[big]) big = i;
+            --n[big];
+        }
+        c->nc = Cells{n[0], n[1], n[2]}; c->ncell = n[0] * n[1] * n[2];
+    }
     c->have_nbrs = false; c->nbr_pending = false; c->fine_bins_valid = false;
     return PSE_OK;
 }
@@ -413,7 +424,7 @@ pse_status pse_step(pse_ctx *c, float *d_pos, double dt, const float *d_noise_re
                 user_pos = d_pos;
                 d_pos = c->d_stage_pos; d_noise_real = c->d_stage_a; d_noise_wave = c->d_stage_noise;
             }
-            const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap, c->nc, c->deformed};
+            const StepGraphKey key = {d_pos, d_noise_real, d_noise_wave, dt, mL, mG, c->n_bonds, c->nbr_cap, c->nc.x, c->nc.y, c->nc.z, c->deformed};
             if (!c->step_graph[0] || !(key == c->graph_key)) {
                 for (int g = 0; g < 3; ++g) if (c->step_graph[g]) { cudaGraphExecDestroy(c->step_graph[g]); c->step_graph[g] = nullptr; }
                 const long long l0 = c->launches;

@@ -140,7 +140,7 @@ __device__ __forceinline__ float dist2(float4 a, float4 b, float L, float invL, 
     return __fadd_rn(__fadd_rn(__fmul_rn(rx, rx), __fmul_rn(ry, ry)), __fmul_rn(dz, dz));
 }
 
-__global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int nc, float cell_inv,
+__global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, Cells nc, float3 cell_inv,
                              float4 *posw, int *cell_of, int *cell_count, float inv_h, int M, int P, int nt, int *tile_of, int *tile_count, const Lat *__restrict__ latp) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -149,8 +149,8 @@ __global__ void wrap_and_bin(const float4 *pos, int N, float L, float invL, int 
     p.x = __fadd_rn(__fmul_rn(lat.i11, p.x), __fmul_rn(lat.i12, p.y)); p.y = __fmul_rn(lat.i22, p.y);     // s = A^-1 x (exact on the cube)
     p.x = wrap_coord(p.x, L, invL); p.y = wrap_coord(p.y, L, invL); p.z = wrap_coord(p.z, L, invL); p.w = 0.f;
     posw[i] = p;
-    int cx = min(nc - 1, (int)(p.x * cell_inv)), cy = min(nc - 1, (int)(p.y * cell_inv)), cz = min(nc - 1, (int)(p.z * cell_inv));
-    int cell = (cx * nc + cy) * nc + cz;
+    int cx = min(nc.x - 1, (int)(p.x * cell_inv.x)), cy = min(nc.y - 1, (int)(p.y * cell_inv.y)), cz = min(nc.z - 1, (int)(p.z * cell_inv.z));
+    int cell = (cx * nc.y + cy) * nc.z + cz;
     cell_of[i] = cell;
     atomicAdd(&cell_count[cell], 1);
     const int t = pse_tile_of(p, inv_h, M, P, nt);              // spread / interpolate tile bin of the same particle
@@ -199,7 +199,7 @@ constexpr int NS_CHUNK = 1024, NS_THREADS = 128;
 
 template <bool FILL>
 __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start,
-                                                                   int nc, float L, float invL, float rc2, int *__restrict__ cursor,
+                                                                   Cells nc, float L, float invL, float rc2, int *__restrict__ cursor,
                                                                    const unsigned long long *__restrict__ off, int *__restrict__ idx, const Lat *__restrict__ latp) {
     __shared__ float4 cpos[NS_CHUNK];
     __shared__ int run_lo[18], run_cum[19];
@@ -207,20 +207,21 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
     const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int first = cell_start[cell], np = cell_start[cell + 1] - first;
     if (np == 0) return;
-    const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
-    const int span = nc >= 3 ? 3 : nc;
+    const int cz = cell % nc.z, cy = (cell / nc.z) % nc.y, cx = cell / (nc.y * nc.z);
+    const int spanx = nc.x >= 3 ? 3 : nc.x, spany = nc.y >= 3 ? 3 : nc.y;
     if (tid < 32) {
-        // lane r < 2*span*span describes run r: column (r>>1), part (r&1)
+        // lane r < 2*spanx*spany describes run r: column (r>>1), part (r&1)
         int lo = 0, len = 0;
         const int col_i = lane >> 1, part = lane & 1;
-        if (col_i < span * span) {
-            int ccx = col_i / span, ccy = col_i % span;
-            if (nc >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + ccy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
-            const int col = (ccx * nc + ccy) * nc;
-            const int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
+        if (col_i < spanx * spany) {
+            int ccx = col_i / spany, ccy = col_i % spany;
+            if (nc.x >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc.x : 0; ccx -= ccx >= nc.x ? nc.x : 0; }
+            if (nc.y >= 3) { ccy = cy + ccy - 1; ccy += ccy < 0 ? nc.y : 0; ccy -= ccy >= nc.y ? nc.y : 0; }
+            const int col = (ccx * nc.y + ccy) * nc.z;
+            const int z0 = nc.z >= 3 ? cz - 1 : 0, z1 = nc.z >= 3 ? cz + 1 : nc.z - 1;
             int a0, a1, b0 = 0, b1 = 0;                    // run A = cells [a0,a1), run B = cells [b0,b1)
-            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc - 1; b1 = nc; }
-            else if (z1 >= nc) { a0 = 0; a1 = 1; b0 = z0; b1 = nc; }
+            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc.z - 1; b1 = nc.z; }
+            else if (z1 >= nc.z) { a0 = 0; a1 = 1; b0 = z0; b1 = nc.z; }
             else { a0 = z0; a1 = z1 + 1; }
             const int c0 = part ? b0 : a0, c1 = part ? b1 : a1;
             lo = cell_start[col + c0]; len = cell_start[col + c1] - lo;
@@ -278,7 +279,7 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_sweep_cell(const float4 *
 constexpr int NB_MAXP = 64, NB_WORDS = NS_CHUNK / 32, NB_PB = 4;
 
 template <bool DEF>                                           // DEF: deformed lattice, the screened separation is mapped by A as well
-__global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, int nc,
+__global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *__restrict__ pos, const int *__restrict__ cell_start, Cells nc,
                                                                    float L, float invL, float rc2, float band0, int *__restrict__ count,
                                                                    unsigned long long *__restrict__ off, int *__restrict__ idx,
                                                                    unsigned long long cap, unsigned long long *__restrict__ cursor,
@@ -295,19 +296,20 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     const int cell = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int first = cell_start[cell], np = cell_start[cell + 1] - first;
     if (np == 0) return;
-    const int cz = cell % nc, cy = (cell / nc) % nc, cx = cell / (nc * nc);
-    const int span = nc >= 3 ? 3 : nc;
+    const int cz = cell % nc.z, cy = (cell / nc.z) % nc.y, cx = cell / (nc.y * nc.z);
+    const int spanx = nc.x >= 3 ? 3 : nc.x, spany = nc.y >= 3 ? 3 : nc.y;
     if (tid < 32) {
         int lo = 0, len = 0;
         const int col_i = lane >> 1, part = lane & 1;
-        if (col_i < span * span) {
-            int ccx = col_i / span, ccy = col_i % span;
-            if (nc >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc : 0; ccx -= ccx >= nc ? nc : 0; ccy = cy + ccy - 1; ccy += ccy < 0 ? nc : 0; ccy -= ccy >= nc ? nc : 0; }
-            const int col = (ccx * nc + ccy) * nc;
-            const int z0 = nc >= 3 ? cz - 1 : 0, z1 = nc >= 3 ? cz + 1 : nc - 1;
+        if (col_i < spanx * spany) {
+            int ccx = col_i / spany, ccy = col_i % spany;
+            if (nc.x >= 3) { ccx = cx + ccx - 1; ccx += ccx < 0 ? nc.x : 0; ccx -= ccx >= nc.x ? nc.x : 0; }
+            if (nc.y >= 3) { ccy = cy + ccy - 1; ccy += ccy < 0 ? nc.y : 0; ccy -= ccy >= nc.y ? nc.y : 0; }
+            const int col = (ccx * nc.y + ccy) * nc.z;
+            const int z0 = nc.z >= 3 ? cz - 1 : 0, z1 = nc.z >= 3 ? cz + 1 : nc.z - 1;
             int a0, a1, b0 = 0, b1 = 0;
-            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc - 1; b1 = nc; }
-            else if (z1 >= nc) { a0 = 0; a1 = 1; b0 = z0; b1 = nc; }
+            if (z0 < 0) { a0 = 0; a1 = z1 + 1; b0 = nc.z - 1; b1 = nc.z; }
+            else if (z1 >= nc.z) { a0 = 0; a1 = 1; b0 = z0; b1 = nc.z; }
             else { a0 = z0; a1 = z1 + 1; }
             const int c0 = part ? b0 : a0, c1 = part ? b1 : a1;
             lo = cell_start[col + c0]; len = cell_start[col + c1] - lo;
@@ -328,8 +330,8 @@ __global__ void __launch_bounds__(NS_THREADS) neighbor_build_cell(const float4 *
     // staged already shifted to that image and the test is a plain difference.  The decision itself stays the R16
     // arithmetic: whenever the screened d^2 falls within `band` of r_c^2 (far wider than the rounding difference between
     // the two forms) the pair is re-evaluated with dist2 on the unshifted position.
-    const bool fast = nc >= 5;
-    const float edge = L / (float)nc, mx = ((float)cx + 0.5f) * edge, my = ((float)cy + 0.5f) * edge, mz = ((float)cz + 0.5f) * edge;
+    const bool fast = nc.x >= 5 && nc.y >= 5 && nc.z >= 5;
+    const float mx = ((float)cx + 0.5f) * (L / (float)nc.x), my = ((float)cy + 0.5f) * (L / (float)nc.y), mz = ((float)cz + 0.5f) * (L / (float)nc.z);
     const int nwords = (total + 31) >> 5;
     for (int r = wid; r < 18; r += NS_THREADS / 32) {            // staging: a warp per run, no search for the run of a candidate
         const int lo = run_lo[r], c0 = run_cum[r], len = run_cum[r + 1] - c0;
@@ -512,14 +514,16 @@ pse_status pse_scan_i32(pse_ctx *c, const int *d_in, int *d_out, size_t n) { ret
 pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
     ScopedPhase ph(c, PSE_T_NEIGHBORS);
     const int N = c->N, T = 256, nb = (N + T - 1) / T;
-    const float L = (float)c->L, invL = 1.0f / L, cell_inv = (float)(c->nc / c->L);
+    const float L = (float)c->L, invL = 1.0f / L;
+    const Cells nc = c->nc;
+    const float3 cell_inv = make_float3((float)(nc.x / c->L), (float)(nc.y / c->L), (float)(nc.z / c->L));
     const float rc = (float)c->rcut, rc2 = rc * rc;
     const Lat *lat = c->d_lat;
     // >> 2 r_c ulp(L): rounding gap between screened and R16 distances (the map by A adds a few more roundings of the same size)
     const float band = 32.f * rc * L * 1.2e-7f;      // the kernel widens it by 4 (|a11| + |a12| + |a22|) on a deformed lattice
     c->have_nbrs = false;
     CUDA_TRY(c, cudaMemsetAsync(c->d_bins, 0, c->bins_n * sizeof(int), c->stream));      // cell and tile counters, one memset
-    wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, c->nc, cell_inv,
+    wrap_and_bin<<<nb, T, 0, c->stream>>>(reinterpret_cast<const float4 *>(d_pos_in), N, L, invL, nc, cell_inv,
                                            c->d_posw, c->d_cell_of, c->d_cell_count, (float)(1.0 / c->h), c->M, c->P, c->nt,
                                            c->d_tile_of, c->d_tile_count, lat); KERNEL_CHECK(c);
     if (c->ncell <= SCAN1_MAX && c->ntile <= SCAN1_MAX) {
@@ -545,11 +549,11 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         // the kernel and are looked at by pse_neighbors_settle, never here
         CUDA_TRY(c, cudaMemsetAsync(c->d_nbr_ctl, 0, 2 * sizeof(unsigned long long), c->stream));
         if (c->deformed)
-            neighbor_build_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
+            neighbor_build_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
                                                                              c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
                                                                              reinterpret_cast<int *>(c->d_nbr_ctl + 1), lat);
         else
-            neighbor_build_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
+            neighbor_build_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, nc, L, invL, rc2, band, c->d_nbr_count, c->d_nbr_off,
                                                                               c->d_nbr_idx, (unsigned long long)c->nbr_cap, c->d_nbr_ctl,
                                                                               reinterpret_cast<int *>(c->d_nbr_ctl + 1), lat);
         KERNEL_CHECK(c);
@@ -558,7 +562,7 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
         CUDA_TRY(c, cudaEventRecord(c->ev_nbr, c->stream));
         c->nbr_pending = true;
     } else {                                                         // general two-pass path (count, scan, fill); synchronises
-        neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_nbr_count,
+        neighbor_sweep_cell<false><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, nc, L, invL, rc2, c->d_nbr_count,
                                                                             nullptr, nullptr, lat); KERNEL_CHECK(c);
         PSE_TRY(pse_scan_u64(c, c->d_nbr_count, c->d_nbr_off, (size_t)N));
         unsigned long long total = 0;
@@ -572,7 +576,7 @@ pse_status pse_neighbors_impl(pse_ctx *c, const float *d_pos_in) {
             c->nbr_cap = cap;
         }
         c->nbr_total = (size_t)total;
-        neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, c->nc, L, invL, rc2, c->d_cell_of,
+        neighbor_sweep_cell<true><<<c->ncell, NS_THREADS, 0, c->stream>>>(c->d_pos, c->d_cell_start, nc, L, invL, rc2, c->d_cell_of,
                                                                            c->d_nbr_off, c->d_nbr_idx, lat); KERNEL_CHECK(c);
         c->nbr_pending = false;
     }

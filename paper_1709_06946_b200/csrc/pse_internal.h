@@ -28,13 +28,16 @@ struct Timer { cudaEvent_t a, b; int phase; };
 // are those of the cube; physical separations r = A d (d = minimum image of s_a - s_b) and wave vectors k = (2 pi/L) A^-T n
 // appear only where distances and the Green's function are evaluated (reading R22).  i** = entries of A^-1.
 struct Lat { float a11, a12, a22, i11, i12, i22; };
+// cells of the neighbour search per lattice direction: edge L/n_i >= r_cut * (norm of row i of A^-1), so a deformed cell is not searched
+// with cubes sized for its worst direction
+struct Cells { int x, y, z; };
 
 // everything baked into the captured graph of a step
 struct StepGraphKey {
-    const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap; int nc; bool deformed;
+    const void *pos, *noise_real, *noise_wave; double dt; int mL, mG, n_bonds; size_t nbr_cap; int ncx, ncy, ncz; bool deformed;
     bool operator==(const StepGraphKey &o) const {
         return pos == o.pos && noise_real == o.noise_real && noise_wave == o.noise_wave && dt == o.dt && mL == o.mL && mG == o.mG &&
-               n_bonds == o.n_bonds && nbr_cap == o.nbr_cap && nc == o.nc && deformed == o.deformed;
+               n_bonds == o.n_bonds && nbr_cap == o.nbr_cap && ncx == o.ncx && ncy == o.ncy && ncz == o.ncz && deformed == o.deformed;
     }
 };
 
@@ -82,7 +85,8 @@ struct pse_ctx {
     float *d_table = nullptr;                // [PSE_NTAB][8]
     double tab_dr = 0;
     // ---- cell list / neighbour list (all in cell-sorted numbering unless noted) ----
-    int nc = 0, ncell = 0;                   // cells per dimension, total
+    Cells nc = {0, 0, 0};                    // cells per lattice direction
+    int ncell = 0, ncell_cap = 0;            // their product; what the cell arrays were allocated for (the cube's count)
     bool have_nbrs = false;
     float4 *d_pos = nullptr;                 // [N] wrapped positions, sorted
     int *d_order = nullptr;                  // [N] sorted -> original
