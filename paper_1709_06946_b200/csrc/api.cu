@@ -36,9 +36,15 @@ const struct { int m; float us; } kFftCost[] = {
     {288, 1653}, {300, 2053}, {320, 2381}, {324, 2310}, {336, 3089}, {343, 2156}, {350, 3931}, {360, 3217}, {375, 4921},
     {384, 3964}, {400, 6977}};
 
+// What a grid of M^3 points costs a product beside its transforms: spread stores, scaling and interpolation loads grow with M^3,
+// about 20 us per 10^6 points and product at config 3 / its sheared cells (100^3: 64 us, 128^3: 85, 144^3: 107), where the two
+// transforms of a product take 1.5x the table's figure; in the table's units that is 13 us per 10^6 points.
 int choose_grid(int mmin) {
     int best = 0; float cost = 1e30f;
-    for (const auto &e : kFftCost) if (e.m >= mmin && e.us < cost) { best = e.m; cost = e.us; }
+    for (const auto &e : kFftCost) {
+        const float total = e.us + 13.3e-6f * (float)e.m * (float)e.m * (float)e.m;
+        if (e.m >= mmin && total < cost) { best = e.m; cost = total; }
+    }
     if (best) return best;
     int M = mmin;
     while (!smooth7(M)) ++M;

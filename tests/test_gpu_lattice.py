@@ -221,12 +221,12 @@ def test_full_couplet_and_paper_window_on_a_sheared_lattice():
 
 
 def test_config3_in_a_sheared_cell_against_the_lattice_reference():
-    """`bench.py --shear 0.5`'s workload (N = 65 536, phi = 0.30, tol = 1e-3, xi = 0.575 -> grid 128, P = 4): U and E of the full
+    """`bench.py --shear 0.5`'s workload (N = 65 536, phi = 0.30, tol = 1e-3, xi = 0.575 -> grid 112, P = 4): U and E of the full
     product on 128 sampled particles against the fp64 lattice reference tier at its own xi = 0.45, tol 1e-7."""
     N, xi, tol, l3 = 65536, 0.575, 1e-3, SHEAR
     x32, L = deformed_suspension(N, 0.30, l3, seed=100, images=False)
     ctx, _ = make(N, L, xi, tol, l3, x32)
-    assert (ctx.grid, ctx.P) == (128, 4)
+    assert (ctx.grid, ctx.P) == (112, 4)
     F, S = synth.gaussian_inputs(N, 1)
     rows = np.sort(np.random.default_rng(5).choice(N, 128, replace=False))
     Uo, Eo = lat.LatticeReference(L, matrix(l3), A, ETA, 0.45, tol=1e-7).apply(x32.astype(np.float64), F, S, rows)
