@@ -76,7 +76,8 @@ pse_status pse_destroy(pse_ctx *ctx);
  * A = [[a11, a12, 0], [0, a22, 0], [0, 0, 1]], i.e. the lattice vectors are the columns of L A.  Simple shear (Lees-Edwards,
  * Eq. 56): a11 = a22 = 1, a12 = gamma; planar extension (Kraynik-Reinelt, Eq. 58): a11 = epsilon,
  * a22 = 1/epsilon, a12 = 0; any other volume-preserving lattice in the x-y plane B (a Kraynik-Reinelt cell in the lab frame) is
- * B = Q A with A of this form and Q a rotation about z: pass A and work in the frame x' = Q^T x.  Positions, forces, velocities stay PHYSICAL (Cartesian) vectors; any periodic image of a position is
+ * B = Q A with A of this form and Q a rotation about z: pass A and work in the frame x' = Q^T x.  The grid grows with the longest
+ * lattice vector (column of A), so describe the lattice by its shortest (Gauss-reduced) basis.  Positions, forces, velocities stay PHYSICAL (Cartesian) vectors; any periodic image of a position is
  * accepted.  Inside, particles are carried in lattice coordinates s = A^-1 x, so cells, spreading and interpolation are those of
  * the cube, separations are r = A d and wave vectors k = (2 pi/L) A^-T n (reading R22): P is that of the cube, the grid
  * must be pse_suggest_params_lattice's.  Call before pse_neighbors; the neighbour structures are invalidated; pse_step then leaves
