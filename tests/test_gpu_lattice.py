@@ -106,8 +106,8 @@ def test_identity_lattice_is_the_cube_bit_for_bit():
 
 @pytest.mark.parametrize('l3,tol', [(SHEAR, 1e-3), (SHEAR, 1e-4), (EXT, 1e-3)])
 def test_product_on_deformed_lattice_against_direct_sums(l3, tol):
-    """N = 400 all rows: total, and the real and wave halves separately (relative to the total)."""
-    N, xi = 400, 0.55
+    """N = 300 all rows: total, and the real and wave halves separately (relative to the total)."""
+    N, xi = 300, 0.55
     x32, L = deformed_suspension(N, 0.20, l3, seed=7)
     ctx, _ = make(N, L, xi, tol, l3, x32)
     F, S = synth.gaussian_inputs(N, 3)
