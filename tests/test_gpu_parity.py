@@ -176,6 +176,27 @@ def test_brownian_wave_part_alone(config1):
     assert rel(np.hstack([UB.cpu().numpy(), EB.cpu().numpy()]), amp * np.hstack([Uw, Ew])) < c['tol']
 
 
+def test_brownian_wave_part_at_a_large_grid_with_an_odd_finer_grid():
+    """The wave half of the sample at tol 1e-4 on a 192^3 product grid (config 5's size at that tolerance), whose finer grid
+    (reading R19) is the odd 243^3: sqrt(2kT/dt) A_w w2 on sampled particles against the oracle's direct sum over the grid's modes."""
+    import paper_1709_06946_b200 as pse
+    N, tol, xi, dt, Lbox = 3000, 1e-4, 0.30, 0.5, 300.0
+    x, L = synth.rsa(N, N * 4 * np.pi / 3 / Lbox**3, seed=9)
+    x32 = x.astype(np.float32)
+    st, grid, P, rcut = pse.pse_suggest_params(N, L, A, tol, xi)
+    assert st == 0 and (grid, P) == (192, 5)
+    ctx = make_ctx(N, L, xi, grid, P, rcut, tol)
+    ctx.pse_neighbors(dev(pos4(x32)))
+    _, w2 = synth.brownian_noise(N, grid, 3)
+    UB, EB = torch.empty(N, 3, device='cuda'), torch.empty(N, 5, device='cuda')
+    ctx.pse_brownian(dt, torch.zeros(N, 8, device='cuda'), dev(w2), UB, EB)
+    rows = np.sort(np.random.default_rng(1).choice(N, 16, replace=False))
+    Uw, Ew = brn.wave_sqrt_apply(x32.astype(np.float64), L, A, ETA, xi, grid, w2, rows=rows)
+    amp = np.sqrt(2 * KT / dt)
+    assert rel(UB.cpu().numpy()[rows], amp * Uw) < bar(tol) and rel(EB.cpu().numpy()[rows], amp * Ew) < bar(tol)
+    ctx.close()
+
+
 def test_constrained_solve_and_hard_sphere_forces(config1):
     c = config1
     ctx, N = c['ctx'], 64
